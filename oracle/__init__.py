@@ -1,0 +1,218 @@
+"""CPU oracle for the SailFFish spectral Poisson hot path -- TEST INFRASTRUCTURE ONLY.
+
+A thin ctypes binding over ``oracle/sf_oracle.c`` (plain C, fp64, written from PAPER.md).  Nothing
+under ``paper_2301_01145_b200/`` may import this package; only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs do.
+The oracle and the CUDA path share no code; see the header of ``sf_oracle.c`` for the passages of
+the paper each function follows and for the pins that tie it to something other than itself.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "sf_oracle.c"
+_LIB = _HERE / "libsf_oracle.so"
+
+OP_PS, OP_FD2 = 0, 1
+
+
+def build(force: bool = False) -> Path:
+    """Compile the oracle with gcc (OpenMP over independent pencils only)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".{os.getpid()}.tmp")
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-o", str(tmp), str(_SRC), "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(str(_LIB))
+        L.orc_num_threads.restype = C.c_int
+        L.orc_green_gauss2.restype = C.c_double
+        L.orc_green_gauss2.argtypes = [C.c_double, C.c_double]
+        L.orc_unbounded_spec_size.restype = C.c_longlong
+        _lib = L
+    return _lib
+
+
+def _i64x3(v):
+    return (C.c_longlong * 3)(*[int(x) for x in v])
+
+
+def _f64x3(v):
+    return (C.c_double * 3)(*[float(x) for x in v])
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _chk(err, what):
+    if err != 0:
+        raise RuntimeError(f"oracle: {what} failed with status {err}")
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().orc_set_num_threads(C.c_int(int(n)))
+
+
+# ---------------------------------------------------------------- 1-D transforms (pin P1)
+def dft_direct(x, sign=-1):
+    x = np.ascontiguousarray(x, dtype=np.complex128)
+    out = np.empty_like(x)
+    lib().orc_dft_direct(C.c_int(x.size), C.c_int(sign), _ptr(x), _ptr(out))
+    return out
+
+
+def fft_pow2(x, sign=-1):
+    x = np.ascontiguousarray(x, dtype=np.complex128)
+    out = np.empty_like(x)
+    _chk(lib().orc_fft_pow2(C.c_int(x.size), C.c_int(sign), _ptr(x), _ptr(out)), "fft_pow2")
+    return out
+
+
+def _r2r(name, x):
+    x = _f64(x)
+    out = np.empty_like(x)
+    getattr(lib(), name)(C.c_int(x.size), _ptr(x), _ptr(out))
+    return out
+
+
+def dst1(x):
+    return _r2r("orc_dst1_direct", x)
+
+
+def dct2(x):
+    return _r2r("orc_dct2_direct", x)
+
+
+def dct3(x):
+    return _r2r("orc_dct3_direct", x)
+
+
+# ---------------------------------------------------------------- solvers
+def _dims(shape):
+    """numpy shape (z, y, x) / (y, x) -> (nd, n[3]) with x first."""
+    nd = len(shape)
+    n = list(reversed(shape)) + [1] * (3 - nd)
+    return nd, n
+
+
+def periodic(f, L, op=OP_PS, rhs_sign=1.0, want_grad=False):
+    """O-PER.  f: numpy array indexed [z, y, x] (or [y, x]); L: domain length per axis (x, y, z).
+    Returns psi, or (psi, grad) with grad[a] = d psi / d x_a, a in x, y(, z) order."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    Lx = list(L) + [1.0] * (3 - len(L))
+    psi = np.empty_like(f)
+    grad = np.empty((nd,) + f.shape, dtype=np.float64) if want_grad else None
+    _chk(lib().orc_periodic(C.c_int(nd), _i64x3(n), _f64x3(Lx), C.c_int(op), C.c_double(rhs_sign),
+                            _ptr(f), _ptr(psi), _ptr(grad) if want_grad else None), "periodic")
+    return (psi, grad) if want_grad else psi
+
+
+def _faces_arg(faces):
+    """faces: dict {(axis, side): array} or None -> (const double*[6], keepalive)."""
+    arr = (C.c_void_p * 6)()
+    keep = []
+    if faces:
+        for (axis, side), g in faces.items():
+            if g is None:
+                continue
+            g = _f64(g)
+            keep.append(g)
+            arr[2 * axis + side] = g.ctypes.data
+    return arr, keep
+
+
+def dirichlet_regular(f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
+    """O-DIR.  f[z, y, x] on interior nodes; h = (hx, hy, hz); faces[(axis, side)] arrays indexed
+    [upper remaining axis, lower remaining axis] (lower axis fastest)."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    assert nd == 3
+    psi = np.empty_like(f)
+    arr, keep = _faces_arg(faces)
+    _chk(lib().orc_dirichlet_regular(_i64x3(n), _f64x3(h), C.c_int(op), C.c_double(rhs_sign), _ptr(f), arr,
+                                     _ptr(psi)), "dirichlet_regular")
+    return psi
+
+
+def neumann_staggered(f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
+    """O-NEU.  Same conventions; face values are d psi / d x_axis along +axis on both sides."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    assert nd == 3
+    psi = np.empty_like(f)
+    arr, keep = _faces_arg(faces)
+    _chk(lib().orc_neumann_staggered(_i64x3(n), _f64x3(h), C.c_int(op), C.c_double(rhs_sign), _ptr(f), arr,
+                                     _ptr(psi)), "neumann_staggered")
+    return psi
+
+
+def green_gauss2(r, eps):
+    return float(lib().orc_green_gauss2(float(r), float(eps)))
+
+
+def unbounded_green(n_xyz, h, eps):
+    """Green's spectrum on the doubled grid: complex array [2 nz, 2 ny, nx + 1]."""
+    n = [int(v) for v in n_xyz]
+    ghat = np.empty((2 * n[2], 2 * n[1], n[0] + 1), dtype=np.complex128)
+    _chk(lib().orc_unbounded_green(_i64x3(n), _f64x3(h), C.c_double(eps), _ptr(ghat)), "unbounded_green")
+    return ghat
+
+
+def unbounded_solve(f, h, ghat, rhs_sign=1.0, want_curl=False):
+    """O-UNB / O-VEC.  f[z, y, x] (scalar) or f[c, z, y, x] (ncomp fields)."""
+    f = _f64(f)
+    vec = f.ndim == 4
+    ncomp = f.shape[0] if vec else 1
+    nd, n = _dims(f.shape[1:] if vec else f.shape)
+    assert nd == 3
+    out = np.empty_like(f)
+    ghat = np.ascontiguousarray(ghat, dtype=np.complex128)
+    assert ghat.shape == (2 * n[2], 2 * n[1], n[0] + 1)
+    _chk(lib().orc_unbounded_solve(_i64x3(n), _f64x3(h), _ptr(ghat), C.c_int(ncomp), C.c_double(rhs_sign),
+                                   _ptr(f), C.c_int(1 if want_curl else 0), _ptr(out)), "unbounded_solve")
+    return out
+
+
+def unbounded_direct(f, h, eps, rhs_sign=1.0):
+    """Direct O(N^6) sum of the definition -- tiny grids only."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    psi = np.empty_like(f)
+    lib().orc_unbounded_direct(_i64x3(n), _f64x3(h), C.c_double(eps), C.c_double(rhs_sign), _ptr(f), _ptr(psi))
+    return psi
+
+
+def unbounded_direct_samples(f, h, eps, idx, rhs_sign=1.0):
+    """Direct sum of the definition at the linear grid indices ``idx`` (x fastest)."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    idx = np.ascontiguousarray(idx, dtype=np.int64)
+    psi = np.empty(idx.size, dtype=np.float64)
+    lib().orc_unbounded_direct_samples(_i64x3(n), _f64x3(h), C.c_double(eps), C.c_double(rhs_sign), _ptr(f),
+                                       C.c_longlong(idx.size), _ptr(idx), _ptr(psi))
+    return psi

@@ -1,0 +1,792 @@
+/*
+ * sf_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * A plain, slow, double-precision CPU restatement of the spectral Poisson solve of
+ * SailFFish (arxiv 2301.01145), written from the paper only.  It shares no code with the
+ * CUDA path under paper_2301_01145_b200/ and must never be imported, linked or executed by
+ * it.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may call it.
+ *
+ * What it follows (PAPER.md = /root/reference/PAPER.md):
+ *   - the four-step solve: forward DFT, multiply by the spectral multiplier, optional
+ *     spectral operations, backward DFT                         (sec 2.2)
+ *   - DFT definitions, unnormalised forward, 1/N on the inverse  (eq. 8)
+ *   - N-D transforms as successive 1-D pencils, inverse in reverse order
+ *   - Table 1: transform type and eigenvalues per BC / grid type
+ *   - k = 0 mode set to zero
+ *   - spectral differentiation by multiplying with ik            (eq. 10)
+ *   - inhomogeneous BC values folded into boundary-adjacent source cells, FD2 only
+ *
+ *   - Hockney-Eastwood: doubled domain, mirrored Green's function, zero-padded source,
+ *     periodic solve, extraction                                 (sec 2.5)
+ *   - Green's function evaluated in real space and forward transformed once
+ *   - 3-D vector solver = component-wise scalar solves
+ * Readings of silent / garbled passages are those of SURVEY.md sec 8(c) (A1-A24), restated in
+ * DESIGN.md.
+ *
+ * Structure: transforms are a recursive radix-2 FFT (power-of-two lengths) and direct O(N^2)
+ * sine / cosine sums (DST-I, DCT-II, DCT-III); every trigonometric argument is reduced in
+ * integer arithmetic before sin/cos is called.  N-D transforms copy one pencil at a time to a
+ * contiguous buffer, transform it and copy it back; OpenMP runs independent pencils in
+ * parallel and nothing else.  The unbounded solver treats the WHOLE doubled domain, as the
+ * paper does: no pruning.
+ *
+ * Array layout everywhere: x fastest, index = ix + nx*(iy + ny*iz); vector fields are
+ * component-major.
+ *
+ * Pins (tests/test_oracle_*.py): P1-P12 of SURVEY.md sec 8(c).  No function here is
+ * "parity unpinned".
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef double complex cplx;
+typedef long long i64;
+
+#define ORC_OK 0
+#define ORC_ERR_ARG (-1)
+#define ORC_ERR_ALLOC (-3)
+
+static const double PI = 3.14159265358979323846264338327950288;
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------
+ * sin(2 pi p/q), cos(2 pi p/q) with the argument reduced exactly: p mod q in integers, then
+ * reflections down to the first octant so that libm only ever sees an angle in [0, pi/4].
+ * ---------------------------------------------------------------------------------------- */
+static void sincos2pi(i64 p, i64 q, double *s, double *c)
+{
+    int neg_s = 0, neg_c = 0, swap = 0;
+    p %= q;
+    if (p < 0) p += q;
+    if (2 * p > q) { p = q - p; neg_s = 1; }               /* a -> 2pi - a                 */
+    if (4 * p > q) { p = q - 2 * p; q = 2 * q; neg_c = 1; } /* a -> pi - a   (p/q in [0,1/4]) */
+    if (8 * p > q) { p = q - 4 * p; q = 4 * q; swap = 1; }  /* a -> pi/2 - a (p/q in [0,1/8]) */
+    double a = 2.0 * PI * ((double)p / (double)q);
+    double sv = sin(a), cv = cos(a);
+    if (swap) { double t = sv; sv = cv; cv = t; }
+    *s = neg_s ? -sv : sv;
+    *c = neg_c ? -cv : cv;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * 1-D transforms
+ * ---------------------------------------------------------------------------------------- */
+
+/* Brute-force DFT straight from eq. (8), unnormalised in both directions:
+ * out[k] = sum_n in[n] exp(sign * 2 pi i n k / N), sign = -1 forward, +1 backward. */
+void orc_dft_direct(int n, int sign, const cplx *in, cplx *out)
+{
+    for (int k = 0; k < n; ++k) {
+        long double sr = 0.0L, si = 0.0L;
+        for (int j = 0; j < n; ++j) {
+            double s, c;
+            sincos2pi((i64)j * k, n, &s, &c);
+            if (sign < 0) s = -s;
+            double xr = creal(in[j]), xi = cimag(in[j]);
+            sr += (long double)xr * c - (long double)xi * s;
+            si += (long double)xr * s + (long double)xi * c;
+        }
+        out[k] = (double)sr + I * (double)si;
+    }
+}
+
+/* twiddle table for a power-of-two length: tw[j] = exp(-2 pi i j / n), j < n */
+static cplx *make_twiddles(int n)
+{
+    cplx *tw = (cplx *)malloc(sizeof(cplx) * (size_t)(n > 0 ? n : 1));
+    if (!tw) return NULL;
+    for (int j = 0; j < n; ++j) {
+        double s, c;
+        sincos2pi(j, n, &s, &c);
+        tw[j] = c - I * s;
+    }
+    return tw;
+}
+
+/* Recursive decimation-in-time radix-2 FFT (Cooley-Tukey, PAPER.md ref. [16]):
+ *   X[k]       = E[k] + w^k O[k]
+ *   X[k + n/2] = E[k] - w^k O[k],  w = exp(sign 2 pi i / n)
+ * with E, O the transforms of the even / odd samples.  tw holds exp(-2 pi i j / ntop) and is
+ * read with stride ntop/n; the backward transform conjugates it.  scratch has n entries. */
+static void fft_rec(int n, int sign, const cplx *in, int istride, cplx *out, cplx *scratch,
+                    const cplx *tw, int twstride)
+{
+    if (n == 1) { out[0] = in[0]; return; }
+    int h = n / 2;
+    fft_rec(h, sign, in, 2 * istride, scratch, out, tw, 2 * twstride);
+    fft_rec(h, sign, in + istride, 2 * istride, scratch + h, out + h, tw, 2 * twstride);
+    for (int k = 0; k < h; ++k) {
+        cplx w = tw[(size_t)k * twstride];
+        if (sign > 0) w = conj(w);
+        cplx e = scratch[k], o = w * scratch[k + h];
+        out[k] = e + o;
+        out[k + h] = e - o;
+    }
+}
+
+static int is_pow2(i64 n) { return n >= 1 && (n & (n - 1)) == 0; }
+
+/* power-of-two FFT, unnormalised, sign = -1 forward / +1 backward. */
+int orc_fft_pow2(int n, int sign, const cplx *in, cplx *out)
+{
+    if (!is_pow2(n)) return ORC_ERR_ARG;
+    cplx *tw = make_twiddles(n);
+    cplx *scratch = (cplx *)malloc(sizeof(cplx) * (size_t)n);
+    cplx *tmp = (cplx *)malloc(sizeof(cplx) * (size_t)n);
+    if (!tw || !scratch || !tmp) { free(tw); free(scratch); free(tmp); return ORC_ERR_ALLOC; }
+    memcpy(tmp, in, sizeof(cplx) * (size_t)n);
+    fft_rec(n, sign, tmp, 1, out, scratch, tw, 1);
+    free(tw); free(scratch); free(tmp);
+    return ORC_OK;
+}
+
+/* DST-I:  Y_k = 2 sum_{j=0}^{N-1} X_j sin(pi (j+1)(k+1)/(N+1))   (Table 1 row 1; odd extension) */
+void orc_dst1_direct(int n, const double *in, double *out)
+{
+    i64 q = 2 * ((i64)n + 1);
+    for (int k = 0; k < n; ++k) {
+        long double acc = 0.0L;
+        for (int j = 0; j < n; ++j) {
+            double s, c;
+            sincos2pi((i64)(j + 1) * (k + 1), q, &s, &c);
+            acc += (long double)in[j] * s;
+        }
+        out[k] = (double)(2.0L * acc);
+    }
+}
+
+/* DCT-II: Y_k = 2 sum_{j=0}^{N-1} X_j cos(pi (j+1/2) k / N)      (Table 1 row 4; even extension) */
+void orc_dct2_direct(int n, const double *in, double *out)
+{
+    i64 q = 4 * (i64)n;
+    for (int k = 0; k < n; ++k) {
+        long double acc = 0.0L;
+        for (int j = 0; j < n; ++j) {
+            double s, c;
+            sincos2pi((i64)(2 * j + 1) * k, q, &s, &c);
+            acc += (long double)in[j] * c;
+        }
+        out[k] = (double)(2.0L * acc);
+    }
+}
+
+/* DCT-III: Y_j = X_0 + 2 sum_{k=1}^{N-1} X_k cos(pi k (j+1/2) / N)   (inverse of DCT-II up to 2N) */
+void orc_dct3_direct(int n, const double *in, double *out)
+{
+    i64 q = 4 * (i64)n;
+    for (int j = 0; j < n; ++j) {
+        long double acc = 0.0L;
+        for (int k = 1; k < n; ++k) {
+            double s, c;
+            sincos2pi((i64)(2 * j + 1) * k, q, &s, &c);
+            acc += (long double)in[k] * c;
+        }
+        out[j] = (double)((long double)in[0] + 2.0L * acc);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Table-driven versions of the same sums for the N-D solvers (the table is the list of all
+ * sin / cos values of the reduced integer argument; the sum is unchanged).
+ * ---------------------------------------------------------------------------------------- */
+typedef struct { int n; i64 q; double *sn; double *cs; } trig_table;
+
+static int trig_table_init(trig_table *t, int n, i64 q)
+{
+    t->n = n; t->q = q;
+    t->sn = (double *)malloc(sizeof(double) * (size_t)q);
+    t->cs = (double *)malloc(sizeof(double) * (size_t)q);
+    if (!t->sn || !t->cs) return ORC_ERR_ALLOC;
+    for (i64 m = 0; m < q; ++m) sincos2pi(m, q, &t->sn[m], &t->cs[m]);
+    return ORC_OK;
+}
+static void trig_table_free(trig_table *t) { free(t->sn); free(t->cs); t->sn = t->cs = NULL; }
+
+static void dst1_tab(const trig_table *t, const double *in, double *out)
+{
+    int n = t->n;
+    for (int k = 0; k < n; ++k) {
+        long double acc = 0.0L;
+        for (int j = 0; j < n; ++j)
+            acc += (long double)in[j] * t->sn[((i64)(j + 1) * (k + 1)) % t->q];
+        out[k] = (double)(2.0L * acc);
+    }
+}
+static void dct2_tab(const trig_table *t, const double *in, double *out)
+{
+    int n = t->n;
+    for (int k = 0; k < n; ++k) {
+        long double acc = 0.0L;
+        for (int j = 0; j < n; ++j)
+            acc += (long double)in[j] * t->cs[((i64)(2 * j + 1) * k) % t->q];
+        out[k] = (double)(2.0L * acc);
+    }
+}
+static void dct3_tab(const trig_table *t, const double *in, double *out)
+{
+    int n = t->n;
+    for (int j = 0; j < n; ++j) {
+        long double acc = 0.0L;
+        for (int k = 1; k < n; ++k)
+            acc += (long double)in[k] * t->cs[((i64)(2 * j + 1) * k) % t->q];
+        out[j] = (double)((long double)in[0] + 2.0L * acc);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * N-D helpers: apply a 1-D transform to every pencil along one axis of a dense array
+ * (PAPER.md:89-97).  One pencil is copied to a contiguous buffer, transformed, copied back.
+ * ---------------------------------------------------------------------------------------- */
+static void axis_geometry(const i64 dims[3], int axis, i64 *len, i64 *stride, i64 *na, i64 *sa,
+                          i64 *nb, i64 *sb)
+{
+    i64 st[3] = { 1, dims[0], dims[0] * dims[1] };
+    int a = (axis + 1) % 3, b = (axis + 2) % 3;
+    *len = dims[axis]; *stride = st[axis];
+    *na = dims[a]; *sa = st[a];
+    *nb = dims[b]; *sb = st[b];
+}
+
+/* complex FFT (power of two) along one axis, in place, unnormalised */
+static int fft_axis(cplx *a, const i64 dims[3], int axis, int sign)
+{
+    i64 len, stride, na, sa, nb, sb;
+    axis_geometry(dims, axis, &len, &stride, &na, &sa, &nb, &sb);
+    if (!is_pow2(len)) return ORC_ERR_ARG;
+    if (len == 1) return ORC_OK;
+    cplx *tw = make_twiddles((int)len);
+    if (!tw) return ORC_ERR_ALLOC;
+    int err = ORC_OK;
+#pragma omp parallel
+    {
+        cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)len * 3);
+        if (!buf) {
+#pragma omp critical
+            err = ORC_ERR_ALLOC;
+        }
+#pragma omp for collapse(2) schedule(static)
+        for (i64 ib = 0; ib < nb; ++ib)
+            for (i64 ia = 0; ia < na; ++ia) {
+                if (!buf) continue;
+                cplx *p = a + ia * sa + ib * sb;
+                cplx *in = buf, *out = buf + len, *scr = buf + 2 * len;
+                for (i64 j = 0; j < len; ++j) in[j] = p[j * stride];
+                fft_rec((int)len, sign, in, 1, out, scr, tw, 1);
+                for (i64 j = 0; j < len; ++j) p[j * stride] = out[j];
+            }
+        free(buf);
+    }
+    free(tw);
+    return err;
+}
+
+typedef void (*real_xform)(const trig_table *, const double *, double *);
+
+/* real-to-real transform along one axis of a dense real array, in place */
+static int r2r_axis(double *a, const i64 dims[3], int axis, real_xform fn, const trig_table *t)
+{
+    i64 len, stride, na, sa, nb, sb;
+    axis_geometry(dims, axis, &len, &stride, &na, &sa, &nb, &sb);
+    int err = ORC_OK;
+#pragma omp parallel
+    {
+        double *buf = (double *)malloc(sizeof(double) * (size_t)len * 2);
+        if (!buf) {
+#pragma omp critical
+            err = ORC_ERR_ALLOC;
+        }
+#pragma omp for collapse(2) schedule(static)
+        for (i64 ib = 0; ib < nb; ++ib)
+            for (i64 ia = 0; ia < na; ++ia) {
+                if (!buf) continue;
+                double *p = a + ia * sa + ib * sb;
+                double *in = buf, *out = buf + len;
+                for (i64 j = 0; j < len; ++j) in[j] = p[j * stride];
+                fn(t, in, out);
+                for (i64 j = 0; j < len; ++j) p[j * stride] = out[j];
+            }
+        free(buf);
+    }
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-PER: periodic solver (configs 1, 2).
+ *
+ * nd = 2 or 3 (unused axes have n = 1).  Real data are stored as complex with zero imaginary
+ * part and transformed with the plain C2C DFT, as the paper does.
+ *   op = 0: pseudo-spectral  Lambda = - sum_a kappa_a^2, kappa_a = 2 pi m_a / L_a,
+ *           m_a = k_a (k_a < N_a/2) else k_a - N_a             (Table 1)
+ *   op = 1: FD2              Lambda = - sum_a (4/h_a^2) sin^2(pi k_a / N_a)
+ * psi_hat = rhs_sign * F / Lambda, zero at the all-zero index; the 1/N of eq. (8)
+ * is applied on the inverse.  Gradient: g_a = IDFT(i kappa_a psi_hat) (eq. 10) with
+ * kappa_a := 0 at the Nyquist index (reading A20).
+ * f, psi: n0*n1*n2 reals; grad (may be NULL): nd fields of that size, component-major.
+ * ---------------------------------------------------------------------------------------- */
+int orc_periodic(int nd, const i64 n[3], const double L[3], int op, double rhs_sign,
+                 const double *f, double *psi, double *grad)
+{
+    if (nd < 1 || nd > 3) return ORC_ERR_ARG;
+    i64 dims[3] = { n[0], nd > 1 ? n[1] : 1, nd > 2 ? n[2] : 1 };
+    i64 tot = dims[0] * dims[1] * dims[2];
+    for (int a = 0; a < 3; ++a) if (!is_pow2(dims[a])) return ORC_ERR_ARG;
+
+    cplx *F = (cplx *)malloc(sizeof(cplx) * (size_t)tot);
+    cplx *W = grad ? (cplx *)malloc(sizeof(cplx) * (size_t)tot) : NULL;
+    double *kap[3] = { 0, 0, 0 }, *lam[3] = { 0, 0, 0 };
+    int err = ORC_OK;
+    if (!F || (grad && !W)) { err = ORC_ERR_ALLOC; goto done; }
+
+    /* per-axis wavenumbers and eigenvalue contributions */
+    for (int a = 0; a < 3; ++a) {
+        i64 N = dims[a];
+        kap[a] = (double *)calloc((size_t)N, sizeof(double));
+        lam[a] = (double *)calloc((size_t)N, sizeof(double));
+        if (!kap[a] || !lam[a]) { err = ORC_ERR_ALLOC; goto done; }
+        if (a >= nd) continue; /* unused axis: single zero mode */
+        double h = L[a] / (double)N;
+        for (i64 k = 0; k < N; ++k) {
+            i64 m = (2 * k < N) ? k : k - N;
+            double kappa = 2.0 * PI * (double)m / L[a];
+            kap[a][k] = (2 * k == N) ? 0.0 : kappa; /* used for ik only */
+            if (op == 0) {
+                lam[a][k] = -kappa * kappa;
+            } else {
+                double s, c;
+                sincos2pi(k, 2 * N, &s, &c); /* sin(pi k / N) */
+                lam[a][k] = -(4.0 / (h * h)) * s * s;
+            }
+        }
+    }
+
+    /* 1. forward transform (x, then y, then z) */
+#pragma omp parallel for schedule(static)
+    for (i64 i = 0; i < tot; ++i) F[i] = f[i];
+    for (int a = 0; a < nd; ++a)
+        if ((err = fft_axis(F, dims, a, -1)) != ORC_OK) goto done;
+
+    /* 2. convolution: divide by the eigenvalue, zero mode -> 0 */
+#pragma omp parallel for collapse(2) schedule(static)
+    for (i64 kz = 0; kz < dims[2]; ++kz)
+        for (i64 ky = 0; ky < dims[1]; ++ky)
+            for (i64 kx = 0; kx < dims[0]; ++kx) {
+                i64 i = kx + dims[0] * (ky + dims[1] * kz);
+                if (kx == 0 && ky == 0 && kz == 0) { F[i] = 0.0; continue; }
+                double Lam = lam[0][kx] + lam[1][ky] + lam[2][kz];
+                F[i] = rhs_sign * F[i] / Lam;
+            }
+
+    /* 3. spectral operations + 4. backward transform (z, y, x), 1/N on the inverse */
+    double inv_n = 1.0 / (double)tot;
+    if (grad) {
+        for (int g = 0; g < nd; ++g) {
+#pragma omp parallel for collapse(2) schedule(static)
+            for (i64 kz = 0; kz < dims[2]; ++kz)
+                for (i64 ky = 0; ky < dims[1]; ++ky)
+                    for (i64 kx = 0; kx < dims[0]; ++kx) {
+                        i64 i = kx + dims[0] * (ky + dims[1] * kz);
+                        i64 kk[3] = { kx, ky, kz };
+                        W[i] = I * kap[g][kk[g]] * F[i];
+                    }
+            for (int a = nd - 1; a >= 0; --a)
+                if ((err = fft_axis(W, dims, a, +1)) != ORC_OK) goto done;
+            double *out = grad + (size_t)g * (size_t)tot;
+#pragma omp parallel for schedule(static)
+            for (i64 i = 0; i < tot; ++i) out[i] = creal(W[i]) * inv_n;
+        }
+    }
+    for (int a = nd - 1; a >= 0; --a)
+        if ((err = fft_axis(F, dims, a, +1)) != ORC_OK) goto done;
+#pragma omp parallel for schedule(static)
+    for (i64 i = 0; i < tot; ++i) psi[i] = creal(F[i]) * inv_n;
+
+done:
+    for (int a = 0; a < 3; ++a) { free(kap[a]); free(lam[a]); }
+    free(F); free(W);
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Boundary-value folding (weights: reading A18).
+ * faces[2*axis + side] (side 0 = lower, 1 = upper) holds the values on that face over the two
+ * remaining axes, lower axis fastest; NULL = homogeneous.
+ * ---------------------------------------------------------------------------------------- */
+static void fold_faces(double *fp, const i64 n[3], const double h[3], const double *const faces[6],
+                       int neumann)
+{
+    for (int axis = 0; axis < 3; ++axis) {
+        int a = (axis == 0) ? 1 : 0;           /* lower remaining axis (fastest in the face) */
+        int b = (axis == 2) ? 1 : 2;           /* upper remaining axis */
+        i64 st[3] = { 1, n[0], n[0] * n[1] };
+        for (int side = 0; side < 2; ++side) {
+            const double *g = faces ? faces[2 * axis + side] : NULL;
+            if (!g) continue;
+            i64 ic = side ? n[axis] - 1 : 0;   /* boundary-adjacent layer */
+            double w;
+            if (!neumann) w = -1.0 / (h[axis] * h[axis]);          /* Dirichlet, cell-boundary */
+            else w = side ? -1.0 / h[axis] : +1.0 / h[axis];       /* Neumann, cell-centre     */
+            for (i64 jb = 0; jb < n[b]; ++jb)
+                for (i64 ja = 0; ja < n[a]; ++ja)
+                    fp[ic * st[axis] + ja * st[a] + jb * st[b]] += w * g[ja + n[a] * jb];
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-DIR: Dirichlet, cell-boundary (REGULAR) grid, DST-I forward and backward (Table 1 row 1).
+ * n = interior nodes per axis; node j sits at (j+1) h; L = (n+1) h.
+ *   op = 1 (FD2): Lambda = -sum_a (4/h_a^2) sin^2(pi (k_a+1) / (2 (N_a+1)))
+ *   op = 0 (PS):  Lambda = -sum_a (pi (k_a+1) / L_a)^2       (homogeneous faces only)
+ * psi = DST-I_3(rhs_sign * DST-I_3(f') / Lambda) / prod_a (2 (N_a+1)).
+ * ---------------------------------------------------------------------------------------- */
+int orc_dirichlet_regular(const i64 n[3], const double h[3], int op, double rhs_sign, const double *f,
+                          const double *const faces[6], double *psi)
+{
+    i64 tot = n[0] * n[1] * n[2];
+    trig_table tab[3];
+    double *lam[3] = { 0, 0, 0 };
+    int err = ORC_OK, ntab = 0;
+    memcpy(psi, f, sizeof(double) * (size_t)tot);
+    if (op == 1) fold_faces(psi, n, h, faces, 0);
+    for (int a = 0; a < 3; ++a) {
+        if ((err = trig_table_init(&tab[a], (int)n[a], 2 * (n[a] + 1))) != ORC_OK) { ntab = a + 1; goto done; }
+        ntab = a + 1;
+        lam[a] = (double *)malloc(sizeof(double) * (size_t)n[a]);
+        if (!lam[a]) { err = ORC_ERR_ALLOC; goto done; }
+        double Ldom = (double)(n[a] + 1) * h[a];
+        for (i64 k = 0; k < n[a]; ++k) {
+            if (op == 0) {
+                double kk = PI * (double)(k + 1) / Ldom;
+                lam[a][k] = -kk * kk;
+            } else {
+                double s, c;
+                sincos2pi(k + 1, 4 * (n[a] + 1), &s, &c); /* sin(pi (k+1) / (2(N+1))) */
+                lam[a][k] = -(4.0 / (h[a] * h[a])) * s * s;
+            }
+        }
+    }
+    for (int a = 0; a < 3; ++a)
+        if ((err = r2r_axis(psi, n, a, dst1_tab, &tab[a])) != ORC_OK) goto done;
+    double norm = 1.0;
+    for (int a = 0; a < 3; ++a) norm *= 2.0 * (double)(n[a] + 1);
+#pragma omp parallel for collapse(2) schedule(static)
+    for (i64 kz = 0; kz < n[2]; ++kz)
+        for (i64 ky = 0; ky < n[1]; ++ky)
+            for (i64 kx = 0; kx < n[0]; ++kx) {
+                i64 i = kx + n[0] * (ky + n[1] * kz);
+                psi[i] = rhs_sign * psi[i] / (lam[0][kx] + lam[1][ky] + lam[2][kz]);
+            }
+    for (int a = 2; a >= 0; --a)
+        if ((err = r2r_axis(psi, n, a, dst1_tab, &tab[a])) != ORC_OK) goto done;
+#pragma omp parallel for schedule(static)
+    for (i64 i = 0; i < tot; ++i) psi[i] /= norm;
+done:
+    for (int a = 0; a < ntab; ++a) trig_table_free(&tab[a]);
+    for (int a = 0; a < 3; ++a) free(lam[a]);
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-NEU: Neumann, cell-centre (STAGGERED) grid, DCT-II forward, DCT-III backward (Table 1 row 4;
+ * the printed "DST-III" is read as DCT-III, reading A2).  n = cells per axis, x_j = (j+1/2) h.
+ *   op = 1 (FD2): Lambda = -sum_a (4/h_a^2) sin^2(pi k_a / (2 N_a))
+ *   op = 0 (PS):  Lambda = -sum_a (pi k_a / L_a)^2, L_a = N_a h_a   (reading A1)
+ * Zero mode -> 0.  psi = DCT-III_3(rhs_sign * DCT-II_3(f') / Lambda) / prod_a (2 N_a).
+ * ---------------------------------------------------------------------------------------- */
+int orc_neumann_staggered(const i64 n[3], const double h[3], int op, double rhs_sign, const double *f,
+                          const double *const faces[6], double *psi)
+{
+    i64 tot = n[0] * n[1] * n[2];
+    trig_table tab[3];
+    double *lam[3] = { 0, 0, 0 };
+    int err = ORC_OK, ntab = 0;
+    memcpy(psi, f, sizeof(double) * (size_t)tot);
+    if (op == 1) fold_faces(psi, n, h, faces, 1);
+    for (int a = 0; a < 3; ++a) {
+        if ((err = trig_table_init(&tab[a], (int)n[a], 4 * n[a])) != ORC_OK) { ntab = a + 1; goto done; }
+        ntab = a + 1;
+        lam[a] = (double *)malloc(sizeof(double) * (size_t)n[a]);
+        if (!lam[a]) { err = ORC_ERR_ALLOC; goto done; }
+        double Ldom = (double)n[a] * h[a];
+        for (i64 k = 0; k < n[a]; ++k) {
+            if (op == 0) {
+                double kk = PI * (double)k / Ldom;
+                lam[a][k] = -kk * kk;
+            } else {
+                double s, c;
+                sincos2pi(k, 4 * n[a], &s, &c); /* sin(pi k / (2N)) */
+                lam[a][k] = -(4.0 / (h[a] * h[a])) * s * s;
+            }
+        }
+    }
+    for (int a = 0; a < 3; ++a)
+        if ((err = r2r_axis(psi, n, a, dct2_tab, &tab[a])) != ORC_OK) goto done;
+    double norm = 1.0;
+    for (int a = 0; a < 3; ++a) norm *= 2.0 * (double)n[a];
+#pragma omp parallel for collapse(2) schedule(static)
+    for (i64 kz = 0; kz < n[2]; ++kz)
+        for (i64 ky = 0; ky < n[1]; ++ky)
+            for (i64 kx = 0; kx < n[0]; ++kx) {
+                i64 i = kx + n[0] * (ky + n[1] * kz);
+                if (kx == 0 && ky == 0 && kz == 0) { psi[i] = 0.0; continue; }
+                psi[i] = rhs_sign * psi[i] / (lam[0][kx] + lam[1][ky] + lam[2][kz]);
+            }
+    for (int a = 2; a >= 0; --a)
+        if ((err = r2r_axis(psi, n, a, dct3_tab, &tab[a])) != ORC_OK) goto done;
+#pragma omp parallel for schedule(static)
+    for (i64 i = 0; i < tot; ++i) psi[i] /= norm;
+done:
+    for (int a = 0; a < ntab; ++a) trig_table_free(&tab[a]);
+    for (int a = 0; a < 3; ++a) free(lam[a]);
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-UNB / O-VEC: unbounded solver, Hockney-Eastwood on the whole doubled domain.
+ *
+ * Real-space kernel: 2nd-order Gaussian-regularised Green's function of Hejlesen (
+ * formula not printed in the paper -- reading A10):
+ *     G(r) = -erf(r / (sqrt(2) eps)) / (4 pi r),   G(0) = -1 / ((2 pi)^(3/2) eps),
+ * so that lap G -> delta (sign of PAPER.md:38).
+ * Definition being computed (discretised eq. (3); weight hx hy hz: reading A11):
+ *     psi_i = rhs_sign * hx hy hz * sum_j G(|x_i - x_j|) f_j .
+ * ---------------------------------------------------------------------------------------- */
+double orc_green_gauss2(double r, double eps)
+{
+    if (r == 0.0) return -1.0 / (pow(2.0 * PI, 1.5) * eps);
+    return -erf(r / (sqrt(2.0) * eps)) / (4.0 * PI * r);
+}
+
+/* half-spectrum geometry on the doubled grid: [P2][P1][N0+1] complex, x fastest */
+static i64 unb_spec_size(const i64 n[3]) { return (n[0] + 1) * (2 * n[1]) * (2 * n[2]); }
+i64 orc_unbounded_spec_size(const i64 n[3]) { return unb_spec_size(n); }
+
+/* forward transform of a real field given on the doubled grid by a callback-free rule:
+ * src is either the n-sized source (zero-padded, pad = 1) or a full doubled real array (pad = 0).
+ * x: full complex DFT of length P0 of each (padded) row, outputs k = 0..N0 kept (the rest follow
+ * from Hermitian symmetry); then y; then z. */
+static int unb_forward(const i64 n[3], const double *src, int pad, cplx *spec)
+{
+    i64 P0 = 2 * n[0], P1 = 2 * n[1], P2 = 2 * n[2], H0 = n[0] + 1;
+    cplx *tw = make_twiddles((int)P0);
+    if (!tw) return ORC_ERR_ALLOC;
+    int err = ORC_OK;
+#pragma omp parallel
+    {
+        cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)P0 * 3);
+        if (!buf) {
+#pragma omp critical
+            err = ORC_ERR_ALLOC;
+        }
+#pragma omp for collapse(2) schedule(static)
+        for (i64 iz = 0; iz < P2; ++iz)
+            for (i64 iy = 0; iy < P1; ++iy) {
+                if (!buf) continue;
+                cplx *in = buf, *out = buf + P0, *scr = buf + 2 * P0;
+                for (i64 ix = 0; ix < P0; ++ix) {
+                    double v;
+                    if (pad) v = (ix < n[0] && iy < n[1] && iz < n[2]) ? src[ix + n[0] * (iy + n[1] * iz)] : 0.0;
+                    else v = src[ix + P0 * (iy + P1 * iz)];
+                    in[ix] = v;
+                }
+                fft_rec((int)P0, -1, in, 1, out, scr, tw, 1);
+                cplx *row = spec + H0 * (iy + P1 * iz);
+                for (i64 k = 0; k < H0; ++k) row[k] = out[k];
+            }
+        free(buf);
+    }
+    free(tw);
+    if (err != ORC_OK) return err;
+    i64 sdims[3] = { H0, P1, P2 };
+    if ((err = fft_axis(spec, sdims, 1, -1)) != ORC_OK) return err;
+    return fft_axis(spec, sdims, 2, -1);
+}
+
+/* backward transform of a half-spectrum (z, then y, then x), 1/(P0 P1 P2) applied, first octant
+ * extracted.  spec is destroyed. */
+static int unb_backward_extract(const i64 n[3], cplx *spec, double *out)
+{
+    i64 P0 = 2 * n[0], P1 = 2 * n[1], P2 = 2 * n[2], H0 = n[0] + 1;
+    i64 sdims[3] = { H0, P1, P2 };
+    int err;
+    if ((err = fft_axis(spec, sdims, 2, +1)) != ORC_OK) return err;
+    if ((err = fft_axis(spec, sdims, 1, +1)) != ORC_OK) return err;
+    cplx *tw = make_twiddles((int)P0);
+    if (!tw) return ORC_ERR_ALLOC;
+    double inv = 1.0 / ((double)P0 * (double)P1 * (double)P2);
+#pragma omp parallel
+    {
+        cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)P0 * 3);
+        if (!buf) {
+#pragma omp critical
+            err = ORC_ERR_ALLOC;
+        }
+#pragma omp for collapse(2) schedule(static)
+        for (i64 iz = 0; iz < n[2]; ++iz)
+            for (i64 iy = 0; iy < n[1]; ++iy) {
+                if (!buf) continue;
+                cplx *in = buf, *o = buf + P0, *scr = buf + 2 * P0;
+                const cplx *row = spec + H0 * (iy + P1 * iz);
+                for (i64 k = 0; k < H0; ++k) in[k] = row[k];
+                for (i64 k = 1; k < n[0]; ++k) in[P0 - k] = conj(row[k]); /* Hermitian half */
+                fft_rec((int)P0, +1, in, 1, o, scr, tw, 1);
+                for (i64 ix = 0; ix < n[0]; ++ix) out[ix + n[0] * (iy + n[1] * iz)] = creal(o[ix]) * inv;
+            }
+        free(buf);
+    }
+    free(tw);
+    return err;
+}
+
+/* Green's spectrum: G on the doubled grid at mirrored distance d_a = min(i_a, P_a - i_a) h_a
+ * (reading A12), times the cell volume, forward transformed once.
+ * ghat: (n0+1) * 2 n1 * 2 n2 complex. */
+int orc_unbounded_green(const i64 n[3], const double h[3], double eps, cplx *ghat)
+{
+    for (int a = 0; a < 3; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
+    i64 P0 = 2 * n[0], P1 = 2 * n[1], P2 = 2 * n[2];
+    double *g = (double *)malloc(sizeof(double) * (size_t)(P0 * P1 * P2));
+    if (!g) return ORC_ERR_ALLOC;
+    double vol = h[0] * h[1] * h[2];
+#pragma omp parallel for collapse(2) schedule(static)
+    for (i64 iz = 0; iz < P2; ++iz)
+        for (i64 iy = 0; iy < P1; ++iy)
+            for (i64 ix = 0; ix < P0; ++ix) {
+                double dx = (double)(ix < P0 - ix ? ix : P0 - ix) * h[0];
+                double dy = (double)(iy < P1 - iy ? iy : P1 - iy) * h[1];
+                double dz = (double)(iz < P2 - iz ? iz : P2 - iz) * h[2];
+                g[ix + P0 * (iy + P1 * iz)] = vol * orc_green_gauss2(sqrt(dx * dx + dy * dy + dz * dz), eps);
+            }
+    int err = unb_forward(n, g, 0, ghat);
+    free(g);
+    return err;
+}
+
+/* Solve with a stored Green's spectrum.
+ * f: ncomp fields of n0*n1*n2 (component-major).  out: ncomp fields; if want_curl (ncomp == 3)
+ * out = u = curl psi computed in the same spectral pass: u_hat = i kappa x psi_hat, with
+ * kappa_a = 2 pi m_a / (P_a h_a), m_a in [-N_a, N_a) on the DOUBLED grid, Nyquist -> 0
+ * (reading A20).  Otherwise out = psi. */
+int orc_unbounded_solve(const i64 n[3], const double h[3], const cplx *ghat, int ncomp, double rhs_sign,
+                        const double *f, int want_curl, double *out)
+{
+    if (want_curl && ncomp != 3) return ORC_ERR_ARG;
+    for (int a = 0; a < 3; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
+    i64 tot = n[0] * n[1] * n[2], ns = unb_spec_size(n);
+    i64 P[3] = { 2 * n[0], 2 * n[1], 2 * n[2] }, H0 = n[0] + 1;
+    cplx *spec[3] = { 0, 0, 0 };
+    cplx *work = NULL;
+    double *kap[3] = { 0, 0, 0 };
+    int err = ORC_OK;
+
+    for (int c = 0; c < ncomp; ++c) {
+        spec[c] = (cplx *)malloc(sizeof(cplx) * (size_t)ns);
+        if (!spec[c]) { err = ORC_ERR_ALLOC; goto done; }
+        if ((err = unb_forward(n, f + (size_t)c * (size_t)tot, 1, spec[c])) != ORC_OK) goto done;
+#pragma omp parallel for schedule(static)
+        for (i64 i = 0; i < ns; ++i) spec[c][i] = rhs_sign * ghat[i] * spec[c][i];
+        if (!want_curl) {
+            if ((err = unb_backward_extract(n, spec[c], out + (size_t)c * (size_t)tot)) != ORC_OK) goto done;
+            free(spec[c]); spec[c] = NULL;
+        }
+    }
+    if (want_curl) {
+        for (int a = 0; a < 3; ++a) {
+            kap[a] = (double *)malloc(sizeof(double) * (size_t)P[a]);
+            if (!kap[a]) { err = ORC_ERR_ALLOC; goto done; }
+            for (i64 k = 0; k < P[a]; ++k) {
+                i64 m = (k < n[a]) ? k : k - P[a];
+                kap[a][k] = (k == n[a]) ? 0.0 : 2.0 * PI * (double)m / ((double)P[a] * h[a]);
+            }
+        }
+        work = (cplx *)malloc(sizeof(cplx) * (size_t)ns);
+        if (!work) { err = ORC_ERR_ALLOC; goto done; }
+        for (int a = 0; a < 3; ++a) {
+            int b = (a + 1) % 3, c = (a + 2) % 3; /* u_a = d_b psi_c - d_c psi_b */
+#pragma omp parallel for collapse(2) schedule(static)
+            for (i64 kz = 0; kz < P[2]; ++kz)
+                for (i64 ky = 0; ky < P[1]; ++ky)
+                    for (i64 kx = 0; kx < H0; ++kx) {
+                        i64 i = kx + H0 * (ky + P[1] * kz);
+                        i64 kk[3] = { kx, ky, kz };
+                        work[i] = I * (kap[b][kk[b]] * spec[c][i] - kap[c][kk[c]] * spec[b][i]);
+                    }
+            if ((err = unb_backward_extract(n, work, out + (size_t)a * (size_t)tot)) != ORC_OK) goto done;
+        }
+    }
+done:
+    for (int c = 0; c < 3; ++c) { free(spec[c]); free(kap[c]); }
+    free(work);
+    return err;
+}
+
+/* Direct O(N^6) evaluation of the definition above (scalar), for tiny grids only (pin P6). */
+void orc_unbounded_direct(const i64 n[3], const double h[3], double eps, double rhs_sign, const double *f,
+                          double *psi)
+{
+    double vol = h[0] * h[1] * h[2];
+#pragma omp parallel for collapse(2) schedule(static)
+    for (i64 iz = 0; iz < n[2]; ++iz)
+        for (i64 iy = 0; iy < n[1]; ++iy)
+            for (i64 ix = 0; ix < n[0]; ++ix) {
+                long double acc = 0.0L;
+                for (i64 jz = 0; jz < n[2]; ++jz)
+                    for (i64 jy = 0; jy < n[1]; ++jy)
+                        for (i64 jx = 0; jx < n[0]; ++jx) {
+                            double dx = (double)(ix - jx) * h[0], dy = (double)(iy - jy) * h[1],
+                                   dz = (double)(iz - jz) * h[2];
+                            acc += (long double)orc_green_gauss2(sqrt(dx * dx + dy * dy + dz * dz), eps) *
+                                   f[jx + n[0] * (jy + n[1] * jz)];
+                        }
+                psi[ix + n[0] * (iy + n[1] * iz)] = (double)(rhs_sign * vol * acc);
+            }
+}
+
+/* Direct evaluation of the definition at a list of output points (full-size sampled parity):
+ * psi(idx[s]) for s < ns, idx = linear grid indices. */
+void orc_unbounded_direct_samples(const i64 n[3], const double h[3], double eps, double rhs_sign,
+                                  const double *f, i64 ns, const i64 *idx, double *psi)
+{
+    double vol = h[0] * h[1] * h[2];
+    for (i64 s = 0; s < ns; ++s) {
+        i64 ix = idx[s] % n[0], iy = (idx[s] / n[0]) % n[1], iz = idx[s] / (n[0] * n[1]);
+        double acc = 0.0;
+#pragma omp parallel for reduction(+ : acc) schedule(static)
+        for (i64 jz = 0; jz < n[2]; ++jz) {
+            long double a = 0.0L;
+            for (i64 jy = 0; jy < n[1]; ++jy)
+                for (i64 jx = 0; jx < n[0]; ++jx) {
+                    double fv = f[jx + n[0] * (jy + n[1] * jz)];
+                    if (fv == 0.0) continue;
+                    double dx = (double)(ix - jx) * h[0], dy = (double)(iy - jy) * h[1],
+                           dz = (double)(iz - jz) * h[2];
+                    a += (long double)orc_green_gauss2(sqrt(dx * dx + dy * dy + dz * dz), eps) * fv;
+                }
+            acc += (double)a;
+        }
+        psi[s] = rhs_sign * vol * acc;
+    }
+}

@@ -1,0 +1,132 @@
+"""Pins P5, P6, P7, P10, P11 for the unbounded (Hockney-Eastwood) oracle."""
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+from analytic import gaussian_blob_potential, gaussian_blob_potential_gradient, rel_l2
+
+
+def test_kernel_values():
+    eps = 0.3
+    # G(0) is the r -> 0 limit of -erf(r/(sqrt2 eps))/(4 pi r); far field -> -1/(4 pi r)
+    assert np.isclose(O.green_gauss2(0.0, eps), O.green_gauss2(1e-7, eps), rtol=1e-10)
+    assert np.isclose(O.green_gauss2(0.0, eps), -1.0 / ((2 * np.pi) ** 1.5 * eps), rtol=1e-15)
+    assert np.isclose(O.green_gauss2(10.0, eps), -1.0 / (4 * np.pi * 10.0), rtol=1e-15)
+
+
+@pytest.mark.parametrize("shape", [(8, 8, 8), (16, 16, 16), (16, 4, 8)])
+def test_direct_summation_of_the_definition(shape):
+    # P6: the doubled-domain FFT convolution equals the O(N^6) sum (linear, not circular)
+    rng = np.random.default_rng(1)
+    f = rng.normal(size=shape)
+    n = tuple(reversed(shape))
+    h = (0.11, 0.07, 0.13)
+    eps = 2 * max(h)
+    gh = O.unbounded_green(n, h, eps)
+    psi = O.unbounded_solve(f, h, gh)
+    ref = O.unbounded_direct(f, h, eps)
+    assert np.abs(psi - ref).max() < 1e-14 * np.abs(ref).max() * 50
+    idx = np.array([0, 5, f.size - 1, f.size // 2 + 3])
+    assert np.allclose(O.unbounded_direct_samples(f, h, eps, idx), ref.ravel()[idx], rtol=1e-13)
+    assert np.array_equal(O.unbounded_solve(f, h, gh, rhs_sign=-1.0), -psi)
+
+
+def test_green_spectrum_is_real_and_even():
+    # P7
+    n = (16, 8, 32)
+    gh = O.unbounded_green(n, (0.1, 0.2, 0.05), 0.4)
+    assert np.abs(gh.imag).max() <= 1e-15 * np.abs(gh.real).max()
+    P2, P1 = gh.shape[0], gh.shape[1]
+    kz = (-np.arange(P2)) % P2
+    ky = (-np.arange(P1)) % P1
+    assert np.abs(gh.real - gh.real[kz][:, ky]).max() <= 1e-15 * np.abs(gh.real).max()
+
+
+def test_gaussian_charge_closed_form_single_blob():
+    # P5 (north_star: phi = -erf(r/(sqrt2 sigma))/(4 pi r) for a Gaussian charge; with the regularised
+    # kernel the width is s = sqrt(sigma^2 + eps^2), reading A10)
+    n = 64
+    g = W.gaussian_blobs(n, nblobs=1, sigma_h=(2.0, 2.0), inner=(0.45, 0.55))
+    eps = 2 * g["h"][0]
+    gh = O.unbounded_green(g["n"], g["h"], eps)
+    psi = O.unbounded_solve(g["f"], g["h"], gh)
+    ref = gaussian_blob_potential(g, eps)
+    assert rel_l2(psi, ref) < 1e-14
+    assert np.abs(psi - ref).max() < 1e-13
+    # eps -> 0 form of north_star holds only to O(eps^2)
+    ref0 = gaussian_blob_potential(g, 0.0)
+    assert 1e-3 < rel_l2(psi, ref0) < 1e-1
+
+
+def test_gaussian_charge_closed_form_many_blobs():
+    n = 128
+    g = W.gaussian_blobs(n, nblobs=16, sigma_h=(2.0, 4.0), inner=(0.3, 0.7))
+    eps = 2 * g["h"][0]
+    gh = O.unbounded_green(g["n"], g["h"], eps)
+    psi = O.unbounded_solve(g["f"], g["h"], gh)
+    assert rel_l2(psi, gaussian_blob_potential(g, eps)) < 1e-13
+
+
+@pytest.mark.slow
+def test_cfg4_full_size_closed_form():
+    g = W.gaussian_blobs(256)
+    eps = 2 * g["h"][0]
+    gh = O.unbounded_green(g["n"], g["h"], eps)
+    psi = O.unbounded_solve(g["f"], g["h"], gh)
+    assert rel_l2(psi, gaussian_blob_potential(g, eps)) < 1e-13
+
+
+@pytest.mark.parametrize("comp", [0, 1, 2])
+def test_curl_of_a_gaussian_vorticity_component(comp):
+    # P10: omega = G e_c, lap psi = -omega => psi_c = +q erf(r/(sqrt2 s))/(4 pi r), u = curl psi
+    n = 64
+    g = W.gaussian_blobs(n, nblobs=1, sigma_h=(2.5, 2.5), inner=(0.45, 0.55))
+    eps = 2 * g["h"][0]
+    gh = O.unbounded_green(g["n"], g["h"], eps)
+    omega = np.zeros((3, n, n, n))
+    omega[comp] = g["f"]
+    psi = O.unbounded_solve(omega, g["h"], gh, rhs_sign=-1.0)
+    ref = gaussian_blob_potential(g, eps, sign=+1.0)
+    assert rel_l2(psi[comp], ref) < 1e-13
+    u = O.unbounded_solve(omega, g["h"], gh, rhs_sign=-1.0, want_curl=True)
+    d = gaussian_blob_potential_gradient(g, eps, sign=+1.0)  # (d/dx, d/dy, d/dz) of psi_c
+    b, c = (comp + 1) % 3, (comp + 2) % 3
+    # u_a = d_b psi_c - d_c psi_b with only psi_comp non-zero
+    expect = [np.zeros_like(ref) for _ in range(3)]
+    expect[b] = d[c]          # u_b = d_c psi_comp   (cyclic: u_b = d_c psi_a - d_a psi_c, a = comp)
+    expect[c] = -d[b]         # u_c = d_a psi_b - d_b psi_a = -d_b psi_comp
+    scale = max(np.abs(d[0]).max(), np.abs(d[1]).max(), np.abs(d[2]).max())
+    for a in range(3):
+        assert np.abs(u[a] - expect[a]).max() < 1e-10 * scale
+
+
+def test_vector_solver_is_componentwise_and_linear():
+    # P11 / PAPER.md:119: the 3DV solver applies the scalar solver component by component
+    rng = np.random.default_rng(4)
+    n = 16
+    h = (1.0 / n,) * 3
+    gh = O.unbounded_green((n, n, n), h, 2.0 / n)
+    w = rng.normal(size=(3, n, n, n))
+    psi = O.unbounded_solve(w, h, gh, rhs_sign=-1.0)
+    for c in range(3):
+        assert np.array_equal(psi[c], O.unbounded_solve(w[c], h, gh, rhs_sign=-1.0))
+    u = O.unbounded_solve(w, h, gh, rhs_sign=-1.0, want_curl=True)
+    usum = np.zeros_like(u)
+    for c in range(3):
+        wc = np.zeros_like(w)
+        wc[c] = w[c]
+        usum += O.unbounded_solve(wc, h, gh, rhs_sign=-1.0, want_curl=True)
+    assert np.abs(u - usum).max() < 1e-13 * np.abs(u).max()
+
+
+def test_vortex_ring_centre_velocity():
+    # P11 sanity: thin ring, u_axis(centre) ~ Gamma / (2 R)
+    n = 64
+    r = W.vortex_ring(n, sigma_h=2.0, tilt=0.0)
+    gh = O.unbounded_green(r["n"], r["h"], 2 * r["h"][0])
+    u = O.unbounded_solve(r["omega"], r["h"], gh, rhs_sign=-1.0, want_curl=True)
+    c = n // 2
+    uz = u[2, c - 1:c + 1, c - 1:c + 1, c - 1:c + 1].mean()
+    assert abs(uz - r["gamma"] / (2 * r["radius"])) < 0.05 * r["gamma"] / (2 * r["radius"])
+    assert abs(u[0, c - 1:c + 1, c - 1:c + 1, c - 1:c + 1].mean()) < 1e-3
