@@ -1,0 +1,193 @@
+/*
+ * sailffish.h -- C ABI of the B200-native spectral Poisson hot path (SailFFish, arxiv 2301.01145).
+ *
+ * The library (libsailffish_b200.so, built from paper_2301_01145_b200/csrc/) links the CUDA runtime
+ * only: no torch types, no C++ types and no exceptions cross this boundary.  Every entry point
+ * returns an sf_status; a human-readable message for the last failure on a plan is available from
+ * sf_last_error().  Citations "PAPER.md:<line>" refer to the paper text under /root/reference/.
+ *
+ * What a plan computes (sec 2.2 "four-step spectral solve"):
+ *     1. forward transform of the source along every axis
+ *        - periodic:  real-to-complex DFT                        (eq. 8)
+ *        - Dirichlet, cell-boundary grid:  DST-I                 (Table 1 row 1)
+ *        - Neumann,   cell-centre   grid:  DCT-II                (Table 1 row 4)
+ *        - unbounded: zero-padded to twice the length, real-to-complex DFT
+ *                     (Hockney-Eastwood, sec 2.5; only non-zero pencils are
+ *                     transformed -- the "pruned" variant of PAPER.md:213)
+ *     2. multiply by the spectral multiplier: 1 / eigenvalue of the chosen operator
+ *        (pseudo-spectral or second-order finite difference, Table 1, zero mode
+ *        set to zero) or by the stored transform of the regularised free-space Green's
+ *        function
+ *     3. optional spectral differentiation: multiply by i k (eq. 10) -> gradient
+ *        of the solution, or curl of a 3-component solution
+ *     4. backward transform (DST-I / DCT-III / complex-to-real DFT), unbounded: keep the first octant
+ *
+ * Array layout (all calls): dense, x fastest: index = ix + n[0]*(iy + n[1]*iz); vector fields are
+ * component-major (component c starts at c*n[0]*n[1]*n[2]).  Element type is float (SF_F32) or
+ * double (SF_F64) as chosen at plan creation.
+ *
+ * Threading: calls on one plan must not be issued concurrently; separate plans are independent.
+ * All compute calls are asynchronous on the plan's stream; sf_get_output to host memory and
+ * sf_synchronize block until the stream has drained.
+ */
+#ifndef SAILFFISH_B200_H
+#define SAILFFISH_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sf_plan_s* sf_plan;
+
+typedef enum {
+    SF_OK = 0,
+    SF_ERR_INVALID_ARG = -1, /* NULL pointer, non-positive size, unknown enum value            */
+    SF_ERR_UNSUPPORTED = -2, /* a combination the method / this build does not cover (see below) */
+    SF_ERR_ALLOC = -3,       /* device or host allocation failed                                */
+    SF_ERR_CUDA = -4,        /* a CUDA runtime call or kernel launch failed                     */
+    SF_ERR_STATE = -5        /* call out of order (solve before source, output before solve)    */
+} sf_status;
+
+/* Boundary condition per axis.  The paper's solvers use one type on all axes
+ * (PAPER.md:126); mixed types return SF_ERR_UNSUPPORTED. */
+typedef enum { SF_BC_PERIODIC = 0, SF_BC_DIRICHLET = 1, SF_BC_NEUMANN = 2, SF_BC_UNBOUNDED = 3 } sf_bc;
+
+/* Grid type (eq. 9): REGULAR = cell-boundary nodes, STAGGERED = cell centres. */
+typedef enum { SF_GRID_CELL_BOUNDARY = 0, SF_GRID_CELL_CENTRE = 1 } sf_grid;
+
+/* Operator / multiplier (PAPER.md:173 eigenvalue type; PAPER.md:189 Green's function type). */
+typedef enum {
+    SF_OP_PSEUDO_SPECTRAL = 0, /* -k^2 symbol (Table 1 "PS" column)                               */
+    SF_OP_FD2 = 1,             /* eigenvalues of the 2nd-order finite-difference stencil ("FD2")    */
+    SF_OP_GREEN_GAUSS2 = 2     /* unbounded: Gaussian-regularised kernel of order 2, */
+                               /* G(r) = -erf(r/(sqrt(2) eps))/(4 pi r), eps = eps_over_h * max(h)  */
+} sf_operator;
+
+typedef enum { SF_F32 = 0, SF_F64 = 1 } sf_precision;
+typedef enum { SF_MEM_HOST = 0, SF_MEM_DEVICE = 1 } sf_mem;
+
+/* Output selectors for sf_get_output / sf_output_device_ptr. */
+typedef enum {
+    SF_OUT_PSI = 0,  /* solution; comp = component (0 for scalar plans)                          */
+    SF_OUT_GRAD = 1, /* after sf_gradient: comp = axis (0=x,1=y,2=z) of grad psi (scalar plans)   */
+    SF_OUT_CURL = 2  /* after sf_curl:     comp = component of curl psi (ncomp == 3 plans)        */
+} sf_field;
+
+typedef struct {
+    int ncomp;         /* 1 = scalar, 3 = vector solved component-wise; 0 -> 1     */
+    void* stream;      /* cudaStream_t the plan enqueues on; NULL = legacy default stream          */
+    double rhs_sign;   /* +1: lap(psi) = f (paper eq. 2); -1: lap(psi) = -f (vorticity, eq. 17); 0 -> +1 */
+    double eps_over_h; /* Gaussian regularisation width in units of max(h); 0 -> 2.0               */
+} sf_options;
+
+/*
+ * sf_plan_create -- the paper's initialisation sequence (grid setup, FFT data setup, eigenvalue /
+ * Green's function setup, differential-operator setup).
+ *   out    [host, written]  receives the plan handle; the plan owns every table and workspace it
+ *                           allocates (all on the current CUDA device) until sf_plan_destroy.
+ *   ndim   2 or 3.
+ *   n      [host] stored unknowns per axis (n[a] for a >= ndim is ignored and treated as 1).
+ *          periodic, Neumann cell-centre, unbounded: n[a] a power of two >= 8 (x) / >= 4 (y, z);
+ *          Dirichlet cell-boundary: n[a] = 2^k - 1 interior nodes (boundary nodes are not stored).
+ *          Upper bound 4096 per axis (2048 for unbounded, whose transforms are 2 n[a] long).
+ *   h      [host] grid spacing per axis.  Domain length follows (Table 1): periodic
+ *          and cell-centre L = n h; Dirichlet cell-boundary L = (n + 1) h.
+ *   bc     [host] boundary condition per axis; all axes must agree.
+ *   grid   Dirichlet requires SF_GRID_CELL_BOUNDARY, Neumann SF_GRID_CELL_CENTRE (the other two
+ *          Table-1 rows are not built yet: SF_ERR_UNSUPPORTED); periodic and unbounded accept both
+ *          (identical numerics).
+ *   op     PS / FD2 for periodic, Dirichlet, Neumann; GREEN_GAUSS2 for unbounded (3-D only).
+ *   prec   arithmetic and storage type of every array passed later.
+ *   opt    [host] may be NULL (defaults above).
+ * For unbounded plans this call evaluates G on the doubled grid, transforms it with the library's
+ * own fp64 kernels and stores the real, even spectrum as a compact (n+1)^3 table.
+ * Errors: INVALID_ARG, UNSUPPORTED (mixed BCs, sizes above, 2-D unbounded, ncomp not 1 or 3,
+ * PS/FD2 on unbounded or GREEN on bounded plans), ALLOC, CUDA.
+ */
+sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const double h[3], const sf_bc bc[3],
+                         sf_grid grid, sf_operator op, sf_precision prec, const sf_options* opt);
+
+/*
+ * sf_set_source -- the paper's Set_Input.
+ *   src    ncomp dense fields of n[0]*n[1]*n[2] elements of the plan's precision.
+ *   where  SF_MEM_DEVICE: the pointer is BORROWED -- it must stay valid and unchanged until the
+ *          solve that consumes it has completed on the plan's stream; nothing is copied.
+ *          SF_MEM_HOST: the data are copied to a plan-owned device buffer on the plan's stream
+ *          (the host buffer may be reused after the call returns only if it is pageable; for
+ *          pinned memory after sf_synchronize or the next blocking call).
+ */
+sf_status sf_set_source(sf_plan plan, const void* src, sf_mem where);
+
+/*
+ * sf_set_bc_values -- inhomogeneous boundary values, folded into the boundary-adjacent source cells
+ * before the forward transform (FD2 operator only).
+ *   axis 0..ndim-1, side 0 = lower face, 1 = upper face.
+ *   face   values over the two remaining axes, lower axis fastest (for axis 0: iy + n[1]*iz; axis 1:
+ *          ix + n[0]*iz; axis 2: ix + n[0]*iy); NULL resets the face to homogeneous.
+ *          Dirichlet: psi on the boundary node next to the layer; weight -1/h^2.
+ *          Neumann:   d psi / d x_axis along +axis on both faces (eq. 15);
+ *                     weights +1/h (lower), -1/h (upper).
+ *   where  as for sf_set_source (device pointers borrowed, host data copied).
+ * Errors: UNSUPPORTED for periodic / unbounded plans or the PS operator.
+ */
+sf_status sf_set_bc_values(sf_plan plan, int axis, int side, const void* face, sf_mem where);
+
+/* sf_solve -- forward transform, multiply, backward transform: psi for every
+ * component.  Asynchronous.  Errors: STATE (no source), CUDA. */
+sf_status sf_solve(sf_plan plan);
+
+/* sf_gradient -- as sf_solve, and additionally d psi / d x_a = IDFT(i k_a psi_hat) for every axis
+ * from the same spectrum (eq. 10).  Scalar periodic plans only (UNSUPPORTED otherwise);
+ * the wavenumber at the Nyquist index is taken as zero. */
+sf_status sf_gradient(sf_plan plan);
+
+/* sf_curl -- ncomp == 3 plans: solve the three components and return u = curl psi = IDFT(i k x
+ * psi_hat) in the same spectral pass (eq. 17).  Wavenumbers on the
+ * transform grid (doubled for unbounded plans).  psi itself is not produced by this call. */
+sf_status sf_curl(sf_plan plan);
+
+/*
+ * sf_get_output -- the paper's Get_Output.
+ *   field, comp   see sf_field.
+ *   dst    caller-owned, n[0]*n[1]*n[2] elements; SF_MEM_HOST blocks until the copy is complete,
+ *          SF_MEM_DEVICE enqueues a device-to-device copy on the plan's stream.
+ * Errors: STATE if the requested field was not produced by the last compute call.
+ */
+sf_status sf_get_output(sf_plan plan, int field, int comp, void* dst, sf_mem where);
+
+/* Borrow the plan-owned device buffer holding a result (valid until the next compute call or
+ * sf_plan_destroy); *ptr receives a device pointer.  Same errors as sf_get_output. */
+sf_status sf_output_device_ptr(sf_plan plan, int field, int comp, void** ptr);
+
+/* Block until every operation enqueued by this plan has completed. */
+sf_status sf_synchronize(sf_plan plan);
+
+/* Number of kernels the last compute call launched (for launch accounting in benchmarks). */
+int sf_last_launch_count(sf_plan plan);
+
+/* Bytes of device memory owned by the plan (tables + workspaces + outputs). */
+long long sf_device_bytes(sf_plan plan);
+
+/*
+ * Per-step timing for profiling: when enabled, the next compute calls record CUDA events around
+ * each of the five steps (X forward, Y forward, Z fused, Y backward, X backward) on the plan's
+ * stream; sf_step_times_ms blocks and writes the five durations of the LAST compute call
+ * (milliseconds; steps that do not exist for the plan are 0).
+ */
+sf_status sf_enable_step_timing(sf_plan plan, int enable);
+sf_status sf_step_times_ms(sf_plan plan, float ms[5]);
+
+/* Message for the last error on this plan (or, with plan == NULL, of the last failed
+ * sf_plan_create on this thread).  Never NULL; owned by the library. */
+const char* sf_last_error(sf_plan plan);
+
+/* Free everything the plan owns.  Never frees caller memory.  NULL is accepted. */
+sf_status sf_plan_destroy(sf_plan plan);
+
+/* Library version string and the compute architecture it was built for ("sm_100a"). */
+const char* sf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SAILFFISH_B200_H */

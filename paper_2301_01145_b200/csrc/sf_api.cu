@@ -1,0 +1,709 @@
+// sf_api.cu -- the C ABI of include/sailffish.h: plan construction (tables, Green's spectrum,
+// workspaces) and the five-launch solve sequence S1..S5.
+// Host code plus the two small plan-time kernels (Green's function evaluation, compact-table
+// extraction).  No CPU fallback exists anywhere: every step of the path is a CUDA kernel.
+#include "../../include/sailffish.h"
+#include "sf_launch.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace sf;
+
+namespace {
+
+thread_local std::string g_create_error = "";
+
+constexpr int kMaxFields = 4;
+constexpr long double PI_L = 3.14159265358979323846264338327950288L;
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t bytes = 0;
+};
+
+} // namespace
+
+struct sf_plan_s {
+    int ndim = 3;
+    long long n[3] = { 1, 1, 1 };
+    double h[3] = { 1, 1, 1 };
+    sf_bc bc = SF_BC_PERIODIC;
+    sf_grid grid = SF_GRID_CELL_CENTRE;
+    sf_operator op = SF_OP_PSEUDO_SPECTRAL;
+    sf_precision prec = SF_F32;
+    int ncomp = 1;
+    cudaStream_t stream = nullptr;
+    double rhs_sign = 1.0, eps_over_h = 2.0;
+    size_t esize = 4;
+
+    // transform geometry
+    int xmode = X_PERIODIC, r2r = R2R_NONE;
+    int Lx = 0;          // complex length of the packed x rows
+    int Mx = 0;          // real transform length along x
+    int La[3] = { 0, 0, 0 }; // complex FFT length of the strided passes along y, z (index 1, 2)
+    int P[3] = { 1, 1, 1 };  // transform length per axis as seen by the multiplier (index folding)
+    int nspec_x = 0;     // valid spectral columns (H = Lx + 1 complex, or n0 reals)
+    long long pitch = 0; // padded column count of the work arrays
+    int nfields = 1;     // fields the workspaces can hold
+    long long w1_field = 0, w2_field = 0; // elements per field in W1 ([n2][n1][pitch]) / W2 ([n2][P1][pitch])
+    bool padded = false; // unbounded: W2 differs from W1
+
+    // device memory
+    std::vector<void*> allocs;
+    long long dev_bytes = 0;
+    void* W1 = nullptr;
+    void* W2 = nullptr;
+    void* out = nullptr;       // nfields dense real fields
+    void* tw[3] = { nullptr, nullptr, nullptr };
+    void* ptw[3] = { nullptr, nullptr, nullptr };
+    void* lam[3] = { nullptr, nullptr, nullptr };
+    void* kap[3] = { nullptr, nullptr, nullptr };
+    void* zero1 = nullptr;
+    int LT[3] = { 0, 0, 0 };
+    void* green = nullptr;
+    double scale = 1.0;
+
+    // per-solve state
+    const void* src = nullptr;
+    void* src_own = nullptr;
+    const void* face[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
+    void* face_own[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
+    int last_kind = -1; // OUT_* of the last compute call
+    int launches = 0;
+    bool timing = false;
+    cudaEvent_t ev[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
+    bool ev_valid = false;
+    std::string err = "";
+};
+
+namespace {
+
+sf_status fail(sf_plan p, sf_status st, const std::string& msg)
+{
+    if (p) p->err = msg;
+    else g_create_error = msg;
+    return st;
+}
+
+sf_status dev_alloc(sf_plan p, void** out, size_t bytes)
+{
+    void* d = nullptr;
+    cudaError_t e = cudaMalloc(&d, bytes ? bytes : 1);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(p, SF_ERR_ALLOC, std::string("cudaMalloc of ") + std::to_string(bytes) + " bytes failed: " + cudaGetErrorString(e));
+    }
+    p->allocs.push_back(d);
+    p->dev_bytes += (long long)bytes;
+    *out = d;
+    return SF_OK;
+}
+
+void dev_free(sf_plan p, void* d)
+{
+    for (size_t i = 0; i < p->allocs.size(); ++i)
+        if (p->allocs[i] == d) {
+            cudaFree(d);
+            p->allocs.erase(p->allocs.begin() + i);
+            return;
+        }
+}
+
+bool is_pow2(long long v) { return v >= 1 && (v & (v - 1)) == 0; }
+long long round_up(long long v, long long m) { return (v + m - 1) / m * m; }
+
+// exp(-2 pi i j / len), j < len, computed in extended precision and rounded once
+template <typename T> sf_status upload_twiddles(sf_plan p, void** dst, int len)
+{
+    std::vector<T> h((size_t)2 * len);
+    for (int j = 0; j < len; ++j) {
+        long double a = 2.0L * PI_L * (long double)j / (long double)len;
+        h[2 * j] = (T)cosl(a);
+        h[2 * j + 1] = (T)(-sinl(a));
+    }
+    sf_status st = dev_alloc(p, dst, h.size() * sizeof(T));
+    if (st != SF_OK) return st;
+    if (cudaMemcpy(*dst, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess)
+        return fail(p, SF_ERR_CUDA, "twiddle upload failed");
+    return SF_OK;
+}
+
+// exp(-i pi k / (2 n)), k < n  (quarter-wave shift of the DCT-II / DCT-III)
+template <typename T> sf_status upload_dct_shift(sf_plan p, void** dst, int n)
+{
+    std::vector<T> h((size_t)2 * n);
+    for (int k = 0; k < n; ++k) {
+        long double a = PI_L * (long double)k / (2.0L * (long double)n);
+        h[2 * k] = (T)cosl(a);
+        h[2 * k + 1] = (T)(-sinl(a));
+    }
+    sf_status st = dev_alloc(p, dst, h.size() * sizeof(T));
+    if (st != SF_OK) return st;
+    if (cudaMemcpy(*dst, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess)
+        return fail(p, SF_ERR_CUDA, "table upload failed");
+    return SF_OK;
+}
+
+template <typename T> sf_status upload_real(sf_plan p, void** dst, const std::vector<long double>& v)
+{
+    std::vector<T> h(v.size());
+    for (size_t i = 0; i < v.size(); ++i) h[i] = (T)v[i];
+    sf_status st = dev_alloc(p, dst, h.size() * sizeof(T));
+    if (st != SF_OK) return st;
+    if (cudaMemcpy(*dst, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess)
+        return fail(p, SF_ERR_CUDA, "table upload failed");
+    return SF_OK;
+}
+
+// Per-axis eigenvalue contribution and wavenumber (Table 1; readings A1, A4, A5,
+// A20 of DESIGN.md).  count = number of spectral indices stored along the axis.
+void axis_tables(const sf_plan_s& pl, int a, int count, std::vector<long double>& lam, std::vector<long double>& kap)
+{
+    lam.assign(count, 0.0L);
+    kap.assign(count, 0.0L);
+    const long long n = pl.n[a];
+    const long double h = pl.h[a];
+    for (int k = 0; k < count; ++k) {
+        switch (pl.bc) {
+        case SF_BC_PERIODIC: {
+            const long double Ld = (long double)n * h;
+            const long long m = (2 * k < n) ? k : k - n;
+            const long double kappa = 2.0L * PI_L * (long double)m / Ld;
+            kap[k] = (2 * k == n) ? 0.0L : kappa;
+            if (pl.op == SF_OP_PSEUDO_SPECTRAL) lam[k] = -kappa * kappa;
+            else { long double s = sinl(PI_L * (long double)k / (long double)n); lam[k] = -(4.0L / (h * h)) * s * s; }
+            break;
+        }
+        case SF_BC_DIRICHLET: {
+            const long double Ld = (long double)(n + 1) * h;
+            if (pl.op == SF_OP_PSEUDO_SPECTRAL) { long double kk = PI_L * (long double)(k + 1) / Ld; lam[k] = -kk * kk; }
+            else { long double s = sinl(PI_L * (long double)(k + 1) / (2.0L * (long double)(n + 1))); lam[k] = -(4.0L / (h * h)) * s * s; }
+            break;
+        }
+        case SF_BC_NEUMANN: {
+            const long double Ld = (long double)n * h;
+            if (pl.op == SF_OP_PSEUDO_SPECTRAL) { long double kk = PI_L * (long double)k / Ld; lam[k] = -kk * kk; }
+            else { long double s = sinl(PI_L * (long double)k / (2.0L * (long double)n)); lam[k] = -(4.0L / (h * h)) * s * s; }
+            break;
+        }
+        case SF_BC_UNBOUNDED: {
+            const long long P = 2 * n;
+            const long long m = (k < n) ? k : k - P;
+            kap[k] = (k == n) ? 0.0L : 2.0L * PI_L * (long double)m / ((long double)P * h);
+            break;
+        }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- plan-time kernels (fp64)
+// G on the doubled grid at the mirrored distance min(i, P - i) h (reading A12), times
+// the cell volume (reading A11).  Kernel: 2nd-order Gaussian regularisation (reading A10).
+__global__ void green_eval_kernel(double* g, int Px, int Py, int Pz, double hx, double hy, double hz, double eps, double vol)
+{
+    const long long tot = (long long)Px * Py * Pz;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < tot; i += (long long)gridDim.x * blockDim.x) {
+        const int ix = (int)(i % Px), iy = (int)((i / Px) % Py), iz = (int)(i / ((long long)Px * Py));
+        const double dx = (double)min(ix, Px - ix) * hx, dy = (double)min(iy, Py - iy) * hy, dz = (double)min(iz, Pz - iz) * hz;
+        const double r = sqrt(dx * dx + dy * dy + dz * dz);
+        double v;
+        if (r == 0.0) v = -1.0 / (15.749609945722419 * eps); // (2 pi)^(3/2)
+        else v = -erf(r * 0.70710678118654752440 / eps) / (12.566370614359172954 * r);
+        g[i] = vol * v;
+    }
+}
+
+// real part of the spectrum on the non-negative wavenumbers -> compact table, scaled and rounded
+template <typename T>
+__global__ void green_compact_kernel(const double2* spec, long long s_py, long long s_pz, T* tab, long long t_py, long long t_pz,
+                                     int gx, int gy, int gz, double factor)
+{
+    const long long tot = (long long)gx * gy * gz;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < tot; i += (long long)gridDim.x * blockDim.x) {
+        const int kx = (int)(i % gx), ky = (int)((i / gx) % gy), kz = (int)(i / ((long long)gx * gy));
+        tab[kx + ky * t_py + kz * t_pz] = (T)(spec[kx + ky * s_py + kz * s_pz].x * factor);
+    }
+}
+
+#define SF_CUDA(p, call)                                                                                   \
+    do {                                                                                                   \
+        cudaError_t e__ = (call);                                                                          \
+        if (e__ != cudaSuccess) {                                                                          \
+            cudaGetLastError();                                                                            \
+            return fail(p, SF_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__));             \
+        }                                                                                                  \
+    } while (0)
+
+// Green's spectrum: evaluate on the doubled grid, transform with the library's own fp64 passes
+// (periodic R2C along x, forward strided passes along y and z), keep Re on [0, n]^3.
+template <typename T> sf_status build_green(sf_plan p)
+{
+    const int Px = 2 * (int)p->n[0], Py = 2 * (int)p->n[1], Pz = 2 * (int)p->n[2];
+    const long long hp = p->pitch; // >= Px/2 + 1
+    double* g = nullptr;
+    double2* spec = nullptr;
+    void *twx = nullptr, *twy = nullptr, *twz = nullptr;
+    const size_t gbytes = (size_t)Px * Py * Pz * sizeof(double), sbytes = (size_t)hp * Py * Pz * sizeof(double2);
+    sf_status st;
+    if ((st = dev_alloc(p, (void**)&g, gbytes)) != SF_OK) return st;
+    if ((st = dev_alloc(p, (void**)&spec, sbytes)) != SF_OK) return st;
+    if ((st = upload_twiddles<double>(p, &twx, Px)) != SF_OK) return st;
+    if ((st = upload_twiddles<double>(p, &twy, Py)) != SF_OK) return st;
+    if ((st = upload_twiddles<double>(p, &twz, Pz)) != SF_OK) return st;
+    const double eps = p->eps_over_h * fmax(p->h[0], fmax(p->h[1], p->h[2]));
+    const double vol = p->h[0] * p->h[1] * p->h[2];
+    green_eval_kernel<<<148 * 8, 256, 0, p->stream>>>(g, Px, Py, Pz, p->h[0], p->h[1], p->h[2], eps, vol);
+    SF_CUDA(p, cudaGetLastError());
+
+    XParams<double> xp;
+    memset(&xp, 0, sizeof(xp));
+    xp.real_in = g; xp.spec_out = spec;
+    xp.rin_py = Px; xp.rin_pz = (long long)Px * Py; xp.rin_pc = 0;
+    xp.sp_py = hp; xp.sp_pz = hp * Py; xp.sp_pc = 0;
+    xp.n = Px; xp.ny = Py; xp.nz = Pz; xp.mode = X_PERIODIC;
+    xp.LT = Px; xp.tw = (const double2*)twx;
+    SF_CUDA(p, launch_xfwd<double>(Px / 2, xp, 1, p->stream));
+
+    SParams<double> sp;
+    memset(&sp, 0, sizeof(sp));
+    sp.in = spec; sp.out = spec;
+    sp.nx = Px / 2 + 1; sp.r2r = R2R_NONE;
+    // along y
+    sp.in_ps = sp.out_ps = hp; sp.in_bs = sp.out_bs = hp * Py;
+    sp.n_in = Py; sp.n_out = Py; sp.LT = Py; sp.tw = (const double2*)twy;
+    SF_CUDA(p, launch_spass<double>(Py, 0, sp, Pz, 1, 1, p->stream));
+    // along z
+    sp.in_ps = sp.out_ps = hp * Py; sp.in_bs = sp.out_bs = hp;
+    sp.n_in = Pz; sp.n_out = Pz; sp.LT = Pz; sp.tw = (const double2*)twz;
+    SF_CUDA(p, launch_spass<double>(Pz, 0, sp, Py, 1, 1, p->stream));
+
+    const int gx = (int)p->n[0] + 1, gy = (int)p->n[1] + 1, gz = (int)p->n[2] + 1;
+    if ((st = dev_alloc(p, &p->green, (size_t)hp * gy * gz * sizeof(T))) != SF_OK) return st;
+    SF_CUDA(p, cudaMemsetAsync(p->green, 0, (size_t)hp * gy * gz * sizeof(T), p->stream));
+    const double factor = p->rhs_sign / ((double)Px * (double)Py * (double)Pz);
+    green_compact_kernel<T><<<148 * 8, 256, 0, p->stream>>>(spec, hp, hp * Py, (T*)p->green, hp, hp * gy, gx, gy, gz, factor);
+    SF_CUDA(p, cudaGetLastError());
+    SF_CUDA(p, cudaStreamSynchronize(p->stream));
+    dev_free(p, g); dev_free(p, spec); dev_free(p, twx); dev_free(p, twy); dev_free(p, twz);
+    p->dev_bytes -= (long long)(gbytes + sbytes + (size_t)(Px + Py + Pz) * 16);
+    return SF_OK;
+}
+
+template <typename T> sf_status build_tables(sf_plan p)
+{
+    sf_status st;
+    // twiddles: x table has the real transform length; strided tables the complex length, or the
+    // real-extension length 2L for DST / DCT pencils (their split / merge steps need w_2L)
+    p->LT[0] = p->Mx;
+    if ((st = upload_twiddles<T>(p, &p->tw[0], p->LT[0])) != SF_OK) return st;
+    for (int a = 1; a < p->ndim; ++a) {
+        p->LT[a] = (p->r2r == R2R_NONE) ? p->La[a] : 2 * p->La[a];
+        if ((st = upload_twiddles<T>(p, &p->tw[a], p->LT[a])) != SF_OK) return st;
+    }
+    if (p->bc == SF_BC_NEUMANN)
+        for (int a = 0; a < p->ndim; ++a)
+            if ((st = upload_dct_shift<T>(p, &p->ptw[a], (int)p->n[a])) != SF_OK) return st;
+    std::vector<long double> z1(1, 0.0L);
+    if ((st = upload_real<T>(p, &p->zero1, z1)) != SF_OK) return st;
+    for (int a = 0; a < p->ndim; ++a) {
+        int count;
+        if (p->bc == SF_BC_UNBOUNDED) count = (a == 0) ? (int)p->n[0] + 1 : 2 * (int)p->n[a];
+        else if (p->bc == SF_BC_PERIODIC) count = (a == 0) ? (int)p->n[0] / 2 + 1 : (int)p->n[a];
+        else count = (int)p->n[a];
+        std::vector<long double> lam, kap;
+        axis_tables(*p, a, count, lam, kap);
+        if ((st = upload_real<T>(p, &p->lam[a], lam)) != SF_OK) return st;
+        if ((st = upload_real<T>(p, &p->kap[a], kap)) != SF_OK) return st;
+    }
+    if (p->bc == SF_BC_UNBOUNDED) return build_green<T>(p);
+    return SF_OK;
+}
+
+// ---------------------------------------------------------------- the solve sequence
+template <typename T> sf_status run(sf_plan p, int outk)
+{
+    typedef SF_CX C;
+    const int nd = p->ndim;
+    const int n0 = (int)p->n[0], n1 = (int)p->n[1], n2 = (nd == 3) ? (int)p->n[2] : 1;
+    const long long hp = p->pitch;
+    const int ncomp = p->ncomp;
+    const int nf_out = (outk == OUT_GRAD) ? 1 + nd : ncomp;
+    const int P1 = p->padded ? 2 * n1 : n1;
+    cudaStream_t st = p->stream;
+    p->launches = 0;
+    p->ev_valid = false;
+    auto mark = [&](int i) { if (p->timing) cudaEventRecord(p->ev[i], st); };
+
+    // S1: X forward
+    XParams<T> xp;
+    memset(&xp, 0, sizeof(xp));
+    xp.real_in = (const T*)p->src;
+    xp.rin_py = n0; xp.rin_pz = (long long)n0 * n1; xp.rin_pc = (long long)n0 * n1 * n2;
+    xp.spec_out = p->W1; xp.real_out = (T*)p->W1;
+    xp.sp_py = hp; xp.sp_pz = hp * n1; xp.sp_pc = p->w1_field;
+    xp.n = n0; xp.ny = n1; xp.nz = n2; xp.mode = p->xmode;
+    xp.LT = p->LT[0]; xp.tw = (const C*)p->tw[0]; xp.ptw = (const C*)p->ptw[0];
+    if (p->bc == SF_BC_DIRICHLET || p->bc == SF_BC_NEUMANN) {
+        for (int a = 0; a < nd; ++a)
+            for (int s = 0; s < 2; ++s) {
+                xp.face[2 * a + s] = (const T*)p->face[2 * a + s];
+                if (xp.face[2 * a + s]) xp.has_faces = 1;
+                if (p->bc == SF_BC_DIRICHLET) xp.wface[2 * a + s] = (T)(-1.0 / (p->h[a] * p->h[a]));
+                else xp.wface[2 * a + s] = (T)((s ? -1.0 : 1.0) / p->h[a]);
+            }
+    }
+    mark(0);
+    SF_CUDA(p, launch_xfwd<T>(p->Lx, xp, ncomp, st));
+    p->launches++;
+    mark(1);
+
+    SParams<T> sp;
+    memset(&sp, 0, sizeof(sp));
+    sp.nx = p->nspec_x; sp.r2r = p->r2r;
+    sp.mul = (p->bc == SF_BC_UNBOUNDED) ? MUL_GREEN : MUL_SYMBOL;
+    sp.scale = (T)p->scale;
+    sp.zero_mode = (p->bc == SF_BC_PERIODIC || p->bc == SF_BC_NEUMANN) ? 1 : 0;
+    sp.green = (const T*)p->green;
+
+    if (nd == 3) {
+        // S2: Y forward (W1 -> W2; in place when not padded)
+        sp.in = p->W1; sp.out = p->W2;
+        sp.in_ps = hp; sp.in_bs = hp * n1; sp.in_cs = p->w1_field;
+        sp.out_ps = hp; sp.out_bs = hp * P1; sp.out_cs = p->w2_field;
+        sp.n_in = n1; sp.n_out = (p->r2r == R2R_NONE) ? p->La[1] : n1;
+        sp.LT = p->LT[1]; sp.tw = (const C*)p->tw[1]; sp.ptw = (const C*)p->ptw[1];
+        SF_CUDA(p, launch_spass<T>(p->La[1], 0, sp, n2, ncomp, 1, st));
+        p->launches++;
+    }
+    mark(2);
+    {
+        // S3: forward along the last axis, multiply, backward along the last axis
+        const int ax = nd - 1;
+        const int nlast = (int)p->n[ax];
+        sp.outk = outk; sp.pencil_axis = ax;
+        sp.in = p->W2; sp.out = p->W2;
+        if (nd == 3) {
+            sp.in_ps = sp.out_ps = hp * P1; sp.in_bs = sp.out_bs = hp;
+            sp.lam_b = (const T*)p->lam[1]; sp.kap_b = (const T*)p->kap[1];
+            sp.Pb = p->P[1];
+            sp.g_pb = hp; sp.g_pp = hp * (n1 + 1);
+        } else {
+            sp.in_ps = sp.out_ps = hp; sp.in_bs = sp.out_bs = 0;
+            sp.lam_b = (const T*)p->zero1; sp.kap_b = (const T*)p->zero1;
+            sp.Pb = 1;
+        }
+        sp.in_cs = sp.out_cs = p->w2_field;
+        sp.lam_x = (const T*)p->lam[0]; sp.kap_x = (const T*)p->kap[0];
+        sp.lam_p = (const T*)p->lam[ax]; sp.kap_p = (const T*)p->kap[ax];
+        sp.Pp = p->P[ax];
+        sp.n_in = nlast; sp.n_out = nlast;
+        sp.LT = p->LT[ax]; sp.tw = (const C*)p->tw[ax]; sp.ptw = (const C*)p->ptw[ax];
+        const int nb = (nd == 3) ? P1 : 1;
+        const int nbuf = (outk == OUT_CURL) ? 3 : (outk == OUT_GRAD ? 2 : 1);
+        const int gz = (outk == OUT_SOLVE) ? ncomp : 1;
+        SF_CUDA(p, launch_spass<T>(p->La[ax], 2, sp, nb, gz, nbuf, st));
+        p->launches++;
+    }
+    mark(3);
+    if (nd == 3) {
+        // S4: Y backward (W2 -> W1)
+        sp.in = p->W2; sp.out = p->W1;
+        sp.in_ps = hp; sp.in_bs = hp * P1; sp.in_cs = p->w2_field;
+        sp.out_ps = hp; sp.out_bs = hp * n1; sp.out_cs = p->w1_field;
+        sp.n_in = (p->r2r == R2R_NONE) ? p->La[1] : n1; sp.n_out = n1;
+        sp.LT = p->LT[1]; sp.tw = (const C*)p->tw[1]; sp.ptw = (const C*)p->ptw[1];
+        SF_CUDA(p, launch_spass<T>(p->La[1], 1, sp, n2, nf_out, 1, st));
+        p->launches++;
+    }
+    mark(4);
+    // S5: X backward
+    xp.spec_in = p->W1; xp.real_out = (T*)p->out;
+    SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+    p->launches++;
+    mark(5);
+    p->ev_valid = p->timing;
+    p->last_kind = outk;
+    return SF_OK;
+}
+
+sf_status run_any(sf_plan p, int outk)
+{
+    if (!p) return SF_ERR_INVALID_ARG;
+    if (!p->src) return fail(p, SF_ERR_STATE, "no source set: call sf_set_source first");
+    return p->prec == SF_F32 ? run<float>(p, outk) : run<double>(p, outk);
+}
+
+size_t field_elems(const sf_plan_s* p) { return (size_t)p->n[0] * (size_t)p->n[1] * (size_t)(p->ndim == 3 ? p->n[2] : 1); }
+
+} // namespace
+
+// ==================================================================================== C ABI
+extern "C" {
+
+const char* sf_version(void) { return "sailffish-b200 0.1 (sm_100a)"; }
+
+const char* sf_last_error(sf_plan plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
+
+sf_status sf_plan_destroy(sf_plan plan)
+{
+    if (!plan) return SF_OK;
+    for (void* d : plan->allocs) cudaFree(d);
+    for (int i = 0; i < 6; ++i)
+        if (plan->ev[i]) cudaEventDestroy(plan->ev[i]);
+    delete plan;
+    return SF_OK;
+}
+
+sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const double h[3], const sf_bc bc[3], sf_grid grid,
+                         sf_operator op, sf_precision prec, const sf_options* opt)
+{
+    if (!out) return fail(nullptr, SF_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!n || !h || !bc) return fail(nullptr, SF_ERR_INVALID_ARG, "n, h and bc must not be NULL");
+    if (ndim != 2 && ndim != 3) return fail(nullptr, ndim == 1 ? SF_ERR_UNSUPPORTED : SF_ERR_INVALID_ARG, "ndim must be 2 or 3");
+    if (prec != SF_F32 && prec != SF_F64) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown precision");
+    if (grid != SF_GRID_CELL_BOUNDARY && grid != SF_GRID_CELL_CENTRE) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown grid type");
+    if (op != SF_OP_PSEUDO_SPECTRAL && op != SF_OP_FD2 && op != SF_OP_GREEN_GAUSS2) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown operator");
+    for (int a = 0; a < ndim; ++a) {
+        if (bc[a] < SF_BC_PERIODIC || bc[a] > SF_BC_UNBOUNDED) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown boundary condition");
+        if (n[a] <= 0) return fail(nullptr, SF_ERR_INVALID_ARG, "sizes must be positive");
+        if (!(h[a] > 0.0) || !std::isfinite(h[a])) return fail(nullptr, SF_ERR_INVALID_ARG, "spacings must be positive and finite");
+        if (bc[a] != bc[0]) return fail(nullptr, SF_ERR_UNSUPPORTED, "mixed boundary conditions per axis are not part of the method (PAPER.md:126)");
+    }
+    int ncomp = (opt && opt->ncomp) ? opt->ncomp : 1;
+    if (ncomp != 1 && ncomp != 3) return fail(nullptr, SF_ERR_UNSUPPORTED, "ncomp must be 1 or 3");
+    if (ncomp == 3 && ndim != 3) return fail(nullptr, SF_ERR_UNSUPPORTED, "vector plans are 3-D");
+    const sf_bc b = bc[0];
+    if (b == SF_BC_UNBOUNDED) {
+        if (op != SF_OP_GREEN_GAUSS2) return fail(nullptr, SF_ERR_UNSUPPORTED, "unbounded plans use a Green's function operator");
+        if (ndim != 3) return fail(nullptr, SF_ERR_UNSUPPORTED, "2-D unbounded plans are not built");
+    } else if (op == SF_OP_GREEN_GAUSS2) {
+        return fail(nullptr, SF_ERR_UNSUPPORTED, "Green's function operators need unbounded boundary conditions");
+    }
+    if (b == SF_BC_DIRICHLET && grid != SF_GRID_CELL_BOUNDARY) return fail(nullptr, SF_ERR_UNSUPPORTED, "Dirichlet on a cell-centre grid (DST-II/III) is not built");
+    if (b == SF_BC_NEUMANN && grid != SF_GRID_CELL_CENTRE) return fail(nullptr, SF_ERR_UNSUPPORTED, "Neumann on a cell-boundary grid (DCT-I) is not built");
+
+    sf_plan p = new (std::nothrow) sf_plan_s();
+    if (!p) return fail(nullptr, SF_ERR_ALLOC, "host allocation failed");
+    p->ndim = ndim;
+    for (int a = 0; a < 3; ++a) { p->n[a] = (a < ndim) ? n[a] : 1; p->h[a] = (a < ndim) ? h[a] : 1.0; }
+    p->bc = b; p->grid = grid; p->op = op; p->prec = prec; p->ncomp = ncomp;
+    p->stream = opt ? (cudaStream_t)opt->stream : nullptr;
+    p->rhs_sign = (opt && opt->rhs_sign != 0.0) ? opt->rhs_sign : 1.0;
+    p->eps_over_h = (opt && opt->eps_over_h != 0.0) ? opt->eps_over_h : 2.0;
+    p->esize = (prec == SF_F32) ? 4 : 8;
+
+    auto bail = [&](sf_status st, const std::string& msg) {
+        std::string m = msg.empty() ? p->err : msg;
+        sf_plan_destroy(p);
+        return fail(nullptr, st, m);
+    };
+
+    // transform lengths
+    double norm = 1.0;
+    for (int a = 0; a < ndim; ++a) {
+        const long long na = p->n[a];
+        long long len; // complex FFT length of the pass along this axis
+        switch (b) {
+        case SF_BC_PERIODIC:
+            if (!is_pow2(na)) return bail(SF_ERR_UNSUPPORTED, "periodic sizes must be powers of two");
+            len = (a == 0) ? na / 2 : na; p->P[a] = (int)na; norm *= (double)na; break;
+        case SF_BC_UNBOUNDED:
+            if (!is_pow2(na)) return bail(SF_ERR_UNSUPPORTED, "unbounded sizes must be powers of two");
+            len = (a == 0) ? na : 2 * na; p->P[a] = (int)(2 * na); norm *= 2.0 * (double)na; break;
+        case SF_BC_DIRICHLET:
+            if (!is_pow2(na + 1)) return bail(SF_ERR_UNSUPPORTED, "Dirichlet cell-boundary sizes must be 2^k - 1 interior nodes");
+            len = na + 1; p->P[a] = (int)na; norm *= 2.0 * (double)(na + 1); break;
+        default:
+            if (!is_pow2(na)) return bail(SF_ERR_UNSUPPORTED, "Neumann cell-centre sizes must be powers of two");
+            len = na; p->P[a] = (int)na; norm *= 2.0 * (double)na; break;
+        }
+        if (!length_built((int)len) || len > 2048) return bail(SF_ERR_UNSUPPORTED, "transform length outside the built range (complex length 4..2048 per pass)");
+        if (a == 0) p->Lx = (int)len; else p->La[a] = (int)len;
+    }
+    p->Mx = 2 * p->Lx;
+    p->scale = p->rhs_sign / norm;
+    p->padded = (b == SF_BC_UNBOUNDED);
+    switch (b) {
+    case SF_BC_PERIODIC: p->xmode = X_PERIODIC; p->r2r = R2R_NONE; break;
+    case SF_BC_UNBOUNDED: p->xmode = X_ZEROPAD; p->r2r = R2R_NONE; break;
+    case SF_BC_DIRICHLET: p->xmode = X_DST1; p->r2r = R2R_DST1; break;
+    default: p->xmode = X_DCT2; p->r2r = R2R_DCT; break;
+    }
+    p->nspec_x = (p->r2r == R2R_NONE) ? p->Lx + 1 : (int)p->n[0];
+    p->pitch = round_up(p->nspec_x, 16);
+    p->nfields = (ncomp == 3) ? 3 : ((b == SF_BC_PERIODIC) ? 1 + ndim : 1);
+    const long long n1 = p->n[1], n2 = (ndim == 3) ? p->n[2] : 1;
+    const long long P1 = p->padded ? 2 * n1 : n1;
+    p->w1_field = p->pitch * n1 * n2;
+    p->w2_field = p->pitch * P1 * n2;
+    const size_t welem = (p->r2r == R2R_NONE) ? 2 * p->esize : p->esize;
+
+    // shared-memory feasibility of the fused kernel for this plan's worst case
+    {
+        const int ax = ndim - 1;
+        const int nbuf = (ncomp == 3) ? 3 : ((b == SF_BC_PERIODIC) ? 2 : 1);
+        const size_t need = (prec == SF_F32) ? spass_smem_bytes<float>(p->La[ax], nbuf) : spass_smem_bytes<double>(p->La[ax], nbuf);
+        if (need > 227 * 1024) return bail(SF_ERR_UNSUPPORTED, "fused pass does not fit in shared memory for this size / precision / field count");
+    }
+
+    sf_status st;
+    if ((st = dev_alloc(p, &p->W1, (size_t)p->w1_field * p->nfields * welem)) != SF_OK) return bail(st, "");
+    if (p->padded) {
+        if ((st = dev_alloc(p, &p->W2, (size_t)p->w2_field * p->nfields * welem)) != SF_OK) return bail(st, "");
+    } else {
+        p->W2 = p->W1;
+    }
+    if ((st = dev_alloc(p, &p->out, field_elems(p) * p->nfields * p->esize)) != SF_OK) return bail(st, "");
+    // pitch padding columns are read by the strided passes' neighbours only through masked loads,
+    // but keep the workspaces defined
+    if (cudaMemsetAsync(p->W1, 0, (size_t)p->w1_field * p->nfields * welem, p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
+    if (p->padded && cudaMemsetAsync(p->W2, 0, (size_t)p->w2_field * p->nfields * welem, p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
+
+    st = (prec == SF_F32) ? build_tables<float>(p) : build_tables<double>(p);
+    if (st != SF_OK) return bail(st, "");
+    if (cudaStreamSynchronize(p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "plan construction failed on the device");
+    *out = p;
+    return SF_OK;
+}
+
+sf_status sf_set_source(sf_plan plan, const void* src, sf_mem where)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (!src) return fail(plan, SF_ERR_INVALID_ARG, "src is NULL");
+    if (where == SF_MEM_DEVICE) {
+        if (((uintptr_t)src & 15) != 0) return fail(plan, SF_ERR_INVALID_ARG, "device source must be 16-byte aligned");
+        plan->src = src;
+        return SF_OK;
+    }
+    if (where != SF_MEM_HOST) return fail(plan, SF_ERR_INVALID_ARG, "unknown memory space");
+    const size_t bytes = field_elems(plan) * plan->ncomp * plan->esize;
+    if (!plan->src_own) {
+        sf_status st = dev_alloc(plan, &plan->src_own, bytes);
+        if (st != SF_OK) return st;
+    }
+    SF_CUDA(plan, cudaMemcpyAsync(plan->src_own, src, bytes, cudaMemcpyHostToDevice, plan->stream));
+    plan->src = plan->src_own;
+    return SF_OK;
+}
+
+sf_status sf_set_bc_values(sf_plan plan, int axis, int side, const void* face, sf_mem where)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (axis < 0 || axis >= plan->ndim || side < 0 || side > 1) return fail(plan, SF_ERR_INVALID_ARG, "axis / side out of range");
+    if (plan->bc != SF_BC_DIRICHLET && plan->bc != SF_BC_NEUMANN)
+        return fail(plan, SF_ERR_UNSUPPORTED, "boundary values apply to Dirichlet / Neumann plans only (PAPER.md:302)");
+    if (plan->op != SF_OP_FD2) return fail(plan, SF_ERR_UNSUPPORTED, "boundary values need the FD2 operator (PAPER.md:173)");
+    const int i = 2 * axis + side;
+    if (!face) { plan->face[i] = nullptr; return SF_OK; }
+    if (where == SF_MEM_DEVICE) { plan->face[i] = face; return SF_OK; }
+    if (where != SF_MEM_HOST) return fail(plan, SF_ERR_INVALID_ARG, "unknown memory space");
+    size_t cnt = 1;
+    for (int a = 0; a < plan->ndim; ++a) if (a != axis) cnt *= (size_t)plan->n[a];
+    if (!plan->face_own[i]) {
+        sf_status st = dev_alloc(plan, &plan->face_own[i], cnt * plan->esize);
+        if (st != SF_OK) return st;
+    }
+    SF_CUDA(plan, cudaMemcpyAsync(plan->face_own[i], face, cnt * plan->esize, cudaMemcpyHostToDevice, plan->stream));
+    plan->face[i] = plan->face_own[i];
+    return SF_OK;
+}
+
+sf_status sf_solve(sf_plan plan) { return run_any(plan, OUT_SOLVE); }
+
+sf_status sf_gradient(sf_plan plan)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (plan->bc != SF_BC_PERIODIC || plan->ncomp != 1)
+        return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient is built for scalar periodic plans");
+    return run_any(plan, OUT_GRAD);
+}
+
+sf_status sf_curl(sf_plan plan)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (plan->ncomp != 3) return fail(plan, SF_ERR_UNSUPPORTED, "sf_curl needs an ncomp == 3 plan");
+    if (plan->bc != SF_BC_PERIODIC && plan->bc != SF_BC_UNBOUNDED)
+        return fail(plan, SF_ERR_UNSUPPORTED, "sf_curl is built for periodic and unbounded plans");
+    return run_any(plan, OUT_CURL);
+}
+
+sf_status sf_output_device_ptr(sf_plan plan, int field, int comp, void** ptr)
+{
+    if (!plan || !ptr) return SF_ERR_INVALID_ARG;
+    int idx = -1;
+    if (plan->last_kind < 0) return fail(plan, SF_ERR_STATE, "no result yet: call sf_solve / sf_gradient / sf_curl first");
+    if (field == SF_OUT_PSI) {
+        if (plan->last_kind == OUT_CURL) return fail(plan, SF_ERR_STATE, "sf_curl does not produce psi");
+        if (comp < 0 || comp >= plan->ncomp) return fail(plan, SF_ERR_INVALID_ARG, "component out of range");
+        idx = comp;
+    } else if (field == SF_OUT_GRAD) {
+        if (plan->last_kind != OUT_GRAD) return fail(plan, SF_ERR_STATE, "gradient was not produced by the last call");
+        if (comp < 0 || comp >= plan->ndim) return fail(plan, SF_ERR_INVALID_ARG, "axis out of range");
+        idx = 1 + comp;
+    } else if (field == SF_OUT_CURL) {
+        if (plan->last_kind != OUT_CURL) return fail(plan, SF_ERR_STATE, "curl was not produced by the last call");
+        if (comp < 0 || comp >= 3) return fail(plan, SF_ERR_INVALID_ARG, "component out of range");
+        idx = comp;
+    } else {
+        return fail(plan, SF_ERR_INVALID_ARG, "unknown field");
+    }
+    *ptr = (char*)plan->out + (size_t)idx * field_elems(plan) * plan->esize;
+    return SF_OK;
+}
+
+sf_status sf_get_output(sf_plan plan, int field, int comp, void* dst, sf_mem where)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (!dst) return fail(plan, SF_ERR_INVALID_ARG, "dst is NULL");
+    void* src = nullptr;
+    sf_status st = sf_output_device_ptr(plan, field, comp, &src);
+    if (st != SF_OK) return st;
+    const size_t bytes = field_elems(plan) * plan->esize;
+    if (where == SF_MEM_DEVICE) {
+        SF_CUDA(plan, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, plan->stream));
+    } else if (where == SF_MEM_HOST) {
+        SF_CUDA(plan, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, plan->stream));
+        SF_CUDA(plan, cudaStreamSynchronize(plan->stream));
+    } else {
+        return fail(plan, SF_ERR_INVALID_ARG, "unknown memory space");
+    }
+    return SF_OK;
+}
+
+sf_status sf_synchronize(sf_plan plan)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    SF_CUDA(plan, cudaStreamSynchronize(plan->stream));
+    return SF_OK;
+}
+
+int sf_last_launch_count(sf_plan plan) { return plan ? plan->launches : 0; }
+long long sf_device_bytes(sf_plan plan) { return plan ? plan->dev_bytes : 0; }
+
+sf_status sf_enable_step_timing(sf_plan plan, int enable)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (enable && !plan->ev[0])
+        for (int i = 0; i < 6; ++i) SF_CUDA(plan, cudaEventCreate(&plan->ev[i]));
+    plan->timing = enable != 0;
+    plan->ev_valid = false;
+    return SF_OK;
+}
+
+sf_status sf_step_times_ms(sf_plan plan, float ms[5])
+{
+    if (!plan || !ms) return SF_ERR_INVALID_ARG;
+    if (!plan->ev_valid) return fail(plan, SF_ERR_STATE, "no timed compute call: enable step timing, then solve");
+    SF_CUDA(plan, cudaEventSynchronize(plan->ev[5]));
+    for (int i = 0; i < 5; ++i) SF_CUDA(plan, cudaEventElapsedTime(&ms[i], plan->ev[i], plan->ev[i + 1]));
+    return SF_OK;
+}
+
+} // extern "C"
