@@ -50,7 +50,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 4)) as ex:
         objs = list(ex.map(_compile, UNITS))
     tmp = LIB.with_suffix(f".{os.getpid()}.tmp.so")
-    cmd = [NVCC, "-shared", "-o", str(tmp)] + ARCH + objs + ["-lcudart"]
+    cmd = [NVCC, "-shared", "--cudart", "static", "-o", str(tmp)] + ARCH + objs
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{' '.join(cmd)}\n{r.stdout}\n{r.stderr}")
