@@ -1,0 +1,453 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the spectral Poisson hot path on B200 (BASELINE.json metric: grid
+points/s per Poisson solve, 3-D unbounded fp32, and % of the HBM roofline).
+
+One "step" = one pass of the whole hot path S1..S5 (X forward, Y forward, Z forward x Green's
+spectrum x Z backward, Y backward, X backward) = one ``sf_solve`` through
+the C ABI on one batch of synthetic input.  The workload is BASELINE.json configs[3]: 3-D unbounded
+Poisson, 256^3 cell-centre grid zero-padded to 512^3 (Hockney-Eastwood), fp32, 16 seeded Gaussian
+blobs, the Green's spectrum precomputed once at plan time and reused by every solve.
+The paper times exactly this region (forward transform + convolution + backward transform, mean of
+repeated runs).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+N > 1 (under torchrun): every rank solves its own independent problem (replicas only, DESIGN.md
+"Multi-GPU"); no data-path collective; value = points of all ranks / max-over-ranks time.
+
+``--impl reference`` times the CPU oracle (oracle/, plain fp64 C) on the host cores instead; it is
+the only leg besides ``cpu_baseline`` that executes anything under oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import csv
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "grid points/s per Poisson solve"
+UNIT = "points/s"
+
+# ---------------------------------------------------------------------------------------- workloads
+# name -> (config number, n, precision, call); algorithmic bytes come from model_bytes() below
+WORKLOADS = {
+    "cfg4_unbounded_256_f32": dict(cfg=4, n=256, prec="f32", kind="unbounded", call="solve", ncomp=1),
+    "cfg4_unbounded_256_f64": dict(cfg=4, n=256, prec="f64", kind="unbounded", call="solve", ncomp=1),
+    "cfg2_periodic_256_f32": dict(cfg=2, n=256, prec="f32", kind="periodic", call="solve", ncomp=1),
+    "cfg2_periodic_256_f32_grad": dict(cfg=2, n=256, prec="f32", kind="periodic", call="gradient", ncomp=1),
+    "cfg2_periodic_256_f64_grad": dict(cfg=2, n=256, prec="f64", kind="periodic", call="gradient", ncomp=1),
+    "cfg3_dirichlet_255_f64": dict(cfg=3, n=255, prec="f64", kind="dirichlet", call="solve", ncomp=1),
+    "cfg3_neumann_256_f64": dict(cfg=3, n=256, prec="f64", kind="neumann", call="solve", ncomp=1),
+    "cfg5_vector_512_f32_curl": dict(cfg=5, n=512, prec="f32", kind="unbounded", call="curl", ncomp=3),
+    "cfg5_vector_128_f32_curl": dict(cfg=5, n=128, prec="f32", kind="unbounded", call="curl", ncomp=3),
+}
+DEFAULT_WORKLOAD = "cfg4_unbounded_256_f32"
+
+
+def model_bytes(w):
+    """Algorithmic HBM bytes per step of each of the five kernels: every pass reads its input once and
+    writes its output once, pruned (zero rows are neither read nor written), plus the compact Green's
+    table in S3."""
+    n, r = w["n"], (4 if w["prec"] == "f32" else 8)
+    c = 2 * r
+    nc = w["ncomp"]
+    if w["kind"] == "unbounded":
+        hx, p = n + 1, 2 * n
+        nout = nc
+        s1 = nc * (n * n * n * r + n * n * hx * c)
+        s2 = nc * (n * n * hx * c + n * p * hx * c)
+        s3 = nc * (n * p * hx * c) + nout * (n * p * hx * c) + (n + 1) * (n + 1) * hx * r
+        s4 = nout * (n * p * hx * c + n * n * hx * c)
+        s5 = nout * (n * n * hx * c + n * n * n * r)
+    elif w["kind"] == "periodic":
+        h = n // 2 + 1
+        nout = 4 if w["call"] == "gradient" else 1
+        spec = n * n * h * c
+        s1 = n * n * n * r + spec
+        s2 = 2 * spec
+        s3 = spec + nout * spec
+        s4 = nout * 2 * spec
+        s5 = nout * (spec + n * n * n * r)
+    else:  # real-to-real passes
+        f = n * n * n * r
+        s1 = s2 = s3 = s4 = s5 = 2 * f
+    return [s1, s2, s3, s4, s5]
+
+
+STEP_NAMES = ["S1 xfwd_kernel", "S2 spass_kernel<MODE 0>", "S3 spass_kernel<MODE 2>", "S4 spass_kernel<MODE 1>",
+              "S5 xinv_kernel"]
+
+
+def make_input(w, rank=0):
+    """Seeded synthetic source for the workload (workloads/: generators only, no method arithmetic)."""
+    import workloads as W
+
+    dt = np.float32 if w["prec"] == "f32" else np.float64
+    n = w["n"]
+    seed = W.seed_for(w["cfg"]) + 7919 * rank
+    if w["kind"] == "unbounded" and w["ncomp"] == 1:
+        g = W.gaussian_blobs(n, seed=seed)
+        return dict(f=np.ascontiguousarray(g["f"].astype(dt)), h=g["h"], faces={})
+    if w["kind"] == "unbounded":
+        g = W.vortex_ring(n, seed=seed)
+        return dict(f=np.ascontiguousarray(g["omega"].astype(dt)), h=g["h"], faces={})
+    if w["kind"] == "periodic":
+        g = W.periodic3d_spectrum(n, seed=seed)
+        return dict(f=np.ascontiguousarray(g["f"].astype(dt)), h=tuple(L / n for L in g["L"]), faces={})
+    if w["kind"] == "dirichlet":
+        g = W.dirichlet3d_manufactured(nc=n + 1, seed=seed)
+    else:
+        g = W.neumann3d_manufactured(nc=n, seed=seed)
+    return dict(f=np.ascontiguousarray(g["f"].astype(dt)), h=g["h"],
+                faces={k: np.ascontiguousarray(v.astype(dt)) for k, v in g["faces"].items()})
+
+
+# ---------------------------------------------------------------------------------------- clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+               0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, index, period=0.004):
+        super().__init__(daemon=True)
+        self.period = period
+        self.samples = []  # (t, sm_mhz, reasons bitmask)
+        self.stop_flag = False
+        self.ok = False
+        try:
+            import pynvml
+
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # no NVML: the JSON line says so
+            self.err = repr(e)
+            self.max_mhz = None
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                mhz = int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    rs = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    rs = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.samples.append((time.perf_counter(), mhz, rs))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def summary(self, t0, t1):
+        inside = [s for s in self.samples if t0 <= s[0] <= t1]
+        where = "timed region"
+        if not inside:  # region shorter than one NVML query: use the nearest samples under load
+            inside = sorted(self.samples, key=lambda s: min(abs(s[0] - t0), abs(s[0] - t1)))[:3]
+            where = "nearest samples (timed region shorter than one NVML query)"
+        if not inside:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0,
+                    "note": getattr(self, "err", "no samples")}
+        bits = 0
+        for s in inside:
+            bits |= s[2]
+        reasons = [name for bit, name in self.REASONS.items() if bits & bit]
+        return {"sm_mhz": float(np.median([s[1] for s in inside])), "sm_max_mhz": self.max_mhz, "reasons": reasons,
+                "samples": len(inside), "where": where}
+
+
+# ---------------------------------------------------------------------------------------- ncu traffic
+def ncu_traffic(workload, step_index):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary
+    (profiles/traffic.csv: workload,step,kernel,dram_read_bytes,dram_write_bytes,source); None if
+    that capture does not exist for this workload / kernel."""
+    f = ROOT / "profiles" / "traffic.csv"
+    if not f.exists():
+        return None
+    best = None
+    with open(f) as fh:
+        for row in csv.DictReader(line for line in fh if not line.startswith("#")):
+            if row["workload"] == workload and int(row["step"]) == step_index + 1:
+                best = float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+    return best
+
+
+def load_peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        try:
+            return float(json.load(open(f))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---------------------------------------------------------------------------------------- reference arm
+def oracle_solve_timer(n_sample, prec="f32"):
+    """Returns (callable running ONE oracle solve of the cfg-4 workload at n_sample^3 -> (2 n_sample)^3,
+    threads).  The Green's spectrum is precomputed outside the timed call."""
+    import oracle as O
+    import workloads as W
+
+    g = W.gaussian_blobs(n_sample)
+    f = g["f"].astype(np.float32).astype(np.float64) if prec == "f32" else g["f"]
+    ghat = O.unbounded_green(g["n"], g["h"], 2.0 * g["h"][0])
+
+    def run():
+        return O.unbounded_solve(f, g["h"], ghat)
+
+    return run, O.num_threads()
+
+
+def pick_oracle_sample(budget_s, calls):
+    """Largest of 64^3 / 128^3 / 256^3 whose `calls` solves fit in budget_s (calibrated on 64^3)."""
+    run, _ = oracle_solve_timer(64)
+    run()
+    t0 = time.perf_counter()
+    run()
+    t64 = time.perf_counter() - t0
+    n = 64
+    for cand, factor in ((128, 9.5), (256, 9.5 * 9.5)):
+        if t64 * factor * calls <= budget_s:
+            n = cand
+    return n
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    steps = args.steps if args.steps is not None else 3
+    warmup = args.warmup if args.warmup is not None else 1
+    n_s = pick_oracle_sample(150.0, steps + warmup)
+    run, threads = oracle_solve_timer(n_s)
+    for _ in range(warmup):
+        run()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        run()
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    value = n_s ** 3 / dt
+    sample = (f"cfg-4 workload at {n_s}^3 padded to {2 * n_s}^3 (fp64 oracle, full doubled domain, "
+              f"Green's spectrum precompute excluded), {steps} solves")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": DEFAULT_WORKLOAD, "grid": "256^3 cell-centre padded to 512^3", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def cpu_baseline():
+    """The oracle as it stands on the host cores: one full-size cfg-4 solve if it is predicted to take
+    under ~40 s, else the 128^3 -> 256^3 copy."""
+    n_s = pick_oracle_sample(40.0, 2)
+    run, threads = oracle_solve_timer(n_s)
+    run()  # page in
+    t0 = time.perf_counter()
+    run()
+    dt = time.perf_counter() - t0
+    return {"value": n_s ** 3 / dt, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": dt,
+            "sample": f"1 solve of the cfg-4 workload at {n_s}^3 padded to {2 * n_s}^3, fp64 oracle on the full doubled "
+                      f"domain, Green's spectrum precompute excluded"}
+
+
+# ---------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2301_01145_b200 as sf
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    steps = args.steps if args.steps is not None else 200
+    warmup = max(args.warmup if args.warmup is not None else 10, 3)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    wname = args.workload
+    w = WORKLOADS[wname]
+    n, ncomp = w["n"], w["ncomp"]
+    inp = make_input(w, rank)
+    tdt = torch.float32 if w["prec"] == "f32" else torch.float64
+    stream = torch.cuda.Stream()
+    bc = {"unbounded": sf.SF_BC_UNBOUNDED, "periodic": sf.SF_BC_PERIODIC, "dirichlet": sf.SF_BC_DIRICHLET,
+          "neumann": sf.SF_BC_NEUMANN}[w["kind"]]
+    op = {"unbounded": sf.SF_OP_GREEN_GAUSS2, "periodic": sf.SF_OP_PSEUDO_SPECTRAL, "dirichlet": sf.SF_OP_FD2,
+          "neumann": sf.SF_OP_FD2}[w["kind"]]
+    grid = sf.SF_GRID_CELL_BOUNDARY if w["kind"] == "dirichlet" else sf.SF_GRID_CELL_CENTRE
+    plan = sf.sf_plan_create([n, n, n], inp["h"], bc, grid=grid, op=op, prec=sf.SF_F32 if w["prec"] == "f32" else sf.SF_F64,
+                             ncomp=ncomp, stream=stream.cuda_stream, rhs_sign=-1.0 if w["call"] == "curl" else 1.0)
+    call = {"solve": sf.sf_solve, "gradient": sf.sf_gradient, "curl": sf.sf_curl}[w["call"]]
+    out_field = sf.SF_OUT_CURL if w["call"] == "curl" else sf.SF_OUT_PSI
+
+    # inputs resident in HBM before the timed region
+    src_host = torch.from_numpy(inp["f"]).pin_memory()
+    src_dev = src_host.to("cuda", non_blocking=False)
+    keep = []
+    for (axis, side), g in inp["faces"].items():
+        t = torch.from_numpy(g).cuda()
+        keep.append(t)
+        sf.sf_set_bc_values(plan, axis, side, t)
+    sf.sf_set_source(plan, src_dev)
+    torch.cuda.synchronize()
+
+    # ---- warm-up
+    for _ in range(warmup):
+        call(plan)
+    sf.sf_synchronize(plan)
+    launches_per_step = sf.sf_last_launch_count(plan)
+
+    # ---- timed region: K steps, CUDA events on the plan's stream (the stream the kernels run on),
+    # per-step events of the library enabled so the dominant kernel's duration is measured live
+    sf.sf_enable_step_timing(plan, min(steps, 4096))
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_start = time.perf_counter()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(steps):
+            call(plan)
+        e1.record(stream)
+    barrier()
+    t_end = time.perf_counter()
+    sampler.stop_flag = True
+    total_ms = e0.elapsed_time(e1)
+    step_ms = sf.sf_step_times_ms(plan)
+    sf.sf_enable_step_timing(plan, 0)
+    clocks = sampler.summary(t_start, t_end)
+
+    # ---- the same K steps without the library's inner events (cross-check of the event overhead)
+    barrier()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(steps):
+            call(plan)
+        e1.record(stream)
+    barrier()
+    total_ms_noev = e0.elapsed_time(e1)
+
+    # ---- end to end through the public API with HOST buffers: H2D of the source, solve, D2H of the
+    # result, every step, inside the timed region
+    nfields_out = ncomp if w["call"] != "gradient" else 1
+    dst_host = torch.empty((nfields_out, n, n, n), dtype=tdt).pin_memory()
+    e2e_steps = max(3, min(steps, 20))
+    for _ in range(2):
+        sf.sf_set_source(plan, src_host)
+        call(plan)
+        for c in range(nfields_out):
+            sf.sf_get_output(plan, out_field, c, dst_host[c])
+    barrier()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+    for _ in range(e2e_steps):
+        sf.sf_set_source(plan, src_host)
+        call(plan)
+        for c in range(nfields_out):
+            sf.sf_get_output(plan, out_field, c, dst_host[c])
+    with torch.cuda.stream(stream):
+        e1.record(stream)
+    barrier()
+    e2e_ms = e0.elapsed_time(e1) / e2e_steps
+    h2d = src_host.numel() * src_host.element_size()
+    d2h = dst_host.numel() * dst_host.element_size()
+    checksum = float(dst_host.double().abs().mean())
+    sf.sf_set_source(plan, src_dev)
+
+    # ---- max over ranks
+    tt = torch.tensor([total_ms, total_ms_noev, e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    total_ms, total_ms_noev, e2e_ms = (float(v) for v in tt.cpu())
+    dev_bytes = sf.sf_device_bytes(plan)
+    sf.sf_plan_destroy(plan)
+
+    if rank == 0:
+        ms_per_step = total_ms / steps
+        pts = float(n) ** 3 * world
+        mb = model_bytes(w)
+        peak, peak_src = load_peaks()
+        dom = int(np.argmax(step_ms))
+        ach = mb[dom] / (step_ms[dom] * 1e-3) / 1e9
+        traffic = ncu_traffic(wname, dom)
+        line = {
+            "metric": METRIC, "value": pts / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": steps,
+            "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": w["prec"], "data": "synthetic",
+            "config": {"workload": wname, "grid": f"{n}^3" + (f" padded to {2 * n}^3" if w["kind"] == "unbounded" else ""),
+                       "call": "sf_" + w["call"], "ncomp": ncomp, "parallelism": f"replicas x{world}",
+                       "l2": "no flush needed: every step streams its whole working set through HBM "
+                             f"({sum(mb) / 1e6:.0f} MB algorithmic per step, plan holds {dev_bytes / 1e6:.0f} MB) >> 126 MB L2",
+                       "timed_region": "sf_solve x K back to back, source and output resident in HBM, Green's spectrum "
+                                       "precomputed at plan time (PAPER.md:53, :344)"},
+            "clocks": clocks,
+            "e2e": {"value": pts / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "steps": e2e_steps, "result_checksum_mean_abs": checksum,
+                    "path": "sf_set_source(pinned host) -> sf_" + w["call"] + " -> sf_get_output(pinned host)"},
+            "gpu_launches": launches_per_step * steps,
+            "roofline": {"bound": "hbm", "kernel": STEP_NAMES[dom], "achieved": ach, "peak": peak, "unit": "GB/s",
+                         "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": mb[dom], "kernel_ms": step_ms[dom]},
+            "steps_ms": {STEP_NAMES[i]: step_ms[i] for i in range(5)},
+            "steps_gbs": {STEP_NAMES[i]: (mb[i] / (step_ms[i] * 1e-3) / 1e9 if step_ms[i] > 0 else None) for i in range(5)},
+            "solve_roofline": {"algorithmic_bytes_per_step": sum(mb), "achieved_gbs": sum(mb) / (ms_per_step * 1e-3) / 1e9,
+                               "frac_of_measured_peak": sum(mb) / (ms_per_step * 1e-3) / 1e9 / peak,
+                               "frac_of_8TBs_nominal": sum(mb) / (ms_per_step * 1e-3) / 1e9 / 8000.0},
+            "ms_per_step_without_step_events": total_ms_noev / steps,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline()
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

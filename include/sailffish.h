@@ -169,12 +169,14 @@ int sf_last_launch_count(sf_plan plan);
 long long sf_device_bytes(sf_plan plan);
 
 /*
- * Per-step timing for profiling: when enabled, the next compute calls record CUDA events around
- * each of the five steps (X forward, Y forward, Z fused, Y backward, X backward) on the plan's
- * stream; sf_step_times_ms blocks and writes the five durations of the LAST compute call
- * (milliseconds; steps that do not exist for the plan are 0).
+ * Per-step timing for profiling: with slots > 0, each of the following compute calls records CUDA
+ * events around its five steps (X forward, Y forward, Z fused, Y backward, X backward) on the
+ * plan's stream, into a ring of `slots` event sets (<= 4096); slots == 0 switches timing off.
+ * sf_step_times_ms blocks and writes, per step, the MEAN duration over the min(slots, calls)
+ * compute calls recorded since timing was enabled (milliseconds; steps that do not exist for the
+ * plan are ~0).  Errors: STATE if nothing was recorded.
  */
-sf_status sf_enable_step_timing(sf_plan plan, int enable);
+sf_status sf_enable_step_timing(sf_plan plan, int slots);
 sf_status sf_step_times_ms(sf_plan plan, float ms[5]);
 
 /* Message for the last error on this plan (or, with plan == NULL, of the last failed

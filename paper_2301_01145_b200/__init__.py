@@ -168,8 +168,8 @@ def sf_device_bytes(plan) -> int:
     return int(lib().sf_device_bytes(plan))
 
 
-def sf_enable_step_timing(plan, enable=True):
-    _check(plan, lib().sf_enable_step_timing(plan, 1 if enable else 0))
+def sf_enable_step_timing(plan, slots=1):
+    _check(plan, lib().sf_enable_step_timing(plan, int(slots)))
 
 
 def sf_step_times_ms(plan):

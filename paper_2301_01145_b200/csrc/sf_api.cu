@@ -76,9 +76,9 @@ struct sf_plan_s {
     void* face_own[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
     int last_kind = -1; // OUT_* of the last compute call
     int launches = 0;
-    bool timing = false;
-    cudaEvent_t ev[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
-    bool ev_valid = false;
+    int tslots = 0;               // step timing: compute calls remembered (0 = off)
+    long long tcount = 0;         // compute calls recorded since timing was enabled
+    std::vector<cudaEvent_t> ev;  // 6 events per slot
     std::string err = "";
 };
 
@@ -337,8 +337,8 @@ template <typename T> sf_status run(sf_plan p, int outk)
     const int P1 = p->padded ? 2 * n1 : n1;
     cudaStream_t st = p->stream;
     p->launches = 0;
-    p->ev_valid = false;
-    auto mark = [&](int i) { if (p->timing) cudaEventRecord(p->ev[i], st); };
+    const int slot = p->tslots ? (int)(p->tcount % p->tslots) : 0;
+    auto mark = [&](int i) { if (p->tslots) cudaEventRecord(p->ev[6 * slot + i], st); };
 
     // S1: X forward
     XParams<T> xp;
@@ -427,7 +427,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
     SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
     p->launches++;
     mark(5);
-    p->ev_valid = p->timing;
+    if (p->tslots) p->tcount++;
     p->last_kind = outk;
     return SF_OK;
 }
@@ -454,8 +454,7 @@ sf_status sf_plan_destroy(sf_plan plan)
 {
     if (!plan) return SF_OK;
     for (void* d : plan->allocs) cudaFree(d);
-    for (int i = 0; i < 6; ++i)
-        if (plan->ev[i]) cudaEventDestroy(plan->ev[i]);
+    for (cudaEvent_t e : plan->ev) cudaEventDestroy(e);
     delete plan;
     return SF_OK;
 }
@@ -687,22 +686,35 @@ sf_status sf_synchronize(sf_plan plan)
 int sf_last_launch_count(sf_plan plan) { return plan ? plan->launches : 0; }
 long long sf_device_bytes(sf_plan plan) { return plan ? plan->dev_bytes : 0; }
 
-sf_status sf_enable_step_timing(sf_plan plan, int enable)
+sf_status sf_enable_step_timing(sf_plan plan, int slots)
 {
     if (!plan) return SF_ERR_INVALID_ARG;
-    if (enable && !plan->ev[0])
-        for (int i = 0; i < 6; ++i) SF_CUDA(plan, cudaEventCreate(&plan->ev[i]));
-    plan->timing = enable != 0;
-    plan->ev_valid = false;
+    if (slots < 0 || slots > 4096) return fail(plan, SF_ERR_INVALID_ARG, "slots must be in [0, 4096]");
+    while ((int)plan->ev.size() < 6 * slots) {
+        cudaEvent_t e = nullptr;
+        SF_CUDA(plan, cudaEventCreate(&e));
+        plan->ev.push_back(e);
+    }
+    plan->tslots = slots;
+    plan->tcount = 0;
     return SF_OK;
 }
 
 sf_status sf_step_times_ms(sf_plan plan, float ms[5])
 {
     if (!plan || !ms) return SF_ERR_INVALID_ARG;
-    if (!plan->ev_valid) return fail(plan, SF_ERR_STATE, "no timed compute call: enable step timing, then solve");
-    SF_CUDA(plan, cudaEventSynchronize(plan->ev[5]));
-    for (int i = 0; i < 5; ++i) SF_CUDA(plan, cudaEventElapsedTime(&ms[i], plan->ev[i], plan->ev[i + 1]));
+    if (!plan->tslots || plan->tcount == 0) return fail(plan, SF_ERR_STATE, "no timed compute call: enable step timing, then solve");
+    const int nrec = (int)(plan->tcount < plan->tslots ? plan->tcount : plan->tslots);
+    double acc[5] = { 0, 0, 0, 0, 0 };
+    for (int s = 0; s < nrec; ++s) {
+        SF_CUDA(plan, cudaEventSynchronize(plan->ev[6 * s + 5]));
+        for (int i = 0; i < 5; ++i) {
+            float t = 0.f;
+            SF_CUDA(plan, cudaEventElapsedTime(&t, plan->ev[6 * s + i], plan->ev[6 * s + i + 1]));
+            acc[i] += t;
+        }
+    }
+    for (int i = 0; i < 5; ++i) ms[i] = (float)(acc[i] / nrec);
     return SF_OK;
 }
 

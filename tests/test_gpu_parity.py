@@ -285,7 +285,7 @@ def test_user_stream_and_step_timing():
     with Plan(f.shape, tuple(L / n for L in w["L"]), sf.SF_BC_PERIODIC, prec="f32", stream=s.cuda_stream) as p:
         p.set_source(f)
         torch.cuda.synchronize()
-        sf.sf_enable_step_timing(p.plan, True)
+        sf.sf_enable_step_timing(p.plan, 1)
         sf.sf_solve(p.plan)
         ms = sf.sf_step_times_ms(p.plan)
         assert len(ms) == 5 and all(t > 0 for t in ms)
