@@ -94,7 +94,7 @@ def make_input(w, rank=0):
 
     dt = np.float32 if w["prec"] == "f32" else np.float64
     n = w["n"]
-    seed = W.seed_for(w["cfg"]) + 7919 * rank
+    seed = rank_seed(w["cfg"], rank)
     if w["kind"] == "unbounded" and w["ncomp"] == 1:
         g = W.gaussian_blobs(n, seed=seed)
         return dict(f=np.ascontiguousarray(g["f"].astype(dt)), h=g["h"], faces={})
@@ -272,6 +272,24 @@ def cpu_baseline():
 
 
 # ---------------------------------------------------------------------------------------- our arm
+def rank_seed(cfg, rank):
+    """Every rank solves its own independent problem (replicas only): one seed per rank."""
+    import workloads as W
+
+    return W.seed_for(cfg) + 7919 * int(rank)
+
+
+def max_over_ranks(values, world, device):
+    """Multi-GPU timings are the max over ranks (the only collective of the bench; none on the data path)."""
+    import torch
+    import torch.distributed as dist
+
+    tt = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return [float(v) for v in tt.cpu()]
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -386,10 +404,7 @@ def run_ours(args):
     sf.sf_set_source(plan, src_dev)
 
     # ---- max over ranks
-    tt = torch.tensor([total_ms, total_ms_noev, e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    total_ms, total_ms_noev, e2e_ms = (float(v) for v in tt.cpu())
+    total_ms, total_ms_noev, e2e_ms = max_over_ranks([total_ms, total_ms_noev, e2e_ms], world, "cuda")
     dev_bytes = sf.sf_device_bytes(plan)
     sf.sf_plan_destroy(plan)
 
