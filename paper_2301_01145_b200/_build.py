@@ -1,7 +1,7 @@
 """Build libsailffish_b200.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-The kernel instantiations are spread over eight translation units (precision x kernel family) plus
-the API unit; they are compiled in parallel and linked into one shared library that depends on the
+The kernel instantiations are spread over eight translation units (precision x kernel family), the
+fp32 fast-path unit and the API unit; they are compiled in parallel and linked into one shared library that depends on the
 CUDA runtime only.  Run as ``python -m paper_2301_01145_b200._build`` or through
 ``__graft_entry__.build()``.
 """
@@ -22,7 +22,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-std=c++17", "-O3", "-lineinfo", "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"] + ARCH
 
-UNITS = [("sf_api", "sf_api.cu", [])]
+UNITS = [("sf_api", "sf_api.cu", []), ("sf_fast", "sf_fast.cu", [])]
 for kind in range(4):
     for tname, t in (("f32", "float"), ("f64", "double")):
         UNITS.append((f"sf_inst_k{kind}_{tname}", "sf_inst.cu", [f"-DSF_INST_KIND={kind}", f"-DSF_INST_T={t}"]))

@@ -3,6 +3,7 @@
 // Host code plus the two small plan-time kernels (Green's function evaluation, compact-table
 // extraction).  No CPU fallback exists anywhere: every step of the path is a CUDA kernel.
 #include "../../include/sailffish.h"
+#include "sf_fast_api.h"
 #include "sf_launch.cuh"
 
 #include <cmath>
@@ -68,6 +69,9 @@ struct sf_plan_s {
     int LT[3] = { 0, 0, 0 };
     void* green = nullptr;
     double scale = 1.0;
+    // kernel generation 2 (sf_fast.cuh): fp32 unbounded plans with 256-long y and z pencils
+    bool fast = false;
+    sf2::TileMap map_s2, map_s3, map_s4;
 
     // per-solve state
     const void* src = nullptr;
@@ -371,6 +375,42 @@ template <typename T> sf_status run(sf_plan p, int outk)
     sp.zero_mode = (p->bc == SF_BC_PERIODIC || p->bc == SF_BC_NEUMANN) ? 1 : 0;
     sp.green = (const T*)p->green;
 
+    if (p->fast && outk == OUT_SOLVE) {
+        // kernel generation 2: S2, S3, S4 as persistent TMA-fed register-FFT kernels
+        sf2::FastParams fp;
+        memset(&fp, 0, sizeof(fp));
+        fp.nct = p->nspec_x / sf2::kTile;
+        fp.nyq_col = (p->nspec_x % sf2::kTile) ? fp.nct * sf2::kTile : -1;
+        // S2: W1 [z][y][hp] -> W2 [z][ky][hp]
+        fp.in = (const sf2::C*)p->W1; fp.out = (sf2::C*)p->W2;
+        fp.in_ps = hp; fp.in_bs = hp * n1; fp.out_ps = hp; fp.out_bs = hp * P1; fp.nb = n2;
+        SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_FWD, fp, p->map_s2, st));
+        p->launches++;
+        mark(2);
+        // S3: W2 in place along z
+        fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W2;
+        fp.in_ps = fp.out_ps = hp * P1; fp.in_bs = fp.out_bs = hp; fp.nb = P1;
+        fp.pair_batches = 1;
+        fp.green = (const float*)p->green; fp.g_pb = hp; fp.g_pp = hp * (n1 + 1); fp.Pb = P1;
+        SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_FUSED, fp, p->map_s3, st));
+        p->launches++;
+        mark(3);
+        // S4: W2 [z][ky][hp] -> W1 [z][y][hp]
+        fp.pair_batches = 0;
+        fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W1;
+        fp.in_ps = hp; fp.in_bs = hp * P1; fp.out_ps = hp; fp.out_bs = hp * n1; fp.nb = n2;
+        SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_INV, fp, p->map_s4, st));
+        p->launches++;
+        mark(4);
+        xp.spec_in = p->W1; xp.real_out = (T*)p->out;
+        SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        p->launches++;
+        mark(5);
+        if (p->tslots) p->tcount++;
+        p->last_kind = outk;
+        return SF_OK;
+    }
+
     if (nd == 3) {
         // S2: Y forward (W1 -> W2; in place when not padded)
         sp.in = p->W1; sp.out = p->W2;
@@ -567,6 +607,32 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
 
     st = (prec == SF_F32) ? build_tables<float>(p) : build_tables<double>(p);
     if (st != SF_OK) return bail(st, "");
+
+    // kernel generation 2 covers fp32 scalar unbounded plans whose y and z pencils are 256 long
+    if (prec == SF_F32 && b == SF_BC_UNBOUNDED && ndim == 3 && ncomp == 1 && p->n[1] == 256 && p->n[2] == 256 &&
+        (p->nspec_x % sf2::kTile) <= 1 && p->nspec_x >= sf2::kTile && !getenv("SF_DISABLE_FAST")) {
+        if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fp32 fast path failed"); }
+        const unsigned long long hpB = (unsigned long long)p->pitch * 8ull, N1 = 256, N2 = 256, PP = 512;
+        const unsigned long long hpc = (unsigned long long)p->pitch;
+        cudaError_t e1, e2, e3;
+        {
+            const unsigned long long d[4] = { hpc, N1, N2, 1 }, sb[3] = { hpB, hpB * N1, hpB * N1 * N2 };
+            const unsigned bx[4] = { 16, 256, 1, 1 };
+            e1 = sf2::fast_make_map(&p->map_s2, p->W1, d, sb, bx);
+        }
+        {
+            const unsigned long long d[4] = { hpc, PP, N2, 1 }, sb[3] = { hpB, hpB * PP, hpB * PP * N2 };
+            const unsigned bx[4] = { 16, 1, 256, 1 };
+            e2 = sf2::fast_make_map(&p->map_s3, p->W2, d, sb, bx);
+        }
+        {
+            const unsigned long long d[4] = { hpc, 2, 256, N2 }, sb[3] = { hpB, 2 * hpB, hpB * PP };
+            const unsigned bx[4] = { 16, 1, 256, 1 };
+            e3 = sf2::fast_make_map(&p->map_s4, p->W2, d, sb, bx);
+        }
+        if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) return bail(SF_ERR_CUDA, "tensor map encoding failed");
+        p->fast = true;
+    }
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "plan construction failed on the device");
     *out = p;
     return SF_OK;

@@ -1,0 +1,82 @@
+// sf_fast.cu -- the one translation unit of kernel generation 2 (sf_fast.cuh): constant tables,
+// shared-memory opt-in and the persistent-grid launchers.
+#include "sf_fast.cuh"
+
+#include <cmath>
+#include <mutex>
+#include <vector>
+
+namespace sf2 {
+
+namespace {
+std::mutex g_mu;
+int g_ready_dev = -1;
+int g_sms = 0;
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+constexpr size_t kSmemPad = 3 * (size_t)kTileElems * sizeof(C); // two ring slots + the exchange buffer
+} // namespace
+
+cudaError_t fast_init()
+{
+    std::lock_guard<std::mutex> lk(g_mu);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (g_ready_dev == dev) return cudaSuccess;
+    std::vector<float2> tw(1024);
+    const long double pi = 3.14159265358979323846264338327950288L;
+    for (int j = 0; j < 1024; ++j) {
+        const long double a = 2.0L * pi * (long double)j / 1024.0L;
+        tw[j] = make_float2((float)cosl(a), (float)(-sinl(a)));
+    }
+    if ((e = cudaMemcpyToSymbol(c_tw1024, tw.data(), sizeof(float2) * 1024)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemPad)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemPad)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemPad)) != cudaSuccess) return e;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres)) != cudaSuccess) return e;
+    if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+    g_encode = (EncodeTiledFn)fn;
+    g_ready_dev = dev;
+    return cudaSuccess;
+}
+
+static_assert(sizeof(CUtensorMap) == sizeof(TileMap), "TileMap must be able to hold a CUtensorMap");
+
+cudaError_t fast_make_map(TileMap* out, const void* base, const unsigned long long dims[4],
+                          const unsigned long long strides_bytes[3], const unsigned box[4])
+{
+    if (!g_encode) return cudaErrorNotReady;
+    cuuint64_t gd[4] = { dims[0], dims[1], dims[2], dims[3] };
+    cuuint64_t gs[3] = { strides_bytes[0], strides_bytes[1], strides_bytes[2] };
+    cuuint32_t bx[4] = { box[0], box[1], box[2], box[3] };
+    cuuint32_t es[4] = { 1, 1, 1, 1 };
+    // 8-byte elements (one complex fp32 number); the data are moved, not interpreted
+    CUresult r = g_encode(reinterpret_cast<CUtensorMap*>(out), CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, const_cast<void*>(base), gd, gs, bx,
+                          es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map, cudaStream_t st)
+{
+    const CUtensorMap& tm = reinterpret_cast<const CUtensorMap&>(in_map);
+    const int ntiles = fast_ntiles(p.nb, p.nct, p.nyq_col);
+    int grid = 2 * g_sms;
+    if (grid > ntiles) grid = ntiles;
+    if (grid <= 0) return cudaErrorInvalidValue;
+    switch (mode) {
+    case FMODE_FWD: fast_pad_kernel<FMODE_FWD><<<grid, kThreads, kSmemPad, st>>>(p, tm); break;
+    case FMODE_INV: fast_pad_kernel<FMODE_INV><<<grid, kThreads, kSmemPad, st>>>(p, tm); break;
+    case FMODE_FUSED: fast_pad_kernel<FMODE_FUSED><<<grid, kThreads, kSmemPad, st>>>(p, tm); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+} // namespace sf2

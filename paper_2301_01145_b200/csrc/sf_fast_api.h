@@ -1,0 +1,45 @@
+// sf_fast_api.h -- host-visible interface of kernel generation 2 (sf_fast.cuh / sf_fast.cu):
+// parameter block and launchers of the fp32 256 -> 512 padded strided passes.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace sf2 {
+
+typedef float2 C;
+
+constexpr int kTile = 16;            // pencils per tile
+
+enum { FMODE_FWD = 0, FMODE_INV = 1, FMODE_FUSED = 2 };
+
+struct FastParams {
+    const C* in;
+    C* out;
+    long long in_ps, in_bs;     // row (pencil-axis) and batch strides of the input, complex elements
+    long long out_ps, out_bs;
+    int nb;                     // batches
+    int nct;                    // full 16-column tiles per batch
+    int nyq_col;                // column handled 16 batches at a time (the Nyquist column), -1: none
+    int pair_batches;           // fused: visit batches as 0, P/2, 1, P-1, 2, P-2, ... (mirror pairs share table rows)
+    // fused multiply: compact real Green's table [fp][fb][kx] (rhs sign and normalisation folded in)
+    const float* green;
+    long long g_pb, g_pp;
+    int Pb;                     // transform length along the batch axis (index folding k -> min(k, P-k))
+};
+
+
+__host__ __device__ inline int fast_ntiles(int nb, int nct, int nyq_col) { return nb * nct + (nyq_col >= 0 ? (nb + kTile - 1) / kTile : 0); }
+
+// opaque storage of a CUtensorMap (TMA descriptor): 128 bytes, 64-byte aligned
+struct alignas(64) TileMap { unsigned char bytes[128]; };
+
+// one-time per-process set-up: twiddle constants, shared-memory opt-in, SM count, driver entry point
+cudaError_t fast_init();
+// rank-4 tensor map over 8-byte elements: dims[0] fastest; strides_bytes[i] = stride of dims[i+1]
+// (multiples of 16); box = tile image moved by one TMA instruction (dense, no swizzle)
+cudaError_t fast_make_map(TileMap* out, const void* base, const unsigned long long dims[4],
+                          const unsigned long long strides_bytes[3], const unsigned box[4]);
+// launch one padded pass (mode = FMODE_*) as a persistent grid of two CTAs per SM; `in_map`
+// describes p.in as documented at fast_pad_kernel
+cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map, cudaStream_t st);
+
+} // namespace sf2
