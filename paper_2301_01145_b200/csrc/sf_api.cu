@@ -71,6 +71,7 @@ struct sf_plan_s {
     double scale = 1.0;
     // kernel generation 2 (sf_fast.cuh): fp32 unbounded plans with 256-long y and z pencils
     bool fast = false;
+    bool fast_x = false;   // S1 / S5 too (x extent 256)
     sf2::TileMap map_s2, map_s3, map_s4;
 
     // per-solve state
@@ -363,7 +364,16 @@ template <typename T> sf_status run(sf_plan p, int outk)
             }
     }
     mark(0);
-    SF_CUDA(p, launch_xfwd<T>(p->Lx, xp, ncomp, st));
+    const bool fast_x = p->fast_x && outk == OUT_SOLVE && !xp.has_faces;
+    sf2::FastXParams fx;
+    memset(&fx, 0, sizeof(fx));
+    if (fast_x) {
+        fx.real_in = (const float*)p->src; fx.real_out = (float*)p->out;
+        fx.spec = (sf2::C*)p->W1; fx.spec_pitch = hp; fx.nrows = n1 * n2;
+        SF_CUDA(p, sf2::launch_fast_x(false, fx, st));
+    } else {
+        SF_CUDA(p, launch_xfwd<T>(p->Lx, xp, ncomp, st));
+    }
     p->launches++;
     mark(1);
 
@@ -403,7 +413,8 @@ template <typename T> sf_status run(sf_plan p, int outk)
         p->launches++;
         mark(4);
         xp.spec_in = p->W1; xp.real_out = (T*)p->out;
-        SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        if (fast_x) SF_CUDA(p, sf2::launch_fast_x(true, fx, st));
+        else SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
         p->launches++;
         mark(5);
         if (p->tslots) p->tcount++;
@@ -625,13 +636,10 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
             const unsigned bx[4] = { 16, 1, 256, 1 };
             e2 = sf2::fast_make_map(&p->map_s3, p->W2, d, sb, bx);
         }
-        {
-            const unsigned long long d[4] = { hpc, 2, 256, N2 }, sb[3] = { hpB, 2 * hpB, hpB * PP };
-            const unsigned bx[4] = { 16, 1, 256, 1 };
-            e3 = sf2::fast_make_map(&p->map_s4, p->W2, d, sb, bx);
-        }
+        p->map_s4 = p->map_s3; e3 = cudaSuccess;   // S4 loads straight into registers: no map of its own
         if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) return bail(SF_ERR_CUDA, "tensor map encoding failed");
         p->fast = true;
+        p->fast_x = (p->n[0] == 256) && p->pitch >= 258 && !getenv("SF_DISABLE_FAST_X");
     }
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "plan construction failed on the device");
     *out = p;

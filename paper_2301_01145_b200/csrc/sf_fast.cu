@@ -16,7 +16,6 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn g_encode = nullptr;
-constexpr size_t kSmemPad = 3 * (size_t)kTileElems * sizeof(C); // two ring slots + the exchange buffer
 } // namespace
 
 cudaError_t fast_init()
@@ -34,9 +33,11 @@ cudaError_t fast_init()
     }
     if ((e = cudaMemcpyToSymbol(c_tw1024, tw.data(), sizeof(float2) * 1024)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemPad)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemPad)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemPad)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_FWD>::kSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_INV>::kSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_FUSED>::kSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_x_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_x_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres)) != cudaSuccess) return e;
@@ -71,11 +72,21 @@ cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map
     if (grid > ntiles) grid = ntiles;
     if (grid <= 0) return cudaErrorInvalidValue;
     switch (mode) {
-    case FMODE_FWD: fast_pad_kernel<FMODE_FWD><<<grid, kThreads, kSmemPad, st>>>(p, tm); break;
-    case FMODE_INV: fast_pad_kernel<FMODE_INV><<<grid, kThreads, kSmemPad, st>>>(p, tm); break;
-    case FMODE_FUSED: fast_pad_kernel<FMODE_FUSED><<<grid, kThreads, kSmemPad, st>>>(p, tm); break;
+    case FMODE_FWD: fast_pad_kernel<FMODE_FWD><<<grid, kThreads, FastCfg<FMODE_FWD>::kSmem, st>>>(p, tm); break;
+    case FMODE_INV: fast_pad_kernel<FMODE_INV><<<grid, kThreads, FastCfg<FMODE_INV>::kSmem, st>>>(p, tm); break;
+    case FMODE_FUSED: fast_pad_kernel<FMODE_FUSED><<<grid, kThreads, FastCfg<FMODE_FUSED>::kSmem, st>>>(p, tm); break;
     default: return cudaErrorInvalidValue;
     }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fast_x(bool inv, const FastXParams& p, cudaStream_t st)
+{
+    if (p.nrows <= 0 || p.nrows % kXRows) return cudaErrorInvalidValue;
+    int grid = 2 * g_sms;
+    if (grid > p.nrows / kXRows) grid = p.nrows / kXRows;
+    if (inv) fast_x_kernel<true><<<grid, kXThreads, kXSmem, st>>>(p);
+    else fast_x_kernel<false><<<grid, kXThreads, kXSmem, st>>>(p);
     return cudaGetLastError();
 }
 

@@ -6,10 +6,11 @@
 // transforms), specialised to complex pencils of length 256 that are zero-padded to 512
 // (unbounded, PAD) or transformed as they are (periodic).
 //
-// Mapping.  A CTA of 256 threads owns a tile of 16 neighbouring pencils (16 complex columns = one
-// 128-byte run per row).  Lane bits 0..3 = pencil, lane bit 4 and the warp index = o in 0..15:
-// thread (o, pencil) holds the 16 elements n = o + 16 r of its pencil in registers.  A 256-point
-// transform is
+// Mapping.  A CTA of 512 threads owns a tile of 16 neighbouring pencils (16 complex columns = one
+// 128-byte run per row).  Warp index = o in 0..15 (warp-uniform, so every twiddle factor is a
+// uniform-register operand); lane bits 0..3 = pencil; lane bit 4 = h selects which HALF of the
+// padded problem the thread works on (below).  Thread (o, pencil, h) holds the 16 elements
+// n = o + 16 r of its pencil in registers.  A 256-point transform is
 //     radix-16 DFT over r (registers)  ->  twiddle w256^(q o)  ->  ONE shared-memory exchange
 //     (q, o) -> (o, o')  ->  radix-16 DFT over o' (registers)
 // and leaves X[o + 16 k2] in thread (o, pencil): input and output distributions are the same, so
@@ -20,20 +21,24 @@
 // (one issue slot per complex add, two per complex multiply, +-i free as an operand swizzle).
 //
 // Zero padding never exists: the 512-point transform of (x, 0) is two 256-point transforms, of x
-// (even outputs) and of x w512^n (odd outputs); the truncated backward transform is the mirror,
-// x_j = IDFT256(E)_j + conj(w512^j) IDFT256(O)_j for j < 256.
+// (even outputs, h = 0) and of x w512^n (odd outputs, h = 1); the truncated backward transform is
+// the mirror, x_j = IDFT256(E)_j + conj(w512^j) IDFT256(O)_j for j < 256.  The two halves run side
+// by side in the two half-warps and meet in one warp shuffle at the end.
 //
-// Tiles arrive by cp.async.bulk (one 128-byte row per copy, completion on an mbarrier) into a
-// two-deep ring, issued one tile ahead by warp 0; results go from registers to global memory as
-// 128-byte runs.  Two CTAs share an SM so that one computes while the other waits at its barrier.
+// Tiles of the forward and fused passes arrive by TMA (cp.async.bulk.tensor, one instruction per
+// tile, completion on an mbarrier) in a shared-memory slot that is refilled for the next tile as
+// soon as the current one sits in registers; results go from registers to global memory as
+// 128-byte runs.  Persistent CTAs, two per SM (64 registers per thread): the two CTAs are
+// independent barrier domains, so one does arithmetic while the other exchanges, loads or stores.
 #pragma once
 #include "sf_fast_api.h"
 #include <cuda.h>
 #include <stdint.h>
+#include <type_traits>
 
 namespace sf2 {
 
-constexpr int kThreads = 256;
+constexpr int kThreads = 512;
 constexpr int kL = 256;              // transform length
 constexpr int kTileElems = kL * kTile;
 
@@ -113,9 +118,9 @@ template <int S, bool INV> struct dft_rec<1, S, INV> {
 template <bool INV> __device__ __forceinline__ void dft16(C (&v)[16]) { dft_rec<16, 1, INV>::run(v); }
 
 // ------------------------------------------------------------------------------------ 256-point transform
-// Exchange buffer: 16 x 16 slots of kTile complex.  Orientation A: slot (a, b) at (a*16 + b)*kTile;
-// thread o writes (q, o), reads (o, o').  Orientation B is the transpose.  `ea` / `eb` are the
-// thread's two base offsets (o*16 + pencil with stride 256, o*256 + pencil with stride 16).
+// Exchange buffer: 16 x 16 slots of 32 complex (one per lane).  Orientation A: slot (a, b) at
+// (a*16 + b)*32; thread o writes (q, o), reads (o, o').  Orientation B is the transpose.  `ea` /
+// `eb` are the thread's two base offsets (o*32 + lane with stride 512, o*512 + lane with stride 32).
 struct Xchg {
     C* base;
     int ea, eb;
@@ -128,7 +133,7 @@ template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256_a(C (&
 #pragma unroll
     for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], c_tw1024[4 * q * o]);
     C* w = x.base + (ORIENT_B ? x.eb : x.ea);
-    constexpr int ws = (ORIENT_B ? 16 : 256);
+    constexpr int ws = (ORIENT_B ? 32 : 512);
 #pragma unroll
     for (int q = 0; q < 16; ++q) w[q * ws] = v[brev4(q)];
 }
@@ -136,7 +141,7 @@ template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256_a(C (&
 template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256_b(C (&v)[16], const Xchg& x)
 {
     const C* r = x.base + (ORIENT_B ? x.ea : x.eb);
-    constexpr int rs = (ORIENT_B ? 256 : 16);
+    constexpr int rs = (ORIENT_B ? 512 : 32);
 #pragma unroll
     for (int i = 0; i < 16; ++i) v[i] = r[i * rs];
     dft16<INV>(v);
@@ -170,6 +175,24 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, in
                  "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
                  : "memory");
 }
+
+// one contiguous run global -> shared, completion counted in bytes on the mbarrier
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+// one contiguous run shared -> global (bulk async-group completion)
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// all bulk stores of this thread have finished READING shared memory
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// generic-proxy writes to shared memory become visible to the async proxy (bulk stores)
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------ tiles
 // tile -> (batch, first column) and per-pencil geometry
@@ -206,203 +229,362 @@ __device__ __forceinline__ TileGeom tile_geom(const FastParams& p, int t)
 //   FMODE_FWD   : in rows n < 256        -> out rows k < 512            (S2)
 //   FMODE_INV   : in rows k < 512        -> out rows j < 256            (S4)
 //   FMODE_FUSED : in rows n < 256 -> x Green -> out rows j < 256        (S3; in == out allowed)
-// `tm` describes `in` as a rank-4 tensor whose box is one tile image [256 rows][16 columns]:
+// `tm` describes `in` as a rank-4 tensor whose box is one tile image, rows of 16 columns:
 //   FWD   dims (column, row, batch, 1)         box {16, 256, 1, 1}   coordinates {col, 0, b, 0}
 //   FUSED dims (column, batch, row, 1)         box {16, 1, 256, 1}   coordinates {col, b, 0, 0}
-//   INV   dims (column, parity, row/2, batch)  box {16, 1, 256, 1}   coordinates {col, half, 0, b}
+// (INV reads its rows straight into registers and ignores `tm`.)
+template <int MODE> struct FastCfg {
+    // FWD / FUSED stage the next tile in one shared-memory slot by TMA while the current one is
+    // being transformed; INV (tile image twice as large) loads straight into registers.
+    static constexpr bool kTma = (MODE != FMODE_INV);
+    static constexpr int kSlotElems = kTma ? kL * kTile : 0;
+    static constexpr int kXchgElems = 16 * 16 * 32;
+    static constexpr size_t kSmem = ((size_t)kSlotElems + kXchgElems) * sizeof(C);
+};
+
 template <int MODE>
 __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams p, const __grid_constant__ CUtensorMap tm)
 {
+    typedef FastCfg<MODE> Cfg;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    C* ring0 = reinterpret_cast<C*>(smem_raw);
-    C* ring1 = ring0 + kTileElems;
-    C* xbuf = ring1 + kTileElems;
-    __shared__ __align__(8) uint64_t bars[2];
+    C* xbuf = reinterpret_cast<C*>(smem_raw);
+    C* slot = xbuf + Cfg::kXchgElems;
+    __shared__ __align__(8) uint64_t bar;
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int pen = lane & 15;
-    const int o = ((tid >> 5) << 1) | (lane >> 4);
+    const int h = lane >> 4;
+    const int o = (int)__reduce_max_sync(0xffffffffu, (unsigned)(tid >> 5));   // warp-uniform: REDUX lands in a uniform register
     Xchg xc;
     xc.base = xbuf;
-    xc.ea = o * 16 + pen;
-    xc.eb = o * 256 + pen;
+    xc.ea = o * 32 + lane;
+    xc.eb = o * 512 + lane;
 
-    if (tid == 0) {
-        mbar_init(&bars[0], 1);
-        mbar_init(&bars[1], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if (Cfg::kTma) {
+        if (tid == 0) {
+            mbar_init(&bar, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
     }
-    __syncthreads();
 
     const int ntiles = fast_ntiles(p.nb, p.nct, p.nyq_col);
     const int ips = (int)p.in_ps, ops = (int)p.out_ps;
-    uint32_t ph0 = 0, ph1 = 0;   // parity to wait for on bars[0] / bars[1]
+    const int nit = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles of this CTA
+    uint32_t parity = 0;   // phase of `bar` the next full tile completes
 
-    // A "unit" is one 256-row tile image: FWD / FUSED: one per tile; INV: two per tile (even rows, odd rows).
-    // issue the TMA load of unit (tile t, half hf) into ring[slot]: one thread, one instruction
-    auto issue = [&](int t, int hf, int slot) {
-        if (tid != 0 || t >= ntiles) return;
-        const TileGeom g = tile_geom(p, t);
-        if (!g.full) return;   // gathered synchronously by the consumer
-        uint64_t* bar = &bars[slot];
-        mbar_expect_tx(bar, kTileElems * (uint32_t)sizeof(C));
-        C* dst = slot ? ring1 : ring0;
-        if (MODE == FMODE_FWD) tma_load_4d(dst, &tm, g.col, 0, g.b, 0, bar);
-        else if (MODE == FMODE_FUSED) tma_load_4d(dst, &tm, g.col, g.b, 0, 0, bar);
-        else tma_load_4d(dst, &tm, g.col, hf, 0, g.b, bar);
+    // issue the TMA load of this CTA's iteration `i` into the slot: one thread, one instruction.
+    // Tiles that are not 16 neighbouring columns (the Nyquist column) are loaded by their consumer.
+    auto issue = [&](int i) {
+        if (!Cfg::kTma || tid != 0 || i >= nit) return;
+        const TileGeom g = tile_geom(p, (int)blockIdx.x + i * (int)gridDim.x);
+        if (!g.full) return;
+        mbar_expect_tx(&bar, Cfg::kSlotElems * (uint32_t)sizeof(C));
+        if (MODE == FMODE_FWD) tma_load_4d(slot, &tm, g.col, 0, g.b, 0, &bar);
+        else tma_load_4d(slot, &tm, g.col, g.b, 0, 0, &bar);
     };
-    // make unit (t, hf) readable in ring[slot]
-    auto acquire = [&](const TileGeom& g, int hf, int slot) {
+    // v[r] = x[o + 16 r] of this thread's pencil (FWD / FUSED), then mark the slot reusable
+    auto load_x = [&](const TileGeom& g, C (&v)[16]) {
         if (g.full) {
-            if (slot) { mbar_wait(&bars[1], ph1); ph1 ^= 1; }
-            else { mbar_wait(&bars[0], ph0); ph0 ^= 1; }
+            mbar_wait(&bar, parity);
+            parity ^= 1;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = slot[(o + 16 * r) * kTile + pen];
         } else {
-            C* dst = slot ? ring1 : ring0;
-            const int rs = (MODE == FMODE_INV) ? 2 * ips : ips;
-            for (int idx = tid; idx < kTileElems; idx += kThreads) {
-                const int pp = idx & 15, row = idx >> 4;
-                C v = make_float2(0.f, 0.f);
-                if (g.b + pp < p.nb)
-                    v = p.in[(long long)(g.b + pp) * p.in_bs + g.col + (MODE == FMODE_INV ? hf * ips : 0) + row * rs];
-                dst[idx] = v;
-            }
-            __syncthreads();
+            const C* inp = p.in + (long long)min(g.b + pen, p.nb - 1) * p.in_bs + g.col + o * ips;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = __ldg(inp + r * 16 * ips);
         }
     };
 
-    int t = blockIdx.x;
-    if (MODE == FMODE_INV) { issue(t, 0, 0); issue(t, 1, 1); }
-    else issue(t, 0, 0);
-
-    int it = 0;
-    for (; t < ntiles; t += gridDim.x, ++it) {
-        const TileGeom g = tile_geom(p, t);
-        const int tn = t + gridDim.x;
+    // one tile; ORIENT = orientation of the exchange buffer its first transform starts with
+    auto tile = [&](int i, auto orient_tag) {
+        constexpr bool OB = decltype(orient_tag)::value;
+        const TileGeom g = tile_geom(p, (int)blockIdx.x + i * (int)gridDim.x);
         // this thread's pencil: output pointer, validity
         const bool pvalid = g.full || (g.b + pen < p.nb);
         const long long ob = g.full ? ((long long)g.b * p.out_bs + g.col + pen) : ((long long)(g.b + pen) * p.out_bs + g.col);
         C* outp = p.out + ob;
-
         C v[16];
+
         if constexpr (MODE == FMODE_FWD) {
-            const int slot = it & 1;
-            issue(tn, 0, slot ^ 1);
-            acquire(g, 0, slot);
-            const C* xs = (slot ? ring1 : ring0) + o * kTile + pen;
-            // even outputs: rows 2 (o + 16 k2)
+            load_x(g, v);
+            // h = 0: x -> even outputs;  h = 1: x w512^n -> odd outputs
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = xs[r * 16 * kTile];
-            fft256_a<false, false>(v, o, xc);
+            for (int r = 0; r < 16; ++r) {
+                const C w = c_tw1024[2 * (o + 16 * r)];
+                v[r] = cmul(v[r], make_float2(h ? w.x : 1.f, h ? w.y : 0.f));
+            }
+            fft256_a<false, OB>(v, o, xc);
             __syncthreads();
-            fft256_b<false, false>(v, xc);
+            issue(i + 1);   // every thread has taken its elements out of the slot
+            fft256_b<false, OB>(v, xc);
             if (pvalid) {
-                C* q = outp + 2 * o * ops;
+                C* q = outp + (2 * o + h) * ops;   // row 2 (o + 16 k2) + h
 #pragma unroll
                 for (int k2 = 0; k2 < 16; ++k2) q[k2 * 32 * ops] = v[brev4(k2)];
-            }
-            // odd outputs: rows 2 (o + 16 k2) + 1
-#pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(xs[r * 16 * kTile], c_tw1024[2 * (o + 16 * r)]);
-            fft256_a<false, true>(v, o, xc);
-            __syncthreads();
-            fft256_b<false, true>(v, xc);
-            if (pvalid) {
-                C* q = outp + (2 * o + 1) * ops;
-#pragma unroll
-                for (int k2 = 0; k2 < 16; ++k2) q[k2 * 32 * ops] = v[brev4(k2)];
-            }
-        } else if constexpr (MODE == FMODE_INV) {
-            C e[16];
-            acquire(g, 0, 0);
-            {
-                const C* xs = ring0 + o * kTile + pen;
-#pragma unroll
-                for (int k2 = 0; k2 < 16; ++k2) v[k2] = xs[k2 * 16 * kTile];
-            }
-            fft256_a<true, false>(v, o, xc);
-            __syncthreads();
-            issue(tn, 0, 0);
-            fft256_b<true, false>(v, xc);
-#pragma unroll
-            for (int r = 0; r < 16; ++r) e[r] = v[brev4(r)];
-            acquire(g, 1, 1);
-            {
-                const C* xs = ring1 + o * kTile + pen;
-#pragma unroll
-                for (int k2 = 0; k2 < 16; ++k2) v[k2] = xs[k2 * 16 * kTile];
-            }
-            fft256_a<true, true>(v, o, xc);
-            __syncthreads();
-            issue(tn, 1, 1);
-            fft256_b<true, true>(v, xc);
-            if (pvalid) {
-                C* q = outp + o * ops;
-#pragma unroll
-                for (int r = 0; r < 16; ++r) q[r * 16 * ops] = cadd(e[r], cmulc(v[brev4(r)], c_tw1024[2 * (o + 16 * r)]));
             }
         } else {
-            // fused: forward (padded), multiply by the Green's spectrum, backward (truncated)
-            const int slot = it & 1;
-            issue(tn, 0, slot ^ 1);
-            acquire(g, 0, slot);
-            const C* xs = (slot ? ring1 : ring0) + o * kTile + pen;
-            // table pointer of this thread's pencil: row fb = min(kb, Pb - kb), column kx
-            const int kb = g.full ? g.b : min(g.b + pen, p.nb - 1);
-            const int kx = g.full ? g.col + pen : g.col;
-            const float* gp = p.green + (long long)min(kb, p.Pb - kb) * p.g_pb + kx;
-            const int gpp = (int)p.g_pp;
-            float gm[16];
-            C e[16];
-            // ---- even half of the spectrum: kp = 2 (o + 16 k2), folded to min(kp, 512 - kp)
-            {
-                const float* glo = gp + 2 * o * gpp;               // kp = 2 o + 32 k2        (k2 < 8)
-                const float* ghi = gp + (2 * kL - 2 * o) * gpp;    // 512 - kp, kp = 2 o + 32 k2 (k2 >= 8)
+            if constexpr (MODE == FMODE_FUSED) {
+                float gm[16];
+                // table row of this thread's pencil: fb = min(kb, Pb - kb), column kx; the thread's
+                // spectral indices kp = 2 (o + 16 k2) + h fold to min(kp, 512 - kp)
+                const int kb = g.full ? g.b : min(g.b + pen, p.nb - 1);
+                const int kx = g.full ? g.col + pen : g.col;
+                const float* gp = p.green + (long long)min(kb, p.Pb - kb) * p.g_pb + kx;
+                const int gpp = (int)p.g_pp;
+                const float* glo = gp + (2 * o + h) * gpp;              // kp            (k2 < 8)
+                const float* ghi = gp + (2 * kL - 2 * o - h) * gpp;     // 512 - kp      (k2 >= 8)
 #pragma unroll
                 for (int k2 = 0; k2 < 16; ++k2) gm[k2] = __ldg(k2 < 8 ? glo + k2 * 32 * gpp : ghi - k2 * 32 * gpp);
-            }
+                load_x(g, v);
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = xs[r * 16 * kTile];
-            fft256_a<false, false>(v, o, xc);
-            __syncthreads();
-            fft256_b<false, false>(v, xc);
-            {
-                C u[16];
-#pragma unroll
-                for (int k2 = 0; k2 < 16; ++k2) u[k2] = cscale(v[brev4(k2)], gm[k2]);
-                fft256_a<true, true>(u, o, xc);
-                __syncthreads();
-                fft256_b<true, true>(u, xc);
-#pragma unroll
-                for (int r = 0; r < 16; ++r) e[r] = u[brev4(r)];
-            }
-            // ---- odd half: kp = 2 (o + 16 k2) + 1
-            {
-                const float* glo = gp + (2 * o + 1) * gpp;
-                const float* ghi = gp + (2 * kL - 2 * o - 1) * gpp;
-#pragma unroll
-                for (int k2 = 0; k2 < 16; ++k2) gm[k2] = __ldg(k2 < 8 ? glo + k2 * 32 * gpp : ghi - k2 * 32 * gpp);
-            }
-#pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(xs[r * 16 * kTile], c_tw1024[2 * (o + 16 * r)]);
-            fft256_a<false, false>(v, o, xc);
-            __syncthreads();
-            fft256_b<false, false>(v, xc);
-            {
-                C u[16];
-#pragma unroll
-                for (int k2 = 0; k2 < 16; ++k2) u[k2] = cscale(v[brev4(k2)], gm[k2]);
-                fft256_a<true, true>(u, o, xc);
-                __syncthreads();
-                fft256_b<true, true>(u, xc);
-                if (pvalid) {
-                    C* q = outp + o * ops;
-#pragma unroll
-                    for (int r = 0; r < 16; ++r) q[r * 16 * ops] = cadd(e[r], cmulc(u[brev4(r)], c_tw1024[2 * (o + 16 * r)]));
+                for (int r = 0; r < 16; ++r) {
+                    const C w = c_tw1024[2 * (o + 16 * r)];
+                    v[r] = cmul(v[r], make_float2(h ? w.x : 1.f, h ? w.y : 0.f));
                 }
+                fft256_a<false, OB>(v, o, xc);
+                __syncthreads();
+                issue(i + 1);   // every thread has taken its elements out of the slot
+                fft256_b<false, OB>(v, xc);
+                C u[16];
+#pragma unroll
+                for (int k2 = 0; k2 < 16; ++k2) u[k2] = cscale(v[brev4(k2)], gm[k2]);
+#pragma unroll
+                for (int k2 = 0; k2 < 16; ++k2) v[k2] = u[k2];
+                fft256_a<true, !OB>(v, o, xc);
+                __syncthreads();
+                fft256_b<true, !OB>(v, xc);
+            } else {
+                // rows 2 k + h, k = o + 16 k2: h = 0 even spectrum E, h = 1 odd spectrum O; each half-warp
+                // reads one 128-byte run per row (16 batches of one column for the Nyquist tiles)
+                const C* inp = p.in + (g.full ? ((long long)g.b * p.in_bs + g.col + pen) : ((long long)min(g.b + pen, p.nb - 1) * p.in_bs + g.col)) +
+                               (2 * o + h) * ips;
+#pragma unroll
+                for (int k2 = 0; k2 < 16; ++k2) v[k2] = __ldg(inp + k2 * 32 * ips);
+                fft256_a<true, OB>(v, o, xc);
+                __syncthreads();
+                fft256_b<true, OB>(v, xc);
+            }
+            // x_j = e_j + conj(w512^j) o_j, j = o + 16 r: h = 0 holds e, h = 1 holds o.  The half-warps
+            // swap half of their values: h = 0 finishes r < 8, h = 1 finishes r >= 8.
+            C* q = outp + (o + 128 * h) * ops;
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                const C wl = c_tw1024[2 * (o + 16 * r)], wh = c_tw1024[2 * (o + 16 * (r + 8))];
+                const C a = v[brev4(r)], b = v[brev4(r + 8)];
+                // h = 1: t_lo = conj(w) o_r (sent), t_hi = conj(w) o_{r+8} (kept);  h = 0: e_{r+8} sent, e_r kept
+                const C tl = cmulc(a, wl), th = cmulc(b, wh);
+                const C send = h ? tl : b;
+                const C keep = h ? th : a;
+                C recv;
+                recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
+                recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+                const C x = cadd(keep, recv);
+                if (pvalid) q[r * 16 * ops] = x;
+            }
+        }
+    };
+
+    issue(0);
+    if constexpr (MODE == FMODE_FUSED) {
+        // two transforms per tile: the orientation is back where it started
+        for (int i = 0; i < nit; ++i) tile(i, std::false_type());
+    } else {
+        // one transform per tile: orientations alternate
+        for (int i = 0; i < nit; i += 2) {
+            tile(i, std::false_type());
+            if (i + 1 < nit) tile(i + 1, std::true_type());
+        }
+    }
+}
+
+// ==================================================================================== X passes
+// S1 (X forward) and S5 (X backward) for rows of 256 reals zero-padded to 512 (PAPER.md:87 real
+// transform / half spectrum; PAPER.md:181 padding).  Rows are contiguous in memory, so a tile of 16
+// rows is staged through shared memory by bulk copies (one per row) and transposed there: lanes
+// 0..3 = row, lane bit 4 = h, warp = w in 0..7.
+//   forward: the padded real row of length 512 is packed as z[n] = x[2n] + i x[2n+1], n < 256,
+//   non-zero for n < 128.  Z = DFT256(z) is two 128-point transforms, of z (even outputs, h = 0)
+//   and of z w256^n (odd outputs, h = 1); then the real-transform split
+//       X[k] = ( (Z[k] + conj Z[256-k]) - i w512^k (Z[k] - conj Z[256-k]) ) / 2,   k = 0..256
+//   is done pairwise in place in the staged rows, which leave by one bulk store per row.
+//   backward: the exact mirror (merge, two truncated inverse transforms, unpack).
+// A 128-point transform is radix-16 over r (n = w + 8 r), twiddle w128^(q w), one exchange,
+// two radix-8 over o' for q = w and q = w + 8: thread w ends with the outputs k = w + 8 j.
+constexpr int kXThreads = 256;
+constexpr int kXRows = 16;
+constexpr int kXN = 256;                 // stored reals per row
+constexpr int kXInPitch = kXN + 4;       // floats per staged real row: 1040 B = 16 (mod 128): lanes hit distinct banks
+constexpr int kXSpPitch = kXN + 2;       // complex per staged spectrum row: 2064 B = 16 (mod 128), multiple of 16
+constexpr size_t kXSmem = (size_t)kXRows * kXInPitch * sizeof(float) + (size_t)16 * 8 * 32 * sizeof(C) + (size_t)kXRows * kXSpPitch * sizeof(C);
+
+__host__ __device__ constexpr int brev3(int q) { return ((q & 1) << 2) | (q & 2) | ((q & 4) >> 2); }
+template <bool INV> __device__ __forceinline__ void dft8(C (&v)[8]) { dft_rec<8, 1, INV>::run(v); }
+
+// v[r] = a[w + 8 r] in; writes the twiddled radix-16 outputs into the exchange buffer
+template <bool INV> __device__ __forceinline__ void fft128_a(C (&v)[16], int w, C* xw)
+{
+    dft16<INV>(v);
+#pragma unroll
+    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], c_tw1024[8 * q * w]);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) xw[q * 8 * 32] = v[brev4(q)];
+}
+// after a barrier: A[w + 16 k2] at a[brev3(k2)], A[w + 8 + 16 k2] at b[brev3(k2)]
+template <bool INV> __device__ __forceinline__ void fft128_b(C (&a)[8], C (&b)[8], const C* xr)
+{
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { a[i] = xr[i * 32]; b[i] = xr[(64 + i) * 32]; }
+    dft8<INV>(a);
+    dft8<INV>(b);
+}
+
+
+template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kernel(const FastXParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* rbuf = reinterpret_cast<float*>(smem_raw);                               // [16][kXInPitch] reals
+    C* xbuf = reinterpret_cast<C*>(smem_raw + (size_t)kXRows * kXInPitch * sizeof(float));   // exchange [16 q][8 o][32 lanes]
+    C* sbuf = xbuf + 16 * 8 * 32;                                                   // [16][kXSpPitch] complex
+    __shared__ __align__(8) uint64_t bar;
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int pen = lane & 15;
+    const int h = lane >> 4;
+    const int w = (int)__reduce_max_sync(0xffffffffu, (unsigned)(tid >> 5));
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (!INV)
+        for (int idx = tid; idx < kXRows * kXSpPitch; idx += kXThreads) sbuf[idx] = make_float2(0.f, 0.f);   // pad column 257 leaves as zero
+    __syncthreads();
+
+    const int ntiles = p.nrows / kXRows;
+    const int nit = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    uint32_t parity = 0;
+    C* xw = xbuf + w * 32 + lane;          // slot (q, w)
+    const C* xr = xbuf + w * 8 * 32 + lane; // slots (w, o'), (w + 8, o')
+    C* srow = sbuf + pen * kXSpPitch;      // this thread's staged spectrum row
+
+    // bulk loads of iteration i: one row per lane of warp 0
+    auto issue = [&](int i) {
+        if (tid >= kXRows || i >= nit) return;
+        const long long row = ((long long)blockIdx.x + (long long)i * gridDim.x) * kXRows + tid;
+        if (tid == 0) mbar_expect_tx(&bar, INV ? kXRows * kXSpPitch * (uint32_t)sizeof(C) : kXRows * kXN * (uint32_t)sizeof(float));
+        __syncwarp(0xffffu);
+        if (INV) bulk_g2s(sbuf + tid * kXSpPitch, p.spec + row * p.spec_pitch, kXSpPitch * (uint32_t)sizeof(C), &bar);
+        else bulk_g2s(rbuf + tid * kXInPitch, p.real_in + row * kXN, kXN * (uint32_t)sizeof(float), &bar);
+    };
+
+    issue(0);
+    for (int i = 0; i < nit; ++i) {
+        const long long row0 = ((long long)blockIdx.x + (long long)i * gridDim.x) * kXRows;
+        C v[16];
+        if constexpr (!INV) {
+            // ---------------------------------------------------------------- S1
+            mbar_wait(&bar, parity);
+            parity ^= 1;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const C z = *reinterpret_cast<const C*>(rbuf + pen * kXInPitch + 2 * (w + 8 * r));
+                const C t = c_tw1024[4 * (w + 8 * r)];   // w256^n
+                v[r] = cmul(z, make_float2(h ? t.x : 1.f, h ? t.y : 0.f));
+            }
+            fft128_a<false>(v, w, xw);
+            if (tid < kXRows) bulk_wait_read();   // the previous tile's stores have left sbuf
+            __syncthreads();
+            issue(i + 1);                         // rbuf is in registers everywhere
+            C a[8], b[8];
+            fft128_b<false>(a, b, xr);
+            // Z[2 k' + h], k' = w + 16 k2 (a) and w + 8 + 16 k2 (b), natural order into the staged row
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) {
+                srow[2 * (w + 16 * k2) + h] = a[brev3(k2)];
+                srow[2 * (w + 8 + 16 * k2) + h] = b[brev3(k2)];
+            }
+            __syncthreads();
+            // split in place: the 16 threads of a row own the pairs (k, 256 - k), k = idx + 16 m
+            const int idx = 2 * w + h;
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const int k = idx + 16 * m;
+                if (m < 8 || idx == 0) {
+                    const C te = c_tw1024[2 * (2 * w + 16 * m)], to = c_tw1024[2 * (2 * w + 1 + 16 * m)];   // w512^k
+                    const C tw = make_float2(h ? to.x : te.x, h ? to.y : te.y);
+                    const C zk = srow[k], zm = srow[(kXN - k) & (kXN - 1)];
+                    const C e = cadd(zk, make_float2(zm.x, -zm.y));
+                    const C d = csub(zk, make_float2(zm.x, -zm.y));
+                    const C wd = cmul(d, tw);
+                    // X[k] = (e - i wd) / 2,  X[256 - k] = (conj e - i conj wd) / 2
+                    srow[k] = cscale(cadd(e, make_float2(wd.y, -wd.x)), 0.5f);
+                    srow[kXN - k] = cscale(make_float2(e.x - wd.y, -e.y - wd.x), 0.5f);
+                }
+            }
+            fence_async_smem();
+            __syncthreads();
+            if (tid < kXRows) {
+                bulk_s2g(p.spec + (row0 + tid) * p.spec_pitch, sbuf + tid * kXSpPitch, kXSpPitch * (uint32_t)sizeof(C));
+                bulk_commit();
+            }
+        } else {
+            // ---------------------------------------------------------------- S5
+            mbar_wait(&bar, parity);
+            parity ^= 1;
+            // merge in place: Z[k] = e + i conj(w512^k) d, Z[256 - k] = conj e + i conj(conj(w512^k) d)
+            const int idx = 2 * w + h;
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const int k = idx + 16 * m;
+                if (m < 8 || idx == 0) {
+                    const C te = c_tw1024[2 * (2 * w + 16 * m)], to = c_tw1024[2 * (2 * w + 1 + 16 * m)];
+                    const C tw = make_float2(h ? to.x : te.x, h ? to.y : te.y);
+                    const C xk = srow[k], xm = srow[kXN - k];
+                    const C e = cadd(xk, make_float2(xm.x, -xm.y));
+                    const C d = csub(xk, make_float2(xm.x, -xm.y));
+                    const C wd = cmulc(d, tw);
+                    srow[k] = cadd(e, make_float2(-wd.y, wd.x));
+                    if (k > 0) srow[kXN - k] = make_float2(e.x + wd.y, wd.x - e.y);
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = srow[2 * (w + 8 * j) + h];   // Z[2 k' + h], k' = w + 8 j
+            fft128_a<true>(v, w, xw);
+            if (tid < kXRows) bulk_wait_read();   // the previous tile's stores have left rbuf
+            fence_async_smem();                   // the merged values in sbuf are overwritten by the next bulk load
+            __syncthreads();
+            issue(i + 1);                         // sbuf is in registers everywhere
+            C a[8], b[8];
+            fft128_b<true>(a, b, xr);
+            // z[n] = z0[n] + conj(w256^n) z1[n], n = w + 16 k2 (a) / w + 8 + 16 k2 (b): h = 0 holds z0,
+            // h = 1 holds z1; h = 0 finishes the a set, h = 1 the b set
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) {
+                const C wa = c_tw1024[4 * (w + 16 * k2)], wb = c_tw1024[4 * (w + 8 + 16 * k2)];
+                const C va = a[brev3(k2)], vb = b[brev3(k2)];
+                const C ta = cmulc(va, wa), tb = cmulc(vb, wb);
+                const C send = h ? ta : vb;
+                const C keep = h ? tb : va;
+                C recv;
+                recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
+                recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+                const C z = cadd(keep, recv);
+                const int n = w + 8 * h + 16 * k2;
+                *reinterpret_cast<C*>(rbuf + pen * kXInPitch + 2 * n) = z;   // (x[2n], x[2n+1])
+            }
+            fence_async_smem();
+            __syncthreads();
+            if (tid < kXRows) {
+                bulk_s2g(p.real_out + (row0 + tid) * kXN, rbuf + tid * kXInPitch, kXN * (uint32_t)sizeof(float));
+                bulk_commit();
             }
         }
     }
+    if (tid < kXRows) bulk_wait_read();
 }
 
 } // namespace sf2

@@ -29,6 +29,15 @@ struct FastParams {
 
 __host__ __device__ inline int fast_ntiles(int nb, int nct, int nyq_col) { return nb * nct + (nyq_col >= 0 ? (nb + kTile - 1) / kTile : 0); }
 
+// S1 / S5 for rows of 256 reals padded to 512 (fast_x_kernel)
+struct FastXParams {
+    const float* real_in;   // S1: [rows][256]
+    float* real_out;        // S5: [rows][256]
+    C* spec;                // half spectra, row pitch spec_pitch complex (>= 258, rows 16-byte aligned)
+    long long spec_pitch;
+    int nrows;              // multiple of 16
+};
+
 // opaque storage of a CUtensorMap (TMA descriptor): 128 bytes, 64-byte aligned
 struct alignas(64) TileMap { unsigned char bytes[128]; };
 
@@ -41,5 +50,8 @@ cudaError_t fast_make_map(TileMap* out, const void* base, const unsigned long lo
 // launch one padded pass (mode = FMODE_*) as a persistent grid of two CTAs per SM; `in_map`
 // describes p.in as documented at fast_pad_kernel
 cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map, cudaStream_t st);
+
+// launch S1 (inv = false) or S5 (inv = true) as a persistent grid of two CTAs per SM
+cudaError_t launch_fast_x(bool inv, const FastXParams& p, cudaStream_t st);
 
 } // namespace sf2

@@ -24,10 +24,10 @@ def _check(name, got, ref, prec):
     assert np.isfinite(e) and e <= TOL[prec], f"{name}: rel-L2 {e:.3e} > {TOL[prec]:.0e}"
 
 
-@pytest.mark.parametrize("nx", [16, 32, 64])
+@pytest.mark.parametrize("nx", [16, 32, 64, 256])
 def test_fast_path_white_noise_narrow_x(nx):
     """z = y = 256 selects the fast S2/S3/S4 kernels; x extent nx gives nx/16 full column tiles plus
-    the Nyquist column."""
+    the Nyquist column; nx = 256 also selects the fast S1 / S5 kernels."""
     shape = (256, 256, nx)
     f = rounded(W.Rng(4000 + nx).normal(int(np.prod(shape))).reshape(shape), "f32")
     h = (1.0 / 256, 1.0 / 256, 1.0 / 256)
