@@ -68,6 +68,7 @@ struct sf_plan_s {
     void* zero1 = nullptr;
     int LT[3] = { 0, 0, 0 };
     void* green = nullptr;
+    void* green_tiles = nullptr;   // fast path: the same table, tile-major (sf_fast_api.h)
     double scale = 1.0;
     // kernel generation 2 (sf_fast.cuh): fp32 unbounded plans with 256-long y and z pencils
     bool fast = false;
@@ -401,7 +402,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W2;
         fp.in_ps = fp.out_ps = hp * P1; fp.in_bs = fp.out_bs = hp; fp.nb = P1;
         fp.pair_batches = 1;
-        fp.green = (const float*)p->green; fp.g_pb = hp; fp.g_pp = hp * (n1 + 1); fp.Pb = P1;
+        fp.green_tiles = (const float*)p->green_tiles; fp.Pb = P1;
         SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_FUSED, fp, p->map_s3, st));
         p->launches++;
         mark(3);
@@ -638,6 +639,14 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         }
         p->map_s4 = p->map_s3; e3 = cudaSuccess;   // S4 loads straight into registers: no map of its own
         if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) return bail(SF_ERR_CUDA, "tensor map encoding failed");
+        {
+            const int nct = p->nspec_x / sf2::kTile, nyq = (p->nspec_x % sf2::kTile) ? nct * sf2::kTile : -1;
+            const size_t ne = sf2::fast_green_tiles_elems(512, nct, nyq);
+            if ((st = dev_alloc(p, &p->green_tiles, ne * sizeof(float))) != SF_OK) return bail(st, "");
+            if (sf2::fast_green_tiles((float*)p->green_tiles, (const float*)p->green, p->pitch, p->pitch * (p->n[1] + 1), 512, nct, nyq,
+                                      p->stream) != cudaSuccess)
+                return bail(SF_ERR_CUDA, "building the tile-major Green's table failed");
+        }
         p->fast = true;
         p->fast_x = (p->n[0] == 256) && p->pitch >= 258 && !getenv("SF_DISABLE_FAST_X");
     }

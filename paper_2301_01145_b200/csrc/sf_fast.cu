@@ -64,6 +64,37 @@ cudaError_t fast_make_map(TileMap* out, const void* base, const unsigned long lo
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
+namespace {
+__global__ void green_tiles_kernel(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
+                                   long long total)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int pen = (int)(i % kTile);
+        const int fp = (int)((i / kTile) % kGreenRows);
+        const long long t = i / ((long long)kTile * kGreenRows);
+        const long long nfull = (long long)(Pb / 2 + 1) * nct;
+        int fb, kx;
+        if (t < nfull) {
+            fb = (int)(t / nct);
+            kx = (int)(t % nct) * kTile + pen;
+        } else {
+            const int kb = min((int)(t - nfull) * kTile + pen, Pb - 1);
+            fb = min(kb, Pb - kb);
+            kx = nyq_col;
+        }
+        tiles[i] = green[kx + fb * g_pb + fp * g_pp];
+    }
+}
+} // namespace
+
+cudaError_t fast_green_tiles(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
+                             cudaStream_t st)
+{
+    const long long total = (long long)fast_green_tiles_elems(Pb, nct, nyq_col);
+    green_tiles_kernel<<<148 * 8, 256, 0, st>>>(tiles, green, g_pb, g_pp, Pb, nct, nyq_col, total);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map, cudaStream_t st)
 {
     const CUtensorMap& tm = reinterpret_cast<const CUtensorMap&>(in_map);

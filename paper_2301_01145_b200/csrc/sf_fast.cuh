@@ -127,11 +127,13 @@ struct Xchg {
 };
 
 // first half: radix-16 over r, twiddle, write.  v[r] = x[o + 16 r] in; nothing valid out.
-template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256_a(C (&v)[16], int o, const Xchg& x)
+// Twiddles come from a per-warp row of a shared-memory table: base register + immediate, no
+// address arithmetic, and a latency the other warps cover.
+template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256_a(C (&v)[16], const C* tw256, const Xchg& x)
 {
     dft16<INV>(v);
 #pragma unroll
-    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], c_tw1024[4 * q * o]);
+    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], tw256[q]);   // w256^(q o), row o of the table
     C* w = x.base + (ORIENT_B ? x.eb : x.ea);
     constexpr int ws = (ORIENT_B ? 32 : 512);
 #pragma unroll
@@ -208,6 +210,13 @@ __device__ __forceinline__ int batch_order(const FastParams& p, int bi)
     const int j = bi >> 1;
     return (bi & 1) ? p.nb - j : j;
 }
+// chunk of the tile-major Green's table that belongs to a tile: full tiles (fb, column tile) first,
+// then the Nyquist-column tiles (16 batches each)
+__device__ __forceinline__ int green_tile_index(const FastParams& p, const TileGeom& g)
+{
+    if (g.full) return min(g.b, p.Pb - g.b) * p.nct + g.col / kTile;
+    return (p.Pb / 2 + 1) * p.nct + g.b / kTile;
+}
 __device__ __forceinline__ TileGeom tile_geom(const FastParams& p, int t)
 {
     TileGeom g;
@@ -261,6 +270,19 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
     xc.ea = o * 32 + lane;
     xc.eb = o * 512 + lane;
 
+    // twiddle tables: s_tw256[o][q] = w256^(q o);  s_tw512[h][o][r] = w512^(o + 16 r) for h = 1, 1 for h = 0
+    __shared__ __align__(16) C s_tw256[16][16];
+    __shared__ __align__(16) C s_tw512[2][16][16];
+    for (int idx = tid; idx < 256; idx += kThreads) {
+        const int a = idx >> 4, b = idx & 15;
+        s_tw256[a][b] = c_tw1024[4 * a * b];
+        s_tw512[0][a][b] = make_float2(1.f, 0.f);
+        s_tw512[1][a][b] = c_tw1024[2 * (a + 16 * b)];
+    }
+    const C* t256 = &s_tw256[o][0];
+    const C* t512 = &s_tw512[h][o][0];
+    if (!Cfg::kTma) __syncthreads();
+
     if (Cfg::kTma) {
         if (tid == 0) {
             mbar_init(&bar, 1);
@@ -312,11 +334,8 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
             load_x(g, v);
             // h = 0: x -> even outputs;  h = 1: x w512^n -> odd outputs
 #pragma unroll
-            for (int r = 0; r < 16; ++r) {
-                const C w = c_tw1024[2 * (o + 16 * r)];
-                v[r] = cmul(v[r], make_float2(h ? w.x : 1.f, h ? w.y : 0.f));
-            }
-            fft256_a<false, OB>(v, o, xc);
+            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], t512[r]);
+            fft256_a<false, OB>(v, t256, xc);
             __syncthreads();
             issue(i + 1);   // every thread has taken its elements out of the slot
             fft256_b<false, OB>(v, xc);
@@ -328,23 +347,17 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
         } else {
             if constexpr (MODE == FMODE_FUSED) {
                 float gm[16];
-                // table row of this thread's pencil: fb = min(kb, Pb - kb), column kx; the thread's
-                // spectral indices kp = 2 (o + 16 k2) + h fold to min(kp, 512 - kp)
-                const int kb = g.full ? g.b : min(g.b + pen, p.nb - 1);
-                const int kx = g.full ? g.col + pen : g.col;
-                const float* gp = p.green + (long long)min(kb, p.Pb - kb) * p.g_pb + kx;
-                const int gpp = (int)p.g_pp;
-                const float* glo = gp + (2 * o + h) * gpp;              // kp            (k2 < 8)
-                const float* ghi = gp + (2 * kL - 2 * o - h) * gpp;     // 512 - kp      (k2 >= 8)
+                // the tile's chunk of the tile-major table [257 fp][16 pencils]; the thread's spectral
+                // indices kp = 2 (o + 16 k2) + h fold to fp = min(kp, 512 - kp): every offset is an immediate
+                const float* gt = p.green_tiles + (long long)green_tile_index(p, g) * (kGreenRows * kTile) + pen;
+                const float* glo = gt + (2 * o + h) * kTile;              // kp            (k2 < 8)
+                const float* ghi = gt + (2 * kL - 2 * o - h) * kTile;     // 512 - kp      (k2 >= 8)
 #pragma unroll
-                for (int k2 = 0; k2 < 16; ++k2) gm[k2] = __ldg(k2 < 8 ? glo + k2 * 32 * gpp : ghi - k2 * 32 * gpp);
+                for (int k2 = 0; k2 < 16; ++k2) gm[k2] = __ldg(k2 < 8 ? glo + k2 * 32 * kTile : ghi - k2 * 32 * kTile);
                 load_x(g, v);
 #pragma unroll
-                for (int r = 0; r < 16; ++r) {
-                    const C w = c_tw1024[2 * (o + 16 * r)];
-                    v[r] = cmul(v[r], make_float2(h ? w.x : 1.f, h ? w.y : 0.f));
-                }
-                fft256_a<false, OB>(v, o, xc);
+                for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], t512[r]);
+                fft256_a<false, OB>(v, t256, xc);
                 __syncthreads();
                 issue(i + 1);   // every thread has taken its elements out of the slot
                 fft256_b<false, OB>(v, xc);
@@ -353,7 +366,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                 for (int k2 = 0; k2 < 16; ++k2) u[k2] = cscale(v[brev4(k2)], gm[k2]);
 #pragma unroll
                 for (int k2 = 0; k2 < 16; ++k2) v[k2] = u[k2];
-                fft256_a<true, !OB>(v, o, xc);
+                fft256_a<true, !OB>(v, t256, xc);
                 __syncthreads();
                 fft256_b<true, !OB>(v, xc);
             } else {
@@ -363,7 +376,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                                (2 * o + h) * ips;
 #pragma unroll
                 for (int k2 = 0; k2 < 16; ++k2) v[k2] = __ldg(inp + k2 * 32 * ips);
-                fft256_a<true, OB>(v, o, xc);
+                fft256_a<true, OB>(v, t256, xc);
                 __syncthreads();
                 fft256_b<true, OB>(v, xc);
             }
@@ -372,12 +385,11 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
             C* q = outp + (o + 128 * h) * ops;
 #pragma unroll
             for (int r = 0; r < 8; ++r) {
-                const C wl = c_tw1024[2 * (o + 16 * r)], wh = c_tw1024[2 * (o + 16 * (r + 8))];
-                const C a = v[brev4(r)], b = v[brev4(r + 8)];
                 // h = 1: t_lo = conj(w) o_r (sent), t_hi = conj(w) o_{r+8} (kept);  h = 0: e_{r+8} sent, e_r kept
-                const C tl = cmulc(a, wl), th = cmulc(b, wh);
-                const C send = h ? tl : b;
-                const C keep = h ? th : a;
+                // (the table row of h = 0 is all ones)
+                const C tl = cmulc(v[brev4(r)], t512[r]), th = cmulc(v[brev4(r + 8)], t512[r + 8]);
+                const C send = h ? tl : th;
+                const C keep = h ? th : tl;
                 C recv;
                 recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
                 recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
@@ -424,11 +436,11 @@ __host__ __device__ constexpr int brev3(int q) { return ((q & 1) << 2) | (q & 2)
 template <bool INV> __device__ __forceinline__ void dft8(C (&v)[8]) { dft_rec<8, 1, INV>::run(v); }
 
 // v[r] = a[w + 8 r] in; writes the twiddled radix-16 outputs into the exchange buffer
-template <bool INV> __device__ __forceinline__ void fft128_a(C (&v)[16], int w, C* xw)
+template <bool INV> __device__ __forceinline__ void fft128_a(C (&v)[16], const C* tw128, C* xw)
 {
     dft16<INV>(v);
 #pragma unroll
-    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], c_tw1024[8 * q * w]);
+    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], tw128[q]);   // w128^(q w), row w of the table
 #pragma unroll
     for (int q = 0; q < 16; ++q) xw[q * 8 * 32] = v[brev4(q)];
 }
@@ -461,6 +473,25 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
     }
     if (!INV)
         for (int idx = tid; idx < kXRows * kXSpPitch; idx += kXThreads) sbuf[idx] = make_float2(0.f, 0.f);   // pad column 257 leaves as zero
+    // twiddle tables (base register + immediate addressing, no selects):
+    //   s_tw128[w][q] = w128^(q w);  s_twin[h][w][j] = w256^(w + 8 j) for h = 1, 1 for h = 0;
+    //   s_twsp[h][w][m] = w512^(2 w + h + 16 m)
+    __shared__ __align__(16) C s_tw128[8][16];
+    __shared__ __align__(16) C s_twin[2][8][16];
+    __shared__ __align__(16) C s_twsp[2][8][10];
+    for (int idx = tid; idx < 128; idx += kXThreads) {
+        const int a = idx >> 4, b = idx & 15;
+        s_tw128[a][b] = c_tw1024[8 * a * b];
+        s_twin[0][a][b] = make_float2(1.f, 0.f);
+        s_twin[1][a][b] = c_tw1024[4 * (a + 8 * b)];
+        if (b < 9) {
+            s_twsp[0][a][b] = c_tw1024[2 * (2 * a + 16 * b)];
+            s_twsp[1][a][b] = c_tw1024[2 * (2 * a + 1 + 16 * b)];
+        }
+    }
+    const C* t128 = &s_tw128[w][0];
+    const C* tin = &s_twin[h][w][0];
+    const C* tsp = &s_twsp[h][w][0];
     __syncthreads();
 
     const int ntiles = p.nrows / kXRows;
@@ -489,12 +520,9 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
             mbar_wait(&bar, parity);
             parity ^= 1;
 #pragma unroll
-            for (int r = 0; r < 16; ++r) {
-                const C z = *reinterpret_cast<const C*>(rbuf + pen * kXInPitch + 2 * (w + 8 * r));
-                const C t = c_tw1024[4 * (w + 8 * r)];   // w256^n
-                v[r] = cmul(z, make_float2(h ? t.x : 1.f, h ? t.y : 0.f));
-            }
-            fft128_a<false>(v, w, xw);
+            for (int r = 0; r < 16; ++r)
+                v[r] = cmul(*reinterpret_cast<const C*>(rbuf + pen * kXInPitch + 2 * (w + 8 * r)), tin[r]);   // h = 1: z w256^n
+            fft128_a<false>(v, t128, xw);
             if (tid < kXRows) bulk_wait_read();   // the previous tile's stores have left sbuf
             __syncthreads();
             issue(i + 1);                         // rbuf is in registers everywhere
@@ -509,19 +537,24 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
             __syncthreads();
             // split in place: the 16 threads of a row own the pairs (k, 256 - k), k = idx + 16 m
             const int idx = 2 * w + h;
+            {
+                C zk[9], zm[9];
 #pragma unroll
-            for (int m = 0; m < 9; ++m) {
-                const int k = idx + 16 * m;
-                if (m < 8 || idx == 0) {
-                    const C te = c_tw1024[2 * (2 * w + 16 * m)], to = c_tw1024[2 * (2 * w + 1 + 16 * m)];   // w512^k
-                    const C tw = make_float2(h ? to.x : te.x, h ? to.y : te.y);
-                    const C zk = srow[k], zm = srow[(kXN - k) & (kXN - 1)];
-                    const C e = cadd(zk, make_float2(zm.x, -zm.y));
-                    const C d = csub(zk, make_float2(zm.x, -zm.y));
-                    const C wd = cmul(d, tw);
-                    // X[k] = (e - i wd) / 2,  X[256 - k] = (conj e - i conj wd) / 2
-                    srow[k] = cscale(cadd(e, make_float2(wd.y, -wd.x)), 0.5f);
-                    srow[kXN - k] = cscale(make_float2(e.x - wd.y, -e.y - wd.x), 0.5f);
+                for (int m = 0; m < 9; ++m) {
+                    const int k = idx + 16 * m;
+                    if (m < 8 || idx == 0) { zk[m] = srow[k]; zm[m] = srow[(kXN - k) & (kXN - 1)]; }
+                }
+#pragma unroll
+                for (int m = 0; m < 9; ++m) {
+                    const int k = idx + 16 * m;
+                    if (m < 8 || idx == 0) {
+                        const C e = cadd(zk[m], make_float2(zm[m].x, -zm[m].y));
+                        const C d = csub(zk[m], make_float2(zm[m].x, -zm[m].y));
+                        const C wd = cmul(d, tsp[m]);   // w512^k d
+                        // X[k] = (e - i wd) / 2,  X[256 - k] = (conj e - i conj wd) / 2
+                        srow[k] = cscale(cadd(e, make_float2(wd.y, -wd.x)), 0.5f);
+                        srow[kXN - k] = cscale(make_float2(e.x - wd.y, -e.y - wd.x), 0.5f);
+                    }
                 }
             }
             fence_async_smem();
@@ -536,24 +569,29 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
             parity ^= 1;
             // merge in place: Z[k] = e + i conj(w512^k) d, Z[256 - k] = conj e + i conj(conj(w512^k) d)
             const int idx = 2 * w + h;
+            {
+                C xk[9], xm[9];
 #pragma unroll
-            for (int m = 0; m < 9; ++m) {
-                const int k = idx + 16 * m;
-                if (m < 8 || idx == 0) {
-                    const C te = c_tw1024[2 * (2 * w + 16 * m)], to = c_tw1024[2 * (2 * w + 1 + 16 * m)];
-                    const C tw = make_float2(h ? to.x : te.x, h ? to.y : te.y);
-                    const C xk = srow[k], xm = srow[kXN - k];
-                    const C e = cadd(xk, make_float2(xm.x, -xm.y));
-                    const C d = csub(xk, make_float2(xm.x, -xm.y));
-                    const C wd = cmulc(d, tw);
-                    srow[k] = cadd(e, make_float2(-wd.y, wd.x));
-                    if (k > 0) srow[kXN - k] = make_float2(e.x + wd.y, wd.x - e.y);
+                for (int m = 0; m < 9; ++m) {
+                    const int k = idx + 16 * m;
+                    if (m < 8 || idx == 0) { xk[m] = srow[k]; xm[m] = srow[kXN - k]; }
+                }
+#pragma unroll
+                for (int m = 0; m < 9; ++m) {
+                    const int k = idx + 16 * m;
+                    if (m < 8 || idx == 0) {
+                        const C e = cadd(xk[m], make_float2(xm[m].x, -xm[m].y));
+                        const C d = csub(xk[m], make_float2(xm[m].x, -xm[m].y));
+                        const C wd = cmulc(d, tsp[m]);   // conj(w512^k) d
+                        srow[k] = cadd(e, make_float2(-wd.y, wd.x));
+                        if (k > 0) srow[kXN - k] = make_float2(e.x + wd.y, wd.x - e.y);
+                    }
                 }
             }
             __syncthreads();
 #pragma unroll
             for (int j = 0; j < 16; ++j) v[j] = srow[2 * (w + 8 * j) + h];   // Z[2 k' + h], k' = w + 8 j
-            fft128_a<true>(v, w, xw);
+            fft128_a<true>(v, t128, xw);
             if (tid < kXRows) bulk_wait_read();   // the previous tile's stores have left rbuf
             fence_async_smem();                   // the merged values in sbuf are overwritten by the next bulk load
             __syncthreads();
@@ -564,11 +602,10 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
             // h = 1 holds z1; h = 0 finishes the a set, h = 1 the b set
 #pragma unroll
             for (int k2 = 0; k2 < 8; ++k2) {
-                const C wa = c_tw1024[4 * (w + 16 * k2)], wb = c_tw1024[4 * (w + 8 + 16 * k2)];
-                const C va = a[brev3(k2)], vb = b[brev3(k2)];
-                const C ta = cmulc(va, wa), tb = cmulc(vb, wb);
-                const C send = h ? ta : vb;
-                const C keep = h ? tb : va;
+                // (the table row of h = 0 is all ones)
+                const C ta = cmulc(a[brev3(k2)], tin[2 * k2]), tb = cmulc(b[brev3(k2)], tin[2 * k2 + 1]);
+                const C send = h ? ta : tb;
+                const C keep = h ? tb : ta;
                 C recv;
                 recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
                 recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);

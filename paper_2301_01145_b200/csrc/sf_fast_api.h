@@ -8,6 +8,7 @@ namespace sf2 {
 typedef float2 C;
 
 constexpr int kTile = 16;            // pencils per tile
+constexpr int kGreenRows = 257;      // folded spectral indices along the pencil axis (0 .. 256)
 
 enum { FMODE_FWD = 0, FMODE_INV = 1, FMODE_FUSED = 2 };
 
@@ -20,9 +21,9 @@ struct FastParams {
     int nct;                    // full 16-column tiles per batch
     int nyq_col;                // column handled 16 batches at a time (the Nyquist column), -1: none
     int pair_batches;           // fused: visit batches as 0, P/2, 1, P-1, 2, P-2, ... (mirror pairs share table rows)
-    // fused multiply: compact real Green's table [fp][fb][kx] (rhs sign and normalisation folded in)
-    const float* green;
-    long long g_pb, g_pp;
+    // fused multiply: real Green's table (rhs sign and normalisation folded in), tile-major:
+    // chunk [kGreenRows fp][16 pencils] per tile, see green_tile_index / fast_green_tiles
+    const float* green_tiles;
     int Pb;                     // transform length along the batch axis (index folding k -> min(k, P-k))
 };
 
@@ -47,6 +48,14 @@ cudaError_t fast_init();
 // (multiples of 16); box = tile image moved by one TMA instruction (dense, no swizzle)
 cudaError_t fast_make_map(TileMap* out, const void* base, const unsigned long long dims[4],
                           const unsigned long long strides_bytes[3], const unsigned box[4]);
+// number of floats of the tile-major Green's table for nb = P batches, nct column tiles (+ Nyquist column)
+inline size_t fast_green_tiles_elems(int Pb, int nct, int nyq_col)
+{
+    return ((size_t)(Pb / 2 + 1) * nct + (nyq_col >= 0 ? (size_t)(Pb + kTile - 1) / kTile : 0)) * kGreenRows * kTile;
+}
+// re-lay the compact table green[fp][fb][kx] (pitches g_pp, g_pb) tile-major into `tiles`
+cudaError_t fast_green_tiles(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
+                             cudaStream_t st);
 // launch one padded pass (mode = FMODE_*) as a persistent grid of two CTAs per SM; `in_map`
 // describes p.in as documented at fast_pad_kernel
 cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map, cudaStream_t st);
