@@ -84,8 +84,8 @@ def model_bytes(w):
     return [s1, s2, s3, s4, s5]
 
 
-STEP_NAMES = ["S1 xfwd_kernel", "S2 spass_kernel<MODE 0>", "S3 spass_kernel<MODE 2>", "S4 spass_kernel<MODE 1>",
-              "S5 xinv_kernel"]
+STEP_NAMES = ["S1 fast_x_kernel<fwd>", "S2 fast_pad_kernel<FWD>", "S3 fast_pad_kernel<FUSED>", "S4 fast_pad_kernel<INV>",
+              "S5 fast_x_kernel<inv>"]
 
 
 def make_input(w, rank=0):

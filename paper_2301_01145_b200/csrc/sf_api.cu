@@ -395,7 +395,9 @@ template <typename T> sf_status run(sf_plan p, int outk)
         // S2: W1 [z][y][hp] -> W2 [z][ky][hp]
         fp.in = (const sf2::C*)p->W1; fp.out = (sf2::C*)p->W2;
         fp.in_ps = hp; fp.in_bs = hp * n1; fp.out_ps = hp; fp.out_bs = hp * P1; fp.nb = n2;
+        fp.reverse_batches = 1;   // S1 wrote plane z last: start there while it is in L2
         SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_FWD, fp, p->map_s2, st));
+        fp.reverse_batches = 0;
         p->launches++;
         mark(2);
         // S3: W2 in place along z
@@ -414,6 +416,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         p->launches++;
         mark(4);
         xp.spec_in = p->W1; xp.real_out = (T*)p->out;
+        fx.reverse = 1;           // S4 wrote the last planes last
         if (fast_x) SF_CUDA(p, sf2::launch_fast_x(true, fx, st));
         else SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
         p->launches++;

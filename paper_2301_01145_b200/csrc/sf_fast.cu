@@ -32,6 +32,27 @@ cudaError_t fast_init()
         tw[j] = make_float2((float)cosl(a), (float)(-sinl(a)));
     }
     if ((e = cudaMemcpyToSymbol(c_tw1024, tw.data(), sizeof(float2) * 1024)) != cudaSuccess) return e;
+    {
+        std::vector<float2> tp(768), tx(544, make_float2(0.f, 0.f));
+        for (int a = 0; a < 16; ++a)
+            for (int b = 0; b < 16; ++b) {
+                tp[a * 16 + b] = tw[4 * a * b];
+                tp[256 + a * 16 + b] = make_float2(1.f, 0.f);
+                tp[256 + (16 + a) * 16 + b] = tw[2 * (a + 16 * b)];
+            }
+        for (int a = 0; a < 8; ++a)
+            for (int b = 0; b < 16; ++b) {
+                tx[a * 16 + b] = tw[8 * a * b];
+                tx[128 + a * 16 + b] = make_float2(1.f, 0.f);
+                tx[128 + (8 + a) * 16 + b] = tw[4 * (a + 8 * b)];
+                if (b < 9) {
+                    tx[384 + a * 10 + b] = tw[2 * (2 * a + 16 * b)];
+                    tx[384 + (8 + a) * 10 + b] = tw[2 * (2 * a + 1 + 16 * b)];
+                }
+            }
+        if ((e = cudaMemcpyToSymbol(g_tab_pad, tp.data(), sizeof(float2) * 768)) != cudaSuccess) return e;
+        if ((e = cudaMemcpyToSymbol(g_tab_x, tx.data(), sizeof(float2) * 544)) != cudaSuccess) return e;
+    }
     if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_FWD>::kSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_INV>::kSmem)) != cudaSuccess) return e;

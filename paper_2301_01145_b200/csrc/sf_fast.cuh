@@ -44,6 +44,13 @@ constexpr int kTileElems = kL * kTile;
 
 // exp(-2 pi i j / 1024), j < 1024 (this header is compiled into one translation unit: sf_fast.cu)
 __constant__ float2 c_tw1024[1024];
+// the per-kernel twiddle tables, laid out as the kernels keep them in shared memory (filled once by
+// fast_init; a CTA copies them with coalesced 16-byte loads):
+//   strided passes: [0, 256) tw256[o][q] = w256^(q o); [256, 768) tw512[h][o][r] = h ? w512^(o + 16 r) : 1
+//   X passes:       [0, 128) tw128[w][q] = w128^(q w); [128, 384) twin[h][w][j] = h ? w256^(w + 8 j) : 1;
+//                   [384, 544) twsp[h][w][m] = w512^(2 w + h + 16 m), m < 10
+__device__ float2 g_tab_pad[768];
+__device__ float2 g_tab_x[544];
 
 // ------------------------------------------------------------------------------------ complex, packed
 __device__ __forceinline__ C cadd(C a, C b) { return __fadd2_rn(a, b); }
@@ -129,11 +136,13 @@ struct Xchg {
 // first half: radix-16 over r, twiddle, write.  v[r] = x[o + 16 r] in; nothing valid out.
 // Twiddles come from a per-warp row of a shared-memory table: base register + immediate, no
 // address arithmetic, and a latency the other warps cover.
-template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256_a(C (&v)[16], const C* tw256, const Xchg& x)
+// (TWC: from the constant bank through uniform registers instead -- ptxas does that for the fused
+// and backward kernels, where it is cheaper than the shared-memory reads)
+template <bool INV, bool ORIENT_B, bool TWC> __device__ __forceinline__ void fft256_a(C (&v)[16], const C* tw256, int o, const Xchg& x)
 {
     dft16<INV>(v);
 #pragma unroll
-    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], tw256[q]);   // w256^(q o), row o of the table
+    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], TWC ? c_tw1024[4 * q * o] : tw256[q]);   // w256^(q o)
     C* w = x.base + (ORIENT_B ? x.eb : x.ea);
     constexpr int ws = (ORIENT_B ? 32 : 512);
 #pragma unroll
@@ -204,6 +213,7 @@ struct TileGeom {
 };
 __device__ __forceinline__ int batch_order(const FastParams& p, int bi)
 {
+    if (p.reverse_batches) return p.nb - 1 - bi;   // consume the producer's most recent output first: it is still in L2
     if (!p.pair_batches) return bi;
     if (bi == 0) return 0;
     if (bi == 1) return p.nb / 2;
@@ -271,16 +281,10 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
     xc.eb = o * 512 + lane;
 
     // twiddle tables: s_tw256[o][q] = w256^(q o);  s_tw512[h][o][r] = w512^(o + 16 r) for h = 1, 1 for h = 0
-    __shared__ __align__(16) C s_tw256[16][16];
-    __shared__ __align__(16) C s_tw512[2][16][16];
-    for (int idx = tid; idx < 256; idx += kThreads) {
-        const int a = idx >> 4, b = idx & 15;
-        s_tw256[a][b] = c_tw1024[4 * a * b];
-        s_tw512[0][a][b] = make_float2(1.f, 0.f);
-        s_tw512[1][a][b] = c_tw1024[2 * (a + 16 * b)];
-    }
-    const C* t256 = &s_tw256[o][0];
-    const C* t512 = &s_tw512[h][o][0];
+    __shared__ __align__(16) C s_tab[768];
+    if (tid < 384) reinterpret_cast<float4*>(s_tab)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid];
+    const C* t256 = s_tab + o * 16;
+    const C* t512 = s_tab + 256 + (h * 16 + o) * 16;
     if (!Cfg::kTma) __syncthreads();
 
     if (Cfg::kTma) {
@@ -335,7 +339,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
             // h = 0: x -> even outputs;  h = 1: x w512^n -> odd outputs
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], t512[r]);
-            fft256_a<false, OB>(v, t256, xc);
+            fft256_a<false, OB, MODE != FMODE_FWD>(v, t256, o, xc);
             __syncthreads();
             issue(i + 1);   // every thread has taken its elements out of the slot
             fft256_b<false, OB>(v, xc);
@@ -357,7 +361,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                 load_x(g, v);
 #pragma unroll
                 for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], t512[r]);
-                fft256_a<false, OB>(v, t256, xc);
+                fft256_a<false, OB, MODE != FMODE_FWD>(v, t256, o, xc);
                 __syncthreads();
                 issue(i + 1);   // every thread has taken its elements out of the slot
                 fft256_b<false, OB>(v, xc);
@@ -366,7 +370,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                 for (int k2 = 0; k2 < 16; ++k2) u[k2] = cscale(v[brev4(k2)], gm[k2]);
 #pragma unroll
                 for (int k2 = 0; k2 < 16; ++k2) v[k2] = u[k2];
-                fft256_a<true, !OB>(v, t256, xc);
+                fft256_a<true, !OB, MODE != FMODE_FWD>(v, t256, o, xc);
                 __syncthreads();
                 fft256_b<true, !OB>(v, xc);
             } else {
@@ -376,7 +380,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                                (2 * o + h) * ips;
 #pragma unroll
                 for (int k2 = 0; k2 < 16; ++k2) v[k2] = __ldg(inp + k2 * 32 * ips);
-                fft256_a<true, OB>(v, t256, xc);
+                fft256_a<true, OB, MODE != FMODE_FWD>(v, t256, o, xc);
                 __syncthreads();
                 fft256_b<true, OB>(v, xc);
             }
@@ -476,22 +480,11 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
     // twiddle tables (base register + immediate addressing, no selects):
     //   s_tw128[w][q] = w128^(q w);  s_twin[h][w][j] = w256^(w + 8 j) for h = 1, 1 for h = 0;
     //   s_twsp[h][w][m] = w512^(2 w + h + 16 m)
-    __shared__ __align__(16) C s_tw128[8][16];
-    __shared__ __align__(16) C s_twin[2][8][16];
-    __shared__ __align__(16) C s_twsp[2][8][10];
-    for (int idx = tid; idx < 128; idx += kXThreads) {
-        const int a = idx >> 4, b = idx & 15;
-        s_tw128[a][b] = c_tw1024[8 * a * b];
-        s_twin[0][a][b] = make_float2(1.f, 0.f);
-        s_twin[1][a][b] = c_tw1024[4 * (a + 8 * b)];
-        if (b < 9) {
-            s_twsp[0][a][b] = c_tw1024[2 * (2 * a + 16 * b)];
-            s_twsp[1][a][b] = c_tw1024[2 * (2 * a + 1 + 16 * b)];
-        }
-    }
-    const C* t128 = &s_tw128[w][0];
-    const C* tin = &s_twin[h][w][0];
-    const C* tsp = &s_twsp[h][w][0];
+    __shared__ __align__(16) C s_tab[544];
+    for (int idx = tid; idx < 272; idx += kXThreads) reinterpret_cast<float4*>(s_tab)[idx] = reinterpret_cast<const float4*>(g_tab_x)[idx];
+    const C* t128 = s_tab + w * 16;
+    const C* tin = s_tab + 128 + (h * 8 + w) * 16;
+    const C* tsp = s_tab + 384 + (h * 8 + w) * 10;
     __syncthreads();
 
     const int ntiles = p.nrows / kXRows;
@@ -504,7 +497,8 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
     // bulk loads of iteration i: one row per lane of warp 0
     auto issue = [&](int i) {
         if (tid >= kXRows || i >= nit) return;
-        const long long row = ((long long)blockIdx.x + (long long)i * gridDim.x) * kXRows + tid;
+        const long long tl = (long long)blockIdx.x + (long long)i * gridDim.x;
+        const long long row = (p.reverse ? ntiles - 1 - tl : tl) * kXRows + tid;
         if (tid == 0) mbar_expect_tx(&bar, INV ? kXRows * kXSpPitch * (uint32_t)sizeof(C) : kXRows * kXN * (uint32_t)sizeof(float));
         __syncwarp(0xffffu);
         if (INV) bulk_g2s(sbuf + tid * kXSpPitch, p.spec + row * p.spec_pitch, kXSpPitch * (uint32_t)sizeof(C), &bar);
@@ -513,7 +507,8 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
 
     issue(0);
     for (int i = 0; i < nit; ++i) {
-        const long long row0 = ((long long)blockIdx.x + (long long)i * gridDim.x) * kXRows;
+        const long long tl0 = (long long)blockIdx.x + (long long)i * gridDim.x;
+        const long long row0 = (p.reverse ? ntiles - 1 - tl0 : tl0) * kXRows;
         C v[16];
         if constexpr (!INV) {
             // ---------------------------------------------------------------- S1

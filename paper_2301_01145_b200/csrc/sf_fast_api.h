@@ -20,6 +20,7 @@ struct FastParams {
     int nb;                     // batches
     int nct;                    // full 16-column tiles per batch
     int nyq_col;                // column handled 16 batches at a time (the Nyquist column), -1: none
+    int reverse_batches;        // visit batches last to first (the producer kernel wrote them first to last)
     int pair_batches;           // fused: visit batches as 0, P/2, 1, P-1, 2, P-2, ... (mirror pairs share table rows)
     // fused multiply: real Green's table (rhs sign and normalisation folded in), tile-major:
     // chunk [kGreenRows fp][16 pencils] per tile, see green_tile_index / fast_green_tiles
@@ -37,6 +38,7 @@ struct FastXParams {
     C* spec;                // half spectra, row pitch spec_pitch complex (>= 258, rows 16-byte aligned)
     long long spec_pitch;
     int nrows;              // multiple of 16
+    int reverse;            // visit row tiles last to first
 };
 
 // opaque storage of a CUtensorMap (TMA descriptor): 128 bytes, 64-byte aligned
