@@ -20,7 +20,7 @@ LIB = HERE / "libsailffish_b200.so"
 
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-COMMON = ["-std=c++17", "-O3", "-lineinfo", "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"] + ARCH
+COMMON = ["-std=c++17", "-O3", "-lineinfo", "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"] + ARCH + os.environ.get("SF_NVCC_EXTRA", "").split()
 
 UNITS = [("sf_api", "sf_api.cu", []), ("sf_fast", "sf_fast.cu", [])]
 for kind in range(4):

@@ -475,8 +475,7 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
         mbar_init(&bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (!INV)
-        for (int idx = tid; idx < kXRows * kXSpPitch; idx += kXThreads) sbuf[idx] = make_float2(0.f, 0.f);   // pad column 257 leaves as zero
+    if (!INV && tid < kXRows) sbuf[tid * kXSpPitch + kXN + 1] = make_float2(0.f, 0.f);   // pad column 257 leaves as zero
     // twiddle tables (base register + immediate addressing, no selects):
     //   s_tw128[w][q] = w128^(q w);  s_twin[h][w][j] = w256^(w + 8 j) for h = 1, 1 for h = 0;
     //   s_twsp[h][w][m] = w512^(2 w + h + 16 m)
