@@ -65,3 +65,60 @@ def test_cfg4_full_size(prec):
     e = rel_l2(got, exact)
     print(f"cfg4 256^3 {prec} vs closed form: rel-L2 {e:.3e}")
     assert e <= (5e-6 if prec == "f32" else 1e-9)
+
+
+def test_fast_path_options_and_generation1_agreement(monkeypatch):
+    """rhs_sign = -1, a non-default regularisation width, anisotropic spacing and a user stream on the
+    fast path; and the same plan built with SF_DISABLE_FAST=1 (kernel generation 1) must agree with it
+    to fp32 rounding."""
+    import torch
+
+    shape = (256, 256, 32)
+    f = rounded(W.Rng(4321).normal(int(np.prod(shape))).reshape(shape), "f32")
+    h = (0.010, 0.013, 0.009)
+    eps = 1.5 * max(h)
+    gh = O.unbounded_green((32, 256, 256), h, eps)
+    ref = O.unbounded_solve(f.astype(np.float64), h, gh, rhs_sign=-1.0)
+    stream = torch.cuda.Stream()
+    got = {}
+    for name, disable in (("generation 2", False), ("generation 1", True)):
+        if disable:
+            monkeypatch.setenv("SF_DISABLE_FAST", "1")
+        else:
+            monkeypatch.delenv("SF_DISABLE_FAST", raising=False)
+        with Plan(shape, h, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec="f32", rhs_sign=-1.0, eps_over_h=1.5,
+                  stream=stream.cuda_stream) as p:
+            with torch.cuda.stream(stream):
+                p.set_source(f)
+            stream.synchronize()
+            sf.sf_solve(p.plan)
+            sf.sf_solve(p.plan)
+            got[name] = p.get(sf.SF_OUT_PSI)
+        _check(f"psi {name}", got[name], ref, "f32")
+    e = rel_l2(got["generation 2"], got["generation 1"].astype(np.float64))
+    print(f"generation 2 vs generation 1: rel-L2 {e:.3e}")
+    assert e <= 1e-6
+
+
+def test_fast_path_zero_and_delta_sources():
+    """degenerate inputs: an all-zero source gives exactly zero; a single unit source reproduces the
+    regularised kernel h^3 G(|x - x0|) itself (reading A10 / A11), i.e. the definition with one term."""
+    shape = (256, 256, 256)
+    hh = (1.0 / 256,) * 3
+    eps = 2.0 * hh[0]
+    with Plan(shape, hh, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec="f32") as p:
+        p.set_source(np.zeros(shape, dtype=np.float32))
+        sf.sf_solve(p.plan)
+        assert not p.get(sf.SF_OUT_PSI).any()
+        f = np.zeros(shape, dtype=np.float32)
+        x0 = (200, 17, 255)   # z, y, x: off-centre, on the last column
+        f[x0] = 1.0
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI).astype(np.float64)
+    ref = O.unbounded_solve(f.astype(np.float64), hh, O.unbounded_green((256, 256, 256), hh, eps))
+    _check("psi of a unit source", got, ref, "f32")
+    for pt in ((200, 17, 255), (0, 0, 0), (255, 255, 0), (201, 17, 255), (100, 100, 100)):
+        r = hh[0] * float(np.sqrt(sum((pt[a] - x0[a]) ** 2 for a in range(3))))
+        want = hh[0] ** 3 * O.green_gauss2(r, eps)
+        assert abs(got[pt] - want) <= 2e-5 * abs(want) + 1e-12, (pt, got[pt], want)
