@@ -391,6 +391,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         sf2::FastParams fp;
         memset(&fp, 0, sizeof(fp));
         fp.nct = p->nspec_x / sf2::kTile;
+        for (fp.nct_shift = 0; (1 << fp.nct_shift) < fp.nct; ++fp.nct_shift) {}
         fp.nyq_col = (p->nspec_x % sf2::kTile) ? fp.nct * sf2::kTile : -1;
         // S2: W1 [z][y][hp] -> W2 [z][ky][hp]
         fp.in = (const sf2::C*)p->W1; fp.out = (sf2::C*)p->W2;
@@ -625,7 +626,8 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
 
     // kernel generation 2 covers fp32 scalar unbounded plans whose y and z pencils are 256 long
     if (prec == SF_F32 && b == SF_BC_UNBOUNDED && ndim == 3 && ncomp == 1 && p->n[1] == 256 && p->n[2] == 256 &&
-        (p->nspec_x % sf2::kTile) <= 1 && p->nspec_x >= sf2::kTile && !getenv("SF_DISABLE_FAST")) {
+        (p->nspec_x % sf2::kTile) <= 1 && p->nspec_x >= sf2::kTile && is_pow2(p->nspec_x / sf2::kTile) && p->n[0] <= 2048 &&
+        !getenv("SF_DISABLE_FAST")) {
         if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fp32 fast path failed"); }
         const unsigned long long hpB = (unsigned long long)p->pitch * 8ull, N1 = 256, N2 = 256, PP = 512;
         const unsigned long long hpc = (unsigned long long)p->pitch;

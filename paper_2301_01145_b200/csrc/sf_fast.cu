@@ -119,6 +119,10 @@ cudaError_t fast_green_tiles(float* tiles, const float* green, long long g_pb, l
 cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map, cudaStream_t st)
 {
     const CUtensorMap& tm = reinterpret_cast<const CUtensorMap&>(in_map);
+    if (p.nct <= 0 || (1 << p.nct_shift) != p.nct) return cudaErrorInvalidValue;
+    // the kernels index with 32-bit element offsets
+    if ((long long)p.nb * p.in_bs + 256 * p.in_ps >= (1ll << 31) || (long long)p.nb * p.out_bs + 512 * p.out_ps >= (1ll << 31))
+        return cudaErrorInvalidValue;
     const int ntiles = fast_ntiles(p.nb, p.nct, p.nyq_col);
     int grid = 2 * g_sms;
     if (grid > ntiles) grid = ntiles;

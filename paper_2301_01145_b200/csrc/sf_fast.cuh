@@ -224,17 +224,17 @@ __device__ __forceinline__ int batch_order(const FastParams& p, int bi)
 // then the Nyquist-column tiles (16 batches each)
 __device__ __forceinline__ int green_tile_index(const FastParams& p, const TileGeom& g)
 {
-    if (g.full) return min(g.b, p.Pb - g.b) * p.nct + g.col / kTile;
-    return (p.Pb / 2 + 1) * p.nct + g.b / kTile;
+    if (g.full) return (min(g.b, p.Pb - g.b) << p.nct_shift) + (g.col >> 4);
+    return ((p.Pb / 2 + 1) << p.nct_shift) + (g.b >> 4);
 }
 __device__ __forceinline__ TileGeom tile_geom(const FastParams& p, int t)
 {
     TileGeom g;
-    const int nfull = p.nb * p.nct;
+    const int nfull = p.nb << p.nct_shift;   // nct is a power of two: no integer division per tile
     if (t < nfull) {
         g.full = true;
-        g.b = batch_order(p, t / p.nct);
-        g.col = (t % p.nct) * kTile;
+        g.b = batch_order(p, t >> p.nct_shift);
+        g.col = (t & (p.nct - 1)) * kTile;
     } else {
         g.full = false;
         g.b = (t - nfull) * kTile;
@@ -296,7 +296,8 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
     }
 
     const int ntiles = fast_ntiles(p.nb, p.nct, p.nyq_col);
-    const int ips = (int)p.in_ps, ops = (int)p.out_ps;
+    // element offsets fit 32 bits: an eligible plan's work arrays hold < 2^31 complex numbers (checked by the launcher)
+    const int ips = (int)p.in_ps, ops = (int)p.out_ps, ibs = (int)p.in_bs, obs = (int)p.out_bs;
     const int nit = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles of this CTA
     uint32_t parity = 0;   // phase of `bar` the next full tile completes
 
@@ -318,7 +319,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = slot[(o + 16 * r) * kTile + pen];
         } else {
-            const C* inp = p.in + (long long)min(g.b + pen, p.nb - 1) * p.in_bs + g.col + o * ips;
+            const C* inp = p.in + (min(g.b + pen, p.nb - 1) * ibs + g.col + o * ips);
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = __ldg(inp + r * 16 * ips);
         }
@@ -330,7 +331,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
         const TileGeom g = tile_geom(p, (int)blockIdx.x + i * (int)gridDim.x);
         // this thread's pencil: output pointer, validity
         const bool pvalid = g.full || (g.b + pen < p.nb);
-        const long long ob = g.full ? ((long long)g.b * p.out_bs + g.col + pen) : ((long long)(g.b + pen) * p.out_bs + g.col);
+        const int ob = g.full ? (g.b * obs + g.col + pen) : ((g.b + pen) * obs + g.col);
         C* outp = p.out + ob;
         C v[16];
 
@@ -353,7 +354,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                 float gm[16];
                 // the tile's chunk of the tile-major table [257 fp][16 pencils]; the thread's spectral
                 // indices kp = 2 (o + 16 k2) + h fold to fp = min(kp, 512 - kp): every offset is an immediate
-                const float* gt = p.green_tiles + (long long)green_tile_index(p, g) * (kGreenRows * kTile) + pen;
+                const float* gt = p.green_tiles + (green_tile_index(p, g) * (kGreenRows * kTile) + pen);
                 const float* glo = gt + (2 * o + h) * kTile;              // kp            (k2 < 8)
                 const float* ghi = gt + (2 * kL - 2 * o - h) * kTile;     // 512 - kp      (k2 >= 8)
 #pragma unroll
@@ -376,8 +377,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
             } else {
                 // rows 2 k + h, k = o + 16 k2: h = 0 even spectrum E, h = 1 odd spectrum O; each half-warp
                 // reads one 128-byte run per row (16 batches of one column for the Nyquist tiles)
-                const C* inp = p.in + (g.full ? ((long long)g.b * p.in_bs + g.col + pen) : ((long long)min(g.b + pen, p.nb - 1) * p.in_bs + g.col)) +
-                               (2 * o + h) * ips;
+                const C* inp = p.in + ((g.full ? (g.b * ibs + g.col + pen) : (min(g.b + pen, p.nb - 1) * ibs + g.col)) + (2 * o + h) * ips);
 #pragma unroll
                 for (int k2 = 0; k2 < 16; ++k2) v[k2] = __ldg(inp + k2 * 32 * ips);
                 fft256_a<true, OB, MODE != FMODE_FWD>(v, t256, o, xc);

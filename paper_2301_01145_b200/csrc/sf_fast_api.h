@@ -18,7 +18,8 @@ struct FastParams {
     long long in_ps, in_bs;     // row (pencil-axis) and batch strides of the input, complex elements
     long long out_ps, out_bs;
     int nb;                     // batches
-    int nct;                    // full 16-column tiles per batch
+    int nct;                    // full 16-column tiles per batch: a power of two
+    int nct_shift;              // log2(nct)
     int nyq_col;                // column handled 16 batches at a time (the Nyquist column), -1: none
     int reverse_batches;        // visit batches last to first (the producer kernel wrote them first to last)
     int pair_batches;           // fused: visit batches as 0, P/2, 1, P-1, 2, P-2, ... (mirror pairs share table rows)
