@@ -43,11 +43,11 @@ cudaError_t fast_init()
         for (int a = 0; a < 8; ++a)
             for (int b = 0; b < 16; ++b) {
                 tx[a * 16 + b] = tw[8 * a * b];
-                tx[128 + a * 16 + b] = make_float2(1.f, 0.f);
-                tx[128 + (8 + a) * 16 + b] = tw[4 * (a + 8 * b)];
+                tx[128 + (a * 16 + b) * 2] = make_float2(1.f, 0.f);
+                tx[128 + (a * 16 + b) * 2 + 1] = tw[4 * (a + 8 * b)];
                 if (b < 9) {
-                    tx[384 + a * 10 + b] = tw[2 * (2 * a + 16 * b)];
-                    tx[384 + (8 + a) * 10 + b] = tw[2 * (2 * a + 1 + 16 * b)];
+                    tx[384 + (a * 10 + b) * 2] = tw[2 * (2 * a + 16 * b)];
+                    tx[384 + (a * 10 + b) * 2 + 1] = tw[2 * (2 * a + 1 + 16 * b)];
                 }
             }
         if ((e = cudaMemcpyToSymbol(g_tab_pad, tp.data(), sizeof(float2) * 768)) != cudaSuccess) return e;

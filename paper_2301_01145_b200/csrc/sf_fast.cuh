@@ -47,8 +47,9 @@ __constant__ float2 c_tw1024[1024];
 // the per-kernel twiddle tables, laid out as the kernels keep them in shared memory (filled once by
 // fast_init; a CTA copies them with coalesced 16-byte loads):
 //   strided passes: [0, 256) tw256[o][q] = w256^(q o); [256, 768) tw512[h][o][r] = h ? w512^(o + 16 r) : 1
-//   X passes:       [0, 128) tw128[w][q] = w128^(q w); [128, 384) twin[h][w][j] = h ? w256^(w + 8 j) : 1;
-//                   [384, 544) twsp[h][w][m] = w512^(2 w + h + 16 m), m < 10
+//   X passes:       [0, 128) tw128[w][q] = w128^(q w); [128, 384) twin[w][j][h] = h ? w256^(w + 8 j) : 1;
+//                   [384, 544) twsp[w][m][h] = w512^(2 w + h + 16 m), m < 10  (h innermost: the two
+//                   halves of a lane pair read one 16-byte word)
 __device__ float2 g_tab_pad[768];
 __device__ float2 g_tab_x[544];
 
@@ -419,8 +420,8 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
 // ==================================================================================== X passes
 // S1 (X forward) and S5 (X backward) for rows of 256 reals zero-padded to 512 (PAPER.md:87 real
 // transform / half spectrum; PAPER.md:181 padding).  Rows are contiguous in memory, so a tile of 16
-// rows is staged through shared memory by bulk copies (one per row) and transposed there: lanes
-// 0..3 = row, lane bit 4 = h, warp = w in 0..7.
+// rows is staged through shared memory by bulk copies (one per row) and transposed there: lane =
+// 2 * row + h, warp = w in 0..7.
 //   forward: the padded real row of length 512 is packed as z[n] = x[2n] + i x[2n+1], n < 256,
 //   non-zero for n < 128.  Z = DFT256(z) is two 128-point transforms, of z (even outputs, h = 0)
 //   and of z w256^n (odd outputs, h = 1); then the real-transform split
@@ -468,8 +469,10 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
-    const int pen = lane & 15;
-    const int h = lane >> 4;
+    // lane = 2 * row + h: the 16 lanes of a half-warp (8 rows x 2 halves) then touch 16 different
+    // 8-byte bank pairs of the staged rows, whose pitches are 16 (mod 128) bytes
+    const int pen = lane >> 1;
+    const int h = lane & 1;
     const int w = (int)__reduce_max_sync(0xffffffffu, (unsigned)(tid >> 5));
     if (tid == 0) {
         mbar_init(&bar, 1);
@@ -482,8 +485,8 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
     __shared__ __align__(16) C s_tab[544];
     for (int idx = tid; idx < 272; idx += kXThreads) reinterpret_cast<float4*>(s_tab)[idx] = reinterpret_cast<const float4*>(g_tab_x)[idx];
     const C* t128 = s_tab + w * 16;
-    const C* tin = s_tab + 128 + (h * 8 + w) * 16;
-    const C* tsp = s_tab + 384 + (h * 8 + w) * 10;
+    const C* tin = s_tab + 128 + w * 32 + h;   // twin[w][j][h]: index 2 j
+    const C* tsp = s_tab + 384 + w * 20 + h;   // twsp[w][m][h]: index 2 m
     __syncthreads();
 
     const int ntiles = p.nrows / kXRows;
@@ -515,7 +518,7 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
             parity ^= 1;
 #pragma unroll
             for (int r = 0; r < 16; ++r)
-                v[r] = cmul(*reinterpret_cast<const C*>(rbuf + pen * kXInPitch + 2 * (w + 8 * r)), tin[r]);   // h = 1: z w256^n
+                v[r] = cmul(*reinterpret_cast<const C*>(rbuf + pen * kXInPitch + 2 * (w + 8 * r)), tin[2 * r]);   // h = 1: z w256^n
             fft128_a<false>(v, t128, xw);
             if (tid < kXRows) bulk_wait_read();   // the previous tile's stores have left sbuf
             __syncthreads();
@@ -544,7 +547,7 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
                     if (m < 8 || idx == 0) {
                         const C e = cadd(zk[m], make_float2(zm[m].x, -zm[m].y));
                         const C d = csub(zk[m], make_float2(zm[m].x, -zm[m].y));
-                        const C wd = cmul(d, tsp[m]);   // w512^k d
+                        const C wd = cmul(d, tsp[2 * m]);   // w512^k d
                         // X[k] = (e - i wd) / 2,  X[256 - k] = (conj e - i conj wd) / 2
                         srow[k] = cscale(cadd(e, make_float2(wd.y, -wd.x)), 0.5f);
                         srow[kXN - k] = cscale(make_float2(e.x - wd.y, -e.y - wd.x), 0.5f);
@@ -576,7 +579,7 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
                     if (m < 8 || idx == 0) {
                         const C e = cadd(xk[m], make_float2(xm[m].x, -xm[m].y));
                         const C d = csub(xk[m], make_float2(xm[m].x, -xm[m].y));
-                        const C wd = cmulc(d, tsp[m]);   // conj(w512^k) d
+                        const C wd = cmulc(d, tsp[2 * m]);   // conj(w512^k) d
                         srow[k] = cadd(e, make_float2(-wd.y, wd.x));
                         if (k > 0) srow[kXN - k] = make_float2(e.x + wd.y, wd.x - e.y);
                     }
@@ -597,12 +600,12 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
 #pragma unroll
             for (int k2 = 0; k2 < 8; ++k2) {
                 // (the table row of h = 0 is all ones)
-                const C ta = cmulc(a[brev3(k2)], tin[2 * k2]), tb = cmulc(b[brev3(k2)], tin[2 * k2 + 1]);
+                const C ta = cmulc(a[brev3(k2)], tin[4 * k2]), tb = cmulc(b[brev3(k2)], tin[4 * k2 + 2]);
                 const C send = h ? ta : tb;
                 const C keep = h ? tb : ta;
                 C recv;
-                recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
-                recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+                recv.x = __shfl_xor_sync(0xffffffffu, send.x, 1);
+                recv.y = __shfl_xor_sync(0xffffffffu, send.y, 1);
                 const C z = cadd(keep, recv);
                 const int n = w + 8 * h + 16 * k2;
                 *reinterpret_cast<C*>(rbuf + pen * kXInPitch + 2 * n) = z;   // (x[2n], x[2n+1])
