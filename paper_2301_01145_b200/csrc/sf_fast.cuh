@@ -8,7 +8,7 @@
 //
 // Mapping.  A CTA of 512 threads owns a tile of 16 neighbouring pencils (16 complex columns = one
 // 128-byte run per row).  Warp index = o in 0..15 (warp-uniform, so every twiddle factor is a
-// uniform-register operand); lane bits 0..3 = pencil; lane bit 4 = h selects which HALF of the
+// uniform-register or broadcast shared-memory operand); lane bits 0..3 = pencil; lane bit 4 = h selects which HALF of the
 // padded problem the thread works on (below).  Thread (o, pencil, h) holds the 16 elements
 // n = o + 16 r of its pencil in registers.  A 256-point transform is
 //     radix-16 DFT over r (registers)  ->  twiddle w256^(q o)  ->  ONE shared-memory exchange
@@ -18,7 +18,9 @@
 // the orientation of the exchange buffer, which makes every location be rewritten by the thread
 // that read it last: one __syncthreads per transform.
 // Complex numbers live in aligned register pairs and all arithmetic is FADD2 / FMUL2 / FFMA2
-// (one issue slot per complex add, two per complex multiply, +-i free as an operand swizzle).
+// (one instruction per complex add, two per complex multiply, +-i free as an operand swizzle; on
+// this part a packed instruction costs two issue cycles, like the two scalar ones it replaces, so
+// the gain is in instruction count and register moves -- profiles/r01_b.md).
 //
 // Zero padding never exists: the 512-point transform of (x, 0) is two 256-point transforms, of x
 // (even outputs, h = 0) and of x w512^n (odd outputs, h = 1); the truncated backward transform is
@@ -27,8 +29,8 @@
 //
 // Tiles of the forward and fused passes arrive by TMA (cp.async.bulk.tensor, one instruction per
 // tile, completion on an mbarrier) in a shared-memory slot that is refilled for the next tile as
-// soon as the current one sits in registers; results go from registers to global memory as
-// 128-byte runs.  Persistent CTAs, two per SM (64 registers per thread): the two CTAs are
+// soon as the current one sits in registers; the backward pass (tile image twice as large) loads
+// straight into registers; results go from registers to global memory as 128-byte runs.  Persistent CTAs, two per SM (64 registers per thread): the two CTAs are
 // independent barrier domains, so one does arithmetic while the other exchanges, loads or stores.
 #pragma once
 #include "sf_fast_api.h"
