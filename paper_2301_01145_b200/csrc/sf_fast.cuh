@@ -4,12 +4,12 @@
 // Same steps as sf_spass.cuh (S2 Y forward, S3 Z forward x multiplier x Z backward, S4 Y backward;
 // PAPER.md:89-97 pencils, :103-109 four-step solve, :181 / :213 padded and pruned Hockney-Eastwood
 // transforms), specialised to complex pencils of length 256 that are zero-padded to 512
-// (unbounded, PAD) or transformed as they are (periodic).
+// (unbounded plans).
 //
 // Mapping.  A CTA of 512 threads owns a tile of 16 neighbouring pencils (16 complex columns = one
 // 128-byte run per row).  Warp index = o in 0..15 (warp-uniform, so every twiddle factor is a
-// uniform-register or broadcast shared-memory operand); lane bits 0..3 = pencil; lane bit 4 = h selects which HALF of the
-// padded problem the thread works on (below).  Thread (o, pencil, h) holds the 16 elements
+// uniform-register or broadcast shared-memory operand); lane bits 0..3 = pencil; lane bit 4 = h
+// selects which HALF of the padded problem the thread works on (below).  Thread (o, pencil, h) holds the 16 elements
 // n = o + 16 r of its pencil in registers.  A 256-point transform is
 //     radix-16 DFT over r (registers)  ->  twiddle w256^(q o)  ->  ONE shared-memory exchange
 //     (q, o) -> (o, o')  ->  radix-16 DFT over o' (registers)
@@ -30,8 +30,9 @@
 // Tiles of the forward and fused passes arrive by TMA (cp.async.bulk.tensor, one instruction per
 // tile, completion on an mbarrier) in a shared-memory slot that is refilled for the next tile as
 // soon as the current one sits in registers; the backward pass (tile image twice as large) loads
-// straight into registers; results go from registers to global memory as 128-byte runs.  Persistent CTAs, two per SM (64 registers per thread): the two CTAs are
-// independent barrier domains, so one does arithmetic while the other exchanges, loads or stores.
+// straight into registers; results go from registers to global memory as 128-byte runs.
+// Persistent CTAs, two per SM (64 registers per thread): the two CTAs are independent barrier
+// domains, so one does arithmetic while the other exchanges, loads or stores.
 #pragma once
 #include "sf_fast_api.h"
 #include <cuda.h>
