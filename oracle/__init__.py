@@ -43,6 +43,8 @@ def lib() -> C.CDLL:
         L.orc_num_threads.restype = C.c_int
         L.orc_green_gauss2.restype = C.c_double
         L.orc_green_gauss2.argtypes = [C.c_double, C.c_double]
+        L.orc_green_gauss.restype = C.c_double
+        L.orc_green_gauss.argtypes = [C.c_int, C.c_double, C.c_double]
         L.orc_unbounded_spec_size.restype = C.c_longlong
         _lib = L
     return _lib
@@ -175,11 +177,17 @@ def green_gauss2(r, eps):
     return float(lib().orc_green_gauss2(float(r), float(eps)))
 
 
-def unbounded_green(n_xyz, h, eps):
+def green_gauss(order, r, eps):
+    """Gaussian-regularised kernel of order 2, 4 or 6 at distance r."""
+    return float(lib().orc_green_gauss(int(order), float(r), float(eps)))
+
+
+def unbounded_green(n_xyz, h, eps, order=2):
     """Green's spectrum on the doubled grid: complex array [2 nz, 2 ny, nx + 1]."""
     n = [int(v) for v in n_xyz]
     ghat = np.empty((2 * n[2], 2 * n[1], n[0] + 1), dtype=np.complex128)
-    _chk(lib().orc_unbounded_green(_i64x3(n), _f64x3(h), C.c_double(eps), _ptr(ghat)), "unbounded_green")
+    _chk(lib().orc_unbounded_green_order(_i64x3(n), _f64x3(h), C.c_double(eps), C.c_int(order), _ptr(ghat)),
+         "unbounded_green")
     return ghat
 
 

@@ -580,6 +580,26 @@ double orc_green_gauss2(double r, double eps)
     return -erf(r / (sqrt(2.0) * eps)) / (4.0 * PI * r);
 }
 
+/* Hejlesen's Gaussian kernels of order P = 2, 4, 6 ("Gaussian approximations of order
+ * P = 2, 4, ... 10"; formulas not printed -- reading A25 of DESIGN.md).  In spectral space the
+ * order-P kernel is  G^_P(k) = -zeta^_P(eps k) / k^2  with
+ *     zeta^_P(s) = exp(-s^2/2) * sum_{n < P/2} (s^2/2)^n / n! ,
+ * i.e. the Gaussian times the Taylor polynomial that cancels its deviation from 1 up to s^(P-2).
+ * Term n of the sum is  -(eps^2/2)^n / n! * k^(2n-2) exp(-eps^2 k^2 / 2); with g(r) the unit
+ * Gaussian of width eps, (2 pi eps^2)^(-3/2) exp(-r^2 / (2 eps^2)), and  -k^2 <-> lap:
+ *     G_4(r) = G_2(r) - (eps^2 / 2) g(r)
+ *     G_6(r) = G_4(r) + (eps^4 / 8) lap g(r),   lap g = (r^2 / eps^4 - 3 / eps^2) g . */
+double orc_green_gauss(int order, double r, double eps)
+{
+    double G = orc_green_gauss2(r, eps);
+    if (order >= 4) {
+        double g = pow(2.0 * PI * eps * eps, -1.5) * exp(-r * r / (2.0 * eps * eps));
+        G -= 0.5 * eps * eps * g;
+        if (order >= 6) G += (r * r - 3.0 * eps * eps) / 8.0 * g;
+    }
+    return G;
+}
+
 /* half-spectrum geometry on the doubled grid: [P2][P1][N0+1] complex, x fastest */
 static i64 unb_spec_size(const i64 n[3]) { return (n[0] + 1) * (2 * n[1]) * (2 * n[2]); }
 i64 orc_unbounded_spec_size(const i64 n[3]) { return unb_spec_size(n); }
@@ -664,8 +684,15 @@ static int unb_backward_extract(const i64 n[3], cplx *spec, double *out)
 /* Green's spectrum: G on the doubled grid at mirrored distance d_a = min(i_a, P_a - i_a) h_a
  * (reading A12), times the cell volume, forward transformed once.
  * ghat: (n0+1) * 2 n1 * 2 n2 complex. */
+int orc_unbounded_green_order(const i64 n[3], const double h[3], double eps, int order, cplx *ghat);
 int orc_unbounded_green(const i64 n[3], const double h[3], double eps, cplx *ghat)
 {
+    return orc_unbounded_green_order(n, h, eps, 2, ghat);
+}
+/* the same with the kernel of order 2, 4 or 6 */
+int orc_unbounded_green_order(const i64 n[3], const double h[3], double eps, int order, cplx *ghat)
+{
+    if (order != 2 && order != 4 && order != 6) return ORC_ERR_ARG;
     for (int a = 0; a < 3; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
     i64 P0 = 2 * n[0], P1 = 2 * n[1], P2 = 2 * n[2];
     double *g = (double *)malloc(sizeof(double) * (size_t)(P0 * P1 * P2));
@@ -678,7 +705,7 @@ int orc_unbounded_green(const i64 n[3], const double h[3], double eps, cplx *gha
                 double dx = (double)(ix < P0 - ix ? ix : P0 - ix) * h[0];
                 double dy = (double)(iy < P1 - iy ? iy : P1 - iy) * h[1];
                 double dz = (double)(iz < P2 - iz ? iz : P2 - iz) * h[2];
-                g[ix + P0 * (iy + P1 * iz)] = vol * orc_green_gauss2(sqrt(dx * dx + dy * dy + dz * dz), eps);
+                g[ix + P0 * (iy + P1 * iz)] = vol * orc_green_gauss(order, sqrt(dx * dx + dy * dy + dz * dz), eps);
             }
     int err = unb_forward(n, g, 0, ghat);
     free(g);

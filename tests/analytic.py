@@ -78,3 +78,22 @@ def gaussian_blob_potential_gradient(g, eps, sign=-1.0):
 
 def rel_l2(a, b):
     return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+def gaussian_blob_potential_order(g, eps, order, sign=-1.0):
+    """pin for the kernels of order P = 2, 4, 6 (reading A25): in spectral space the blob
+    q exp(-sigma^2 k^2/2) times G^_P = -exp(-eps^2 k^2/2) sum_{n<P/2} (eps^2 k^2/2)^n / n! / k^2 is
+    -q exp(-s^2 k^2/2) [1/k^2 + eps^2/2 + eps^4 k^2/8], s^2 = sigma^2 + eps^2, hence
+        phi_P = -q erf(r/(sqrt2 s))/(4 pi r) - [P>=4] q (eps^2/2) g_s(r) + [P>=6] q (eps^4/8) lap g_s(r)
+    with g_s the unit Gaussian of width s and lap g_s = (r^2/s^4 - 3/s^2) g_s."""
+    x = g["x"]
+    out = gaussian_blob_potential(g, eps, sign)
+    for c, sig, q in zip(g["centres"], g["sigmas"], g["q"]):
+        s2 = sig ** 2 + eps ** 2
+        r2 = (x[:, None, None] - c[2]) ** 2 + (x[None, :, None] - c[1]) ** 2 + (x[None, None, :] - c[0]) ** 2
+        gs = (2 * np.pi * s2) ** -1.5 * np.exp(-r2 / (2 * s2))
+        if order >= 4:
+            out += sign * q * (eps ** 2 / 2) * gs
+        if order >= 6:
+            out -= sign * q * (eps ** 4 / 8) * (r2 / s2 ** 2 - 3 / s2) * gs
+    return out
