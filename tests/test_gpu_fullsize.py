@@ -122,3 +122,16 @@ def test_fast_path_zero_and_delta_sources():
         r = hh[0] * float(np.sqrt(sum((pt[a] - x0[a]) ** 2 for a in range(3))))
         want = hh[0] ** 3 * O.green_gauss2(r, eps)
         assert abs(got[pt] - want) <= 2e-5 * abs(want) + 1e-12, (pt, got[pt], want)
+
+
+def test_fast_path_order4_kernel():
+    """the order-4 kernel through the fast path (plan-time change only)"""
+    shape = (256, 256, 32)
+    f = rounded(W.Rng(4444).normal(int(np.prod(shape))).reshape(shape), "f32")
+    h = (1.0 / 256,) * 3
+    ref = O.unbounded_solve(f.astype(np.float64), h, O.unbounded_green((32, 256, 256), h, 2.0 * h[0], order=4))
+    with Plan(shape, h, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS4, prec="f32") as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI)
+    _check("psi order 4, 256x256x32 f32", got, ref, "f32")

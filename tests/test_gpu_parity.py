@@ -213,6 +213,26 @@ def test_cfg4_unbounded_noncubic_white_noise(shape):
     assert np.allclose(got.ravel()[idx], ref, rtol=1e-11, atol=1e-13 * np.abs(psi_o).max())
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("order,op", [(4, sf.SF_OP_GREEN_GAUSS4), (6, sf.SF_OP_GREEN_GAUSS6)])
+def test_cfg4_higher_order_kernels(prec, order, op):
+    """Hejlesen's Gaussian kernels of order 4 and 6 -- plan-time only, the
+    solve kernels are the same; vs the oracle and vs the closed form of a Gaussian charge."""
+    from analytic import gaussian_blob_potential_order
+    n = 64
+    g = W.gaussian_blobs(n, nblobs=1, sigma_h=(2.0, 2.0), inner=(0.45, 0.55))
+    f = rounded(g["f"], prec)
+    eps = 2.0 * g["h"][0]
+    psi_o = O.unbounded_solve(f.astype(np.float64), g["h"], O.unbounded_green(g["n"], g["h"], eps, order=order))
+    with Plan(f.shape, g["h"], sf.SF_BC_UNBOUNDED, op=op, prec=prec) as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI)
+    _report(f"psi order {order}", got, psi_o, prec)
+    e = rel_l2(got, gaussian_blob_potential_order(g, eps, order))
+    assert e <= (5e-6 if prec == "f32" else 1e-11), e
+
+
 # ------------------------------------------------------------------------------- config 5
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_cfg5_vortex_ring_curl(prec):
