@@ -178,7 +178,7 @@ def green_gauss2(r, eps):
 
 
 def green_gauss(order, r, eps):
-    """Gaussian-regularised kernel of order 2, 4 or 6 at distance r."""
+    """Gaussian-regularised kernel of order 2, 4, 6, 8 or 10 at distance r."""
     return float(lib().orc_green_gauss(int(order), float(r), float(eps)))
 
 

@@ -580,23 +580,24 @@ double orc_green_gauss2(double r, double eps)
     return -erf(r / (sqrt(2.0) * eps)) / (4.0 * PI * r);
 }
 
-/* Hejlesen's Gaussian kernels of order P = 2, 4, 6 ("Gaussian approximations of order
- * P = 2, 4, ... 10"; formulas not printed -- reading A25 of DESIGN.md).  In spectral space the
+/* Hejlesen's Gaussian kernels of order P = 2, 4, ... 10 ("Gaussian approximations of
+ * order P = 2, 4, ... 10"; formulas not printed -- reading A25 of DESIGN.md).  In spectral space the
  * order-P kernel is  G^_P(k) = -zeta^_P(eps k) / k^2  with
  *     zeta^_P(s) = exp(-s^2/2) * sum_{n < P/2} (s^2/2)^n / n! ,
  * i.e. the Gaussian times the Taylor polynomial that cancels its deviation from 1 up to s^(P-2).
- * Term n of the sum is  -(eps^2/2)^n / n! * k^(2n-2) exp(-eps^2 k^2 / 2); with g(r) the unit
- * Gaussian of width eps, (2 pi eps^2)^(-3/2) exp(-r^2 / (2 eps^2)), and  -k^2 <-> lap:
- *     G_4(r) = G_2(r) - (eps^2 / 2) g(r)
- *     G_6(r) = G_4(r) + (eps^4 / 8) lap g(r),   lap g = (r^2 / eps^4 - 3 / eps^2) g . */
+ * Term n >= 1 is  -(eps^2/2)^n / n! * k^(2n-2) exp(-eps^2 k^2 / 2)  <->  -(eps^2/2)^n / n! (-lap)^(n-1) g,
+ * g(r) = (2 pi eps^2)^(-3/2) exp(-r^2 / (2 eps^2)) the unit Gaussian of width eps, and in 3-D
+ *     lap^m g = (-1)^m 2^m m! / eps^(2m) * L_m^(1/2)(r^2 / (2 eps^2)) * g      (generalised Laguerre)
+ * so term n = -(eps^2 / (2 n)) L_(n-1)^(1/2)(x) g,  x = r^2 / (2 eps^2):
+ *     G_4 = G_2 - (eps^2/2) g,   G_6 = G_4 - (eps^2/4) L_1 g,   G_8 = G_6 - (eps^2/6) L_2 g,   G_10 = G_8 - (eps^2/8) L_3 g
+ *     L_1 = 3/2 - x,  L_2 = x^2/2 - 5x/2 + 15/8,  L_3 = -x^3/6 + 7x^2/4 - 35x/8 + 35/16 . */
 double orc_green_gauss(int order, double r, double eps)
 {
     double G = orc_green_gauss2(r, eps);
-    if (order >= 4) {
-        double g = pow(2.0 * PI * eps * eps, -1.5) * exp(-r * r / (2.0 * eps * eps));
-        G -= 0.5 * eps * eps * g;
-        if (order >= 6) G += (r * r - 3.0 * eps * eps) / 8.0 * g;
-    }
+    double x = r * r / (2.0 * eps * eps);
+    double g = pow(2.0 * PI * eps * eps, -1.5) * exp(-x);
+    double L[4] = { 1.0, 1.5 - x, x * x / 2.0 - 2.5 * x + 15.0 / 8.0, -x * x * x / 6.0 + 7.0 * x * x / 4.0 - 35.0 * x / 8.0 + 35.0 / 16.0 };
+    for (int n = 1; n < order / 2 && n <= 4; ++n) G -= eps * eps / (2.0 * n) * L[n - 1] * g;
     return G;
 }
 
@@ -689,10 +690,10 @@ int orc_unbounded_green(const i64 n[3], const double h[3], double eps, cplx *gha
 {
     return orc_unbounded_green_order(n, h, eps, 2, ghat);
 }
-/* the same with the kernel of order 2, 4 or 6 */
+/* the same with the kernel of order 2, 4, 6, 8 or 10 */
 int orc_unbounded_green_order(const i64 n[3], const double h[3], double eps, int order, cplx *ghat)
 {
-    if (order != 2 && order != 4 && order != 6) return ORC_ERR_ARG;
+    if (order < 2 || order > 10 || (order & 1)) return ORC_ERR_ARG;
     for (int a = 0; a < 3; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
     i64 P0 = 2 * n[0], P1 = 2 * n[1], P2 = 2 * n[2];
     double *g = (double *)malloc(sizeof(double) * (size_t)(P0 * P1 * P2));

@@ -1,5 +1,7 @@
 """Closed forms used to pin the oracle (and, through it, the CUDA path).  Pure mathematics of the
 test functions -- none of this is part of either implementation."""
+import math
+
 import numpy as np
 from scipy.special import erf
 
@@ -81,19 +83,30 @@ def rel_l2(a, b):
 
 
 def gaussian_blob_potential_order(g, eps, order, sign=-1.0):
-    """pin for the kernels of order P = 2, 4, 6 (reading A25): in spectral space the blob
+    """pin for the kernels of order P = 2 .. 10 (reading A25): in spectral space the blob
     q exp(-sigma^2 k^2/2) times G^_P = -exp(-eps^2 k^2/2) sum_{n<P/2} (eps^2 k^2/2)^n / n! / k^2 is
-    -q exp(-s^2 k^2/2) [1/k^2 + eps^2/2 + eps^4 k^2/8], s^2 = sigma^2 + eps^2, hence
-        phi_P = -q erf(r/(sqrt2 s))/(4 pi r) - [P>=4] q (eps^2/2) g_s(r) + [P>=6] q (eps^4/8) lap g_s(r)
-    with g_s the unit Gaussian of width s and lap g_s = (r^2/s^4 - 3/s^2) g_s."""
+    -q exp(-s^2 k^2/2) [1/k^2 + sum_{n>=1} (eps^2/2)^n/n! k^(2n-2)], s^2 = sigma^2 + eps^2, hence
+        phi_P = -q erf(r/(sqrt2 s))/(4 pi r) - q sum_{n=1}^{P/2-1} (eps^2/2)^n/n! (-lap)^(n-1) g_s(r)
+    with g_s the unit Gaussian of width s; lap^m g_s is taken here by repeated application of the
+    radial Laplacian f'' + 2 f'/r to the polynomial prefactor (sympy-free, exact polynomial algebra)."""
+    from numpy.polynomial import polynomial as P
     x = g["x"]
     out = gaussian_blob_potential(g, eps, sign)
     for c, sig, q in zip(g["centres"], g["sigmas"], g["q"]):
         s2 = sig ** 2 + eps ** 2
         r2 = (x[:, None, None] - c[2]) ** 2 + (x[None, :, None] - c[1]) ** 2 + (x[None, None, :] - c[0]) ** 2
         gs = (2 * np.pi * s2) ** -1.5 * np.exp(-r2 / (2 * s2))
-        if order >= 4:
-            out += sign * q * (eps ** 2 / 2) * gs
-        if order >= 6:
-            out -= sign * q * (eps ** 4 / 8) * (r2 / s2 ** 2 - 3 / s2) * gs
+        # f = p(t) exp(-t/(2 s2)) with t = r^2:  lap f = [4 t p'' + (6 - 4 t/(2 s2)... ] -- derived below
+        # d/dr = 2 r d/dt;  f'' + 2 f'/r = 4 t f_tt + 6 f_t  (f_t = d f/dt), and with f = p e^{-a t}, a = 1/(2 s2):
+        #   f_t = (p' - a p) e,  f_tt = (p'' - 2 a p' + a^2 p) e
+        a = 1.0 / (2 * s2)
+        p = np.array([1.0])          # polynomial in t, lowest degree first
+        for n in range(1, order // 2):
+            # term n uses (-lap)^(n-1) g_s
+            out += sign * q * (eps ** 2 / 2) ** n / math.factorial(n) * P.polyval(r2, p) * gs
+            d1, d2 = P.polyder(p), P.polyder(p, 2)
+            ft = P.polysub(d1, a * p)
+            ftt = P.polyadd(P.polysub(d2, 2 * a * d1), a * a * p)
+            lap = P.polyadd(P.polymul([0.0, 4.0], ftt), 6.0 * ft)
+            p = -lap                 # next power of (-lap)
     return out
