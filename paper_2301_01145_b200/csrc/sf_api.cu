@@ -211,8 +211,8 @@ void axis_tables(const sf_plan_s& pl, int a, int count, std::vector<long double>
 // ---------------------------------------------------------------- plan-time kernels (fp64)
 // G on the doubled grid at the mirrored distance min(i, P - i) h (reading A12), times
 // the cell volume (reading A11).  Kernel: 2nd-order Gaussian regularisation (reading A10).
-// order 4 and 6 (reading A25): G_4 = G_2 - (eps^2/2) g, G_6 = G_4 + ((r^2 - 3 eps^2)/8) g,
-// g the unit Gaussian of width eps.
+// orders 4 .. 10 (reading A25): G_P = G_2 - sum_{n=1}^{P/2-1} eps^2/(2n) L_{n-1}^(1/2)(x) g,
+// x = r^2 / (2 eps^2), g the unit Gaussian of width eps.
 __global__ void green_eval_kernel(double* g, int Px, int Py, int Pz, double hx, double hy, double hz, double eps, double vol, int order)
 {
     const long long tot = (long long)Px * Py * Pz;
@@ -224,9 +224,13 @@ __global__ void green_eval_kernel(double* g, int Px, int Py, int Pz, double hx, 
         if (r == 0.0) v = -1.0 / (15.749609945722419 * eps); // (2 pi)^(3/2)
         else v = -erf(r * 0.70710678118654752440 / eps) / (12.566370614359172954 * r);
         if (order >= 4) {
-            const double gs = exp(-r * r / (2.0 * eps * eps)) / (15.749609945722419 * eps * eps * eps);
-            v -= 0.5 * eps * eps * gs;
-            if (order >= 6) v += (r * r - 3.0 * eps * eps) * 0.125 * gs;
+            const double x = r * r / (2.0 * eps * eps);
+            const double gs = exp(-x) / (15.749609945722419 * eps * eps * eps);
+            double poly = 0.5;                                                                       // n = 1: L_0 / 2
+            if (order >= 6) poly += (1.5 - x) * 0.25;                                                // n = 2: L_1 / 4
+            if (order >= 8) poly += ((0.5 * x - 2.5) * x + 1.875) / 6.0;                             // n = 3: L_2 / 6
+            if (order >= 10) poly += (((-x / 6.0 + 1.75) * x - 4.375) * x + 2.1875) * 0.125;         // n = 4: L_3 / 8
+            v -= eps * eps * poly * gs;
         }
         g[i] = vol * v;
     }
@@ -271,7 +275,7 @@ template <typename T> sf_status build_green(sf_plan p)
     if ((st = upload_twiddles<double>(p, &twz, Pz)) != SF_OK) return st;
     const double eps = p->eps_over_h * fmax(p->h[0], fmax(p->h[1], p->h[2]));
     const double vol = p->h[0] * p->h[1] * p->h[2];
-    const int order = (p->op == SF_OP_GREEN_GAUSS6) ? 6 : (p->op == SF_OP_GREEN_GAUSS4 ? 4 : 2);
+    const int order = 2 * ((int)p->op - (int)SF_OP_GREEN_GAUSS2 + 1);
     green_eval_kernel<<<148 * 8, 256, 0, p->stream>>>(g, Px, Py, Pz, p->h[0], p->h[1], p->h[2], eps, vol, order);
     SF_CUDA(p, cudaGetLastError());
 
@@ -532,8 +536,8 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
     if (ndim != 2 && ndim != 3) return fail(nullptr, ndim == 1 ? SF_ERR_UNSUPPORTED : SF_ERR_INVALID_ARG, "ndim must be 2 or 3");
     if (prec != SF_F32 && prec != SF_F64) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown precision");
     if (grid != SF_GRID_CELL_BOUNDARY && grid != SF_GRID_CELL_CENTRE) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown grid type");
-    if (op < SF_OP_PSEUDO_SPECTRAL || op > SF_OP_GREEN_GAUSS6) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown operator");
-    const bool green_op = (op == SF_OP_GREEN_GAUSS2 || op == SF_OP_GREEN_GAUSS4 || op == SF_OP_GREEN_GAUSS6);
+    if (op < SF_OP_PSEUDO_SPECTRAL || op > SF_OP_GREEN_GAUSS10) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown operator");
+    const bool green_op = (op >= SF_OP_GREEN_GAUSS2 && op <= SF_OP_GREEN_GAUSS10);
     for (int a = 0; a < ndim; ++a) {
         if (bc[a] < SF_BC_PERIODIC || bc[a] > SF_BC_UNBOUNDED) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown boundary condition");
         if (n[a] <= 0) return fail(nullptr, SF_ERR_INVALID_ARG, "sizes must be positive");

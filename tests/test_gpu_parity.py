@@ -214,9 +214,10 @@ def test_cfg4_unbounded_noncubic_white_noise(shape):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("order,op", [(4, sf.SF_OP_GREEN_GAUSS4), (6, sf.SF_OP_GREEN_GAUSS6)])
+@pytest.mark.parametrize("order,op", [(4, sf.SF_OP_GREEN_GAUSS4), (6, sf.SF_OP_GREEN_GAUSS6), (8, sf.SF_OP_GREEN_GAUSS8),
+                                      (10, sf.SF_OP_GREEN_GAUSS10)])
 def test_cfg4_higher_order_kernels(prec, order, op):
-    """Hejlesen's Gaussian kernels of order 4 and 6 -- plan-time only, the
+    """Hejlesen's Gaussian kernels of order 4 .. 10 -- plan-time only, the
     solve kernels are the same; vs the oracle and vs the closed form of a Gaussian charge."""
     from analytic import gaussian_blob_potential_order
     n = 64
