@@ -174,3 +174,19 @@ def test_kernel_order_is_the_order_of_accuracy():
         e2 = np.abs(gaussian_blob_potential_order(g, 0.01, order) - exact).max()
         rate = np.log2(e1 / e2)
         assert abs(rate - order) < 0.35, (order, rate)   # pre-asymptotic at eps/sigma = 1/4 .. 1/8
+
+
+@pytest.mark.parametrize("order", [2, 4, 6, 8, 10])
+def test_kernel_is_the_inverse_transform_of_its_spectrum(order):
+    """reading A25 defines the kernels in spectral space, G^_P(k) = -exp(-s^2/2) sum_{n<P/2} (s^2/2)^n/n! / k^2,
+    s = eps k; the oracle evaluates real-space closed forms.  Tie the two by quadrature of the radial
+    inverse transform  G(r) = 1/(2 pi^2 r) int_0^inf G^(k) k sin(k r) dk  (integrand smooth, Gaussian tail)."""
+    import math
+    eps = 0.3
+    k = np.linspace(0.0, 60.0 / eps, 2_400_001)[1:]          # s up to 60: exp(-1800) tail
+    s2 = (eps * k) ** 2 / 2
+    zeta = np.exp(-s2) * sum(s2 ** n / math.factorial(n) for n in range(order // 2))
+    for r in (0.05, 0.3, 0.9, 2.5):
+        integrand = -zeta * np.sin(k * r) / k
+        val = np.trapezoid(np.concatenate(([-r], integrand)), np.concatenate(([0.0], k))) / (2 * np.pi ** 2 * r)
+        assert abs(val - O.green_gauss(order, r, eps)) <= 2e-9 * abs(val), (order, r, val)
