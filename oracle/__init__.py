@@ -43,6 +43,10 @@ def lib() -> C.CDLL:
         L.orc_num_threads.restype = C.c_int
         L.orc_green_gauss2.restype = C.c_double
         L.orc_green_gauss2.argtypes = [C.c_double, C.c_double]
+        L.orc_sine_integral.restype = C.c_double
+        L.orc_sine_integral.argtypes = [C.c_double]
+        L.orc_green_spectral.restype = C.c_double
+        L.orc_green_spectral.argtypes = [C.c_double, C.c_double]
         L.orc_green_gauss.restype = C.c_double
         L.orc_green_gauss.argtypes = [C.c_int, C.c_double, C.c_double]
         L.orc_unbounded_spec_size.restype = C.c_longlong
@@ -182,8 +186,18 @@ def green_gauss(order, r, eps):
     return float(lib().orc_green_gauss(int(order), float(r), float(eps)))
 
 
+def sine_integral(x):
+    return float(lib().orc_sine_integral(float(x)))
+
+
+def green_spectral(r, h):
+    """Hejlesen's spectrally compact kernel -Si(pi r/h)/(2 pi^2 r) at distance r."""
+    return float(lib().orc_green_spectral(float(r), float(h)))
+
+
 def unbounded_green(n_xyz, h, eps, order=2):
-    """Green's spectrum on the doubled grid: complex array [2 nz, 2 ny, nx + 1]."""
+    """Green's spectrum on the doubled grid: complex array [2 nz, 2 ny, nx + 1].
+    order = 2 .. 10: Gaussian kernels of width eps; order = 0: spectrally compact kernel, eps = max(h)."""
     n = [int(v) for v in n_xyz]
     ghat = np.empty((2 * n[2], 2 * n[1], n[0] + 1), dtype=np.complex128)
     _chk(lib().orc_unbounded_green_order(_i64x3(n), _f64x3(h), C.c_double(eps), C.c_int(order), _ptr(ghat)),

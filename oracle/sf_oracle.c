@@ -601,6 +601,46 @@ double orc_green_gauss(int order, double r, double eps)
     return G;
 }
 
+/* Sine integral Si(x) = int_0^x sin(t)/t dt, x >= 0: Maclaurin series sum (-1)^n x^(2n+1)/((2n+1)(2n+1)!)
+ * for x < 3, else from the exponential integral, E1(i x) = -Ci(x) + i (Si(x) - pi/2), with E1 by its
+ * continued fraction e^(-z) / (z + 1 - 1^2/(z + 3 - 2^2/(z + 5 - ...))) (modified Lentz). */
+double orc_sine_integral(double x)
+{
+    if (x < 3.0) {
+        double term = x, sum = x, x2 = x * x;
+        for (int n = 1; n < 40; ++n) {
+            term *= -x2 / ((2.0 * n) * (2.0 * n + 1.0));
+            double add = term / (2.0 * n + 1.0);
+            sum += add;
+            if (fabs(add) < 1e-18 * fabs(sum)) break;
+        }
+        return sum;
+    }
+    double complex z = I * x;
+    double complex b = z + 1.0, c = 1e300, d = 1.0 / b, hh = d;
+    for (int i = 1; i < 500; ++i) {
+        double a = -(double)i * (double)i;
+        b += 2.0;
+        d = 1.0 / (a * d + b);
+        c = b + a / c;
+        double complex del = c * d;
+        hh *= del;
+        if (cabs(del - 1.0) < 1e-16) break;
+    }
+    double complex e1 = hh * cexp(-z);
+    return PI / 2.0 + cimag(e1);   /* E1(ix) = -Ci(x) + i (Si(x) - pi/2)  =>  Si = pi/2 + Im E1(ix) */
+}
+
+/* Hejlesen's spectrally compact kernel, 3-D ("spectrally compact kernel which achieves
+ * spectral accuracy"; formula not printed -- reading A26): the singular spectrum -1/k^2 kept inside the
+ * ball |k| <= pi/h that the grid resolves and dropped outside; its radial inverse transform is
+ *     G(r) = -1/(2 pi^2 r) int_0^(pi/h) sin(k r)/k dk = -Si(pi r / h) / (2 pi^2 r),   G(0) = -1/(2 pi h). */
+double orc_green_spectral(double r, double h)
+{
+    if (r == 0.0) return -1.0 / (2.0 * PI * h);
+    return -orc_sine_integral(PI * r / h) / (2.0 * PI * PI * r);
+}
+
 /* half-spectrum geometry on the doubled grid: [P2][P1][N0+1] complex, x fastest */
 static i64 unb_spec_size(const i64 n[3]) { return (n[0] + 1) * (2 * n[1]) * (2 * n[2]); }
 i64 orc_unbounded_spec_size(const i64 n[3]) { return unb_spec_size(n); }
@@ -693,7 +733,7 @@ int orc_unbounded_green(const i64 n[3], const double h[3], double eps, cplx *gha
 /* the same with the kernel of order 2, 4, 6, 8 or 10 */
 int orc_unbounded_green_order(const i64 n[3], const double h[3], double eps, int order, cplx *ghat)
 {
-    if (order < 2 || order > 10 || (order & 1)) return ORC_ERR_ARG;
+    if (order != 0 && (order < 2 || order > 10 || (order & 1))) return ORC_ERR_ARG;   /* 0: spectrally compact kernel, eps = h */
     for (int a = 0; a < 3; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
     i64 P0 = 2 * n[0], P1 = 2 * n[1], P2 = 2 * n[2];
     double *g = (double *)malloc(sizeof(double) * (size_t)(P0 * P1 * P2));
@@ -706,7 +746,8 @@ int orc_unbounded_green_order(const i64 n[3], const double h[3], double eps, int
                 double dx = (double)(ix < P0 - ix ? ix : P0 - ix) * h[0];
                 double dy = (double)(iy < P1 - iy ? iy : P1 - iy) * h[1];
                 double dz = (double)(iz < P2 - iz ? iz : P2 - iz) * h[2];
-                g[ix + P0 * (iy + P1 * iz)] = vol * orc_green_gauss(order, sqrt(dx * dx + dy * dy + dz * dz), eps);
+                double rr = sqrt(dx * dx + dy * dy + dz * dz);
+                g[ix + P0 * (iy + P1 * iz)] = vol * (order ? orc_green_gauss(order, rr, eps) : orc_green_spectral(rr, eps));
             }
     int err = unb_forward(n, g, 0, ghat);
     free(g);

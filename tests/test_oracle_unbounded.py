@@ -190,3 +190,39 @@ def test_kernel_is_the_inverse_transform_of_its_spectrum(order):
         integrand = -zeta * np.sin(k * r) / k
         val = np.trapezoid(np.concatenate(([-r], integrand)), np.concatenate(([0.0], k))) / (2 * np.pi ** 2 * r)
         assert abs(val - O.green_gauss(order, r, eps)) <= 2e-9 * abs(val), (order, r, val)
+
+
+# ---------------------------------------------------------------------------- spectrally compact kernel
+def test_sine_integral_against_library_and_series():
+    """Si(x): scipy.special.sici as a third opinion, across the series / continued-fraction switch at 3,
+    up to the largest argument a 512^3 doubled grid produces (pi sqrt(3) 1024 ~ 5600); Si(inf) = pi/2."""
+    from scipy.special import sici
+    for x in (0.0, 1e-8, 0.5, 2.999999, 3.0, 3.000001, 7.0, 31.4, 1000.0, 5600.0):
+        assert abs(O.sine_integral(x) - sici(x)[0]) <= 4e-16 * max(1.0, sici(x)[0])
+    assert abs(O.sine_integral(1e7) - np.pi / 2) < 2e-7
+
+
+def test_spectral_kernel_is_the_truncated_inverse_transform():
+    """reading A26: G(r) = 1/(2 pi^2 r) int_0^(pi/h) (-1/k^2) k sin(k r) dk, by quadrature; G(0) is its limit."""
+    h = 0.25
+    k = np.linspace(0.0, np.pi / h, 2_000_001)[1:]
+    for r in (0.01, 0.3, 1.0, 7.7):
+        integrand = -np.sin(k * r) / k
+        val = np.trapezoid(np.concatenate(([-r], integrand)), np.concatenate(([0.0], k))) / (2 * np.pi ** 2 * r)
+        assert abs(val - O.green_spectral(r, h)) <= 1e-9 * abs(val)
+    assert np.isclose(O.green_spectral(0.0, h), O.green_spectral(1e-7, h), rtol=1e-10)
+    assert np.isclose(O.green_spectral(0.0, h), -1.0 / (2 * np.pi * h), rtol=1e-15)
+
+
+def test_spectral_kernel_is_spectrally_accurate():
+    """the spectrally compact kernel reproduces the free-space solution of a
+    well-resolved smooth charge to rounding level, where every Gaussian order stops at eps^P:
+    Gaussian blob, sigma = 3 h, compared with the singular-kernel potential -q erf(r/(sqrt2 sigma))/(4 pi r)."""
+    g = W.gaussian_blobs(64, nblobs=1, sigma_h=(3.0, 3.0), inner=(0.47, 0.53))
+    exact = gaussian_blob_potential(g, 0.0)
+    h = g["h"][0]
+    psi = O.unbounded_solve(g["f"], g["h"], O.unbounded_green(g["n"], g["h"], h, order=0))
+    e_spec = rel_l2(psi, exact)
+    e10 = rel_l2(O.unbounded_solve(g["f"], g["h"], O.unbounded_green(g["n"], g["h"], 2 * h, order=10)), exact)
+    print(f"spectral kernel {e_spec:.2e}, order 10 {e10:.2e}")
+    assert e_spec < 1e-9 and e_spec < e10
