@@ -64,7 +64,9 @@ typedef enum {
     SF_OP_GREEN_GAUSS4 = 3,    /* orders 4 .. 10 of the same family: with g the unit Gaussian */
     SF_OP_GREEN_GAUSS6 = 4,    /* of width eps, x = r^2/(2 eps^2) and L_m the generalised Laguerre           */
     SF_OP_GREEN_GAUSS8 = 5,    /* polynomials L_m^(1/2):  G_P = G_2 - sum_{n=1}^{P/2-1} eps^2/(2n) L_{n-1}(x) g */
-    SF_OP_GREEN_GAUSS10 = 6    /* (spectrum -exp(-s^2/2) sum_{n<P/2} (s^2/2)^n/n! / k^2, s = eps k)           */
+    SF_OP_GREEN_GAUSS10 = 6,   /* (spectrum -exp(-s^2/2) sum_{n<P/2} (s^2/2)^n/n! / k^2, s = eps k)           */
+    SF_OP_GREEN_SPECTRAL = 7   /* spectrally compact kernel: -1/k^2 inside |k| <= pi/h,        */
+                               /* G(r) = -Si(pi r/h) / (2 pi^2 r), h = max spacing; eps_over_h is ignored     */
 } sf_operator;
 
 typedef enum { SF_F32 = 0, SF_F64 = 1 } sf_precision;
@@ -100,7 +102,7 @@ typedef struct {
  *   grid   Dirichlet requires SF_GRID_CELL_BOUNDARY, Neumann SF_GRID_CELL_CENTRE (the other two
  *          Table-1 rows are not built yet: SF_ERR_UNSUPPORTED); periodic and unbounded accept both
  *          (identical numerics).
- *   op     PS / FD2 for periodic, Dirichlet, Neumann; GREEN_GAUSS2 .. GREEN_GAUSS10 for unbounded (3-D only).
+ *   op     PS / FD2 for periodic, Dirichlet, Neumann; GREEN_GAUSS2 .. GREEN_GAUSS10 or GREEN_SPECTRAL for unbounded (3-D only).
  *   prec   arithmetic and storage type of every array passed later.
  *   opt    [host] may be NULL (defaults above).
  * For unbounded plans this call evaluates G on the doubled grid, transforms it with the library's

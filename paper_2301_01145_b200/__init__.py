@@ -21,7 +21,7 @@ SF_OK, SF_ERR_INVALID_ARG, SF_ERR_UNSUPPORTED, SF_ERR_ALLOC, SF_ERR_CUDA, SF_ERR
 SF_BC_PERIODIC, SF_BC_DIRICHLET, SF_BC_NEUMANN, SF_BC_UNBOUNDED = 0, 1, 2, 3
 SF_GRID_CELL_BOUNDARY, SF_GRID_CELL_CENTRE = 0, 1
 SF_OP_PSEUDO_SPECTRAL, SF_OP_FD2, SF_OP_GREEN_GAUSS2, SF_OP_GREEN_GAUSS4, SF_OP_GREEN_GAUSS6 = 0, 1, 2, 3, 4
-SF_OP_GREEN_GAUSS8, SF_OP_GREEN_GAUSS10 = 5, 6
+SF_OP_GREEN_GAUSS8, SF_OP_GREEN_GAUSS10, SF_OP_GREEN_SPECTRAL = 5, 6, 7
 SF_F32, SF_F64 = 0, 1
 SF_MEM_HOST, SF_MEM_DEVICE = 0, 1
 SF_OUT_PSI, SF_OUT_GRAD, SF_OUT_CURL = 0, 1, 2

@@ -213,6 +213,46 @@ void axis_tables(const sf_plan_s& pl, int a, int count, std::vector<long double>
 // the cell volume (reading A11).  Kernel: 2nd-order Gaussian regularisation (reading A10).
 // orders 4 .. 10 (reading A25): G_P = G_2 - sum_{n=1}^{P/2-1} eps^2/(2n) L_{n-1}^(1/2)(x) g,
 // x = r^2 / (2 eps^2), g the unit Gaussian of width eps.
+// order 0: the spectrally compact kernel -Si(pi r / h) / (2 pi^2 r), h passed in `eps` (reading A26).
+// Si: power series below 3, above it pi/2 + Im E1(i x) with E1 by its continued fraction (modified Lentz),
+// complex arithmetic written out.
+__device__ double sine_integral(double x)
+{
+    if (x < 3.0) {
+        double term = x, sum = x;
+        const double x2 = x * x;
+        for (int n = 1; n < 40; ++n) {
+            term *= -x2 / ((2.0 * n) * (2.0 * n + 1.0));
+            sum += term / (2.0 * n + 1.0);
+        }
+        return sum;
+    }
+    // z = i x;  b = z + 1;  c = huge;  d = 1/b;  h = d
+    double br = 1.0, bi = x, cr = 1e300, ci = 0.0;
+    double den = br * br + bi * bi;
+    double dr = br / den, di = -bi / den, hr = dr, hi = di;
+    for (int i = 1; i < 500; ++i) {
+        const double a = -(double)i * (double)i;
+        br += 2.0;
+        // d = 1 / (a d + b)
+        double tr = a * dr + br, ti = a * di + bi;
+        den = tr * tr + ti * ti;
+        dr = tr / den; di = -ti / den;
+        // c = b + a / c
+        den = cr * cr + ci * ci;
+        tr = br + a * cr / den; ti = bi - a * ci / den;
+        cr = tr; ci = ti;
+        // del = c d;  h *= del
+        const double er = cr * dr - ci * di, ei = cr * di + ci * dr;
+        tr = hr * er - hi * ei; ti = hr * ei + hi * er;
+        hr = tr; hi = ti;
+        if (fabs(er - 1.0) + fabs(ei) < 1e-16) break;
+    }
+    // E1(i x) = h exp(-i x);  Si = pi/2 + Im E1
+    double sn, cs;
+    sincos(x, &sn, &cs);
+    return 1.5707963267948966192 + (hi * cs - hr * sn);
+}
 __global__ void green_eval_kernel(double* g, int Px, int Py, int Pz, double hx, double hy, double hz, double eps, double vol, int order)
 {
     const long long tot = (long long)Px * Py * Pz;
@@ -221,7 +261,8 @@ __global__ void green_eval_kernel(double* g, int Px, int Py, int Pz, double hx, 
         const double dx = (double)min(ix, Px - ix) * hx, dy = (double)min(iy, Py - iy) * hy, dz = (double)min(iz, Pz - iz) * hz;
         const double r = sqrt(dx * dx + dy * dy + dz * dz);
         double v;
-        if (r == 0.0) v = -1.0 / (15.749609945722419 * eps); // (2 pi)^(3/2)
+        if (order == 0) v = (r == 0.0) ? -1.0 / (6.2831853071795864769 * eps) : -sine_integral(3.14159265358979323846 * r / eps) / (19.739208802178717238 * r);
+        else if (r == 0.0) v = -1.0 / (15.749609945722419 * eps); // (2 pi)^(3/2)
         else v = -erf(r * 0.70710678118654752440 / eps) / (12.566370614359172954 * r);
         if (order >= 4) {
             const double x = r * r / (2.0 * eps * eps);
@@ -273,9 +314,9 @@ template <typename T> sf_status build_green(sf_plan p)
     if ((st = upload_twiddles<double>(p, &twx, Px)) != SF_OK) return st;
     if ((st = upload_twiddles<double>(p, &twy, Py)) != SF_OK) return st;
     if ((st = upload_twiddles<double>(p, &twz, Pz)) != SF_OK) return st;
-    const double eps = p->eps_over_h * fmax(p->h[0], fmax(p->h[1], p->h[2]));
+    const double eps = (p->op == SF_OP_GREEN_SPECTRAL ? 1.0 : p->eps_over_h) * fmax(p->h[0], fmax(p->h[1], p->h[2]));
     const double vol = p->h[0] * p->h[1] * p->h[2];
-    const int order = 2 * ((int)p->op - (int)SF_OP_GREEN_GAUSS2 + 1);
+    const int order = (p->op == SF_OP_GREEN_SPECTRAL) ? 0 : 2 * ((int)p->op - (int)SF_OP_GREEN_GAUSS2 + 1);
     green_eval_kernel<<<148 * 8, 256, 0, p->stream>>>(g, Px, Py, Pz, p->h[0], p->h[1], p->h[2], eps, vol, order);
     SF_CUDA(p, cudaGetLastError());
 
@@ -536,8 +577,8 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
     if (ndim != 2 && ndim != 3) return fail(nullptr, ndim == 1 ? SF_ERR_UNSUPPORTED : SF_ERR_INVALID_ARG, "ndim must be 2 or 3");
     if (prec != SF_F32 && prec != SF_F64) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown precision");
     if (grid != SF_GRID_CELL_BOUNDARY && grid != SF_GRID_CELL_CENTRE) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown grid type");
-    if (op < SF_OP_PSEUDO_SPECTRAL || op > SF_OP_GREEN_GAUSS10) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown operator");
-    const bool green_op = (op >= SF_OP_GREEN_GAUSS2 && op <= SF_OP_GREEN_GAUSS10);
+    if (op < SF_OP_PSEUDO_SPECTRAL || op > SF_OP_GREEN_SPECTRAL) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown operator");
+    const bool green_op = (op >= SF_OP_GREEN_GAUSS2 && op <= SF_OP_GREEN_SPECTRAL);
     for (int a = 0; a < ndim; ++a) {
         if (bc[a] < SF_BC_PERIODIC || bc[a] > SF_BC_UNBOUNDED) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown boundary condition");
         if (n[a] <= 0) return fail(nullptr, SF_ERR_INVALID_ARG, "sizes must be positive");

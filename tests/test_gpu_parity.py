@@ -234,6 +234,30 @@ def test_cfg4_higher_order_kernels(prec, order, op):
     assert e <= (5e-6 if prec == "f32" else 1e-11), e
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_cfg4_spectrally_compact_kernel(prec):
+    """Hejlesen's spectrally compact kernel -- vs the oracle on white noise
+    (anisotropic spacing: h = max spacing, reading A26) and vs the free-space potential of a resolved
+    Gaussian charge, which it reproduces to rounding."""
+    from analytic import gaussian_blob_potential
+    shape = (16, 32, 64)
+    f = rounded(_rand(shape, 77), prec)
+    hs = (0.11, 0.07, 0.13)
+    psi_o = O.unbounded_solve(f.astype(np.float64), hs, O.unbounded_green((64, 32, 16), hs, max(hs), order=0))
+    with Plan(shape, hs, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_SPECTRAL, prec=prec, eps_over_h=123.0) as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        _report("psi spectral kernel, white noise", p.get(sf.SF_OUT_PSI), psi_o, prec)
+    g = W.gaussian_blobs(64, nblobs=1, sigma_h=(3.0, 3.0), inner=(0.47, 0.53))
+    f = rounded(g["f"], prec)
+    with Plan(f.shape, g["h"], sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_SPECTRAL, prec=prec) as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        e = rel_l2(p.get(sf.SF_OUT_PSI), gaussian_blob_potential(g, 0.0))
+    print(f"spectral kernel vs free-space potential: rel-L2 {e:.3e}")
+    assert e <= (5e-6 if prec == "f32" else 1e-11)
+
+
 # ------------------------------------------------------------------------------- config 5
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_cfg5_vortex_ring_curl(prec):
