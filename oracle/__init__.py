@@ -220,6 +220,20 @@ def unbounded_solve(f, h, ghat, rhs_sign=1.0, want_curl=False):
     return out
 
 
+def unbounded_gradient(f, h, ghat, rhs_sign=1.0):
+    """scalar unbounded solve with spectral gradient: returns psi[z, y, x], grad[3, z, y, x] (d/dx, d/dy, d/dz)."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    assert nd == 3
+    psi = np.empty_like(f)
+    grad = np.empty((3,) + f.shape)
+    ghat = np.ascontiguousarray(ghat, dtype=np.complex128)
+    assert ghat.shape == (2 * n[2], 2 * n[1], n[0] + 1)
+    _chk(lib().orc_unbounded_gradient(_i64x3(n), _f64x3(h), _ptr(ghat), C.c_double(rhs_sign), _ptr(f), _ptr(psi),
+                                      _ptr(grad)), "unbounded_gradient")
+    return psi, grad
+
+
 def unbounded_direct(f, h, eps, rhs_sign=1.0):
     """Direct O(N^6) sum of the definition -- tiny grids only."""
     f = _f64(f)

@@ -812,6 +812,43 @@ done:
     return err;
 }
 
+/* Scalar solve with spectral gradient (eq. (10)): psi as above and
+ * g_a = IDFT(i kappa_a psi_hat) extracted on the first octant, kappa on the DOUBLED grid as for the
+ * curl (kappa_a = 2 pi m_a / (P_a h_a), Nyquist -> 0; reading A20).  grad: 3 fields (d/dx, d/dy, d/dz). */
+int orc_unbounded_gradient(const i64 n[3], const double h[3], const cplx *ghat, double rhs_sign, const double *f,
+                           double *psi, double *grad)
+{
+    for (int a = 0; a < 3; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
+    i64 tot = n[0] * n[1] * n[2], ns = unb_spec_size(n);
+    i64 P[3] = { 2 * n[0], 2 * n[1], 2 * n[2] }, H0 = n[0] + 1;
+    int err = ORC_OK;
+    cplx *spec = (cplx *)malloc(sizeof(cplx) * (size_t)ns), *work = (cplx *)malloc(sizeof(cplx) * (size_t)ns);
+    double *kap = (double *)malloc(sizeof(double) * (size_t)(P[0] > P[1] ? (P[0] > P[2] ? P[0] : P[2]) : (P[1] > P[2] ? P[1] : P[2])));
+    if (!spec || !work || !kap) { err = ORC_ERR_ALLOC; goto done; }
+    if ((err = unb_forward(n, f, 1, spec)) != ORC_OK) goto done;
+#pragma omp parallel for schedule(static)
+    for (i64 i = 0; i < ns; ++i) spec[i] = rhs_sign * ghat[i] * spec[i];
+    for (int a = 0; a < 3; ++a) {
+        for (i64 k = 0; k < P[a]; ++k) {
+            i64 m = (k < n[a]) ? k : k - P[a];
+            kap[k] = (k == n[a]) ? 0.0 : 2.0 * PI * (double)m / ((double)P[a] * h[a]);
+        }
+#pragma omp parallel for collapse(2) schedule(static)
+        for (i64 kz = 0; kz < P[2]; ++kz)
+            for (i64 ky = 0; ky < P[1]; ++ky)
+                for (i64 kx = 0; kx < H0; ++kx) {
+                    i64 i = kx + H0 * (ky + P[1] * kz);
+                    i64 kk[3] = { kx, ky, kz };
+                    work[i] = I * kap[kk[a]] * spec[i];
+                }
+        if ((err = unb_backward_extract(n, work, grad + (size_t)a * (size_t)tot)) != ORC_OK) goto done;
+    }
+    err = unb_backward_extract(n, spec, psi);   /* last: the backward transform works in place */
+done:
+    free(spec); free(work); free(kap);
+    return err;
+}
+
 /* Direct O(N^6) evaluation of the definition above (scalar), for tiny grids only (pin P6). */
 void orc_unbounded_direct(const i64 n[3], const double h[3], double eps, double rhs_sign, const double *f,
                           double *psi)
