@@ -143,8 +143,10 @@ sf_status sf_set_bc_values(sf_plan plan, int axis, int side, const void* face, s
 sf_status sf_solve(sf_plan plan);
 
 /* sf_gradient -- as sf_solve, and additionally d psi / d x_a = IDFT(i k_a psi_hat) for every axis
- * from the same spectrum (eq. 10).  Scalar periodic plans only (UNSUPPORTED otherwise);
- * the wavenumber at the Nyquist index is taken as zero. */
+ * from the same spectrum (eq. 10).  Scalar periodic and unbounded plans (UNSUPPORTED
+ * otherwise); on unbounded plans k_a are the wavenumbers of the doubled grid, as for sf_curl, and the
+ * first call allocates a four-field set of work arrays (ALLOC on failure).  The wavenumber at the
+ * Nyquist index is taken as zero. */
 sf_status sf_gradient(sf_plan plan);
 
 /* sf_curl -- ncomp == 3 plans: solve the three components and return u = curl psi = IDFT(i k x

@@ -12,6 +12,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 using namespace sf;
@@ -61,6 +62,10 @@ struct sf_plan_s {
     void* W1 = nullptr;
     void* W2 = nullptr;
     void* out = nullptr;       // nfields dense real fields
+    // scalar unbounded plans: a second, four-field set of work / output arrays, allocated by the first
+    // sf_gradient (the solve path keeps its single-field arrays and their tensor maps)
+    void *gW1 = nullptr, *gW2 = nullptr, *gout = nullptr;
+    void* out_last = nullptr;  // array the last compute call wrote its fields to
     void* tw[3] = { nullptr, nullptr, nullptr };
     void* ptw[3] = { nullptr, nullptr, nullptr };
     void* lam[3] = { nullptr, nullptr, nullptr };
@@ -477,6 +482,8 @@ template <typename T> sf_status run(sf_plan p, int outk)
         mark(5);
         if (p->tslots) p->tcount++;
         p->last_kind = outk;
+    p->out_last = p->out;
+        p->out_last = p->out;
         return SF_OK;
     }
 
@@ -538,6 +545,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
     mark(5);
     if (p->tslots) p->tcount++;
     p->last_kind = outk;
+    p->out_last = p->out;
     return SF_OK;
 }
 
@@ -761,9 +769,29 @@ sf_status sf_solve(sf_plan plan) { return run_any(plan, OUT_SOLVE); }
 sf_status sf_gradient(sf_plan plan)
 {
     if (!plan) return SF_ERR_INVALID_ARG;
-    if (plan->bc != SF_BC_PERIODIC || plan->ncomp != 1)
-        return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient is built for scalar periodic plans");
-    return run_any(plan, OUT_GRAD);
+    if ((plan->bc != SF_BC_PERIODIC && plan->bc != SF_BC_UNBOUNDED) || plan->ncomp != 1)
+        return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient is built for scalar periodic and unbounded plans");
+    if (plan->bc == SF_BC_PERIODIC) return run_any(plan, OUT_GRAD);
+    // unbounded: psi and its three derivatives need four fields of work space
+    const int nf = 1 + plan->ndim;
+    const size_t welem = 2 * plan->esize;
+    if (!plan->gW1) {
+        sf_status st;
+        const size_t b1 = (size_t)plan->w1_field * nf * welem, b2 = (size_t)plan->w2_field * nf * welem;
+        if ((st = dev_alloc(plan, &plan->gW1, b1)) != SF_OK) return st;
+        if ((st = dev_alloc(plan, &plan->gW2, b2)) != SF_OK) return st;
+        if ((st = dev_alloc(plan, &plan->gout, field_elems(plan) * nf * plan->esize)) != SF_OK) return st;
+        SF_CUDA(plan, cudaMemsetAsync(plan->gW1, 0, b1, plan->stream));
+        SF_CUDA(plan, cudaMemsetAsync(plan->gW2, 0, b2, plan->stream));
+    }
+    std::swap(plan->W1, plan->gW1);
+    std::swap(plan->W2, plan->gW2);
+    std::swap(plan->out, plan->gout);
+    const sf_status st = run_any(plan, OUT_GRAD);
+    std::swap(plan->W1, plan->gW1);
+    std::swap(plan->W2, plan->gW2);
+    std::swap(plan->out, plan->gout);
+    return st;
 }
 
 sf_status sf_curl(sf_plan plan)
@@ -795,7 +823,7 @@ sf_status sf_output_device_ptr(sf_plan plan, int field, int comp, void** ptr)
     } else {
         return fail(plan, SF_ERR_INVALID_ARG, "unknown field");
     }
-    *ptr = (char*)plan->out + (size_t)idx * field_elems(plan) * plan->esize;
+    *ptr = (char*)plan->out_last + (size_t)idx * field_elems(plan) * plan->esize;
     return SF_OK;
 }
 

@@ -135,3 +135,23 @@ def test_fast_path_order4_kernel():
         sf.sf_solve(p.plan)
         got = p.get(sf.SF_OUT_PSI)
     _check("psi order 4, 256x256x32 f32", got, ref, "f32")
+
+
+def test_gradient_on_a_fast_path_plan():
+    """sf_gradient (generation-1 kernels, own four-field work arrays) and sf_solve (generation 2) on the
+    same fp32 plan, interleaved"""
+    shape = (256, 256, 32)
+    f = rounded(W.Rng(555).normal(int(np.prod(shape))).reshape(shape), "f32")
+    h = (1.0 / 256,) * 3
+    gh = O.unbounded_green((32, 256, 256), h, 2.0 * h[0])
+    psi_o, grad_o = O.unbounded_gradient(f.astype(np.float64), h, gh)
+    with Plan(shape, h, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec="f32") as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        _check("psi (solve)", p.get(sf.SF_OUT_PSI), psi_o, "f32")
+        sf.sf_gradient(p.plan)
+        _check("psi (gradient)", p.get(sf.SF_OUT_PSI), psi_o, "f32")
+        for a in range(3):
+            _check(f"grad[{a}]", p.get(sf.SF_OUT_GRAD, a), grad_o[a], "f32")
+        sf.sf_solve(p.plan)
+        _check("psi (solve again)", p.get(sf.SF_OUT_PSI), psi_o, "f32")

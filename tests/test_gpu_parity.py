@@ -258,6 +258,29 @@ def test_cfg4_spectrally_compact_kernel(prec):
     assert e <= (5e-6 if prec == "f32" else 1e-11)
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_cfg4_unbounded_gradient(prec):
+    """sf_gradient on a scalar unbounded plan (north_star: ik gradients from the same spectrum):
+    psi and the three derivatives vs the oracle on a non-cubic white-noise case, then a solve on the
+    same plan still returns psi (the gradient call uses its own work arrays)."""
+    shape = (16, 32, 64)
+    f = rounded(_rand(shape, 91), prec)
+    hs = (0.11, 0.07, 0.13)
+    gh = O.unbounded_green((64, 32, 16), hs, 2.0 * max(hs))
+    psi_o, grad_o = O.unbounded_gradient(f.astype(np.float64), hs, gh, rhs_sign=-1.0)
+    with Plan(shape, hs, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec=prec, rhs_sign=-1.0) as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        with pytest.raises(sf.SailffishError):
+            p.get(sf.SF_OUT_GRAD, 0)
+        sf.sf_gradient(p.plan)
+        _report("psi(gradient)", p.get(sf.SF_OUT_PSI), psi_o, prec)
+        for a in range(3):
+            _report(f"grad[{a}]", p.get(sf.SF_OUT_GRAD, a), grad_o[a], prec)
+        sf.sf_solve(p.plan)
+        _report("psi(solve after gradient)", p.get(sf.SF_OUT_PSI), psi_o, prec)
+
+
 # ------------------------------------------------------------------------------- config 5
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_cfg5_vortex_ring_curl(prec):
