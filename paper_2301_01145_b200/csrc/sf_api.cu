@@ -74,6 +74,7 @@ struct sf_plan_s {
     int LT[3] = { 0, 0, 0 };
     void* green = nullptr;
     void* green_tiles = nullptr;   // fast path: the same table, tile-major (sf_fast_api.h)
+    void* sched = nullptr;         // fast path: the dynamic tile counter of the strided kernels
     double scale = 1.0;
     // kernel generation 2 (sf_fast.cuh): fp32 unbounded plans with 256-long y and z pencils
     bool fast = false;
@@ -448,6 +449,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         // kernel generation 2: S2, S3, S4 as persistent TMA-fed register-FFT kernels
         sf2::FastParams fp;
         memset(&fp, 0, sizeof(fp));
+        fp.sched = (int*)p->sched;
         fp.nct = p->nspec_x / sf2::kTile;
         for (fp.nct_shift = 0; (1 << fp.nct_shift) < fp.nct; ++fp.nct_shift) {}
         fp.nyq_col = (p->nspec_x % sf2::kTile) ? fp.nct * sf2::kTile : -1;
@@ -463,12 +465,14 @@ template <typename T> sf_status run(sf_plan p, int outk)
         fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W2;
         fp.in_ps = fp.out_ps = hp * P1; fp.in_bs = fp.out_bs = hp; fp.nb = P1;
         fp.pair_batches = 1;
+        fp.nyq_first = 1;
         fp.green_tiles = (const float*)p->green_tiles; fp.Pb = P1;
         SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_FUSED, fp, p->map_s3, st));
         p->launches++;
         mark(3);
         // S4: W2 [z][ky][hp] -> W1 [z][y][hp]
         fp.pair_batches = 0;
+        fp.nyq_first = 0;
         fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W1;
         fp.in_ps = hp; fp.in_bs = hp * P1; fp.out_ps = hp; fp.out_bs = hp * n1; fp.nb = n2;
         SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_INV, fp, p->map_s4, st));
@@ -714,6 +718,8 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
                                       p->stream) != cudaSuccess)
                 return bail(SF_ERR_CUDA, "building the tile-major Green's table failed");
         }
+        if ((st = dev_alloc(p, &p->sched, 2 * sizeof(int))) != SF_OK) return bail(st, "");
+        if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
         p->fast = true;
         p->fast_x = (p->n[0] == 256) && p->pitch >= 258 && !getenv("SF_DISABLE_FAST_X");
     }

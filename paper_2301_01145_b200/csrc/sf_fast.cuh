@@ -233,15 +233,22 @@ __device__ __forceinline__ int green_tile_index(const FastParams& p, const TileG
 }
 __device__ __forceinline__ TileGeom tile_geom(const FastParams& p, int t)
 {
+    // The few Nyquist-column tiles are gathered and cost about three full tiles each.  nyq_first puts
+    // them at the head of the dynamic tile queue, where the CTAs that take one simply take fewer full
+    // tiles afterwards; measured, that shortens the fused pass (225 -> 201 us) and lengthens the other
+    // two, which keep them at the tail.
     TileGeom g;
     const int nfull = p.nb << p.nct_shift;   // nct is a power of two: no integer division per tile
-    if (t < nfull) {
+    const int nnyq = (p.nyq_col >= 0) ? (p.nb + kTile - 1) / kTile : 0;
+    const int tf = p.nyq_first ? t - nnyq : t;          // index among the full tiles
+    const int tn = p.nyq_first ? t : t - nfull;         // index among the Nyquist tiles
+    if (tf >= 0 && tf < nfull) {
         g.full = true;
-        g.b = batch_order(p, t >> p.nct_shift);
-        g.col = (t & (p.nct - 1)) * kTile;
+        g.b = batch_order(p, tf >> p.nct_shift);
+        g.col = (tf & (p.nct - 1)) * kTile;
     } else {
         g.full = false;
-        g.b = (t - nfull) * kTile;
+        g.b = tn * kTile;
         g.col = p.nyq_col;
     }
     return g;
@@ -302,14 +309,18 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
     const int ntiles = fast_ntiles(p.nb, p.nct, p.nyq_col);
     // element offsets fit 32 bits: an eligible plan's work arrays hold < 2^31 complex numbers (checked by the launcher)
     const int ips = (int)p.in_ps, ops = (int)p.out_ps, ibs = (int)p.in_bs, obs = (int)p.out_bs;
-    const int nit = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles of this CTA
     uint32_t parity = 0;   // phase of `bar` the next full tile completes
+    // dynamic tile scheduling: p.sched[0] is the next unclaimed tile.  s_tile[it & 1] is the tile of
+    // this CTA's iteration `it`; thread 0 claims the tile of iteration it + 2 once iteration it has
+    // read its index (after its first barrier), so the index is always known one tile ahead for the
+    // TMA prefetch and the atomic's latency is off the critical path.
+    __shared__ int s_tile[2];
 
     // issue the TMA load of this CTA's iteration `i` into the slot: one thread, one instruction.
     // Tiles that are not 16 neighbouring columns (the Nyquist column) are loaded by their consumer.
-    auto issue = [&](int i) {
-        if (!Cfg::kTma || tid != 0 || i >= nit) return;
-        const TileGeom g = tile_geom(p, (int)blockIdx.x + i * (int)gridDim.x);
+    auto issue = [&](int t) {
+        if (!Cfg::kTma || tid != 0 || t >= ntiles) return;
+        const TileGeom g = tile_geom(p, t);
         if (!g.full) return;
         mbar_expect_tx(&bar, Cfg::kSlotElems * (uint32_t)sizeof(C));
         if (MODE == FMODE_FWD) tma_load_4d(slot, &tm, g.col, 0, g.b, 0, &bar);
@@ -329,10 +340,18 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
         }
     };
 
+    // after the first barrier of iteration `it` (every thread has its tile index and its elements of
+    // the slot): prefetch the next tile, claim the one after
+    auto advance = [&](int it) {
+        if (tid != 0) return;
+        issue(s_tile[(it + 1) & 1]);
+        s_tile[it & 1] = atomicAdd(p.sched, 1);
+    };
+
     // one tile; ORIENT = orientation of the exchange buffer its first transform starts with
-    auto tile = [&](int i, auto orient_tag) {
+    auto tile = [&](int t, int it, auto orient_tag) {
         constexpr bool OB = decltype(orient_tag)::value;
-        const TileGeom g = tile_geom(p, (int)blockIdx.x + i * (int)gridDim.x);
+        const TileGeom g = tile_geom(p, t);
         // this thread's pencil: output pointer, validity
         const bool pvalid = g.full || (g.b + pen < p.nb);
         const int ob = g.full ? (g.b * obs + g.col + pen) : ((g.b + pen) * obs + g.col);
@@ -346,7 +365,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
             for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], t512[r]);
             fft256_a<false, OB, MODE != FMODE_FWD>(v, t256, o, xc);
             __syncthreads();
-            issue(i + 1);   // every thread has taken its elements out of the slot
+            advance(it);
             fft256_b<false, OB>(v, xc);
             if (pvalid) {
                 C* q = outp + (2 * o + h) * ops;   // row 2 (o + 16 k2) + h
@@ -368,7 +387,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                 for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], t512[r]);
                 fft256_a<false, OB, MODE != FMODE_FWD>(v, t256, o, xc);
                 __syncthreads();
-                issue(i + 1);   // every thread has taken its elements out of the slot
+                advance(it);
                 fft256_b<false, OB>(v, xc);
                 C u[16];
 #pragma unroll
@@ -386,6 +405,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                 for (int k2 = 0; k2 < 16; ++k2) v[k2] = __ldg(inp + k2 * 32 * ips);
                 fft256_a<true, OB, MODE != FMODE_FWD>(v, t256, o, xc);
                 __syncthreads();
+                advance(it);
                 fft256_b<true, OB>(v, xc);
             }
             // x_j = e_j + conj(w512^j) o_j, j = o + 16 r: h = 0 holds e, h = 1 holds o.  The half-warps
@@ -407,18 +427,44 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
         }
     };
 
-    issue(0);
+    if (tid == 0) {
+        s_tile[0] = atomicAdd(p.sched, 1);
+        s_tile[1] = atomicAdd(p.sched, 1);
+        issue(s_tile[0]);
+    }
+    __syncthreads();
     if constexpr (MODE == FMODE_FUSED) {
         // two transforms per tile: the orientation is back where it started
-        for (int i = 0; i < nit; ++i) tile(i, std::false_type());
+        for (int it = 0;; ++it) {
+            const int t = s_tile[it & 1];
+            if (t >= ntiles) break;
+            tile(t, it, std::false_type());
+        }
     } else {
         // one transform per tile: orientations alternate
-        for (int i = 0; i < nit; i += 2) {
-            tile(i, std::false_type());
-            if (i + 1 < nit) tile(i + 1, std::true_type());
+        for (int it = 0;; it += 2) {
+            int t = s_tile[0];
+            if (t >= ntiles) break;
+            tile(t, it, std::false_type());
+            t = s_tile[1];
+            if (t >= ntiles) break;
+            tile(t, it + 1, std::true_type());
+        }
+    }
+    // the last CTA to finish re-arms the counter for the next launch
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(p.sched + 1, 1) == (int)gridDim.x - 1) {
+            p.sched[0] = 0;
+            p.sched[1] = 0;
+            __threadfence();
         }
     }
 }
+
+} // namespace sf2
+
+namespace sf2 {
 
 // ==================================================================================== X passes
 // S1 (X forward) and S5 (X backward) for rows of 256 reals zero-padded to 512 (PAPER.md:87 real

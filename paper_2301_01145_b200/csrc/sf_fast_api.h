@@ -22,6 +22,8 @@ struct FastParams {
     int nct_shift;              // log2(nct)
     int nyq_col;                // column handled 16 batches at a time (the Nyquist column), -1: none
     int reverse_batches;        // visit batches last to first (the producer kernel wrote them first to last)
+    int* sched;                 // device: { next unclaimed tile, CTAs finished }, zero between launches
+    int nyq_first;              // Nyquist-column tiles at the head of the tile queue instead of its tail
     int pair_batches;           // fused: visit batches as 0, P/2, 1, P-1, 2, P-2, ... (mirror pairs share table rows)
     // fused multiply: real Green's table (rhs sign and normalisation folded in), tile-major:
     // chunk [kGreenRows fp][16 pencils] per tile, see green_tile_index / fast_green_tiles
