@@ -75,6 +75,7 @@ struct sf_plan_s {
     void* green = nullptr;
     void* green_tiles = nullptr;   // fast path: the same table, tile-major (sf_fast_api.h)
     void* sched = nullptr;         // fast path: the dynamic tile counter of the strided kernels
+    void *nyqA = nullptr, *nyqB = nullptr;   // fast path with fast X passes: the Nyquist column as [y][z] and [z][ky]
     double scale = 1.0;
     // kernel generation 2 (sf_fast.cuh): fp32 unbounded plans with 256-long y and z pencils
     bool fast = false;
@@ -430,6 +431,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
     if (fast_x) {
         fx.real_in = (const float*)p->src; fx.real_out = (float*)p->out;
         fx.spec = (sf2::C*)p->W1; fx.spec_pitch = hp; fx.nrows = n1 * n2;
+        fx.nyq = (sf2::C*)p->nyqA; fx.n1 = n1; fx.n2 = n2;
         SF_CUDA(p, sf2::launch_fast_x(false, fx, st));
     } else {
         SF_CUDA(p, launch_xfwd<T>(p->Lx, xp, ncomp, st));
@@ -456,6 +458,8 @@ template <typename T> sf_status run(sf_plan p, int outk)
         // S2: W1 [z][y][hp] -> W2 [z][ky][hp]
         fp.in = (const sf2::C*)p->W1; fp.out = (sf2::C*)p->W2;
         fp.in_ps = hp; fp.in_bs = hp * n1; fp.out_ps = hp; fp.out_bs = hp * P1; fp.nb = n2;
+        if (fast_x) { fp.nyq_in = (const sf2::C*)p->nyqA; fp.nyq_out = (sf2::C*)p->nyqB; }
+        fp.nyq_first = fast_x ? 1 : 0;
         fp.reverse_batches = 1;   // S1 wrote plane z last: start there while it is in L2
         SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_FWD, fp, p->map_s2, st));
         fp.reverse_batches = 0;
@@ -464,6 +468,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         // S3: W2 in place along z
         fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W2;
         fp.in_ps = fp.out_ps = hp * P1; fp.in_bs = fp.out_bs = hp; fp.nb = P1;
+        if (fast_x) { fp.nyq_in = (const sf2::C*)p->nyqB; fp.nyq_out = (sf2::C*)p->nyqB; }
         fp.pair_batches = 1;
         fp.nyq_first = 1;
         fp.green_tiles = (const float*)p->green_tiles; fp.Pb = P1;
@@ -471,8 +476,9 @@ template <typename T> sf_status run(sf_plan p, int outk)
         p->launches++;
         mark(3);
         // S4: W2 [z][ky][hp] -> W1 [z][y][hp]
+        if (fast_x) { fp.nyq_in = (const sf2::C*)p->nyqB; fp.nyq_out = (sf2::C*)p->nyqA; }
         fp.pair_batches = 0;
-        fp.nyq_first = 0;
+        fp.nyq_first = fast_x ? 1 : 0;
         fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W1;
         fp.in_ps = hp; fp.in_bs = hp * P1; fp.out_ps = hp; fp.out_bs = hp * n1; fp.nb = n2;
         SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_INV, fp, p->map_s4, st));
@@ -722,6 +728,10 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
         p->fast = true;
         p->fast_x = (p->n[0] == 256) && p->pitch >= 258 && !getenv("SF_DISABLE_FAST_X");
+        if (p->fast_x) {
+            if ((st = dev_alloc(p, &p->nyqA, (size_t)256 * 256 * 8)) != SF_OK) return bail(st, "");
+            if ((st = dev_alloc(p, &p->nyqB, (size_t)256 * 512 * 8)) != SF_OK) return bail(st, "");
+        }
     }
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "plan construction failed on the device");
     *out = p;

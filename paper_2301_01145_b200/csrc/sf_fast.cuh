@@ -333,12 +333,20 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
             parity ^= 1;
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = slot[(o + 16 * r) * kTile + pen];
+        } else if (p.nyq_in) {
+            // Nyquist column from its side array [row][batch]: the 16 batches are contiguous
+            const C* inp = p.nyq_in + (o * p.nb + g.b + pen);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = __ldg(inp + r * 16 * p.nb);
         } else {
             const C* inp = p.in + (min(g.b + pen, p.nb - 1) * ibs + g.col + o * ips);
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = __ldg(inp + r * 16 * ips);
         }
     };
+    // staging of a Nyquist tile image in the exchange buffer for a transposing copy: element
+    // (row, pencil) at row * 16 + ((pencil + row) & 15) -- conflict-free both along pencils and along rows
+    auto stage = [&](int row, int pencil) -> C& { return xbuf[row * kTile + ((pencil + row) & 15)]; };
 
     // after the first barrier of iteration `it` (every thread has its tile index and its elements of
     // the slot): prefetch the next tile, claim the one after
@@ -354,8 +362,11 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
         const TileGeom g = tile_geom(p, t);
         // this thread's pencil: output pointer, validity
         const bool pvalid = g.full || (g.b + pen < p.nb);
+        const bool side = !g.full && p.nyq_in != nullptr;   // Nyquist tile served by the side arrays
         const int ob = g.full ? (g.b * obs + g.col + pen) : ((g.b + pen) * obs + g.col);
-        C* outp = p.out + ob;
+        C* outp = side ? p.nyq_out + (g.b + pen) : p.out + ob;
+        const int ost = side ? p.nb : ops;                  // row stride of the output
+        (void)ost;
         C v[16];
 
         if constexpr (MODE == FMODE_FWD) {
@@ -367,7 +378,19 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
             __syncthreads();
             advance(it);
             fft256_b<false, OB>(v, xc);
-            if (pvalid) {
+            if (side) {
+                // the consumer (S3) wants this column as [pencil of S2 = z][ky]: transpose through the
+                // exchange buffer and write 512 contiguous ky per z
+                __syncthreads();   // every thread is done reading the exchange buffer
+#pragma unroll
+                for (int k2 = 0; k2 < 16; ++k2) stage(2 * (o + 16 * k2) + h, pen) = v[brev4(k2)];
+                __syncthreads();
+                for (int idx = tid; idx < 2 * kL * kTile; idx += kThreads) {
+                    const int pp = idx >> 9, ky = idx & (2 * kL - 1);
+                    if (g.b + pp < p.nb) p.nyq_out[(g.b + pp) * (2 * kL) + ky] = stage(ky, pp);
+                }
+                __syncthreads();   // before the next tile's exchange
+            } else if (pvalid) {
                 C* q = outp + (2 * o + h) * ops;   // row 2 (o + 16 k2) + h
 #pragma unroll
                 for (int k2 = 0; k2 < 16; ++k2) q[k2 * 32 * ops] = v[brev4(k2)];
@@ -400,9 +423,22 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
             } else {
                 // rows 2 k + h, k = o + 16 k2: h = 0 even spectrum E, h = 1 odd spectrum O; each half-warp
                 // reads one 128-byte run per row (16 batches of one column for the Nyquist tiles)
-                const C* inp = p.in + ((g.full ? (g.b * ibs + g.col + pen) : (min(g.b + pen, p.nb - 1) * ibs + g.col)) + (2 * o + h) * ips);
+                if (side) {
+                    // the producer (S3) left this column as [pencil of S4 = z][ky]: read 512 contiguous ky
+                    // per z and transpose through the exchange buffer
+                    for (int idx = tid; idx < 2 * kL * kTile; idx += kThreads) {
+                        const int pp = idx >> 9, ky = idx & (2 * kL - 1);
+                        stage(ky, pp) = (g.b + pp < p.nb) ? __ldg(p.nyq_in + (g.b + pp) * (2 * kL) + ky) : make_float2(0.f, 0.f);
+                    }
+                    __syncthreads();
 #pragma unroll
-                for (int k2 = 0; k2 < 16; ++k2) v[k2] = __ldg(inp + k2 * 32 * ips);
+                    for (int k2 = 0; k2 < 16; ++k2) v[k2] = stage(2 * (o + 16 * k2) + h, pen);
+                    __syncthreads();   // before the exchange overwrites the staging
+                } else {
+                    const C* inp = p.in + ((g.full ? (g.b * ibs + g.col + pen) : (min(g.b + pen, p.nb - 1) * ibs + g.col)) + (2 * o + h) * ips);
+#pragma unroll
+                    for (int k2 = 0; k2 < 16; ++k2) v[k2] = __ldg(inp + k2 * 32 * ips);
+                }
                 fft256_a<true, OB, MODE != FMODE_FWD>(v, t256, o, xc);
                 __syncthreads();
                 advance(it);
@@ -410,7 +446,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
             }
             // x_j = e_j + conj(w512^j) o_j, j = o + 16 r: h = 0 holds e, h = 1 holds o.  The half-warps
             // swap half of their values: h = 0 finishes r < 8, h = 1 finishes r >= 8.
-            C* q = outp + (o + 128 * h) * ops;
+            C* q = outp + (o + 128 * h) * ost;
 #pragma unroll
             for (int r = 0; r < 8; ++r) {
                 // h = 1: t_lo = conj(w) o_r (sent), t_hi = conj(w) o_{r+8} (kept);  h = 0: e_{r+8} sent, e_r kept
@@ -422,7 +458,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                 recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
                 recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
                 const C x = cadd(keep, recv);
-                if (pvalid) q[r * 16 * ops] = x;
+                if (pvalid) q[r * 16 * ost] = x;
             }
         }
     };
@@ -556,6 +592,14 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
         else bulk_g2s(rbuf + tid * kXInPitch, p.real_in + row * kXN, kXN * (uint32_t)sizeof(float), &bar);
     };
 
+    // S5: the Nyquist coefficient of this thread's row of iteration i, for the thread that merges the pair (0, 256)
+    auto load_nyq = [&](int i) -> C {
+        if (!INV || !p.nyq || w != 0 || h != 0 || i >= nit) return make_float2(0.f, 0.f);
+        const long long tl = (long long)blockIdx.x + (long long)i * gridDim.x;
+        const int row = (int)((p.reverse ? ntiles - 1 - tl : tl) * kXRows) + pen;
+        return __ldg(p.nyq + (row % p.n1) * p.n2 + row / p.n1);
+    };
+    C xnyq_next = load_nyq(0);
     issue(0);
     for (int i = 0; i < nit; ++i) {
         const long long tl0 = (long long)blockIdx.x + (long long)i * gridDim.x;
@@ -608,9 +652,18 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
             if (tid < kXRows) {
                 bulk_s2g(p.spec + (row0 + tid) * p.spec_pitch, sbuf + tid * kXSpPitch, kXSpPitch * (uint32_t)sizeof(C));
                 bulk_commit();
+                // the Nyquist coefficient X[256] of row (z, y) also goes to the side array [y][z] that the
+                // strided passes read it from in 128-byte runs
+                if (p.nyq) {
+                    const int row = (int)(row0 + tid);
+                    p.nyq[(row % p.n1) * p.n2 + row / p.n1] = sbuf[tid * kXSpPitch + kXN];
+                }
             }
         } else {
             // ---------------------------------------------------------------- S5
+            // X[256] of this thread's row comes from the side array [y][z] (only the owner of the pair
+            // (0, 256) needs it); it was requested one tile ahead
+            const C xnyq = xnyq_next;
             mbar_wait(&bar, parity);
             parity ^= 1;
             // merge in place: Z[k] = e + i conj(w512^k) d, Z[256 - k] = conj e + i conj(conj(w512^k) d)
@@ -621,6 +674,7 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
                 for (int m = 0; m < 9; ++m) {
                     const int k = idx + 16 * m;
                     if (m < 8 || idx == 0) { xk[m] = srow[k]; xm[m] = srow[kXN - k]; }
+                    if (m == 0 && idx == 0 && p.nyq) xm[0] = xnyq;
                 }
 #pragma unroll
                 for (int m = 0; m < 9; ++m) {
@@ -642,6 +696,7 @@ template <bool INV> __global__ void __launch_bounds__(kXThreads, 2) fast_x_kerne
             fence_async_smem();                   // the merged values in sbuf are overwritten by the next bulk load
             __syncthreads();
             issue(i + 1);                         // sbuf is in registers everywhere
+            xnyq_next = load_nyq(i + 1);
             C a[8], b[8];
             fft128_b<true>(a, b, xr);
             // z[n] = z0[n] + conj(w256^n) z1[n], n = w + 16 k2 (a) / w + 8 + 16 k2 (b): h = 0 holds z0,

@@ -21,6 +21,13 @@ struct FastParams {
     int nct;                    // full 16-column tiles per batch: a power of two
     int nct_shift;              // log2(nct)
     int nyq_col;                // column handled 16 batches at a time (the Nyquist column), -1: none
+    // Optional side arrays that hold the Nyquist column instead of column nyq_col of in / out, laid out
+    // so that its tiles move in 128-byte runs too (NULL: gather / scatter column nyq_col):
+    //   FWD   nyq_in [row y][batch z]   -> nyq_out [batch z][row ky] (512 per z)
+    //   FUSED nyq_in = nyq_out [row z][batch ky]
+    //   INV   nyq_in [batch z][row ky]  -> nyq_out [row y][batch z]
+    const C* nyq_in;
+    C* nyq_out;
     int reverse_batches;        // visit batches last to first (the producer kernel wrote them first to last)
     int* sched;                 // device: { next unclaimed tile, CTAs finished }, zero between launches
     int nyq_first;              // Nyquist-column tiles at the head of the tile queue instead of its tail
@@ -42,6 +49,8 @@ struct FastXParams {
     long long spec_pitch;
     int nrows;              // multiple of 16
     int reverse;            // visit row tiles last to first
+    C* nyq;                 // optional side array [y][z] (n1 x n2) of the Nyquist coefficient X[256] of row z * n1 + y:
+    int n1, n2;             // S1 writes it (besides column 256 of spec), S5 reads it (instead); NULL: column 256 only
 };
 
 // opaque storage of a CUtensorMap (TMA descriptor): 128 bytes, 64-byte aligned
