@@ -186,6 +186,10 @@ long long sf_device_bytes(sf_plan plan);
  */
 sf_status sf_enable_step_timing(sf_plan plan, int slots);
 sf_status sf_step_times_ms(sf_plan plan, float ms[5]);
+/* Record only every `stride`-th compute call (default 1) while step timing is on: the event records
+ * between the steps cost a few microseconds per call, which a throughput measurement that wants the
+ * per-step times from inside its own timed region can dilute this way.  Errors: INVALID_ARG if stride < 1. */
+sf_status sf_set_step_timing_stride(sf_plan plan, int stride);
 
 /* Message for the last error on this plan (or, with plan == NULL, of the last failed
  * sf_plan_create on this thread).  Never NULL; owned by the library. */

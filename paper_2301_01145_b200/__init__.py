@@ -30,7 +30,7 @@ SF_OUT_PSI, SF_OUT_GRAD, SF_OUT_CURL = 0, 1, 2
 EXPORTS = (
     "sf_plan_create", "sf_set_source", "sf_set_bc_values", "sf_solve", "sf_gradient", "sf_curl",
     "sf_get_output", "sf_output_device_ptr", "sf_synchronize", "sf_last_launch_count", "sf_device_bytes",
-    "sf_enable_step_timing", "sf_step_times_ms", "sf_last_error", "sf_plan_destroy", "sf_version",
+    "sf_enable_step_timing", "sf_step_times_ms", "sf_set_step_timing_stride", "sf_last_error", "sf_plan_destroy", "sf_version",
 )
 
 
@@ -71,6 +71,7 @@ def lib() -> C.CDLL:
         L.sf_device_bytes.restype = ll
         L.sf_enable_step_timing.argtypes = [vp, i]
         L.sf_step_times_ms.argtypes = [vp, C.POINTER(C.c_float)]
+        L.sf_set_step_timing_stride.argtypes = [vp, i]
         L.sf_last_error.argtypes = [vp]
         L.sf_last_error.restype = C.c_char_p
         L.sf_plan_destroy.argtypes = [vp]
@@ -171,6 +172,10 @@ def sf_device_bytes(plan) -> int:
 
 def sf_enable_step_timing(plan, slots=1):
     _check(plan, lib().sf_enable_step_timing(plan, int(slots)))
+
+
+def sf_set_step_timing_stride(plan, stride=1):
+    _check(plan, lib().sf_set_step_timing_stride(plan, int(stride)))
 
 
 def sf_step_times_ms(plan):

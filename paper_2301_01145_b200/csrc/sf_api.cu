@@ -91,6 +91,8 @@ struct sf_plan_s {
     int launches = 0;
     int tslots = 0;               // step timing: compute calls remembered (0 = off)
     long long tcount = 0;         // compute calls recorded since timing was enabled
+    int tstride = 1;              // record every tstride-th compute call
+    long long tcalls = 0;         // compute calls seen since timing was enabled
     std::vector<cudaEvent_t> ev;  // 6 events per slot
     std::string err = "";
 };
@@ -403,8 +405,9 @@ template <typename T> sf_status run(sf_plan p, int outk)
     const int P1 = p->padded ? 2 * n1 : n1;
     cudaStream_t st = p->stream;
     p->launches = 0;
+    const bool timed = p->tslots && (p->tcalls++ % p->tstride) == 0;
     const int slot = p->tslots ? (int)(p->tcount % p->tslots) : 0;
-    auto mark = [&](int i) { if (p->tslots) cudaEventRecord(p->ev[6 * slot + i], st); };
+    auto mark = [&](int i) { if (timed) cudaEventRecord(p->ev[6 * slot + i], st); };
 
     // S1: X forward
     XParams<T> xp;
@@ -490,7 +493,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         else SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
         p->launches++;
         mark(5);
-        if (p->tslots) p->tcount++;
+        if (timed) p->tcount++;
         p->last_kind = outk;
     p->out_last = p->out;
         p->out_last = p->out;
@@ -553,7 +556,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
     SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
     p->launches++;
     mark(5);
-    if (p->tslots) p->tcount++;
+    if (timed) p->tcount++;
     p->last_kind = outk;
     p->out_last = p->out;
     return SF_OK;
@@ -883,6 +886,15 @@ sf_status sf_enable_step_timing(sf_plan plan, int slots)
     }
     plan->tslots = slots;
     plan->tcount = 0;
+    plan->tcalls = 0;
+    return SF_OK;
+}
+
+sf_status sf_set_step_timing_stride(sf_plan plan, int stride)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (stride < 1) return fail(plan, SF_ERR_INVALID_ARG, "stride must be >= 1");
+    plan->tstride = stride;
     return SF_OK;
 }
 
