@@ -155,3 +155,181 @@ def test_gradient_on_a_fast_path_plan():
             _check(f"grad[{a}]", p.get(sf.SF_OUT_GRAD, a), grad_o[a], "f32")
         sf.sf_solve(p.plan)
         _check("psi (solve again)", p.get(sf.SF_OUT_PSI), psi_o, "f32")
+
+
+# ------------------------------------------------------------------- configs 2, 3 and 5 at full size
+@pytest.mark.parametrize("prec,op", [("f32", "ps"), ("f64", "fd2")])
+def test_cfg2_full_size(prec, op):
+    """BASELINE.json configs[1]: 256^3 periodic, |f_k| ~ |k|^-2 up to k = 64, psi and its spectral gradient"""
+    w = W.periodic3d_spectrum(256, kmax=64)
+    f = rounded(w["f"], prec)
+    oop, sop = (O.OP_PS, sf.SF_OP_PSEUDO_SPECTRAL) if op == "ps" else (O.OP_FD2, sf.SF_OP_FD2)
+    psi_o, grad_o = O.periodic(f.astype(np.float64), w["L"], oop, want_grad=True)
+    h = tuple(L / 256 for L in w["L"])
+    with Plan(f.shape, h, sf.SF_BC_PERIODIC, op=sop, prec=prec) as p:
+        p.set_source(f)
+        sf.sf_gradient(p.plan)
+        _check(f"cfg2 256^3 {prec} {op} psi", p.get(sf.SF_OUT_PSI), psi_o, prec)
+        for a in range(3):
+            _check(f"cfg2 256^3 {prec} {op} grad[{a}]", p.get(sf.SF_OUT_GRAD, a), grad_o[a], prec)
+        sf.sf_solve(p.plan)
+        _check(f"cfg2 256^3 {prec} {op} psi (solve)", p.get(sf.SF_OUT_PSI), psi_o, prec)
+
+
+def _fd2_residual(psi, f, h, faces, kind):
+    """the seven-point equation the FD2 operator solves (eq. (12)-(13)), evaluated on the whole
+    grid with the boundary values in ghost layers: Dirichlet cell-boundary grids carry psi on the face
+    nodes, Neumann cell-centre grids a ghost cell psi_ghost = psi_first -/+ h dpsi/dn.  Returns the
+    relative L2 norm of lap_h psi - f (Neumann: of its zero-mean part -- the
+    discrete problem is solvable only up to the compatibility defect of the data, a constant, which the
+    zero-mode convention drops, reading A21)."""
+    e = np.pad(psi, 1)
+    for axis in range(3):          # axis 0 = x (last array axis)
+        ax = 2 - axis
+        lo, hi = faces[(axis, 0)], faces[(axis, 1)]
+        sl_lo = [slice(1, -1)] * 3
+        sl_hi = [slice(1, -1)] * 3
+        sl_lo[ax], sl_hi[ax] = 0, -1
+        if kind == "dirichlet":
+            e[tuple(sl_lo)], e[tuple(sl_hi)] = lo, hi
+        else:
+            first = [slice(1, -1)] * 3
+            last = [slice(1, -1)] * 3
+            first[ax], last[ax] = 1, -2
+            e[tuple(sl_lo)] = e[tuple(first)] - h[axis] * lo
+            e[tuple(sl_hi)] = e[tuple(last)] + h[axis] * hi
+    lap = np.zeros_like(psi)
+    c = e[1:-1, 1:-1, 1:-1]
+    lap += (e[1:-1, 1:-1, 2:] - 2 * c + e[1:-1, 1:-1, :-2]) / h[0] ** 2
+    lap += (e[1:-1, 2:, 1:-1] - 2 * c + e[1:-1, :-2, 1:-1]) / h[1] ** 2
+    lap += (e[2:, 1:-1, 1:-1] - 2 * c + e[:-2, 1:-1, 1:-1]) / h[2] ** 2
+    r = lap - f
+    if kind == "neumann":
+        r = r - r.mean()
+    return float(np.linalg.norm(r) / np.linalg.norm(f))
+
+
+def test_cfg3_dirichlet_full_size():
+    """BASELINE.json configs[2]: 255^3 interior nodes, fp64, FD2, inhomogeneous faces; against the oracle
+    (direct DST-I sums, ~15 s on the host) and against the discrete equation itself"""
+    d = W.dirichlet3d_manufactured(nc=256, inhomogeneous=True)
+    assert d["f"].shape == (255, 255, 255)
+    psi_o = O.dirichlet_regular(d["f"], d["h"], d["faces"])
+    with Plan(d["f"].shape, d["h"], sf.SF_BC_DIRICHLET, grid=sf.SF_GRID_CELL_BOUNDARY, op=sf.SF_OP_FD2,
+              prec="f64") as p:
+        p.set_source(d["f"])
+        p.set_faces(d["faces"])
+        sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI)
+    _check("cfg3 Dirichlet 255^3 f64", got, psi_o, "f64")
+    res = _fd2_residual(got, d["f"], d["h"], d["faces"], "dirichlet")
+    print(f"cfg3 Dirichlet 255^3: relative residual of the seven-point equation {res:.3e}")
+    assert res <= 1e-10  # lap_h amplifies rounding by ~ 12 / h^2 |psi| / |f|; measured 6e-14
+
+
+def test_cfg3_neumann_full_size():
+    """the Neumann variant of configs[2]: 256^3 cell-centre grid, fp64, FD2, inhomogeneous fluxes"""
+    d = W.neumann3d_manufactured(nc=256, inhomogeneous=True)
+    psi_o = O.neumann_staggered(d["f"], d["h"], d["faces"])
+    with Plan(d["f"].shape, d["h"], sf.SF_BC_NEUMANN, grid=sf.SF_GRID_CELL_CENTRE, op=sf.SF_OP_FD2, prec="f64") as p:
+        p.set_source(d["f"])
+        p.set_faces(d["faces"])
+        sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI)
+    _check("cfg3 Neumann 256^3 f64", got - got.mean(), psi_o - psi_o.mean(), "f64")
+    e_res = _fd2_residual(got, d["f"], d["h"], d["faces"], "neumann")
+    print(f"cfg3 Neumann 256^3: relative residual of the seven-point equation {e_res:.3e}")
+    assert e_res <= 1e-10   # measured 3e-14
+
+
+def _gauss2_vec(r, eps):
+    """the order-2 regularised kernel for an array of distances (reading A10), restated here for the
+    sampled sums below and checked against the oracle's scalar routine where it is used"""
+    from scipy.special import erf
+    r = np.asarray(r, dtype=np.float64)
+    out = np.empty_like(r)
+    nz = r > 0
+    out[nz] = -erf(r[nz] / (np.sqrt(2.0) * eps)) / (4.0 * np.pi * r[nz])
+    out[~nz] = -np.sqrt(2.0 / np.pi) / (4.0 * np.pi * eps)
+    return out
+
+
+def test_cfg5_narrow_against_the_oracle():
+    """the vector plan with two axes at the full 512 (1024 padded) extent of BASELINE.json configs[4] and a
+    narrow third one, white noise, against the whole oracle"""
+    shape = (512, 16, 512)   # z, y, x
+    om = rounded(W.Rng(5005).normal(3 * int(np.prod(shape))).reshape((3,) + shape), "f32")
+    h = (1.0 / 512,) * 3
+    gh = O.unbounded_green((512, 16, 512), h, 2.0 * h[0])
+    u_o = O.unbounded_solve(om.astype(np.float64), h, gh, rhs_sign=-1.0, want_curl=True)
+    with Plan(shape, h, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec="f32", ncomp=3, rhs_sign=-1.0) as p:
+        p.set_source(om)
+        sf.sf_curl(p.plan)
+        for c in range(3):
+            _check(f"u[{c}] 512x16x512 f32", p.get(sf.SF_OUT_CURL, c), u_o[c], "f32")
+
+
+def test_cfg5_full_size():
+    """BASELINE.json configs[4] at its full size: 512^3 (padded 1024^3), fp32, three components, curl in
+    the same spectral pass.  The oracle's whole-domain solve needs ~100 GB at this size, so:
+    (1) psi at sampled nodes against the definition the oracle implements, the discrete convolution
+        psi_c(x_i) = rhs_sign h^3 sum_j G(|x_i - x_j|) omega_c(x_j), summed in fp64 over every non-zero source node;
+    (2) u = curl psi: the spectral curl against fourth-order central differences of the computed psi
+        (holds at any size; with the smooth core sigma = 4 h the difference error is ~ 3e-5);
+    (3) div u = 0 to the same accuracy, and the ring's symmetry: u along the axis at the centre."""
+    n = 512
+    v = W.vortex_ring(n)
+    om = rounded(v["omega"], "f32")
+    h = v["h"][0]
+    eps = 2.0 * h
+    with Plan(om.shape[1:], v["h"], sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec="f32", ncomp=3,
+              rhs_sign=-1.0) as p:
+        p.set_source(om)
+        sf.sf_curl(p.plan)
+        assert sf.sf_last_launch_count(p.plan) == 5
+        u = np.stack([p.get(sf.SF_OUT_CURL, c) for c in range(3)])
+        sf.sf_solve(p.plan)
+        psi = np.stack([p.get(sf.SF_OUT_PSI, c) for c in range(3)])
+    assert np.isfinite(u).all() and np.isfinite(psi).all()
+
+    # (1) sampled nodes: the corners (largest linear indices), the centre, on the core, random ones
+    rng = np.random.default_rng(5)
+    pts = [(0, 0, 0), (n - 1, n - 1, n - 1), (n - 1, 0, n - 1), (n // 2, n // 2, n // 2), (n // 2, n // 2, n // 2 + n // 4)]
+    pts += [tuple(int(t) for t in rng.integers(0, n, 3)) for _ in range(5)]
+    rs = rng.uniform(0, 10 * eps, 50)
+    assert np.allclose(_gauss2_vec(rs, eps), [O.green_gauss2(r, eps) for r in rs], rtol=1e-14, atol=0)
+    assert _gauss2_vec(np.zeros(1), eps)[0] == pytest.approx(O.green_gauss2(0.0, eps), rel=1e-14)
+    for c in range(3):
+        iz, iy, ix = np.nonzero(om[c])
+        w = om[c][iz, iy, ix].astype(np.float64)
+        scale = float(np.abs(psi[c]).max())
+        for (pz, py, px) in pts:
+            r = h * np.sqrt((iz - pz) ** 2.0 + (iy - py) ** 2.0 + (ix - px) ** 2.0)
+            want = -(h ** 3) * float(np.dot(_gauss2_vec(r, eps), w))
+            got = float(psi[c][pz, py, px])
+            assert abs(got - want) <= 5e-6 * scale, (c, (pz, py, px), got, want, scale)
+
+    # (2), (3) on the interior box (two nodes from every face for the five-point differences)
+    def d(a, axis):   # fourth-order central difference along array axis `axis` of the interior box
+        s = lambda k: tuple(slice(2 + k, a.shape[i] - 2 + k) if i == axis else slice(2, a.shape[i] - 2) for i in range(3))
+        return (8.0 * (a[s(1)].astype(np.float64) - a[s(-1)]) - (a[s(2)].astype(np.float64) - a[s(-2)])) / (12.0 * h)
+    inner = (slice(2, -2),) * 3
+    # components: 0 = x (array axis 2), 1 = y (axis 1), 2 = z (axis 0)
+    curl = [d(psi[2], 1) - d(psi[1], 0), d(psi[0], 0) - d(psi[2], 2), d(psi[1], 2) - d(psi[0], 1)]
+    unorm = np.sqrt(sum(float(np.sum(u[c][inner].astype(np.float64) ** 2)) for c in range(3)))
+    for c in range(3):
+        e = float(np.linalg.norm(curl[c] - u[c][inner])) / unorm
+        print(f"cfg5 512^3: |u[{c}] - curl_h(psi)[{c}]| / |u| = {e:.3e}")
+        assert e <= 5e-4     # measured 2.9e-5
+    del curl
+    div = d(u[0], 2) + d(u[1], 1) + d(u[2], 0)
+    e = float(np.linalg.norm(div)) * h / unorm
+    print(f"cfg5 512^3: h |div_h u| / |u| = {e:.3e}")
+    assert e <= 5e-4         # measured 5.6e-6
+    # the induced velocity at the ring's centre points along the ring axis; thin-ring value Gamma / (2 R)
+    c0 = n // 2
+    uc = np.array([u[a][c0 - 1:c0 + 1, c0 - 1:c0 + 1, c0 - 1:c0 + 1].astype(np.float64).mean() for a in range(3)])
+    cosang = abs(float(np.dot(uc, v["axis"]))) / float(np.linalg.norm(uc))
+    print(f"cfg5 512^3: u(centre) = {uc}, |u| 2R/Gamma = {np.linalg.norm(uc) * 2 * v['radius'] / v['gamma']:.4f}, cos = {cosang:.6f}")
+    assert cosang >= 0.9999
+    assert np.linalg.norm(uc) * 2 * v["radius"] / v["gamma"] == pytest.approx(1.0, abs=0.02)
