@@ -138,6 +138,29 @@ def periodic(f, L, op=OP_PS, rhs_sign=1.0, want_grad=False):
     return (psi, grad) if want_grad else psi
 
 
+def periodic_divergence(f, L, op=OP_PS, rhs_sign=1.0):
+    """DIV on a periodic vector plan: f[nd, (z,) y, x] -> div psi, psi_c the solution for source f_c."""
+    f = _f64(f)
+    nd, n = _dims(f.shape[1:])
+    assert f.shape[0] == nd
+    Lx = list(L) + [1.0] * (3 - len(L))
+    out = np.empty(f.shape[1:])
+    _chk(lib().orc_periodic_divlap(C.c_int(nd), _i64x3(n), _f64x3(Lx), C.c_int(op), C.c_double(rhs_sign), C.c_int(nd),
+                                   _ptr(f), C.c_int(0), _ptr(out)), "periodic_divergence")
+    return out
+
+
+def periodic_laplacian(f, L, op=OP_PS, rhs_sign=1.0, ncomp=1):
+    """NABLA on a periodic plan: lap psi per component (f[(z,) y, x], or f[c, ...] with ncomp = c)."""
+    f = _f64(f)
+    nd, n = _dims(f.shape[1:] if ncomp > 1 else f.shape)
+    Lx = list(L) + [1.0] * (3 - len(L))
+    out = np.empty_like(f)
+    _chk(lib().orc_periodic_divlap(C.c_int(nd), _i64x3(n), _f64x3(Lx), C.c_int(op), C.c_double(rhs_sign),
+                                   C.c_int(ncomp), _ptr(f), C.c_int(1), _ptr(out)), "periodic_laplacian")
+    return out
+
+
 def _faces_arg(faces):
     """faces: dict {(axis, side): array} or None -> (const double*[6], keepalive)."""
     arr = (C.c_void_p * 6)()
@@ -232,6 +255,32 @@ def unbounded_gradient(f, h, ghat, rhs_sign=1.0):
     _chk(lib().orc_unbounded_gradient(_i64x3(n), _f64x3(h), _ptr(ghat), C.c_double(rhs_sign), _ptr(f), _ptr(psi),
                                       _ptr(grad)), "unbounded_gradient")
     return psi, grad
+
+
+def unbounded_divergence(f, h, ghat, rhs_sign=1.0):
+    """DIV on an unbounded vector plan: f[3, z, y, x] -> div psi[z, y, x], psi_c = rhs_sign G * f_c."""
+    f = _f64(f)
+    assert f.ndim == 4 and f.shape[0] == 3
+    nd, n = _dims(f.shape[1:])
+    out = np.empty(f.shape[1:])
+    ghat = np.ascontiguousarray(ghat, dtype=np.complex128)
+    assert ghat.shape == (2 * n[2], 2 * n[1], n[0] + 1)
+    _chk(lib().orc_unbounded_divlap(_i64x3(n), _f64x3(h), _ptr(ghat), C.c_int(3), C.c_double(rhs_sign), _ptr(f),
+                                    C.c_int(0), _ptr(out)), "unbounded_divergence")
+    return out
+
+
+def unbounded_laplacian(f, h, ghat, rhs_sign=1.0):
+    """NABLA on an unbounded plan: lap psi per component, f[z, y, x] or f[c, z, y, x]."""
+    f = _f64(f)
+    vec = f.ndim == 4
+    nd, n = _dims(f.shape[1:] if vec else f.shape)
+    out = np.empty_like(f)
+    ghat = np.ascontiguousarray(ghat, dtype=np.complex128)
+    assert ghat.shape == (2 * n[2], 2 * n[1], n[0] + 1)
+    _chk(lib().orc_unbounded_divlap(_i64x3(n), _f64x3(h), _ptr(ghat), C.c_int(f.shape[0] if vec else 1),
+                                    C.c_double(rhs_sign), _ptr(f), C.c_int(1), _ptr(out)), "unbounded_laplacian")
+    return out
 
 
 def unbounded_direct(f, h, eps, rhs_sign=1.0):

@@ -849,6 +849,144 @@ done:
     return err;
 }
 
+/* DIV and NABLA on an unbounded plan ("DIV: resolves the divergence ... NABLA: resolves
+ * the Laplacian of the input field", applied with the convolution kernel as eq. (10) is, PAPER.md:141-143;
+ * reading A27): psi_c = rhs_sign G * f_c per component, then in the same spectral pass
+ *   kind 0 (DIV,   ncomp == 3): out = sum_a IDFT(i kappa_a psi_hat_a)                 one field
+ *   kind 1 (NABLA, any ncomp):  out_c = IDFT(sum_a (i kappa_a)^2 psi_hat_c)           ncomp fields
+ * with the kappa_a of the gradient and the curl (doubled grid, Nyquist -> 0, reading A20): NABLA is DIV of
+ * GRAD, two successive multiplications by i kappa. */
+int orc_unbounded_divlap(const i64 n[3], const double h[3], const cplx *ghat, int ncomp, double rhs_sign,
+                         const double *f, int kind, double *out)
+{
+    if (kind != 0 && kind != 1) return ORC_ERR_ARG;
+    if (kind == 0 && ncomp != 3) return ORC_ERR_ARG;
+    for (int a = 0; a < 3; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
+    i64 tot = n[0] * n[1] * n[2], ns = unb_spec_size(n);
+    i64 P[3] = { 2 * n[0], 2 * n[1], 2 * n[2] }, H0 = n[0] + 1;
+    int err = ORC_OK;
+    cplx *spec = (cplx *)malloc(sizeof(cplx) * (size_t)ns), *acc = NULL;
+    double *kap[3] = { 0, 0, 0 };
+    if (!spec) { err = ORC_ERR_ALLOC; goto done; }
+    for (int a = 0; a < 3; ++a) {
+        kap[a] = (double *)malloc(sizeof(double) * (size_t)P[a]);
+        if (!kap[a]) { err = ORC_ERR_ALLOC; goto done; }
+        for (i64 k = 0; k < P[a]; ++k) {
+            i64 m = (k < n[a]) ? k : k - P[a];
+            kap[a][k] = (k == n[a]) ? 0.0 : 2.0 * PI * (double)m / ((double)P[a] * h[a]);
+        }
+    }
+    if (kind == 0) {
+        acc = (cplx *)calloc((size_t)ns, sizeof(cplx));
+        if (!acc) { err = ORC_ERR_ALLOC; goto done; }
+    }
+    for (int c = 0; c < ncomp; ++c) {
+        if ((err = unb_forward(n, f + (size_t)c * (size_t)tot, 1, spec)) != ORC_OK) goto done;
+#pragma omp parallel for collapse(2) schedule(static)
+        for (i64 kz = 0; kz < P[2]; ++kz)
+            for (i64 ky = 0; ky < P[1]; ++ky)
+                for (i64 kx = 0; kx < H0; ++kx) {
+                    i64 i = kx + H0 * (ky + P[1] * kz);
+                    i64 kk[3] = { kx, ky, kz };
+                    cplx psi = rhs_sign * ghat[i] * spec[i];
+                    if (kind == 0) {
+                        acc[i] += I * kap[c][kk[c]] * psi;
+                    } else {
+                        cplx s = 0.0;
+                        for (int a = 0; a < 3; ++a) s += (I * kap[a][kk[a]]) * (I * kap[a][kk[a]]) * psi;
+                        spec[i] = s;
+                    }
+                }
+        if (kind == 1 && (err = unb_backward_extract(n, spec, out + (size_t)c * (size_t)tot)) != ORC_OK) goto done;
+    }
+    if (kind == 0) err = unb_backward_extract(n, acc, out);
+done:
+    for (int a = 0; a < 3; ++a) free(kap[a]);
+    free(spec); free(acc);
+    return err;
+}
+
+/* DIV and NABLA on a periodic plan (same passage; reading A27): psi_hat_c = rhs_sign F_c / Lambda as in
+ * orc_periodic (zero mode -> 0), then
+ *   kind 0 (DIV,   ncomp == nd): out = sum_a IDFT(i kappa_a psi_hat_a)
+ *   kind 1 (NABLA):              out_c = IDFT(sum_a (i kappa_a)^2 psi_hat_c)
+ * kappa_a = 2 pi m_a / L_a, zero at the Nyquist index (reading A20).  With op = 0 NABLA returns the source
+ * less its mean and its Nyquist planes; with op = 1 it returns the source filtered by kappa^2 / |Lambda_FD|. */
+int orc_periodic_divlap(int nd, const i64 n[3], const double L[3], int op, double rhs_sign, int ncomp,
+                        const double *f, int kind, double *out)
+{
+    if (nd < 1 || nd > 3 || (kind != 0 && kind != 1)) return ORC_ERR_ARG;
+    if (kind == 0 && ncomp != nd) return ORC_ERR_ARG;
+    i64 dims[3] = { n[0], nd > 1 ? n[1] : 1, nd > 2 ? n[2] : 1 };
+    i64 tot = dims[0] * dims[1] * dims[2];
+    for (int a = 0; a < 3; ++a) if (!is_pow2(dims[a])) return ORC_ERR_ARG;
+    cplx *F = (cplx *)malloc(sizeof(cplx) * (size_t)tot);
+    cplx *A = (kind == 0) ? (cplx *)calloc((size_t)tot, sizeof(cplx)) : NULL;
+    double *kap[3] = { 0, 0, 0 }, *lam[3] = { 0, 0, 0 };
+    int err = ORC_OK;
+    if (!F || (kind == 0 && !A)) { err = ORC_ERR_ALLOC; goto done; }
+    for (int a = 0; a < 3; ++a) {
+        i64 N = dims[a];
+        kap[a] = (double *)calloc((size_t)N, sizeof(double));
+        lam[a] = (double *)calloc((size_t)N, sizeof(double));
+        if (!kap[a] || !lam[a]) { err = ORC_ERR_ALLOC; goto done; }
+        if (a >= nd) continue;
+        double hh = L[a] / (double)N;
+        for (i64 k = 0; k < N; ++k) {
+            i64 m = (2 * k < N) ? k : k - N;
+            double kappa = 2.0 * PI * (double)m / L[a];
+            kap[a][k] = (2 * k == N) ? 0.0 : kappa;
+            if (op == 0) lam[a][k] = -kappa * kappa;
+            else {
+                double sn, cs;
+                sincos2pi(k, 2 * N, &sn, &cs);
+                lam[a][k] = -(4.0 / (hh * hh)) * sn * sn;
+            }
+        }
+    }
+    double inv_n = 1.0 / (double)tot;
+    for (int c = 0; c < ncomp; ++c) {
+        const double *fc = f + (size_t)c * (size_t)tot;
+#pragma omp parallel for schedule(static)
+        for (i64 i = 0; i < tot; ++i) F[i] = fc[i];
+        for (int a = 0; a < nd; ++a)
+            if ((err = fft_axis(F, dims, a, -1)) != ORC_OK) goto done;
+#pragma omp parallel for collapse(2) schedule(static)
+        for (i64 kz = 0; kz < dims[2]; ++kz)
+            for (i64 ky = 0; ky < dims[1]; ++ky)
+                for (i64 kx = 0; kx < dims[0]; ++kx) {
+                    i64 i = kx + dims[0] * (ky + dims[1] * kz);
+                    i64 kk[3] = { kx, ky, kz };
+                    cplx psi = 0.0;
+                    if (kx || ky || kz) psi = rhs_sign * F[i] / (lam[0][kx] + lam[1][ky] + lam[2][kz]);
+                    if (kind == 0) {
+                        A[i] += I * kap[c][kk[c]] * psi;
+                    } else {
+                        cplx s = 0.0;
+                        for (int a = 0; a < 3; ++a) s += (I * kap[a][kk[a]]) * (I * kap[a][kk[a]]) * psi;
+                        F[i] = s;
+                    }
+                }
+        if (kind == 1) {
+            for (int a = nd - 1; a >= 0; --a)
+                if ((err = fft_axis(F, dims, a, +1)) != ORC_OK) goto done;
+            double *oc = out + (size_t)c * (size_t)tot;
+#pragma omp parallel for schedule(static)
+            for (i64 i = 0; i < tot; ++i) oc[i] = creal(F[i]) * inv_n;
+        }
+    }
+    if (kind == 0) {
+        for (int a = nd - 1; a >= 0; --a)
+            if ((err = fft_axis(A, dims, a, +1)) != ORC_OK) goto done;
+#pragma omp parallel for schedule(static)
+        for (i64 i = 0; i < tot; ++i) out[i] = creal(A[i]) * inv_n;
+    }
+done:
+    for (int a = 0; a < 3; ++a) { free(kap[a]); free(lam[a]); }
+    free(F); free(A);
+    return err;
+}
+
 /* Direct O(N^6) evaluation of the definition above (scalar), for tiny grids only (pin P6). */
 void orc_unbounded_direct(const i64 n[3], const double h[3], double eps, double rhs_sign, const double *f,
                           double *psi)
