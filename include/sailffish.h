@@ -76,7 +76,9 @@ typedef enum { SF_MEM_HOST = 0, SF_MEM_DEVICE = 1 } sf_mem;
 typedef enum {
     SF_OUT_PSI = 0,  /* solution; comp = component (0 for scalar plans)                          */
     SF_OUT_GRAD = 1, /* after sf_gradient: comp = axis (0=x,1=y,2=z) of grad psi (scalar plans)   */
-    SF_OUT_CURL = 2  /* after sf_curl:     comp = component of curl psi (ncomp == 3 plans)        */
+    SF_OUT_CURL = 2, /* after sf_curl:     comp = component of curl psi (ncomp == 3 plans)        */
+    SF_OUT_DIV = 3,  /* after sf_divergence: div psi, comp = 0 (ncomp == 3 plans)                  */
+    SF_OUT_LAP = 4   /* after sf_laplacian:  lap psi, comp = component                            */
 } sf_field;
 
 typedef struct {
@@ -153,6 +155,19 @@ sf_status sf_gradient(sf_plan plan);
  * psi_hat) in the same spectral pass (eq. 17).  Wavenumbers on the
  * transform grid (doubled for unbounded plans).  psi itself is not produced by this call. */
 sf_status sf_curl(sf_plan plan);
+
+/* sf_divergence -- the paper's DIV operator: ncomp == 3 plans; solve the three components
+ * and return div psi = IDFT(sum_a i k_a psi_hat_a) in the same spectral pass (three spectra in, one
+ * out).  Wavenumbers as for sf_curl (transform grid, zero at the Nyquist index).  Periodic and
+ * unbounded plans; psi itself is not produced.  Read the result with SF_OUT_DIV. */
+sf_status sf_divergence(sf_plan plan);
+
+/* sf_laplacian -- the paper's NABLA operator: for every component lap psi =
+ * IDFT(sum_a (i k_a)^2 psi_hat), i.e. DIV of GRAD with the same k_a (zero at the Nyquist index).  With
+ * the pseudo-spectral operator this returns the source less its mean and Nyquist planes; with FD2 or
+ * a regularised Green's function the source filtered by k^2 / |symbol|.  Periodic and unbounded plans;
+ * psi itself is not produced.  Read the result with SF_OUT_LAP. */
+sf_status sf_laplacian(sf_plan plan);
 
 /*
  * sf_get_output -- the paper's Get_Output.

@@ -24,12 +24,12 @@ SF_OP_PSEUDO_SPECTRAL, SF_OP_FD2, SF_OP_GREEN_GAUSS2, SF_OP_GREEN_GAUSS4, SF_OP_
 SF_OP_GREEN_GAUSS8, SF_OP_GREEN_GAUSS10, SF_OP_GREEN_SPECTRAL = 5, 6, 7
 SF_F32, SF_F64 = 0, 1
 SF_MEM_HOST, SF_MEM_DEVICE = 0, 1
-SF_OUT_PSI, SF_OUT_GRAD, SF_OUT_CURL = 0, 1, 2
+SF_OUT_PSI, SF_OUT_GRAD, SF_OUT_CURL, SF_OUT_DIV, SF_OUT_LAP = 0, 1, 2, 3, 4
 
 # every symbol include/sailffish.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = (
     "sf_plan_create", "sf_set_source", "sf_set_bc_values", "sf_solve", "sf_gradient", "sf_curl",
-    "sf_get_output", "sf_output_device_ptr", "sf_synchronize", "sf_last_launch_count", "sf_device_bytes",
+    "sf_divergence", "sf_laplacian", "sf_get_output", "sf_output_device_ptr", "sf_synchronize", "sf_last_launch_count", "sf_device_bytes",
     "sf_enable_step_timing", "sf_step_times_ms", "sf_set_step_timing_stride", "sf_last_error", "sf_plan_destroy", "sf_version",
 )
 
@@ -63,6 +63,8 @@ def lib() -> C.CDLL:
         L.sf_solve.argtypes = [vp]
         L.sf_gradient.argtypes = [vp]
         L.sf_curl.argtypes = [vp]
+        L.sf_divergence.argtypes = [vp]
+        L.sf_laplacian.argtypes = [vp]
         L.sf_get_output.argtypes = [vp, i, i, vp, i]
         L.sf_output_device_ptr.argtypes = [vp, i, i, C.POINTER(vp)]
         L.sf_synchronize.argtypes = [vp]
@@ -145,6 +147,14 @@ def sf_gradient(plan):
 
 def sf_curl(plan):
     _check(plan, lib().sf_curl(plan))
+
+
+def sf_divergence(plan):
+    _check(plan, lib().sf_divergence(plan))
+
+
+def sf_laplacian(plan):
+    _check(plan, lib().sf_laplacian(plan))
 
 
 def sf_get_output(plan, field, comp, dst):

@@ -401,7 +401,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
     const int n0 = (int)p->n[0], n1 = (int)p->n[1], n2 = (nd == 3) ? (int)p->n[2] : 1;
     const long long hp = p->pitch;
     const int ncomp = p->ncomp;
-    const int nf_out = (outk == OUT_GRAD) ? 1 + nd : ncomp;
+    const int nf_out = (outk == OUT_GRAD) ? 1 + nd : (outk == OUT_DIV ? 1 : ncomp);
     const int P1 = p->padded ? 2 * n1 : n1;
     cudaStream_t st = p->stream;
     p->launches = 0;
@@ -495,7 +495,6 @@ template <typename T> sf_status run(sf_plan p, int outk)
         mark(5);
         if (timed) p->tcount++;
         p->last_kind = outk;
-    p->out_last = p->out;
         p->out_last = p->out;
         return SF_OK;
     }
@@ -534,8 +533,8 @@ template <typename T> sf_status run(sf_plan p, int outk)
         sp.n_in = nlast; sp.n_out = nlast;
         sp.LT = p->LT[ax]; sp.tw = (const C*)p->tw[ax]; sp.ptw = (const C*)p->ptw[ax];
         const int nb = (nd == 3) ? P1 : 1;
-        const int nbuf = (outk == OUT_CURL) ? 3 : (outk == OUT_GRAD ? 2 : 1);
-        const int gz = (outk == OUT_SOLVE) ? ncomp : 1;
+        const int nbuf = (outk == OUT_CURL || outk == OUT_DIV) ? 3 : (outk == OUT_GRAD ? 2 : 1);
+        const int gz = (outk == OUT_SOLVE || outk == OUT_LAP) ? ncomp : 1;
         SF_CUDA(p, launch_spass<T>(p->La[ax], 2, sp, nb, gz, nbuf, st));
         p->launches++;
     }
@@ -822,13 +821,31 @@ sf_status sf_curl(sf_plan plan)
     return run_any(plan, OUT_CURL);
 }
 
+sf_status sf_divergence(sf_plan plan)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (plan->ncomp != 3) return fail(plan, SF_ERR_UNSUPPORTED, "sf_divergence needs an ncomp == 3 plan");
+    if (plan->bc != SF_BC_PERIODIC && plan->bc != SF_BC_UNBOUNDED)
+        return fail(plan, SF_ERR_UNSUPPORTED, "sf_divergence is built for periodic and unbounded plans");
+    return run_any(plan, OUT_DIV);
+}
+
+sf_status sf_laplacian(sf_plan plan)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (plan->bc != SF_BC_PERIODIC && plan->bc != SF_BC_UNBOUNDED)
+        return fail(plan, SF_ERR_UNSUPPORTED, "sf_laplacian is built for periodic and unbounded plans");
+    return run_any(plan, OUT_LAP);
+}
+
 sf_status sf_output_device_ptr(sf_plan plan, int field, int comp, void** ptr)
 {
     if (!plan || !ptr) return SF_ERR_INVALID_ARG;
     int idx = -1;
     if (plan->last_kind < 0) return fail(plan, SF_ERR_STATE, "no result yet: call sf_solve / sf_gradient / sf_curl first");
     if (field == SF_OUT_PSI) {
-        if (plan->last_kind == OUT_CURL) return fail(plan, SF_ERR_STATE, "sf_curl does not produce psi");
+        if (plan->last_kind != OUT_SOLVE && plan->last_kind != OUT_GRAD)
+            return fail(plan, SF_ERR_STATE, "psi was not produced by the last call (sf_curl, sf_divergence and sf_laplacian return only their own field)");
         if (comp < 0 || comp >= plan->ncomp) return fail(plan, SF_ERR_INVALID_ARG, "component out of range");
         idx = comp;
     } else if (field == SF_OUT_GRAD) {
@@ -838,6 +855,14 @@ sf_status sf_output_device_ptr(sf_plan plan, int field, int comp, void** ptr)
     } else if (field == SF_OUT_CURL) {
         if (plan->last_kind != OUT_CURL) return fail(plan, SF_ERR_STATE, "curl was not produced by the last call");
         if (comp < 0 || comp >= 3) return fail(plan, SF_ERR_INVALID_ARG, "component out of range");
+        idx = comp;
+    } else if (field == SF_OUT_DIV) {
+        if (plan->last_kind != OUT_DIV) return fail(plan, SF_ERR_STATE, "divergence was not produced by the last call");
+        if (comp != 0) return fail(plan, SF_ERR_INVALID_ARG, "the divergence is one field: comp must be 0");
+        idx = 0;
+    } else if (field == SF_OUT_LAP) {
+        if (plan->last_kind != OUT_LAP) return fail(plan, SF_ERR_STATE, "Laplacian was not produced by the last call");
+        if (comp < 0 || comp >= plan->ncomp) return fail(plan, SF_ERR_INVALID_ARG, "component out of range");
         idx = comp;
     } else {
         return fail(plan, SF_ERR_INVALID_ARG, "unknown field");

@@ -11,8 +11,8 @@
 // kernels fold the permutation into the global row address.
 //   MODE 0: forward only   (S2; also plan-time transforms of the Green's function)
 //   MODE 1: backward only  (S4)
-//   MODE 2: forward, multiply, backward (S3) with 1 -> 1 (solve), 1 -> 1+d (gradient) or
-//           3 -> 3 (curl) fields
+//   MODE 2: forward, multiply, backward (S3) with 1 -> 1 (solve, Laplacian), 1 -> 1+d (gradient),
+//           3 -> 3 (curl) or 3 -> 1 (divergence) fields
 // Zero padding is fused into the load (rows >= n_in are zeros), truncation into the store (rows
 // >= n_out are dropped).  Dirichlet / Neumann pencils are real: they are extended (odd / even) to
 // length 2L on load, packed as L complex numbers, and the real-transform split / merge steps are
@@ -23,7 +23,7 @@
 namespace sf {
 
 enum { MUL_SYMBOL = 0, MUL_GREEN = 1 };
-enum { OUT_SOLVE = 0, OUT_GRAD = 1, OUT_CURL = 2 };
+enum { OUT_SOLVE = 0, OUT_GRAD = 1, OUT_CURL = 2, OUT_DIV = 3, OUT_LAP = 4 };
 enum { R2R_NONE = 0, R2R_DST1 = 1, R2R_DCT = 2 };
 
 template <typename T> struct SParams {
@@ -89,7 +89,8 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
     const int ib = blockIdx.y;
     const int tx_ = threadIdx.x % TX;
     const bool xok = (x0 + tx_) < p.nx;          // a thread keeps its column in every tx-fastest loop
-    const bool curl = (MODE == 2) && (p.outk == OUT_CURL);
+    const bool div = (MODE == 2) && (p.outk == OUT_DIV);
+    const bool curl = (MODE == 2) && (p.outk == OUT_CURL || div);   // all three spectra in one CTA
     const int nfield_in = curl ? 3 : 1;
     const long long fz = curl ? 0 : blockIdx.z;   // independent components ride on gridDim.z
 
@@ -147,9 +148,27 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
         if constexpr (MODE == 2) {
             const int kx = min(x0 + tx_, p.nx - 1);
             if (!curl) {
+                const bool lap = (p.outk == OUT_LAP);
+                const T qx = __ldg(p.kap_x + kx), qy = __ldg(p.kap_b + ib);
                 for (int idx = threadIdx.x; idx < TILE; idx += NT) {
                     const int kp = k_of_pos<L>(idx / TX);
-                    s0[idx] = cscale(s0[idx], s_multiplier(p, kx, ib, kp));
+                    T m = s_multiplier(p, kx, ib, kp);
+                    if (lap) {
+                        // NABLA = DIV of GRAD: (i kappa)^2 summed over the axes
+                        const T qz = __ldg(p.kap_p + kp);
+                        m *= -(qx * qx + qy * qy + qz * qz);
+                    }
+                    s0[idx] = cscale(s0[idx], m);
+                }
+            } else if (div) {
+                const T qx = __ldg(p.kap_x + kx), qy = __ldg(p.kap_b + ib);
+                for (int idx = threadIdx.x; idx < TILE; idx += NT) {
+                    const int kp = k_of_pos<L>(idx / TX);
+                    const T m = s_multiplier(p, kx, ib, kp);
+                    const T qz = __ldg(p.kap_p + kp);
+                    const C a = s0[idx], b = s0[TILE + idx], c = s0[2 * TILE + idx];
+                    // div psi = i kappa . psi
+                    s0[idx] = cmuli(mk<T>(m * (qx * a.x + qy * b.x + qz * c.x), m * (qx * a.y + qy * b.y + qz * c.y)));
                 }
             } else {
                 const T qx = __ldg(p.kap_x + kx), qy = __ldg(p.kap_b + ib);
@@ -168,7 +187,7 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
         }
         if constexpr (MODE != 0) {
             const int nd = (MODE == 2 && p.outk == OUT_GRAD) ? p.pencil_axis + 1 : 0;
-            const int nfield_out = curl ? 3 : 1 + nd;
+            const int nfield_out = div ? 1 : (curl ? 3 : 1 + nd);
             // gradient fields first (they are derived from buffer 0 into buffer 1), psi last
             for (int f = nfield_out - 1; f >= 0; --f) {
                 C* s = s0;
