@@ -117,6 +117,18 @@ def dct3(x):
     return _r2r("orc_dct3_direct", x)
 
 
+def dst2(x):
+    return _r2r("orc_dst2_direct", x)
+
+
+def dst3(x):
+    return _r2r("orc_dst3_direct", x)
+
+
+def dct1(x):
+    return _r2r("orc_dct1_direct", x)
+
+
 # ---------------------------------------------------------------- solvers
 def _dims(shape):
     """numpy shape (z, y, x) / (y, x) -> (nd, n[3]) with x first."""
@@ -185,6 +197,30 @@ def dirichlet_regular(f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
     arr, keep = _faces_arg(faces)
     _chk(lib().orc_dirichlet_regular(_i64x3(n), _f64x3(h), C.c_int(op), C.c_double(rhs_sign), _ptr(f), arr,
                                      _ptr(psi)), "dirichlet_regular")
+    return psi
+
+
+def dirichlet_staggered(f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
+    """O-DIRS.  Dirichlet on a cell-centre grid (DST-II / DST-III); conventions as dirichlet_regular."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    assert nd == 3
+    psi = np.empty_like(f)
+    arr, keep = _faces_arg(faces)
+    _chk(lib().orc_dirichlet_staggered(_i64x3(n), _f64x3(h), C.c_int(op), C.c_double(rhs_sign), _ptr(f), arr,
+                                       _ptr(psi)), "dirichlet_staggered")
+    return psi
+
+
+def neumann_regular(f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
+    """O-NEUR.  Neumann on a cell-boundary grid, boundary nodes stored (DCT-I); conventions as neumann_staggered."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    assert nd == 3
+    psi = np.empty_like(f)
+    arr, keep = _faces_arg(faces)
+    _chk(lib().orc_neumann_regular(_i64x3(n), _f64x3(h), C.c_int(op), C.c_double(rhs_sign), _ptr(f), arr,
+                                   _ptr(psi)), "neumann_regular")
     return psi
 
 

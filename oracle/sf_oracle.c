@@ -208,6 +208,53 @@ void orc_dct3_direct(int n, const double *in, double *out)
     }
 }
 
+/* DST-II: Y_k = 2 sum_{j=0}^{N-1} X_j sin(pi (j+1/2) (k+1) / N)   (Table 1 row 2; odd extension about the
+ * faces of a cell-centre grid) */
+void orc_dst2_direct(int n, const double *in, double *out)
+{
+    i64 q = 4 * (i64)n;
+    for (int k = 0; k < n; ++k) {
+        long double acc = 0.0L;
+        for (int j = 0; j < n; ++j) {
+            double s, c;
+            sincos2pi((i64)(2 * j + 1) * (k + 1), q, &s, &c);
+            acc += (long double)in[j] * s;
+        }
+        out[k] = (double)(2.0L * acc);
+    }
+}
+
+/* DST-III: Y_j = (-1)^j X_{N-1} + 2 sum_{k=0}^{N-2} X_k sin(pi (k+1) (j+1/2) / N)   (inverse of DST-II up to 2N) */
+void orc_dst3_direct(int n, const double *in, double *out)
+{
+    i64 q = 4 * (i64)n;
+    for (int j = 0; j < n; ++j) {
+        long double acc = 0.0L;
+        for (int k = 0; k + 1 < n; ++k) {
+            double s, c;
+            sincos2pi((i64)(2 * j + 1) * (k + 1), q, &s, &c);
+            acc += (long double)in[k] * s;
+        }
+        out[j] = (double)(((j & 1) ? -1.0L : 1.0L) * (long double)in[n - 1] + 2.0L * acc);
+    }
+}
+
+/* DCT-I: Y_k = X_0 + (-1)^k X_{N-1} + 2 sum_{j=1}^{N-2} X_j cos(pi j k / (N-1))   (Table 1 row 3; even extension
+ * about the end nodes of a cell-boundary grid; its own inverse up to 2 (N-1)) */
+void orc_dct1_direct(int n, const double *in, double *out)
+{
+    i64 q = 2 * (i64)(n - 1);
+    for (int k = 0; k < n; ++k) {
+        long double acc = 0.0L;
+        for (int j = 1; j + 1 < n; ++j) {
+            double s, c;
+            sincos2pi((i64)j * k, q, &s, &c);
+            acc += (long double)in[j] * c;
+        }
+        out[k] = (double)((long double)in[0] + ((k & 1) ? -1.0L : 1.0L) * (long double)in[n - 1] + 2.0L * acc);
+    }
+}
+
 /* ------------------------------------------------------------------------------------------
  * Table-driven versions of the same sums for the N-D solvers (the table is the list of all
  * sin / cos values of the reduced integer argument; the sum is unchanged).
@@ -253,6 +300,37 @@ static void dct3_tab(const trig_table *t, const double *in, double *out)
         for (int k = 1; k < n; ++k)
             acc += (long double)in[k] * t->cs[((i64)(2 * j + 1) * k) % t->q];
         out[j] = (double)((long double)in[0] + 2.0L * acc);
+    }
+}
+
+static void dst2_tab(const trig_table *t, const double *in, double *out)
+{
+    int n = t->n;
+    for (int k = 0; k < n; ++k) {
+        long double acc = 0.0L;
+        for (int j = 0; j < n; ++j)
+            acc += (long double)in[j] * t->sn[((i64)(2 * j + 1) * (k + 1)) % t->q];
+        out[k] = (double)(2.0L * acc);
+    }
+}
+static void dst3_tab(const trig_table *t, const double *in, double *out)
+{
+    int n = t->n;
+    for (int j = 0; j < n; ++j) {
+        long double acc = 0.0L;
+        for (int k = 0; k + 1 < n; ++k)
+            acc += (long double)in[k] * t->sn[((i64)(2 * j + 1) * (k + 1)) % t->q];
+        out[j] = (double)(((j & 1) ? -1.0L : 1.0L) * (long double)in[n - 1] + 2.0L * acc);
+    }
+}
+static void dct1_tab(const trig_table *t, const double *in, double *out)
+{
+    int n = t->n;
+    for (int k = 0; k < n; ++k) {
+        long double acc = 0.0L;
+        for (int j = 1; j + 1 < n; ++j)
+            acc += (long double)in[j] * t->cs[((i64)j * k) % t->q];
+        out[k] = (double)((long double)in[0] + ((k & 1) ? -1.0L : 1.0L) * (long double)in[n - 1] + 2.0L * acc);
     }
 }
 
@@ -556,6 +634,140 @@ int orc_neumann_staggered(const i64 n[3], const double h[3], int op, double rhs_
             }
     for (int a = 2; a >= 0; --a)
         if ((err = r2r_axis(psi, n, a, dct3_tab, &tab[a])) != ORC_OK) goto done;
+#pragma omp parallel for schedule(static)
+    for (i64 i = 0; i < tot; ++i) psi[i] /= norm;
+done:
+    for (int a = 0; a < ntab; ++a) trig_table_free(&tab[a]);
+    for (int a = 0; a < 3; ++a) free(lam[a]);
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * The other two rows of Table 1.
+ *
+ * O-DIRS: Dirichlet, cell-centre (STAGGERED) grid, DST-II forward, DST-III backward.  n = cells per axis,
+ * x_j = (j+1/2) h, faces at 0 and L = n h.  The ghost cell psi_ghost = 2 g - psi_first puts the face value g
+ * between the two cell centres, so the folded source is f' = f - 2 g / h^2 in the boundary-adjacent layer
+ * (reading A18).
+ *   op = 1 (FD2): Lambda = -sum_a (4/h_a^2) sin^2(pi (k_a+1) / (2 N_a))
+ *   op = 0 (PS):  Lambda = -sum_a (pi (k_a+1) / L_a)^2                     (homogeneous faces only)
+ * psi = DST-III_3(rhs_sign * DST-II_3(f') / Lambda) / prod_a (2 N_a).
+ *
+ * O-NEUR: Neumann, cell-boundary (REGULAR) grid, DCT-I forward and backward.  n = nodes per axis including the
+ * two boundary nodes, x_j = j h, L = (n-1) h.  The ghost node psi_ghost = psi_second -/+ 2 h g mirrors about
+ * the boundary node, so f' = f + 2 g_lo / h on the first layer and f - 2 g_hi / h on the last (reading A18).
+ *   op = 1 (FD2): Lambda = -sum_a (4/h_a^2) sin^2(pi k_a / (2 (N_a-1)))
+ *   op = 0 (PS):  Lambda = -sum_a (pi k_a / L_a)^2
+ * Zero mode -> 0.  psi = DCT-I_3(rhs_sign * DCT-I_3(f') / Lambda) / prod_a (2 (N_a-1)).
+ * ---------------------------------------------------------------------------------------- */
+static void fold_faces_f3(double *fp, const i64 n[3], const double h[3], const double *const faces[6], int neumann)
+{
+    for (int axis = 0; axis < 3; ++axis) {
+        int a = (axis == 0) ? 1 : 0;
+        int b = (axis == 2) ? 1 : 2;
+        i64 st[3] = { 1, n[0], n[0] * n[1] };
+        for (int side = 0; side < 2; ++side) {
+            const double *g = faces ? faces[2 * axis + side] : NULL;
+            if (!g) continue;
+            i64 ic = side ? n[axis] - 1 : 0;
+            double w;
+            if (!neumann) w = -2.0 / (h[axis] * h[axis]);          /* Dirichlet, cell-centre   */
+            else w = side ? -2.0 / h[axis] : +2.0 / h[axis];       /* Neumann, cell-boundary   */
+            for (i64 jb = 0; jb < n[b]; ++jb)
+                for (i64 ja = 0; ja < n[a]; ++ja)
+                    fp[ic * st[axis] + ja * st[a] + jb * st[b]] += w * g[ja + n[a] * jb];
+        }
+    }
+}
+
+int orc_dirichlet_staggered(const i64 n[3], const double h[3], int op, double rhs_sign, const double *f,
+                            const double *const faces[6], double *psi)
+{
+    i64 tot = n[0] * n[1] * n[2];
+    trig_table tab[3];
+    double *lam[3] = { 0, 0, 0 };
+    int err = ORC_OK, ntab = 0;
+    memcpy(psi, f, sizeof(double) * (size_t)tot);
+    if (op == 1) fold_faces_f3(psi, n, h, faces, 0);
+    for (int a = 0; a < 3; ++a) {
+        if ((err = trig_table_init(&tab[a], (int)n[a], 4 * n[a])) != ORC_OK) { ntab = a + 1; goto done; }
+        ntab = a + 1;
+        lam[a] = (double *)malloc(sizeof(double) * (size_t)n[a]);
+        if (!lam[a]) { err = ORC_ERR_ALLOC; goto done; }
+        double Ldom = (double)n[a] * h[a];
+        for (i64 k = 0; k < n[a]; ++k) {
+            if (op == 0) {
+                double kk = PI * (double)(k + 1) / Ldom;
+                lam[a][k] = -kk * kk;
+            } else {
+                double s, c;
+                sincos2pi(k + 1, 4 * n[a], &s, &c); /* sin(pi (k+1) / (2N)) */
+                lam[a][k] = -(4.0 / (h[a] * h[a])) * s * s;
+            }
+        }
+    }
+    for (int a = 0; a < 3; ++a)
+        if ((err = r2r_axis(psi, n, a, dst2_tab, &tab[a])) != ORC_OK) goto done;
+    double norm = 1.0;
+    for (int a = 0; a < 3; ++a) norm *= 2.0 * (double)n[a];
+#pragma omp parallel for collapse(2) schedule(static)
+    for (i64 kz = 0; kz < n[2]; ++kz)
+        for (i64 ky = 0; ky < n[1]; ++ky)
+            for (i64 kx = 0; kx < n[0]; ++kx) {
+                i64 i = kx + n[0] * (ky + n[1] * kz);
+                psi[i] = rhs_sign * psi[i] / (lam[0][kx] + lam[1][ky] + lam[2][kz]);
+            }
+    for (int a = 2; a >= 0; --a)
+        if ((err = r2r_axis(psi, n, a, dst3_tab, &tab[a])) != ORC_OK) goto done;
+#pragma omp parallel for schedule(static)
+    for (i64 i = 0; i < tot; ++i) psi[i] /= norm;
+done:
+    for (int a = 0; a < ntab; ++a) trig_table_free(&tab[a]);
+    for (int a = 0; a < 3; ++a) free(lam[a]);
+    return err;
+}
+
+int orc_neumann_regular(const i64 n[3], const double h[3], int op, double rhs_sign, const double *f,
+                        const double *const faces[6], double *psi)
+{
+    i64 tot = n[0] * n[1] * n[2];
+    trig_table tab[3];
+    double *lam[3] = { 0, 0, 0 };
+    int err = ORC_OK, ntab = 0;
+    for (int a = 0; a < 3; ++a) if (n[a] < 2) return ORC_ERR_ARG;
+    memcpy(psi, f, sizeof(double) * (size_t)tot);
+    if (op == 1) fold_faces_f3(psi, n, h, faces, 1);
+    for (int a = 0; a < 3; ++a) {
+        if ((err = trig_table_init(&tab[a], (int)n[a], 2 * (n[a] - 1))) != ORC_OK) { ntab = a + 1; goto done; }
+        ntab = a + 1;
+        lam[a] = (double *)malloc(sizeof(double) * (size_t)n[a]);
+        if (!lam[a]) { err = ORC_ERR_ALLOC; goto done; }
+        double Ldom = (double)(n[a] - 1) * h[a];
+        for (i64 k = 0; k < n[a]; ++k) {
+            if (op == 0) {
+                double kk = PI * (double)k / Ldom;
+                lam[a][k] = -kk * kk;
+            } else {
+                double s, c;
+                sincos2pi(k, 4 * (n[a] - 1), &s, &c); /* sin(pi k / (2 (N-1))) */
+                lam[a][k] = -(4.0 / (h[a] * h[a])) * s * s;
+            }
+        }
+    }
+    for (int a = 0; a < 3; ++a)
+        if ((err = r2r_axis(psi, n, a, dct1_tab, &tab[a])) != ORC_OK) goto done;
+    double norm = 1.0;
+    for (int a = 0; a < 3; ++a) norm *= 2.0 * (double)(n[a] - 1);
+#pragma omp parallel for collapse(2) schedule(static)
+    for (i64 kz = 0; kz < n[2]; ++kz)
+        for (i64 ky = 0; ky < n[1]; ++ky)
+            for (i64 kx = 0; kx < n[0]; ++kx) {
+                i64 i = kx + n[0] * (ky + n[1] * kz);
+                if (kx == 0 && ky == 0 && kz == 0) { psi[i] = 0.0; continue; }
+                psi[i] = rhs_sign * psi[i] / (lam[0][kx] + lam[1][ky] + lam[2][kz]);
+            }
+    for (int a = 2; a >= 0; --a)
+        if ((err = r2r_axis(psi, n, a, dct1_tab, &tab[a])) != ORC_OK) goto done;
 #pragma omp parallel for schedule(static)
     for (i64 i = 0; i < tot; ++i) psi[i] /= norm;
 done:

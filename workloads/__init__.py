@@ -178,6 +178,61 @@ def neumann3d_manufactured(nc: int = 256, seed: int | None = None, inhomogeneous
     return {"f": f, "u": u, "faces": faces, "h": (h, h, h), "n": (n, n, n), "m": m, "a": a, "b": b, "x": x}
 
 
+def dirichlet3d_centre_manufactured(nc: int = 256, seed: int | None = None, inhomogeneous: bool = True, modes=None):
+    """The Dirichlet problem of config 3 on a cell-centre grid (Table 1 row 2): x_j = (j+1/2) h, j < nc,
+    h = 1/nc; faces carry u = q on the domain faces x_a = 0, 1 at the cell centres of the other two axes."""
+    m, a, b = _bounded_params(seed_for(3) if seed is None else seed)
+    if modes is not None:
+        m = np.asarray(modes, dtype=np.int64)
+    if not inhomogeneous:
+        a = np.zeros(3)
+        b = np.zeros(3)
+    n = nc
+    h = 1.0 / nc
+    x = (np.arange(n) + 0.5) * h
+    xs = (x, x, x)
+    sx, sy, sz = (np.sin(m[i] * np.pi * x) for i in range(3))
+    prod = sz[:, None, None] * sy[None, :, None] * sx[None, None, :]
+    u = prod + _quad(xs, a, b)
+    f = -(np.pi ** 2) * float(np.sum(m ** 2)) * prod + 2.0 * float(np.sum(a + b))
+    faces = {}
+    if inhomogeneous:
+        for axis in range(3):
+            rem = [i for i in range(3) if i != axis]
+            for side in (0, 1):
+                xb = float(side)
+                qa = a[axis] * (1 - xb) ** 2 + b[axis] * xb ** 2
+                q_lo = a[rem[0]] * (1 - x) ** 2 + b[rem[0]] * x ** 2
+                q_hi = a[rem[1]] * (1 - x) ** 2 + b[rem[1]] * x ** 2
+                faces[(axis, side)] = qa + q_hi[:, None] + q_lo[None, :]
+    return {"f": f, "u": u, "faces": faces, "h": (h, h, h), "n": (n, n, n), "m": m, "a": a, "b": b, "x": x}
+
+
+def neumann3d_boundary_manufactured(nc: int = 256, seed: int | None = None, inhomogeneous: bool = True, modes=None):
+    """The Neumann problem of config 3 on a cell-boundary grid (Table 1 row 3): nodes x_j = j h, j <= nc,
+    h = 1/nc, boundary nodes stored (nc + 1 per axis); faces carry d q / d x_axis (along +axis)."""
+    m, a, b = _bounded_params(seed_for(3) if seed is None else seed)
+    if modes is not None:
+        m = np.asarray(modes, dtype=np.int64)
+    if not inhomogeneous:
+        a = np.zeros(3)
+        b = np.zeros(3)
+    n = nc + 1
+    h = 1.0 / nc
+    x = np.arange(n) * h
+    xs = (x, x, x)
+    cx, cy, cz = (np.cos(m[i] * np.pi * x) for i in range(3))
+    prod = cz[:, None, None] * cy[None, :, None] * cx[None, None, :]
+    u = prod + _quad(xs, a, b)
+    f = -(np.pi ** 2) * float(np.sum(m ** 2)) * prod + 2.0 * float(np.sum(a + b))
+    faces = {}
+    if inhomogeneous:
+        for axis in range(3):
+            faces[(axis, 0)] = np.full((n, n), -2.0 * a[axis])
+            faces[(axis, 1)] = np.full((n, n), +2.0 * b[axis])
+    return {"f": f, "u": u, "faces": faces, "h": (h, h, h), "n": (n, n, n), "m": m, "a": a, "b": b, "x": x}
+
+
 # ------------------------------------------------------------------------------------------------
 # config 4: unbounded, [0,1]^3 cell-centre, 16 Gaussian blobs
 # ------------------------------------------------------------------------------------------------
