@@ -10,7 +10,9 @@
  *     1. forward transform of the source along every axis
  *        - periodic:  real-to-complex DFT                        (eq. 8)
  *        - Dirichlet, cell-boundary grid:  DST-I                 (Table 1 row 1)
- *        - Neumann,   cell-centre   grid:  DCT-II                (Table 1 row 4)
+ *        - Dirichlet, cell-centre   grid:  DST-II  (back: DST-III)  (Table 1 row 2)
+ *        - Neumann,   cell-boundary grid:  DCT-I                 (Table 1 row 3)
+ *        - Neumann,   cell-centre   grid:  DCT-II  (back: DCT-III)  (Table 1 row 4)
  *        - unbounded: zero-padded to twice the length, real-to-complex DFT
  *                     (Hockney-Eastwood, sec 2.5; only non-zero pencils are
  *                     transformed -- the "pruned" variant of PAPER.md:213)
@@ -95,15 +97,16 @@ typedef struct {
  *                           allocates (all on the current CUDA device) until sf_plan_destroy.
  *   ndim   2 or 3.
  *   n      [host] stored unknowns per axis (n[a] for a >= ndim is ignored and treated as 1).
- *          periodic, Neumann cell-centre, unbounded: n[a] a power of two >= 8 (x) / >= 4 (y, z);
- *          Dirichlet cell-boundary: n[a] = 2^k - 1 interior nodes (boundary nodes are not stored).
+ *          periodic, unbounded, Neumann cell-centre, Dirichlet cell-centre: n[a] a power of two >= 8 (x) /
+ *          >= 4 (y, z); Dirichlet cell-boundary: n[a] = 2^k - 1 interior nodes (boundary nodes are not
+ *          stored); Neumann cell-boundary: n[a] = 2^k + 1 nodes (boundary nodes are stored).
  *          Upper bound 4096 per axis (2048 for unbounded, whose transforms are 2 n[a] long).
  *   h      [host] grid spacing per axis.  Domain length follows (Table 1): periodic
- *          and cell-centre L = n h; Dirichlet cell-boundary L = (n + 1) h.
+ *          and cell-centre L = n h; Dirichlet cell-boundary L = (n + 1) h; Neumann cell-boundary L = (n - 1) h.
  *   bc     [host] boundary condition per axis; all axes must agree.
- *   grid   Dirichlet requires SF_GRID_CELL_BOUNDARY, Neumann SF_GRID_CELL_CENTRE (the other two
- *          Table-1 rows are not built yet: SF_ERR_UNSUPPORTED); periodic and unbounded accept both
- *          (identical numerics).
+ *   grid   selects the row of Table 1: Dirichlet cell-boundary DST-I, Dirichlet
+ *          cell-centre DST-II / DST-III, Neumann cell-boundary DCT-I, Neumann cell-centre DCT-II /
+ *          DCT-III; periodic and unbounded accept both (identical numerics).
  *   op     PS / FD2 for periodic, Dirichlet, Neumann; GREEN_GAUSS2 .. GREEN_GAUSS10 or GREEN_SPECTRAL for unbounded (3-D only).
  *   prec   arithmetic and storage type of every array passed later.
  *   opt    [host] may be NULL (defaults above).
@@ -132,9 +135,12 @@ sf_status sf_set_source(sf_plan plan, const void* src, sf_mem where);
  *   axis 0..ndim-1, side 0 = lower face, 1 = upper face.
  *   face   values over the two remaining axes, lower axis fastest (for axis 0: iy + n[1]*iz; axis 1:
  *          ix + n[0]*iz; axis 2: ix + n[0]*iy); NULL resets the face to homogeneous.
- *          Dirichlet: psi on the boundary node next to the layer; weight -1/h^2.
+ *          Dirichlet: psi on the face; cell-boundary grids: the boundary node next to the layer,
+ *                     weight -1/h^2; cell-centre grids: the face half a cell outside the layer
+ *                     (ghost cell 2 g - psi), weight -2/h^2.
  *          Neumann:   d psi / d x_axis along +axis on both faces (eq. 15);
- *                     weights +1/h (lower), -1/h (upper).
+ *                     cell-centre grids: weights +1/h (lower), -1/h (upper); cell-boundary grids
+ *                     (ghost node mirrored through the boundary node): +2/h, -2/h.
  *   where  as for sf_set_source (device pointers borrowed, host data copied).
  * Errors: UNSUPPORTED for periodic / unbounded plans or the PS operator.
  */

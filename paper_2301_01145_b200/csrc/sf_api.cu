@@ -152,8 +152,8 @@ template <typename T> sf_status upload_twiddles(sf_plan p, void** dst, int len)
 // exp(-i pi k / (2 n)), k < n  (quarter-wave shift of the DCT-II / DCT-III)
 template <typename T> sf_status upload_dct_shift(sf_plan p, void** dst, int n)
 {
-    std::vector<T> h((size_t)2 * n);
-    for (int k = 0; k < n; ++k) {
+    std::vector<T> h((size_t)2 * (n + 1));   // k = 0 .. n (DST-II uses the entry k = n, -i)
+    for (int k = 0; k <= n; ++k) {
         long double a = PI_L * (long double)k / (2.0L * (long double)n);
         h[2 * k] = (T)cosl(a);
         h[2 * k + 1] = (T)(-sinl(a));
@@ -196,15 +196,19 @@ void axis_tables(const sf_plan_s& pl, int a, int count, std::vector<long double>
             break;
         }
         case SF_BC_DIRICHLET: {
-            const long double Ld = (long double)(n + 1) * h;
+            // cell-boundary: n interior nodes, L = (n+1) h (DST-I); cell-centre: n cells, L = n h (DST-II)
+            const long double cells = (pl.grid == SF_GRID_CELL_BOUNDARY) ? (long double)(n + 1) : (long double)n;
+            const long double Ld = cells * h;
             if (pl.op == SF_OP_PSEUDO_SPECTRAL) { long double kk = PI_L * (long double)(k + 1) / Ld; lam[k] = -kk * kk; }
-            else { long double s = sinl(PI_L * (long double)(k + 1) / (2.0L * (long double)(n + 1))); lam[k] = -(4.0L / (h * h)) * s * s; }
+            else { long double s = sinl(PI_L * (long double)(k + 1) / (2.0L * cells)); lam[k] = -(4.0L / (h * h)) * s * s; }
             break;
         }
         case SF_BC_NEUMANN: {
-            const long double Ld = (long double)n * h;
+            // cell-centre: n cells, L = n h (DCT-II); cell-boundary: n nodes, L = (n-1) h (DCT-I)
+            const long double cells = (pl.grid == SF_GRID_CELL_CENTRE) ? (long double)n : (long double)(n - 1);
+            const long double Ld = cells * h;
             if (pl.op == SF_OP_PSEUDO_SPECTRAL) { long double kk = PI_L * (long double)k / Ld; lam[k] = -kk * kk; }
-            else { long double s = sinl(PI_L * (long double)k / (2.0L * (long double)n)); lam[k] = -(4.0L / (h * h)) * s * s; }
+            else { long double s = sinl(PI_L * (long double)k / (2.0L * cells)); lam[k] = -(4.0L / (h * h)) * s * s; }
             break;
         }
         case SF_BC_UNBOUNDED: {
@@ -374,7 +378,7 @@ template <typename T> sf_status build_tables(sf_plan p)
         p->LT[a] = (p->r2r == R2R_NONE) ? p->La[a] : 2 * p->La[a];
         if ((st = upload_twiddles<T>(p, &p->tw[a], p->LT[a])) != SF_OK) return st;
     }
-    if (p->bc == SF_BC_NEUMANN)
+    if (p->r2r == R2R_DCT || p->r2r == R2R_DST2)
         for (int a = 0; a < p->ndim; ++a)
             if ((st = upload_dct_shift<T>(p, &p->ptw[a], (int)p->n[a])) != SF_OK) return st;
     std::vector<long double> z1(1, 0.0L);
@@ -423,8 +427,11 @@ template <typename T> sf_status run(sf_plan p, int outk)
             for (int s = 0; s < 2; ++s) {
                 xp.face[2 * a + s] = (const T*)p->face[2 * a + s];
                 if (xp.face[2 * a + s]) xp.has_faces = 1;
-                if (p->bc == SF_BC_DIRICHLET) xp.wface[2 * a + s] = (T)(-1.0 / (p->h[a] * p->h[a]));
-                else xp.wface[2 * a + s] = (T)((s ? -1.0 : 1.0) / p->h[a]);
+                // reading A18: the face sits one spacing (cell-boundary Dirichlet, cell-centre Neumann: weight 1)
+                // or half a spacing / a mirrored ghost node (the other two Table-1 rows: weight 2) from the layer
+                const double wf = ((p->bc == SF_BC_DIRICHLET) == (p->grid == SF_GRID_CELL_BOUNDARY)) ? 1.0 : 2.0;
+                if (p->bc == SF_BC_DIRICHLET) xp.wface[2 * a + s] = (T)(-wf / (p->h[a] * p->h[a]));
+                else xp.wface[2 * a + s] = (T)((s ? -wf : wf) / p->h[a]);
             }
     }
     mark(0);
@@ -615,8 +622,6 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
     } else if (green_op) {
         return fail(nullptr, SF_ERR_UNSUPPORTED, "Green's function operators need unbounded boundary conditions");
     }
-    if (b == SF_BC_DIRICHLET && grid != SF_GRID_CELL_BOUNDARY) return fail(nullptr, SF_ERR_UNSUPPORTED, "Dirichlet on a cell-centre grid (DST-II/III) is not built");
-    if (b == SF_BC_NEUMANN && grid != SF_GRID_CELL_CENTRE) return fail(nullptr, SF_ERR_UNSUPPORTED, "Neumann on a cell-boundary grid (DCT-I) is not built");
 
     sf_plan p = new (std::nothrow) sf_plan_s();
     if (!p) return fail(nullptr, SF_ERR_ALLOC, "host allocation failed");
@@ -647,11 +652,23 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
             if (!is_pow2(na)) return bail(SF_ERR_UNSUPPORTED, "unbounded sizes must be powers of two");
             len = (a == 0) ? na : 2 * na; p->P[a] = (int)(2 * na); norm *= 2.0 * (double)na; break;
         case SF_BC_DIRICHLET:
-            if (!is_pow2(na + 1)) return bail(SF_ERR_UNSUPPORTED, "Dirichlet cell-boundary sizes must be 2^k - 1 interior nodes");
-            len = na + 1; p->P[a] = (int)na; norm *= 2.0 * (double)(na + 1); break;
+            if (grid == SF_GRID_CELL_BOUNDARY) {
+                if (!is_pow2(na + 1)) return bail(SF_ERR_UNSUPPORTED, "Dirichlet cell-boundary sizes must be 2^k - 1 interior nodes");
+                len = na + 1;
+            } else {
+                if (!is_pow2(na)) return bail(SF_ERR_UNSUPPORTED, "Dirichlet cell-centre sizes must be powers of two");
+                len = na;
+            }
+            p->P[a] = (int)na; norm *= 2.0 * (double)len; break;
         default:
-            if (!is_pow2(na)) return bail(SF_ERR_UNSUPPORTED, "Neumann cell-centre sizes must be powers of two");
-            len = na; p->P[a] = (int)na; norm *= 2.0 * (double)na; break;
+            if (grid == SF_GRID_CELL_CENTRE) {
+                if (!is_pow2(na)) return bail(SF_ERR_UNSUPPORTED, "Neumann cell-centre sizes must be powers of two");
+                len = na;
+            } else {
+                if (na < 3 || !is_pow2(na - 1)) return bail(SF_ERR_UNSUPPORTED, "Neumann cell-boundary sizes must be 2^k + 1 nodes");
+                len = na - 1;
+            }
+            p->P[a] = (int)na; norm *= 2.0 * (double)len; break;
         }
         if (!length_built((int)len) || len > 2048) return bail(SF_ERR_UNSUPPORTED, "transform length outside the built range (complex length 4..2048 per pass)");
         if (a == 0) p->Lx = (int)len; else p->La[a] = (int)len;
@@ -662,8 +679,14 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
     switch (b) {
     case SF_BC_PERIODIC: p->xmode = X_PERIODIC; p->r2r = R2R_NONE; break;
     case SF_BC_UNBOUNDED: p->xmode = X_ZEROPAD; p->r2r = R2R_NONE; break;
-    case SF_BC_DIRICHLET: p->xmode = X_DST1; p->r2r = R2R_DST1; break;
-    default: p->xmode = X_DCT2; p->r2r = R2R_DCT; break;
+    case SF_BC_DIRICHLET:
+        if (grid == SF_GRID_CELL_BOUNDARY) { p->xmode = X_DST1; p->r2r = R2R_DST1; }
+        else { p->xmode = X_DST2; p->r2r = R2R_DST2; }
+        break;
+    default:
+        if (grid == SF_GRID_CELL_CENTRE) { p->xmode = X_DCT2; p->r2r = R2R_DCT; }
+        else { p->xmode = X_DCT1; p->r2r = R2R_DCT1; }
+        break;
     }
     p->nspec_x = (p->r2r == R2R_NONE) ? p->Lx + 1 : (int)p->n[0];
     p->pitch = round_up(p->nspec_x, 16);

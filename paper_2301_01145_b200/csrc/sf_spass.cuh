@@ -24,7 +24,7 @@ namespace sf {
 
 enum { MUL_SYMBOL = 0, MUL_GREEN = 1 };
 enum { OUT_SOLVE = 0, OUT_GRAD = 1, OUT_CURL = 2, OUT_DIV = 3, OUT_LAP = 4 };
-enum { R2R_NONE = 0, R2R_DST1 = 1, R2R_DCT = 2 };
+enum { R2R_NONE = 0, R2R_DST1 = 1, R2R_DCT = 2, R2R_DST2 = 3, R2R_DCT1 = 4 };
 
 template <typename T> struct SParams {
     typedef SF_CX C;
@@ -38,7 +38,7 @@ template <typename T> struct SParams {
     int r2r;      // R2R_*
     int LT;       // length of tw (a multiple of the transform length)
     const C* tw;  // exp(-2 pi i j / LT)
-    const C* ptw; // R2R_DCT: exp(-i pi k / (2n)), k < n
+    const C* ptw; // R2R_DCT, R2R_DST2: exp(-i pi k / (2n)), k <= n
     // ---- fused multiply (MODE 2)
     int mul;          // MUL_*
     int outk;         // OUT_*
@@ -107,7 +107,8 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
             }
         }
     } else if (MODE != 1) {
-        // real pencils, extended to length 2L:  DST-I: 0, x, 0, -reverse(x);  DCT-II: x, reverse(x)
+        // real pencils, extended to length 2L:  DST-I: 0, x, 0, -reverse(x);  DCT-II: x, reverse(x);
+        // DST-II: x, -reverse(x);  DCT-I (n = L + 1): x_0 .. x_L, x_{L-1} .. x_1
         const T* gin = reinterpret_cast<const T*>(p.in) + fz * p.in_cs + ib * p.in_bs + x0;
         const int n = p.n_in;
         constexpr int M = 2 * L;
@@ -121,9 +122,12 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
             if (p.r2r == R2R_DST1) {
                 s_real<T, TX>(s0, j + 1, tx) = v;
                 s_real<T, TX>(s0, M - 1 - j, tx) = -v;
+            } else if (p.r2r == R2R_DCT1) {
+                s_real<T, TX>(s0, j, tx) = v;
+                if (j >= 1 && j < L) s_real<T, TX>(s0, M - j, tx) = v;
             } else {
                 s_real<T, TX>(s0, j, tx) = v;
-                s_real<T, TX>(s0, M - 1 - j, tx) = v;
+                s_real<T, TX>(s0, M - 1 - j, tx) = (p.r2r == R2R_DST2) ? -v : v;
             }
         }
     }
@@ -217,9 +221,12 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
         return;
     }
 
-    // ------------------------------------------------------------------ real pencils (DST-I / DCT)
+    // ------------------------------------------------------------------ real pencils (DST / DCT)
     // Pair (k, L-k) of the packed transform Z is turned into the real-transform outputs, multiplied,
-    // turned back and stored in the same two slots: no other thread touches them.
+    // turned back and stored in the same two slots: no other thread touches them.  Slot k of the
+    // half-spectrum X[0..L] of the extended sequence holds stored row k - sh:
+    //   DST-I   Y[k-1] = -Im X[k],            1 <= k <= L-1        DST-II  Y[k-1] = -Im(ptw[k] X[k]),  1 <= k <= L
+    //   DCT-II  Y[k]   = Re(ptw[k] X[k]),     0 <= k <= L-1        DCT-I   Y[k]   = Re X[k],           0 <= k <= L
     {
         constexpr int M = 2 * L;
         const int n = p.n_in;
@@ -227,18 +234,20 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
         const T* yin = reinterpret_cast<const T*>(p.in) + fz * p.in_cs + ib * p.in_bs + x0;
         T* yout = reinterpret_cast<T*>(p.out) + fz * p.out_cs + ib * p.out_bs + x0;
         const int kx = min(x0 + tx_, p.nx - 1);
-        const bool dst = (p.r2r == R2R_DST1);
+        const bool sine = (p.r2r == R2R_DST1 || p.r2r == R2R_DST2);
+        const bool shifted = (p.r2r == R2R_DCT || p.r2r == R2R_DST2);     // outputs carry the half-sample phase ptw
+        const int sh = sine ? 1 : 0;
+        const bool has0 = !sine, hasL = (p.r2r == R2R_DST2 || p.r2r == R2R_DCT1);
         for (int idx = threadIdx.x; idx < (L / 2 + 1) * TX; idx += NT) {
             const int tx = idx % TX, k = idx / TX;
             const int km = L - k;
-            // spectral slots: DST-I: Y[k-1] = -Im X[k] (1 <= k <= L-1);  DCT-II: Y[k] = Re(ptw[k] X[k]) (k < L)
-            const int ik = dst ? k - 1 : k, im = dst ? km - 1 : km;   // stored row of slot k / slot L-k
-            const bool vk = dst ? (k >= 1) : true, vm = dst ? (k >= 1) : (k >= 1);
+            const int ik = k - sh, im = km - sh;                          // stored row of slot k / slot L-k
+            const bool vk = (k >= 1) || has0, vm = (k >= 1) || hasL;
             T yk = 0, ym = 0;
             C wk = mk<T>(1, 0), wm = mk<T>(1, 0);
-            if (!dst) {
+            if (shifted) {
                 wk = __ldg(p.ptw + k);
-                if (k >= 1) wm = __ldg(p.ptw + km);
+                wm = __ldg(p.ptw + km);
             }
             const C w = __ldg(p.tw + k * tws);
             if constexpr (MODE != 1) {
@@ -255,8 +264,8 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
                     xk = mk<T>((T)0.5 * (e.x + wd.y), (T)0.5 * (e.y - wd.x));
                     xm = mk<T>((T)0.5 * (e.x - wd.y), (T)0.5 * (-e.y - wd.x));
                 }
-                if (dst) { yk = -xk.y; ym = -xm.y; }
-                else { yk = wk.x * xk.x - wk.y * xk.y; ym = wm.x * xm.x - wm.y * xm.y; }
+                if (sine) { yk = -(wk.x * xk.y + wk.y * xk.x); ym = -(wm.x * xm.y + wm.y * xm.x); }   // -Im(w X)
+                else { yk = wk.x * xk.x - wk.y * xk.y; ym = wm.x * xm.x - wm.y * xm.y; }              //  Re(w X)
             } else {
                 if (xok && vk) yk = yin[ik * p.in_ps + tx];
                 if (xok && vm && km != k) ym = yin[im * p.in_ps + tx];
@@ -271,13 +280,12 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
                 if (vk) yk *= s_multiplier(p, kx, ib, ik);
                 if (vm) ym *= s_multiplier(p, kx, ib, im);
             }
-            // back to the packed spectrum: X'[k], X'[L-k] -> Z'[k], Z'[L-k]
+            // back to the packed spectrum: X'[k], X'[L-k] -> Z'[k], Z'[L-k]; slots that hold no row are zero
+            if (!vk) yk = (T)0;
+            if (!vm) ym = (T)0;
             C xk, xm;
-            if (dst) { xk = mk<T>(0, vk ? -yk : (T)0); xm = mk<T>(0, vm ? -ym : (T)0); }   // -i Y
-            else {
-                xk = mk<T>(wk.x * yk, -wk.y * yk);                                            // conj(ptw) Y
-                xm = (k >= 1) ? mk<T>(wm.x * ym, -wm.y * ym) : mk<T>(0, 0);                  // X'[L] = 0
-            }
+            if (sine) { xk = mk<T>(-wk.y * yk, -wk.x * yk); xm = mk<T>(-wm.y * ym, -wm.x * ym); }     // -i conj(w) Y
+            else { xk = mk<T>(wk.x * yk, -wk.y * yk); xm = mk<T>(wm.x * ym, -wm.y * ym); }            //    conj(w) Y
             const C e = mk<T>(xk.x + xm.x, xk.y - xm.y);
             const C d = mk<T>(xk.x - xm.x, xk.y + xm.y);
             const C wd = cmulc(d, w);
@@ -287,10 +295,10 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
         if constexpr (MODE == 0) return;
         __syncthreads();
         tile_fft_inv<T, L, TX, NT>(s0, p.tw, p.LT);
-        // extract the stored unknowns:  DST-I: x_j = x~[j+1];  DCT-III: x_j = x~[j]
+        // extract the stored unknowns:  DST-I: x_j = x~[j+1];  the others: x_j = x~[j]
         for (int idx = threadIdx.x; idx < n * TX; idx += NT) {
             const int tx = idx % TX, j = idx / TX;
-            if (xok) yout[j * p.out_ps + tx] = s_real<T, TX>(s0, dst ? j + 1 : j, tx);
+            if (xok) yout[j * p.out_ps + tx] = s_real<T, TX>(s0, (p.r2r == R2R_DST1) ? j + 1 : j, tx);
         }
     }
 }

@@ -11,14 +11,16 @@
 //   X_ZEROPAD   M = 2n           x~ = x, 0                      (Hockney-Eastwood)
 //   X_DST1      M = 2(n+1)       x~ = 0, x, 0, -reverse(x)      DST-I:  Y_k = -Im X~[k+1]
 //   X_DCT2      M = 2n           x~ = x, reverse(x)             DCT-II: Y_k = Re(e^{-i pi k/2n} X~[k])
-// and backward: DST-I again / DCT-III through the complex-to-real path.
+//   X_DST2      M = 2n           x~ = x, -reverse(x)            DST-II: Y_k = -Im(e^{-i pi (k+1)/2n} X~[k+1])
+//   X_DCT1      M = 2(n-1)       x~ = x_0..x_{n-1}, x_{n-2}..x_1  DCT-I:  Y_k = Re X~[k]
+// and backward: DST-I again / DCT-III / DST-III / DCT-I again through the complex-to-real path.
 // Inhomogeneous boundary values are folded into the source as it is loaded.
 #pragma once
 #include "sf_common.cuh"
 
 namespace sf {
 
-enum { X_PERIODIC = 0, X_ZEROPAD = 1, X_DST1 = 2, X_DCT2 = 3 };
+enum { X_PERIODIC = 0, X_ZEROPAD = 1, X_DST1 = 2, X_DCT2 = 3, X_DST2 = 4, X_DCT1 = 5 };
 
 template <typename T> struct XParams {
     typedef SF_CX C;
@@ -33,7 +35,7 @@ template <typename T> struct XParams {
     int mode;           // X_*
     int LT;             // length of tw
     const C* tw;        // exp(-2 pi i j / LT), LT = M
-    const C* ptw;       // X_DCT2: exp(-i pi k / (2n)), k < n
+    const C* ptw;       // X_DCT2, X_DST2: exp(-i pi k / (2n)), k <= n
     // boundary-value folding (forward only): face[2*axis+side], weight w[2*axis+side]; NULL = none
     const T* face[6];
     T wface[6];
@@ -86,6 +88,8 @@ template <typename T> __device__ __forceinline__ T x_ext(const XParams<T>& p, co
     case X_DST1:
         if (m == 0 || m == n + 1) return (T)0;
         return m <= n ? x_src(p, row, m - 1, iy, iz) : -x_src(p, row, M - m - 1, iy, iz);
+    case X_DST2: return m < n ? x_src(p, row, m, iy, iz) : -x_src(p, row, M - 1 - m, iy, iz);
+    case X_DCT1: return m < n ? x_src(p, row, m, iy, iz) : x_src(p, row, M - m, iy, iz);
     default: /* X_DCT2 */ return m < n ? x_src(p, row, m, iy, iz) : x_src(p, row, M - 1 - m, iy, iz);
     }
 }
@@ -178,6 +182,12 @@ __global__ void __launch_bounds__(NT) xfwd_kernel(const XParams<T> p)
                 T y;
                 if (p.mode == X_DST1) {
                     y = -G[r * LP + k + 1].y;
+                } else if (p.mode == X_DCT1) {
+                    y = G[r * LP + k].x;
+                } else if (p.mode == X_DST2) {
+                    const C w = __ldg(p.ptw + k + 1);
+                    const C x = G[r * LP + k + 1];
+                    y = -(w.x * x.y + w.y * x.x);
                 } else {
                     const C w = __ldg(p.ptw + k);
                     const C x = G[r * LP + k];
@@ -231,6 +241,14 @@ __global__ void __launch_bounds__(NT) xinv_kernel(const XParams<T> p)
                 const T* rp = ri + iy * p.sp_py + iz * p.sp_pz;
                 if (p.mode == X_DST1) {
                     if (k >= 1 && k <= n) x = mk<T>(0, -rp[k - 1]);       // X~[k] = -i Y[k-1]
+                } else if (p.mode == X_DCT1) {
+                    if (k < n) x = mk<T>(rp[k], 0);                        // X~[k] = Y[k]
+                } else if (p.mode == X_DST2) {
+                    if (k >= 1 && k <= n) {                                // X~[k] = -i e^{+i pi k/2n} Y[k-1]
+                        const C w = __ldg(p.ptw + k);
+                        const T y = rp[k - 1];
+                        x = mk<T>(-w.y * y, -w.x * y);
+                    }
                 } else {
                     if (k < n) {                                             // X~[k] = e^{+i pi k/2n} Y[k]
                         const C w = __ldg(p.ptw + k);
@@ -267,7 +285,7 @@ __global__ void __launch_bounds__(NT) xinv_kernel(const XParams<T> p)
     // unpack + extract + store
     T* ro = p.real_out + comp * p.rin_pc;
     const int n = p.n;
-    if (p.mode == X_PERIODIC || p.mode == X_ZEROPAD || p.mode == X_DCT2) {
+    if (p.mode == X_PERIODIC || p.mode == X_ZEROPAD || p.mode == X_DCT2 || p.mode == X_DST2) {
         const int nc = n / 2; // stored reals are x~[0..n): the first n/2 packed complex values
         for (int idx = threadIdx.x; idx < ROWS * nc; idx += NT) {
             const int r = idx / nc, j = idx % nc;
@@ -277,13 +295,13 @@ __global__ void __launch_bounds__(NT) xinv_kernel(const XParams<T> p)
                 *reinterpret_cast<C*>(ro + iy * p.rin_py + iz * p.rin_pz + 2 * j) = F[r * LP + j];
             }
         }
-    } else { // X_DST1: x_j = x~[j+1]
+    } else { // X_DST1: x_j = x~[j+1];  X_DCT1 (n odd): x_j = x~[j]
         for (int idx = threadIdx.x; idx < ROWS * n; idx += NT) {
             const int r = idx / n, j = idx % n;
             const long long row = row0 + r;
             if (row < nrows) {
                 const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-                const int m = j + 1;
+                const int m = (p.mode == X_DST1) ? j + 1 : j;
                 const C z = F[r * LP + (m >> 1)];
                 ro[iy * p.rin_py + iz * p.rin_pz + j] = (m & 1) ? z.y : z.x;
             }
