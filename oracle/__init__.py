@@ -224,6 +224,23 @@ def neumann_regular(f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
     return psi
 
 
+BOUNDED_KINDS = {"dirichlet_regular": 0, "neumann_staggered": 1, "dirichlet_staggered": 2, "neumann_regular": 3}
+
+
+def bounded_gradient(kind, f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
+    """psi and its spectral gradient on a Dirichlet / Neumann plan (kind: a key of BOUNDED_KINDS):
+    returns psi[z, y, x], grad[3, z, y, x] (d/dx, d/dy, d/dz)."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    assert nd == 3
+    psi = np.empty_like(f)
+    grad = np.empty((3,) + f.shape)
+    arr, keep = _faces_arg(faces)
+    _chk(lib().orc_bounded_gradient(C.c_int(BOUNDED_KINDS[kind]), _i64x3(n), _f64x3(h), C.c_int(op), C.c_double(rhs_sign),
+                                    _ptr(f), arr, _ptr(psi), _ptr(grad)), "bounded_gradient")
+    return psi, grad
+
+
 def neumann_staggered(f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
     """O-NEU.  Same conventions; face values are d psi / d x_axis along +axis on both sides."""
     f = _f64(f)

@@ -777,6 +777,142 @@ done:
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Spectral gradient on Dirichlet / Neumann plans (eq. (10), applied to the sine / cosine
+ * series of Table 1; SURVEY f3 "sine <-> cosine on the inverse").  The solve gives the coefficients
+ * c_k = rhs_sign * T_3(f') / Lambda of the series psi = (1/norm) S_3(c), S the synthesis (backward) sum of
+ * the row.  d psi / d x_a differentiates the basis functions of axis a analytically and evaluates them at
+ * the same grid points; the other axes keep their synthesis sums.  With kappa_k the wavenumber of term k:
+ *   kind 0  Dirichlet cell-boundary  psi_j = 2 sum_k c_k sin(kappa_k x_j),  x_j = (j+1) h,   kappa_k = pi (k+1) / ((n+1) h)
+ *   kind 1  Neumann   cell-centre    psi_j = c_0 + 2 sum_{k>=1} c_k cos(kappa_k x_j),  x_j = (j+1/2) h,  kappa_k = pi k / (n h)
+ *   kind 2  Dirichlet cell-centre    psi_j = (-1)^j c_{n-1} + 2 sum_{k<n-1} c_k sin(kappa_k x_j),  x_j = (j+1/2) h,  kappa_k = pi (k+1) / (n h)
+ *   kind 3  Neumann   cell-boundary  psi_j = c_0 + (-1)^j c_{n-1} + 2 sum_{1<=k<=n-2} c_k cos(kappa_k x_j),  x_j = j h,  kappa_k = pi k / ((n-1) h)
+ * The alternating terms of kinds 2 and 3 are the Nyquist terms sin / cos(pi x / h): their derivatives vanish at
+ * every grid point of their grids (consistent with reading A20).
+ *   sin -> kappa cos,  cos -> -kappa sin.
+ * psi, grad[3] (d/dx, d/dy, d/dz).
+ * ---------------------------------------------------------------------------------------- */
+typedef struct { int kind; int n; double h; } dsyn_par;
+
+/* derivative synthesis along one pencil: out_j = d/dx [ S(c) ](x_j) */
+static void dsyn_pencil(const dsyn_par *q, const double *c, double *out)
+{
+    int n = q->n;
+    for (int j = 0; j < n; ++j) {
+        long double acc = 0.0L;
+        for (int k = 0; k < n; ++k) {
+            long double kappa, x;
+            switch (q->kind) {
+            case 0: kappa = (long double)PI * (k + 1) / ((long double)(n + 1) * q->h); x = (long double)(j + 1) * q->h;
+                    acc += 2.0L * c[k] * kappa * cosl(kappa * x); break;
+            case 1: if (k == 0) break;
+                    kappa = (long double)PI * k / ((long double)n * q->h); x = ((long double)j + 0.5L) * q->h;
+                    acc -= 2.0L * c[k] * kappa * sinl(kappa * x); break;
+            case 2: if (k == n - 1) break;
+                    kappa = (long double)PI * (k + 1) / ((long double)n * q->h); x = ((long double)j + 0.5L) * q->h;
+                    acc += 2.0L * c[k] * kappa * cosl(kappa * x); break;
+            default: if (k == 0 || k == n - 1) break;
+                    kappa = (long double)PI * k / ((long double)(n - 1) * q->h); x = (long double)j * q->h;
+                    acc -= 2.0L * c[k] * kappa * sinl(kappa * x); break;
+            }
+        }
+        out[j] = (double)acc;
+    }
+}
+
+static int dsyn_axis(double *a, const i64 dims[3], int axis, const dsyn_par *q)
+{
+    i64 len, stride, na, sa, nb, sb;
+    axis_geometry(dims, axis, &len, &stride, &na, &sa, &nb, &sb);
+    int err = ORC_OK;
+#pragma omp parallel
+    {
+        double *buf = (double *)malloc(sizeof(double) * (size_t)len * 2);
+        if (!buf) {
+#pragma omp critical
+            err = ORC_ERR_ALLOC;
+        }
+#pragma omp for collapse(2) schedule(static)
+        for (i64 ib = 0; ib < nb; ++ib)
+            for (i64 ia = 0; ia < na; ++ia) {
+                if (!buf) continue;
+                double *p = a + ia * sa + ib * sb;
+                double *in = buf, *out = buf + len;
+                for (i64 j = 0; j < len; ++j) in[j] = p[j * stride];
+                dsyn_pencil(q, in, out);
+                for (i64 j = 0; j < len; ++j) p[j * stride] = out[j];
+            }
+        free(buf);
+    }
+    return err;
+}
+
+int orc_bounded_gradient(int kind, const i64 n[3], const double h[3], int op, double rhs_sign, const double *f,
+                         const double *const faces[6], double *psi, double *grad)
+{
+    if (kind < 0 || kind > 3) return ORC_ERR_ARG;
+    i64 tot = n[0] * n[1] * n[2];
+    trig_table tab[3];
+    double *lam[3] = { 0, 0, 0 };
+    double *coef = (double *)malloc(sizeof(double) * (size_t)tot);
+    int err = ORC_OK, ntab = 0;
+    real_xform fwd = (kind == 0) ? dst1_tab : (kind == 1) ? dct2_tab : (kind == 2) ? dst2_tab : dct1_tab;
+    real_xform bwd = (kind == 0) ? dst1_tab : (kind == 1) ? dct3_tab : (kind == 2) ? dst3_tab : dct1_tab;
+    int neumann = (kind == 1 || kind == 3);
+    if (!coef) return ORC_ERR_ALLOC;
+    memcpy(coef, f, sizeof(double) * (size_t)tot);
+    if (op == 1) { if (kind < 2) fold_faces(coef, n, h, faces, neumann); else fold_faces_f3(coef, n, h, faces, neumann); }
+    double norm = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        i64 N = n[a];
+        i64 q = (kind == 0) ? 2 * (N + 1) : (kind == 3) ? 2 * (N - 1) : 4 * N;
+        double cells = (kind == 0) ? (double)(N + 1) : (kind == 3) ? (double)(N - 1) : (double)N;
+        if ((err = trig_table_init(&tab[a], (int)N, q)) != ORC_OK) { ntab = a + 1; goto done; }
+        ntab = a + 1;
+        lam[a] = (double *)malloc(sizeof(double) * (size_t)N);
+        if (!lam[a]) { err = ORC_ERR_ALLOC; goto done; }
+        norm *= 2.0 * cells;
+        for (i64 k = 0; k < N; ++k) {
+            double idx = neumann ? (double)k : (double)(k + 1);
+            if (op == 0) {
+                double kk = PI * idx / (cells * h[a]);
+                lam[a][k] = -kk * kk;
+            } else {
+                double sn = sin(PI * idx / (2.0 * cells));
+                lam[a][k] = -(4.0 / (h[a] * h[a])) * sn * sn;
+            }
+        }
+    }
+    for (int a = 0; a < 3; ++a)
+        if ((err = r2r_axis(coef, n, a, fwd, &tab[a])) != ORC_OK) goto done;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (i64 kz = 0; kz < n[2]; ++kz)
+        for (i64 ky = 0; ky < n[1]; ++ky)
+            for (i64 kx = 0; kx < n[0]; ++kx) {
+                i64 i = kx + n[0] * (ky + n[1] * kz);
+                if (neumann && kx == 0 && ky == 0 && kz == 0) { coef[i] = 0.0; continue; }
+                coef[i] = rhs_sign * coef[i] / (lam[0][kx] + lam[1][ky] + lam[2][kz]) / norm;
+            }
+    for (int g = 0; g < 3; ++g) {
+        double *out = grad + (size_t)g * (size_t)tot;
+        memcpy(out, coef, sizeof(double) * (size_t)tot);
+        for (int a = 2; a >= 0; --a) {
+            if (a == g) {
+                dsyn_par q = { kind, (int)n[a], h[a] };
+                if ((err = dsyn_axis(out, n, a, &q)) != ORC_OK) goto done;
+            } else if ((err = r2r_axis(out, n, a, bwd, &tab[a])) != ORC_OK) goto done;
+        }
+    }
+    memcpy(psi, coef, sizeof(double) * (size_t)tot);
+    for (int a = 2; a >= 0; --a)
+        if ((err = r2r_axis(psi, n, a, bwd, &tab[a])) != ORC_OK) goto done;
+done:
+    for (int a = 0; a < ntab; ++a) trig_table_free(&tab[a]);
+    for (int a = 0; a < 3; ++a) free(lam[a]);
+    free(coef);
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------------
  * O-UNB / O-VEC: unbounded solver, Hockney-Eastwood on the whole doubled domain.
  *
  * Real-space kernel: 2nd-order Gaussian-regularised Green's function of Hejlesen (

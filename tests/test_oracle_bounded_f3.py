@@ -161,3 +161,68 @@ def test_f3_second_order_convergence_and_ps_exactness():
     d = W.neumann3d_boundary_manufactured(32, inhomogeneous=False)
     psi = O.neumann_regular(d["f"], d["h"], None, op=O.OP_PS)
     assert np.abs((psi - psi.mean()) - (d["u"] - d["u"].mean())).max() < 1e-13
+
+
+# ------------------------------------------------------------------- spectral gradient on bounded plans
+def _grid_of(kind, n, L):
+    """grid points and basis functions of the four Table-1 rows on [0, L]"""
+    if kind == "dirichlet_regular":
+        h = L / (n + 1)
+        return h, (np.arange(n) + 1.0) * h, np.sin, np.cos, 1.0
+    if kind == "dirichlet_staggered":
+        h = L / n
+        return h, (np.arange(n) + 0.5) * h, np.sin, np.cos, 1.0
+    if kind == "neumann_staggered":
+        h = L / n
+        return h, (np.arange(n) + 0.5) * h, np.cos, np.sin, -1.0
+    h = L / (n - 1)
+    return h, np.arange(n) * h, np.cos, np.sin, -1.0
+
+
+@pytest.mark.parametrize("kind,shape", [("dirichlet_regular", (7, 15, 31)), ("dirichlet_staggered", (8, 16, 32)),
+                                        ("neumann_staggered", (8, 16, 32)), ("neumann_regular", (9, 17, 33))])
+def test_bounded_gradient_of_the_basis_functions(kind, shape):
+    """u = prod_a sin|cos(m_a pi x_a / L_a) on a non-cubic, anisotropic box: with the pseudo-spectral eigenvalues
+    the solve returns u and the gradient m_a pi / L_a cos|(-sin)(...) to rounding; with FD2 both
+    carry the amplitude ratio of the eigenvalues.  Different m, n and L per axis: components cannot be swapped."""
+    nz, ny, nx = shape
+    L = (1.0, 0.7, 1.3)
+    m = (3, 2, 5)
+    hs, xs, t, dt = [], [], [], []
+    for a, n in enumerate((nx, ny, nz)):
+        h, x, fn, dfn, sg = _grid_of(kind, n, L[a])
+        kap = m[a] * np.pi / L[a]
+        hs.append(h); xs.append(x); t.append(fn(kap * x)); dt.append(sg * kap * dfn(kap * x))
+    outer = lambda v: v[2][:, None, None] * v[1][None, :, None] * v[0][None, None, :]
+    u = outer(t)
+    k2 = sum((m[a] * np.pi / L[a]) ** 2 for a in range(3))
+    f = -k2 * u
+    psi, grad = O.bounded_gradient(kind, f, hs, None, op=O.OP_PS)
+    assert np.abs(psi - u).max() < 1e-13
+    for a in range(3):
+        want = outer([dt[i] if i == a else t[i] for i in range(3)])
+        assert np.abs(grad[a] - want).max() < 1e-12 * np.abs(want).max(), (kind, a)
+    lam_fd = sum((4 / hs[a] ** 2) * np.sin(m[a] * np.pi * hs[a] / (2 * L[a])) ** 2 for a in range(3))
+    psi2, grad2 = O.bounded_gradient(kind, f, hs, None, op=O.OP_FD2, rhs_sign=-1.0)
+    assert np.abs(psi2 + (k2 / lam_fd) * u).max() < 1e-13
+    for a in range(3):
+        assert np.abs(grad2[a] + (k2 / lam_fd) * grad[a]).max() < 1e-11 * np.abs(grad[a]).max()
+    # psi is the plain solver's
+    assert np.abs(psi2 - getattr(O, kind)(f, hs, None, op=O.OP_FD2, rhs_sign=-1.0)).max() < 1e-14 * np.abs(psi2).max()
+
+
+def test_bounded_gradient_is_linear_and_axis_specific():
+    """white noise on a non-cubic anisotropic grid: the gradient is linear in the source, flips with rhs_sign,
+    and d/dx_a of a field that varies along x_a only has no other component"""
+    rng = np.random.default_rng(21)
+    shape, h = (8, 16, 32), (0.11, 0.07, 0.13)
+    f1, f2 = rng.normal(size=shape), rng.normal(size=shape)
+    for kind in ("dirichlet_staggered", "neumann_staggered"):
+        _, g1 = O.bounded_gradient(kind, f1, h)
+        _, g2 = O.bounded_gradient(kind, f2, h)
+        _, g12 = O.bounded_gradient(kind, 2 * f1 - 3 * f2, h, rhs_sign=-1.0)
+        assert np.abs(g12 + 2 * g1 - 3 * g2).max() < 1e-12 * np.abs(g12).max()
+        fx = np.broadcast_to(rng.normal(size=(1, 1, 32)), shape).copy()
+        _, g = O.bounded_gradient(kind, fx, h)
+        if kind.startswith("neumann"):     # constant along y, z is a basis function (k = 0): pure x dependence
+            assert np.abs(g[1]).max() < 1e-12 * np.abs(g[0]).max() and np.abs(g[2]).max() < 1e-12 * np.abs(g[0]).max()
