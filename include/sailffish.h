@@ -151,10 +151,13 @@ sf_status sf_set_bc_values(sf_plan plan, int axis, int side, const void* face, s
 sf_status sf_solve(sf_plan plan);
 
 /* sf_gradient -- as sf_solve, and additionally d psi / d x_a = IDFT(i k_a psi_hat) for every axis
- * from the same spectrum (eq. 10).  Scalar periodic and unbounded plans (UNSUPPORTED
- * otherwise); on unbounded plans k_a are the wavenumbers of the doubled grid, as for sf_curl, and the
- * first call allocates a four-field set of work arrays (ALLOC on failure).  The wavenumber at the
- * Nyquist index is taken as zero. */
+ * from the same spectrum (eq. 10).  Scalar plans (UNSUPPORTED otherwise).  On unbounded
+ * plans k_a are the wavenumbers of the doubled grid, as for sf_curl.  On 3-D Dirichlet / Neumann
+ * plans the sine / cosine series of Table 1 is differentiated term by term (a sine series along the
+ * differentiated axis comes back as a cosine series and vice versa, k_a = pi k / L_a); this is the
+ * derivative of the series, meaningful for homogeneous boundary values (with folded face values the
+ * odd / even extension is not smooth).  The wavenumber at the Nyquist index is taken as zero.  On
+ * non-periodic plans the first call allocates a (1 + ndim)-field set of work arrays (ALLOC on failure). */
 sf_status sf_gradient(sf_plan plan);
 
 /* sf_curl -- ncomp == 3 plans: solve the three components and return u = curl psi = IDFT(i k x

@@ -70,6 +70,7 @@ struct sf_plan_s {
     void* ptw[3] = { nullptr, nullptr, nullptr };
     void* lam[3] = { nullptr, nullptr, nullptr };
     void* kap[3] = { nullptr, nullptr, nullptr };
+    void* kap_ext[3] = { nullptr, nullptr, nullptr };   // Dirichlet / Neumann: pi k / L_domain per slot k <= L of the extended sequence
     void* zero1 = nullptr;
     int LT[3] = { 0, 0, 0 };
     void* green = nullptr;
@@ -392,6 +393,14 @@ template <typename T> sf_status build_tables(sf_plan p)
         axis_tables(*p, a, count, lam, kap);
         if ((st = upload_real<T>(p, &p->lam[a], lam)) != SF_OK) return st;
         if ((st = upload_real<T>(p, &p->kap[a], kap)) != SF_OK) return st;
+        if (p->r2r != R2R_NONE) {
+            // the extended sequence of length 2L has period 2 L_domain: slot k carries pi k / L_domain;
+            // the Nyquist slot k = L is taken as zero (reading A20)
+            const int Lh = (a == 0) ? p->Lx : p->La[a];
+            std::vector<long double> ke((size_t)Lh + 1, 0.0L);
+            for (int k = 0; k < Lh; ++k) ke[k] = PI_L * (long double)k / ((long double)Lh * (long double)p->h[a]);
+            if ((st = upload_real<T>(p, &p->kap_ext[a], ke)) != SF_OK) return st;
+        }
     }
     if (p->bc == SF_BC_UNBOUNDED) return build_green<T>(p);
     return SF_OK;
@@ -539,6 +548,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         sp.Pp = p->P[ax];
         sp.n_in = nlast; sp.n_out = nlast;
         sp.LT = p->LT[ax]; sp.tw = (const C*)p->tw[ax]; sp.ptw = (const C*)p->ptw[ax];
+        sp.kap_ext = (const T*)p->kap_ext[ax];
         const int nb = (nd == 3) ? P1 : 1;
         const int nbuf = (outk == OUT_CURL || outk == OUT_DIV) ? 3 : (outk == OUT_GRAD ? 2 : 1);
         const int gz = (outk == OUT_SOLVE || outk == OUT_LAP) ? ncomp : 1;
@@ -553,12 +563,16 @@ template <typename T> sf_status run(sf_plan p, int outk)
         sp.out_ps = hp; sp.out_bs = hp * n1; sp.out_cs = p->w1_field;
         sp.n_in = (p->r2r == R2R_NONE) ? p->La[1] : n1; sp.n_out = n1;
         sp.LT = p->LT[1]; sp.tw = (const C*)p->tw[1]; sp.ptw = (const C*)p->ptw[1];
+        sp.kap_ext = (const T*)p->kap_ext[1];
+        sp.dfield1 = (p->r2r != R2R_NONE && outk == OUT_GRAD) ? 3 : 0;   // field 2 = d psi / dy
         SF_CUDA(p, launch_spass<T>(p->La[1], 1, sp, n2, nf_out, 1, st));
         p->launches++;
     }
     mark(4);
     // S5: X backward
     xp.spec_in = p->W1; xp.real_out = (T*)p->out;
+    xp.kap_ext = (const T*)p->kap_ext[0];
+    xp.dfield1 = (p->r2r != R2R_NONE && outk == OUT_GRAD) ? 2 : 0;       // field 1 = d psi / dx
     SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
     p->launches++;
     mark(5);
@@ -810,20 +824,30 @@ sf_status sf_solve(sf_plan plan) { return run_any(plan, OUT_SOLVE); }
 sf_status sf_gradient(sf_plan plan)
 {
     if (!plan) return SF_ERR_INVALID_ARG;
-    if ((plan->bc != SF_BC_PERIODIC && plan->bc != SF_BC_UNBOUNDED) || plan->ncomp != 1)
-        return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient is built for scalar periodic and unbounded plans");
+    if (plan->ncomp != 1) return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient is built for scalar plans");
     if (plan->bc == SF_BC_PERIODIC) return run_any(plan, OUT_GRAD);
-    // unbounded: psi and its three derivatives need four fields of work space
+    if (plan->ndim != 3) return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient on Dirichlet / Neumann plans is built for 3-D");
+    // unbounded, Dirichlet, Neumann: psi and its derivatives need 1 + ndim fields of work space
     const int nf = 1 + plan->ndim;
-    const size_t welem = 2 * plan->esize;
+    {
+        // the fused pass holds two tiles (psi and the derivative along its axis)
+        const int ax = plan->ndim - 1;
+        const size_t need = (plan->prec == SF_F32) ? spass_smem_bytes<float>(plan->La[ax], 2) : spass_smem_bytes<double>(plan->La[ax], 2);
+        if (need > 227 * 1024) return fail(plan, SF_ERR_UNSUPPORTED, "gradient: the fused pass does not fit in shared memory for this size / precision");
+    }
+    const size_t welem = (plan->r2r == R2R_NONE) ? 2 * plan->esize : plan->esize;
     if (!plan->gW1) {
         sf_status st;
         const size_t b1 = (size_t)plan->w1_field * nf * welem, b2 = (size_t)plan->w2_field * nf * welem;
         if ((st = dev_alloc(plan, &plan->gW1, b1)) != SF_OK) return st;
-        if ((st = dev_alloc(plan, &plan->gW2, b2)) != SF_OK) return st;
-        if ((st = dev_alloc(plan, &plan->gout, field_elems(plan) * nf * plan->esize)) != SF_OK) return st;
         SF_CUDA(plan, cudaMemsetAsync(plan->gW1, 0, b1, plan->stream));
-        SF_CUDA(plan, cudaMemsetAsync(plan->gW2, 0, b2, plan->stream));
+        if (plan->padded) {
+            if ((st = dev_alloc(plan, &plan->gW2, b2)) != SF_OK) return st;
+            SF_CUDA(plan, cudaMemsetAsync(plan->gW2, 0, b2, plan->stream));
+        } else {
+            plan->gW2 = plan->gW1;
+        }
+        if ((st = dev_alloc(plan, &plan->gout, field_elems(plan) * nf * plan->esize)) != SF_OK) return st;
     }
     std::swap(plan->W1, plan->gW1);
     std::swap(plan->W2, plan->gW2);

@@ -50,6 +50,9 @@ template <typename T> struct SParams {
     const T* green;   // compact real table [fp][fb][kx], rhs_sign and normalisation folded in
     long long g_pb, g_pp;
     int Pb, Pp;       // transform lengths along batch / pencil axes (index folding k -> min(k, P-k))
+    // ---- real pencils: spectral derivative along the pencil axis (sine <-> cosine series, eq. (10))
+    int dfield1;      // MODE 1: 1 + index of the field (blockIdx.z) whose backward transform differentiates; 0: none
+    const T* kap_ext; // wavenumber pi k / L_domain of slot k of the extended sequence, k <= L, zero at k = L
 };
 
 template <typename T, int L> __host__ __device__ constexpr int s_tx()
@@ -286,6 +289,21 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
             C xk, xm;
             if (sine) { xk = mk<T>(-wk.y * yk, -wk.x * yk); xm = mk<T>(-wm.y * ym, -wm.x * ym); }     // -i conj(w) Y
             else { xk = mk<T>(wk.x * yk, -wk.y * yk); xm = mk<T>(wm.x * ym, -wm.y * ym); }            //    conj(w) Y
+            // d/dx of the series: X'[k] -> i kappa_k X'[k] (a sine series becomes a cosine series and back)
+            const bool dgrad = (MODE == 2 && p.outk == OUT_GRAD);
+            const bool dthis = (MODE == 1 && p.dfield1 == (int)blockIdx.z + 1);
+            if (dgrad || dthis) {
+                const T qk = __ldg(p.kap_ext + k), qm = __ldg(p.kap_ext + km);
+                const C dk = mk<T>(-qk * xk.y, qk * xk.x), dm = mk<T>(-qm * xm.y, qm * xm.x);
+                if (dthis) { xk = dk; xm = dm; }
+                else {
+                    const C e = mk<T>(dk.x + dm.x, dk.y - dm.y);
+                    const C d = mk<T>(dk.x - dm.x, dk.y + dm.y);
+                    const C wd = cmulc(d, w);
+                    s0[TILE + pos_of_k<L>(k) * TX + tx] = mk<T>(e.x - wd.y, e.y + wd.x);
+                    if (k > 0) s0[TILE + pos_of_k<L>(km) * TX + tx] = mk<T>(e.x + wd.y, -e.y + wd.x);
+                }
+            }
             const C e = mk<T>(xk.x + xm.x, xk.y - xm.y);
             const C d = mk<T>(xk.x - xm.x, xk.y + xm.y);
             const C wd = cmulc(d, w);
@@ -295,10 +313,19 @@ __global__ void __launch_bounds__(NT) spass_kernel(const SParams<T> p)
         if constexpr (MODE == 0) return;
         __syncthreads();
         tile_fft_inv<T, L, TX, NT>(s0, p.tw, p.LT);
-        // extract the stored unknowns:  DST-I: x_j = x~[j+1];  the others: x_j = x~[j]
-        for (int idx = threadIdx.x; idx < n * TX; idx += NT) {
-            const int tx = idx % TX, j = idx / TX;
-            if (xok) yout[j * p.out_ps + tx] = s_real<T, TX>(s0, (p.r2r == R2R_DST1) ? j + 1 : j, tx);
+        const bool grad = (MODE == 2 && p.outk == OUT_GRAD);
+        if (grad) tile_fft_inv<T, L, TX, NT>(s0 + TILE, p.tw, p.LT);
+        // extract the stored unknowns:  DST-I: x_j = x~[j+1];  the others: x_j = x~[j].  Gradient: the
+        // field differentiated along this axis takes the second buffer, psi and the other derivative
+        // fields (differentiated by the later passes) the first
+        const int nfo = grad ? p.pencil_axis + 2 : 1;
+        for (int f = 0; f < nfo; ++f) {
+            const C* sb = (grad && f == p.pencil_axis + 1) ? s0 + TILE : s0;
+            T* yo = yout + f * p.out_cs;
+            for (int idx = threadIdx.x; idx < n * TX; idx += NT) {
+                const int tx = idx % TX, j = idx / TX;
+                if (xok) yo[j * p.out_ps + tx] = s_real<T, TX>(const_cast<C*>(sb), (p.r2r == R2R_DST1) ? j + 1 : j, tx);
+            }
         }
     }
 }

@@ -40,6 +40,9 @@ template <typename T> struct XParams {
     const T* face[6];
     T wface[6];
     int has_faces;
+    // backward, real modes: spectral derivative along x of one field (sine <-> cosine series, eq. (10))
+    int dfield1;        // 1 + index of the field (blockIdx.y) that is differentiated; 0: none
+    const T* kap_ext;   // pi k / L_domain for slot k <= L of the extended sequence, zero at k = L
 };
 
 // rows per CTA: two Stockham buffers of ROWS x LP complex; prefer a footprint that lets several CTAs
@@ -255,6 +258,10 @@ __global__ void __launch_bounds__(NT) xinv_kernel(const XParams<T> p)
                         const T y = rp[k];
                         x = mk<T>(w.x * y, -w.y * y);
                     }
+                }
+                if (p.dfield1 == comp + 1) {                                // X~[k] -> i kappa_k X~[k]
+                    const T q = __ldg(p.kap_ext + k);
+                    x = mk<T>(-q * x.y, q * x.x);
                 }
             }
             A[r * LP + k] = x;
