@@ -68,17 +68,33 @@ template <typename T, bool INV> static cudaError_t launch_x_any(int L, const XPa
     }
 }
 
+template <typename T, int L, int MODE, int NT> static cudaError_t launch_s_nt(const SParams<T>& p, int nb, int nz, size_t smem, cudaStream_t st)
+{
+    constexpr int TX = s_tx<T, L>();
+    dim3 grid((unsigned)((p.nx + TX - 1) / TX), (unsigned)nb, (unsigned)nz);
+    auto kernel = spass_kernel<T, L, TX, NT, MODE>;
+    cudaError_t e = set_smem(kernel, smem);
+    if (e != cudaSuccess) return e;
+    kernel<<<grid, NT, smem, st>>>(p);
+    return cudaGetLastError();
+}
+
 template <typename T, int L, int MODE> static cudaError_t launch_s_one(const SParams<T>& p, int nb, int nz, int nbuf, cudaStream_t st)
 {
     constexpr int TX = s_tx<T, L>();
     const size_t smem = (size_t)nbuf * L * TX * sizeof(SF_CX);
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
-    dim3 grid((unsigned)((p.nx + TX - 1) / TX), (unsigned)nb, (unsigned)nz);
-    auto kernel = spass_kernel<T, L, TX, kThreads, MODE>;
-    cudaError_t e = set_smem(kernel, smem);
-    if (e != cudaSuccess) return e;
-    kernel<<<grid, kThreads, smem, st>>>(p);
-    return cudaGetLastError();
+    // The fused pass with two or three tiles (gradient, curl, divergence) of a long transform fills most
+    // of an SM's shared memory: when only one or two CTAs fit, give each more threads so that the SM
+    // still holds 1024 (cfg 5: 192 KB per CTA, one CTA of 1024 threads instead of 256).
+    if constexpr (MODE == 2 && L >= 256) {
+        if (smem > 113 * 1024) {
+            constexpr int NTB = (sizeof(T) == 4) ? 1024 : 512;    // 64 / 128 registers per thread
+            return launch_s_nt<T, L, MODE, NTB>(p, nb, nz, smem, st);
+        }
+        if (smem > 75 * 1024) return launch_s_nt<T, L, MODE, 512>(p, nb, nz, smem, st);
+    }
+    return launch_s_nt<T, L, MODE, kThreads>(p, nb, nz, smem, st);
 }
 
 template <typename T, int MODE> static cudaError_t launch_s_any(int L, const SParams<T>& p, int nb, int nz, int nbuf, cudaStream_t st)
