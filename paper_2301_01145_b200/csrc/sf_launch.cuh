@@ -50,10 +50,12 @@ template <typename T, int L, bool INV> static cudaError_t launch_x_one(const XPa
     const size_t smem = (size_t)2 * ROWS * LP * sizeof(SF_CX);
     const long long rows = (long long)p.ny * p.nz;
     dim3 grid((unsigned)((rows + ROWS - 1) / ROWS), (unsigned)ncomp);
-    auto kernel = INV ? xinv_kernel<T, L, kThreads> : xfwd_kernel<T, L, kThreads>;
+    // fp32 rows of 512 and more complex points: three or fewer CTAs fit per SM, so give each 512 threads
+    constexpr int NT = (sizeof(T) == 4 && L >= 512) ? 512 : kThreads;
+    auto kernel = INV ? xinv_kernel<T, L, NT> : xfwd_kernel<T, L, NT>;
     cudaError_t e = set_smem(kernel, smem);
     if (e != cudaSuccess) return e;
-    kernel<<<grid, kThreads, smem, st>>>(p);
+    kernel<<<grid, NT, smem, st>>>(p);
     return cudaGetLastError();
 }
 
