@@ -49,6 +49,10 @@ def lib() -> C.CDLL:
         L.orc_green_spectral.argtypes = [C.c_double, C.c_double]
         L.orc_green_gauss.restype = C.c_double
         L.orc_green_gauss.argtypes = [C.c_int, C.c_double, C.c_double]
+        L.orc_exp1.restype = C.c_double
+        L.orc_exp1.argtypes = [C.c_double]
+        L.orc_green2d_gauss.restype = C.c_double
+        L.orc_green2d_gauss.argtypes = [C.c_int, C.c_double, C.c_double]
         L.orc_unbounded_spec_size.restype = C.c_longlong
         _lib = L
     return _lib
@@ -334,6 +338,54 @@ def unbounded_laplacian(f, h, ghat, rhs_sign=1.0):
     _chk(lib().orc_unbounded_divlap(_i64x3(n), _f64x3(h), _ptr(ghat), C.c_int(f.shape[0] if vec else 1),
                                     C.c_double(rhs_sign), _ptr(f), C.c_int(1), _ptr(out)), "unbounded_laplacian")
     return out
+
+
+def exp1(u):
+    return float(lib().orc_exp1(float(u)))
+
+
+def green2d_gauss(order, r, eps):
+    """2-D Gaussian-regularised kernel of order 2 .. 10 at distance r (reading A28)."""
+    return float(lib().orc_green2d_gauss(int(order), float(r), float(eps)))
+
+
+def _i64x2(n):
+    return (C.c_longlong * 2)(int(n[0]), int(n[1]))
+
+
+def _f64x2(h):
+    return (C.c_double * 2)(float(h[0]), float(h[1]))
+
+
+def unbounded2d_green(n_xy, h, eps, order=2):
+    """Green's spectrum on the doubled 2-D grid: complex array [2 ny, nx + 1]."""
+    n = [int(v) for v in n_xy]
+    ghat = np.empty((2 * n[1], n[0] + 1), dtype=np.complex128)
+    _chk(lib().orc_unbounded2d_green(_i64x2(n), _f64x2(h), C.c_double(eps), C.c_int(order), _ptr(ghat)), "unbounded2d_green")
+    return ghat
+
+
+def unbounded2d_solve(f, h, ghat, rhs_sign=1.0, want_grad=False):
+    """O-UNB2.  f[y, x]; returns psi, or (psi, grad[2, y, x]) with grad = (d/dx, d/dy)."""
+    f = _f64(f)
+    assert f.ndim == 2
+    n = (f.shape[1], f.shape[0])
+    psi = np.empty_like(f)
+    grad = np.empty((2,) + f.shape) if want_grad else None
+    ghat = np.ascontiguousarray(ghat, dtype=np.complex128)
+    assert ghat.shape == (2 * n[1], n[0] + 1)
+    _chk(lib().orc_unbounded2d_solve(_i64x2(n), _f64x2(h), _ptr(ghat), C.c_double(rhs_sign), _ptr(f), _ptr(psi),
+                                     _ptr(grad) if want_grad else None), "unbounded2d_solve")
+    return (psi, grad) if want_grad else psi
+
+
+def unbounded2d_direct(f, h, eps, order=2, rhs_sign=1.0):
+    """Direct O(N^4) sum of the 2-D definition -- tiny grids only."""
+    f = _f64(f)
+    n = (f.shape[1], f.shape[0])
+    psi = np.empty_like(f)
+    lib().orc_unbounded2d_direct(_i64x2(n), _f64x2(h), C.c_double(eps), C.c_int(order), C.c_double(rhs_sign), _ptr(f), _ptr(psi))
+    return psi
 
 
 def unbounded_direct(f, h, eps, rhs_sign=1.0):

@@ -1335,6 +1335,167 @@ done:
     return err;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * O-UNB2: 2-D unbounded solver (PAPER.md:189 lists the regularised kernels for 1-D, 2-D and 3-D,
+ * formulas not printed -- reading A28).  Free-space kernel of the 2-D Laplacian: G_0 = ln(r) / (2 pi)
+ * (lap G_0 = delta, sign of PAPER.md:38).  Regularised with the unit Gaussian of width eps,
+ * G_2 = G_0 * zeta_eps: the radial field is G_2'(r) = (1 - exp(-r^2 / (2 eps^2))) / (2 pi r), hence
+ *     G_2(r) = ( ln r + E_1(r^2 / (2 eps^2)) / 2 ) / (2 pi),    G_2(0) = ( ln(2 eps^2) - gamma ) / (4 pi),
+ * E_1 the exponential integral, gamma Euler's constant.  Higher orders as in 3-D (reading A25): term n >= 1 of
+ * zeta^_P is -(eps^2/2)^n / n! (-lap)^(n-1) g with g the 2-D unit Gaussian and, in 2-D,
+ * lap^m g = (-1)^m 2^m m! / eps^(2m) L_m(x) g, x = r^2 / (2 eps^2), L_m the ordinary Laguerre polynomial:
+ *     G_P = G_2 - sum_{n=1}^{P/2-1} eps^2 / (2 n) L_{n-1}(x) g .
+ * Definition computed: psi_i = rhs_sign hx hy sum_j G(|x_i - x_j|) f_j, by Hockney-Eastwood doubling.
+ * ---------------------------------------------------------------------------------------- */
+#define EULER_GAMMA 0.57721566490153286060651209008240243
+/* E_1(u), u > 0: series -gamma - ln u - sum_{k>=1} (-u)^k / (k k!) for u <= 1, else the continued fraction
+ * e^-u / (u + 1 - 1/(u + 3 - 4/(u + 5 - ...))) by the modified Lentz method */
+double orc_exp1(double u)
+{
+    if (u <= 1.0) {
+        double sum = 0.0, term = 1.0;
+        for (int k = 1; k < 60; ++k) {
+            term *= -u / (double)k;
+            double add = term / (double)k;
+            sum += add;
+            if (fabs(add) < 1e-18 * fabs(sum)) break;
+        }
+        return -EULER_GAMMA - log(u) - sum;
+    }
+    double b = u + 1.0, c = 1e300, d = 1.0 / b, hh = d;
+    for (int i = 1; i < 500; ++i) {
+        double a = -(double)i * (double)i;
+        b += 2.0;
+        d = 1.0 / (a * d + b);
+        c = b + a / c;
+        double del = c * d;
+        hh *= del;
+        if (fabs(del - 1.0) < 1e-16) break;
+    }
+    return hh * exp(-u);
+}
+
+double orc_green2d_gauss(int order, double r, double eps)
+{
+    double x = r * r / (2.0 * eps * eps);
+    double G = (r == 0.0) ? (log(2.0 * eps * eps) - EULER_GAMMA) / (4.0 * PI) : (log(r) + 0.5 * orc_exp1(x)) / (2.0 * PI);
+    double g = exp(-x) / (2.0 * PI * eps * eps);
+    double L[4] = { 1.0, 1.0 - x, 1.0 - 2.0 * x + x * x / 2.0, 1.0 - 3.0 * x + 1.5 * x * x - x * x * x / 6.0 };
+    for (int n = 1; n < order / 2 && n <= 4; ++n) G -= eps * eps / (2.0 * n) * L[n - 1] * g;
+    return G;
+}
+
+/* forward transform on the doubled 2-D grid, half spectrum [P1][N0+1] (x first, then y) */
+static int unb2_forward(const i64 n[2], const double *src, int pad, cplx *spec)
+{
+    i64 P0 = 2 * n[0], P1 = 2 * n[1], H0 = n[0] + 1;
+    cplx *tw = make_twiddles((int)P0);
+    cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)P0 * 3);
+    if (!tw || !buf) { free(tw); free(buf); return ORC_ERR_ALLOC; }
+    for (i64 iy = 0; iy < P1; ++iy) {
+        cplx *in = buf, *out = buf + P0, *scr = buf + 2 * P0;
+        for (i64 ix = 0; ix < P0; ++ix) {
+            double v;
+            if (pad) v = (ix < n[0] && iy < n[1]) ? src[ix + n[0] * iy] : 0.0;
+            else v = src[ix + P0 * iy];
+            in[ix] = v;
+        }
+        fft_rec((int)P0, -1, in, 1, out, scr, tw, 1);
+        for (i64 k = 0; k < H0; ++k) spec[k + H0 * iy] = out[k];
+    }
+    free(tw); free(buf);
+    i64 sdims[3] = { H0, P1, 1 };
+    return fft_axis(spec, sdims, 1, -1);
+}
+
+/* backward (y, then x), 1/(P0 P1), first quadrant extracted; spec is destroyed */
+static int unb2_backward_extract(const i64 n[2], cplx *spec, double *out)
+{
+    i64 P0 = 2 * n[0], P1 = 2 * n[1], H0 = n[0] + 1;
+    i64 sdims[3] = { H0, P1, 1 };
+    int err = fft_axis(spec, sdims, 1, +1);
+    if (err != ORC_OK) return err;
+    cplx *tw = make_twiddles((int)P0);
+    cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)P0 * 3);
+    if (!tw || !buf) { free(tw); free(buf); return ORC_ERR_ALLOC; }
+    double inv = 1.0 / ((double)P0 * (double)P1);
+    for (i64 iy = 0; iy < n[1]; ++iy) {
+        cplx *in = buf, *o = buf + P0, *scr = buf + 2 * P0;
+        const cplx *row = spec + H0 * iy;
+        for (i64 k = 0; k < H0; ++k) in[k] = row[k];
+        for (i64 k = 1; k < n[0]; ++k) in[P0 - k] = conj(row[k]);
+        fft_rec((int)P0, +1, in, 1, o, scr, tw, 1);
+        for (i64 ix = 0; ix < n[0]; ++ix) out[ix + n[0] * iy] = creal(o[ix]) * inv;
+    }
+    free(tw); free(buf);
+    return ORC_OK;
+}
+
+int orc_unbounded2d_green(const i64 n[2], const double h[2], double eps, int order, cplx *ghat)
+{
+    if (order < 2 || order > 10 || (order & 1)) return ORC_ERR_ARG;
+    for (int a = 0; a < 2; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
+    i64 P0 = 2 * n[0], P1 = 2 * n[1];
+    double *g = (double *)malloc(sizeof(double) * (size_t)(P0 * P1));
+    if (!g) return ORC_ERR_ALLOC;
+    double area = h[0] * h[1];
+    for (i64 iy = 0; iy < P1; ++iy)
+        for (i64 ix = 0; ix < P0; ++ix) {
+            double dx = (double)(ix < P0 - ix ? ix : P0 - ix) * h[0];
+            double dy = (double)(iy < P1 - iy ? iy : P1 - iy) * h[1];
+            g[ix + P0 * iy] = area * orc_green2d_gauss(order, sqrt(dx * dx + dy * dy), eps);
+        }
+    int err = unb2_forward(n, g, 0, ghat);
+    free(g);
+    return err;
+}
+
+/* psi and, if grad != NULL, d psi / dx, d psi / dy (eq. (10), wavenumbers of the doubled grid, Nyquist -> 0) */
+int orc_unbounded2d_solve(const i64 n[2], const double h[2], const cplx *ghat, double rhs_sign, const double *f,
+                          double *psi, double *grad)
+{
+    for (int a = 0; a < 2; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
+    i64 P[2] = { 2 * n[0], 2 * n[1] }, H0 = n[0] + 1, ns = H0 * P[1], tot = n[0] * n[1];
+    cplx *spec = (cplx *)malloc(sizeof(cplx) * (size_t)ns), *work = (cplx *)malloc(sizeof(cplx) * (size_t)ns);
+    int err = ORC_OK;
+    if (!spec || !work) { err = ORC_ERR_ALLOC; goto done; }
+    if ((err = unb2_forward(n, f, 1, spec)) != ORC_OK) goto done;
+    for (i64 i = 0; i < ns; ++i) spec[i] = rhs_sign * ghat[i] * spec[i];
+    if (grad) {
+        for (int a = 0; a < 2; ++a) {
+            for (i64 ky = 0; ky < P[1]; ++ky)
+                for (i64 kx = 0; kx < H0; ++kx) {
+                    i64 kk = a ? ky : kx;
+                    i64 m = (kk < n[a]) ? kk : kk - P[a];
+                    double kap = (kk == n[a]) ? 0.0 : 2.0 * PI * (double)m / ((double)P[a] * h[a]);
+                    work[kx + H0 * ky] = I * kap * spec[kx + H0 * ky];
+                }
+            if ((err = unb2_backward_extract(n, work, grad + (size_t)a * (size_t)tot)) != ORC_OK) goto done;
+        }
+    }
+    err = unb2_backward_extract(n, spec, psi);
+done:
+    free(spec); free(work);
+    return err;
+}
+
+/* the definition by direct O(N^4) summation, tiny grids only */
+void orc_unbounded2d_direct(const i64 n[2], const double h[2], double eps, int order, double rhs_sign, const double *f,
+                            double *psi)
+{
+    double area = h[0] * h[1];
+    for (i64 iy = 0; iy < n[1]; ++iy)
+        for (i64 ix = 0; ix < n[0]; ++ix) {
+            long double acc = 0.0L;
+            for (i64 jy = 0; jy < n[1]; ++jy)
+                for (i64 jx = 0; jx < n[0]; ++jx) {
+                    double dx = (double)(ix - jx) * h[0], dy = (double)(iy - jy) * h[1];
+                    acc += (long double)orc_green2d_gauss(order, sqrt(dx * dx + dy * dy), eps) * f[jx + n[0] * jy];
+                }
+            psi[ix + n[0] * iy] = (double)(rhs_sign * area * acc);
+        }
+}
+
 /* Direct O(N^6) evaluation of the definition above (scalar), for tiny grids only (pin P6). */
 void orc_unbounded_direct(const i64 n[3], const double h[3], double eps, double rhs_sign, const double *f,
                           double *psi)
