@@ -107,12 +107,14 @@ typedef struct {
  *   grid   selects the row of Table 1: Dirichlet cell-boundary DST-I, Dirichlet
  *          cell-centre DST-II / DST-III, Neumann cell-boundary DCT-I, Neumann cell-centre DCT-II /
  *          DCT-III; periodic and unbounded accept both (identical numerics).
- *   op     PS / FD2 for periodic, Dirichlet, Neumann; GREEN_GAUSS2 .. GREEN_GAUSS10 or GREEN_SPECTRAL for unbounded (3-D only).
+ *   op     PS / FD2 for periodic, Dirichlet, Neumann; GREEN_GAUSS2 .. GREEN_GAUSS10 for unbounded plans
+ *          (3-D: -erf(r / sqrt2 eps) / (4 pi r) and its higher orders; 2-D: (ln r + E1(r^2 / 2 eps^2) / 2) / (2 pi)
+ *          and its higher orders), GREEN_SPECTRAL for 3-D unbounded plans.
  *   prec   arithmetic and storage type of every array passed later.
  *   opt    [host] may be NULL (defaults above).
  * For unbounded plans this call evaluates G on the doubled grid, transforms it with the library's
  * own fp64 kernels and stores the real, even spectrum as a compact (n+1)^3 table.
- * Errors: INVALID_ARG, UNSUPPORTED (mixed BCs, sizes above, 2-D unbounded, ncomp not 1 or 3,
+ * Errors: INVALID_ARG, UNSUPPORTED (mixed BCs, sizes above, GREEN_SPECTRAL in 2-D, ncomp not 1 or 3,
  * PS/FD2 on unbounded or GREEN on bounded plans), ALLOC, CUDA.
  */
 sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const double h[3], const sf_bc bc[3],
@@ -174,7 +176,7 @@ sf_status sf_divergence(sf_plan plan);
 /* sf_laplacian -- the paper's NABLA operator: for every component lap psi =
  * IDFT(sum_a (i k_a)^2 psi_hat), i.e. DIV of GRAD with the same k_a (zero at the Nyquist index).  With
  * the pseudo-spectral operator this returns the source less its mean and Nyquist planes; with FD2 or
- * a regularised Green's function the source filtered by k^2 / |symbol|.  Periodic and unbounded plans;
+ * a regularised Green's function the source filtered by k^2 / |symbol|.  Periodic and 3-D unbounded plans;
  * psi itself is not produced.  Read the result with SF_OUT_LAP. */
 sf_status sf_laplacian(sf_plan plan);
 

@@ -267,13 +267,57 @@ __device__ double sine_integral(double x)
     sincos(x, &sn, &cs);
     return 1.5707963267948966192 + (hi * cs - hr * sn);
 }
-__global__ void green_eval_kernel(double* g, int Px, int Py, int Pz, double hx, double hy, double hz, double eps, double vol, int order)
+// exponential integral E_1(u), u > 0 (2-D kernels): power series about 0 up to u = 1, continued fraction beyond
+__device__ double exp_integral1(double u)
+{
+    if (u <= 1.0) {
+        double sum = 0.0, term = 1.0;
+        for (int k = 1; k < 60; ++k) {
+            term *= -u / (double)k;
+            const double add = term / (double)k;
+            sum += add;
+            if (fabs(add) < 1e-18 * fabs(sum)) break;
+        }
+        return -0.57721566490153286061 - log(u) - sum;
+    }
+    double b = u + 1.0, c = 1e300, d = 1.0 / b, hh = d;
+    for (int i = 1; i < 500; ++i) {
+        const double a = -(double)i * (double)i;
+        b += 2.0;
+        d = 1.0 / (a * d + b);
+        c = b + a / c;
+        const double del = c * d;
+        hh *= del;
+        if (fabs(del - 1.0) < 1e-16) break;
+    }
+    return hh * exp(-u);
+}
+// 2-D kernels (reading A28): G_2 = (ln r + E_1(r^2 / 2 eps^2) / 2) / (2 pi), orders 4 .. 10 subtract
+// eps^2 / (2 n) L_{n-1}(x) g with the ordinary Laguerre polynomials and the 2-D unit Gaussian g
+__device__ double green2d_value(double r, double eps, int order)
+{
+    const double x = r * r / (2.0 * eps * eps);
+    double v = (r == 0.0) ? (log(2.0 * eps * eps) - 0.57721566490153286061) / 12.566370614359172954
+                          : (log(r) + 0.5 * exp_integral1(x)) / 6.2831853071795864769;
+    if (order >= 4) {
+        const double gs = exp(-x) / (6.2831853071795864769 * eps * eps);
+        double poly = 0.5;                                                              // n = 1: L_0 / 2
+        if (order >= 6) poly += (1.0 - x) * 0.25;                                       // n = 2: L_1 / 4
+        if (order >= 8) poly += ((0.5 * x - 2.0) * x + 1.0) / 6.0;                      // n = 3: L_2 / 6
+        if (order >= 10) poly += (((-x / 6.0 + 1.5) * x - 3.0) * x + 1.0) * 0.125;      // n = 4: L_3 / 8
+        v -= eps * eps * poly * gs;
+    }
+    return v;
+}
+__global__ void green_eval_kernel(double* g, int Px, int Py, int Pz, double hx, double hy, double hz, double eps, double vol, int order,
+                                  int dim2)
 {
     const long long tot = (long long)Px * Py * Pz;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < tot; i += (long long)gridDim.x * blockDim.x) {
         const int ix = (int)(i % Px), iy = (int)((i / Px) % Py), iz = (int)(i / ((long long)Px * Py));
         const double dx = (double)min(ix, Px - ix) * hx, dy = (double)min(iy, Py - iy) * hy, dz = (double)min(iz, Pz - iz) * hz;
         const double r = sqrt(dx * dx + dy * dy + dz * dz);
+        if (dim2) { g[i] = vol * green2d_value(sqrt(dx * dx + dy * dy), eps, order); continue; }
         double v;
         if (order == 0) v = (r == 0.0) ? -1.0 / (6.2831853071795864769 * eps) : -sine_integral(3.14159265358979323846 * r / eps) / (19.739208802178717238 * r);
         else if (r == 0.0) v = -1.0 / (15.749609945722419 * eps); // (2 pi)^(3/2)
@@ -316,7 +360,8 @@ __global__ void green_compact_kernel(const double2* spec, long long s_py, long l
 // (periodic R2C along x, forward strided passes along y and z), keep Re on [0, n]^3.
 template <typename T> sf_status build_green(sf_plan p)
 {
-    const int Px = 2 * (int)p->n[0], Py = 2 * (int)p->n[1], Pz = 2 * (int)p->n[2];
+    const bool two_d = (p->ndim == 2);
+    const int Px = 2 * (int)p->n[0], Py = 2 * (int)p->n[1], Pz = two_d ? 1 : 2 * (int)p->n[2];
     const long long hp = p->pitch; // >= Px/2 + 1
     double* g = nullptr;
     double2* spec = nullptr;
@@ -327,11 +372,12 @@ template <typename T> sf_status build_green(sf_plan p)
     if ((st = dev_alloc(p, (void**)&spec, sbytes)) != SF_OK) return st;
     if ((st = upload_twiddles<double>(p, &twx, Px)) != SF_OK) return st;
     if ((st = upload_twiddles<double>(p, &twy, Py)) != SF_OK) return st;
-    if ((st = upload_twiddles<double>(p, &twz, Pz)) != SF_OK) return st;
-    const double eps = (p->op == SF_OP_GREEN_SPECTRAL ? 1.0 : p->eps_over_h) * fmax(p->h[0], fmax(p->h[1], p->h[2]));
-    const double vol = p->h[0] * p->h[1] * p->h[2];
+    if (!two_d && (st = upload_twiddles<double>(p, &twz, Pz)) != SF_OK) return st;
+    const double hmax = two_d ? fmax(p->h[0], p->h[1]) : fmax(p->h[0], fmax(p->h[1], p->h[2]));
+    const double eps = (p->op == SF_OP_GREEN_SPECTRAL ? 1.0 : p->eps_over_h) * hmax;
+    const double vol = two_d ? p->h[0] * p->h[1] : p->h[0] * p->h[1] * p->h[2];
     const int order = (p->op == SF_OP_GREEN_SPECTRAL) ? 0 : 2 * ((int)p->op - (int)SF_OP_GREEN_GAUSS2 + 1);
-    green_eval_kernel<<<148 * 8, 256, 0, p->stream>>>(g, Px, Py, Pz, p->h[0], p->h[1], p->h[2], eps, vol, order);
+    green_eval_kernel<<<148 * 8, 256, 0, p->stream>>>(g, Px, Py, Pz, p->h[0], p->h[1], p->h[2], eps, vol, order, two_d ? 1 : 0);
     SF_CUDA(p, cudaGetLastError());
 
     XParams<double> xp;
@@ -352,19 +398,22 @@ template <typename T> sf_status build_green(sf_plan p)
     sp.n_in = Py; sp.n_out = Py; sp.LT = Py; sp.tw = (const double2*)twy;
     SF_CUDA(p, launch_spass<double>(Py, 0, sp, Pz, 1, 1, p->stream));
     // along z
-    sp.in_ps = sp.out_ps = hp * Py; sp.in_bs = sp.out_bs = hp;
-    sp.n_in = Pz; sp.n_out = Pz; sp.LT = Pz; sp.tw = (const double2*)twz;
-    SF_CUDA(p, launch_spass<double>(Pz, 0, sp, Py, 1, 1, p->stream));
+    if (!two_d) {
+        sp.in_ps = sp.out_ps = hp * Py; sp.in_bs = sp.out_bs = hp;
+        sp.n_in = Pz; sp.n_out = Pz; sp.LT = Pz; sp.tw = (const double2*)twz;
+        SF_CUDA(p, launch_spass<double>(Pz, 0, sp, Py, 1, 1, p->stream));
+    }
 
-    const int gx = (int)p->n[0] + 1, gy = (int)p->n[1] + 1, gz = (int)p->n[2] + 1;
+    const int gx = (int)p->n[0] + 1, gy = (int)p->n[1] + 1, gz = two_d ? 1 : (int)p->n[2] + 1;
     if ((st = dev_alloc(p, &p->green, (size_t)hp * gy * gz * sizeof(T))) != SF_OK) return st;
     SF_CUDA(p, cudaMemsetAsync(p->green, 0, (size_t)hp * gy * gz * sizeof(T), p->stream));
     const double factor = p->rhs_sign / ((double)Px * (double)Py * (double)Pz);
     green_compact_kernel<T><<<148 * 8, 256, 0, p->stream>>>(spec, hp, hp * Py, (T*)p->green, hp, hp * gy, gx, gy, gz, factor);
     SF_CUDA(p, cudaGetLastError());
     SF_CUDA(p, cudaStreamSynchronize(p->stream));
-    dev_free(p, g); dev_free(p, spec); dev_free(p, twx); dev_free(p, twy); dev_free(p, twz);
-    p->dev_bytes -= (long long)(gbytes + sbytes + (size_t)(Px + Py + Pz) * 16);
+    dev_free(p, g); dev_free(p, spec); dev_free(p, twx); dev_free(p, twy);
+    if (!two_d) dev_free(p, twz);
+    p->dev_bytes -= (long long)(gbytes + sbytes + (size_t)(Px + Py + (two_d ? 0 : Pz)) * 16);
     return SF_OK;
 }
 
@@ -538,11 +587,14 @@ template <typename T> sf_status run(sf_plan p, int outk)
             sp.Pb = p->P[1];
             sp.g_pb = hp; sp.g_pp = hp * (n1 + 1);
         } else {
+            // 2-D: the fused pass follows S1 directly, in place on W1 (rows >= n of a padded pencil exist only in shared memory)
+            sp.in = p->W1; sp.out = p->W1;
             sp.in_ps = sp.out_ps = hp; sp.in_bs = sp.out_bs = 0;
             sp.lam_b = (const T*)p->zero1; sp.kap_b = (const T*)p->zero1;
             sp.Pb = 1;
+            sp.g_pb = 0; sp.g_pp = hp;
         }
-        sp.in_cs = sp.out_cs = p->w2_field;
+        sp.in_cs = sp.out_cs = (nd == 3) ? p->w2_field : p->w1_field;
         sp.lam_x = (const T*)p->lam[0]; sp.kap_x = (const T*)p->kap[0];
         sp.lam_p = (const T*)p->lam[ax]; sp.kap_p = (const T*)p->kap[ax];
         sp.Pp = p->P[ax];
@@ -632,7 +684,7 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
     const sf_bc b = bc[0];
     if (b == SF_BC_UNBOUNDED) {
         if (!green_op) return fail(nullptr, SF_ERR_UNSUPPORTED, "unbounded plans use a Green's function operator");
-        if (ndim != 3) return fail(nullptr, SF_ERR_UNSUPPORTED, "2-D unbounded plans are not built");
+        if (ndim != 3 && op == SF_OP_GREEN_SPECTRAL) return fail(nullptr, SF_ERR_UNSUPPORTED, "the spectrally compact kernel is built for 3-D");
     } else if (green_op) {
         return fail(nullptr, SF_ERR_UNSUPPORTED, "Green's function operators need unbounded boundary conditions");
     }
@@ -826,7 +878,8 @@ sf_status sf_gradient(sf_plan plan)
     if (!plan) return SF_ERR_INVALID_ARG;
     if (plan->ncomp != 1) return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient is built for scalar plans");
     if (plan->bc == SF_BC_PERIODIC) return run_any(plan, OUT_GRAD);
-    if (plan->ndim != 3) return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient on Dirichlet / Neumann plans is built for 3-D");
+    if (plan->ndim != 3 && plan->bc != SF_BC_UNBOUNDED)
+        return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient on Dirichlet / Neumann plans is built for 3-D");
     // unbounded, Dirichlet, Neumann: psi and its derivatives need 1 + ndim fields of work space
     const int nf = 1 + plan->ndim;
     {
@@ -882,6 +935,7 @@ sf_status sf_laplacian(sf_plan plan)
     if (!plan) return SF_ERR_INVALID_ARG;
     if (plan->bc != SF_BC_PERIODIC && plan->bc != SF_BC_UNBOUNDED)
         return fail(plan, SF_ERR_UNSUPPORTED, "sf_laplacian is built for periodic and unbounded plans");
+    if (plan->bc == SF_BC_UNBOUNDED && plan->ndim != 3) return fail(plan, SF_ERR_UNSUPPORTED, "sf_laplacian on unbounded plans is built for 3-D");
     return run_any(plan, OUT_LAP);
 }
 

@@ -1,0 +1,82 @@
+"""Parity of 2-D unbounded plans (reading A28) through the C ABI against the oracle."""
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+import paper_2301_01145_b200 as sf
+from gpu_solve import TOL, Plan, rel_l2, rounded
+
+pytestmark = pytest.mark.gpu
+
+_OPS = {2: sf.SF_OP_GREEN_GAUSS2, 4: sf.SF_OP_GREEN_GAUSS4, 6: sf.SF_OP_GREEN_GAUSS6, 8: sf.SF_OP_GREEN_GAUSS8,
+        10: sf.SF_OP_GREEN_GAUSS10}
+
+
+def _rand(shape, seed):
+    return W.Rng(seed).normal(int(np.prod(shape))).reshape(shape)
+
+
+def _report(name, got, ref, prec):
+    e = rel_l2(got, ref)
+    print(f"{name}: rel-L2 {e:.3e} (tol {TOL[prec]:.0e})")
+    assert np.isfinite(e) and e <= TOL[prec], f"{name}: rel-L2 {e:.3e} > {TOL[prec]:.0e}"
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("order", [2, 4, 10])
+@pytest.mark.parametrize("shape", [(64, 128), (256, 32)])
+def test_unbounded_2d_white_noise(shape, order, prec):
+    ny, nx = shape
+    f = rounded(_rand(shape, 300 + order), prec)
+    h = (0.011, 0.017)
+    eps = 2.0 * max(h)
+    gh = O.unbounded2d_green((nx, ny), h, eps, order)
+    psi_o, grad_o = O.unbounded2d_solve(f.astype(np.float64), h, gh, rhs_sign=-1.0, want_grad=True)
+    with Plan(shape, h, sf.SF_BC_UNBOUNDED, op=_OPS[order], prec=prec, rhs_sign=-1.0) as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        assert sf.sf_last_launch_count(p.plan) == 3      # S1, fused S3 along y, S5
+        _report(f"psi 2-D order {order}", p.get(sf.SF_OUT_PSI), psi_o, prec)
+        sf.sf_gradient(p.plan)
+        _report("psi (gradient call)", p.get(sf.SF_OUT_PSI), psi_o, prec)
+        for a in range(2):
+            _report(f"grad[{a}]", p.get(sf.SF_OUT_GRAD, a), grad_o[a], prec)
+        sf.sf_solve(p.plan)
+        _report("psi again", p.get(sf.SF_OUT_PSI), psi_o, prec)
+
+
+def test_unbounded_2d_unit_source_and_closed_form():
+    """a unit source returns h^2 G itself; a Gaussian charge the closed form (ln r + E1(r^2/2s^2)/2)/(2 pi)"""
+    import scipy.special as sp
+    n, h = 128, 1.0 / 128
+    eps = 2 * h
+    with Plan((n, n), (h, h), sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec="f64") as p:
+        e = np.zeros((n, n))
+        e[70, 5] = 1.0
+        p.set_source(e)
+        sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI)
+        for (iy, ix) in ((70, 5), (0, 0), (127, 127), (71, 5), (70, 9)):
+            r = h * float(np.hypot(ix - 5, iy - 70))
+            assert got[iy, ix] == pytest.approx(h * h * O.green2d_gauss(2, r, eps), rel=1e-11, abs=1e-17)
+        x = (np.arange(n) + 0.5) * h
+        sig, cx, cy = 3.0 * h, 0.47, 0.55
+        r2 = (x[None, :] - cx) ** 2 + (x[:, None] - cy) ** 2
+        f = np.exp(-r2 / (2 * sig * sig)) / (2 * np.pi * sig * sig)
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        s2 = sig * sig + eps * eps
+        want = (0.5 * np.log(r2) + 0.5 * sp.exp1(r2 / (2 * s2))) / (2 * np.pi)
+        assert np.abs(p.get(sf.SF_OUT_PSI) - want).max() < 1e-9 * np.abs(want).max()
+
+
+def test_unbounded_2d_unsupported_calls():
+    with pytest.raises(sf.SailffishError) as ei:
+        Plan((64, 64), (0.1, 0.1), sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_SPECTRAL)
+    assert ei.value.status == sf.SF_ERR_UNSUPPORTED
+    with Plan((64, 64), (0.1, 0.1), sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2) as p:
+        p.set_source(_rand((64, 64), 1))
+        with pytest.raises(sf.SailffishError) as ei:
+            sf.sf_laplacian(p.plan)
+        assert ei.value.status == sf.SF_ERR_UNSUPPORTED
