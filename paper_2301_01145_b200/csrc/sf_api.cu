@@ -93,6 +93,7 @@ struct sf_plan_s {
     int tslots = 0;               // step timing: compute calls remembered (0 = off)
     long long tcount = 0;         // compute calls recorded since timing was enabled
     int tstride = 1;              // record every tstride-th compute call
+    bool fastper = false;         // periodic fp32 plans with 256-point y / z pencils: generation-2 strided passes
     long long tcalls = 0;         // compute calls seen since timing was enabled
     std::vector<cudaEvent_t> ev;  // 6 events per slot
     std::string err = "";
@@ -502,7 +503,9 @@ template <typename T> sf_status run(sf_plan p, int outk)
         fx.nyq = (sf2::C*)p->nyqA; fx.n1 = n1; fx.n2 = n2;
         SF_CUDA(p, sf2::launch_fast_x(false, fx, st));
     } else {
+        if (p->fastper && outk == OUT_SOLVE) xp.nyq_side = p->nyqA;
         SF_CUDA(p, launch_xfwd<T>(p->Lx, xp, ncomp, st));
+        xp.nyq_side = nullptr;
     }
     p->launches++;
     mark(1);
@@ -556,6 +559,47 @@ template <typename T> sf_status run(sf_plan p, int outk)
         fx.reverse = 1;           // S4 wrote the last planes last
         if (fast_x) SF_CUDA(p, sf2::launch_fast_x(true, fx, st));
         else SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        p->launches++;
+        mark(5);
+        if (timed) p->tcount++;
+        p->last_kind = outk;
+        p->out_last = p->out;
+        return SF_OK;
+    }
+
+    if (p->fastper && outk == OUT_SOLVE) {
+        // kernel generation 2, periodic: S2, S3, S4 in place on W1 as persistent register-FFT kernels
+        sf2::FastPerParams fp;
+        memset(&fp, 0, sizeof(fp));
+        fp.sched = (int*)p->sched;
+        fp.in = (const sf2::C*)p->W1; fp.out = (sf2::C*)p->W1;
+        fp.nx = p->nspec_x;
+        fp.nct = p->nspec_x / sf2::kPerTileCols;
+        fp.nyq_col = (p->nspec_x % sf2::kPerTileCols) ? fp.nct * sf2::kPerTileCols : -1;
+        fp.nyq = (sf2::C*)p->nyqA;
+        // S2 along y: batches = z planes
+        fp.in_ps = fp.out_ps = hp; fp.in_bs = fp.out_bs = hp * n1; fp.nb = n2;
+        fp.nyq_ps = 1; fp.nyq_bs = n1;
+        SF_CUDA(p, sf2::launch_fast_per(sf2::FMODE_FWD, fp, st));
+        p->launches++;
+        mark(2);
+        // S3 along z: batches = ky
+        fp.in_ps = fp.out_ps = hp * n1; fp.in_bs = fp.out_bs = hp; fp.nb = n1;
+        fp.nyq_ps = n1; fp.nyq_bs = 1;
+        fp.lam_x = (const float*)p->lam[0]; fp.lam_b = (const float*)p->lam[1]; fp.lam_p = (const float*)p->lam[2];
+        fp.scale = (float)p->scale; fp.zero_mode = 1;
+        SF_CUDA(p, sf2::launch_fast_per(sf2::FMODE_FUSED, fp, st));
+        p->launches++;
+        mark(3);
+        // S4 along y
+        fp.in_ps = fp.out_ps = hp; fp.in_bs = fp.out_bs = hp * n1; fp.nb = n2;
+        fp.nyq_ps = 1; fp.nyq_bs = n1;
+        SF_CUDA(p, sf2::launch_fast_per(sf2::FMODE_INV, fp, st));
+        p->launches++;
+        mark(4);
+        xp.spec_in = p->W1; xp.real_out = (T*)p->out;
+        xp.nyq_side = p->nyqA;
+        SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
         p->launches++;
         mark(5);
         if (timed) p->tcount++;
@@ -823,6 +867,15 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
             if ((st = dev_alloc(p, &p->nyqA, (size_t)256 * 256 * 8)) != SF_OK) return bail(st, "");
             if ((st = dev_alloc(p, &p->nyqB, (size_t)256 * 512 * 8)) != SF_OK) return bail(st, "");
         }
+    }
+    // ... and periodic fp32 scalar plans with 256-point y and z pencils (strided passes only)
+    if (prec == SF_F32 && b == SF_BC_PERIODIC && ndim == 3 && ncomp == 1 && p->n[1] == 256 && p->n[2] == 256 &&
+        p->nspec_x >= sf2::kPerTileCols && (p->nspec_x % sf2::kPerTileCols) <= 1 && p->n[0] <= 4096 && !getenv("SF_DISABLE_FAST")) {
+        if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fp32 fast path failed"); }
+        if ((st = dev_alloc(p, &p->sched, 2 * sizeof(int))) != SF_OK) return bail(st, "");
+        if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
+        if ((st = dev_alloc(p, &p->nyqA, (size_t)p->n[1] * p->n[2] * 8)) != SF_OK) return bail(st, "");   // Nyquist column [z][y]
+        p->fastper = true;
     }
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "plan construction failed on the device");
     *out = p;

@@ -1,8 +1,10 @@
 // sf_fast.cu -- the one translation unit of kernel generation 2 (sf_fast.cuh): constant tables,
 // shared-memory opt-in and the persistent-grid launchers.
 #include "sf_fast.cuh"
+#include "sf_fastper.cuh"
 
 #include <cmath>
+#include <cstdlib>
 #include <mutex>
 #include <vector>
 
@@ -57,6 +59,9 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_FWD>::kSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_INV>::kSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_FUSED>::kSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     void* fn = nullptr;
@@ -131,6 +136,24 @@ cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map
     case FMODE_FWD: fast_pad_kernel<FMODE_FWD><<<grid, kThreads, FastCfg<FMODE_FWD>::kSmem, st>>>(p, tm); break;
     case FMODE_INV: fast_pad_kernel<FMODE_INV><<<grid, kThreads, FastCfg<FMODE_INV>::kSmem, st>>>(p, tm); break;
     case FMODE_FUSED: fast_pad_kernel<FMODE_FUSED><<<grid, kThreads, FastCfg<FMODE_FUSED>::kSmem, st>>>(p, tm); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st)
+{
+    if (p.nyq_col >= 0 && !p.nyq) return cudaErrorInvalidValue;
+    if (p.nct <= 0 || p.nb <= 0) return cudaErrorInvalidValue;
+    if ((long long)p.nb * p.in_bs + 256 * p.in_ps >= (1ll << 31) || (long long)p.nb * p.out_bs + 256 * p.out_ps >= (1ll << 31))
+        return cudaErrorInvalidValue;
+    const int ntiles = p.nb * p.nct + (p.nyq_col >= 0 ? (p.nb + kPerTile - 1) / kPerTile : 0);
+    int grid = 2 * g_sms;
+    if (grid > ntiles) grid = ntiles;
+    switch (mode) {
+    case FMODE_FWD: fast_per_kernel<FMODE_FWD><<<grid, kThreads, kPerSmem, st>>>(p); break;
+    case FMODE_INV: fast_per_kernel<FMODE_INV><<<grid, kThreads, kPerSmem, st>>>(p); break;
+    case FMODE_FUSED: fast_per_kernel<FMODE_FUSED><<<grid, kThreads, kPerSmem, st>>>(p); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

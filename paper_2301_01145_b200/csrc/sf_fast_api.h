@@ -53,6 +53,25 @@ struct FastXParams {
     int n1, n2;             // S1 writes it (besides column 256 of spec), S5 reads it (instead); NULL: column 256 only
 };
 
+constexpr int kPerTileCols = 32;
+// strided passes of periodic plans with 256-point pencils (fast_per_kernel): tiles of 32 columns
+struct FastPerParams {
+    const C* in;
+    C* out;
+    long long in_ps, in_bs, out_ps, out_bs;   // row and batch strides, complex elements
+    int nb;          // batches
+    int nx;          // valid columns
+    int nct;         // full 32-column tiles per batch
+    int nyq_col;     // column handled 32 batches at a time, -1: none
+    int* sched;      // device: { next unclaimed tile, CTAs finished }, zero between launches
+    C* nyq;          // side array that holds column nyq_col: element (row, batch) at row * nyq_ps + batch * nyq_bs
+    long long nyq_ps, nyq_bs;
+    // fused multiply: scale / (lam_x[column] + lam_b[batch] + lam_p[row]), zero mode -> 0
+    const float* lam_x; const float* lam_b; const float* lam_p;
+    float scale;
+    int zero_mode;
+};
+
 // opaque storage of a CUtensorMap (TMA descriptor): 128 bytes, 64-byte aligned
 struct alignas(64) TileMap { unsigned char bytes[128]; };
 
@@ -76,5 +95,7 @@ cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map
 
 // launch S1 (inv = false) or S5 (inv = true) as a persistent grid of two CTAs per SM
 cudaError_t launch_fast_x(bool inv, const FastXParams& p, cudaStream_t st);
+// launch one periodic strided pass (mode = FMODE_*) as a persistent grid of two CTAs per SM
+cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st);
 
 } // namespace sf2

@@ -1,0 +1,199 @@
+// sf_fastper.cuh -- kernel generation 2 for periodic fp32 plans whose y and z pencils are 256 long
+// (BASELINE.json configs[1]): the strided passes S2 (Y forward), S3 (Z forward x 1 / eigenvalue x
+// Z backward, fused) and S4 (Y backward) with the register-resident 256-point transform of
+// sf_fast.cuh (PAPER.md:89-97 pencils, :103-109 four-step solve, Table 1 PAPER.md:160-167 periodic
+// eigenvalues, zero mode PAPER.md:69).
+//
+// There is no padding here, so a thread has one transform to do instead of the two halves of the
+// padded kernels: lane = pencil, and a CTA of 512 threads owns 32 neighbouring pencils -- every row
+// of a tile is one 256-byte run, read straight into registers (the tile image is the 16 elements
+// n = o + 16 r that thread (o, pencil) needs anyway) and written straight back.  Warp = o as in
+// sf_fast.cuh; persistent CTAs, two per SM, tiles handed out by an atomic counter.
+// The column count of a real-to-complex spectrum is n/2 + 1 = 4 * 32 + 1: the last (Nyquist)
+// column is kept in a compact side array [z][y] that S1 writes and S5 reads instead of that column,
+// and is handled 32 batches at a time (lane = batch), first in the queue.
+#pragma once
+#include "sf_fast.cuh"
+
+namespace sf2 {
+
+constexpr int kPerTile = 32;
+constexpr size_t kPerSmem = (size_t)16 * 16 * 32 * sizeof(C);   // the exchange buffer
+
+// tile t -> geometry
+struct PerGeom {
+    bool full;
+    int b, col;   // full: batch, first column; else: first batch, the column
+};
+__device__ __forceinline__ PerGeom per_geom(const FastPerParams& p, int t)
+{
+    PerGeom g;
+    const int nnyq = (p.nyq_col >= 0) ? (p.nb + kPerTile - 1) / kPerTile : 0;
+    if (t < nnyq) {
+        g.full = false;
+        g.b = t * kPerTile;
+        g.col = p.nyq_col;
+    } else {
+        const int tf = t - nnyq;
+        g.full = true;
+        g.b = tf / p.nct;
+        g.col = (tf - g.b * p.nct) * kPerTile;
+    }
+    return g;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(kThreads, 2) fast_per_kernel(const FastPerParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    C* xbuf = reinterpret_cast<C*>(smem_raw);
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int o = (int)__reduce_max_sync(0xffffffffu, (unsigned)(tid >> 5));
+    Xchg xc;
+    xc.base = xbuf;
+    xc.ea = o * 32 + lane;
+    xc.eb = o * 512 + lane;
+
+    __shared__ __align__(16) C s_t256[256];      // w256^(q o), row o
+    __shared__ float s_lamp[256];                // fused: eigenvalue contribution of the pencil axis
+    __shared__ int s_tile[2];
+    if (tid < 128) reinterpret_cast<float4*>(s_t256)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid];
+    if (MODE == FMODE_FUSED && tid < 256) s_lamp[tid] = __ldg(p.lam_p + tid);
+    const C* t256 = s_t256 + o * 16;
+    if (tid == 0) {
+        s_tile[0] = atomicAdd(p.sched, 1);
+        s_tile[1] = atomicAdd(p.sched, 1);
+    }
+    __syncthreads();
+
+    const int ntiles = p.nb * p.nct + ((p.nyq_col >= 0) ? (p.nb + kPerTile - 1) / kPerTile : 0);
+    const int ips = (int)p.in_ps, ops = (int)p.out_ps, ibs = (int)p.in_bs, obs = (int)p.out_bs;
+
+    // one tile; OB = orientation of the exchange buffer its first transform starts with
+    auto tile = [&](int t, int it, auto orient_tag) {
+        constexpr bool OB = decltype(orient_tag)::value;
+        const PerGeom g = per_geom(p, t);
+        const bool valid = g.full ? (g.col + lane < p.nx) : (g.b + lane < p.nb);
+        // Nyquist-column tiles live in a compact side array (element (row, batch) at row * nyq_ps +
+        // batch * nyq_bs): column nyq_col of the work array itself would be gathered in 8-byte pieces a
+        // whole plane apart, which costs more than all full tiles together (measured)
+        const C* ibase = g.full ? p.in + (g.b * ibs + g.col + lane) : p.nyq + min(g.b + lane, p.nb - 1) * (int)p.nyq_bs;
+        C* obase = g.full ? p.out + (g.b * obs + g.col + lane) : p.nyq + (g.b + lane) * (int)p.nyq_bs;
+        const int irs = g.full ? ips : (int)p.nyq_ps, ors = g.full ? ops : (int)p.nyq_ps;
+        // side-array tiles whose rows are contiguous in memory (the y passes: [z][y], lane = z) are moved as
+        // 256-byte runs and transposed in the exchange buffer, idle at both ends of a tile: element
+        // (row, pencil) at row * 32 + ((pencil + row) & 31), conflict-free along rows and along pencils
+        const bool transposed = !g.full && p.nyq_ps == 1;
+        auto stage = [&](int row, int pencil) -> C& { return xbuf[row * 32 + ((pencil + row) & 31)]; };
+        C v[16];
+        if (transposed) {
+#pragma unroll 4
+            for (int j = 0; j < 16; ++j) {
+                const int idx = tid + kThreads * j, pl = idx >> 8, row = idx & 255;
+                stage(row, pl) = (g.b + pl < p.nb) ? __ldg(p.nyq + (g.b + pl) * (int)p.nyq_bs + row) : make_float2(0.f, 0.f);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = stage(o + 16 * r, lane);
+            __syncthreads();
+        } else {
+            const C* ip = ibase + o * irs;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = valid ? __ldg(ip + r * 16 * irs) : make_float2(0.f, 0.f);
+        }
+        // mirror of the transposing load for the results v[brev4(k)] = element o + 16 k
+        auto store_transposed = [&](const C (&u)[16]) {
+            __syncthreads();   // every thread is done reading the exchange buffer
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) stage(o + 16 * k2, lane) = u[brev4(k2)];
+            __syncthreads();
+#pragma unroll 4
+            for (int j = 0; j < 16; ++j) {
+                const int idx = tid + kThreads * j, pl = idx >> 8, row = idx & 255;
+                if (g.b + pl < p.nb) p.nyq[(g.b + pl) * (int)p.nyq_bs + row] = stage(row, pl);
+            }
+            __syncthreads();   // before the next tile's exchange
+        };
+        // after the tile's first barrier every thread has read this tile's index: claim the tile after next
+        // (the next tile's barrier publishes it)
+        auto claim = [&]() { if (tid == 0) s_tile[it & 1] = atomicAdd(p.sched, 1); };
+        if constexpr (MODE == FMODE_FWD) {
+            fft256_a<false, OB, false>(v, t256, o, xc);
+            __syncthreads();
+            claim();
+            fft256_b<false, OB>(v, xc);
+            if (transposed) {
+                store_transposed(v);
+            } else if (valid) {
+                C* q = obase + o * ors;
+#pragma unroll
+                for (int k2 = 0; k2 < 16; ++k2) q[k2 * 16 * ors] = v[brev4(k2)];
+            }
+        } else if constexpr (MODE == FMODE_INV) {
+            fft256_a<true, OB, true>(v, t256, o, xc);
+            __syncthreads();
+            claim();
+            fft256_b<true, OB>(v, xc);
+            if (transposed) {
+                store_transposed(v);
+            } else if (valid) {
+                C* q = obase + o * ors;
+#pragma unroll
+                for (int j2 = 0; j2 < 16; ++j2) q[j2 * 16 * ors] = v[brev4(j2)];
+            }
+        } else {
+            fft256_a<false, OB, true>(v, t256, o, xc);
+            __syncthreads();
+            claim();
+            fft256_b<false, OB>(v, xc);
+            // X[k = o + 16 k2] at v[brev4(k2)]: multiply by scale / (lambda_x + lambda_b + lambda_p[k]), zero mode -> 0
+            const int kx = g.full ? min(g.col + lane, p.nx - 1) : g.col;
+            const int kb = g.full ? g.b : min(g.b + lane, p.nb - 1);
+            const float lxb = __ldg(p.lam_x + kx) + __ldg(p.lam_b + kb);
+            const bool zero0 = p.zero_mode && kx == 0 && kb == 0 && o == 0;
+            C w[16];
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) {
+                float m = p.scale * __frcp_rn(lxb + s_lamp[o + 16 * k2]);
+                if (k2 == 0 && zero0) m = 0.f;
+                w[k2] = cscale(v[brev4(k2)], m);
+            }
+            fft256_a<true, !OB, true>(w, t256, o, xc);
+            __syncthreads();
+            fft256_b<true, !OB>(w, xc);
+            if (valid) {
+                C* q = obase + o * ors;
+#pragma unroll
+                for (int j2 = 0; j2 < 16; ++j2) q[j2 * 16 * ors] = w[brev4(j2)];
+            }
+        }
+    };
+
+    if constexpr (MODE == FMODE_FUSED) {
+        for (int it = 0;; ++it) {
+            const int t = s_tile[it & 1];
+            if (t >= ntiles) break;
+            tile(t, it, std::false_type());
+        }
+    } else {
+        for (int it = 0;; it += 2) {
+            int t = s_tile[0];
+            if (t >= ntiles) break;
+            tile(t, it, std::false_type());
+            t = s_tile[1];
+            if (t >= ntiles) break;
+            tile(t, it + 1, std::true_type());
+        }
+    }
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(p.sched + 1, 1) == (int)gridDim.x - 1) {
+            p.sched[0] = 0;
+            p.sched[1] = 0;
+            __threadfence();
+        }
+    }
+}
+
+} // namespace sf2

@@ -40,6 +40,9 @@ template <typename T> struct XParams {
     const T* face[6];
     T wface[6];
     int has_faces;
+    // periodic / zero-padded: optional side array [row] that holds the last column (k = L, the Nyquist
+    // coefficient) of every row instead of the spectrum array (sf_fastper.cuh)
+    void* nyq_side;
     // backward, real modes: spectral derivative along x of one field (sine <-> cosine series, eq. (10))
     int dfield1;        // 1 + index of the field (blockIdx.y) that is differentiated; 0: none
     const T* kap_ext;   // pi k / L_domain for slot k <= L of the extended sequence, zero at k = L
@@ -171,7 +174,8 @@ __global__ void __launch_bounds__(NT) xfwd_kernel(const XParams<T> p)
             const long long row = row0 + r;
             if (row < nrows) {
                 const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-                so[iy * p.sp_py + iz * p.sp_pz + k] = G[r * LP + k];
+                if (k == L && p.nyq_side) reinterpret_cast<C*>(p.nyq_side)[row] = G[r * LP + k];
+                else so[iy * p.sp_py + iz * p.sp_pz + k] = G[r * LP + k];
             }
         }
     } else {
@@ -228,7 +232,8 @@ __global__ void __launch_bounds__(NT) xinv_kernel(const XParams<T> p)
             C x = mk<T>(0, 0);
             if (row < nrows) {
                 const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-                x = si[iy * p.sp_py + iz * p.sp_pz + k];
+                if (k == L && p.nyq_side) x = reinterpret_cast<const C*>(p.nyq_side)[row];
+                else x = si[iy * p.sp_py + iz * p.sp_pz + k];
             }
             A[r * LP + k] = x;
         }

@@ -333,3 +333,40 @@ def test_cfg5_full_size():
     print(f"cfg5 512^3: u(centre) = {uc}, |u| 2R/Gamma = {np.linalg.norm(uc) * 2 * v['radius'] / v['gamma']:.4f}, cos = {cosang:.6f}")
     assert cosang >= 0.9999
     assert np.linalg.norm(uc) * 2 * v["radius"] / v["gamma"] == pytest.approx(1.0, abs=0.02)
+
+
+# ------------------------------------------------------------------- periodic fast path (sf_fastper.cuh)
+@pytest.mark.parametrize("nx,op", [(64, "fd2"), (128, "ps"), (256, "fd2"), (512, "ps")])
+def test_periodic_fast_path_white_noise(nx, op, monkeypatch):
+    """fp32 periodic plans with 256-point y and z pencils take the generation-2 strided passes (32-column
+    tiles plus the Nyquist column, lane = batch): white noise against the oracle, plane by plane, and
+    against the generation-1 kernels of the same plan"""
+    shape = (256, 256, nx)
+    f = rounded(W.Rng(7000 + nx).normal(int(np.prod(shape))).reshape(shape), "f32")
+    f -= f.mean(dtype=np.float64).astype(np.float32)
+    L = (2.0, 1.0, 3.0)
+    h = (L[0] / nx, L[1] / 256, L[2] / 256)
+    oop, sop = (O.OP_PS, sf.SF_OP_PSEUDO_SPECTRAL) if op == "ps" else (O.OP_FD2, sf.SF_OP_FD2)
+    ref = O.periodic(f.astype(np.float64), L, oop, rhs_sign=-1.0)
+    got = {}
+    for name, disable in (("generation 2", False), ("generation 1", True)):
+        if disable:
+            monkeypatch.setenv("SF_DISABLE_FAST", "1")
+        else:
+            monkeypatch.delenv("SF_DISABLE_FAST", raising=False)
+        with Plan(shape, h, sf.SF_BC_PERIODIC, op=sop, prec="f32", rhs_sign=-1.0) as p:
+            p.set_source(f)
+            for _ in range(3):   # the tile counter must be re-armed between launches
+                sf.sf_solve(p.plan)
+            assert sf.sf_last_launch_count(p.plan) == 5
+            got[name] = p.get(sf.SF_OUT_PSI)
+            _check(f"periodic 256x256x{nx} {op} {name}", got[name], ref, "f32")
+            if not disable:
+                sf.sf_gradient(p.plan)     # generation-1 kernels on the same plan
+                _check("psi (gradient call)", p.get(sf.SF_OUT_PSI), ref, "f32")
+                sf.sf_solve(p.plan)
+                _check("psi (solve again)", p.get(sf.SF_OUT_PSI), ref, "f32")
+    err = np.linalg.norm((got["generation 2"].astype(np.float64) - ref).reshape(256, -1), axis=1)
+    nrm = np.linalg.norm(ref.reshape(256, -1), axis=1)
+    assert (err <= 10 * TOL["f32"] * nrm).all()
+    assert rel_l2(got["generation 2"], got["generation 1"].astype(np.float64)) <= 1e-6
