@@ -94,6 +94,7 @@ struct sf_plan_s {
     long long tcount = 0;         // compute calls recorded since timing was enabled
     int tstride = 1;              // record every tstride-th compute call
     bool fastper = false;         // periodic fp32 plans with 256-point y / z pencils: generation-2 strided passes
+    bool fastper_x = false;       // ... and rows of 256 reals: generation-2 X passes
     long long tcalls = 0;         // compute calls seen since timing was enabled
     std::vector<cudaEvent_t> ev;  // 6 events per slot
     std::string err = "";
@@ -502,6 +503,12 @@ template <typename T> sf_status run(sf_plan p, int outk)
         fx.spec = (sf2::C*)p->W1; fx.spec_pitch = hp; fx.nrows = n1 * n2;
         fx.nyq = (sf2::C*)p->nyqA; fx.n1 = n1; fx.n2 = n2;
         SF_CUDA(p, sf2::launch_fast_x(false, fx, st));
+    } else if (p->fastper && p->fastper_x && outk == OUT_SOLVE && !xp.has_faces) {
+        sf2::FastXPerParams px;
+        memset(&px, 0, sizeof(px));
+        px.real_in = (const float*)p->src; px.spec = (sf2::C*)p->W1; px.spec_pitch = hp; px.nrows = n1 * n2;
+        px.nyq = (sf2::C*)p->nyqA;
+        SF_CUDA(p, sf2::launch_fast_xper(false, px, st));
     } else {
         if (p->fastper && outk == OUT_SOLVE) xp.nyq_side = p->nyqA;
         SF_CUDA(p, launch_xfwd<T>(p->Lx, xp, ncomp, st));
@@ -599,7 +606,15 @@ template <typename T> sf_status run(sf_plan p, int outk)
         mark(4);
         xp.spec_in = p->W1; xp.real_out = (T*)p->out;
         xp.nyq_side = p->nyqA;
-        SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        if (p->fastper_x) {
+            sf2::FastXPerParams px;
+            memset(&px, 0, sizeof(px));
+            px.real_out = (float*)p->out; px.spec = (sf2::C*)p->W1; px.spec_pitch = hp; px.nrows = n1 * n2;
+            px.nyq = (sf2::C*)p->nyqA;
+            SF_CUDA(p, sf2::launch_fast_xper(true, px, st));
+        } else {
+            SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        }
         p->launches++;
         mark(5);
         if (timed) p->tcount++;
@@ -876,6 +891,7 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
         if ((st = dev_alloc(p, &p->nyqA, (size_t)p->n[1] * p->n[2] * 8)) != SF_OK) return bail(st, "");   // Nyquist column [z][y]
         p->fastper = true;
+        p->fastper_x = (p->n[0] == 256) && !getenv("SF_DISABLE_FAST_X");
     }
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "plan construction failed on the device");
     *out = p;

@@ -59,6 +59,8 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_FWD>::kSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_INV>::kSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_FUSED>::kSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_xper_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXpSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_xper_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXpSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
@@ -156,6 +158,16 @@ cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st)
     case FMODE_FUSED: fast_per_kernel<FMODE_FUSED><<<grid, kThreads, kPerSmem, st>>>(p); break;
     default: return cudaErrorInvalidValue;
     }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st)
+{
+    if (p.nrows <= 0 || p.nrows % kXpRows || !p.nyq) return cudaErrorInvalidValue;
+    int grid = 2 * g_sms;
+    if (grid > p.nrows / kXpRows) grid = p.nrows / kXpRows;
+    if (inv) fast_xper_kernel<true><<<grid, kXpThreads, kXpSmem, st>>>(p);
+    else fast_xper_kernel<false><<<grid, kXpThreads, kXpSmem, st>>>(p);
     return cudaGetLastError();
 }
 

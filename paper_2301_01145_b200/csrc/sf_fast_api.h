@@ -72,6 +72,16 @@ struct FastPerParams {
     int zero_mode;
 };
 
+// S1 / S5 of periodic plans for rows of 256 reals (fast_xper_kernel)
+struct FastXPerParams {
+    const float* real_in;   // S1: [rows][256]
+    float* real_out;        // S5: [rows][256]
+    C* spec;                // half spectra X[0..127], row pitch spec_pitch complex
+    long long spec_pitch;
+    int nrows;              // multiple of 32
+    C* nyq;                 // side array [row] of X[128]
+};
+
 // opaque storage of a CUtensorMap (TMA descriptor): 128 bytes, 64-byte aligned
 struct alignas(64) TileMap { unsigned char bytes[128]; };
 
@@ -97,5 +107,6 @@ cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map
 cudaError_t launch_fast_x(bool inv, const FastXParams& p, cudaStream_t st);
 // launch one periodic strided pass (mode = FMODE_*) as a persistent grid of two CTAs per SM
 cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st);
+cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st);
 
 } // namespace sf2

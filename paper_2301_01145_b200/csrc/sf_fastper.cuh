@@ -197,3 +197,129 @@ __global__ void __launch_bounds__(kThreads, 2) fast_per_kernel(const FastPerPara
 }
 
 } // namespace sf2
+
+namespace sf2 {
+
+// ==================================================================================== X passes, periodic
+// S1 (real-to-complex) and S5 (complex-to-real) for rows of 256 reals (PAPER.md:87 half spectrum).
+// A row is packed as z[n] = x[2n] + i x[2n+1], n < 128; Z = DFT128(z) by the 128-point transform of
+// the padded X kernels (radix-16 over r, n = w + 8 r; twiddle; one exchange; two radix-8), then
+//     X[k] = ( (Z[k] + conj Z[128-k]) - i w256^k (Z[k] - conj Z[128-k]) ) / 2,   k = 0..128.
+// CTA of 256 threads = 8 warps (w) x 32 lanes, lane = row: a tile is 32 rows, staged in shared
+// memory with odd 8-byte pitches (lanes on distinct banks) and moved to and from global memory as
+// whole contiguous rows.  X[0..127] go to the spectrum array, X[128] to the side array [row].
+constexpr int kXpThreads = 256;
+constexpr int kXpRows = 32;
+constexpr int kXpRealPitch = 258;   // floats: 1032 B = 8 (mod 128)
+constexpr int kXpSpecPitch = 129;   // complex: 1032 B
+constexpr size_t kXpSmem = (size_t)kXpRows * kXpRealPitch * sizeof(float) + (size_t)16 * 8 * 32 * sizeof(C) + (size_t)kXpRows * kXpSpecPitch * sizeof(C);
+
+template <bool INV> __global__ void __launch_bounds__(kXpThreads, 2) fast_xper_kernel(const FastXPerParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* rbuf = reinterpret_cast<float*>(smem_raw);
+    C* xbuf = reinterpret_cast<C*>(smem_raw + (size_t)kXpRows * kXpRealPitch * sizeof(float));
+    C* sbuf = xbuf + 16 * 8 * 32;
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int w = (int)__reduce_max_sync(0xffffffffu, (unsigned)(tid >> 5));
+    __shared__ __align__(16) C s_t128[128];     // w128^(q w), row w
+    if (tid < 64) reinterpret_cast<float4*>(s_t128)[tid] = reinterpret_cast<const float4*>(g_tab_x)[tid];
+    const C* t128 = s_t128 + w * 16;
+    C* xw = xbuf + w * 32 + lane;
+    const C* xr = xbuf + w * 8 * 32 + lane;
+    C* srow = sbuf + lane * kXpSpecPitch;
+    float* rrow = rbuf + lane * kXpRealPitch;
+    __syncthreads();
+
+    const int ntiles = p.nrows / kXpRows;
+    for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const long long row0 = (long long)t * kXpRows;
+        if constexpr (!INV) {
+            // rows in, as 8-byte pieces (coalesced)
+            const float2* gin = reinterpret_cast<const float2*>(p.real_in + row0 * 256);
+#pragma unroll 4
+            for (int j = 0; j < 16; ++j) {
+                const int idx = tid + kXpThreads * j, r = idx >> 7, n = idx & 127;
+                *reinterpret_cast<float2*>(rbuf + r * kXpRealPitch + 2 * n) = __ldg(gin + idx);
+            }
+            __syncthreads();
+            C v[16];
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = *reinterpret_cast<const C*>(rrow + 2 * (w + 8 * r));
+            fft128_a<false>(v, t128, xw);
+            __syncthreads();
+            C a[8], b[8];
+            fft128_b<false>(a, b, xr);
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) {
+                srow[w + 16 * k2] = a[brev3(k2)];
+                srow[w + 8 + 16 * k2] = b[brev3(k2)];
+            }
+            __syncthreads();
+            // split in place: thread w owns the pairs (k, 128 - k), k = w + 8 m, m < 8 (and k = 64 for w = 0)
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const int k = (m < 8) ? w + 8 * m : 64;
+                if (m == 8 && w != 0) break;
+                const C zk = srow[k], zm = srow[(128 - k) & 127];
+                const C e = make_float2(zk.x + zm.x, zk.y - zm.y);
+                const C d = make_float2(zk.x - zm.x, zk.y + zm.y);
+                const C wd = cmul(d, c_tw1024[4 * k]);   // w256^k d
+                srow[k] = make_float2(0.5f * (e.x + wd.y), 0.5f * (e.y - wd.x));
+                if (k != 64) srow[128 - k] = make_float2(0.5f * (e.x - wd.y), 0.5f * (-e.y - wd.x));
+            }
+            __syncthreads();
+#pragma unroll 4
+            for (int j = 0; j < 16; ++j) {
+                const int idx = tid + kXpThreads * j, r = idx >> 7, k = idx & 127;
+                p.spec[(row0 + r) * p.spec_pitch + k] = sbuf[r * kXpSpecPitch + k];
+            }
+            if (tid < kXpRows) p.nyq[row0 + tid] = sbuf[tid * kXpSpecPitch + 128];
+            // (the next tile writes rbuf and the exchange buffer first; its barriers order the reuse of sbuf)
+        } else {
+#pragma unroll 4
+            for (int j = 0; j < 16; ++j) {
+                const int idx = tid + kXpThreads * j, r = idx >> 7, k = idx & 127;
+                sbuf[r * kXpSpecPitch + k] = __ldg(p.spec + (row0 + r) * p.spec_pitch + k);
+            }
+            if (tid < kXpRows) sbuf[tid * kXpSpecPitch + 128] = __ldg(p.nyq + row0 + tid);
+            __syncthreads();
+            // merge in place: Z[k] = e + i conj(w256^k) d,  Z[128 - k] = conj e + i conj(conj(w256^k) d)
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const int k = (m < 8) ? w + 8 * m : 64;
+                if (m == 8 && w != 0) break;
+                const C xk = srow[k], xm = srow[128 - k];
+                const C e = make_float2(xk.x + xm.x, xk.y - xm.y);
+                const C d = make_float2(xk.x - xm.x, xk.y + xm.y);
+                const C wd = cmulc(d, c_tw1024[4 * k]);
+                srow[k] = make_float2(e.x - wd.y, e.y + wd.x);
+                if (k != 0 && k != 64) srow[128 - k] = make_float2(e.x + wd.y, -e.y + wd.x);
+            }
+            __syncthreads();
+            C v[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = srow[w + 8 * j];
+            fft128_a<true>(v, t128, xw);
+            __syncthreads();
+            C a[8], b[8];
+            fft128_b<true>(a, b, xr);
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) {
+                *reinterpret_cast<C*>(rrow + 2 * (w + 16 * k2)) = a[brev3(k2)];
+                *reinterpret_cast<C*>(rrow + 2 * (w + 8 + 16 * k2)) = b[brev3(k2)];
+            }
+            __syncthreads();
+            float2* gout = reinterpret_cast<float2*>(p.real_out + row0 * 256);
+#pragma unroll 4
+            for (int j = 0; j < 16; ++j) {
+                const int idx = tid + kXpThreads * j, r = idx >> 7, n = idx & 127;
+                gout[idx] = *reinterpret_cast<const float2*>(rbuf + r * kXpRealPitch + 2 * n);
+            }
+            // (the next tile's first barrier follows its writes to sbuf only; rbuf is rewritten after two more)
+        }
+    }
+}
+
+} // namespace sf2
