@@ -214,6 +214,14 @@ constexpr int kXpRealPitch = 258;   // floats: 1032 B = 8 (mod 128)
 constexpr int kXpSpecPitch = 129;   // complex: 1032 B
 constexpr size_t kXpSmem = (size_t)kXpRows * kXpRealPitch * sizeof(float) + (size_t)16 * 8 * 32 * sizeof(C) + (size_t)kXpRows * kXpSpecPitch * sizeof(C);
 
+// 8-byte asynchronous copy global -> shared (LDGSTS), completion by cp.async groups
+__device__ __forceinline__ void cp_async8(void* dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 template <bool INV> __global__ void __launch_bounds__(kXpThreads, 2) fast_xper_kernel(const FastXPerParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -233,22 +241,40 @@ template <bool INV> __global__ void __launch_bounds__(kXpThreads, 2) fast_xper_k
     __syncthreads();
 
     const int ntiles = p.nrows / kXpRows;
-    for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    // the rows of tile t arrive by asynchronous 8-byte copies (coalesced), issued one tile ahead as soon as
+    // the staging buffer of the current tile has been read by every thread
+    auto fetch = [&](int t) {
+        if (t >= ntiles) return;
         const long long row0 = (long long)t * kXpRows;
         if constexpr (!INV) {
-            // rows in, as 8-byte pieces (coalesced)
             const float2* gin = reinterpret_cast<const float2*>(p.real_in + row0 * 256);
 #pragma unroll 4
             for (int j = 0; j < 16; ++j) {
                 const int idx = tid + kXpThreads * j, r = idx >> 7, n = idx & 127;
-                *reinterpret_cast<float2*>(rbuf + r * kXpRealPitch + 2 * n) = __ldg(gin + idx);
+                cp_async8(rbuf + r * kXpRealPitch + 2 * n, gin + idx);
             }
-            __syncthreads();
+        } else {
+#pragma unroll 4
+            for (int j = 0; j < 16; ++j) {
+                const int idx = tid + kXpThreads * j, r = idx >> 7, k = idx & 127;
+                cp_async8(sbuf + r * kXpSpecPitch + k, p.spec + (row0 + r) * p.spec_pitch + k);
+            }
+            if (tid < kXpRows) cp_async8(sbuf + tid * kXpSpecPitch + 128, p.nyq + row0 + tid);
+        }
+        cp_async_commit();
+    };
+    fetch(blockIdx.x);
+    for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const long long row0 = (long long)t * kXpRows;
+        cp_async_wait_all();
+        __syncthreads();
+        if constexpr (!INV) {
             C v[16];
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = *reinterpret_cast<const C*>(rrow + 2 * (w + 8 * r));
             fft128_a<false>(v, t128, xw);
             __syncthreads();
+            fetch(t + gridDim.x);   // rbuf is in registers everywhere
             C a[8], b[8];
             fft128_b<false>(a, b, xr);
 #pragma unroll
@@ -276,15 +302,8 @@ template <bool INV> __global__ void __launch_bounds__(kXpThreads, 2) fast_xper_k
                 p.spec[(row0 + r) * p.spec_pitch + k] = sbuf[r * kXpSpecPitch + k];
             }
             if (tid < kXpRows) p.nyq[row0 + tid] = sbuf[tid * kXpSpecPitch + 128];
-            // (the next tile writes rbuf and the exchange buffer first; its barriers order the reuse of sbuf)
+            // (sbuf is rewritten after the next tile's second barrier)
         } else {
-#pragma unroll 4
-            for (int j = 0; j < 16; ++j) {
-                const int idx = tid + kXpThreads * j, r = idx >> 7, k = idx & 127;
-                sbuf[r * kXpSpecPitch + k] = __ldg(p.spec + (row0 + r) * p.spec_pitch + k);
-            }
-            if (tid < kXpRows) sbuf[tid * kXpSpecPitch + 128] = __ldg(p.nyq + row0 + tid);
-            __syncthreads();
             // merge in place: Z[k] = e + i conj(w256^k) d,  Z[128 - k] = conj e + i conj(conj(w256^k) d)
 #pragma unroll
             for (int m = 0; m < 9; ++m) {
@@ -303,6 +322,7 @@ template <bool INV> __global__ void __launch_bounds__(kXpThreads, 2) fast_xper_k
             for (int j = 0; j < 16; ++j) v[j] = srow[w + 8 * j];
             fft128_a<true>(v, t128, xw);
             __syncthreads();
+            fetch(t + gridDim.x);   // sbuf is in registers everywhere
             C a[8], b[8];
             fft128_b<true>(a, b, xr);
 #pragma unroll
@@ -317,7 +337,7 @@ template <bool INV> __global__ void __launch_bounds__(kXpThreads, 2) fast_xper_k
                 const int idx = tid + kXpThreads * j, r = idx >> 7, n = idx & 127;
                 gout[idx] = *reinterpret_cast<const float2*>(rbuf + r * kXpRealPitch + 2 * n);
             }
-            // (the next tile's first barrier follows its writes to sbuf only; rbuf is rewritten after two more)
+            // (rbuf is rewritten after the next tile's third barrier)
         }
     }
 }
