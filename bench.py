@@ -93,7 +93,7 @@ def step_names(wname):
     """the kernel behind each of the five steps for this workload"""
     if wname == "cfg4_unbounded_256_f32":
         return STEP_NAMES
-    if wname == "cfg2_periodic_256_f32":
+    if wname in ("cfg2_periodic_256_f32", "cfg2_periodic_256_f32_grad"):
         return ["S1 fast_xper_kernel<fwd>", "S2 fast_per_kernel<FWD>", "S3 fast_per_kernel<FUSED>", "S4 fast_per_kernel<INV>",
                 "S5 fast_xper_kernel<inv>"]
     return ["S1 xfwd_kernel", "S2 spass_kernel<0>", "S3 spass_kernel<2>", "S4 spass_kernel<1>", "S5 xinv_kernel"]

@@ -503,14 +503,14 @@ template <typename T> sf_status run(sf_plan p, int outk)
         fx.spec = (sf2::C*)p->W1; fx.spec_pitch = hp; fx.nrows = n1 * n2;
         fx.nyq = (sf2::C*)p->nyqA; fx.n1 = n1; fx.n2 = n2;
         SF_CUDA(p, sf2::launch_fast_x(false, fx, st));
-    } else if (p->fastper && p->fastper_x && outk == OUT_SOLVE && !xp.has_faces) {
+    } else if (p->fastper && p->fastper_x && (outk == OUT_SOLVE || outk == OUT_GRAD) && !xp.has_faces) {
         sf2::FastXPerParams px;
         memset(&px, 0, sizeof(px));
         px.real_in = (const float*)p->src; px.spec = (sf2::C*)p->W1; px.spec_pitch = hp; px.nrows = n1 * n2;
         px.nyq = (sf2::C*)p->nyqA;
         SF_CUDA(p, sf2::launch_fast_xper(false, px, st));
     } else {
-        if (p->fastper && outk == OUT_SOLVE) xp.nyq_side = p->nyqA;
+        if (p->fastper && (outk == OUT_SOLVE || outk == OUT_GRAD)) xp.nyq_side = p->nyqA;
         SF_CUDA(p, launch_xfwd<T>(p->Lx, xp, ncomp, st));
         xp.nyq_side = nullptr;
     }
@@ -574,7 +574,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         return SF_OK;
     }
 
-    if (p->fastper && outk == OUT_SOLVE) {
+    if (p->fastper && (outk == OUT_SOLVE || outk == OUT_GRAD)) {
         // kernel generation 2, periodic: S2, S3, S4 in place on W1 as persistent register-FFT kernels
         sf2::FastPerParams fp;
         memset(&fp, 0, sizeof(fp));
@@ -595,11 +595,17 @@ template <typename T> sf_status run(sf_plan p, int outk)
         fp.nyq_ps = n1; fp.nyq_bs = 1;
         fp.lam_x = (const float*)p->lam[0]; fp.lam_b = (const float*)p->lam[1]; fp.lam_p = (const float*)p->lam[2];
         fp.scale = (float)p->scale; fp.zero_mode = 1;
+        if (outk == OUT_GRAD) {
+            fp.grad = 1;
+            fp.kap_x = (const float*)p->kap[0]; fp.kap_b = (const float*)p->kap[1]; fp.kap_p = (const float*)p->kap[2];
+            fp.out_cs = p->w1_field; fp.nyq_cs = (long long)n1 * n2;
+        }
         SF_CUDA(p, sf2::launch_fast_per(sf2::FMODE_FUSED, fp, st));
+        fp.grad = 0;
         p->launches++;
         mark(3);
-        // S4 along y
-        fp.in_ps = fp.out_ps = hp; fp.in_bs = fp.out_bs = hp * n1; fp.nb = n2;
+        // S4 along y; the fields are contiguous, so the output fields are just more batches
+        fp.in_ps = fp.out_ps = hp; fp.in_bs = fp.out_bs = hp * n1; fp.nb = n2 * nf_out;
         fp.nyq_ps = 1; fp.nyq_bs = n1;
         SF_CUDA(p, sf2::launch_fast_per(sf2::FMODE_INV, fp, st));
         p->launches++;
@@ -609,7 +615,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         if (p->fastper_x) {
             sf2::FastXPerParams px;
             memset(&px, 0, sizeof(px));
-            px.real_out = (float*)p->out; px.spec = (sf2::C*)p->W1; px.spec_pitch = hp; px.nrows = n1 * n2;
+            px.real_out = (float*)p->out; px.spec = (sf2::C*)p->W1; px.spec_pitch = hp; px.nrows = n1 * n2 * nf_out;
             px.nyq = (sf2::C*)p->nyqA;
             SF_CUDA(p, sf2::launch_fast_xper(true, px, st));
         } else {
@@ -889,7 +895,7 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fp32 fast path failed"); }
         if ((st = dev_alloc(p, &p->sched, 2 * sizeof(int))) != SF_OK) return bail(st, "");
         if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
-        if ((st = dev_alloc(p, &p->nyqA, (size_t)p->n[1] * p->n[2] * 8)) != SF_OK) return bail(st, "");   // Nyquist column [z][y]
+        if ((st = dev_alloc(p, &p->nyqA, (size_t)p->nfields * p->n[1] * p->n[2] * 8)) != SF_OK) return bail(st, "");   // Nyquist column [field][z][y]
         p->fastper = true;
         p->fastper_x = (p->n[0] == 256) && !getenv("SF_DISABLE_FAST_X");
     }

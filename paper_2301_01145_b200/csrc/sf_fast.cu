@@ -64,6 +64,7 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FUSED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     void* fn = nullptr;
@@ -149,13 +150,22 @@ cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st)
     if (p.nct <= 0 || p.nb <= 0) return cudaErrorInvalidValue;
     if ((long long)p.nb * p.in_bs + 256 * p.in_ps >= (1ll << 31) || (long long)p.nb * p.out_bs + 256 * p.out_ps >= (1ll << 31))
         return cudaErrorInvalidValue;
+    if (p.grad && ((long long)p.nb * p.out_bs + 256 * p.out_ps + 3 * p.out_cs >= (1ll << 31) || mode != FMODE_FUSED)) return cudaErrorInvalidValue;
     const int ntiles = p.nb * p.nct + (p.nyq_col >= 0 ? (p.nb + kPerTile - 1) / kPerTile : 0);
     int grid = 2 * g_sms;
     if (grid > ntiles) grid = ntiles;
     switch (mode) {
     case FMODE_FWD: fast_per_kernel<FMODE_FWD><<<grid, kThreads, kPerSmem, st>>>(p); break;
     case FMODE_INV: fast_per_kernel<FMODE_INV><<<grid, kThreads, kPerSmem, st>>>(p); break;
-    case FMODE_FUSED: fast_per_kernel<FMODE_FUSED><<<grid, kThreads, kPerSmem, st>>>(p); break;
+    case FMODE_FUSED:
+        if (p.grad) {
+            // one CTA per SM (96 registers per thread)
+            if (grid > g_sms) grid = g_sms;
+            fast_per_kernel<FMODE_FUSED, true><<<grid, kThreads, kPerSmem, st>>>(p);
+        } else {
+            fast_per_kernel<FMODE_FUSED><<<grid, kThreads, kPerSmem, st>>>(p);
+        }
+        break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

@@ -70,6 +70,10 @@ struct FastPerParams {
     const float* lam_x; const float* lam_b; const float* lam_p;
     float scale;
     int zero_mode;
+    // gradient (fused mode): fields 1 .. 3 = d/dx, d/dy (batch axis), d/dz (pencil axis) of the result
+    int grad;
+    const float* kap_x; const float* kap_b; const float* kap_p;   // wavenumbers, zero at the Nyquist index
+    long long out_cs, nyq_cs;                                     // field strides of out and of the side array
 };
 
 // S1 / S5 of periodic plans for rows of 256 reals (fast_xper_kernel)

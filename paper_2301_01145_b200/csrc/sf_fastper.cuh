@@ -42,8 +42,23 @@ __device__ __forceinline__ PerGeom per_geom(const FastPerParams& p, int t)
     return g;
 }
 
-template <int MODE>
-__global__ void __launch_bounds__(kThreads, 2) fast_per_kernel(const FastPerParams p)
+// backward transform of u (natural order in) and store of rows o + 16 j to q (row stride ors)
+template <bool OB> __device__ __forceinline__ void per_inverse_store(C (&u)[16], const C* t256, int o, const Xchg& xc, C* q, int ors, bool valid)
+{
+    fft256_a<true, OB, true>(u, t256, o, xc);
+    __syncthreads();
+    fft256_b<true, OB>(u, xc);
+    if (valid) {
+#pragma unroll
+        for (int j2 = 0; j2 < 16; ++j2) q[j2 * 16 * ors] = u[brev4(j2)];
+    }
+}
+
+// GRAD (fused mode only): besides psi, the three derivative spectra i kappa_a psi_hat (eq. (10))
+// are transformed back from the same registers into fields 1..3 -- five transforms per tile, 32 more live
+// registers, hence one CTA per SM
+template <int MODE, bool GRAD = false>
+__global__ void __launch_bounds__(kThreads, GRAD ? 1 : 2) fast_per_kernel(const FastPerParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     C* xbuf = reinterpret_cast<C*>(smem_raw);
@@ -57,9 +72,11 @@ __global__ void __launch_bounds__(kThreads, 2) fast_per_kernel(const FastPerPara
 
     __shared__ __align__(16) C s_t256[256];      // w256^(q o), row o
     __shared__ float s_lamp[256];                // fused: eigenvalue contribution of the pencil axis
+    __shared__ float s_kapp[GRAD ? 256 : 1];     // gradient: wavenumber along the pencil axis
     __shared__ int s_tile[2];
     if (tid < 128) reinterpret_cast<float4*>(s_t256)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid];
     if (MODE == FMODE_FUSED && tid < 256) s_lamp[tid] = __ldg(p.lam_p + tid);
+    if (GRAD && tid < 256) s_kapp[tid] = __ldg(p.kap_p + tid);
     const C* t256 = s_t256 + o * 16;
     if (tid == 0) {
         s_tile[0] = atomicAdd(p.sched, 1);
@@ -159,18 +176,29 @@ __global__ void __launch_bounds__(kThreads, 2) fast_per_kernel(const FastPerPara
                 if (k2 == 0 && zero0) m = 0.f;
                 w[k2] = cscale(v[brev4(k2)], m);
             }
-            fft256_a<true, !OB, true>(w, t256, o, xc);
-            __syncthreads();
-            fft256_b<true, !OB>(w, xc);
-            if (valid) {
+            if constexpr (GRAD) {
+                const float qx = __ldg(p.kap_x + kx), qy = __ldg(p.kap_b + kb);
+                const int ocs = g.full ? (int)p.out_cs : (int)p.nyq_cs;   // field stride
                 C* q = obase + o * ors;
+                C u[16];
 #pragma unroll
-                for (int j2 = 0; j2 < 16; ++j2) q[j2 * 16 * ors] = w[brev4(j2)];
+                for (int k2 = 0; k2 < 16; ++k2) u[k2] = cmuli(cscale(w[k2], s_kapp[o + 16 * k2]));
+                per_inverse_store<!OB>(u, t256, o, xc, q + 3 * ocs, ors, valid);
+#pragma unroll
+                for (int k2 = 0; k2 < 16; ++k2) u[k2] = cmuli(cscale(w[k2], qy));
+                per_inverse_store<OB>(u, t256, o, xc, q + 2 * ocs, ors, valid);
+#pragma unroll
+                for (int k2 = 0; k2 < 16; ++k2) u[k2] = cmuli(cscale(w[k2], qx));
+                per_inverse_store<!OB>(u, t256, o, xc, q + ocs, ors, valid);
+                per_inverse_store<OB>(w, t256, o, xc, q, ors, valid);
+            } else {
+                per_inverse_store<!OB>(w, t256, o, xc, obase + o * ors, ors, valid);
             }
         }
     };
 
-    if constexpr (MODE == FMODE_FUSED) {
+    if constexpr (MODE == FMODE_FUSED && !GRAD) {
+        // two transforms per tile: the orientation is back where it started
         for (int it = 0;; ++it) {
             const int t = s_tile[it & 1];
             if (t >= ntiles) break;

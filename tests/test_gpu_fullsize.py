@@ -362,8 +362,11 @@ def test_periodic_fast_path_white_noise(nx, op, monkeypatch):
             got[name] = p.get(sf.SF_OUT_PSI)
             _check(f"periodic 256x256x{nx} {op} {name}", got[name], ref, "f32")
             if not disable:
-                sf.sf_gradient(p.plan)     # generation-1 kernels on the same plan
+                sf.sf_gradient(p.plan)     # generation 2 as well: four fields out of the fused pass
                 _check("psi (gradient call)", p.get(sf.SF_OUT_PSI), ref, "f32")
+                _, grad_o = O.periodic(f.astype(np.float64), L, oop, rhs_sign=-1.0, want_grad=True)
+                for a in range(3):
+                    _check(f"grad[{a}]", p.get(sf.SF_OUT_GRAD, a), grad_o[a], "f32")
                 sf.sf_solve(p.plan)
                 _check("psi (solve again)", p.get(sf.SF_OUT_PSI), ref, "f32")
     err = np.linalg.norm((got["generation 2"].astype(np.float64) - ref).reshape(256, -1), axis=1)
