@@ -511,8 +511,9 @@ template <typename T> sf_status run(sf_plan p, int outk)
         SF_CUDA(p, sf2::launch_fast_xper(false, px, st));
     } else {
         if (p->fastper && (outk == OUT_SOLVE || outk == OUT_GRAD)) xp.nyq_side = p->nyqA;
+        if (p->fast && outk == OUT_SOLVE && p->nyqA) { xp.nyq_side = p->nyqA; xp.nyq_side_yz = 1; }   // [y][z], as fast_x_kernel writes it
         SF_CUDA(p, launch_xfwd<T>(p->Lx, xp, ncomp, st));
-        xp.nyq_side = nullptr;
+        xp.nyq_side = nullptr; xp.nyq_side_yz = 0;
     }
     p->launches++;
     mark(1);
@@ -536,8 +537,9 @@ template <typename T> sf_status run(sf_plan p, int outk)
         // S2: W1 [z][y][hp] -> W2 [z][ky][hp]
         fp.in = (const sf2::C*)p->W1; fp.out = (sf2::C*)p->W2;
         fp.in_ps = hp; fp.in_bs = hp * n1; fp.out_ps = hp; fp.out_bs = hp * P1; fp.nb = n2;
-        if (fast_x) { fp.nyq_in = (const sf2::C*)p->nyqA; fp.nyq_out = (sf2::C*)p->nyqB; }
-        fp.nyq_first = fast_x ? 1 : 0;
+        const bool side = p->nyqA != nullptr;   // Nyquist column in the side arrays (written by either X kernel)
+        if (side) { fp.nyq_in = (const sf2::C*)p->nyqA; fp.nyq_out = (sf2::C*)p->nyqB; }
+        fp.nyq_first = side ? 1 : 0;
         fp.reverse_batches = 1;   // S1 wrote plane z last: start there while it is in L2
         SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_FWD, fp, p->map_s2, st));
         fp.reverse_batches = 0;
@@ -546,7 +548,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         // S3: W2 in place along z
         fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W2;
         fp.in_ps = fp.out_ps = hp * P1; fp.in_bs = fp.out_bs = hp; fp.nb = P1;
-        if (fast_x) { fp.nyq_in = (const sf2::C*)p->nyqB; fp.nyq_out = (sf2::C*)p->nyqB; }
+        if (side) { fp.nyq_in = (const sf2::C*)p->nyqB; fp.nyq_out = (sf2::C*)p->nyqB; }
         fp.pair_batches = 1;
         fp.nyq_first = 1;
         fp.green_tiles = (const float*)p->green_tiles; fp.Pb = P1;
@@ -554,9 +556,9 @@ template <typename T> sf_status run(sf_plan p, int outk)
         p->launches++;
         mark(3);
         // S4: W2 [z][ky][hp] -> W1 [z][y][hp]
-        if (fast_x) { fp.nyq_in = (const sf2::C*)p->nyqB; fp.nyq_out = (sf2::C*)p->nyqA; }
+        if (side) { fp.nyq_in = (const sf2::C*)p->nyqB; fp.nyq_out = (sf2::C*)p->nyqA; }
         fp.pair_batches = 0;
-        fp.nyq_first = fast_x ? 1 : 0;
+        fp.nyq_first = side ? 1 : 0;
         fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W1;
         fp.in_ps = hp; fp.in_bs = hp * P1; fp.out_ps = hp; fp.out_bs = hp * n1; fp.nb = n2;
         SF_CUDA(p, sf2::launch_fast_pad(sf2::FMODE_INV, fp, p->map_s4, st));
@@ -564,8 +566,13 @@ template <typename T> sf_status run(sf_plan p, int outk)
         mark(4);
         xp.spec_in = p->W1; xp.real_out = (T*)p->out;
         fx.reverse = 1;           // S4 wrote the last planes last
-        if (fast_x) SF_CUDA(p, sf2::launch_fast_x(true, fx, st));
-        else SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        if (fast_x) {
+            SF_CUDA(p, sf2::launch_fast_x(true, fx, st));
+        } else {
+            if (side) { xp.nyq_side = p->nyqA; xp.nyq_side_yz = 1; }
+            SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+            xp.nyq_side = nullptr; xp.nyq_side_yz = 0;
+        }
         p->launches++;
         mark(5);
         if (timed) p->tcount++;
@@ -884,7 +891,7 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
         p->fast = true;
         p->fast_x = (p->n[0] == 256) && p->pitch >= 258 && !getenv("SF_DISABLE_FAST_X");
-        if (p->fast_x) {
+        if (p->nspec_x % sf2::kTile) {   // the Nyquist column lives in two side arrays ([y][z] and [z][ky])
             if ((st = dev_alloc(p, &p->nyqA, (size_t)256 * 256 * 8)) != SF_OK) return bail(st, "");
             if ((st = dev_alloc(p, &p->nyqB, (size_t)256 * 512 * 8)) != SF_OK) return bail(st, "");
         }

@@ -43,6 +43,7 @@ template <typename T> struct XParams {
     // periodic / zero-padded: optional side array [field][row] that holds the last column (k = L, the Nyquist
     // coefficient) of every row instead of the spectrum array (sf_fastper.cuh)
     void* nyq_side;
+    int nyq_side_yz;    // 0: [field][row = iz * ny + iy];  1: transposed, [iy][iz] (single field)
     // backward, real modes: spectral derivative along x of one field (sine <-> cosine series, eq. (10))
     int dfield1;        // 1 + index of the field (blockIdx.y) that is differentiated; 0: none
     const T* kap_ext;   // pi k / L_domain for slot k <= L of the extended sequence, zero at k = L
@@ -174,7 +175,7 @@ __global__ void __launch_bounds__(NT) xfwd_kernel(const XParams<T> p)
             const long long row = row0 + r;
             if (row < nrows) {
                 const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-                if (k == L && p.nyq_side) reinterpret_cast<C*>(p.nyq_side)[comp * nrows + row] = G[r * LP + k];
+                if (k == L && p.nyq_side) reinterpret_cast<C*>(p.nyq_side)[p.nyq_side_yz ? (long long)iy * p.nz + iz : comp * nrows + row] = G[r * LP + k];
                 else so[iy * p.sp_py + iz * p.sp_pz + k] = G[r * LP + k];
             }
         }
@@ -232,7 +233,7 @@ __global__ void __launch_bounds__(NT) xinv_kernel(const XParams<T> p)
             C x = mk<T>(0, 0);
             if (row < nrows) {
                 const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-                if (k == L && p.nyq_side) x = reinterpret_cast<const C*>(p.nyq_side)[comp * nrows + row];
+                if (k == L && p.nyq_side) x = reinterpret_cast<const C*>(p.nyq_side)[p.nyq_side_yz ? (long long)iy * p.nz + iz : comp * nrows + row];
                 else x = si[iy * p.sp_py + iz * p.sp_pz + k];
             }
             A[r * LP + k] = x;
