@@ -11,6 +11,11 @@ example (its results are figures), so the closed forms below are the values "the
                      phi(r) = -q erf(r / (sqrt(2) s)) / (4 pi r), s^2 = sigma^2 + eps^2  (pin P5)
   fd2_dirichlet.txt  amplification A = pi^2 sum m_a^2 / ((4/h^2) sum sin^2(m_a pi h / 2)) of the product
                      of sines under the 7-point stencil (Table 1 row 1; pin P3)
+  green_orders.txt   the regularised kernels at the origin and far away, where closed forms need no special
+                     function: 3-D G_P(0) = -(1, 3/2, 15/8, 35/16, 315/128) / ((2 pi)^(3/2) eps) for P = 2 .. 10,
+                     spectrally compact G(0) = -1 / (2 pi h); 2-D G_P(0) = (ln(2 eps^2) - gamma) / (4 pi)
+                     - (1 / 4 pi) sum_{n < P/2} 1/n; far field -1 / (4 pi r) and ln(r) / (2 pi)
+                     (readings A25, A26, A28)
   periodic_mode.txt  phi = -(a cos th + b sin th) / (4 pi^2 (p^2 + q^2)) for one Fourier mode (eq. 5,
                      PAPER.md:50; pin P2) at a few cell-centre points of the 64^2 grid of cfg 1
 """
@@ -44,6 +49,18 @@ def main():
             lam = sum(-(4 / h ** 2) * math.sin(mm * math.pi * h / 2) ** 2 for mm in m)
             A = -(math.pi ** 2) * sum(mm * mm for mm in m) / lam
             f.write(f"{nc} {m[0]} {m[1]} {m[2]} {A!r}\n")
+    with open(HERE / "green_orders.txt", "w") as f:
+        f.write("# dim order r eps G   -- order 0 = spectrally compact kernel (eps = h); PAPER.md:189, DESIGN.md A25 / A26 / A28\n")
+        gamma = 0.5772156649015329
+        c3 = {2: 1.0, 4: 1.5, 6: 15.0 / 8, 8: 35.0 / 16, 10: 315.0 / 128}
+        for eps in (0.0078125, 0.05):
+            for order in (2, 4, 6, 8, 10):
+                f.write(f"3 {order} 0.0 {eps!r} {-c3[order] / ((2 * math.pi) ** 1.5 * eps)!r}\n")
+                f.write(f"3 {order} {40 * eps!r} {eps!r} {-1.0 / (4 * math.pi * 40 * eps)!r}\n")
+                g0 = (math.log(2 * eps * eps) - gamma) / (4 * math.pi) - sum(1.0 / n for n in range(1, order // 2)) / (4 * math.pi)
+                f.write(f"2 {order} 0.0 {eps!r} {g0!r}\n")
+                f.write(f"2 {order} {40 * eps!r} {eps!r} {math.log(40 * eps) / (2 * math.pi)!r}\n")
+            f.write(f"3 0 0.0 {eps!r} {-1.0 / (2 * math.pi * eps)!r}\n")
     with open(HERE / "periodic_mode.txt", "w") as f:
         f.write("# n p q a b ix iy phi dphidx dphidy   -- f = a cos th + b sin th, th = 2 pi (p x + q y), x=(ix+.5)/n; PAPER.md:50, :141\n")
         n = 64

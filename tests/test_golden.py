@@ -18,6 +18,18 @@ def test_green_kernel_values():
         assert abs(O.green_gauss2(float(r), float(eps)) - float(g)) <= 2e-15 * abs(float(g))
 
 
+def test_green_kernel_orders_and_dimensions():
+    for dim, order, r, eps, g in _rows("green_orders.txt"):
+        dim, order, r, eps, g = int(dim), int(order), float(r), float(eps), float(g)
+        if dim == 3 and order == 0:
+            got = O.green_spectral(r, eps)
+        elif dim == 3:
+            got = O.green_gauss(order, r, eps)
+        else:
+            got = O.green2d_gauss(order, r, eps)
+        assert abs(got - g) <= 1e-13 * abs(g), (dim, order, r, eps, got, g)
+
+
 def test_gaussian_blob_potential():
     rows = _rows("gaussian_blob.txt")
     for sh, eh in sorted({(r[1], r[2]) for r in rows}):
