@@ -293,24 +293,15 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
 
     // twiddle tables: s_tw256[o][q] = w256^(q o);  s_tw512[h][o][r] = w512^(o + 16 r) for h = 1, 1 for h = 0
     __shared__ __align__(16) C s_tab[768];
-    if (tid < 384) reinterpret_cast<float4*>(s_tab)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid];
     const C* t256 = s_tab + o * 16;
     const C* t512 = s_tab + 256 + (h * 16 + o) * 16;
-    if (!Cfg::kTma) __syncthreads();
-
-    if (Cfg::kTma) {
-        if (tid == 0) {
-            mbar_init(&bar, 1);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        }
-        __syncthreads();
-    }
 
     const int ntiles = fast_ntiles(p.nb, p.nct, p.nyq_col);
     // element offsets fit 32 bits: an eligible plan's work arrays hold < 2^31 complex numbers (checked by the launcher)
     const int ips = (int)p.in_ps, ops = (int)p.out_ps, ibs = (int)p.in_bs, obs = (int)p.out_bs;
     uint32_t parity = 0;   // phase of `bar` the next full tile completes
-    // dynamic tile scheduling: p.sched[0] is the next unclaimed tile.  s_tile[it & 1] is the tile of
+    // dynamic tile scheduling: a CTA's first two tiles are blockIdx.x and blockIdx.x + gridDim.x (no atomic in
+    // the prologue), the rest come from p.sched[0] (+ 2 gridDim.x), the next unclaimed tile.  s_tile[it & 1] is the tile of
     // this CTA's iteration `it`; thread 0 claims the tile of iteration it + 2 once iteration it has
     // read its index (after its first barrier), so the index is always known one tile ahead for the
     // TMA prefetch and the atomic's latency is off the critical path.
@@ -353,7 +344,7 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
     auto advance = [&](int it) {
         if (tid != 0) return;
         issue(s_tile[(it + 1) & 1]);
-        s_tile[it & 1] = atomicAdd(p.sched, 1);
+        s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;
     };
 
     // one tile; ORIENT = orientation of the exchange buffer its first transform starts with
@@ -463,11 +454,17 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
         }
     };
 
+    // prologue: thread 0 arms the barrier and starts the first tile's TMA load while the others copy the tables
     if (tid == 0) {
-        s_tile[0] = atomicAdd(p.sched, 1);
-        s_tile[1] = atomicAdd(p.sched, 1);
+        if (Cfg::kTma) {
+            mbar_init(&bar, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        s_tile[0] = (int)blockIdx.x;
+        s_tile[1] = (int)(blockIdx.x + gridDim.x);
         issue(s_tile[0]);
     }
+    if (tid < 384) reinterpret_cast<float4*>(s_tab)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid];
     __syncthreads();
     if constexpr (MODE == FMODE_FUSED) {
         // two transforms per tile: the orientation is back where it started

@@ -78,9 +78,9 @@ __global__ void __launch_bounds__(kThreads, GRAD ? 1 : 2) fast_per_kernel(const 
     if (MODE == FMODE_FUSED && tid < 256) s_lamp[tid] = __ldg(p.lam_p + tid);
     if (GRAD && tid < 256) s_kapp[tid] = __ldg(p.kap_p + tid);
     const C* t256 = s_t256 + o * 16;
-    if (tid == 0) {
-        s_tile[0] = atomicAdd(p.sched, 1);
-        s_tile[1] = atomicAdd(p.sched, 1);
+    if (tid == 0) {   // the first two tiles are static, the rest come from the counter (+ 2 gridDim.x)
+        s_tile[0] = (int)blockIdx.x;
+        s_tile[1] = (int)(blockIdx.x + gridDim.x);
     }
     __syncthreads();
 
@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(kThreads, GRAD ? 1 : 2) fast_per_kernel(const 
         };
         // after the tile's first barrier every thread has read this tile's index: claim the tile after next
         // (the next tile's barrier publishes it)
-        auto claim = [&]() { if (tid == 0) s_tile[it & 1] = atomicAdd(p.sched, 1); };
+        auto claim = [&]() { if (tid == 0) s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x; };
         if constexpr (MODE == FMODE_FWD) {
             fft256_a<false, OB, false>(v, t256, o, xc);
             __syncthreads();
