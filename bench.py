@@ -99,6 +99,27 @@ def step_names(wname):
     return ["S1 xfwd_kernel", "S2 spass_kernel<0>", "S3 spass_kernel<2>", "S4 spass_kernel<1>", "S5 xinv_kernel"]
 
 
+# Issue cycles per warp-tile of the fused S3 kernel of the default workload, counted from the ncu source page of
+# capture d (profiles/r01_d.md): 476 packed fp32x2 instructions at two issue cycles each plus
+# 370 others; 8224 tiles x 16 warps per launch; 148 SMs x 4 schedulers issue one warp instruction per clock.
+S3_ISSUE_CYCLES_PER_WARP_TILE = 2 * 476 + 370
+S3_WARP_TILES = 8224 * 16
+ISSUE_SLOTS_PER_CLOCK = 148 * 4
+
+
+def issue_view(wname, dom, kernel_ms, clocks):
+    """The dominant kernel of the default workload is bound by instruction issue, not by HBM (profiles/r01_b.md):
+    besides the HBM roofline the line carries its issue-slot utilisation, from the static instruction count above
+    and the SM clock sampled during the timed region.  None for other workloads / kernels."""
+    if wname != DEFAULT_WORKLOAD or dom != 2 or not clocks or not clocks.get("sm_mhz"):
+        return None
+    cycles = S3_ISSUE_CYCLES_PER_WARP_TILE * S3_WARP_TILES
+    t_peak_ms = cycles / (ISSUE_SLOTS_PER_CLOCK * clocks["sm_mhz"] * 1e6) * 1e3
+    return {"bound": "alu", "kernel": STEP_NAMES[2], "issue_cycles_per_launch": cycles,
+            "ms_at_one_warp_instruction_per_scheduler_clock": t_peak_ms, "kernel_ms": kernel_ms, "frac": t_peak_ms / kernel_ms,
+            "source": "instruction counts of profiles/r01_d (ncu source page), SM clock of this run"}
+
+
 def make_input(w, rank=0):
     """Seeded synthetic source for the workload (workloads/: generators only, no method arithmetic)."""
     import workloads as W
@@ -450,6 +471,7 @@ def run_ours(args):
                          "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": mb[dom], "kernel_ms": step_ms[dom]},
             "steps_ms": {names[i]: step_ms[i] for i in range(5)},
+            "issue_view": issue_view(wname, dom, step_ms[dom], clocks),
             "steps_gbs": {names[i]: (mb[i] / (step_ms[i] * 1e-3) / 1e9 if step_ms[i] > 0 else None) for i in range(5)},
             "solve_roofline": {"algorithmic_bytes_per_step": sum(mb), "achieved_gbs": sum(mb) / (ms_per_step * 1e-3) / 1e9,
                                "frac_of_measured_peak": sum(mb) / (ms_per_step * 1e-3) / 1e9 / peak,
