@@ -838,7 +838,7 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
     // shared-memory feasibility of the fused kernel for this plan's worst case
     {
         const int ax = ndim - 1;
-        const int nbuf = (ncomp == 3) ? 3 : ((b == SF_BC_PERIODIC) ? 2 : 1);
+        const int nbuf = (ncomp == 3) ? 3 : 1;   // sf_gradient checks its own two tiles when it is called
         const size_t need = (prec == SF_F32) ? spass_smem_bytes<float>(p->La[ax], nbuf) : spass_smem_bytes<double>(p->La[ax], nbuf);
         if (need > 227 * 1024) return bail(SF_ERR_UNSUPPORTED, "fused pass does not fit in shared memory for this size / precision / field count");
     }
@@ -959,17 +959,18 @@ sf_status sf_gradient(sf_plan plan)
 {
     if (!plan) return SF_ERR_INVALID_ARG;
     if (plan->ncomp != 1) return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient is built for scalar plans");
+    {
+        // the fused pass holds two tiles (psi and one derivative)
+        const int ax = plan->ndim - 1;
+        const size_t need = (plan->prec == SF_F32) ? spass_smem_bytes<float>(plan->La[ax], 2) : spass_smem_bytes<double>(plan->La[ax], 2);
+        if (need > 227 * 1024 && !plan->fastper)
+            return fail(plan, SF_ERR_UNSUPPORTED, "gradient: the fused pass does not fit in shared memory for this size / precision");
+    }
     if (plan->bc == SF_BC_PERIODIC) return run_any(plan, OUT_GRAD);
     if (plan->ndim != 3 && plan->bc != SF_BC_UNBOUNDED)
         return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient on Dirichlet / Neumann plans is built for 3-D");
     // unbounded, Dirichlet, Neumann: psi and its derivatives need 1 + ndim fields of work space
     const int nf = 1 + plan->ndim;
-    {
-        // the fused pass holds two tiles (psi and the derivative along its axis)
-        const int ax = plan->ndim - 1;
-        const size_t need = (plan->prec == SF_F32) ? spass_smem_bytes<float>(plan->La[ax], 2) : spass_smem_bytes<double>(plan->La[ax], 2);
-        if (need > 227 * 1024) return fail(plan, SF_ERR_UNSUPPORTED, "gradient: the fused pass does not fit in shared memory for this size / precision");
-    }
     const size_t welem = (plan->r2r == R2R_NONE) ? 2 * plan->esize : plan->esize;
     if (!plan->gW1) {
         sf_status st;
