@@ -100,7 +100,11 @@ typedef struct {
  *          periodic, unbounded, Neumann cell-centre, Dirichlet cell-centre: n[a] a power of two >= 8 (x) /
  *          >= 4 (y, z); Dirichlet cell-boundary: n[a] = 2^k - 1 interior nodes (boundary nodes are not
  *          stored); Neumann cell-boundary: n[a] = 2^k + 1 nodes (boundary nodes are stored).
- *          Upper bound 4096 per axis (2048 for unbounded, whose transforms are 2 n[a] long).
+ *          Upper bounds (every pass is a complex transform of 4 .. 2048 points): periodic n[0] <= 4096,
+ *          n[1], n[2] <= 2048; unbounded n[0] <= 2048, n[1], n[2] <= 1024 (transforms are 2 n[a] long);
+ *          Dirichlet / Neumann: extended length / 2 <= 2048, i.e. n[a] <= 2047 / 2048 / 2048 / 2049 for the four
+ *          rows of Table 1.  The fused pass must also fit the shared memory of an SM (checked here for the
+ *          solve, by sf_gradient / sf_curl for their extra fields): UNSUPPORTED otherwise.
  *   h      [host] grid spacing per axis.  Domain length follows (Table 1): periodic
  *          and cell-centre L = n h; Dirichlet cell-boundary L = (n + 1) h; Neumann cell-boundary L = (n - 1) h.
  *   bc     [host] boundary condition per axis; all axes must agree.
