@@ -103,8 +103,9 @@ typedef struct {
  *          Upper bounds (every pass is a complex transform of 4 .. 2048 points): periodic n[0] <= 4096,
  *          n[1], n[2] <= 2048; unbounded n[0] <= 2048, n[1], n[2] <= 1024 (transforms are 2 n[a] long);
  *          Dirichlet / Neumann: extended length / 2 <= 2048, i.e. n[a] <= 2047 / 2048 / 2048 / 2049 for the four
- *          rows of Table 1.  The fused pass must also fit the shared memory of an SM (checked here for the
- *          solve, by sf_gradient / sf_curl for their extra fields): UNSUPPORTED otherwise.
+ *          rows of Table 1.  The fused pass must also fit the shared memory of an SM: checked here for sf_solve
+ *          (on ncomp == 3 plans for the three tiles of sf_curl / sf_divergence), by sf_gradient for its second
+ *          tile when it is called; UNSUPPORTED otherwise.
  *   h      [host] grid spacing per axis.  Domain length follows (Table 1): periodic
  *          and cell-centre L = n h; Dirichlet cell-boundary L = (n + 1) h; Neumann cell-boundary L = (n - 1) h.
  *   bc     [host] boundary condition per axis; all axes must agree.
