@@ -24,7 +24,7 @@ def _check(name, got, ref, prec):
     assert np.isfinite(e) and e <= TOL[prec], f"{name}: rel-L2 {e:.3e} > {TOL[prec]:.0e}"
 
 
-@pytest.mark.parametrize("nx", [16, 32, 64, 256])
+@pytest.mark.parametrize("nx", [16, 32, 64, 256, 512])
 def test_fast_path_white_noise_narrow_x(nx):
     """z = y = 256 selects the fast S2/S3/S4 kernels; x extent nx gives nx/16 full column tiles plus
     the Nyquist column; nx = 256 also selects the fast S1 / S5 kernels."""
