@@ -226,89 +226,85 @@ void axis_tables(const sf_plan_s& pl, int a, int count, std::vector<long double>
 
 // ---------------------------------------------------------------- plan-time kernels (fp64)
 // G on the doubled grid at the mirrored distance min(i, P - i) h (reading A12), times
-// the cell volume (reading A11).  Kernel: 2nd-order Gaussian regularisation (reading A10).
-// orders 4 .. 10 (reading A25): G_P = G_2 - sum_{n=1}^{P/2-1} eps^2/(2n) L_{n-1}^(1/2)(x) g,
-// x = r^2 / (2 eps^2), g the unit Gaussian of width eps.
-// order 0: the spectrally compact kernel -Si(pi r / h) / (2 pi^2 r), h passed in `eps` (reading A26).
-// Si: power series below 3, above it pi/2 + Im E1(i x) with E1 by its continued fraction (modified Lentz),
-// complex arithmetic written out.
+// the cell volume (reading A11).  Kernels (formulas: DESIGN.md readings A10, A25, A26, A28):
+//   order 2      3-D  -erf(r / (sqrt 2 eps)) / (4 pi r)            2-D  (ln r + E_1(r^2 / 2 eps^2) / 2) / (2 pi)
+//   order 4..10  G_P = G_2 - sum_{n=1}^{P/2-1} eps^2 / (2 n) L_{n-1}^(alpha)(x) g,  x = r^2 / (2 eps^2), g the unit
+//                Gaussian of width eps, alpha = 1/2 in 3-D and 0 in 2-D
+//   order 0      the spectrally compact kernel -Si(pi r / h) / (2 pi^2 r), h passed in `eps`
+//
+// The special functions are evaluated by routes of their own (no expansion shared with the checker):
+//   Si(x), x < 50:   the Bessel-function series  Si(x) = x sum_{n>=0} j_n(x/2)^2  (Abramowitz & Stegun 5.2.15), the
+//                    spherical Bessel functions by Miller's downward recurrence, normalised with sum (2n+1) j_n^2 = 1
+//   Si(x), x >= 50:  Si = pi/2 - f cos x - g sin x with the asymptotic expansions of the auxiliary functions
+//                    f ~ (1/x) sum (-1)^k (2k)! / x^2k,  g ~ (1/x^2) sum (-1)^k (2k+1)! / x^2k  (smallest term < 1e-19)
+//   E_1(u), u < 50:  E_1 = -gamma - ln u + e^-u sum_{n>=1} H_n u^n / n!  (H_n harmonic numbers; all terms positive, so
+//                    the ABSOLUTE error is a few ulp of ln u, which is what (ln r + E_1 / 2) needs)
+//   E_1(u), u >= 50: e^-u / u (1 - 1/u + 2/u^2 - ...), below 1e-23
+//   Laguerre polynomials by their three-term recurrence (k+1) L_{k+1} = (2k + 1 + alpha - x) L_k - (k + alpha) L_{k-1}
 __device__ double sine_integral(double x)
 {
-    if (x < 3.0) {
-        double term = x, sum = x;
-        const double x2 = x * x;
-        for (int n = 1; n < 40; ++n) {
-            term *= -x2 / ((2.0 * n) * (2.0 * n + 1.0));
-            sum += term / (2.0 * n + 1.0);
+    if (x >= 50.0) {
+        const double x2 = 1.0 / (x * x);
+        double tf = 1.0, tg = 1.0, f = 1.0, g = 1.0;
+        for (int k = 1; k < 30; ++k) {
+            const double nf = -tf * (2.0 * k) * (2.0 * k - 1.0) * x2, ng = -tg * (2.0 * k + 1.0) * (2.0 * k) * x2;
+            if (fabs(nf) >= fabs(tf) || fabs(nf) < 1e-20) break;   // past the smallest term, or converged
+            tf = nf; tg = ng;
+            f += tf; g += tg;
         }
-        return sum;
+        double sn, cs;
+        sincos(x, &sn, &cs);
+        return 1.5707963267948966192 - (f / x) * cs - (g * x2) * sn;
     }
-    // z = i x;  b = z + 1;  c = huge;  d = 1/b;  h = d
-    double br = 1.0, bi = x, cr = 1e300, ci = 0.0;
-    double den = br * br + bi * bi;
-    double dr = br / den, di = -bi / den, hr = dr, hi = di;
-    for (int i = 1; i < 500; ++i) {
-        const double a = -(double)i * (double)i;
-        br += 2.0;
-        // d = 1 / (a d + b)
-        double tr = a * dr + br, ti = a * di + bi;
-        den = tr * tr + ti * ti;
-        dr = tr / den; di = -ti / den;
-        // c = b + a / c
-        den = cr * cr + ci * ci;
-        tr = br + a * cr / den; ti = bi - a * ci / den;
-        cr = tr; ci = ti;
-        // del = c d;  h *= del
-        const double er = cr * dr - ci * di, ei = cr * di + ci * dr;
-        tr = hr * er - hi * ei; ti = hr * ei + hi * er;
-        hr = tr; hi = ti;
-        if (fabs(er - 1.0) + fabs(ei) < 1e-16) break;
+    const double z = 0.5 * x;
+    // downward recurrence j_{n-1} = (2n + 1) / z j_n - j_{n+1} from far above the turning point n ~ z
+    const int N = (int)z + 40;
+    double jp = 0.0, jn = 1e-30, s1 = 0.0, s2 = 0.0;   // j_{n+1}, j_n (unnormalised); sum (2n+1) j_n^2, sum j_n^2
+    for (int n = N; n >= 0; --n) {
+        s1 += (2.0 * n + 1.0) * jn * jn;
+        s2 += jn * jn;
+        const double jm = (2.0 * n + 1.0) / z * jn - jp;
+        jp = jn; jn = jm;
+        if (fabs(jn) > 1e120) {   // rescale: only ratios matter
+            jn *= 1e-120; jp *= 1e-120;
+            s1 *= 1e-240; s2 *= 1e-240;
+        }
     }
-    // E1(i x) = h exp(-i x);  Si = pi/2 + Im E1
-    double sn, cs;
-    sincos(x, &sn, &cs);
-    return 1.5707963267948966192 + (hi * cs - hr * sn);
+    return x * s2 / s1;
 }
-// exponential integral E_1(u), u > 0 (2-D kernels): power series about 0 up to u = 1, continued fraction beyond
 __device__ double exp_integral1(double u)
 {
-    if (u <= 1.0) {
-        double sum = 0.0, term = 1.0;
-        for (int k = 1; k < 60; ++k) {
-            term *= -u / (double)k;
-            const double add = term / (double)k;
-            sum += add;
-            if (fabs(add) < 1e-18 * fabs(sum)) break;
-        }
-        return -0.57721566490153286061 - log(u) - sum;
+    if (u >= 50.0) {
+        const double iu = 1.0 / u;
+        return exp(-u) * iu * (1.0 - iu * (1.0 - 2.0 * iu * (1.0 - 3.0 * iu)));
     }
-    double b = u + 1.0, c = 1e300, d = 1.0 / b, hh = d;
-    for (int i = 1; i < 500; ++i) {
-        const double a = -(double)i * (double)i;
-        b += 2.0;
-        d = 1.0 / (a * d + b);
-        c = b + a / c;
-        const double del = c * d;
-        hh *= del;
-        if (fabs(del - 1.0) < 1e-16) break;
+    double term = 1.0, hn = 0.0, sum = 0.0;
+    for (int n = 1; n < 400; ++n) {
+        term *= u / (double)n;     // u^n / n!
+        hn += 1.0 / (double)n;     // H_n
+        const double add = hn * term;
+        sum += add;
+        if ((double)n > u && add < 1e-17 * sum) break;
     }
-    return hh * exp(-u);
+    return (-0.57721566490153286061 - log(u)) + exp(-u) * sum;
 }
-// 2-D kernels (reading A28): G_2 = (ln r + E_1(r^2 / 2 eps^2) / 2) / (2 pi), orders 4 .. 10 subtract
-// eps^2 / (2 n) L_{n-1}(x) g with the ordinary Laguerre polynomials and the 2-D unit Gaussian g
+// sum_{n=1}^{P/2-1} L_{n-1}^(alpha)(x) / (2 n)
+__device__ double laguerre_tail(int order, double alpha, double x)
+{
+    double lm = 0.0, lk = 1.0, acc = 0.0;   // L_{k-1}, L_k
+    for (int k = 0; k + 1 < order / 2; ++k) {
+        acc += lk / (2.0 * (k + 1));
+        const double ln = ((2.0 * k + 1.0 + alpha - x) * lk - (k + alpha) * lm) / (k + 1.0);
+        lm = lk; lk = ln;
+    }
+    return acc;
+}
 __device__ double green2d_value(double r, double eps, int order)
 {
     const double x = r * r / (2.0 * eps * eps);
     double v = (r == 0.0) ? (log(2.0 * eps * eps) - 0.57721566490153286061) / 12.566370614359172954
                           : (log(r) + 0.5 * exp_integral1(x)) / 6.2831853071795864769;
-    if (order >= 4) {
-        const double gs = exp(-x) / (6.2831853071795864769 * eps * eps);
-        double poly = 0.5;                                                              // n = 1: L_0 / 2
-        if (order >= 6) poly += (1.0 - x) * 0.25;                                       // n = 2: L_1 / 4
-        if (order >= 8) poly += ((0.5 * x - 2.0) * x + 1.0) / 6.0;                      // n = 3: L_2 / 6
-        if (order >= 10) poly += (((-x / 6.0 + 1.5) * x - 3.0) * x + 1.0) * 0.125;      // n = 4: L_3 / 8
-        v -= eps * eps * poly * gs;
-    }
+    if (order >= 4) v -= laguerre_tail(order, 0.0, x) * exp(-x) / 6.2831853071795864769;   // eps^2 * g = e^-x / (2 pi)
     return v;
 }
 __global__ void green_eval_kernel(double* g, int Px, int Py, int Pz, double hx, double hy, double hz, double eps, double vol, int order,
@@ -326,12 +322,7 @@ __global__ void green_eval_kernel(double* g, int Px, int Py, int Pz, double hx, 
         else v = -erf(r * 0.70710678118654752440 / eps) / (12.566370614359172954 * r);
         if (order >= 4) {
             const double x = r * r / (2.0 * eps * eps);
-            const double gs = exp(-x) / (15.749609945722419 * eps * eps * eps);
-            double poly = 0.5;                                                                       // n = 1: L_0 / 2
-            if (order >= 6) poly += (1.5 - x) * 0.25;                                                // n = 2: L_1 / 4
-            if (order >= 8) poly += ((0.5 * x - 2.5) * x + 1.875) / 6.0;                             // n = 3: L_2 / 6
-            if (order >= 10) poly += (((-x / 6.0 + 1.75) * x - 4.375) * x + 2.1875) * 0.125;         // n = 4: L_3 / 8
-            v -= eps * eps * poly * gs;
+            v -= laguerre_tail(order, 0.5, x) * exp(-x) / (15.749609945722419 * eps);   // eps^2 * g = e^-x / ((2 pi)^(3/2) eps)
         }
         g[i] = vol * v;
     }

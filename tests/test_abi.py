@@ -42,6 +42,32 @@ def test_binding_has_no_cpu_fallback_and_no_oracle_import():
         assert "oracle" not in f.read_text().lower(), f"{f.name} mentions the oracle"
 
 
+def _shingles(text, k=4):
+    """runs of k consecutive code lines, whitespace removed, type keywords dropped and identifiers folded to one letter (so that a
+    renamed copy still matches); comment-only and trivial lines (braces, short statements) are skipped"""
+    import re
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    lines = []
+    for ln in text.splitlines():
+        ln = ln.split("//")[0]
+        ln = re.sub(r"\b(const|double|float|int|long|unsigned|static|complex)\b", "", ln)
+        ln = re.sub(r"[A-Za-z_][A-Za-z_0-9]*", "v", ln)
+        ln = re.sub(r"\s+", "", ln)
+        if len(ln) >= 8:
+            lines.append(ln)
+    return {tuple(lines[i:i + k]) for i in range(len(lines) - k + 1)}
+
+
+def test_no_routine_of_the_checker_is_restated_in_the_product():
+    """VERDICT r1 'What's weak' 1: the CUDA path and the checker share no code -- not even a transliterated
+    routine.  Mechanical form: no four consecutive non-trivial statements of oracle/sf_oracle.c reappear, up to
+    whitespace and identifier names, in any source file of the product."""
+    ora = _shingles((ROOT / "oracle" / "sf_oracle.c").read_text())
+    for f in sorted((ROOT / "paper_2301_01145_b200" / "csrc").iterdir()):
+        common = ora & _shingles(f.read_text())
+        assert not common, f"{f.name} restates checker code: {sorted(common)[:2]}"
+
+
 def test_null_plan_calls_fail_without_a_device():
     import paper_2301_01145_b200 as sf
 

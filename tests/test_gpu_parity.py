@@ -258,6 +258,32 @@ def test_cfg4_spectrally_compact_kernel(prec):
     assert e <= (5e-6 if prec == "f32" else 1e-11)
 
 
+def test_spectral_kernel_unit_source_against_the_library_sine_integral():
+    """the DEVICE sine integral (Bessel-function series / asymptotic auxiliary functions; shares no expansion
+    with the oracle's series + continued fraction) pinned to scipy's Si: a unit source returns
+    h^3 G(|x - x0|) = -h^3 Si(pi r / h) / (2 pi^2 r) itself (reading A26).  Arguments pi r / h from 3 to 340
+    cross the switch between the two device expansions at 50."""
+    from scipy.special import sici
+    n, h = 64, 1.0 / 64
+    f = np.zeros((n, n, n))
+    x0 = (40, 3, 63)
+    f[x0] = 1.0
+    with Plan(f.shape, (h, h, h), sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_SPECTRAL, prec="f64") as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI)
+    iz, iy, ix = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    r = h * np.sqrt((iz - x0[0]) ** 2.0 + (iy - x0[1]) ** 2.0 + (ix - x0[2]) ** 2.0)
+    want = np.full(r.shape, -1.0 / (2 * np.pi * h))
+    nz = r > 0
+    want[nz] = -sici(np.pi * r[nz] / h)[0] / (2 * np.pi ** 2 * r[nz])
+    want *= h ** 3
+    assert (np.pi * r.max() / h) > 300 and (np.pi * r[nz].min() / h) < 4
+    # the transform round trip adds rounding ~ 1e-16 |G|_max, so the tolerance is absolute against the peak
+    assert np.abs(got - want).max() <= 1e-13 * np.abs(want).max()
+    assert rel_l2(got, want) <= 1e-13
+
+
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_cfg4_unbounded_gradient(prec):
     """sf_gradient on a scalar unbounded plan (north_star: ik gradients from the same spectrum):

@@ -60,6 +60,11 @@ def test_unbounded_2d_unit_source_and_closed_form():
         for (iy, ix) in ((70, 5), (0, 0), (127, 127), (71, 5), (70, 9)):
             r = h * float(np.hypot(ix - 5, iy - 70))
             assert got[iy, ix] == pytest.approx(h * h * O.green2d_gauss(2, r, eps), rel=1e-11, abs=1e-17)
+            # ... and the library's exponential integral directly (third opinion for the DEVICE routine, which
+            # shares no expansion with the oracle's): G_2 = (ln r + E_1(r^2 / 2 eps^2) / 2) / (2 pi), reading A28
+            want = (np.log(r) + 0.5 * sp.exp1(r * r / (2 * eps * eps))) / (2 * np.pi) if r > 0 else \
+                (np.log(2 * eps * eps) - np.euler_gamma) / (4 * np.pi)
+            assert got[iy, ix] == pytest.approx(h * h * want, rel=1e-11, abs=1e-17)
         x = (np.arange(n) + 0.5) * h
         sig, cx, cy = 3.0 * h, 0.47, 0.55
         r2 = (x[None, :] - cx) ** 2 + (x[:, None] - cy) ** 2
