@@ -129,7 +129,8 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
  * sf_set_source -- the paper's Set_Input.
  *   src    ncomp dense fields of n[0]*n[1]*n[2] elements of the plan's precision.
  *   where  SF_MEM_DEVICE: the pointer is BORROWED -- it must stay valid and unchanged until the
- *          solve that consumes it has completed on the plan's stream; nothing is copied.
+ *          solve that consumes it has completed on the plan's stream; nothing is copied.  It must be
+ *          16-byte aligned (rows are moved by 16-byte and bulk copies); INVALID_ARG otherwise.
  *          SF_MEM_HOST: the data are copied to a plan-owned device buffer on the plan's stream
  *          (the host buffer may be reused after the call returns only if it is pageable; for
  *          pinned memory after sf_synchronize or the next blocking call).
@@ -148,6 +149,9 @@ sf_status sf_set_source(sf_plan plan, const void* src, sf_mem where);
  *          Neumann:   d psi / d x_axis along +axis on both faces (eq. 15);
  *                     cell-centre grids: weights +1/h (lower), -1/h (upper); cell-boundary grids
  *                     (ghost node mirrored through the boundary node): +2/h, -2/h.
+ *          The values are those of psi (or of its derivative) whatever rhs_sign is: the discrete equation is
+ *          lap_h psi = rhs_sign f with these values in the ghost layer, so the weights above apply to
+ *          rhs_sign f (the library divides them by rhs_sign before adding them to f).
  *   where  as for sf_set_source (device pointers borrowed, host data copied).
  * Errors: UNSUPPORTED for periodic / unbounded plans or the PS operator.
  */

@@ -509,11 +509,14 @@ done:
 
 /* ------------------------------------------------------------------------------------------
  * Boundary-value folding (weights: reading A18).
+ * The discrete equation is lap_h psi = rhs_sign f with the face values in the ghost layer (eq. (2)
+ * and reading A8), i.e. interior stencil = rhs_sign f + w g; the solvers below multiply the folded source by
+ * rhs_sign, so the fold adds (w / rhs_sign) g to f: the face value itself never changes sign.
  * faces[2*axis + side] (side 0 = lower, 1 = upper) holds the values on that face over the two
  * remaining axes, lower axis fastest; NULL = homogeneous.
  * ---------------------------------------------------------------------------------------- */
 static void fold_faces(double *fp, const i64 n[3], const double h[3], const double *const faces[6],
-                       int neumann)
+                       int neumann, double rhs_sign)
 {
     for (int axis = 0; axis < 3; ++axis) {
         int a = (axis == 0) ? 1 : 0;           /* lower remaining axis (fastest in the face) */
@@ -526,6 +529,7 @@ static void fold_faces(double *fp, const i64 n[3], const double h[3], const doub
             double w;
             if (!neumann) w = -1.0 / (h[axis] * h[axis]);          /* Dirichlet, cell-boundary */
             else w = side ? -1.0 / h[axis] : +1.0 / h[axis];       /* Neumann, cell-centre     */
+            w /= rhs_sign;                                         /* the equation is lap_h psi = rhs_sign f (A8) */
             for (i64 jb = 0; jb < n[b]; ++jb)
                 for (i64 ja = 0; ja < n[a]; ++ja)
                     fp[ic * st[axis] + ja * st[a] + jb * st[b]] += w * g[ja + n[a] * jb];
@@ -548,7 +552,7 @@ int orc_dirichlet_regular(const i64 n[3], const double h[3], int op, double rhs_
     double *lam[3] = { 0, 0, 0 };
     int err = ORC_OK, ntab = 0;
     memcpy(psi, f, sizeof(double) * (size_t)tot);
-    if (op == 1) fold_faces(psi, n, h, faces, 0);
+    if (op == 1) fold_faces(psi, n, h, faces, 0, rhs_sign);
     for (int a = 0; a < 3; ++a) {
         if ((err = trig_table_init(&tab[a], (int)n[a], 2 * (n[a] + 1))) != ORC_OK) { ntab = a + 1; goto done; }
         ntab = a + 1;
@@ -602,7 +606,7 @@ int orc_neumann_staggered(const i64 n[3], const double h[3], int op, double rhs_
     double *lam[3] = { 0, 0, 0 };
     int err = ORC_OK, ntab = 0;
     memcpy(psi, f, sizeof(double) * (size_t)tot);
-    if (op == 1) fold_faces(psi, n, h, faces, 1);
+    if (op == 1) fold_faces(psi, n, h, faces, 1, rhs_sign);
     for (int a = 0; a < 3; ++a) {
         if ((err = trig_table_init(&tab[a], (int)n[a], 4 * n[a])) != ORC_OK) { ntab = a + 1; goto done; }
         ntab = a + 1;
@@ -660,7 +664,8 @@ done:
  *   op = 0 (PS):  Lambda = -sum_a (pi k_a / L_a)^2
  * Zero mode -> 0.  psi = DCT-I_3(rhs_sign * DCT-I_3(f') / Lambda) / prod_a (2 (N_a-1)).
  * ---------------------------------------------------------------------------------------- */
-static void fold_faces_f3(double *fp, const i64 n[3], const double h[3], const double *const faces[6], int neumann)
+static void fold_faces_f3(double *fp, const i64 n[3], const double h[3], const double *const faces[6], int neumann,
+                          double rhs_sign)
 {
     for (int axis = 0; axis < 3; ++axis) {
         int a = (axis == 0) ? 1 : 0;
@@ -673,6 +678,7 @@ static void fold_faces_f3(double *fp, const i64 n[3], const double h[3], const d
             double w;
             if (!neumann) w = -2.0 / (h[axis] * h[axis]);          /* Dirichlet, cell-centre   */
             else w = side ? -2.0 / h[axis] : +2.0 / h[axis];       /* Neumann, cell-boundary   */
+            w /= rhs_sign;
             for (i64 jb = 0; jb < n[b]; ++jb)
                 for (i64 ja = 0; ja < n[a]; ++ja)
                     fp[ic * st[axis] + ja * st[a] + jb * st[b]] += w * g[ja + n[a] * jb];
@@ -688,7 +694,7 @@ int orc_dirichlet_staggered(const i64 n[3], const double h[3], int op, double rh
     double *lam[3] = { 0, 0, 0 };
     int err = ORC_OK, ntab = 0;
     memcpy(psi, f, sizeof(double) * (size_t)tot);
-    if (op == 1) fold_faces_f3(psi, n, h, faces, 0);
+    if (op == 1) fold_faces_f3(psi, n, h, faces, 0, rhs_sign);
     for (int a = 0; a < 3; ++a) {
         if ((err = trig_table_init(&tab[a], (int)n[a], 4 * n[a])) != ORC_OK) { ntab = a + 1; goto done; }
         ntab = a + 1;
@@ -736,7 +742,7 @@ int orc_neumann_regular(const i64 n[3], const double h[3], int op, double rhs_si
     int err = ORC_OK, ntab = 0;
     for (int a = 0; a < 3; ++a) if (n[a] < 2) return ORC_ERR_ARG;
     memcpy(psi, f, sizeof(double) * (size_t)tot);
-    if (op == 1) fold_faces_f3(psi, n, h, faces, 1);
+    if (op == 1) fold_faces_f3(psi, n, h, faces, 1, rhs_sign);
     for (int a = 0; a < 3; ++a) {
         if ((err = trig_table_init(&tab[a], (int)n[a], 2 * (n[a] - 1))) != ORC_OK) { ntab = a + 1; goto done; }
         ntab = a + 1;
@@ -860,7 +866,7 @@ int orc_bounded_gradient(int kind, const i64 n[3], const double h[3], int op, do
     int neumann = (kind == 1 || kind == 3);
     if (!coef) return ORC_ERR_ALLOC;
     memcpy(coef, f, sizeof(double) * (size_t)tot);
-    if (op == 1) { if (kind < 2) fold_faces(coef, n, h, faces, neumann); else fold_faces_f3(coef, n, h, faces, neumann); }
+    if (op == 1) { if (kind < 2) fold_faces(coef, n, h, faces, neumann, rhs_sign); else fold_faces_f3(coef, n, h, faces, neumann, rhs_sign); }
     double norm = 1.0;
     for (int a = 0; a < 3; ++a) {
         i64 N = n[a];

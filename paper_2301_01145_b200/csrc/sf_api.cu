@@ -370,6 +370,9 @@ template <typename T> sf_status build_green(sf_plan p)
     const double eps = (p->op == SF_OP_GREEN_SPECTRAL ? 1.0 : p->eps_over_h) * hmax;
     const double vol = two_d ? p->h[0] * p->h[1] : p->h[0] * p->h[1] * p->h[2];
     const int order = (p->op == SF_OP_GREEN_SPECTRAL) ? 0 : 2 * ((int)p->op - (int)SF_OP_GREEN_GAUSS2 + 1);
+    // the table uploads above are synchronous copies from pageable memory on the legacy stream, which a
+    // non-blocking plan stream does not wait for: drain the device once before the first kernel reads them
+    SF_CUDA(p, cudaDeviceSynchronize());
     green_eval_kernel<<<148 * 8, 256, 0, p->stream>>>(g, Px, Py, Pz, p->h[0], p->h[1], p->h[2], eps, vol, order, two_d ? 1 : 0);
     SF_CUDA(p, cudaGetLastError());
 
@@ -481,8 +484,11 @@ template <typename T> sf_status run(sf_plan p, int outk)
                 // reading A18: the face sits one spacing (cell-boundary Dirichlet, cell-centre Neumann: weight 1)
                 // or half a spacing / a mirrored ghost node (the other two Table-1 rows: weight 2) from the layer
                 const double wf = ((p->bc == SF_BC_DIRICHLET) == (p->grid == SF_GRID_CELL_BOUNDARY)) ? 1.0 : 2.0;
-                if (p->bc == SF_BC_DIRICHLET) xp.wface[2 * a + s] = (T)(-wf / (p->h[a] * p->h[a]));
-                else xp.wface[2 * a + s] = (T)((s ? -wf : wf) / p->h[a]);
+                // the discrete equation is lap_h psi = rhs_sign f with the face value in the ghost layer (eq. (2)
+                // PAPER.md:22, reading A8): interior stencil = rhs_sign f + w g.  The multiplier carries rhs_sign for
+                // the whole folded source, so the fold adds (w / rhs_sign) g -- the face value keeps its sign.
+                if (p->bc == SF_BC_DIRICHLET) xp.wface[2 * a + s] = (T)(-wf / (p->h[a] * p->h[a]) / p->rhs_sign);
+                else xp.wface[2 * a + s] = (T)((s ? -wf : wf) / p->h[a] / p->rhs_sign);
             }
     }
     mark(0);
@@ -897,7 +903,9 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         p->fastper = true;
         p->fastper_x = (p->n[0] == 256) && !getenv("SF_DISABLE_FAST_X");
     }
-    if (cudaStreamSynchronize(p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "plan construction failed on the device");
+    // everything the plan built (uploads on the legacy stream, kernels and memsets on the plan's stream) is complete
+    // before the first compute call can be enqueued
+    if (cudaDeviceSynchronize() != cudaSuccess) return bail(SF_ERR_CUDA, "plan construction failed on the device");
     *out = p;
     return SF_OK;
 }
@@ -963,18 +971,26 @@ sf_status sf_gradient(sf_plan plan)
     // unbounded, Dirichlet, Neumann: psi and its derivatives need 1 + ndim fields of work space
     const int nf = 1 + plan->ndim;
     const size_t welem = (plan->r2r == R2R_NONE) ? 2 * plan->esize : plan->esize;
-    if (!plan->gW1) {
+    if (!plan->gout) {
+        // all three arrays or none: a half-made set must never be swapped in (the next call would launch on NULL)
         sf_status st;
         const size_t b1 = (size_t)plan->w1_field * nf * welem, b2 = (size_t)plan->w2_field * nf * welem;
-        if ((st = dev_alloc(plan, &plan->gW1, b1)) != SF_OK) return st;
-        SF_CUDA(plan, cudaMemsetAsync(plan->gW1, 0, b1, plan->stream));
-        if (plan->padded) {
-            if ((st = dev_alloc(plan, &plan->gW2, b2)) != SF_OK) return st;
-            SF_CUDA(plan, cudaMemsetAsync(plan->gW2, 0, b2, plan->stream));
-        } else {
-            plan->gW2 = plan->gW1;
+        void *w1 = nullptr, *w2 = nullptr, *go = nullptr;
+        st = dev_alloc(plan, &w1, b1);
+        if (st == SF_OK && plan->padded) st = dev_alloc(plan, &w2, b2);
+        if (st == SF_OK) st = dev_alloc(plan, &go, field_elems(plan) * nf * plan->esize);
+        if (st != SF_OK) {
+            const std::string msg = plan->err;
+            if (w1) { dev_free(plan, w1); plan->dev_bytes -= (long long)b1; }
+            if (w2) { dev_free(plan, w2); plan->dev_bytes -= (long long)b2; }
+            plan->err = msg;
+            return st;
         }
-        if ((st = dev_alloc(plan, &plan->gout, field_elems(plan) * nf * plan->esize)) != SF_OK) return st;
+        SF_CUDA(plan, cudaMemsetAsync(w1, 0, b1, plan->stream));
+        if (w2) SF_CUDA(plan, cudaMemsetAsync(w2, 0, b2, plan->stream));
+        plan->gW1 = w1;
+        plan->gW2 = plan->padded ? w2 : w1;
+        plan->gout = go;
     }
     std::swap(plan->W1, plan->gW1);
     std::swap(plan->W2, plan->gW2);

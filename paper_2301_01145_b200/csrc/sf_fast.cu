@@ -72,6 +72,7 @@ cudaError_t fast_init()
     if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres)) != cudaSuccess) return e;
     if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
     g_encode = (EncodeTiledFn)fn;
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return e;   // the symbol uploads above have landed
     g_ready_dev = dev;
     return cudaSuccess;
 }

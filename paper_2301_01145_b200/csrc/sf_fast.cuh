@@ -416,7 +416,9 @@ __global__ void __launch_bounds__(kThreads, 2) fast_pad_kernel(const FastParams 
                 // reads one 128-byte run per row (16 batches of one column for the Nyquist tiles)
                 if (side) {
                     // the producer (S3) left this column as [pencil of S4 = z][ky]: read 512 contiguous ky
-                    // per z and transpose through the exchange buffer
+                    // per z and transpose through the exchange buffer (which the previous tile's second half may
+                    // still be reading when this is not the CTA's first tile)
+                    if (it > 0) __syncthreads();
                     for (int idx = tid; idx < 2 * kL * kTile; idx += kThreads) {
                         const int pp = idx >> 9, ky = idx & (2 * kL - 1);
                         stage(ky, pp) = (g.b + pp < p.nb) ? __ldg(p.nyq_in + (g.b + pp) * (2 * kL) + ky) : make_float2(0.f, 0.f);

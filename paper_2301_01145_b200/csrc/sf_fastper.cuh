@@ -105,6 +105,7 @@ __global__ void __launch_bounds__(kThreads, GRAD ? 1 : 2) fast_per_kernel(const 
         auto stage = [&](int row, int pencil) -> C& { return xbuf[row * 32 + ((pencil + row) & 31)]; };
         C v[16];
         if (transposed) {
+            if (it > 0) __syncthreads();   // the previous tile's second half may still be reading the exchange buffer
 #pragma unroll 4
             for (int j = 0; j < 16; ++j) {
                 const int idx = tid + kThreads * j, pl = idx >> 8, row = idx & 255;
