@@ -177,6 +177,17 @@ def periodic_laplacian(f, L, op=OP_PS, rhs_sign=1.0, ncomp=1):
     return out
 
 
+def periodic_curl(f, L, op=OP_PS, rhs_sign=1.0):
+    """CURL on a periodic 3-D vector plan: f[3, z, y, x] -> u = curl psi, psi_c the solution for source f_c."""
+    f = _f64(f)
+    assert f.ndim == 4 and f.shape[0] == 3
+    nd, n = _dims(f.shape[1:])
+    out = np.empty_like(f)
+    _chk(lib().orc_periodic_curl(_i64x3(n), _f64x3(list(L)), C.c_int(op), C.c_double(rhs_sign), _ptr(f), _ptr(out)),
+         "periodic_curl")
+    return out
+
+
 def _faces_arg(faces):
     """faces: dict {(axis, side): array} or None -> (const double*[6], keepalive)."""
     arr = (C.c_void_p * 6)()

@@ -1341,6 +1341,76 @@ done:
     return err;
 }
 
+/* CURL on a periodic 3-D vector plan (eq. (10); component-wise vector solve PAPER.md:119):
+ * psi_hat_c = rhs_sign F_c / Lambda for each component as in orc_periodic (zero mode -> 0), then
+ *   u_hat = i kappa x psi_hat,  u_a = IDFT(i (kappa_b psi_hat_c - kappa_c psi_hat_b)),  (a, b, c) cyclic,
+ * kappa_a = 2 pi m_a / L_a, zero at the Nyquist index (reading A20).  f, out: three fields, component-major. */
+int orc_periodic_curl(const i64 n[3], const double L[3], int op, double rhs_sign, const double *f, double *out)
+{
+    i64 tot = n[0] * n[1] * n[2];
+    for (int a = 0; a < 3; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
+    cplx *P[3] = { 0, 0, 0 }, *W = NULL;
+    double *kap[3] = { 0, 0, 0 }, *lam[3] = { 0, 0, 0 };
+    int err = ORC_OK;
+    for (int a = 0; a < 3; ++a) {
+        i64 N = n[a];
+        kap[a] = (double *)calloc((size_t)N, sizeof(double));
+        lam[a] = (double *)calloc((size_t)N, sizeof(double));
+        P[a] = (cplx *)malloc(sizeof(cplx) * (size_t)tot);
+        if (!kap[a] || !lam[a] || !P[a]) { err = ORC_ERR_ALLOC; goto done; }
+        double hh = L[a] / (double)N;
+        for (i64 k = 0; k < N; ++k) {
+            i64 m = (2 * k < N) ? k : k - N;
+            double kappa = 2.0 * PI * (double)m / L[a];
+            kap[a][k] = (2 * k == N) ? 0.0 : kappa;
+            if (op == 0) lam[a][k] = -kappa * kappa;
+            else {
+                double sn, cs;
+                sincos2pi(k, 2 * N, &sn, &cs);
+                lam[a][k] = -(4.0 / (hh * hh)) * sn * sn;
+            }
+        }
+    }
+    W = (cplx *)malloc(sizeof(cplx) * (size_t)tot);
+    if (!W) { err = ORC_ERR_ALLOC; goto done; }
+    for (int c = 0; c < 3; ++c) {
+        const double *fc = f + (size_t)c * (size_t)tot;
+#pragma omp parallel for schedule(static)
+        for (i64 i = 0; i < tot; ++i) P[c][i] = fc[i];
+        for (int a = 0; a < 3; ++a)
+            if ((err = fft_axis(P[c], n, a, -1)) != ORC_OK) goto done;
+#pragma omp parallel for collapse(2) schedule(static)
+        for (i64 kz = 0; kz < n[2]; ++kz)
+            for (i64 ky = 0; ky < n[1]; ++ky)
+                for (i64 kx = 0; kx < n[0]; ++kx) {
+                    i64 i = kx + n[0] * (ky + n[1] * kz);
+                    if (kx || ky || kz) P[c][i] = rhs_sign * P[c][i] / (lam[0][kx] + lam[1][ky] + lam[2][kz]);
+                    else P[c][i] = 0.0;
+                }
+    }
+    double inv_n = 1.0 / (double)tot;
+    for (int a = 0; a < 3; ++a) {
+        int b = (a + 1) % 3, c = (a + 2) % 3;   /* u_a = d_b psi_c - d_c psi_b */
+#pragma omp parallel for collapse(2) schedule(static)
+        for (i64 kz = 0; kz < n[2]; ++kz)
+            for (i64 ky = 0; ky < n[1]; ++ky)
+                for (i64 kx = 0; kx < n[0]; ++kx) {
+                    i64 i = kx + n[0] * (ky + n[1] * kz);
+                    i64 kk[3] = { kx, ky, kz };
+                    W[i] = I * (kap[b][kk[b]] * P[c][i] - kap[c][kk[c]] * P[b][i]);
+                }
+        for (int ax = 2; ax >= 0; --ax)
+            if ((err = fft_axis(W, n, ax, +1)) != ORC_OK) goto done;
+        double *oa = out + (size_t)a * (size_t)tot;
+#pragma omp parallel for schedule(static)
+        for (i64 i = 0; i < tot; ++i) oa[i] = creal(W[i]) * inv_n;
+    }
+done:
+    for (int a = 0; a < 3; ++a) { free(kap[a]); free(lam[a]); free(P[a]); }
+    free(W);
+    return err;
+}
+
 /* ------------------------------------------------------------------------------------------
  * O-UNB2: 2-D unbounded solver (PAPER.md:189 lists the regularised kernels for 1-D, 2-D and 3-D,
  * formulas not printed -- reading A28).  Free-space kernel of the 2-D Laplacian: G_0 = ln(r) / (2 pi)

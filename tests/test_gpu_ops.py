@@ -114,3 +114,22 @@ def test_operator_error_paths():
         with pytest.raises(sf.SailffishError) as ei:
             sf.sf_laplacian(p.plan)
         assert ei.value.status == sf.SF_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("op", ["ps", "fd2"])
+def test_periodic_curl(prec, op):
+    """sf_curl on a PERIODIC vector plan (eq. (10) PAPER.md:141-148 on the component-wise solve):
+    white noise on a non-cubic box against the oracle, element by element"""
+    shape = (16, 64, 32)
+    L = (2.0, 1.0, 3.0)
+    f = rounded(_rand((3,) + shape, 99), prec)
+    f -= f.mean(axis=(1, 2, 3), keepdims=True, dtype=np.float64).astype(f.dtype)
+    oop, sop = (O.OP_PS, sf.SF_OP_PSEUDO_SPECTRAL) if op == "ps" else (O.OP_FD2, sf.SF_OP_FD2)
+    u_o = O.periodic_curl(f.astype(np.float64), L, oop, rhs_sign=-1.0)
+    h = (L[0] / shape[2], L[1] / shape[1], L[2] / shape[0])
+    with Plan(shape, h, sf.SF_BC_PERIODIC, op=sop, prec=prec, ncomp=3, rhs_sign=-1.0) as p:
+        p.set_source(f)
+        sf.sf_curl(p.plan)
+        for c in range(3):
+            _report(f"periodic curl {op} u[{c}]", p.get(sf.SF_OUT_CURL, c), u_o[c], prec)
