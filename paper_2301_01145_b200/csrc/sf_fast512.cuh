@@ -1,0 +1,461 @@
+// sf_fast512.cuh -- kernel generation 2 for fp32 unbounded plans with 512-long y / z pencils that are
+// zero-padded to 1024 (BASELINE.json configs[4]: 512^3 -> 1024^3, three components, curl): the strided
+// passes S2 (Y forward), S3 (Z forward x Green x [curl] x Z backward, fused) and S4 (Y backward)
+// (PAPER.md:89-97 pencils, :103-109 four-step solve, :119 component-wise vector solve, :141 spectral curl,
+// :181 / :213 padded and pruned Hockney-Eastwood transforms).
+//
+// Same ideas as sf_fast.cuh, one size up.  The 1024-point transform of (x, 0) is two 512-point transforms
+// (h = 0: x -> even outputs; h = 1: x w1024^n -> odd outputs) that run side by side in the two half-warps.
+// A CTA of 1024 threads owns a tile of 16 neighbouring pencils (one 128-byte run per row): warp index
+// w in 0..31 (warp-uniform), lane = pencil + 16 h.  Thread (w, pencil, h) holds the 16 elements
+// n = w + 32 r of its sequence.  A 512-point transform is
+//     radix-16 over r (registers) -> twiddle w512^(q w) -> ONE shared-memory exchange ->
+//     radix-32 over the 32 values o of slot row q0 = w mod 16, done as a radix-2 step that keeps the
+//     output parity p = w div 16 (16 sums or twiddled differences) and a radix-16 over the rest (registers)
+// and leaves X[w + 32 j] in thread w: input and output distributions agree, so forward, multiply and
+// backward chain without reordering.  One CTA per SM (128 KB exchange buffer + 64 KB TMA slot).
+//
+// Vector plans: sf_curl needs psi_hat of all three components at every spectral point, 393 KB per tile --
+// more than the registers or the shared memory of an SM hold.  The curl is therefore assembled after the
+// backward transform, where truncation has halved the data: with t_c = IDFT_z(psi_hat_c) and
+// d_c = IDFT_z(kappa_z psi_hat_c),
+//     u_x = i (kappa_y t_z - d_y),   u_y = i (d_x - kappa_x t_z),   u_z = i (kappa_x t_y - kappa_y t_x)
+// (kappa_x per column, kappa_y per tile: constants of the backward transform), components processed z, y, x.
+// What has to wait for a later component -- t_z, t_y, and the spectrum of the component that is transformed
+// back twice -- is parked in TENSOR MEMORY (tcgen05.st / tcgen05.ld, 32 lanes x 32-bit columns per warp: each
+// thread parks and fetches its own registers, which is exactly the access TMEM gives a warp): 256 + 128 + 128
+// of the 512 columns.  Three forward and five backward transforms per tile, no extra HBM traffic.
+#pragma once
+#include "sf_fast.cuh"
+
+namespace sf2 {
+
+constexpr int kT5 = 1024;            // threads per CTA
+constexpr int kL5 = 512;             // transform length (stored rows per pencil)
+constexpr int kGreenRows5 = kL5 + 1; // folded spectral indices 0 .. 512
+constexpr int kXchg5Elems = 16 * 32 * 32;                 // 128 KB
+constexpr int kSlot5Elems = kL5 * kTile;                  // 64 KB
+constexpr size_t kSmem5 = ((size_t)kXchg5Elems + kSlot5Elems) * sizeof(C);
+constexpr size_t kSmem5NoSlot = (size_t)kXchg5Elems * sizeof(C);
+
+enum { F5_FWD = 0, F5_INV = 1, F5_FUSED = 2, F5_CURL = 3 };
+
+__host__ __device__ constexpr double cos32(int i)
+{
+    constexpr double c[9] = { 1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
+                              0.70710678118654752440, 0.55557023301960222474, 0.38268343236508977173,
+                              0.19509032201612826785, 0.0 };
+    i &= 31;
+    if (i > 16) i = 32 - i;
+    return i <= 8 ? c[i] : -c[16 - i];
+}
+__host__ __device__ constexpr double sin32(int i) { return cos32(i - 8); }
+// d * exp(-/+ 2 pi i I32 / 32)   (forward: minus)
+template <int I32, bool INV> __device__ __forceinline__ C mul_w32(C d)
+{
+    if constexpr (I32 == 0) {
+        return d;
+    } else if constexpr (I32 == 8) {
+        return INV ? cmuli(d) : cmulmi(d);
+    } else {
+        constexpr float c = (float)cos32(I32);
+        constexpr float s = (float)(INV ? sin32(I32) : -sin32(I32));
+        return cmul(d, make_float2(c, s));
+    }
+}
+
+// first half: radix-16 over r, twiddle w512^(q w) (row w of a shared-memory table), write slots (q, w)
+template <bool INV> __device__ __forceinline__ void fft512_a(C (&v)[16], const C* tw, C* xw)
+{
+    dft16<INV>(v);
+#pragma unroll
+    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], tw[q]);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) xw[q * 1024] = v[brev4(q)];
+}
+// second half (after a barrier): slots (q0, o), o < 32, radix-2 keeping parity p, radix-16.
+// X[w + 32 j] at v[brev4(j)] out.
+template <bool INV, int P> __device__ __forceinline__ void fft512_b_p(C (&v)[16], const C* xr)
+{
+    auto step = [&](auto tag) {
+        constexpr int o2 = decltype(tag)::value;
+        const C a = xr[o2 * 32], b = xr[(o2 + 16) * 32];
+        if constexpr (P == 0) v[o2] = cadd(a, b);
+        else v[o2] = mul_w32<o2, INV>(csub(a, b));
+    };
+    step(std::integral_constant<int, 0>()); step(std::integral_constant<int, 1>());
+    step(std::integral_constant<int, 2>()); step(std::integral_constant<int, 3>());
+    step(std::integral_constant<int, 4>()); step(std::integral_constant<int, 5>());
+    step(std::integral_constant<int, 6>()); step(std::integral_constant<int, 7>());
+    step(std::integral_constant<int, 8>()); step(std::integral_constant<int, 9>());
+    step(std::integral_constant<int, 10>()); step(std::integral_constant<int, 11>());
+    step(std::integral_constant<int, 12>()); step(std::integral_constant<int, 13>());
+    step(std::integral_constant<int, 14>()); step(std::integral_constant<int, 15>());
+    dft16<INV>(v);
+}
+template <bool INV> __device__ __forceinline__ void fft512_b(C (&v)[16], const C* xr, int p)
+{
+    if (p) fft512_b_p<INV, 1>(v, xr);     // p is warp-uniform: no divergence
+    else fft512_b_p<INV, 0>(v, xr);
+}
+
+// ------------------------------------------------------------------------------------ tensor memory as a parking lot
+// 32x32b shape: lane i of the warp reads / writes TMEM lane (32 (warp mod 4) + i), consecutive 32-bit columns
+__device__ __forceinline__ void tmem_alloc512(uint32_t* smem_dst)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_dst)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_free512(uint32_t base)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "r"(512u) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t addr, const C (&v)[8])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(addr),
+                 "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y), "f"(v[2].x), "f"(v[2].y), "f"(v[3].x), "f"(v[3].y),
+                 "f"(v[4].x), "f"(v[4].y), "f"(v[5].x), "f"(v[5].y), "f"(v[6].x), "f"(v[6].y), "f"(v[7].x), "f"(v[7].y)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t addr, C (&v)[8])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y), "=f"(v[2].x), "=f"(v[2].y), "=f"(v[3].x), "=f"(v[3].y),
+                   "=f"(v[4].x), "=f"(v[4].y), "=f"(v[5].x), "=f"(v[5].y), "=f"(v[6].x), "=f"(v[6].y), "=f"(v[7].x), "=f"(v[7].y)
+                 : "r"(addr)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t addr, const C (&v)[16])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+                 "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(addr),
+                 "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y), "f"(v[2].x), "f"(v[2].y), "f"(v[3].x), "f"(v[3].y),
+                 "f"(v[4].x), "f"(v[4].y), "f"(v[5].x), "f"(v[5].y), "f"(v[6].x), "f"(v[6].y), "f"(v[7].x), "f"(v[7].y),
+                 "f"(v[8].x), "f"(v[8].y), "f"(v[9].x), "f"(v[9].y), "f"(v[10].x), "f"(v[10].y), "f"(v[11].x), "f"(v[11].y),
+                 "f"(v[12].x), "f"(v[12].y), "f"(v[13].x), "f"(v[13].y), "f"(v[14].x), "f"(v[14].y), "f"(v[15].x), "f"(v[15].y)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t addr, C (&v)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                 "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                 : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y), "=f"(v[2].x), "=f"(v[2].y), "=f"(v[3].x), "=f"(v[3].y),
+                   "=f"(v[4].x), "=f"(v[4].y), "=f"(v[5].x), "=f"(v[5].y), "=f"(v[6].x), "=f"(v[6].y), "=f"(v[7].x), "=f"(v[7].y),
+                   "=f"(v[8].x), "=f"(v[8].y), "=f"(v[9].x), "=f"(v[9].y), "=f"(v[10].x), "=f"(v[10].y), "=f"(v[11].x), "=f"(v[11].y),
+                   "=f"(v[12].x), "=f"(v[12].y), "=f"(v[13].x), "=f"(v[13].y), "=f"(v[14].x), "=f"(v[14].y), "=f"(v[15].x), "=f"(v[15].y)
+                 : "r"(addr)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// ------------------------------------------------------------------------------------ tiles
+// chunk of the tile-major Green's table that belongs to a tile (as green_tile_index of sf_fast.cuh)
+__device__ __forceinline__ int green_tile_index5(const Fast5Params& p, bool full, int b, int col)
+{
+    if (full) return (min(b, p.Pb - b) << p.nct_shift) + (col >> 4);
+    return ((p.Pb / 2 + 1) << p.nct_shift) + (b >> 4);
+}
+
+// MODE F5_FWD   : in rows n < 512 -> out rows k < 1024                       (S2; components are more batches)
+//      F5_INV   : in rows k < 1024 -> out rows j < 512                       (S4; likewise)
+//      F5_FUSED : in rows n < 512 -> x Green -> out rows j < 512, per component (S3 of sf_solve)
+//      F5_CURL  : three components in, u = curl psi out                      (S3 of sf_curl)
+// `tm` describes `in` as a rank-4 tensor; a tile image is fetched by two boxes of 256 rows:
+//   FWD            dims (column, row, batch, 1)          box {16, 256, 1, 1}   coordinates {col, 0 | 256, b, 0}
+//   FUSED / CURL   dims (column, batch, row, component)  box {16, 1, 256, 1}   coordinates {col, b, 0 | 256, c}
+// The Nyquist column (column nyq_col of every batch) is handled 16 batches at a time with gathered 8-byte accesses.
+template <int MODE>
+__global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, const __grid_constant__ CUtensorMap tm)
+{
+    constexpr bool kTma = (MODE != F5_INV);
+    constexpr bool kMul = (MODE == F5_FUSED || MODE == F5_CURL);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    C* xbuf = reinterpret_cast<C*>(smem_raw);
+    C* slot = xbuf + kXchg5Elems;
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ __align__(16) C s_tw512[32 * 16];        // [w][q] = w512^(q w)
+    __shared__ __align__(16) C s_tw1024[2 * 32 * 16];   // [h][w][r] = h ? w1024^(w + 32 r) : 1
+    __shared__ float s_kapp[MODE == F5_CURL ? 1024 : 1];
+    __shared__ int s_tile[2];
+    __shared__ uint32_t s_tmem;
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int pen = lane & 15;
+    const int h = lane >> 4;
+    const int w = (int)__reduce_max_sync(0xffffffffu, (unsigned)(tid >> 5));
+    const int q0 = w & 15, par = w >> 4;
+    C* xw = xbuf + (w * 32 + lane);                 // slot (q, w) at ((q * 32 + w) * 32 + lane)
+    const C* xr = xbuf + (q0 * 1024 + lane);        // slot (q0, o) at stride 32
+    const C* t512 = s_tw512 + w * 16;
+    const C* t1024 = s_tw1024 + (h * 32 + w) * 16;
+
+    const int ncomp_tiles = (MODE == F5_FUSED) ? p.ncomp : 1;     // FUSED: components are independent tile sets
+    const int nfull = p.nb << p.nct_shift;
+    const int nnyq = (p.nyq_col >= 0) ? (p.nb + kTile - 1) / kTile : 0;
+    const int ntile1 = nfull + nnyq;
+    const int ntiles = ntile1 * ncomp_tiles;
+    const int ips = (int)p.in_ps, ops = (int)p.out_ps, ibs = (int)p.in_bs, obs = (int)p.out_bs;
+    uint32_t parity = 0;
+
+    struct Geom { bool full; int b, col, comp; };
+    auto geom = [&](int t) {
+        Geom g;
+        g.comp = 0;
+        if (MODE == F5_FUSED) { g.comp = t / ntile1; t -= g.comp * ntile1; }
+        if (t < nnyq) {               // Nyquist-column tiles first: they are the slow ones
+            g.full = false;
+            g.b = t * kTile;
+            g.col = p.nyq_col;
+        } else {
+            const int tf = t - nnyq;
+            int bi = tf >> p.nct_shift;
+            if (p.reverse_batches) bi = p.nb - 1 - bi;
+            else if (p.pair_batches) {   // 0, P/2, 1, P-1, 2, P-2, ...: mirror batches share their Green's chunk
+                if (bi == 1) bi = p.nb / 2;
+                else if (bi > 1) bi = (bi & 1) ? p.nb - (bi >> 1) : (bi >> 1);
+            }
+            g.full = true;
+            g.b = bi;
+            g.col = (tf & (p.nct - 1)) * kTile;
+        }
+        return g;
+    };
+    // TMA load of (tile t, component c) into the slot: one thread, two boxes of 256 rows
+    auto issue = [&](int t, int c) {
+        if (!kTma || tid != 0 || t >= ntiles) return;
+        const Geom g = geom(t);
+        if (!g.full) return;
+        mbar_expect_tx(&bar, kSlot5Elems * (uint32_t)sizeof(C));
+        if (MODE == F5_FWD) {
+            tma_load_4d(slot, &tm, g.col, 0, g.b, 0, &bar);
+            tma_load_4d(slot + 256 * kTile, &tm, g.col, 256, g.b, 0, &bar);
+        } else {
+            const int cc = (MODE == F5_CURL) ? c : g.comp;
+            tma_load_4d(slot, &tm, g.col, g.b, 0, cc, &bar);
+            tma_load_4d(slot + 256 * kTile, &tm, g.col, g.b, 256, cc, &bar);
+        }
+    };
+    // v[r] = x[w + 32 r] of this thread's pencil (FWD / FUSED / CURL)
+    auto load_x = [&](const Geom& g, int c, C (&v)[16]) {
+        if (g.full) {
+            mbar_wait(&bar, parity);
+            parity ^= 1;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = slot[(w + 32 * r) * kTile + pen];
+        } else {
+            const C* inp = p.in + ((size_t)c * p.in_cs + (size_t)min(g.b + pen, p.nb - 1) * ibs + g.col + (size_t)w * ips);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = __ldg(inp + (size_t)r * 32 * ips);
+        }
+    };
+    // forward transform of this thread's half: v[r] = x[w + 32 r] in, X_h[w + 32 j] at v[brev4(j)] out.
+    // Leaves with the exchange buffer free to be rewritten only after the next barrier.
+    auto forward = [&](C (&v)[16], auto&& after_first_barrier) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], t1024[r]);
+        fft512_a<false>(v, t512, xw);
+        __syncthreads();
+        after_first_barrier();
+        fft512_b<false>(v, xr, par);
+    };
+    // backward transform (u natural order in: u[j] = U_h[w + 32 j]) and recombination of the halves:
+    // x_j = e_j + conj(w1024^j) o_j, j = w + 32 r.  Thread h = 0 ends with rows w + 32 r (r < 8) in out[r],
+    // thread h = 1 with rows w + 256 + 32 r.  Starts with a barrier (the exchange buffer may still be read).
+    auto backward = [&](C (&u)[16], C (&out)[8]) {
+        __syncthreads();
+        fft512_a<true>(u, t512, xw);
+        __syncthreads();
+        fft512_b<true>(u, xr, par);
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const C tl = cmulc(u[brev4(r)], t1024[r]), th = cmulc(u[brev4(r + 8)], t1024[r + 8]);
+            const C send = h ? tl : th;
+            const C keep = h ? th : tl;
+            C recv;
+            recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
+            recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+            out[r] = cadd(keep, recv);
+        }
+    };
+    // Green's factors of this thread's 16 spectral rows kp = 2 (w + 32 j) + h, folded to min(kp, 1024 - kp)
+    auto load_green = [&](const Geom& g, float (&gm)[16]) {
+        const float* gt = p.green_tiles + ((size_t)green_tile_index5(p, g.full, g.b, g.col) * (kGreenRows5 * kTile) + pen);
+        const float* glo = gt + (2 * w + h) * kTile;              // kp            (j < 8)
+        const float* ghi = gt + (2 * kL5 - 2 * w - h) * kTile;    // 1024 - kp     (j >= 8)
+#pragma unroll
+        for (int j = 0; j < 16; ++j) gm[j] = __ldg(j < 8 ? glo + j * 64 * kTile : ghi - j * 64 * kTile);
+    };
+
+    // ---------------------------------------------------------------- prologue
+    if (tid == 0) {
+        if (kTma) {
+            mbar_init(&bar, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        s_tile[0] = (int)blockIdx.x;
+        s_tile[1] = (int)(blockIdx.x + gridDim.x);
+        issue(s_tile[0], MODE == F5_CURL ? 2 : 0);
+    }
+    if (tid < 512) s_tw512[tid] = c_tw1024[(2 * (tid & 15) * (tid >> 4)) & 1023];
+    {
+        const int r = tid & 15, ww = (tid >> 4) & 31, hh = tid >> 9;
+        s_tw1024[tid] = hh ? c_tw1024[ww + 32 * r] : make_float2(1.f, 0.f);
+    }
+    if (MODE == F5_CURL) s_kapp[tid] = __ldg(p.kap_p + tid);
+    uint32_t tbase = 0;
+    if (MODE == F5_CURL) {
+        if (tid < 32) tmem_alloc512(&s_tmem);
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
+    __syncthreads();
+    if (MODE == F5_CURL) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        tbase = s_tmem + ((uint32_t)(w & 3) << 21);    // lane field (bits 16..31) = 32 (w mod 4)
+    }
+    const uint32_t t_spec = tbase + (uint32_t)(w >> 2) * 32;          // columns   0 .. 255: parked spectrum
+    const uint32_t t_p0 = tbase + 256 + (uint32_t)(w >> 2) * 16;      // columns 256 .. 383: t_z
+    const uint32_t t_p1 = tbase + 384 + (uint32_t)(w >> 2) * 16;      // columns 384 .. 511: t_y
+
+    // ---------------------------------------------------------------- tiles
+    for (int it = 0;; ++it) {
+        const int t = s_tile[it & 1];
+        if (t >= ntiles) break;
+        const Geom g = geom(t);
+        const bool pvalid = g.full || (g.b + pen < p.nb);
+        // after the first barrier of the tile every thread has its tile index (and the slot's first image):
+        // prefetch what comes next, claim the tile after next
+        auto advance = [&]() {
+            if (tid != 0) return;
+            if (MODE == F5_CURL) issue(t, 1);
+            else issue(s_tile[(it + 1) & 1], 0);
+            s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;
+        };
+        C v[16];
+        if constexpr (MODE == F5_FWD) {
+            load_x(g, 0, v);
+            forward(v, advance);
+            if (pvalid) {
+                C* q = p.out + ((size_t)(g.full ? g.b : g.b + pen) * obs + g.col + (g.full ? pen : 0) + (size_t)(2 * w + h) * ops);
+#pragma unroll
+                for (int j = 0; j < 16; ++j) q[(size_t)j * 64 * ops] = v[brev4(j)];    // row 2 (w + 32 j) + h
+            }
+            __syncthreads();   // the exchange buffer has been read by everyone
+        } else if constexpr (MODE == F5_INV) {
+            // rows 2 k + h, k = w + 32 j
+            const C* inp = p.in + ((size_t)(g.full ? g.b : min(g.b + pen, p.nb - 1)) * ibs + g.col + (g.full ? pen : 0) + (size_t)(2 * w + h) * ips);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = __ldg(inp + (size_t)j * 64 * ips);
+            if (tid == 0) s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;   // (this tile's index was read before the previous tile's last barrier)
+            C o8[8];
+            backward(v, o8);
+            if (pvalid) {
+                C* q = p.out + ((size_t)(g.full ? g.b : g.b + pen) * obs + g.col + (g.full ? pen : 0) + (size_t)(w + 256 * h) * ops);
+#pragma unroll
+                for (int r = 0; r < 8; ++r) q[(size_t)r * 32 * ops] = o8[r];
+            }
+        } else if constexpr (MODE == F5_FUSED) {
+            float gm[16];
+            load_green(g, gm);
+            load_x(g, g.comp, v);
+            forward(v, advance);
+            C u[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
+            C o8[8];
+            backward(u, o8);
+            if (pvalid) {
+                C* q = p.out + ((size_t)g.comp * p.out_cs + (size_t)(g.full ? g.b : g.b + pen) * obs + g.col + (g.full ? pen : 0) + (size_t)(w + 256 * h) * ops);
+#pragma unroll
+                for (int r = 0; r < 8; ++r) q[(size_t)r * 32 * ops] = o8[r];
+            }
+            __syncthreads();
+        } else {
+            // ---------------------------------------------------------------- curl
+            const int kx = g.full ? g.col + pen : g.col;
+            const int kb = g.full ? g.b : min(g.b + pen, p.nb - 1);
+            const float qx = __ldg(p.kap_x + kx), qy = __ldg(p.kap_b + kb);
+            C* obase = p.out + ((size_t)(g.full ? g.b : g.b + pen) * obs + g.col + (g.full ? pen : 0) + (size_t)(w + 256 * h) * ops);
+            const float* kz = s_kapp + (2 * w + h);    // kappa_z of spectral row 2 (w + 32 j) + h at kz[64 j]
+            auto store = [&](int c, const C (&o8)[8]) {
+                if (!pvalid) return;
+                C* q = obase + (size_t)c * p.out_cs;
+#pragma unroll
+                for (int r = 0; r < 8; ++r) q[(size_t)r * 32 * ops] = cmuli(o8[r]);   // the factor i of i kappa x psi
+            };
+            C u[16], o8[8], pk[8];
+            float gm[16];
+            // component z: t_z -> parked
+            load_green(g, gm);
+            load_x(g, 2, v);
+            forward(v, advance);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
+            backward(u, o8);
+            tmem_st16(t_p0, o8);
+            // components y, then x
+#pragma unroll 1
+            for (int c = 1; c >= 0; --c) {
+                load_green(g, gm);
+                load_x(g, c, v);
+                forward(v, [&]() {
+                    if (tid != 0) return;
+                    if (c == 1) issue(t, 0);
+                    else issue(s_tile[(it + 1) & 1], 2);
+                });
+#pragma unroll
+                for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
+                tmem_st32(t_spec, u);                       // psi_hat_c, natural order
+#pragma unroll
+                for (int j = 0; j < 16; ++j) u[j] = cscale(u[j], kz[64 * j]);
+                backward(u, o8);                            // d_c
+                tmem_wait_st();
+                tmem_ld16(t_p0, pk);                        // t_z
+                tmem_wait_ld();
+                if (c == 1) {
+                    // u_x = i (kappa_y t_z - d_y)
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) o8[r] = csub(cscale(pk[r], qy), o8[r]);
+                    store(0, o8);
+                } else {
+                    // u_y = i (d_x - kappa_x t_z)
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) o8[r] = csub(o8[r], cscale(pk[r], qx));
+                    store(1, o8);
+                }
+                tmem_ld32(t_spec, u);
+                tmem_wait_ld();
+                backward(u, o8);                            // t_c
+                if (c == 1) {
+                    tmem_st16(t_p1, o8);                    // t_y
+                } else {
+                    tmem_wait_st();
+                    tmem_ld16(t_p1, pk);
+                    tmem_wait_ld();
+                    // u_z = i (kappa_x t_y - kappa_y t_x)
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) o8[r] = csub(cscale(pk[r], qx), cscale(o8[r], qy));
+                    store(2, o8);
+                }
+            }
+            __syncthreads();
+        }
+    }
+    if (MODE == F5_CURL) {
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (tid < 32) tmem_free512(s_tmem);
+    }
+    // the last CTA to finish re-arms the counter for the next launch
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(p.sched + 1, 1) == (int)gridDim.x - 1) {
+            p.sched[0] = 0;
+            p.sched[1] = 0;
+            __threadfence();
+        }
+    }
+}
+
+} // namespace sf2
