@@ -82,6 +82,8 @@ struct sf_plan_s {
     bool fast = false;
     bool fast_x = false;   // S1 / S5 too (x extent 256)
     sf2::TileMap map_s2, map_s3, map_s4;
+    // ... and with 512-long y and z pencils (sf_fast512.cuh), scalar or three components (sf_solve, sf_curl)
+    bool fast5 = false;
 
     // per-solve state
     const void* src = nullptr;
@@ -578,6 +580,49 @@ template <typename T> sf_status run(sf_plan p, int outk)
         return SF_OK;
     }
 
+    if (p->fast5 && (outk == OUT_SOLVE || (outk == OUT_CURL && ncomp == 3))) {
+        // kernel generation 2 for 512-long pencils: S2, S3, S4 as persistent TMA-fed register-FFT kernels, one CTA per SM
+        sf2::Fast5Params fp;
+        memset(&fp, 0, sizeof(fp));
+        fp.sched = (int*)p->sched;
+        fp.nct = p->nspec_x / sf2::kTile;
+        for (fp.nct_shift = 0; (1 << fp.nct_shift) < fp.nct; ++fp.nct_shift) {}
+        fp.nyq_col = (p->nspec_x % sf2::kTile) ? fp.nct * sf2::kTile : -1;
+        fp.ncomp = ncomp;
+        // S2: W1 [c][z][y][hp] -> W2 [c][z][ky][hp]; the components are more batches
+        fp.in = (const sf2::C*)p->W1; fp.out = (sf2::C*)p->W2;
+        fp.in_ps = hp; fp.in_bs = hp * n1; fp.out_ps = hp; fp.out_bs = hp * P1; fp.nb = n2 * ncomp;
+        fp.reverse_batches = 1;   // S1 wrote the last planes last: start there while they are in L2
+        SF_CUDA(p, sf2::launch_fast5(sf2::F5_FWD, fp, p->map_s2, st));
+        fp.reverse_batches = 0;
+        p->launches++;
+        mark(2);
+        // S3: W2 in place along z
+        fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W2;
+        fp.in_ps = fp.out_ps = hp * P1; fp.in_bs = fp.out_bs = hp; fp.in_cs = fp.out_cs = p->w2_field; fp.nb = P1;
+        fp.pair_batches = 1;
+        fp.green_tiles = (const float*)p->green_tiles; fp.Pb = P1;
+        fp.kap_x = (const float*)p->kap[0]; fp.kap_b = (const float*)p->kap[1]; fp.kap_p = (const float*)p->kap[2];
+        SF_CUDA(p, sf2::launch_fast5(outk == OUT_CURL ? sf2::F5_CURL : sf2::F5_FUSED, fp, p->map_s3, st));
+        fp.pair_batches = 0;
+        p->launches++;
+        mark(3);
+        // S4: W2 [c][z][ky][hp] -> W1 [c][z][y][hp]
+        fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W1;
+        fp.in_ps = hp; fp.in_bs = hp * P1; fp.out_ps = hp; fp.out_bs = hp * n1; fp.in_cs = fp.out_cs = 0; fp.nb = n2 * ncomp;
+        SF_CUDA(p, sf2::launch_fast5(sf2::F5_INV, fp, p->map_s4, st));
+        p->launches++;
+        mark(4);
+        xp.spec_in = p->W1; xp.real_out = (T*)p->out;
+        SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        p->launches++;
+        mark(5);
+        if (timed) p->tcount++;
+        p->last_kind = outk;
+        p->out_last = p->out;
+        return SF_OK;
+    }
+
     if (p->fastper && (outk == OUT_SOLVE || outk == OUT_GRAD)) {
         // kernel generation 2, periodic: S2, S3, S4 in place on W1 as persistent register-FFT kernels
         sf2::FastPerParams fp;
@@ -892,6 +937,39 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
             if ((st = dev_alloc(p, &p->nyqA, (size_t)256 * 256 * 8)) != SF_OK) return bail(st, "");
             if ((st = dev_alloc(p, &p->nyqB, (size_t)256 * 512 * 8)) != SF_OK) return bail(st, "");
         }
+    }
+    // ... fp32 unbounded plans whose y and z pencils are 512 long (BASELINE.json configs[4]: three components, curl)
+    if (prec == SF_F32 && b == SF_BC_UNBOUNDED && ndim == 3 && p->n[1] == 512 && p->n[2] == 512 && (p->nspec_x % sf2::kTile) <= 1 &&
+        p->nspec_x >= sf2::kTile && is_pow2(p->nspec_x / sf2::kTile) && p->n[0] <= 1024 && !getenv("SF_DISABLE_FAST")) {
+        if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fp32 fast path failed"); }
+        const unsigned long long hpB = (unsigned long long)p->pitch * 8ull, N1 = 512, N2 = 512, PP = 1024;
+        const unsigned long long hpc = (unsigned long long)p->pitch;
+        cudaError_t e1, e2;
+        {
+            // S2: W1 as (column, y, batch = component * n2 + z)
+            const unsigned long long d[4] = { hpc, N1, N2 * (unsigned long long)ncomp, 1 }, sb[3] = { hpB, hpB * N1, hpB * N1 * N2 * ncomp };
+            const unsigned bx[4] = { 16, 256, 1, 1 };
+            e1 = sf2::fast_make_map(&p->map_s2, p->W1, d, sb, bx);
+        }
+        {
+            // S3: W2 as (column, ky, z, component)
+            const unsigned long long d[4] = { hpc, PP, N2, (unsigned long long)ncomp }, sb[3] = { hpB, hpB * PP, hpB * PP * N2 };
+            const unsigned bx[4] = { 16, 1, 256, 1 };
+            e2 = sf2::fast_make_map(&p->map_s3, p->W2, d, sb, bx);
+        }
+        p->map_s4 = p->map_s3;   // S4 loads straight into registers: no map of its own
+        if (e1 != cudaSuccess || e2 != cudaSuccess) return bail(SF_ERR_CUDA, "tensor map encoding failed");
+        {
+            const int nct = p->nspec_x / sf2::kTile, nyq = (p->nspec_x % sf2::kTile) ? nct * sf2::kTile : -1;
+            const size_t ne = sf2::fast_green_tiles_elems_rows(1024, nct, nyq, sf2::kGreenRows5);
+            if ((st = dev_alloc(p, &p->green_tiles, ne * sizeof(float))) != SF_OK) return bail(st, "");
+            if (sf2::fast_green_tiles_rows((float*)p->green_tiles, (const float*)p->green, p->pitch, p->pitch * (p->n[1] + 1), 1024, nct, nyq,
+                                           sf2::kGreenRows5, p->stream) != cudaSuccess)
+                return bail(SF_ERR_CUDA, "building the tile-major Green's table failed");
+        }
+        if ((st = dev_alloc(p, &p->sched, 2 * sizeof(int))) != SF_OK) return bail(st, "");
+        if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
+        p->fast5 = true;
     }
     // ... and periodic fp32 scalar plans with 256-point y and z pencils (strided passes only)
     if (prec == SF_F32 && b == SF_BC_PERIODIC && ndim == 3 && ncomp == 1 && p->n[1] == 256 && p->n[2] == 256 &&

@@ -2,6 +2,7 @@
 // shared-memory opt-in and the persistent-grid launchers.
 #include "sf_fast.cuh"
 #include "sf_fastper.cuh"
+#include "sf_fast512.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -67,6 +68,10 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FUSED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5NoSlot)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_CURL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres)) != cudaSuccess) return e;
@@ -96,12 +101,12 @@ cudaError_t fast_make_map(TileMap* out, const void* base, const unsigned long lo
 
 namespace {
 __global__ void green_tiles_kernel(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
-                                   long long total)
+                                   int rows, long long total)
 {
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
         const int pen = (int)(i % kTile);
-        const int fp = (int)((i / kTile) % kGreenRows);
-        const long long t = i / ((long long)kTile * kGreenRows);
+        const int fp = (int)((i / kTile) % rows);
+        const long long t = i / ((long long)kTile * rows);
         const long long nfull = (long long)(Pb / 2 + 1) * nct;
         int fb, kx;
         if (t < nfull) {
@@ -117,12 +122,17 @@ __global__ void green_tiles_kernel(float* tiles, const float* green, long long g
 }
 } // namespace
 
+cudaError_t fast_green_tiles_rows(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
+                                  int rows, cudaStream_t st)
+{
+    const long long total = (long long)fast_green_tiles_elems_rows(Pb, nct, nyq_col, rows);
+    green_tiles_kernel<<<148 * 8, 256, 0, st>>>(tiles, green, g_pb, g_pp, Pb, nct, nyq_col, rows, total);
+    return cudaGetLastError();
+}
 cudaError_t fast_green_tiles(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
                              cudaStream_t st)
 {
-    const long long total = (long long)fast_green_tiles_elems(Pb, nct, nyq_col);
-    green_tiles_kernel<<<148 * 8, 256, 0, st>>>(tiles, green, g_pb, g_pp, Pb, nct, nyq_col, total);
-    return cudaGetLastError();
+    return fast_green_tiles_rows(tiles, green, g_pb, g_pp, Pb, nct, nyq_col, kGreenRows, st);
 }
 
 cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map, cudaStream_t st)
@@ -140,6 +150,30 @@ cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map
     case FMODE_FWD: fast_pad_kernel<FMODE_FWD><<<grid, kThreads, FastCfg<FMODE_FWD>::kSmem, st>>>(p, tm); break;
     case FMODE_INV: fast_pad_kernel<FMODE_INV><<<grid, kThreads, FastCfg<FMODE_INV>::kSmem, st>>>(p, tm); break;
     case FMODE_FUSED: fast_pad_kernel<FMODE_FUSED><<<grid, kThreads, FastCfg<FMODE_FUSED>::kSmem, st>>>(p, tm); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fast5(int mode, const Fast5Params& p, const TileMap& in_map, cudaStream_t st)
+{
+    const CUtensorMap& tm = reinterpret_cast<const CUtensorMap&>(in_map);
+    if (p.nct <= 0 || (1 << p.nct_shift) != p.nct || p.nb <= 0) return cudaErrorInvalidValue;
+    // row, batch and column offsets are formed in 32 bits before they are widened
+    if ((long long)p.nb * p.in_bs + 1024 * p.in_ps >= (1ll << 31) || (long long)p.nb * p.out_bs + 1024 * p.out_ps >= (1ll << 31))
+        return cudaErrorInvalidValue;
+    if (mode == F5_CURL && (p.ncomp != 3 || !p.kap_x || !p.kap_b || !p.kap_p)) return cudaErrorInvalidValue;
+    if ((mode == F5_CURL || mode == F5_FUSED) && !p.green_tiles) return cudaErrorInvalidValue;
+    const long long ntiles = (long long)fast_ntiles(p.nb, p.nct, p.nyq_col) * (mode == F5_FUSED ? p.ncomp : 1);
+    if (ntiles + 4ll * g_sms >= (1ll << 31)) return cudaErrorInvalidValue;
+    int grid = g_sms;
+    if (grid > ntiles) grid = (int)ntiles;
+    if (grid <= 0) return cudaErrorInvalidValue;
+    switch (mode) {
+    case F5_FWD: fast5_kernel<F5_FWD><<<grid, kT5, kSmem5, st>>>(p, tm); break;
+    case F5_INV: fast5_kernel<F5_INV><<<grid, kT5, kSmem5NoSlot, st>>>(p, tm); break;
+    case F5_FUSED: fast5_kernel<F5_FUSED><<<grid, kT5, kSmem5, st>>>(p, tm); break;
+    case F5_CURL: fast5_kernel<F5_CURL><<<grid, kT5, kSmem5, st>>>(p, tm); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

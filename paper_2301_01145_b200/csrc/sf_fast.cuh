@@ -73,6 +73,8 @@ __device__ __forceinline__ C cmulc(C a, C w)
 }
 template <bool CONJ> __device__ __forceinline__ C cmul_sel(C a, C w) { return CONJ ? cmulc(a, w) : cmul(a, w); }
 __device__ __forceinline__ C cscale(C a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
+// a * s + b
+__device__ __forceinline__ C cfma(C a, float s, C b) { return __ffma2_rn(a, make_float2(s, s), b); }
 __device__ __forceinline__ C cmuli(C a) { return make_float2(-a.y, a.x); }
 __device__ __forceinline__ C cmulmi(C a) { return make_float2(a.y, -a.x); }
 

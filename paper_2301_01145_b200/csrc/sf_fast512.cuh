@@ -16,15 +16,15 @@
 // backward chain without reordering.  One CTA per SM (128 KB exchange buffer + 64 KB TMA slot).
 //
 // Vector plans: sf_curl needs psi_hat of all three components at every spectral point, 393 KB per tile --
-// more than the registers or the shared memory of an SM hold.  The curl is therefore assembled after the
-// backward transform, where truncation has halved the data: with t_c = IDFT_z(psi_hat_c) and
-// d_c = IDFT_z(kappa_z psi_hat_c),
-//     u_x = i (kappa_y t_z - d_y),   u_y = i (d_x - kappa_x t_z),   u_z = i (kappa_x t_y - kappa_y t_x)
-// (kappa_x per column, kappa_y per tile: constants of the backward transform), components processed z, y, x.
-// What has to wait for a later component -- t_z, t_y, and the spectrum of the component that is transformed
-// back twice -- is parked in TENSOR MEMORY (tcgen05.st / tcgen05.ld, 32 lanes x 32-bit columns per warp: each
-// thread parks and fetches its own registers, which is exactly the access TMEM gives a warp): 256 + 128 + 128
-// of the 512 columns.  Three forward and five backward transforms per tile, no extra HBM traffic.
+// more than the registers or the shared memory of an SM hold next to the exchange buffer.  The two spectra
+// that have to wait are parked in TENSOR MEMORY (tcgen05.st / tcgen05.ld, shape 32x32b: each thread parks and
+// fetches its own registers, which is exactly the access TMEM gives a warp; 2 x 32 of the 512 columns per
+// warp, 8 warps per lane quadrant = all 256 KB).  Components are transformed forward in the order z, y, x:
+//     psi_hat_z -> TMEM A;   psi_hat_y -> TMEM B,  u_hat_x = kappa_y A - kappa_z psi_hat_y -> backward -> u_x;
+//     psi_hat_x:  u_hat_z = kappa_x B - kappa_y psi_hat_x -> TMEM A (over psi_hat_z, chunk by chunk),
+//                 u_hat_y = kappa_z psi_hat_x - kappa_x A -> backward -> u_y;   TMEM A -> backward -> u_z
+// (the common factor i is applied at the store).  Three forward and three backward transforms per tile, every
+// component read once and every velocity component written once.
 #pragma once
 #include "sf_fast.cuh"
 
@@ -32,13 +32,11 @@ namespace sf2 {
 
 constexpr int kT5 = 1024;            // threads per CTA
 constexpr int kL5 = 512;             // transform length (stored rows per pencil)
-constexpr int kGreenRows5 = kL5 + 1; // folded spectral indices 0 .. 512
+static_assert(kGreenRows5 == kL5 + 1, "folded spectral indices 0 .. 512");
 constexpr int kXchg5Elems = 16 * 32 * 32;                 // 128 KB
 constexpr int kSlot5Elems = kL5 * kTile;                  // 64 KB
 constexpr size_t kSmem5 = ((size_t)kXchg5Elems + kSlot5Elems) * sizeof(C);
 constexpr size_t kSmem5NoSlot = (size_t)kXchg5Elems * sizeof(C);
-
-enum { F5_FWD = 0, F5_INV = 1, F5_FUSED = 2, F5_CURL = 3 };
 
 __host__ __device__ constexpr double cos32(int i)
 {
@@ -122,6 +120,19 @@ __device__ __forceinline__ void tmem_ld16(uint32_t addr, C (&v)[8])
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
                  : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y), "=f"(v[2].x), "=f"(v[2].y), "=f"(v[3].x), "=f"(v[3].y),
                    "=f"(v[4].x), "=f"(v[4].y), "=f"(v[5].x), "=f"(v[5].y), "=f"(v[6].x), "=f"(v[6].y), "=f"(v[7].x), "=f"(v[7].y)
+                 : "r"(addr)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t addr, const C (&v)[4])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(addr),
+                 "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y), "f"(v[2].x), "f"(v[2].y), "f"(v[3].x), "f"(v[3].y)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t addr, C (&v)[4])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y), "=f"(v[2].x), "=f"(v[2].y), "=f"(v[3].x), "=f"(v[3].y)
                  : "r"(addr)
                  : "memory");
 }
@@ -238,10 +249,13 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
         }
     };
     // v[r] = x[w + 32 r] of this thread's pencil (FWD / FUSED / CURL)
-    auto load_x = [&](const Geom& g, int c, C (&v)[16]) {
-        if (g.full) {
-            mbar_wait(&bar, parity);
-            parity ^= 1;
+    // (stashed: a Nyquist tile's elements were put into the slot by this very thread, see the curl)
+    auto load_x = [&](const Geom& g, int c, C (&v)[16], bool stashed = false) {
+        if (g.full || stashed) {
+            if (g.full) {
+                mbar_wait(&bar, parity);
+                parity ^= 1;
+            }
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = slot[(w + 32 * r) * kTile + pen];
         } else {
@@ -250,21 +264,25 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
             for (int r = 0; r < 16; ++r) v[r] = __ldg(inp + (size_t)r * 32 * ips);
         }
     };
+    // Every transform starts with a barrier: the exchange buffer may still be read by the previous one (and, at the
+    // start of a tile, every thread has read its tile index and its elements of the slot); `after_barrier` runs
+    // right behind it (prefetch of the next image into the slot, claim of the tile after next).
     // forward transform of this thread's half: v[r] = x[w + 32 r] in, X_h[w + 32 j] at v[brev4(j)] out.
-    // Leaves with the exchange buffer free to be rewritten only after the next barrier.
-    auto forward = [&](C (&v)[16], auto&& after_first_barrier) {
+    auto forward = [&](C (&v)[16], auto&& after_barrier) {
 #pragma unroll
         for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], t1024[r]);
+        __syncthreads();
+        after_barrier();
         fft512_a<false>(v, t512, xw);
         __syncthreads();
-        after_first_barrier();
         fft512_b<false>(v, xr, par);
     };
     // backward transform (u natural order in: u[j] = U_h[w + 32 j]) and recombination of the halves:
     // x_j = e_j + conj(w1024^j) o_j, j = w + 32 r.  Thread h = 0 ends with rows w + 32 r (r < 8) in out[r],
-    // thread h = 1 with rows w + 256 + 32 r.  Starts with a barrier (the exchange buffer may still be read).
-    auto backward = [&](C (&u)[16], C (&out)[8]) {
+    // thread h = 1 with rows w + 256 + 32 r.
+    auto backward = [&](C (&u)[16], C (&out)[8], auto&& after_barrier) {
         __syncthreads();
+        after_barrier();
         fft512_a<true>(u, t512, xw);
         __syncthreads();
         fft512_b<true>(u, xr, par);
@@ -279,6 +297,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
             out[r] = cadd(keep, recv);
         }
     };
+    auto nothing = []() {};
     // Green's factors of this thread's 16 spectral rows kp = 2 (w + 32 j) + h, folded to min(kp, 1024 - kp)
     auto load_green = [&](const Geom& g, float (&gm)[16]) {
         const float* gt = p.green_tiles + ((size_t)green_tile_index5(p, g.full, g.b, g.col) * (kGreenRows5 * kTile) + pen);
@@ -314,9 +333,9 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         tbase = s_tmem + ((uint32_t)(w & 3) << 21);    // lane field (bits 16..31) = 32 (w mod 4)
     }
-    const uint32_t t_spec = tbase + (uint32_t)(w >> 2) * 32;          // columns   0 .. 255: parked spectrum
-    const uint32_t t_p0 = tbase + 256 + (uint32_t)(w >> 2) * 16;      // columns 256 .. 383: t_z
-    const uint32_t t_p1 = tbase + 384 + (uint32_t)(w >> 2) * 16;      // columns 384 .. 511: t_y
+    const uint32_t t_A = tbase + (uint32_t)(w >> 2) * 64;   // this warp's 2 x 32 columns: 16 complex numbers per thread each
+    const uint32_t t_B = t_A + 32;
+    (void)t_A; (void)t_B;
 
     // ---------------------------------------------------------------- tiles
     for (int it = 0;; ++it) {
@@ -329,7 +348,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
         auto advance = [&]() {
             if (tid != 0) return;
             if (MODE == F5_CURL) issue(t, 1);
-            else issue(s_tile[(it + 1) & 1], 0);
+            else issue(s_tile[(it + 1) & 1], 0);   // (FUSED: the component is part of the tile index)
             s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;
         };
         C v[16];
@@ -341,15 +360,13 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
 #pragma unroll
                 for (int j = 0; j < 16; ++j) q[(size_t)j * 64 * ops] = v[brev4(j)];    // row 2 (w + 32 j) + h
             }
-            __syncthreads();   // the exchange buffer has been read by everyone
         } else if constexpr (MODE == F5_INV) {
             // rows 2 k + h, k = w + 32 j
             const C* inp = p.in + ((size_t)(g.full ? g.b : min(g.b + pen, p.nb - 1)) * ibs + g.col + (g.full ? pen : 0) + (size_t)(2 * w + h) * ips);
 #pragma unroll
             for (int j = 0; j < 16; ++j) v[j] = __ldg(inp + (size_t)j * 64 * ips);
-            if (tid == 0) s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;   // (this tile's index was read before the previous tile's last barrier)
             C o8[8];
-            backward(v, o8);
+            backward(v, o8, advance);
             if (pvalid) {
                 C* q = p.out + ((size_t)(g.full ? g.b : g.b + pen) * obs + g.col + (g.full ? pen : 0) + (size_t)(w + 256 * h) * ops);
 #pragma unroll
@@ -364,13 +381,12 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
 #pragma unroll
             for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
             C o8[8];
-            backward(u, o8);
+            backward(u, o8, nothing);
             if (pvalid) {
                 C* q = p.out + ((size_t)g.comp * p.out_cs + (size_t)(g.full ? g.b : g.b + pen) * obs + g.col + (g.full ? pen : 0) + (size_t)(w + 256 * h) * ops);
 #pragma unroll
                 for (int r = 0; r < 8; ++r) q[(size_t)r * 32 * ops] = o8[r];
             }
-            __syncthreads();
         } else {
             // ---------------------------------------------------------------- curl
             const int kx = g.full ? g.col + pen : g.col;
@@ -382,64 +398,84 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
                 if (!pvalid) return;
                 C* q = obase + (size_t)c * p.out_cs;
 #pragma unroll
-                for (int r = 0; r < 8; ++r) q[(size_t)r * 32 * ops] = cmuli(o8[r]);   // the factor i of i kappa x psi
+                for (int r = 0; r < 8; ++r) q[(size_t)r * 32 * ops] = cmuli(o8[r]);   // the factor i of i kappa x psi_hat
             };
-            C u[16], o8[8], pk[8];
-            float gm[16];
-            // component z: t_z -> parked
-            load_green(g, gm);
-            load_x(g, 2, v);
-            forward(v, advance);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
-            backward(u, o8);
-            tmem_st16(t_p0, o8);
-            // components y, then x
-#pragma unroll 1
-            for (int c = 1; c >= 0; --c) {
+            C u[16], o8[8];
+            {
+                // component z: psi_hat_z -> TMEM A
+                float gm[16];
                 load_green(g, gm);
-                load_x(g, c, v);
-                forward(v, [&]() {
-                    if (tid != 0) return;
-                    if (c == 1) issue(t, 0);
-                    else issue(s_tile[(it + 1) & 1], 2);
-                });
+                load_x(g, 2, v);
+                forward(v, advance);
 #pragma unroll
                 for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
-                tmem_st32(t_spec, u);                       // psi_hat_c, natural order
-#pragma unroll
-                for (int j = 0; j < 16; ++j) u[j] = cscale(u[j], kz[64 * j]);
-                backward(u, o8);                            // d_c
-                tmem_wait_st();
-                tmem_ld16(t_p0, pk);                        // t_z
-                tmem_wait_ld();
-                if (c == 1) {
-                    // u_x = i (kappa_y t_z - d_y)
-#pragma unroll
-                    for (int r = 0; r < 8; ++r) o8[r] = csub(cscale(pk[r], qy), o8[r]);
-                    store(0, o8);
-                } else {
-                    // u_y = i (d_x - kappa_x t_z)
-#pragma unroll
-                    for (int r = 0; r < 8; ++r) o8[r] = csub(o8[r], cscale(pk[r], qx));
-                    store(1, o8);
-                }
-                tmem_ld32(t_spec, u);
-                tmem_wait_ld();
-                backward(u, o8);                            // t_c
-                if (c == 1) {
-                    tmem_st16(t_p1, o8);                    // t_y
-                } else {
-                    tmem_wait_st();
-                    tmem_ld16(t_p1, pk);
-                    tmem_wait_ld();
-                    // u_z = i (kappa_x t_y - kappa_y t_x)
-#pragma unroll
-                    for (int r = 0; r < 8; ++r) o8[r] = csub(cscale(pk[r], qx), cscale(o8[r], qy));
-                    store(2, o8);
-                }
+                tmem_st32(t_A, u);
             }
-            __syncthreads();
+            {
+                // component y: psi_hat_y -> TMEM B;  u_hat_x = kappa_y psi_hat_z - kappa_z psi_hat_y
+                float gm[16];
+                load_green(g, gm);
+                load_x(g, 1, v);
+                forward(v, [&]() { if (tid == 0) issue(t, 0); });
+#pragma unroll
+                for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
+                tmem_st32(t_B, u);
+                tmem_wait_st();
+#pragma unroll
+                for (int c4 = 0; c4 < 4; ++c4) {
+                    C pa[4];
+                    tmem_ld8(t_A + 8 * c4, pa);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int j = 4 * c4 + i;
+                        u[j] = cfma(pa[i], qy, cscale(u[j], -kz[64 * j]));
+                    }
+                }
+                backward(u, o8, nothing);
+                // u_x goes where psi_x sits (the pass works in place): psi_x must have left global memory first.
+                // Full tiles: its TMA image has landed in the slot (the wait does not consume the phase); Nyquist
+                // tiles: every thread fetches its own elements now and keeps them in the (otherwise unused) slot.
+                if (g.full) {
+                    mbar_wait(&bar, parity);
+                } else {
+                    load_x(g, 0, u);
+#pragma unroll
+                    for (int r = 0; r < 16; ++r) slot[(w + 32 * r) * kTile + pen] = u[r];
+                }
+                store(0, o8);
+            }
+            {
+                // component x: u_hat_z = kappa_x psi_hat_y - kappa_y psi_hat_x -> TMEM A (over psi_hat_z);
+                //              u_hat_y = kappa_z psi_hat_x - kappa_x psi_hat_z
+                float gm[16];
+                load_green(g, gm);
+                load_x(g, 0, v, true);
+                forward(v, [&]() { if (tid == 0) issue(s_tile[(it + 1) & 1], 2); });
+#pragma unroll
+                for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
+#pragma unroll
+                for (int c4 = 0; c4 < 4; ++c4) {
+                    C pa[4], pb[4];
+                    tmem_ld8(t_A + 8 * c4, pa);
+                    tmem_ld8(t_B + 8 * c4, pb);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int j = 4 * c4 + i;
+                        pb[i] = cfma(pb[i], qx, cscale(u[j], -qy));
+                        u[j] = cfma(pa[i], -qx, cscale(u[j], kz[64 * j]));
+                    }
+                    tmem_st8(t_A + 8 * c4, pb);
+                }
+                backward(u, o8, nothing);
+                store(1, o8);
+                tmem_wait_st();
+                tmem_ld32(t_A, u);
+                tmem_wait_ld();
+                backward(u, o8, nothing);
+                store(2, o8);
+            }
         }
     }
     if (MODE == F5_CURL) {
@@ -456,6 +492,204 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
             __threadfence();
         }
     }
+}
+
+} // namespace sf2
+
+namespace sf2 {
+
+// ==================================================================================== X passes, rows of 512 reals
+// S1 (X forward) and S5 (X backward) for rows of 512 reals zero-padded to 1024 (PAPER.md:87 real transform / half
+// spectrum; PAPER.md:181 padding): fast_x_kernel of sf_fast.cuh one size up.  The padded real row is packed as
+// z[n] = x[2n] + i x[2n+1], n < 512, non-zero for n < 256; Z = DFT512(z) is two 256-point transforms, of z (even
+// outputs, h = 0) and of z w512^n (odd outputs, h = 1); then the real-transform split
+//     X[k] = ( (Z[k] + conj Z[512-k]) - i w1024^k (Z[k] - conj Z[512-k]) ) / 2,   k = 0..512
+// pairwise in place in the staged rows.  A CTA of 256 threads owns 8 contiguous rows (two CTAs per SM): a
+// half-warp = one residue o of the 256-point transform (radix 16 x 16, one exchange), its 16 lanes = 8 rows x 2
+// halves.  Rows arrive and leave by bulk copies (one per row), the next tile's rows while this one is transformed.
+constexpr int kX5Threads = 256;
+constexpr int kX5Rows = 8;
+constexpr int kX5N = 512;                  // stored reals per row
+constexpr int kX5InPitch = kX5N + 4;       // floats per staged real row: 2064 B = 16 (mod 128)
+constexpr int kX5SpPitch = kX5N + 2;       // complex per staged spectrum row: 4112 B = 16 (mod 128), multiple of 16
+constexpr int kX5XchgElems = 16 * 16 * 16;
+constexpr size_t kX5Smem = (size_t)kX5Rows * kX5InPitch * sizeof(float) + (size_t)kX5XchgElems * sizeof(C) + (size_t)kX5Rows * kX5SpPitch * sizeof(C);
+
+template <bool INV> __global__ void __launch_bounds__(kX5Threads, 2) fast_x5_kernel(const FastXParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* rbuf = reinterpret_cast<float*>(smem_raw);                                          // [8][kX5InPitch] reals
+    C* xbuf = reinterpret_cast<C*>(smem_raw + (size_t)kX5Rows * kX5InPitch * sizeof(float));   // exchange [16][16][16 lanes]
+    C* sbuf = xbuf + kX5XchgElems;                                                             // [8][kX5SpPitch] complex
+    __shared__ __align__(8) uint64_t bar;
+    // s_t256[o][q] = w256^(q o);  s_tin[o][r] = w512^(o + 16 r);  s_tsp[k] = w1024^k, k <= 256
+    __shared__ __align__(16) C s_t256[256];
+    __shared__ __align__(16) C s_tin[256];
+    __shared__ __align__(16) C s_tsp[264];
+
+    const int tid = threadIdx.x;
+    const int l16 = tid & 15;
+    const int row = l16 >> 1;
+    const int h = l16 & 1;
+    const int o = tid >> 4;
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (!INV && tid < kX5Rows) sbuf[tid * kX5SpPitch + kX5N + 1] = make_float2(0.f, 0.f);   // pad column 513 leaves as zero
+    s_t256[tid] = c_tw1024[(4 * (tid & 15) * (tid >> 4)) & 1023];
+    s_tin[tid] = c_tw1024[2 * ((tid >> 4) + 16 * (tid & 15))];
+    s_tsp[tid] = c_tw1024[tid];
+    if (tid < 8) s_tsp[256 + tid] = c_tw1024[256 + tid];
+    const C* t256 = s_t256 + o * 16;
+    const C* tin = s_tin + o * 16;
+    __syncthreads();
+
+    const int ntiles = p.nrows / kX5Rows;
+    const int nit = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    uint32_t parity = 0;
+    C* xw = xbuf + o * 16 + l16;           // slot (q, o) at stride 256
+    const C* xr = xbuf + o * 256 + l16;    // slot (o, o') at stride 16
+    C* srow = sbuf + row * kX5SpPitch;     // this thread's staged spectrum row
+    float* rrow = rbuf + row * kX5InPitch;
+    const int idx = 2 * o + h;             // the 32 threads of a row own the pairs (k, 512 - k), k = idx + 32 m
+
+    // bulk loads of iteration i: one row per lane of the first quarter-warp
+    auto issue = [&](int i) {
+        if (tid >= kX5Rows || i >= nit) return;
+        const long long tl = (long long)blockIdx.x + (long long)i * gridDim.x;
+        const long long r0 = (p.reverse ? ntiles - 1 - tl : tl) * kX5Rows + tid;
+        if (tid == 0) mbar_expect_tx(&bar, INV ? kX5Rows * kX5SpPitch * (uint32_t)sizeof(C) : kX5Rows * kX5N * (uint32_t)sizeof(float));
+        __syncwarp(0xffu);
+        if (INV) bulk_g2s(sbuf + tid * kX5SpPitch, p.spec + r0 * p.spec_pitch, kX5SpPitch * (uint32_t)sizeof(C), &bar);
+        else bulk_g2s(rbuf + tid * kX5InPitch, p.real_in + r0 * kX5N, kX5N * (uint32_t)sizeof(float), &bar);
+    };
+
+    issue(0);
+    for (int i = 0; i < nit; ++i) {
+        const long long tl0 = (long long)blockIdx.x + (long long)i * gridDim.x;
+        const long long row0 = (p.reverse ? ntiles - 1 - tl0 : tl0) * kX5Rows;
+        C v[16];
+        if constexpr (!INV) {
+            // ---------------------------------------------------------------- S1
+            mbar_wait(&bar, parity);
+            parity ^= 1;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const C z = *reinterpret_cast<const C*>(rrow + 2 * (o + 16 * r));
+                v[r] = h ? cmul(z, tin[r]) : z;                     // h = 1: z w512^n
+            }
+            dft16<false>(v);
+#pragma unroll
+            for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul(v[brev4(q)], t256[q]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) xw[q * 256] = v[brev4(q)];
+            if (tid < kX5Rows) bulk_wait_read();   // the previous tile's stores have left sbuf
+            __syncthreads();
+            issue(i + 1);                          // rbuf is in registers everywhere
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = xr[j * 16];
+            dft16<false>(v);
+            // Z[2 k' + h], k' = o + 16 k2, natural order into the staged row
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) srow[2 * (o + 16 * k2) + h] = v[brev4(k2)];
+            __syncthreads();
+            // split in place
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                C zk[5], zm[5];
+#pragma unroll
+                for (int mm = 0; mm < 5; ++mm) {
+                    const int m = 4 * half + mm;
+                    const int k = idx + 32 * m;
+                    if (mm < 4 || (half == 1 && idx == 0)) { zk[mm] = srow[k]; zm[mm] = srow[(kX5N - k) & (kX5N - 1)]; }
+                }
+#pragma unroll
+                for (int mm = 0; mm < 5; ++mm) {
+                    const int m = 4 * half + mm;
+                    const int k = idx + 32 * m;
+                    if (mm < 4 || (half == 1 && idx == 0)) {
+                        const C e = cadd(zk[mm], make_float2(zm[mm].x, -zm[mm].y));
+                        const C d = csub(zk[mm], make_float2(zm[mm].x, -zm[mm].y));
+                        const C wd = cmul(d, s_tsp[k]);   // w1024^k d
+                        // X[k] = (e - i wd) / 2,  X[512 - k] = (conj e - i conj wd) / 2
+                        srow[k] = cscale(cadd(e, make_float2(wd.y, -wd.x)), 0.5f);
+                        srow[kX5N - k] = cscale(make_float2(e.x - wd.y, -e.y - wd.x), 0.5f);
+                    }
+                }
+            }
+            fence_async_smem();
+            __syncthreads();
+            if (tid < kX5Rows) {
+                bulk_s2g(p.spec + (row0 + tid) * p.spec_pitch, sbuf + tid * kX5SpPitch, kX5SpPitch * (uint32_t)sizeof(C));
+                bulk_commit();
+            }
+        } else {
+            // ---------------------------------------------------------------- S5
+            mbar_wait(&bar, parity);
+            parity ^= 1;
+            // merge in place: Z[k] = e + i conj(w1024^k) d, Z[512 - k] = conj e + i conj(conj(w1024^k) d)
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                C xk[5], xm[5];
+#pragma unroll
+                for (int mm = 0; mm < 5; ++mm) {
+                    const int m = 4 * half + mm;
+                    const int k = idx + 32 * m;
+                    if (mm < 4 || (half == 1 && idx == 0)) { xk[mm] = srow[k]; xm[mm] = srow[kX5N - k]; }
+                }
+#pragma unroll
+                for (int mm = 0; mm < 5; ++mm) {
+                    const int m = 4 * half + mm;
+                    const int k = idx + 32 * m;
+                    if (mm < 4 || (half == 1 && idx == 0)) {
+                        const C e = cadd(xk[mm], make_float2(xm[mm].x, -xm[mm].y));
+                        const C d = csub(xk[mm], make_float2(xm[mm].x, -xm[mm].y));
+                        const C wd = cmulc(d, s_tsp[k]);   // conj(w1024^k) d
+                        srow[k] = cadd(e, make_float2(-wd.y, wd.x));
+                        if (k > 0) srow[kX5N - k] = make_float2(e.x + wd.y, wd.x - e.y);
+                    }
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = srow[2 * (o + 16 * j) + h];   // Z[2 k' + h], k' = o + 16 j
+            dft16<true>(v);
+#pragma unroll
+            for (int q = 1; q < 16; ++q) v[brev4(q)] = cmulc(v[brev4(q)], t256[q]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) xw[q * 256] = v[brev4(q)];
+            if (tid < kX5Rows) bulk_wait_read();   // the previous tile's stores have left rbuf
+            fence_async_smem();                    // the merged values in sbuf are overwritten by the next bulk load
+            __syncthreads();
+            issue(i + 1);                          // sbuf is in registers everywhere
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = xr[j * 16];
+            dft16<true>(v);
+            // z[n] = z0[n] + conj(w512^n) z1[n], n = o + 16 k2 < 256: h = 0 holds z0, h = 1 holds z1; the two lanes
+            // swap half of their values: h = 0 finishes k2 < 8, h = 1 finishes k2 >= 8
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                const C a = v[brev4(r)], b = v[brev4(r + 8)];
+                const C tl = h ? cmulc(a, tin[r]) : a, th = h ? cmulc(b, tin[r + 8]) : b;
+                const C send = h ? tl : th;
+                const C keep = h ? th : tl;
+                C recv;
+                recv.x = __shfl_xor_sync(0xffffffffu, send.x, 1);
+                recv.y = __shfl_xor_sync(0xffffffffu, send.y, 1);
+                const C z = cadd(keep, recv);
+                const int n = o + 16 * r + 128 * h;
+                *reinterpret_cast<C*>(rrow + 2 * n) = z;   // (x[2n], x[2n+1])
+            }
+            fence_async_smem();
+            __syncthreads();
+            if (tid < kX5Rows) {
+                bulk_s2g(p.real_out + (row0 + tid) * kX5N, rbuf + tid * kX5InPitch, kX5N * (uint32_t)sizeof(float));
+                bulk_commit();
+            }
+        }
+    }
+    if (tid < kX5Rows) bulk_wait_read();
 }
 
 } // namespace sf2

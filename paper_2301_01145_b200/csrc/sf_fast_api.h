@@ -12,6 +12,9 @@ constexpr int kGreenRows = 257;      // folded spectral indices along the pencil
 
 enum { FMODE_FWD = 0, FMODE_INV = 1, FMODE_FUSED = 2 };
 
+// opaque storage of a CUtensorMap (TMA descriptor): 128 bytes, 64-byte aligned
+struct alignas(64) TileMap { unsigned char bytes[128]; };
+
 struct FastParams {
     const C* in;
     C* out;
@@ -86,8 +89,37 @@ struct FastXPerParams {
     C* nyq;                 // side array [row] of X[128]
 };
 
-// opaque storage of a CUtensorMap (TMA descriptor): 128 bytes, 64-byte aligned
-struct alignas(64) TileMap { unsigned char bytes[128]; };
+// strided passes of fp32 unbounded plans with 512-point y / z pencils padded to 1024 (fast5_kernel, sf_fast512.cuh)
+constexpr int kGreenRows5 = 513;     // folded spectral indices along the pencil axis (0 .. 512)
+enum { F5_FWD = 0, F5_INV = 1, F5_FUSED = 2, F5_CURL = 3 };
+struct Fast5Params {
+    const C* in;
+    C* out;
+    long long in_ps, in_bs, in_cs;     // row (pencil-axis), batch and component strides, complex elements
+    long long out_ps, out_bs, out_cs;
+    int nb;                     // batches (FWD / INV: components are more batches)
+    int nct, nct_shift;         // full 16-column tiles per batch: a power of two
+    int nyq_col;                // column handled 16 batches at a time (the Nyquist column), -1: none
+    int ncomp;                  // FUSED: independent components (more tiles); CURL: 3
+    int reverse_batches;        // visit batches last to first
+    int pair_batches;           // visit batches as 0, P/2, 1, P-1, 2, P-2, ... (mirror pairs share the Green's chunk)
+    int* sched;                 // device: { next unclaimed tile, CTAs finished }, zero between launches
+    const float* green_tiles;   // tile-major real Green's table: chunk [kGreenRows5 fp][16 pencils] per tile
+    int Pb;                     // transform length along the batch axis (index folding k -> min(k, P - k))
+    // CURL: wavenumbers of the doubled grid (zero at the Nyquist index): per column, per batch, per pencil row (1024)
+    const float* kap_x; const float* kap_b; const float* kap_p;
+};
+// number of floats of the tile-major Green's table with `rows` folded pencil indices per chunk
+inline size_t fast_green_tiles_elems_rows(int Pb, int nct, int nyq_col, int rows)
+{
+    return ((size_t)(Pb / 2 + 1) * nct + (nyq_col >= 0 ? (size_t)(Pb + kTile - 1) / kTile : 0)) * rows * kTile;
+}
+cudaError_t fast_green_tiles_rows(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
+                                  int rows, cudaStream_t st);
+// launch one 512 -> 1024 padded pass (mode = F5_*) as a persistent grid of one 1024-thread CTA per SM; `in_map`
+// describes p.in as documented at fast5_kernel
+cudaError_t launch_fast5(int mode, const Fast5Params& p, const TileMap& in_map, cudaStream_t st);
+
 
 // one-time per-process set-up: twiddle constants, shared-memory opt-in, SM count, driver entry point
 cudaError_t fast_init();
