@@ -84,6 +84,7 @@ struct sf_plan_s {
     sf2::TileMap map_s2, map_s3, map_s4;
     // ... and with 512-long y and z pencils (sf_fast512.cuh), scalar or three components (sf_solve, sf_curl)
     bool fast5 = false;
+    bool fast5_x = false;  // S1 / S5 too (x extent 512)
 
     // per-solve state
     const void* src = nullptr;
@@ -497,11 +498,17 @@ template <typename T> sf_status run(sf_plan p, int outk)
     const bool fast_x = p->fast_x && outk == OUT_SOLVE && !xp.has_faces;
     sf2::FastXParams fx;
     memset(&fx, 0, sizeof(fx));
+    const bool fast5_x = p->fast5 && p->fast5_x && (outk == OUT_SOLVE || (outk == OUT_CURL && ncomp == 3));
     if (fast_x) {
         fx.real_in = (const float*)p->src; fx.real_out = (float*)p->out;
         fx.spec = (sf2::C*)p->W1; fx.spec_pitch = hp; fx.nrows = n1 * n2;
         fx.nyq = (sf2::C*)p->nyqA; fx.n1 = n1; fx.n2 = n2;
         SF_CUDA(p, sf2::launch_fast_x(false, fx, st));
+    } else if (fast5_x) {
+        // the components are contiguous in the source, the work array and the output: more rows
+        fx.real_in = (const float*)p->src; fx.real_out = (float*)p->out;
+        fx.spec = (sf2::C*)p->W1; fx.spec_pitch = hp; fx.nrows = n1 * n2 * ncomp;
+        SF_CUDA(p, sf2::launch_fast_x5(false, fx, st));
     } else if (p->fastper && p->fastper_x && (outk == OUT_SOLVE || outk == OUT_GRAD) && !xp.has_faces) {
         sf2::FastXPerParams px;
         memset(&px, 0, sizeof(px));
@@ -614,7 +621,12 @@ template <typename T> sf_status run(sf_plan p, int outk)
         p->launches++;
         mark(4);
         xp.spec_in = p->W1; xp.real_out = (T*)p->out;
-        SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        if (fast5_x) {
+            fx.reverse = 1;       // S4 wrote the last planes last
+            SF_CUDA(p, sf2::launch_fast_x5(true, fx, st));
+        } else {
+            SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        }
         p->launches++;
         mark(5);
         if (timed) p->tcount++;
@@ -970,6 +982,7 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         if ((st = dev_alloc(p, &p->sched, 2 * sizeof(int))) != SF_OK) return bail(st, "");
         if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
         p->fast5 = true;
+        p->fast5_x = (p->n[0] == 512) && p->pitch >= 514 && !getenv("SF_DISABLE_FAST_X");
     }
     // ... and periodic fp32 scalar plans with 256-point y and z pencils (strided passes only)
     if (prec == SF_F32 && b == SF_BC_PERIODIC && ndim == 3 && ncomp == 1 && p->n[1] == 256 && p->n[2] == 256 &&

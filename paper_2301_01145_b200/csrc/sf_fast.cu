@@ -72,6 +72,8 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5NoSlot)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_CURL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_x5_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_x5_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres)) != cudaSuccess) return e;
@@ -213,6 +215,16 @@ cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st)
     if (grid > p.nrows / kXpRows) grid = p.nrows / kXpRows;
     if (inv) fast_xper_kernel<true><<<grid, kXpThreads, kXpSmem, st>>>(p);
     else fast_xper_kernel<false><<<grid, kXpThreads, kXpSmem, st>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st)
+{
+    if (p.nrows <= 0 || p.nrows % kX5Rows || p.spec_pitch < kX5SpPitch || p.nyq) return cudaErrorInvalidValue;
+    int grid = 2 * g_sms;
+    if (grid > p.nrows / kX5Rows) grid = p.nrows / kX5Rows;
+    if (inv) fast_x5_kernel<true><<<grid, kX5Threads, kX5Smem, st>>>(p);
+    else fast_x5_kernel<false><<<grid, kX5Threads, kX5Smem, st>>>(p);
     return cudaGetLastError();
 }
 

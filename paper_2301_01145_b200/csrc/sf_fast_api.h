@@ -141,6 +141,9 @@ cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map
 
 // launch S1 (inv = false) or S5 (inv = true) as a persistent grid of two CTAs per SM
 cudaError_t launch_fast_x(bool inv, const FastXParams& p, cudaStream_t st);
+// the same for rows of 512 reals padded to 1024 (fast_x5_kernel; spec_pitch >= 514, no side array: p.nyq must be NULL;
+// nrows a multiple of 8)
+cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st);
 // launch one periodic strided pass (mode = FMODE_*) as a persistent grid of two CTAs per SM
 cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st);
 cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st);
