@@ -36,6 +36,14 @@ cudaError_t fast_init()
     }
     if ((e = cudaMemcpyToSymbol(c_tw1024, tw.data(), sizeof(float2) * 1024)) != cudaSuccess) return e;
     {
+        std::vector<float2> tm(1024);
+        for (int j = 0; j < 1024; ++j) {
+            const long double a = 2.0L * pi * (long double)j / 1024.0L;
+            tm[j] = make_float2((float)(cosl(a) - 1.0L), (float)(-sinl(a)));
+        }
+        if ((e = cudaMemcpyToSymbol(c_tw1024m1, tm.data(), sizeof(float2) * 1024)) != cudaSuccess) return e;
+    }
+    {
         std::vector<float2> tp(768), tx(544, make_float2(0.f, 0.f));
         for (int a = 0; a < 16; ++a)
             for (int b = 0; b < 16; ++b) {
@@ -164,7 +172,7 @@ cudaError_t launch_fast5(int mode, const Fast5Params& p, const TileMap& in_map, 
     // row, batch and column offsets are formed in 32 bits before they are widened
     if ((long long)p.nb * p.in_bs + 1024 * p.in_ps >= (1ll << 31) || (long long)p.nb * p.out_bs + 1024 * p.out_ps >= (1ll << 31))
         return cudaErrorInvalidValue;
-    if (mode == F5_CURL && (p.ncomp != 3 || !p.kap_x || !p.kap_b || !p.kap_p)) return cudaErrorInvalidValue;
+    if (mode == F5_CURL && (p.ncomp != 3 || !p.kap_x || !p.kap_b || !p.kap_p || 3 * p.out_cs >= (1ll << 31))) return cudaErrorInvalidValue;
     if ((mode == F5_CURL || mode == F5_FUSED) && !p.green_tiles) return cudaErrorInvalidValue;
     const long long ntiles = (long long)fast_ntiles(p.nb, p.nct, p.nyq_col) * (mode == F5_FUSED ? p.ncomp : 1);
     if (ntiles + 4ll * g_sms >= (1ll << 31)) return cudaErrorInvalidValue;

@@ -47,6 +47,8 @@ constexpr int kTileElems = kL * kTile;
 
 // exp(-2 pi i j / 1024), j < 1024 (this header is compiled into one translation unit: sf_fast.cu)
 __constant__ float2 c_tw1024[1024];
+// (Re - 1, Im) of the same: 1 + h (w - 1) selects between w and one with one packed multiply-add
+__constant__ float2 c_tw1024m1[1024];
 // the per-kernel twiddle tables, laid out as the kernels keep them in shared memory (filled once by
 // fast_init; a CTA copies them with coalesced 16-byte loads):
 //   strided passes: [0, 256) tw256[o][q] = w256^(q o); [256, 768) tw512[h][o][r] = h ? w512^(o + 16 r) : 1

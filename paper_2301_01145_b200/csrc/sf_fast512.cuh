@@ -63,11 +63,11 @@ template <int I32, bool INV> __device__ __forceinline__ C mul_w32(C d)
 }
 
 // first half: radix-16 over r, twiddle w512^(q w) (row w of a shared-memory table), write slots (q, w)
-template <bool INV> __device__ __forceinline__ void fft512_a(C (&v)[16], const C* tw, C* xw)
+template <bool INV, typename TW> __device__ __forceinline__ void fft512_a(C (&v)[16], TW&& tw, C* xw)
 {
     dft16<INV>(v);
 #pragma unroll
-    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], tw[q]);
+    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], tw(q));
 #pragma unroll
     for (int q = 0; q < 16; ++q) xw[q * 1024] = v[brev4(q)];
 }
@@ -136,6 +136,14 @@ __device__ __forceinline__ void tmem_ld8(uint32_t addr, C (&v)[4])
                  : "r"(addr)
                  : "memory");
 }
+__device__ __forceinline__ void tmem_st4(uint32_t addr, const C (&v)[2])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y) : "memory");
+}
+__device__ __forceinline__ void tmem_ld4(uint32_t addr, C (&v)[2])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y) : "r"(addr) : "memory");
+}
 __device__ __forceinline__ void tmem_st32(uint32_t addr, const C (&v)[16])
 {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
@@ -185,9 +193,19 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
     C* xbuf = reinterpret_cast<C*>(smem_raw);
     C* slot = xbuf + kXchg5Elems;
     __shared__ __align__(8) uint64_t bar;
-    __shared__ __align__(16) C s_tw512[32 * 16];        // [w][q] = w512^(q w)
-    __shared__ __align__(16) C s_tw1024[2 * 32 * 16];   // [h][w][r] = h ? w1024^(w + 32 r) : 1
+    // Twiddle factors: w512^(q w) between the two halves of a transform and w1024^(w + 32 r) of the odd half
+    // (h = 1; the even half multiplies by one).  Both are warp-uniform and live in shared-memory tables (base
+    // register + immediate).  (kTwc: from the constant bank instead -- tried for CURL to get under the 196 KB
+    // shared-memory carve-out; the constants then occupy registers and the kernel spills 416 bytes per thread.)
+    constexpr bool kTwc = false;
     __shared__ float s_kapp[MODE == F5_CURL ? 1024 : 1];
+    // CURL: per-thread values of the current tile that are needed between the transforms only (kappa_x, kappa_y,
+    // output offset): parked here, because the 64 registers of a 1024-thread CTA cannot hold them across the
+    // transforms and a spill to local memory misses the (28 KB) L1
+    __shared__ float s_qx[MODE == F5_CURL ? kT5 : 1], s_qy[MODE == F5_CURL ? kT5 : 1];
+    __shared__ unsigned s_oo[MODE == F5_CURL ? kT5 : 1];
+    __shared__ __align__(16) C s_tw512[kTwc ? 1 : 32 * 16];        // [w][q] = w512^(q w)
+    __shared__ __align__(16) C s_tw1024[kTwc ? 1 : 2 * 32 * 16];   // [h][w][r] = h ? w1024^(w + 32 r) : 1
     __shared__ int s_tile[2];
     __shared__ uint32_t s_tmem;
 
@@ -201,6 +219,14 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
     const C* xr = xbuf + (q0 * 1024 + lane);        // slot (q0, o) at stride 32
     const C* t512 = s_tw512 + w * 16;
     const C* t1024 = s_tw1024 + (h * 32 + w) * 16;
+    const float hf = (float)h;
+    auto tw512 = [&](int q) -> C { return kTwc ? c_tw1024[(2 * q * w) & 1023] : t512[q]; };
+    // 1 + h (w1024^(w + 32 r) - 1): one packed multiply-add on the table of (Re w - 1, Im w)
+    auto tw1024 = [&](int r) -> C {
+        if (!kTwc) return t1024[r];
+        const C m = c_tw1024m1[w + 32 * r];
+        return __ffma2_rn(make_float2(hf, hf), m, make_float2(1.f, 0.f));
+    };
 
     const int ncomp_tiles = (MODE == F5_FUSED) ? p.ncomp : 1;     // FUSED: components are independent tile sets
     const int nfull = p.nb << p.nct_shift;
@@ -270,10 +296,10 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
     // forward transform of this thread's half: v[r] = x[w + 32 r] in, X_h[w + 32 j] at v[brev4(j)] out.
     auto forward = [&](C (&v)[16], auto&& after_barrier) {
 #pragma unroll
-        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], t1024[r]);
+        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], tw1024(r));
         __syncthreads();
         after_barrier();
-        fft512_a<false>(v, t512, xw);
+        fft512_a<false>(v, tw512, xw);
         __syncthreads();
         fft512_b<false>(v, xr, par);
     };
@@ -283,12 +309,12 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
     auto backward = [&](C (&u)[16], C (&out)[8], auto&& after_barrier) {
         __syncthreads();
         after_barrier();
-        fft512_a<true>(u, t512, xw);
+        fft512_a<true>(u, tw512, xw);
         __syncthreads();
         fft512_b<true>(u, xr, par);
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
-            const C tl = cmulc(u[brev4(r)], t1024[r]), th = cmulc(u[brev4(r + 8)], t1024[r + 8]);
+            const C tl = cmulc(u[brev4(r)], tw1024(r)), th = cmulc(u[brev4(r + 8)], tw1024(r + 8));
             const C send = h ? tl : th;
             const C keep = h ? th : tl;
             C recv;
@@ -298,13 +324,13 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
         }
     };
     auto nothing = []() {};
-    // Green's factors of this thread's 16 spectral rows kp = 2 (w + 32 j) + h, folded to min(kp, 1024 - kp)
-    auto load_green = [&](const Geom& g, float (&gm)[16]) {
-        const float* gt = p.green_tiles + ((size_t)green_tile_index5(p, g.full, g.b, g.col) * (kGreenRows5 * kTile) + pen);
-        const float* glo = gt + (2 * w + h) * kTile;              // kp            (j < 8)
-        const float* ghi = gt + (2 * kL5 - 2 * w - h) * kTile;    // 1024 - kp     (j >= 8)
+    // u[j] = G X_h[w + 32 j]: Green's factors of this thread's 16 spectral rows kp = 2 (w + 32 j) + h, folded to
+    // min(kp, 1024 - kp), fetched when they are used (the registers cannot hold them across the transform)
+    auto mul_green = [&](const Geom& g, const C (&v)[16], C (&u)[16]) {
+        const float* glo = p.green_tiles + ((size_t)green_tile_index5(p, g.full, g.b, g.col) * (kGreenRows5 * kTile) + pen + (2 * w + h) * kTile);
+        const float* ghi = glo + (2 * kL5 - 4 * w - 2 * h) * kTile;   // 1024 - kp     (j >= 8)
 #pragma unroll
-        for (int j = 0; j < 16; ++j) gm[j] = __ldg(j < 8 ? glo + j * 64 * kTile : ghi - j * 64 * kTile);
+        for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], __ldg(j < 8 ? glo + j * 64 * kTile : ghi - j * 64 * kTile));
     };
 
     // ---------------------------------------------------------------- prologue
@@ -317,12 +343,12 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
         s_tile[1] = (int)(blockIdx.x + gridDim.x);
         issue(s_tile[0], MODE == F5_CURL ? 2 : 0);
     }
-    if (tid < 512) s_tw512[tid] = c_tw1024[(2 * (tid & 15) * (tid >> 4)) & 1023];
-    {
+    if (MODE == F5_CURL) s_kapp[tid] = __ldg(p.kap_p + tid);
+    if (!kTwc) {
+        if (tid < 512) s_tw512[tid] = c_tw1024[(2 * (tid & 15) * (tid >> 4)) & 1023];
         const int r = tid & 15, ww = (tid >> 4) & 31, hh = tid >> 9;
         s_tw1024[tid] = hh ? c_tw1024[ww + 32 * r] : make_float2(1.f, 0.f);
     }
-    if (MODE == F5_CURL) s_kapp[tid] = __ldg(p.kap_p + tid);
     uint32_t tbase = 0;
     if (MODE == F5_CURL) {
         if (tid < 32) tmem_alloc512(&s_tmem);
@@ -339,7 +365,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
 
     // ---------------------------------------------------------------- tiles
     for (int it = 0;; ++it) {
-        const int t = s_tile[it & 1];
+        const int t = (int)__reduce_max_sync(0xffffffffu, (unsigned)s_tile[it & 1]);   // warp-uniform: tile geometry in uniform registers
         if (t >= ntiles) break;
         const Geom g = geom(t);
         const bool pvalid = g.full || (g.b + pen < p.nb);
@@ -373,13 +399,10 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
                 for (int r = 0; r < 8; ++r) q[(size_t)r * 32 * ops] = o8[r];
             }
         } else if constexpr (MODE == F5_FUSED) {
-            float gm[16];
-            load_green(g, gm);
             load_x(g, g.comp, v);
             forward(v, advance);
             C u[16];
-#pragma unroll
-            for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
+            mul_green(g, v, u);
             C o8[8];
             backward(u, o8, nothing);
             if (pvalid) {
@@ -389,38 +412,40 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
             }
         } else {
             // ---------------------------------------------------------------- curl
-            const int kx = g.full ? g.col + pen : g.col;
-            const int kb = g.full ? g.b : min(g.b + pen, p.nb - 1);
-            const float qx = __ldg(p.kap_x + kx), qy = __ldg(p.kap_b + kb);
-            C* obase = p.out + ((size_t)(g.full ? g.b : g.b + pen) * obs + g.col + (g.full ? pen : 0) + (size_t)(w + 256 * h) * ops);
+            // (two copies of the tile body: the full tiles' one carries no per-lane geometry)
+            auto curl_tile = [&](auto full_tag) {
+            constexpr bool FULL = decltype(full_tag)::value;
+            Geom gg = g;
+            gg.full = FULL;
+            const int kx = FULL ? g.col + pen : g.col;
+            const int kb = FULL ? g.b : min(g.b + pen, p.nb - 1);
+            s_qx[tid] = __ldg(p.kap_x + kx);
+            s_qy[tid] = __ldg(p.kap_b + kb);
+            // element offsets of the outputs fit 32 bits (checked by the launcher)
+            s_oo[tid] = (unsigned)((FULL ? g.b : g.b + pen) * obs + g.col + (FULL ? pen : 0) + (w + 256 * h) * ops);
             const float* kz = s_kapp + (2 * w + h);    // kappa_z of spectral row 2 (w + 32 j) + h at kz[64 j]
             auto store = [&](int c, const C (&o8)[8]) {
-                if (!pvalid) return;
-                C* q = obase + (size_t)c * p.out_cs;
+                if (!FULL && !pvalid) return;
+                C* q = p.out + (s_oo[tid] + (unsigned)c * (unsigned)p.out_cs);
 #pragma unroll
                 for (int r = 0; r < 8; ++r) q[(size_t)r * 32 * ops] = cmuli(o8[r]);   // the factor i of i kappa x psi_hat
             };
             C u[16], o8[8];
             {
                 // component z: psi_hat_z -> TMEM A
-                float gm[16];
-                load_green(g, gm);
-                load_x(g, 2, v);
+                load_x(gg, 2, v);
                 forward(v, advance);
-#pragma unroll
-                for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
+                mul_green(gg, v, u);
                 tmem_st32(t_A, u);
             }
             {
                 // component y: psi_hat_y -> TMEM B;  u_hat_x = kappa_y psi_hat_z - kappa_z psi_hat_y
-                float gm[16];
-                load_green(g, gm);
-                load_x(g, 1, v);
+                load_x(gg, 1, v);
                 forward(v, [&]() { if (tid == 0) issue(t, 0); });
-#pragma unroll
-                for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
+                mul_green(gg, v, u);
                 tmem_st32(t_B, u);
                 tmem_wait_st();
+                const float qy = s_qy[tid];
 #pragma unroll
                 for (int c4 = 0; c4 < 4; ++c4) {
                     C pa[4];
@@ -436,10 +461,10 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
                 // u_x goes where psi_x sits (the pass works in place): psi_x must have left global memory first.
                 // Full tiles: its TMA image has landed in the slot (the wait does not consume the phase); Nyquist
                 // tiles: every thread fetches its own elements now and keeps them in the (otherwise unused) slot.
-                if (g.full) {
+                if (FULL) {
                     mbar_wait(&bar, parity);
                 } else {
-                    load_x(g, 0, u);
+                    load_x(gg, 0, u);
 #pragma unroll
                     for (int r = 0; r < 16; ++r) slot[(w + 32 * r) * kTile + pen] = u[r];
                 }
@@ -448,25 +473,23 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
             {
                 // component x: u_hat_z = kappa_x psi_hat_y - kappa_y psi_hat_x -> TMEM A (over psi_hat_z);
                 //              u_hat_y = kappa_z psi_hat_x - kappa_x psi_hat_z
-                float gm[16];
-                load_green(g, gm);
-                load_x(g, 0, v, true);
+                load_x(gg, 0, v, true);
                 forward(v, [&]() { if (tid == 0) issue(s_tile[(it + 1) & 1], 2); });
+                mul_green(gg, v, u);
+                const float qx = s_qx[tid], qy = s_qy[tid];
 #pragma unroll
-                for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], gm[j]);
-#pragma unroll
-                for (int c4 = 0; c4 < 4; ++c4) {
-                    C pa[4], pb[4];
-                    tmem_ld8(t_A + 8 * c4, pa);
-                    tmem_ld8(t_B + 8 * c4, pb);
+                for (int c2 = 0; c2 < 8; ++c2) {
+                    C pa[2], pb[2];
+                    tmem_ld4(t_A + 4 * c2, pa);
+                    tmem_ld4(t_B + 4 * c2, pb);
                     tmem_wait_ld();
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int j = 4 * c4 + i;
+                    for (int i = 0; i < 2; ++i) {
+                        const int j = 2 * c2 + i;
                         pb[i] = cfma(pb[i], qx, cscale(u[j], -qy));
                         u[j] = cfma(pa[i], -qx, cscale(u[j], kz[64 * j]));
                     }
-                    tmem_st8(t_A + 8 * c4, pb);
+                    tmem_st4(t_A + 4 * c2, pb);
                 }
                 backward(u, o8, nothing);
                 store(1, o8);
@@ -476,6 +499,9 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
                 backward(u, o8, nothing);
                 store(2, o8);
             }
+            };
+            if (g.full) curl_tile(std::true_type());
+            else curl_tile(std::false_type());
         }
     }
     if (MODE == F5_CURL) {
