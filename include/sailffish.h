@@ -202,8 +202,34 @@ sf_status sf_get_output(sf_plan plan, int field, int comp, void* dst, sf_mem whe
  * sf_plan_destroy); *ptr receives a device pointer.  Same errors as sf_get_output. */
 sf_status sf_output_device_ptr(sf_plan plan, int field, int comp, void** ptr);
 
-/* Block until every operation enqueued by this plan has completed. */
+/* Block until every operation enqueued by this plan has completed (the plan's stream and, with a copy
+ * pipeline, its two copy streams). */
 sf_status sf_synchronize(sf_plan plan);
+
+/*
+ * Copy pipeline for callers whose source and result live in HOST memory (the paper's Set_Input / Get_Output
+ * around every solve).  depth = 2 gives the plan a second source and a second result buffer
+ * and two copy streams of its own, ordered against the plan's stream by events, so that the same call sequence
+ *     sf_set_source(HOST) ; sf_solve ; sf_get_output_async     (repeated)
+ * overlaps the upload of step k+1, the compute of step k and the download of step k-1 (PCIe is full duplex).
+ * depth = 1 (the default) is the single-stream behaviour.  The call drains the plan first.  With depth = 2:
+ *   sf_set_source(HOST)   enqueues the copy on the upload stream and returns; the host buffer may be reused after
+ *                         sf_synchronize (pinned) or at once (pageable: the runtime stages it).
+ *   compute calls         wait for that copy, alternate between the two result buffers, and wait for the download
+ *                         that still reads the buffer they are about to overwrite.
+ *   sf_output_device_ptr  the borrowed pointer stays valid until the compute call AFTER the next one.
+ * Errors: INVALID_ARG (depth), ALLOC (the second buffers).
+ */
+sf_status sf_set_pipeline(sf_plan plan, int depth);
+
+/* sf_get_output to HOST memory without blocking: the copy is enqueued (on the download stream of a depth-2
+ * pipeline, else on the plan's stream) and dst is valid after sf_synchronize.  dst should be pinned memory for the
+ * copy to overlap.  Same errors as sf_get_output. */
+sf_status sf_get_output_async(sf_plan plan, int field, int comp, void* dst_host);
+
+/* Make the plan's stream wait for every copy the pipeline has enqueued so far (an event recorded on the plan's
+ * stream after this call completes after them): for callers that time or order work on that stream. */
+sf_status sf_pipeline_join(sf_plan plan);
 
 /* Number of kernels the last compute call launched (for launch accounting in benchmarks). */
 int sf_last_launch_count(sf_plan plan);

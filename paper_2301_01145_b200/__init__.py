@@ -29,7 +29,8 @@ SF_OUT_PSI, SF_OUT_GRAD, SF_OUT_CURL, SF_OUT_DIV, SF_OUT_LAP = 0, 1, 2, 3, 4
 # every symbol include/sailffish.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = (
     "sf_plan_create", "sf_set_source", "sf_set_bc_values", "sf_solve", "sf_gradient", "sf_curl",
-    "sf_divergence", "sf_laplacian", "sf_get_output", "sf_output_device_ptr", "sf_synchronize", "sf_last_launch_count", "sf_device_bytes",
+    "sf_divergence", "sf_laplacian", "sf_get_output", "sf_output_device_ptr", "sf_synchronize",
+    "sf_set_pipeline", "sf_get_output_async", "sf_pipeline_join", "sf_last_launch_count", "sf_device_bytes",
     "sf_enable_step_timing", "sf_step_times_ms", "sf_set_step_timing_stride", "sf_last_error", "sf_plan_destroy", "sf_version",
 )
 
@@ -68,6 +69,9 @@ def lib() -> C.CDLL:
         L.sf_get_output.argtypes = [vp, i, i, vp, i]
         L.sf_output_device_ptr.argtypes = [vp, i, i, C.POINTER(vp)]
         L.sf_synchronize.argtypes = [vp]
+        L.sf_set_pipeline.argtypes = [vp, i]
+        L.sf_get_output_async.argtypes = [vp, i, i, vp]
+        L.sf_pipeline_join.argtypes = [vp]
         L.sf_last_launch_count.argtypes = [vp]
         L.sf_device_bytes.argtypes = [vp]
         L.sf_device_bytes.restype = ll
@@ -170,6 +174,21 @@ def sf_output_device_ptr(plan, field, comp) -> int:
 
 def sf_synchronize(plan):
     _check(plan, lib().sf_synchronize(plan))
+
+
+def sf_set_pipeline(plan, depth=2):
+    _check(plan, lib().sf_set_pipeline(plan, int(depth)))
+
+
+def sf_get_output_async(plan, field, comp, dst):
+    a, where = _addr(dst)
+    if where != SF_MEM_HOST:
+        raise ValueError("sf_get_output_async copies to host memory")
+    _check(plan, lib().sf_get_output_async(plan, int(field), int(comp), a))
+
+
+def sf_pipeline_join(plan):
+    _check(plan, lib().sf_pipeline_join(plan))
 
 
 def sf_last_launch_count(plan) -> int:

@@ -100,6 +100,16 @@ struct sf_plan_s {
     bool fastper_x = false;       // ... and rows of 256 reals: generation-2 X passes
     long long tcalls = 0;         // compute calls seen since timing was enabled
     std::vector<cudaEvent_t> ev;  // 6 events per slot
+    // copy pipeline (sf_set_pipeline): host copies on streams of their own, two source and two result buffers
+    int pipe = 1;
+    int ss = 0, os = 0;           // slot of the last host source / of the last result
+    bool src_piped = false;       // plan->src is psrc[ss], filled on st_h2d
+    cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
+    void* psrc[2] = { nullptr, nullptr };
+    void* pout[2] = { nullptr, nullptr };
+    cudaEvent_t ev_src_ready[2] = { nullptr, nullptr }, ev_src_free[2] = { nullptr, nullptr };
+    cudaEvent_t ev_done[2] = { nullptr, nullptr }, ev_out_free[2] = { nullptr, nullptr };
+    bool src_free_set[2] = { false, false }, out_free_set[2] = { false, false }, done_set[2] = { false, false };
     std::string err = "";
 };
 
@@ -764,7 +774,29 @@ sf_status run_any(sf_plan p, int outk)
 {
     if (!p) return SF_ERR_INVALID_ARG;
     if (!p->src) return fail(p, SF_ERR_STATE, "no source set: call sf_set_source first");
-    return p->prec == SF_F32 ? run<float>(p, outk) : run<double>(p, outk);
+    if (p->pipe < 2) return p->prec == SF_F32 ? run<float>(p, outk) : run<double>(p, outk);
+    // copy pipeline: this call reads the source slot filled last and writes the other result buffer than the
+    // previous call, once the copy that still reads that buffer has finished
+    p->os ^= 1;
+    if (p->src_piped) SF_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_src_ready[p->ss], 0));
+    const bool own_out = (p->out == p->pout[0] || p->out == p->pout[1]);
+    if (own_out) {
+        p->out = p->pout[p->os];
+        if (p->out_free_set[p->os]) SF_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_out_free[p->os], 0));
+    } else {
+        // a work set of sf_gradient: one result buffer, every earlier copy out of it must have finished
+        for (int i = 0; i < 2; ++i)
+            if (p->out_free_set[i]) SF_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_out_free[i], 0));
+    }
+    const sf_status st = p->prec == SF_F32 ? run<float>(p, outk) : run<double>(p, outk);
+    if (st != SF_OK) return st;
+    SF_CUDA(p, cudaEventRecord(p->ev_done[p->os], p->stream));
+    p->done_set[p->os] = true;
+    if (p->src_piped) {
+        SF_CUDA(p, cudaEventRecord(p->ev_src_free[p->ss], p->stream));
+        p->src_free_set[p->ss] = true;
+    }
+    return SF_OK;
 }
 
 size_t field_elems(const sf_plan_s* p) { return (size_t)p->n[0] * (size_t)p->n[1] * (size_t)(p->ndim == 3 ? p->n[2] : 1); }
@@ -783,6 +815,14 @@ sf_status sf_plan_destroy(sf_plan plan)
     if (!plan) return SF_OK;
     for (void* d : plan->allocs) cudaFree(d);
     for (cudaEvent_t e : plan->ev) cudaEventDestroy(e);
+    for (int i = 0; i < 2; ++i) {
+        if (plan->ev_src_ready[i]) cudaEventDestroy(plan->ev_src_ready[i]);
+        if (plan->ev_src_free[i]) cudaEventDestroy(plan->ev_src_free[i]);
+        if (plan->ev_done[i]) cudaEventDestroy(plan->ev_done[i]);
+        if (plan->ev_out_free[i]) cudaEventDestroy(plan->ev_out_free[i]);
+    }
+    if (plan->st_h2d) cudaStreamDestroy(plan->st_h2d);
+    if (plan->st_d2h) cudaStreamDestroy(plan->st_d2h);
     delete plan;
     return SF_OK;
 }
@@ -1008,10 +1048,22 @@ sf_status sf_set_source(sf_plan plan, const void* src, sf_mem where)
     if (where == SF_MEM_DEVICE) {
         if (((uintptr_t)src & 15) != 0) return fail(plan, SF_ERR_INVALID_ARG, "device source must be 16-byte aligned");
         plan->src = src;
+        plan->src_piped = false;
         return SF_OK;
     }
     if (where != SF_MEM_HOST) return fail(plan, SF_ERR_INVALID_ARG, "unknown memory space");
     const size_t bytes = field_elems(plan) * plan->ncomp * plan->esize;
+    if (plan->pipe >= 2) {
+        // the copy runs on its own stream into the slot the compute call before last read
+        plan->ss ^= 1;
+        const int s = plan->ss;
+        if (plan->src_free_set[s]) SF_CUDA(plan, cudaStreamWaitEvent(plan->st_h2d, plan->ev_src_free[s], 0));
+        SF_CUDA(plan, cudaMemcpyAsync(plan->psrc[s], src, bytes, cudaMemcpyHostToDevice, plan->st_h2d));
+        SF_CUDA(plan, cudaEventRecord(plan->ev_src_ready[s], plan->st_h2d));
+        plan->src = plan->psrc[s];
+        plan->src_piped = true;
+        return SF_OK;
+    }
     if (!plan->src_own) {
         sf_status st = dev_alloc(plan, &plan->src_own, bytes);
         if (st != SF_OK) return st;
@@ -1176,6 +1228,73 @@ sf_status sf_synchronize(sf_plan plan)
 {
     if (!plan) return SF_ERR_INVALID_ARG;
     SF_CUDA(plan, cudaStreamSynchronize(plan->stream));
+    if (plan->st_h2d) SF_CUDA(plan, cudaStreamSynchronize(plan->st_h2d));
+    if (plan->st_d2h) SF_CUDA(plan, cudaStreamSynchronize(plan->st_d2h));
+    return SF_OK;
+}
+
+sf_status sf_set_pipeline(sf_plan plan, int depth)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (depth != 1 && depth != 2) return fail(plan, SF_ERR_INVALID_ARG, "pipeline depth must be 1 or 2");
+    sf_status st = sf_synchronize(plan);
+    if (st != SF_OK) return st;
+    if (depth == 2 && !plan->st_h2d) {
+        // second source and result buffers, two copy streams, the events that order them against the plan's stream
+        const size_t sbytes = field_elems(plan) * plan->ncomp * plan->esize, obytes = field_elems(plan) * plan->nfields * plan->esize;
+        if (!plan->src_own && (st = dev_alloc(plan, &plan->src_own, sbytes)) != SF_OK) return st;
+        void *s1 = nullptr, *o1 = nullptr;
+        if ((st = dev_alloc(plan, &s1, sbytes)) != SF_OK) return st;
+        if ((st = dev_alloc(plan, &o1, obytes)) != SF_OK) { dev_free(plan, s1); plan->dev_bytes -= (long long)sbytes; return st; }
+        plan->psrc[0] = plan->src_own; plan->psrc[1] = s1;
+        plan->pout[0] = plan->out; plan->pout[1] = o1;
+        SF_CUDA(plan, cudaStreamCreateWithFlags(&plan->st_h2d, cudaStreamNonBlocking));
+        SF_CUDA(plan, cudaStreamCreateWithFlags(&plan->st_d2h, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            SF_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_src_ready[i], cudaEventDisableTiming));
+            SF_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_src_free[i], cudaEventDisableTiming));
+            SF_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_done[i], cudaEventDisableTiming));
+            SF_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_out_free[i], cudaEventDisableTiming));
+        }
+    }
+    if (depth == 1 && plan->pipe == 2) {
+        // back to one stream: results land in the first buffer again; a piped source stays where it is (the device is idle)
+        if (plan->out == plan->pout[1]) plan->out = plan->pout[0];
+        plan->src_piped = false;
+        for (int i = 0; i < 2; ++i) plan->src_free_set[i] = plan->out_free_set[i] = plan->done_set[i] = false;
+    }
+    plan->pipe = depth;
+    return SF_OK;
+}
+
+sf_status sf_get_output_async(sf_plan plan, int field, int comp, void* dst_host)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (!dst_host) return fail(plan, SF_ERR_INVALID_ARG, "dst is NULL");
+    void* src = nullptr;
+    sf_status st = sf_output_device_ptr(plan, field, comp, &src);
+    if (st != SF_OK) return st;
+    const size_t bytes = field_elems(plan) * plan->esize;
+    if (plan->pipe < 2) {
+        SF_CUDA(plan, cudaMemcpyAsync(dst_host, src, bytes, cudaMemcpyDeviceToHost, plan->stream));
+        return SF_OK;
+    }
+    const int o = plan->os;
+    if (plan->done_set[o]) SF_CUDA(plan, cudaStreamWaitEvent(plan->st_d2h, plan->ev_done[o], 0));
+    SF_CUDA(plan, cudaMemcpyAsync(dst_host, src, bytes, cudaMemcpyDeviceToHost, plan->st_d2h));
+    SF_CUDA(plan, cudaEventRecord(plan->ev_out_free[o], plan->st_d2h));
+    plan->out_free_set[o] = true;
+    return SF_OK;
+}
+
+sf_status sf_pipeline_join(sf_plan plan)
+{
+    if (!plan) return SF_ERR_INVALID_ARG;
+    if (plan->pipe < 2) return SF_OK;
+    for (int i = 0; i < 2; ++i) {
+        if (plan->out_free_set[i]) SF_CUDA(plan, cudaStreamWaitEvent(plan->stream, plan->ev_out_free[i], 0));
+    }
+    if (plan->src_piped) SF_CUDA(plan, cudaStreamWaitEvent(plan->stream, plan->ev_src_ready[plan->ss], 0));
     return SF_OK;
 }
 
