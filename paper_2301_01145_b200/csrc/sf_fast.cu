@@ -3,6 +3,7 @@
 #include "sf_fast.cuh"
 #include "sf_fastper.cuh"
 #include "sf_fast512.cuh"
+#include "sf_fast2p.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -82,6 +83,7 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_CURL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x5_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x5_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_fused2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem2)) != cudaSuccess) return e;
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres)) != cudaSuccess) return e;
@@ -159,7 +161,11 @@ cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map
     switch (mode) {
     case FMODE_FWD: fast_pad_kernel<FMODE_FWD><<<grid, kThreads, FastCfg<FMODE_FWD>::kSmem, st>>>(p, tm); break;
     case FMODE_INV: fast_pad_kernel<FMODE_INV><<<grid, kThreads, FastCfg<FMODE_INV>::kSmem, st>>>(p, tm); break;
-    case FMODE_FUSED: fast_pad_kernel<FMODE_FUSED><<<grid, kThreads, FastCfg<FMODE_FUSED>::kSmem, st>>>(p, tm); break;
+    case FMODE_FUSED:
+        // two pencils per thread (sf_fast2p.cuh) unless switched off; it needs an even number of batches
+        if ((p.nb & 1) == 0 && !getenv("SF_FUSED_1P")) fast_fused2_kernel<<<grid, kT2, kSmem2, st>>>(p, tm);
+        else fast_pad_kernel<FMODE_FUSED><<<grid, kThreads, FastCfg<FMODE_FUSED>::kSmem, st>>>(p, tm);
+        break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
