@@ -85,6 +85,8 @@ struct sf_plan_s {
     // ... and with 512-long y and z pencils (sf_fast512.cuh), scalar or three components (sf_solve, sf_curl)
     bool fast5 = false;
     bool fast5_x = false;  // S1 / S5 too (x extent 512)
+    // ... and in double precision with 256-long y and z pencils (sf_fast64.cuh), scalar
+    bool fast64 = false;
 
     // per-solve state
     const void* src = nullptr;
@@ -597,6 +599,47 @@ template <typename T> sf_status run(sf_plan p, int outk)
         return SF_OK;
     }
 
+    if (p->fast64 && outk == OUT_SOLVE) {
+        // kernel generation 2 in double precision: S2, S3, S4 as persistent TMA-fed register-FFT kernels (tiles of 8 columns)
+        sf2::Fast64Params fp;
+        memset(&fp, 0, sizeof(fp));
+        fp.sched = (int*)p->sched;
+        fp.nct = p->nspec_x / 8;
+        for (fp.nct_shift = 0; (1 << fp.nct_shift) < fp.nct; ++fp.nct_shift) {}
+        fp.nyq_col = (p->nspec_x % 8) ? fp.nct * 8 : -1;
+        // S2: W1 [z][y][hp] -> W2 [z][ky][hp]
+        fp.in = (const double2*)p->W1; fp.out = (double2*)p->W2;
+        fp.in_ps = hp; fp.in_bs = hp * n1; fp.out_ps = hp; fp.out_bs = hp * P1; fp.nb = n2;
+        fp.reverse_batches = 1;
+        SF_CUDA(p, sf2::launch_fast64(sf2::FMODE_FWD, fp, p->map_s2, st));
+        fp.reverse_batches = 0;
+        p->launches++;
+        mark(2);
+        // S3: W2 in place along z
+        fp.in = (const double2*)p->W2; fp.out = (double2*)p->W2;
+        fp.in_ps = fp.out_ps = hp * P1; fp.in_bs = fp.out_bs = hp; fp.nb = P1;
+        fp.pair_batches = 1;
+        fp.green_tiles = (const double*)p->green_tiles; fp.Pb = P1;
+        SF_CUDA(p, sf2::launch_fast64(sf2::FMODE_FUSED, fp, p->map_s3, st));
+        fp.pair_batches = 0;
+        p->launches++;
+        mark(3);
+        // S4: W2 [z][ky][hp] -> W1 [z][y][hp]
+        fp.in = (const double2*)p->W2; fp.out = (double2*)p->W1;
+        fp.in_ps = hp; fp.in_bs = hp * P1; fp.out_ps = hp; fp.out_bs = hp * n1; fp.nb = n2;
+        SF_CUDA(p, sf2::launch_fast64(sf2::FMODE_INV, fp, p->map_s4, st));
+        p->launches++;
+        mark(4);
+        xp.spec_in = p->W1; xp.real_out = (T*)p->out;
+        SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        p->launches++;
+        mark(5);
+        if (timed) p->tcount++;
+        p->last_kind = outk;
+        p->out_last = p->out;
+        return SF_OK;
+    }
+
     if (p->fast5 && (outk == OUT_SOLVE || (outk == OUT_CURL && ncomp == 3))) {
         // kernel generation 2 for 512-long pencils: S2, S3, S4 as persistent TMA-fed register-FFT kernels, one CTA per SM
         sf2::Fast5Params fp;
@@ -989,6 +1032,38 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
             if ((st = dev_alloc(p, &p->nyqA, (size_t)256 * 256 * 8)) != SF_OK) return bail(st, "");
             if ((st = dev_alloc(p, &p->nyqB, (size_t)256 * 512 * 8)) != SF_OK) return bail(st, "");
         }
+    }
+    // ... fp64 scalar unbounded plans whose y and z pencils are 256 long (tiles of 8 columns)
+    if (prec == SF_F64 && b == SF_BC_UNBOUNDED && ndim == 3 && ncomp == 1 && p->n[1] == 256 && p->n[2] == 256 && (p->nspec_x % 8) <= 1 &&
+        p->nspec_x >= 8 && is_pow2(p->nspec_x / 8) && p->n[0] <= 1024 && !getenv("SF_DISABLE_FAST")) {
+        if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fast path failed"); }
+        // the tensor maps address the complex doubles as pairs of 8-byte words
+        const unsigned long long hpB = (unsigned long long)p->pitch * 16ull, N1 = 256, N2 = 256, PP = 512;
+        const unsigned long long hpw = 2ull * (unsigned long long)p->pitch;
+        cudaError_t e1, e2;
+        {
+            const unsigned long long d[4] = { hpw, N1, N2, 1 }, sb[3] = { hpB, hpB * N1, hpB * N1 * N2 };
+            const unsigned bx[4] = { 16, 256, 1, 1 };
+            e1 = sf2::fast_make_map(&p->map_s2, p->W1, d, sb, bx);
+        }
+        {
+            const unsigned long long d[4] = { hpw, PP, N2, 1 }, sb[3] = { hpB, hpB * PP, hpB * PP * N2 };
+            const unsigned bx[4] = { 16, 1, 256, 1 };
+            e2 = sf2::fast_make_map(&p->map_s3, p->W2, d, sb, bx);
+        }
+        p->map_s4 = p->map_s3;
+        if (e1 != cudaSuccess || e2 != cudaSuccess) return bail(SF_ERR_CUDA, "tensor map encoding failed");
+        {
+            const int nct = p->nspec_x / 8, nyq = (p->nspec_x % 8) ? nct * 8 : -1;
+            const size_t ne = sf2::fast64_green_tiles_elems(512, nct, nyq);
+            if ((st = dev_alloc(p, &p->green_tiles, ne * sizeof(double))) != SF_OK) return bail(st, "");
+            if (sf2::fast64_green_tiles((double*)p->green_tiles, (const double*)p->green, p->pitch, p->pitch * (p->n[1] + 1), 512, nct, nyq,
+                                        p->stream) != cudaSuccess)
+                return bail(SF_ERR_CUDA, "building the tile-major Green's table failed");
+        }
+        if ((st = dev_alloc(p, &p->sched, 2 * sizeof(int))) != SF_OK) return bail(st, "");
+        if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
+        p->fast64 = true;
     }
     // ... fp32 unbounded plans whose y and z pencils are 512 long (BASELINE.json configs[4]: three components, curl)
     if (prec == SF_F32 && b == SF_BC_UNBOUNDED && ndim == 3 && p->n[1] == 512 && p->n[2] == 512 && (p->nspec_x % sf2::kTile) <= 1 &&

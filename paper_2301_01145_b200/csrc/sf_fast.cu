@@ -4,6 +4,7 @@
 #include "sf_fastper.cuh"
 #include "sf_fast512.cuh"
 #include "sf_fast2p.cuh"
+#include "sf_fast64.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -84,6 +85,17 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_x5_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x5_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_fused2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem2)) != cudaSuccess) return e;
+    {
+        std::vector<double2> td(1024);
+        for (int j = 0; j < 1024; ++j) {
+            const long double a = 2.0L * pi * (long double)j / 1024.0L;
+            td[j] = make_double2((double)cosl(a), (double)(-sinl(a)));
+        }
+        if ((e = cudaMemcpyToSymbol(c_tw1024d, td.data(), sizeof(double2) * 1024)) != cudaSuccess) return e;
+    }
+    if ((e = cudaFuncSetAttribute(fast64_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem64)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast64_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem64NoSlot)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast64_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem64)) != cudaSuccess) return e;
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres)) != cudaSuccess) return e;
@@ -190,6 +202,34 @@ cudaError_t launch_fast5(int mode, const Fast5Params& p, const TileMap& in_map, 
     case F5_INV: fast5_kernel<F5_INV><<<grid, kT5, kSmem5NoSlot, st>>>(p, tm); break;
     case F5_FUSED: fast5_kernel<F5_FUSED><<<grid, kT5, kSmem5, st>>>(p, tm); break;
     case F5_CURL: fast5_kernel<F5_CURL><<<grid, kT5, kSmem5, st>>>(p, tm); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t fast64_green_tiles(double* tiles, const double* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
+                               cudaStream_t st)
+{
+    const long long total = (long long)fast64_green_tiles_elems(Pb, nct, nyq_col);
+    green_tiles64_kernel<<<148 * 8, 256, 0, st>>>(tiles, green, g_pb, g_pp, Pb, nct, nyq_col, total);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fast64(int mode, const Fast64Params& p, const TileMap& in_map, cudaStream_t st)
+{
+    const CUtensorMap& tm = reinterpret_cast<const CUtensorMap&>(in_map);
+    if (p.nct <= 0 || (1 << p.nct_shift) != p.nct || p.nb <= 0) return cudaErrorInvalidValue;
+    // the kernels index with 32-bit element offsets
+    if ((long long)p.nb * p.in_bs + 512 * p.in_ps >= (1ll << 31) || (long long)p.nb * p.out_bs + 512 * p.out_ps >= (1ll << 31))
+        return cudaErrorInvalidValue;
+    if (mode == FMODE_FUSED && !p.green_tiles) return cudaErrorInvalidValue;
+    const int ntiles = p.nb * p.nct + (p.nyq_col >= 0 ? (p.nb + kTile64 - 1) / kTile64 : 0);
+    int grid = 2 * g_sms;
+    if (grid > ntiles) grid = ntiles;
+    switch (mode) {
+    case FMODE_FWD: fast64_kernel<FMODE_FWD><<<grid, kT64, kSmem64, st>>>(p, tm); break;
+    case FMODE_INV: fast64_kernel<FMODE_INV><<<grid, kT64, kSmem64NoSlot, st>>>(p, tm); break;
+    case FMODE_FUSED: fast64_kernel<FMODE_FUSED><<<grid, kT64, kSmem64, st>>>(p, tm); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

@@ -91,17 +91,30 @@ __host__ __device__ constexpr double cos16(int i)
 }
 __host__ __device__ constexpr double sin16(int i) { return cos16(i - 4); }
 
+// the same complex helpers for double precision (sf_fast64.cuh): plain DADD / DMUL / DFMA
+typedef double2 D;
+__device__ __forceinline__ D cadd(D a, D b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ D csub(D a, D b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ D cmul(D a, D w) { return make_double2(fma(a.x, w.x, -a.y * w.y), fma(a.x, w.y, a.y * w.x)); }
+__device__ __forceinline__ D cmulc(D a, D w) { return make_double2(fma(a.x, w.x, a.y * w.y), fma(a.y, w.x, -a.x * w.y)); }
+template <bool CONJ> __device__ __forceinline__ D cmul_sel(D a, D w) { return CONJ ? cmulc(a, w) : cmul(a, w); }
+__device__ __forceinline__ D cscale(D a, double s) { return make_double2(a.x * s, a.y * s); }
+__device__ __forceinline__ D cmuli(D a) { return make_double2(-a.y, a.x); }
+__device__ __forceinline__ D cmulmi(D a) { return make_double2(a.y, -a.x); }
+__device__ __forceinline__ C mk_c(C, double x, double y) { return make_float2((float)x, (float)y); }
+__device__ __forceinline__ D mk_c(D, double x, double y) { return make_double2(x, y); }
+
 // d * exp(-/+ 2 pi i I16 / 16)   (forward: minus)
-template <int I16, bool INV> __device__ __forceinline__ C mul_w16(C d)
+template <int I16, bool INV, typename CT> __device__ __forceinline__ CT mul_w16(CT d)
 {
     if constexpr (I16 == 0) {
         return d;
     } else if constexpr (I16 == 4) {
         return INV ? cmuli(d) : cmulmi(d);
     } else {
-        constexpr float c = (float)cos16(I16);
-        constexpr float s = (float)(INV ? sin16(I16) : -sin16(I16));
-        return cmul(d, make_float2(c, s));
+        constexpr double c = cos16(I16);
+        constexpr double s = (INV ? sin16(I16) : -sin16(I16));
+        return cmul(d, mk_c(CT(), c, s));
     }
 }
 
@@ -110,16 +123,16 @@ __host__ __device__ constexpr int brev4(int q) { return ((q & 1) << 3) | ((q & 2
 // radix-2 decimation-in-frequency recursion on v[0], v[S], ...: result q of the length-R DFT ends
 // at v[bitrev_R(q) * S]
 template <int R, int S, bool INV> struct dft_rec {
-    template <int I> static __device__ __forceinline__ void level(C* v)
+    template <int I, typename CT> static __device__ __forceinline__ void level(CT* v)
     {
         if constexpr (I < R / 2) {
-            const C a = v[I * S], b = v[(I + R / 2) * S];
+            const CT a = v[I * S], b = v[(I + R / 2) * S];
             v[I * S] = cadd(a, b);
             v[(I + R / 2) * S] = mul_w16<I * (16 / R), INV>(csub(a, b));
             level<I + 1>(v);
         }
     }
-    static __device__ __forceinline__ void run(C* v)
+    template <typename CT> static __device__ __forceinline__ void run(CT* v)
     {
         level<0>(v);
         dft_rec<R / 2, S, INV>::run(v);
@@ -127,10 +140,10 @@ template <int R, int S, bool INV> struct dft_rec {
     }
 };
 template <int S, bool INV> struct dft_rec<1, S, INV> {
-    static __device__ __forceinline__ void run(C*) {}
+    template <typename CT> static __device__ __forceinline__ void run(CT*) {}
 };
 // v[0..16) natural order in; DFT output q at v[brev4(q)]
-template <bool INV> __device__ __forceinline__ void dft16(C (&v)[16]) { dft_rec<16, 1, INV>::run(v); }
+template <bool INV, typename CT> __device__ __forceinline__ void dft16(CT (&v)[16]) { dft_rec<16, 1, INV>::run(v); }
 
 // ------------------------------------------------------------------------------------ 256-point transform
 // Exchange buffer: 16 x 16 slots of 32 complex (one per lane).  Orientation A: slot (a, b) at
@@ -526,7 +539,7 @@ constexpr int kXSpPitch = kXN + 2;       // complex per staged spectrum row: 206
 constexpr size_t kXSmem = (size_t)kXRows * kXInPitch * sizeof(float) + (size_t)16 * 8 * 32 * sizeof(C) + (size_t)kXRows * kXSpPitch * sizeof(C);
 
 __host__ __device__ constexpr int brev3(int q) { return ((q & 1) << 2) | (q & 2) | ((q & 4) >> 2); }
-template <bool INV> __device__ __forceinline__ void dft8(C (&v)[8]) { dft_rec<8, 1, INV>::run(v); }
+template <bool INV, typename CT> __device__ __forceinline__ void dft8(CT (&v)[8]) { dft_rec<8, 1, INV>::run(v); }
 
 // v[r] = a[w + 8 r] in; writes the twiddled radix-16 outputs into the exchange buffer
 template <bool INV> __device__ __forceinline__ void fft128_a(C (&v)[16], const C* tw128, C* xw)

@@ -109,6 +109,31 @@ struct Fast5Params {
     // CURL: wavenumbers of the doubled grid (zero at the Nyquist index): per column, per batch, per pencil row (1024)
     const float* kap_x; const float* kap_b; const float* kap_p;
 };
+// strided passes of fp64 unbounded plans with 256-point y / z pencils padded to 512 (fast64_kernel, sf_fast64.cuh):
+// tiles of 8 pencils
+struct Fast64Params {
+    const double2* in;
+    double2* out;
+    long long in_ps, in_bs;     // row (pencil-axis) and batch strides, complex elements
+    long long out_ps, out_bs;
+    int nb;                     // batches
+    int nct, nct_shift;         // full 8-column tiles per batch: a power of two
+    int nyq_col;                // column handled 8 batches at a time (the Nyquist column), -1: none
+    int reverse_batches, pair_batches;
+    int* sched;                 // device: { next unclaimed tile, CTAs finished }, zero between launches
+    const double* green_tiles;  // tile-major real Green's table: chunk [kGreenRows fp][8 pencils] per tile
+    int Pb;
+};
+inline size_t fast64_green_tiles_elems(int Pb, int nct, int nyq_col)
+{
+    return ((size_t)(Pb / 2 + 1) * nct + (nyq_col >= 0 ? (size_t)(Pb + 7) / 8 : 0)) * kGreenRows * 8;
+}
+cudaError_t fast64_green_tiles(double* tiles, const double* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
+                               cudaStream_t st);
+// launch one fp64 padded pass (mode = FMODE_*) as a persistent grid of two 256-thread CTAs per SM; `in_map` describes
+// p.in in 8-byte words as documented at fast64_kernel
+cudaError_t launch_fast64(int mode, const Fast64Params& p, const TileMap& in_map, cudaStream_t st);
+
 // number of floats of the tile-major Green's table with `rows` folded pencil indices per chunk
 inline size_t fast_green_tiles_elems_rows(int Pb, int nct, int nyq_col, int rows)
 {

@@ -45,6 +45,25 @@ def test_fast_path_white_noise_narrow_x(nx):
     assert (err <= 10 * TOL["f32"] * nrm).all()
 
 
+@pytest.mark.parametrize("nx", [8, 16, 64, 256])
+def test_fast64_white_noise_narrow_x(nx):
+    """the same in double precision (sf_fast64.cuh, tiles of 8 columns): nx / 8 full column tiles plus the Nyquist column"""
+    shape = (256, 256, nx)
+    f = W.Rng(4600 + nx).normal(int(np.prod(shape))).reshape(shape)
+    h = (1.0 / 256, 1.0 / 256, 1.0 / 256)
+    gh = O.unbounded_green((nx, 256, 256), h, 2.0 * h[0])
+    ref = O.unbounded_solve(f, h, gh)
+    with Plan(shape, h, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec="f64") as p:
+        p.set_source(f)
+        for _ in range(3):
+            sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI)
+    _check(f"psi 256x256x{nx} f64 white noise", got, ref, "f64")
+    err = np.linalg.norm((got - ref).reshape(256, -1), axis=1)
+    nrm = np.linalg.norm(ref.reshape(256, -1), axis=1)
+    assert (err <= 10 * TOL["f64"] * nrm).all()
+
+
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 def test_cfg4_full_size(prec):
     g = W.gaussian_blobs(256)
