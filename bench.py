@@ -41,6 +41,7 @@ UNIT = "points/s"
 # ---------------------------------------------------------------------------------------- workloads
 # name -> (config number, n, precision, call); algorithmic bytes come from model_bytes() below
 WORKLOADS = {
+    "cfg1_periodic2d_64_f64_grad": dict(cfg=1, n=64, prec="f64", kind="periodic", call="gradient", ncomp=1, ndim=2),
     "cfg4_unbounded_256_f32": dict(cfg=4, n=256, prec="f32", kind="unbounded", call="solve", ncomp=1),
     "cfg4_unbounded_256_f64": dict(cfg=4, n=256, prec="f64", kind="unbounded", call="solve", ncomp=1),
     "cfg2_periodic_256_f32": dict(cfg=2, n=256, prec="f32", kind="periodic", call="solve", ncomp=1),
@@ -61,6 +62,11 @@ def model_bytes(w):
     n, r = w["n"], (4 if w["prec"] == "f32" else 8)
     c = 2 * r
     nc = w["ncomp"]
+    if w.get("ndim", 3) == 2:   # S1, the fused pass along y, S5 (periodic, gradient: three output fields)
+        h = n // 2 + 1
+        nout = 3 if w["call"] == "gradient" else 1
+        spec = n * h * c
+        return [n * n * r + spec, 0, spec + nout * spec, 0, nout * (spec + n * n * r)]
     if w["kind"] == "unbounded":
         hx, p = n + 1, 2 * n
         nout = nc
@@ -85,7 +91,7 @@ def model_bytes(w):
 
 
 STEP_EVENT_STRIDE = 8   # per-step CUDA events are recorded on every 8th solve of the timed region
-STEP_NAMES = ["S1 fast_x_kernel<fwd>", "S2 fast_pad_kernel<FWD>", "S3 fast_pad_kernel<FUSED>", "S4 fast_pad_kernel<INV>",
+STEP_NAMES = ["S1 fast_x_kernel<fwd>", "S2 fast_pad_kernel<FWD>", "S3 fast_fused2_kernel", "S4 fast_pad_kernel<INV>",
               "S5 fast_x_kernel<inv>"]
 
 
@@ -93,6 +99,8 @@ def step_names(wname):
     """the kernel behind each of the five steps for this workload"""
     if wname == "cfg4_unbounded_256_f32":
         return STEP_NAMES
+    if wname == "cfg4_unbounded_256_f64":
+        return ["S1 xfwd_kernel", "S2 fast64_kernel<FWD>", "S3 fast64_kernel<FUSED>", "S4 fast64_kernel<INV>", "S5 xinv_kernel"]
     if wname in ("cfg2_periodic_256_f32", "cfg2_periodic_256_f32_grad"):
         return ["S1 fast_xper_kernel<fwd>", "S2 fast_per_kernel<FWD>", "S3 fast_per_kernel<FUSED>", "S4 fast_per_kernel<INV>",
                 "S5 fast_xper_kernel<inv>"]
@@ -101,25 +109,54 @@ def step_names(wname):
     return ["S1 xfwd_kernel", "S2 spass_kernel<0>", "S3 spass_kernel<2>", "S4 spass_kernel<1>", "S5 xinv_kernel"]
 
 
-# Issue cycles per warp-tile of the fused S3 kernel of the default workload, counted from the ncu source page of
-# capture d (profiles/r01_d.md): 476 packed fp32x2 instructions at two issue cycles each plus
-# 370 others; 8224 tiles x 16 warps per launch; 148 SMs x 4 schedulers issue one warp instruction per clock.
-S3_ISSUE_CYCLES_PER_WARP_TILE = 2 * 476 + 370
-S3_WARP_TILES = 8224 * 16
+# ncu-derived counts of the dominant kernels (warp instructions, packed fp32x2 instructions, DRAM bytes per launch)
+# live in profiles/ncu_counts.json together with the SHA-256 of the kernel sources they were captured from.  They
+# are used only while that hash matches the sources of this checkout: a changed kernel turns "issue_view" and
+# "traffic" into null instead of letting them go stale silently.
 ISSUE_SLOTS_PER_CLOCK = 148 * 4
+KERNEL_SOURCE_GLOBS = ("paper_2301_01145_b200/csrc/*.cu", "paper_2301_01145_b200/csrc/*.cuh", "paper_2301_01145_b200/csrc/*.h")
 
 
-def issue_view(wname, dom, kernel_ms, clocks):
-    """The dominant kernel of the default workload is bound by instruction issue, not by HBM (profiles/r01_b.md):
-    besides the HBM roofline the line carries its issue-slot utilisation, from the static instruction count above
-    and the SM clock sampled during the timed region.  None for other workloads / kernels."""
-    if wname != DEFAULT_WORKLOAD or dom != 2 or not clocks or not clocks.get("sm_mhz"):
+def kernel_source_hash():
+    import hashlib
+
+    hsh = hashlib.sha256()
+    files = sorted(f for g in KERNEL_SOURCE_GLOBS for f in ROOT.glob(g))
+    for f in files:
+        hsh.update(f.name.encode())
+        hsh.update(f.read_bytes())
+    return hsh.hexdigest()
+
+
+def ncu_counts(wname, step_index):
+    """the committed ncu counts of step `step_index` of a workload, or None when there is no capture or the kernel
+    sources have changed since it was taken"""
+    f = ROOT / "profiles" / "ncu_counts.json"
+    if not f.exists():
         return None
-    cycles = S3_ISSUE_CYCLES_PER_WARP_TILE * S3_WARP_TILES
+    try:
+        doc = json.load(open(f))
+    except Exception:
+        return None
+    if doc.get("kernel_sources_sha256") != kernel_source_hash():
+        return None
+    return doc.get("workloads", {}).get(wname, {}).get(f"S{step_index + 1}")
+
+
+def issue_view(wname, dom, kernel_ms, clocks, names):
+    """The dominant kernel of the default workload is bound by instruction issue, not by HBM (profiles/r02_a.md):
+    besides the HBM roofline the line carries its issue-slot utilisation = (warp instructions + packed fp32x2
+    instructions: a packed instruction occupies its scheduler for two cycles) / (148 SMs x 4 schedulers x the SM clock
+    sampled during the timed region) / measured kernel time.  None without a capture of the current sources."""
+    c = ncu_counts(wname, dom)
+    if not c or not clocks or not clocks.get("sm_mhz") or "warp_instructions" not in c:
+        return None
+    cycles = c["warp_instructions"] + c.get("packed_fp32x2_warp_instructions", 0)
     t_peak_ms = cycles / (ISSUE_SLOTS_PER_CLOCK * clocks["sm_mhz"] * 1e6) * 1e3
-    return {"bound": "alu", "kernel": STEP_NAMES[2], "issue_cycles_per_launch": cycles,
+    return {"bound": "alu", "kernel": names[dom], "issue_cycles_per_launch": cycles,
             "ms_at_one_warp_instruction_per_scheduler_clock": t_peak_ms, "kernel_ms": kernel_ms, "frac": t_peak_ms / kernel_ms,
-            "source": "instruction counts of profiles/r01_d (ncu source page), SM clock of this run"}
+            "source": f"instruction counts of {c.get('capture', 'profiles/ncu_counts.json')} (ncu source page, same kernel sources), "
+                      "SM clock of this run"}
 
 
 def make_input(w, rank=0):
@@ -135,6 +172,9 @@ def make_input(w, rank=0):
     if w["kind"] == "unbounded":
         g = W.vortex_ring(n, seed=seed)
         return dict(f=np.ascontiguousarray(g["omega"].astype(dt)), h=g["h"], faces={})
+    if w["kind"] == "periodic" and w.get("ndim", 3) == 2:
+        g = W.periodic2d_modes(n, seed=seed)
+        return dict(f=np.ascontiguousarray(g["f"].astype(dt)), h=tuple(L / n for L in g["L"]), faces={})
     if w["kind"] == "periodic":
         g = W.periodic3d_spectrum(n, seed=seed)
         return dict(f=np.ascontiguousarray(g["f"].astype(dt)), h=tuple(L / n for L in g["L"]), faces={})
@@ -206,18 +246,12 @@ class ClockSampler(threading.Thread):
 
 # ---------------------------------------------------------------------------------------- ncu traffic
 def ncu_traffic(workload, step_index):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary
-    (profiles/traffic.csv: workload,step,kernel,dram_read_bytes,dram_write_bytes,source); None if
-    that capture does not exist for this workload / kernel."""
-    f = ROOT / "profiles" / "traffic.csv"
-    if not f.exists():
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the committed
+    ncu --set full capture of the current kernel sources (profiles/ncu_counts.json); None otherwise."""
+    c = ncu_counts(workload, step_index)
+    if not c or "dram_read_bytes" not in c:
         return None
-    best = None
-    with open(f) as fh:
-        for row in csv.DictReader(line for line in fh if not line.startswith("#")):
-            if row["workload"] == workload and int(row["step"]) == step_index + 1:
-                best = float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
-    return best
+    return float(c["dram_read_bytes"]) + float(c["dram_write_bytes"])
 
 
 def load_peaks():
@@ -291,18 +325,45 @@ def run_reference(args):
     return 0
 
 
-def cpu_baseline():
-    """The oracle as it stands on the host cores: one full-size cfg-4 solve if it is predicted to take
-    under ~40 s, else the 128^3 -> 256^3 copy."""
-    n_s = pick_oracle_sample(40.0, 2)
-    run, threads = oracle_solve_timer(n_s)
+def cpu_baseline(wname=DEFAULT_WORKLOAD):
+    """The oracle as it stands on the host cores, on a bounded sample of the workload: cfg 4 one full-size solve
+    if it is predicted to take under ~40 s (else the 128^3 -> 256^3 copy); the other workloads one call of the
+    oracle routine the parity tests compare with, at a size that keeps it to seconds."""
+    import oracle as O
+
+    w = WORKLOADS[wname]
+    if wname == DEFAULT_WORKLOAD:
+        n_s = pick_oracle_sample(40.0, 2)
+        run, threads = oracle_solve_timer(n_s)
+        what = f"1 solve of the cfg-4 workload at {n_s}^3 padded to {2 * n_s}^3, fp64 oracle on the full doubled domain, " \
+               "Green's spectrum precompute excluded"
+        npts = n_s ** 3
+    else:
+        ndim = w.get("ndim", 3)
+        # direct O(N^2) sums per pencil for the real-to-real rows, recursive FFTs elsewhere: sizes chosen for seconds
+        n_s = {"periodic": min(w["n"], 256), "dirichlet": 127, "neumann": 128, "unbounded": min(w["n"], 128)}[w["kind"]]
+        ws = dict(w, n=n_s)
+        inp = make_input(ws, 0)
+        f = inp["f"].astype(np.float64)
+        if w["kind"] == "periodic":
+            L = tuple(hh * n_s for hh in inp["h"])
+            run = lambda: O.periodic(f, L, want_grad=(w["call"] == "gradient"))
+        elif w["kind"] == "dirichlet":
+            run = lambda: O.dirichlet_regular(f, inp["h"], faces=inp["faces"])
+        elif w["kind"] == "neumann":
+            run = lambda: O.neumann_staggered(f, inp["h"], faces=inp["faces"])
+        else:
+            gh = O.unbounded_green((n_s,) * 3, inp["h"], 2.0 * inp["h"][0])
+            rs = -1.0 if w["call"] == "curl" else 1.0
+            run = lambda: O.unbounded_solve(f, inp["h"], gh, rhs_sign=rs, want_curl=(w["call"] == "curl"))
+        threads = O.num_threads()
+        what = f"1 call of the oracle routine of this workload ({w['kind']}, sf_{w['call']}) at {n_s}^{ndim}, fp64"
+        npts = n_s ** ndim
     run()  # page in
     t0 = time.perf_counter()
     run()
     dt = time.perf_counter() - t0
-    return {"value": n_s ** 3 / dt, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": dt,
-            "sample": f"1 solve of the cfg-4 workload at {n_s}^3 padded to {2 * n_s}^3, fp64 oracle on the full doubled "
-                      f"domain, Green's spectrum precompute excluded"}
+    return {"value": npts / dt, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": dt, "sample": what}
 
 
 # ---------------------------------------------------------------------------------------- our arm
@@ -357,7 +418,8 @@ def run_ours(args):
     op = {"unbounded": sf.SF_OP_GREEN_GAUSS2, "periodic": sf.SF_OP_PSEUDO_SPECTRAL, "dirichlet": sf.SF_OP_FD2,
           "neumann": sf.SF_OP_FD2}[w["kind"]]
     grid = sf.SF_GRID_CELL_BOUNDARY if w["kind"] == "dirichlet" else sf.SF_GRID_CELL_CENTRE
-    plan = sf.sf_plan_create([n, n, n], inp["h"], bc, grid=grid, op=op, prec=sf.SF_F32 if w["prec"] == "f32" else sf.SF_F64,
+    ndim = w.get("ndim", 3)
+    plan = sf.sf_plan_create([n] * ndim, inp["h"], bc, grid=grid, op=op, prec=sf.SF_F32 if w["prec"] == "f32" else sf.SF_F64,
                              ncomp=ncomp, stream=stream.cuda_stream, rhs_sign=-1.0 if w["call"] == "curl" else 1.0)
     call = {"solve": sf.sf_solve, "gradient": sf.sf_gradient, "curl": sf.sf_curl}[w["call"]]
     out_field = sf.SF_OUT_CURL if w["call"] == "curl" else sf.SF_OUT_PSI
@@ -417,10 +479,10 @@ def run_ours(args):
     # result, every step, inside the timed region.  The plan's copy pipeline (sf_set_pipeline, depth 2) runs the
     # upload of step k+1, the solve of step k and the download of step k-1 side by side; every step still uploads
     # its source and downloads its whole result (gradient: all 1 + ndim fields).
-    nfields_out = ncomp if w["call"] != "gradient" else 4
+    nfields_out = ncomp if w["call"] != "gradient" else 1 + ndim
     fields = [(out_field, c) for c in range(ncomp)] if w["call"] != "gradient" else \
-        [(sf.SF_OUT_PSI, 0)] + [(sf.SF_OUT_GRAD, a) for a in range(3)]
-    dst_host = [torch.empty((nfields_out, n, n, n), dtype=tdt).pin_memory() for _ in range(2)]
+        [(sf.SF_OUT_PSI, 0)] + [(sf.SF_OUT_GRAD, a) for a in range(ndim)]
+    dst_host = [torch.empty((nfields_out,) + (n,) * ndim, dtype=tdt).pin_memory() for _ in range(2)]
     e2e_steps = max(3, min(steps, 20))
     sf.sf_set_pipeline(plan, 2)
 
@@ -470,7 +532,7 @@ def run_ours(args):
 
     if rank == 0:
         ms_per_step = total_ms / steps
-        pts = float(n) ** 3 * world
+        pts = float(n) ** ndim * world
         mb = model_bytes(w)
         peak, peak_src = load_peaks()
         dom = int(np.argmax(step_ms))
@@ -481,10 +543,14 @@ def run_ours(args):
             "metric": METRIC, "value": pts / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": steps,
             "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": w["prec"], "data": "synthetic",
-            "config": {"workload": wname, "grid": f"{n}^3" + (f" padded to {2 * n}^3" if w["kind"] == "unbounded" else ""),
+            "config": {"workload": wname, "grid": f"{n}^{ndim}" + (f" padded to {2 * n}^{ndim}" if w["kind"] == "unbounded" else ""),
                        "call": "sf_" + w["call"], "ncomp": ncomp, "parallelism": f"replicas x{world}",
-                       "l2": "no flush needed: every step streams its whole working set through HBM "
-                             f"({sum(mb) / 1e6:.0f} MB algorithmic per step, plan holds {dev_bytes / 1e6:.0f} MB) >> 126 MB L2",
+                       "l2": ("no flush needed: every step streams its whole working set through HBM "
+                              f"({sum(mb) / 1e6:.0f} MB algorithmic per step, plan holds {dev_bytes / 1e6:.0f} MB) >> 126 MB L2")
+                             if sum(mb) > 4 * 126e6 else
+                             (f"not flushed: the working set ({sum(mb) / 1e6:.1f} MB algorithmic per step) is of the order of / below the "
+                              "126 MB L2, so part of every pass is served from L2; the roofline fraction of this "
+                              "workload is not an HBM statement"),
                        "timed_region": "sf_solve x K back to back, source and output resident in HBM, Green's spectrum "
                                        "precomputed at plan time (PAPER.md:53, :344)"},
             "clocks": clocks,
@@ -499,7 +565,10 @@ def run_ours(args):
                          "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": mb[dom], "kernel_ms": step_ms[dom]},
             "steps_ms": {names[i]: step_ms[i] for i in range(5)},
-            "issue_view": issue_view(wname, dom, step_ms[dom], clocks),
+            "steps_ms_note": "CUDA events of the library around each of the five launches, on every "
+                             f"{STEP_EVENT_STRIDE if steps >= 2 * STEP_EVENT_STRIDE else 1}-th step of the timed region; "
+                             "their sum exceeds ms_per_step by the cost of the event records themselves",
+            "issue_view": issue_view(wname, dom, step_ms[dom], clocks, names),
             "steps_gbs": {names[i]: (mb[i] / (step_ms[i] * 1e-3) / 1e9 if step_ms[i] > 0 else None) for i in range(5)},
             "solve_roofline": {"algorithmic_bytes_per_step": sum(mb), "achieved_gbs": sum(mb) / (ms_per_step * 1e-3) / 1e9,
                                "frac_of_measured_peak": sum(mb) / (ms_per_step * 1e-3) / 1e9 / peak,
@@ -508,7 +577,7 @@ def run_ours(args):
             "step_event_stride": STEP_EVENT_STRIDE if steps >= 2 * STEP_EVENT_STRIDE else 1,
         }
         if world == 1 and not args.no_cpu_baseline and wname == DEFAULT_WORKLOAD:   # the oracle sample is the cfg-4 workload
-            line["cpu_baseline"] = cpu_baseline()
+            line["cpu_baseline"] = cpu_baseline(wname)
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()

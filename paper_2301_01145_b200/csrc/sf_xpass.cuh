@@ -172,21 +172,19 @@ __global__ void __launch_bounds__(NT) xfwd_kernel(const XParams<T> p)
         C* so = reinterpret_cast<C*>(p.spec_out) + comp * p.sp_pc;
         for (int idx = threadIdx.x; idx < ROWS * H; idx += NT) {
             const int r = idx / H, k = idx % H;
-            const long long row = row0 + r;
-            if (row < nrows) {
-                const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-                if (k == L && p.nyq_side) reinterpret_cast<C*>(p.nyq_side)[p.nyq_side_yz ? (long long)iy * p.nz + iz : comp * nrows + row] = G[r * LP + k];
-                else so[iy * p.sp_py + iz * p.sp_pz + k] = G[r * LP + k];
+            const int iy = s_iy[r];
+            if (iy >= 0) {
+                if (k == L && p.nyq_side) reinterpret_cast<C*>(p.nyq_side)[p.nyq_side_yz ? (long long)iy * p.nz + s_iz[r] : comp * nrows + row0 + r] = G[r * LP + k];
+                else so[s_sp[r] + k] = G[r * LP + k];
             }
         }
     } else {
         T* ro = p.real_out + comp * p.sp_pc;
         const int n = p.n;
-        for (int idx = threadIdx.x; idx < ROWS * n; idx += NT) {
-            const int r = idx / n, k = idx % n;
-            const long long row = row0 + r;
-            if (row < nrows) {
-                const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
+        // a warp per row, lanes along the row (n is a run-time number: no division per element)
+        for (int r = threadIdx.x >> 5; r < ROWS; r += NT / 32)
+        for (int k = threadIdx.x & 31; k < n; k += 32) {
+            if (s_iy[r] >= 0) {
                 T y;
                 if (p.mode == X_DST1) {
                     y = -G[r * LP + k + 1].y;
@@ -201,7 +199,7 @@ __global__ void __launch_bounds__(NT) xfwd_kernel(const XParams<T> p)
                     const C x = G[r * LP + k];
                     y = w.x * x.x - w.y * x.y;
                 }
-                ro[iy * p.sp_py + iz * p.sp_pz + k] = y;
+                ro[s_sp[r] + k] = y;
             }
         }
     }
@@ -223,18 +221,29 @@ __global__ void __launch_bounds__(NT) xinv_kernel(const XParams<T> p)
     const long long row0 = (long long)blockIdx.x * ROWS;
     const long long nrows = (long long)p.ny * p.nz;
 
+    // row geometry once per row
+    __shared__ int s_iy[16], s_iz[16];
+    __shared__ long long s_rin[16], s_sp[16];
+    if (threadIdx.x < ROWS) {
+        const long long row = row0 + threadIdx.x;
+        const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
+        s_iy[threadIdx.x] = (row < nrows) ? iy : -1;
+        s_iz[threadIdx.x] = iz;
+        s_rin[threadIdx.x] = iy * p.rin_py + iz * p.rin_pz;
+        s_sp[threadIdx.x] = iy * p.sp_py + iz * p.sp_pz;
+    }
+    __syncthreads();
     // load the half-spectrum X[0..L] (natural order) into A
     if (p.mode == X_PERIODIC || p.mode == X_ZEROPAD) {
         constexpr int H = L + 1;
         const C* si = reinterpret_cast<const C*>(p.spec_in) + comp * p.sp_pc;
         for (int idx = threadIdx.x; idx < ROWS * H; idx += NT) {
             const int r = idx / H, k = idx % H;
-            const long long row = row0 + r;
             C x = mk<T>(0, 0);
-            if (row < nrows) {
-                const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-                if (k == L && p.nyq_side) x = reinterpret_cast<const C*>(p.nyq_side)[p.nyq_side_yz ? (long long)iy * p.nz + iz : comp * nrows + row];
-                else x = si[iy * p.sp_py + iz * p.sp_pz + k];
+            const int iy = s_iy[r];
+            if (iy >= 0) {
+                if (k == L && p.nyq_side) x = reinterpret_cast<const C*>(p.nyq_side)[p.nyq_side_yz ? (long long)iy * p.nz + s_iz[r] : comp * nrows + row0 + r];
+                else x = si[s_sp[r] + k];
             }
             A[r * LP + k] = x;
         }
@@ -243,11 +252,9 @@ __global__ void __launch_bounds__(NT) xinv_kernel(const XParams<T> p)
         const int n = p.n;
         for (int idx = threadIdx.x; idx < ROWS * (L + 1); idx += NT) {
             const int r = idx / (L + 1), k = idx % (L + 1);
-            const long long row = row0 + r;
             C x = mk<T>(0, 0);
-            if (row < nrows) {
-                const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-                const T* rp = ri + iy * p.sp_py + iz * p.sp_pz;
+            if (s_iy[r] >= 0) {
+                const T* rp = ri + s_sp[r];
                 if (p.mode == X_DST1) {
                     if (k >= 1 && k <= n) x = mk<T>(0, -rp[k - 1]);       // X~[k] = -i Y[k-1]
                 } else if (p.mode == X_DCT1) {
@@ -300,23 +307,17 @@ __global__ void __launch_bounds__(NT) xinv_kernel(const XParams<T> p)
     const int n = p.n;
     if (p.mode == X_PERIODIC || p.mode == X_ZEROPAD || p.mode == X_DCT2 || p.mode == X_DST2) {
         const int nc = n / 2; // stored reals are x~[0..n): the first n/2 packed complex values
-        for (int idx = threadIdx.x; idx < ROWS * nc; idx += NT) {
-            const int r = idx / nc, j = idx % nc;
-            const long long row = row0 + r;
-            if (row < nrows) {
-                const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-                *reinterpret_cast<C*>(ro + iy * p.rin_py + iz * p.rin_pz + 2 * j) = F[r * LP + j];
-            }
+        for (int r = threadIdx.x >> 5; r < ROWS; r += NT / 32)
+        for (int j = threadIdx.x & 31; j < nc; j += 32) {
+            if (s_iy[r] >= 0) *reinterpret_cast<C*>(ro + s_rin[r] + 2 * j) = F[r * LP + j];
         }
     } else { // X_DST1: x_j = x~[j+1];  X_DCT1 (n odd): x_j = x~[j]
-        for (int idx = threadIdx.x; idx < ROWS * n; idx += NT) {
-            const int r = idx / n, j = idx % n;
-            const long long row = row0 + r;
-            if (row < nrows) {
-                const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
+        for (int r = threadIdx.x >> 5; r < ROWS; r += NT / 32)
+        for (int j = threadIdx.x & 31; j < n; j += 32) {
+            if (s_iy[r] >= 0) {
                 const int m = (p.mode == X_DST1) ? j + 1 : j;
                 const C z = F[r * LP + (m >> 1)];
-                ro[iy * p.rin_py + iz * p.rin_pz + j] = (m & 1) ? z.y : z.x;
+                ro[s_rin[r] + j] = (m & 1) ? z.y : z.x;
             }
         }
     }
