@@ -385,6 +385,32 @@ def max_over_ranks(values, world, device):
     return [float(v) for v in tt.cpu()]
 
 
+def run_tc_probe():
+    """one radix-16 stage of the 256-point transform as butterflies (variant 0), as a 3 x TF32
+    tcgen05.mma (variant 1) and as a single TF32 product (variant 2); same data, same kernel body around the stage."""
+    import torch
+
+    import paper_2301_01145_b200 as sf
+
+    tiles, reps = 148 * 2 * 8, 64
+    g = torch.Generator(device="cuda").manual_seed(1)
+    src = torch.randn((tiles, 16, 512, 2), generator=g, device="cuda", dtype=torch.float32)
+    dst = torch.empty_like(src)
+    ref = None
+    out = {"probe": "sf_probe_dft16_stage", "tiles": tiles, "stages_per_tile": reps, "variants": {}}
+    for variant, name in ((0, "fp32 pipe: exchange + radix-16 butterflies"), (1, "tcgen05.mma kind::tf32, 3 x TF32 split"),
+                          (2, "tcgen05.mma kind::tf32, single product")):
+        ms = min(sf.sf_probe_dft16_stage(variant, reps, tiles, src, dst) for _ in range(5))
+        res = dst.double()
+        if ref is None:
+            ref = res.clone()
+        err = float((res - ref).norm() / ref.norm())
+        out["variants"][str(variant)] = {"what": name, "ms": ms, "ns_per_tile_stage_per_sm": ms * 1e6 * 148 / (tiles * reps),
+                                         "rel_l2_vs_variant_0": err}
+    print(json.dumps(out), flush=True)
+    return 0
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -593,7 +619,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tc-probe", action="store_true",
+                    help="time the radix-16 exchange + DFT stage on the fp32 pipe and on the tensor cores (sf_probe_dft16_stage) and exit")
     args = ap.parse_args()
+    if args.tc_probe:
+        return run_tc_probe()
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

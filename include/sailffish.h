@@ -231,6 +231,21 @@ sf_status sf_get_output_async(sf_plan plan, int field, int comp, void* dst_host)
  * stream after this call completes after them): for callers that time or order work on that stream. */
 sf_status sf_pipeline_join(sf_plan plan);
 
+/*
+ * sf_probe_dft16_stage -- measurement aid, not part of the solve: the one stage of the 1-D pencil transforms
+ * that could run as a matrix product, implemented three ways on the same data so that the choice
+ * "no tensor cores" rests on a measurement.  A tile is 512 threads x 16 complex fp32 values;
+ * value q of thread (o, lane) is handed to thread (q, lane), which computes the 16-point DFT over o of what it
+ * received (times 1/4), `reps` times over.
+ *   variant 0: shared-memory exchange + radix-16 butterflies on the fp32 pipe (what the library's kernels do);
+ *   variant 1: tcgen05.mma kind::tf32 with the 3 x TF32 split (fp32-level accuracy), accumulators in tensor memory;
+ *   variant 2: one TF32 product only (1e-3 accuracy; the ceiling of the tensor path).
+ *   in_dev / out_dev  [device] ntiles * 16 * 512 complex fp32, element q of thread t of tile i at (i * 16 + q) * 512 + t.
+ *   ms      [host, written] device time of one launch (CUDA events, second of two launches).
+ * Runs on the legacy default stream and blocks.  Errors: INVALID_ARG, CUDA.
+ */
+sf_status sf_probe_dft16_stage(int variant, int reps, int ntiles, const void* in_dev, void* out_dev, float* ms);
+
 /* Number of kernels the last compute call launched (for launch accounting in benchmarks). */
 int sf_last_launch_count(sf_plan plan);
 

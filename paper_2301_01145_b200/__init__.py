@@ -30,7 +30,7 @@ SF_OUT_PSI, SF_OUT_GRAD, SF_OUT_CURL, SF_OUT_DIV, SF_OUT_LAP = 0, 1, 2, 3, 4
 EXPORTS = (
     "sf_plan_create", "sf_set_source", "sf_set_bc_values", "sf_solve", "sf_gradient", "sf_curl",
     "sf_divergence", "sf_laplacian", "sf_get_output", "sf_output_device_ptr", "sf_synchronize",
-    "sf_set_pipeline", "sf_get_output_async", "sf_pipeline_join", "sf_last_launch_count", "sf_device_bytes",
+    "sf_set_pipeline", "sf_get_output_async", "sf_pipeline_join", "sf_probe_dft16_stage", "sf_last_launch_count", "sf_device_bytes",
     "sf_enable_step_timing", "sf_step_times_ms", "sf_set_step_timing_stride", "sf_last_error", "sf_plan_destroy", "sf_version",
 )
 
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
         L.sf_set_pipeline.argtypes = [vp, i]
         L.sf_get_output_async.argtypes = [vp, i, i, vp]
         L.sf_pipeline_join.argtypes = [vp]
+        L.sf_probe_dft16_stage.argtypes = [i, i, i, vp, vp, C.POINTER(C.c_float)]
         L.sf_last_launch_count.argtypes = [vp]
         L.sf_device_bytes.argtypes = [vp]
         L.sf_device_bytes.restype = ll
@@ -185,6 +186,17 @@ def sf_get_output_async(plan, field, comp, dst):
     if where != SF_MEM_HOST:
         raise ValueError("sf_get_output_async copies to host memory")
     _check(plan, lib().sf_get_output_async(plan, int(field), int(comp), a))
+
+
+def sf_probe_dft16_stage(variant, reps, ntiles, src, dst) -> float:
+    """(see include/sailffish.h) returns the device time of one launch in milliseconds"""
+    a, wa = _addr(src)
+    b, wb = _addr(dst)
+    if wa != SF_MEM_DEVICE or wb != SF_MEM_DEVICE:
+        raise ValueError("the probe works on device buffers")
+    ms = C.c_float(0.0)
+    _check(None, lib().sf_probe_dft16_stage(int(variant), int(reps), int(ntiles), a, b, C.byref(ms)))
+    return float(ms.value)
 
 
 def sf_pipeline_join(plan):

@@ -1373,6 +1373,15 @@ sf_status sf_pipeline_join(sf_plan plan)
     return SF_OK;
 }
 
+sf_status sf_probe_dft16_stage(int variant, int reps, int ntiles, const void* in_dev, void* out_dev, float* ms)
+{
+    if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return fail(nullptr, SF_ERR_CUDA, "set-up of the fast path failed"); }
+    const cudaError_t e = sf2::probe_dft16_stage(variant, reps, ntiles, in_dev, out_dev, ms, nullptr);
+    if (e == cudaErrorInvalidValue) { cudaGetLastError(); return fail(nullptr, SF_ERR_INVALID_ARG, "probe: bad argument"); }
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(nullptr, SF_ERR_CUDA, std::string("probe: ") + cudaGetErrorString(e)); }
+    return SF_OK;
+}
+
 int sf_last_launch_count(sf_plan plan) { return plan ? plan->launches : 0; }
 long long sf_device_bytes(sf_plan plan) { return plan ? plan->dev_bytes : 0; }
 

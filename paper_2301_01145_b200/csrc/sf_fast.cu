@@ -5,6 +5,7 @@
 #include "sf_fast512.cuh"
 #include "sf_fast2p.cuh"
 #include "sf_fast64.cuh"
+#include "sf_tcprobe.cuh"
 
 #include <cmath>
 #include <cstdlib>

@@ -173,4 +173,7 @@ cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st);
 cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st);
 cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st);
 
+// tensor-core probe (sf_tcprobe.cuh): `reps` applications of one radix-16 exchange + DFT stage on `ntiles` tiles
+cudaError_t probe_dft16_stage(int variant, int reps, int ntiles, const void* in, void* out, float* ms, cudaStream_t st);
+
 } // namespace sf2

@@ -71,16 +71,20 @@ template <typename T, int L> __host__ __device__ constexpr int x_lp()
 }
 
 // value of the (folded) source at (ix, iy, iz)
+// (only the two x faces depend on the position in the row; whether the row lies in a y / z boundary layer is the
+// same for all its elements and is tested first)
 template <typename T> __device__ __forceinline__ T x_src(const XParams<T>& p, const T* row, int ix, int iy, int iz)
 {
     T v = row[ix];
     if (p.has_faces) {
         if (ix == 0 && p.face[0]) v += p.wface[0] * p.face[0][iy + (long long)p.ny * iz];
         if (ix == p.n - 1 && p.face[1]) v += p.wface[1] * p.face[1][iy + (long long)p.ny * iz];
-        if (iy == 0 && p.face[2]) v += p.wface[2] * p.face[2][ix + (long long)p.n * iz];
-        if (iy == p.ny - 1 && p.face[3]) v += p.wface[3] * p.face[3][ix + (long long)p.n * iz];
-        if (iz == 0 && p.face[4]) v += p.wface[4] * p.face[4][ix + (long long)p.n * iy];
-        if (iz == p.nz - 1 && p.face[5]) v += p.wface[5] * p.face[5][ix + (long long)p.n * iy];
+        if (iy == 0 || iy == p.ny - 1 || iz == 0 || iz == p.nz - 1) {
+            if (iy == 0 && p.face[2]) v += p.wface[2] * p.face[2][ix + (long long)p.n * iz];
+            if (iy == p.ny - 1 && p.face[3]) v += p.wface[3] * p.face[3][ix + (long long)p.n * iz];
+            if (iz == 0 && p.face[4]) v += p.wface[4] * p.face[4][ix + (long long)p.n * iy];
+            if (iz == p.nz - 1 && p.face[5]) v += p.wface[5] * p.face[5][ix + (long long)p.n * iy];
+        }
     }
     return v;
 }
@@ -117,16 +121,28 @@ __global__ void __launch_bounds__(NT) xfwd_kernel(const XParams<T> p)
     const long long row0 = (long long)blockIdx.x * ROWS;
     const long long nrows = (long long)p.ny * p.nz;
     const T* rin = p.real_in + comp * p.rin_pc;
+    // row geometry once per row (the 64-bit divisions and pitch products do not belong in the element loops)
+    __shared__ int s_iy[16], s_iz[16];
+    __shared__ long long s_rin[16], s_sp[16];
+    if (threadIdx.x < ROWS) {
+        const long long row = row0 + threadIdx.x;
+        const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
+        s_iy[threadIdx.x] = (row < nrows) ? iy : -1;
+        s_iz[threadIdx.x] = iz;
+        s_rin[threadIdx.x] = iy * p.rin_py + iz * p.rin_pz;
+        s_sp[threadIdx.x] = iy * p.sp_py + iz * p.sp_pz;
+    }
+    __syncthreads();
 
     // load + extend + fold (position index fastest: coalesced)
     const bool fast = (p.mode == X_PERIODIC || p.mode == X_ZEROPAD) && !p.has_faces;
     for (int idx = threadIdx.x; idx < ROWS * L; idx += NT) {
         const int r = idx / L, j = idx % L;
-        const long long row = row0 + r;
         C z = mk<T>(0, 0);
-        if (row < nrows) {
-            const int iy = (int)(row % p.ny), iz = (int)(row / p.ny);
-            const T* rp = rin + iy * p.rin_py + iz * p.rin_pz;
+        const int iy = s_iy[r];
+        if (iy >= 0) {
+            const int iz = s_iz[r];
+            const T* rp = rin + s_rin[r];
             if (fast) {
                 if (2 * j < p.n) z = *reinterpret_cast<const C*>(rp + 2 * j);
             } else {
