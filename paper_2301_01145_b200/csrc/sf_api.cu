@@ -12,6 +12,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <utility>
 #include <vector>
 
@@ -87,6 +88,7 @@ struct sf_plan_s {
     bool fast5_x = false;  // S1 / S5 too (x extent 512)
     // ... and in double precision with 256-long y and z pencils (sf_fast64.cuh), scalar
     bool fast64 = false;
+    bool xg64 = false;     // fp64 X passes with complex length 256: zero-padded 256, DST-I 255, DCT-II / III 256 (sf_fastx64.cuh)
 
     // per-solve state
     const void* src = nullptr;
@@ -466,6 +468,22 @@ template <typename T> sf_status build_tables(sf_plan p)
     return SF_OK;
 }
 
+// S1 / S5: kernel generation 2 where the plan has it, generation 1 otherwise
+template <typename T> cudaError_t x_forward(sf_plan p, const XParams<T>& xp, int ncomp, cudaStream_t st)
+{
+    if constexpr (std::is_same<T, double>::value) {
+        if (p->xg64 && !xp.nyq_side) return sf2::launch_fast_xg(false, xp, ncomp, st);
+    }
+    return launch_xfwd<T>(p->Lx, xp, ncomp, st);
+}
+template <typename T> cudaError_t x_backward(sf_plan p, const XParams<T>& xp, int nf, cudaStream_t st)
+{
+    if constexpr (std::is_same<T, double>::value) {
+        if (p->xg64 && !xp.nyq_side && !xp.dfield1) return sf2::launch_fast_xg(true, xp, nf, st);
+    }
+    return launch_xinv<T>(p->Lx, xp, nf, st);
+}
+
 // ---------------------------------------------------------------- the solve sequence
 template <typename T> sf_status run(sf_plan p, int outk)
 {
@@ -530,7 +548,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
     } else {
         if (p->fastper && (outk == OUT_SOLVE || outk == OUT_GRAD)) xp.nyq_side = p->nyqA;
         if (p->fast && outk == OUT_SOLVE && p->nyqA) { xp.nyq_side = p->nyqA; xp.nyq_side_yz = 1; }   // [y][z], as fast_x_kernel writes it
-        SF_CUDA(p, launch_xfwd<T>(p->Lx, xp, ncomp, st));
+        SF_CUDA(p, x_forward<T>(p, xp, ncomp, st));
         xp.nyq_side = nullptr; xp.nyq_side_yz = 0;
     }
     p->launches++;
@@ -588,7 +606,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
             SF_CUDA(p, sf2::launch_fast_x(true, fx, st));
         } else {
             if (side) { xp.nyq_side = p->nyqA; xp.nyq_side_yz = 1; }
-            SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+            SF_CUDA(p, x_backward<T>(p, xp, nf_out, st));
             xp.nyq_side = nullptr; xp.nyq_side_yz = 0;
         }
         p->launches++;
@@ -631,7 +649,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         p->launches++;
         mark(4);
         xp.spec_in = p->W1; xp.real_out = (T*)p->out;
-        SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+        SF_CUDA(p, x_backward<T>(p, xp, nf_out, st));
         p->launches++;
         mark(5);
         if (timed) p->tcount++;
@@ -678,7 +696,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
             fx.reverse = 1;       // S4 wrote the last planes last
             SF_CUDA(p, sf2::launch_fast_x5(true, fx, st));
         } else {
-            SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+            SF_CUDA(p, x_backward<T>(p, xp, nf_out, st));
         }
         p->launches++;
         mark(5);
@@ -733,7 +751,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
             px.nyq = (sf2::C*)p->nyqA;
             SF_CUDA(p, sf2::launch_fast_xper(true, px, st));
         } else {
-            SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+            SF_CUDA(p, x_backward<T>(p, xp, nf_out, st));
         }
         p->launches++;
         mark(5);
@@ -804,7 +822,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
     xp.spec_in = p->W1; xp.real_out = (T*)p->out;
     xp.kap_ext = (const T*)p->kap_ext[0];
     xp.dfield1 = (p->r2r != R2R_NONE && outk == OUT_GRAD) ? 2 : 0;       // field 1 = d psi / dx
-    SF_CUDA(p, launch_xinv<T>(p->Lx, xp, nf_out, st));
+    SF_CUDA(p, x_backward<T>(p, xp, nf_out, st));
     p->launches++;
     mark(5);
     if (timed) p->tcount++;
@@ -1108,6 +1126,12 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         if ((st = dev_alloc(p, &p->nyqA, (size_t)p->nfields * p->n[1] * p->n[2] * 8)) != SF_OK) return bail(st, "");   // Nyquist column [field][z][y]
         p->fastper = true;
         p->fastper_x = (p->n[0] == 256) && !getenv("SF_DISABLE_FAST_X");
+    }
+    // fp64 X passes of generation 2: rows whose extended sequence is 512 long
+    if (prec == SF_F64 && p->Lx == 256 && (p->xmode == X_ZEROPAD || p->xmode == X_DST1 || p->xmode == X_DCT2) && !getenv("SF_DISABLE_FAST") &&
+        !getenv("SF_DISABLE_FAST_X")) {
+        if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fast path failed"); }
+        p->xg64 = true;
     }
     // everything the plan built (uploads on the legacy stream, kernels and memsets on the plan's stream) is complete
     // before the first compute call can be enqueued

@@ -6,6 +6,7 @@
 #include "sf_fast2p.cuh"
 #include "sf_fast64.cuh"
 #include "sf_tcprobe.cuh"
+#include "sf_fastx64.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -271,6 +272,36 @@ cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st)
     if (inv) fast_xper_kernel<true><<<grid, kXpThreads, kXpSmem, st>>>(p);
     else fast_xper_kernel<false><<<grid, kXpThreads, kXpSmem, st>>>(p);
     return cudaGetLastError();
+}
+
+namespace {
+template <int MODE> cudaError_t launch_xg_mode(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st)
+{
+    const long long ntiles = ((long long)p.ny * p.nz + kXgRows - 1) / kXgRows;
+    long long gx = 3ll * g_sms;
+    if (gx > ntiles) gx = ntiles;
+    const dim3 grid((unsigned)gx, (unsigned)ncomp);
+    cudaError_t e;
+    if (inv) {
+        if ((e = cudaFuncSetAttribute(fast_xg_kernel<MODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXgSmem)) != cudaSuccess) return e;
+        fast_xg_kernel<MODE, true><<<grid, kXgThreads, kXgSmem, st>>>(p);
+    } else {
+        if ((e = cudaFuncSetAttribute(fast_xg_kernel<MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXgSmem)) != cudaSuccess) return e;
+        fast_xg_kernel<MODE, false><<<grid, kXgThreads, kXgSmem, st>>>(p);
+    }
+    return cudaGetLastError();
+}
+} // namespace
+
+cudaError_t launch_fast_xg(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st)
+{
+    if (p.nyq_side || p.dfield1 || p.ny <= 0 || p.nz <= 0 || ncomp <= 0 || g_sms <= 0) return cudaErrorInvalidValue;
+    switch (p.mode) {
+    case sf::X_ZEROPAD: return p.n == 256 ? launch_xg_mode<sf::X_ZEROPAD>(inv, p, ncomp, st) : cudaErrorInvalidValue;
+    case sf::X_DST1: return p.n == 255 ? launch_xg_mode<sf::X_DST1>(inv, p, ncomp, st) : cudaErrorInvalidValue;
+    case sf::X_DCT2: return (p.n == 256 && p.ptw) ? launch_xg_mode<sf::X_DCT2>(inv, p, ncomp, st) : cudaErrorInvalidValue;
+    default: return cudaErrorInvalidValue;
+    }
 }
 
 cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st)

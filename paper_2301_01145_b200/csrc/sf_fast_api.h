@@ -3,6 +3,10 @@
 #pragma once
 #include <cuda_runtime.h>
 
+namespace sf {
+template <typename T> struct XParams;   // sf_xpass.cuh
+}
+
 namespace sf2 {
 
 typedef float2 C;
@@ -172,6 +176,10 @@ cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st);
 // launch one periodic strided pass (mode = FMODE_*) as a persistent grid of two CTAs per SM
 cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st);
 cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st);
+
+// S1 (inv = false) / S5 (inv = true) in double precision for rows whose extended sequence is 512 long (fast_xg_kernel,
+// sf_fastx64.cuh): p.mode X_ZEROPAD (n = 256), X_DST1 (n = 255) or X_DCT2 (n = 256); no side array, no differentiated field
+cudaError_t launch_fast_xg(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st);
 
 // tensor-core probe (sf_tcprobe.cuh): `reps` applications of one radix-16 exchange + DFT stage on `ntiles` tiles
 cudaError_t probe_dft16_stage(int variant, int reps, int ntiles, const void* in, void* out, float* ms, cudaStream_t st);

@@ -1,0 +1,238 @@
+// sf_fastx64.cuh -- kernel generation 2 for the X passes S1 / S5 in double precision, rows whose extended real
+// sequence has length 512 (complex transform length 256): zero-padded rows of 256 (unbounded plans),
+// DST-I rows of 255 (Dirichlet, cell-boundary grid) and DCT-II / DCT-III rows of 256 (Neumann, cell-centre grid;
+// Table 1, boundary values folded into the source on load).
+//
+// Same steps as sf_xpass.cuh (extension rule on load, packed real transform with split / merge, extraction rule on
+// store; XParams and the folded source x_src are shared with it), with the register-resident 256-point transform
+// of sf_fast.cuh in the middle: a CTA of 128 threads owns 8 contiguous rows; thread (o, row) holds the 16 packed
+// elements n = o + 16 r of its row, radix-16 in registers, twiddle, one exchange through shared memory, radix-16
+// in registers.  The rows are staged in shared memory both ways so that every global access is a coalesced run
+// along a row (a warp per row), and the index rules of the boundary conditions touch shared memory only.  The
+// exchange buffer and the staged spectrum rows share their storage: 57 KB per CTA, three CTAs per SM; persistent
+// grid over the row tiles.
+#pragma once
+#include "sf_fast64.cuh"
+#include "sf_xpass.cuh"
+
+namespace sf2 {
+
+constexpr int kXgThreads = 128;
+constexpr int kXgRows = 8;
+constexpr int kXgRP = 258;     // doubles per staged real row: 2064 B = 16 (mod 128)
+constexpr int kXgSP = 257;     // complex doubles per staged spectrum row: 4112 B = 16 (mod 128)
+constexpr size_t kXgSmem = (size_t)kXgRows * kXgRP * sizeof(double) + (size_t)kXgRows * kXgSP * sizeof(D);
+static_assert(((size_t)kXgRows * kXgRP * sizeof(double)) % 64 == 0 && (size_t)kXgRows * kXgSP >= 16 * 16 * 8, "staging layout");
+
+// extended sequence x~[m], m < 512, from the staged row (the rules of sf_xpass.cuh: x_ext)
+template <int MODE> __device__ __forceinline__ double xg_ext(const double* row, int m, int n)
+{
+    if constexpr (MODE == sf::X_ZEROPAD) {
+        return m < n ? row[m] : 0.0;
+    } else if constexpr (MODE == sf::X_DST1) {
+        if (m == 0 || m == n + 1) return 0.0;
+        return m <= n ? row[m - 1] : -row[511 - m];
+    } else {   // X_DCT2
+        return m < n ? row[m] : row[511 - m];
+    }
+}
+
+template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 3) fast_xg_kernel(const sf::XParams<double> p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* rbuf = reinterpret_cast<double*>(smem_raw);                                         // [8][kXgRP] reals
+    D* sbuf = reinterpret_cast<D*>(smem_raw + (size_t)kXgRows * kXgRP * sizeof(double));       // [8][kXgSP] complex
+    D* xbuf = sbuf;                                                                             // exchange [16 q][16 o][8 rows]
+    __shared__ __align__(16) D s_t256[256];   // [o][q] = w256^(q o)
+    __shared__ __align__(16) D s_tsp[136];    // w512^k, k <= 128
+    __shared__ int s_iy[kXgRows], s_iz[kXgRows];
+    __shared__ long long s_rin[kXgRows], s_sp[kXgRows];
+
+    const int tid = threadIdx.x;
+    const int row = tid & 7;
+    const int o = tid >> 3;
+    const int warp = tid >> 5, lane = tid & 31;
+    const int comp = blockIdx.y;
+    const int n = p.n;
+    for (int i = tid; i < 256; i += kXgThreads) s_t256[i] = c_tw1024d[(4 * (i & 15) * (i >> 4)) & 1023];
+    for (int i = tid; i <= 128; i += kXgThreads) s_tsp[i] = c_tw1024d[2 * i];
+    const D* t256 = s_t256 + o * 16;
+    double* rrow = rbuf + row * kXgRP;
+    D* srow = sbuf + row * kXgSP;
+    D* xw = xbuf + (o * 8 + row);            // slot (q, o) at stride 128
+    const D* xr = xbuf + (o * 128 + row);    // slot (o, o') at stride 8
+
+    const long long nrows = (long long)p.ny * p.nz;
+    const long long ntiles = (nrows + kXgRows - 1) / kXgRows;
+    const double* rin = INV ? nullptr : p.real_in + comp * p.rin_pc;
+
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const long long row0 = tile * kXgRows;
+        __syncthreads();   // the previous tile's stores have read the staged rows; (first tile: the tables are in place)
+        if (tid < kXgRows) {
+            const long long r = row0 + tid;
+            const int iy = (int)(r % p.ny), iz = (int)(r / p.ny);
+            s_iy[tid] = (r < nrows) ? iy : -1;
+            s_iz[tid] = iz;
+            s_rin[tid] = iy * p.rin_py + iz * p.rin_pz;
+            s_sp[tid] = iy * p.sp_py + iz * p.sp_pz;
+        }
+        __syncthreads();
+        D v[16];
+        if constexpr (!INV) {
+            // ---------------------------------------------------------------- S1
+            // stage the (folded) source rows: a warp per row, lanes along the row
+            for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
+                const int iy = s_iy[r];
+                double* dst = rbuf + r * kXgRP;
+                if (iy >= 0) {
+                    // all loads of the row first (n <= 256: eight per lane), then the boundary terms and the stores
+                    const double* rp = rin + s_rin[r];
+                    double t[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) t[j] = (lane + 32 * j < n) ? __ldg(rp + lane + 32 * j) : 0.0;
+                    if (p.has_faces) {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            if (lane + 32 * j < n) t[j] += sf::x_face_term(p, lane + 32 * j, iy, s_iz[r]);
+                    }
+#pragma unroll
+                    for (int j = 0; j < 8; ++j)
+                        if (lane + 32 * j < n) dst[lane + 32 * j] = t[j];
+                } else {
+                    for (int ix = lane; ix < n; ix += 32) dst[ix] = 0.0;
+                }
+            }
+            __syncthreads();
+            // packed extended sequence z[nn] = x~[2 nn] + i x~[2 nn + 1], nn = o + 16 r
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const int nn = o + 16 * r;
+                if (MODE == sf::X_ZEROPAD && r >= 8) v[r] = make_double2(0.0, 0.0);
+                else v[r] = make_double2(xg_ext<MODE>(rrow, 2 * nn, n), xg_ext<MODE>(rrow, 2 * nn + 1, n));
+            }
+            dft16<false>(v);
+#pragma unroll
+            for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul(v[brev4(q)], t256[q]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) xw[q * 128] = v[brev4(q)];
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = xr[j * 8];
+            dft16<false>(v);
+            __syncthreads();   // everyone has read the exchange buffer: its storage becomes the spectrum rows
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) srow[o + 16 * k2] = v[brev4(k2)];   // Z[k], natural order
+            __syncthreads();
+            // split in place: X[k] = ((Z[k] + conj Z[256-k]) - i w512^k (Z[k] - conj Z[256-k])) / 2, pairs (k, 256 - k)
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const int k = o + 16 * m;
+                if (m < 8 || o == 0) {
+                    const D zk = srow[k], zm = srow[(256 - k) & 255];
+                    const D e = make_double2(zk.x + zm.x, zk.y - zm.y);
+                    const D d = make_double2(zk.x - zm.x, zk.y + zm.y);
+                    const D wd = cmul(d, s_tsp[k]);
+                    srow[k] = make_double2(0.5 * (e.x + wd.y), 0.5 * (e.y - wd.x));
+                    srow[256 - k] = make_double2(0.5 * (e.x - wd.y), 0.5 * (-e.y - wd.x));
+                }
+            }
+            __syncthreads();
+            // extraction rule and store, a warp per row
+            for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
+                if (s_iy[r] < 0) continue;
+                const D* sr = sbuf + r * kXgSP;
+                if constexpr (MODE == sf::X_ZEROPAD) {
+                    D* so = reinterpret_cast<D*>(p.spec_out) + comp * p.sp_pc + s_sp[r];
+                    for (int k = lane; k <= 256; k += 32) so[k] = sr[k];
+                } else {
+                    double* ro = p.real_out + comp * p.sp_pc + s_sp[r];
+                    for (int k = lane; k < n; k += 32) {
+                        if constexpr (MODE == sf::X_DST1) {
+                            ro[k] = -sr[k + 1].y;                        // DST-I: Y_k = -Im X~[k+1]
+                        } else {
+                            const D w = __ldg(p.ptw + k), x = sr[k];     // DCT-II: Y_k = Re(e^{-i pi k / 2n} X~[k])
+                            ro[k] = w.x * x.x - w.y * x.y;
+                        }
+                    }
+                }
+            }
+        } else {
+            // ---------------------------------------------------------------- S5
+            // half spectrum X~[0..256] of the extended sequence into the staged rows, a warp per row
+            for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
+                D* sr = sbuf + r * kXgSP;
+                const bool valid = s_iy[r] >= 0;
+                if constexpr (MODE == sf::X_ZEROPAD) {
+                    const D* si = reinterpret_cast<const D*>(p.spec_in) + comp * p.sp_pc + s_sp[r];
+                    D t[9];
+#pragma unroll
+                    for (int j = 0; j < 9; ++j) t[j] = (valid && lane + 32 * j <= 256) ? ldg_d(si + lane + 32 * j) : make_double2(0.0, 0.0);
+#pragma unroll
+                    for (int j = 0; j < 9; ++j)
+                        if (lane + 32 * j <= 256) sr[lane + 32 * j] = t[j];
+                } else {
+                    const double* ri = reinterpret_cast<const double*>(p.spec_in) + comp * p.sp_pc + s_sp[r];
+                    for (int k = lane; k <= 256; k += 32) {
+                        D x = make_double2(0.0, 0.0);
+                        if (valid) {
+                            if constexpr (MODE == sf::X_DST1) {
+                                if (k >= 1 && k <= n) x = make_double2(0.0, -ri[k - 1]);     // X~[k] = -i Y[k-1]
+                            } else if (k < n) {
+                                const D w = __ldg(p.ptw + k);                                // X~[k] = e^{+i pi k / 2n} Y[k]
+                                const double y = ri[k];
+                                x = make_double2(w.x * y, -w.y * y);
+                            }
+                        }
+                        sr[k] = x;
+                    }
+                }
+            }
+            __syncthreads();
+            // merge in place: Z[k] = (X[k] + conj X[256-k]) + i conj(w512^k) (X[k] - conj X[256-k]), pairs (k, 256 - k)
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const int k = o + 16 * m;
+                if (m < 8 || o == 0) {
+                    const D xk = srow[k], xm = srow[256 - k];
+                    const D e = make_double2(xk.x + xm.x, xk.y - xm.y);
+                    const D d = make_double2(xk.x - xm.x, xk.y + xm.y);
+                    const D wd = cmulc(d, s_tsp[k]);
+                    srow[k] = make_double2(e.x - wd.y, e.y + wd.x);
+                    if (k > 0) srow[256 - k] = make_double2(e.x + wd.y, wd.x - e.y);
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = srow[o + 16 * j];
+            __syncthreads();   // the spectrum rows are in registers: their storage becomes the exchange buffer
+            dft16<true>(v);
+#pragma unroll
+            for (int q = 1; q < 16; ++q) v[brev4(q)] = cmulc(v[brev4(q)], t256[q]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) xw[q * 128] = v[brev4(q)];
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = xr[j * 8];
+            dft16<true>(v);
+            // unpack z[nn] = (x~[2 nn], x~[2 nn + 1]), nn = o + 16 k2; the stored unknowns lie in x~[0 .. 256)
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) {
+                const int nn = o + 16 * k2;
+                rrow[2 * nn] = v[brev4(k2)].x;
+                rrow[2 * nn + 1] = v[brev4(k2)].y;
+            }
+            __syncthreads();
+            // extraction rule and store, a warp per row: x_j = x~[j] (zero-padded, DCT) or x~[j + 1] (DST-I)
+            double* ro = p.real_out + comp * p.rin_pc;
+            for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
+                if (s_iy[r] < 0) continue;
+                const double* src = rbuf + r * kXgRP + (MODE == sf::X_DST1 ? 1 : 0);
+                double* dst = ro + s_rin[r];
+                for (int j = lane; j < n; j += 32) dst[j] = src[j];
+            }
+        }
+    }
+}
+
+} // namespace sf2

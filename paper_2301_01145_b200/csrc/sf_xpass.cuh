@@ -73,19 +73,23 @@ template <typename T, int L> __host__ __device__ constexpr int x_lp()
 // value of the (folded) source at (ix, iy, iz)
 // (only the two x faces depend on the position in the row; whether the row lies in a y / z boundary layer is the
 // same for all its elements and is tested first)
+template <typename T> __device__ __forceinline__ T x_face_term(const XParams<T>& p, int ix, int iy, int iz)
+{
+    T v = (T)0;
+    if (ix == 0 && p.face[0]) v += p.wface[0] * p.face[0][iy + (long long)p.ny * iz];
+    if (ix == p.n - 1 && p.face[1]) v += p.wface[1] * p.face[1][iy + (long long)p.ny * iz];
+    if (iy == 0 || iy == p.ny - 1 || iz == 0 || iz == p.nz - 1) {
+        if (iy == 0 && p.face[2]) v += p.wface[2] * p.face[2][ix + (long long)p.n * iz];
+        if (iy == p.ny - 1 && p.face[3]) v += p.wface[3] * p.face[3][ix + (long long)p.n * iz];
+        if (iz == 0 && p.face[4]) v += p.wface[4] * p.face[4][ix + (long long)p.n * iy];
+        if (iz == p.nz - 1 && p.face[5]) v += p.wface[5] * p.face[5][ix + (long long)p.n * iy];
+    }
+    return v;
+}
 template <typename T> __device__ __forceinline__ T x_src(const XParams<T>& p, const T* row, int ix, int iy, int iz)
 {
     T v = row[ix];
-    if (p.has_faces) {
-        if (ix == 0 && p.face[0]) v += p.wface[0] * p.face[0][iy + (long long)p.ny * iz];
-        if (ix == p.n - 1 && p.face[1]) v += p.wface[1] * p.face[1][iy + (long long)p.ny * iz];
-        if (iy == 0 || iy == p.ny - 1 || iz == 0 || iz == p.nz - 1) {
-            if (iy == 0 && p.face[2]) v += p.wface[2] * p.face[2][ix + (long long)p.n * iz];
-            if (iy == p.ny - 1 && p.face[3]) v += p.wface[3] * p.face[3][ix + (long long)p.n * iz];
-            if (iz == 0 && p.face[4]) v += p.wface[4] * p.face[4][ix + (long long)p.n * iy];
-            if (iz == p.nz - 1 && p.face[5]) v += p.wface[5] * p.face[5][ix + (long long)p.n * iy];
-        }
-    }
+    if (p.has_faces) v += x_face_term(p, ix, iy, iz);
     return v;
 }
 
