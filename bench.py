@@ -102,7 +102,8 @@ def step_names(wname):
     if wname == "cfg4_unbounded_256_f64":
         return ["S1 fast_xg_kernel<fwd>", "S2 fast64_kernel<FWD>", "S3 fast64_kernel<FUSED>", "S4 fast64_kernel<INV>", "S5 fast_xg_kernel<inv>"]
     if wname in ("cfg3_dirichlet_255_f64", "cfg3_neumann_256_f64"):
-        return ["S1 fast_xg_kernel<fwd>", "S2 spass_kernel<0>", "S3 spass_kernel<2>", "S4 spass_kernel<1>", "S5 fast_xg_kernel<inv>"]
+        return ["S1 fast_xg_kernel<fwd>", "S2 fast_r2r64_kernel<FWD>", "S3 fast_r2r64_kernel<FUSED>",
+                "S4 fast_r2r64_kernel<" + ("FWD" if "dirichlet" in wname else "INV") + ">", "S5 fast_xg_kernel<inv>"]
     if wname in ("cfg2_periodic_256_f32", "cfg2_periodic_256_f32_grad"):
         return ["S1 fast_xper_kernel<fwd>", "S2 fast_per_kernel<FWD>", "S3 fast_per_kernel<FUSED>", "S4 fast_per_kernel<INV>",
                 "S5 fast_xper_kernel<inv>"]

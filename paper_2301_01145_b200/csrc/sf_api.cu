@@ -88,6 +88,7 @@ struct sf_plan_s {
     bool fast5_x = false;  // S1 / S5 too (x extent 512)
     // ... and in double precision with 256-long y and z pencils (sf_fast64.cuh), scalar
     bool fast64 = false;
+    bool r2r64 = false;    // fp64 Dirichlet (DST-I, 255) / Neumann (DCT, 256) strided passes (sf_fastr2r64.cuh)
     bool xg64 = false;     // fp64 X passes with complex length 256: zero-padded 256, DST-I 255, DCT-II / III 256 (sf_fastx64.cuh)
 
     // per-solve state
@@ -617,6 +618,42 @@ template <typename T> sf_status run(sf_plan p, int outk)
         return SF_OK;
     }
 
+    if (p->r2r64 && outk == OUT_SOLVE) {
+        // kernel generation 2 for the real-to-real strided passes, in place on W1 (pairs of real columns as complex columns)
+        sf2::FastR64Params fp;
+        memset(&fp, 0, sizeof(fp));
+        const int kind = (p->r2r == R2R_DST1) ? 0 : 1;
+        const long long hc = hp / 2;
+        fp.sched = (int*)p->sched;
+        fp.in = (const double2*)p->W1; fp.out = (double2*)p->W1;
+        fp.n = n1; fp.nct = (int)(hp / 16); fp.nx = p->nspec_x;
+        // S2 along y: batches = z planes
+        fp.in_ps = fp.out_ps = hc; fp.in_bs = fp.out_bs = hc * n1; fp.nb = n2; fp.batch_dim = 2;
+        SF_CUDA(p, sf2::launch_fast_r2r64(kind, 0, fp, p->map_s2, st));
+        p->launches++;
+        mark(2);
+        // S3 along z: batches = ky
+        fp.in_ps = fp.out_ps = hc * n1; fp.in_bs = fp.out_bs = hc; fp.nb = n1; fp.batch_dim = 1; fp.n = n2;
+        fp.lam_x = (const double*)p->lam[0]; fp.lam_b = (const double*)p->lam[1]; fp.lam_p = (const double*)p->lam[2];
+        fp.scale = p->scale; fp.zero_mode = sp.zero_mode;
+        SF_CUDA(p, sf2::launch_fast_r2r64(kind, 2, fp, p->map_s3, st));
+        p->launches++;
+        mark(3);
+        // S4 along y (DST-I: the same transform again; DCT: DCT-III)
+        fp.in_ps = fp.out_ps = hc; fp.in_bs = fp.out_bs = hc * n1; fp.nb = n2; fp.batch_dim = 2; fp.n = n1;
+        SF_CUDA(p, sf2::launch_fast_r2r64(kind, kind == 0 ? 0 : 1, fp, p->map_s2, st));
+        p->launches++;
+        mark(4);
+        xp.spec_in = p->W1; xp.real_out = (T*)p->out;
+        SF_CUDA(p, x_backward<T>(p, xp, nf_out, st));
+        p->launches++;
+        mark(5);
+        if (timed) p->tcount++;
+        p->last_kind = outk;
+        p->out_last = p->out;
+        return SF_OK;
+    }
+
     if (p->fast64 && outk == OUT_SOLVE) {
         // kernel generation 2 in double precision: S2, S3, S4 as persistent TMA-fed register-FFT kernels (tiles of 8 columns)
         sf2::Fast64Params fp;
@@ -1126,6 +1163,22 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         if ((st = dev_alloc(p, &p->nyqA, (size_t)p->nfields * p->n[1] * p->n[2] * 8)) != SF_OK) return bail(st, "");   // Nyquist column [field][z][y]
         p->fastper = true;
         p->fastper_x = (p->n[0] == 256) && !getenv("SF_DISABLE_FAST_X");
+    }
+    // fp64 Dirichlet / Neumann plans with 255- / 256-long y and z pencils: generation-2 strided passes
+    if (prec == SF_F64 && ndim == 3 && ncomp == 1 && !getenv("SF_DISABLE_FAST") &&
+        ((p->r2r == R2R_DST1 && p->n[1] == 255 && p->n[2] == 255) || (p->r2r == R2R_DCT && p->n[1] == 256 && p->n[2] == 256))) {
+        if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fast path failed"); }
+        // the real work array as 8-byte words: (column, y, z); a tile is 16 words x all rows of a pencil
+        const unsigned long long hpw = (unsigned long long)p->pitch, hpB = hpw * 8ull, N1 = (unsigned long long)p->n[1], N2 = (unsigned long long)p->n[2];
+        const unsigned long long d[4] = { hpw, N1, N2, 1 }, sb[3] = { hpB, hpB * N1, hpB * N1 * N2 };
+        const unsigned bx2[4] = { 16, (unsigned)N1, 1, 1 }, bx3[4] = { 16, 1, (unsigned)N2, 1 };
+        if (sf2::fast_make_map(&p->map_s2, p->W1, d, sb, bx2) != cudaSuccess || sf2::fast_make_map(&p->map_s3, p->W1, d, sb, bx3) != cudaSuccess)
+            return bail(SF_ERR_CUDA, "tensor map encoding failed");
+        if (!p->sched) {
+            if ((st = dev_alloc(p, &p->sched, 2 * sizeof(int))) != SF_OK) return bail(st, "");
+            if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
+        }
+        p->r2r64 = true;
     }
     // fp64 X passes of generation 2: rows whose extended sequence is 512 long
     if (prec == SF_F64 && p->Lx == 256 && (p->xmode == X_ZEROPAD || p->xmode == X_DST1 || p->xmode == X_DCT2) && !getenv("SF_DISABLE_FAST") &&

@@ -7,6 +7,7 @@
 #include "sf_fast64.cuh"
 #include "sf_tcprobe.cuh"
 #include "sf_fastx64.cuh"
+#include "sf_fastr2r64.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -235,6 +236,36 @@ cudaError_t launch_fast64(int mode, const Fast64Params& p, const TileMap& in_map
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
+}
+
+namespace {
+template <int KIND, int MODE> cudaError_t launch_r64(const FastR64Params& p, const CUtensorMap& tm, int grid, cudaStream_t st)
+{
+    cudaError_t e = cudaFuncSetAttribute(fast_r2r64_kernel<KIND, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemR64);
+    if (e != cudaSuccess) return e;
+    fast_r2r64_kernel<KIND, MODE><<<grid, kT64, kSmemR64, st>>>(p, tm);
+    return cudaGetLastError();
+}
+} // namespace
+
+cudaError_t launch_fast_r2r64(int kind, int mode, const FastR64Params& p, const TileMap& in_map, cudaStream_t st)
+{
+    const CUtensorMap& tm = reinterpret_cast<const CUtensorMap&>(in_map);
+    if (p.nb <= 0 || p.nct <= 0 || (kind == R2RK_DST1 && p.n != 255) || (kind == R2RK_DCT && p.n != 256)) return cudaErrorInvalidValue;
+    if (kind == R2RK_DST1 && mode == RMODE_INV) return cudaErrorInvalidValue;   // DST-I is its own inverse: use RMODE_FWD
+    if (mode == RMODE_FUSED && (!p.lam_x || !p.lam_b || !p.lam_p)) return cudaErrorInvalidValue;
+    const long long ntiles = (long long)p.nb * p.nct;
+    if (ntiles + 4ll * g_sms >= (1ll << 31)) return cudaErrorInvalidValue;
+    int grid = 2 * g_sms;
+    if (grid > ntiles) grid = (int)ntiles;
+    if (kind == R2RK_DST1) {
+        if (mode == RMODE_FWD) return launch_r64<R2RK_DST1, RMODE_FWD>(p, tm, grid, st);
+        return launch_r64<R2RK_DST1, RMODE_FUSED>(p, tm, grid, st);
+    }
+    if (mode == RMODE_FWD) return launch_r64<R2RK_DCT, RMODE_FWD>(p, tm, grid, st);
+    if (mode == RMODE_INV) return launch_r64<R2RK_DCT, RMODE_INV>(p, tm, grid, st);
+    if (mode == RMODE_FUSED) return launch_r64<R2RK_DCT, RMODE_FUSED>(p, tm, grid, st);
+    return cudaErrorInvalidValue;
 }
 
 cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st)

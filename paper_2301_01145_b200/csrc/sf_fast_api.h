@@ -177,6 +177,26 @@ cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st);
 cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st);
 cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st);
 
+// strided passes of fp64 Dirichlet (DST-I, 255 rows) / Neumann (DCT-II / III, 256 rows) plans (fast_r2r64_kernel,
+// sf_fastr2r64.cuh): the real work array is addressed as complex columns (pairs of real columns), tiles of 8
+struct FastR64Params {
+    const double2* in;
+    double2* out;
+    long long in_ps, in_bs, out_ps, out_bs;   // row and batch strides in complex columns (= real strides / 2)
+    int n;                      // stored rows per pencil: 255 (DST-I) or 256 (DCT)
+    int nb;                     // batches
+    int nct;                    // 8-column tiles per batch (pitch / 16)
+    int batch_dim;              // 2: the tensor map is (column, row, batch); 1: (column, batch, row)
+    int* sched;
+    // fused: scale / (lam_x[real column] + lam_b[batch] + lam_p[row]); zero mode -> 0
+    const double* lam_x; const double* lam_b; const double* lam_p;
+    int nx;                     // valid real columns
+    double scale;
+    int zero_mode;
+};
+// kind 0: DST-I, 1: DCT;  mode 0: forward (x -> Y), 1: backward (DCT-III; DST-I uses forward), 2: fused S3
+cudaError_t launch_fast_r2r64(int kind, int mode, const FastR64Params& p, const TileMap& in_map, cudaStream_t st);
+
 // S1 (inv = false) / S5 (inv = true) in double precision for rows whose extended sequence is 512 long (fast_xg_kernel,
 // sf_fastx64.cuh): p.mode X_ZEROPAD (n = 256), X_DST1 (n = 255) or X_DCT2 (n = 256); no side array, no differentiated field
 cudaError_t launch_fast_xg(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st);

@@ -261,6 +261,38 @@ def test_cfg3_neumann_full_size():
     assert e_res <= 1e-10   # measured 3e-14
 
 
+@pytest.mark.parametrize("kind,nx,op", [("dirichlet", 31, "fd2"), ("dirichlet", 63, "ps"), ("neumann", 64, "fd2"),
+                                        ("neumann", 16, "ps")])
+def test_r2r64_fast_path_white_noise_narrow_x(kind, nx, op):
+    """the generation-2 real-to-real strided passes (sf_fastr2r64.cuh: y and z pencils of 255 / 256, fp64) with an x extent
+    whose pitch holds padding columns, white noise, both operators, anisotropic spacing, solved twice (persistent-kernel
+    state), against the oracle and per plane"""
+    ny = 255 if kind == "dirichlet" else 256
+    shape = (ny, ny, nx)
+    f = W.Rng(6100 + nx).normal(int(np.prod(shape))).reshape(shape)
+    h = (0.011, 0.007, 0.009)
+    oop = O.OP_FD2 if op == "fd2" else O.OP_PS
+    sop = sf.SF_OP_FD2 if op == "fd2" else sf.SF_OP_PSEUDO_SPECTRAL
+    if kind == "dirichlet":
+        ref = O.dirichlet_regular(f, h, None, op=oop)
+        bc, grid = sf.SF_BC_DIRICHLET, sf.SF_GRID_CELL_BOUNDARY
+    else:
+        f = f - f.mean()
+        ref = O.neumann_staggered(f, h, None, op=oop)
+        bc, grid = sf.SF_BC_NEUMANN, sf.SF_GRID_CELL_CENTRE
+    with Plan(shape, h, bc, grid=grid, op=sop, prec="f64") as p:
+        p.set_source(f)
+        for _ in range(2):
+            sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI)
+    if kind == "neumann":
+        got, ref = got - got.mean(), ref - ref.mean()
+    _check(f"psi {kind} {ny}x{ny}x{nx} {op} f64 white noise", got, ref, "f64")
+    err = np.linalg.norm((got - ref).reshape(ny, -1), axis=1)
+    nrm = np.linalg.norm(ref.reshape(ny, -1), axis=1)
+    assert (err <= 10 * TOL["f64"] * nrm).all()
+
+
 def _gauss2_vec(r, eps):
     """the order-2 regularised kernel for an array of distances (reading A10), restated here for the
     sampled sums below and checked against the oracle's scalar routine where it is used"""
