@@ -117,23 +117,24 @@ def step_names(wname):
 # are used only while that hash matches the sources of this checkout: a changed kernel turns "issue_view" and
 # "traffic" into null instead of letting them go stale silently.
 ISSUE_SLOTS_PER_CLOCK = 148 * 4
-KERNEL_SOURCE_GLOBS = ("paper_2301_01145_b200/csrc/*.cu", "paper_2301_01145_b200/csrc/*.cuh", "paper_2301_01145_b200/csrc/*.h")
-
-
-def kernel_source_hash():
+def kernel_source_hash(files):
+    """SHA-256 over the named kernel sources (paths relative to the repo root, in the given order)"""
     import hashlib
 
     hsh = hashlib.sha256()
-    files = sorted(f for g in KERNEL_SOURCE_GLOBS for f in ROOT.glob(g))
-    for f in files:
-        hsh.update(f.name.encode())
+    for name in files:
+        f = ROOT / name
+        if not f.exists():
+            return None
+        hsh.update(Path(name).name.encode())
         hsh.update(f.read_bytes())
     return hsh.hexdigest()
 
 
 def ncu_counts(wname, step_index):
-    """the committed ncu counts of step `step_index` of a workload, or None when there is no capture or the kernel
-    sources have changed since it was taken"""
+    """the committed ncu counts of step `step_index` of a workload (profiles/ncu_counts.json: per workload the kernel
+    source files the capture was taken from, their SHA-256, and per step the counts), or None when there is no capture
+    or one of those sources has changed since"""
     f = ROOT / "profiles" / "ncu_counts.json"
     if not f.exists():
         return None
@@ -141,9 +142,13 @@ def ncu_counts(wname, step_index):
         doc = json.load(open(f))
     except Exception:
         return None
-    if doc.get("kernel_sources_sha256") != kernel_source_hash():
+    w = doc.get("workloads", {}).get(wname)
+    if not w or kernel_source_hash(w.get("sources", [])) != w.get("sources_sha256"):
         return None
-    return doc.get("workloads", {}).get(wname, {}).get(f"S{step_index + 1}")
+    c = w.get(f"S{step_index + 1}")
+    if c is not None:
+        c = dict(c, capture=w.get("capture"))
+    return c
 
 
 def issue_view(wname, dom, kernel_ms, clocks, names):

@@ -309,7 +309,7 @@ namespace {
 template <int MODE> cudaError_t launch_xg_mode(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st)
 {
     const long long ntiles = ((long long)p.ny * p.nz + kXgRows - 1) / kXgRows;
-    long long gx = 3ll * g_sms;
+    long long gx = 4ll * g_sms;
     if (gx > ntiles) gx = ntiles;
     const dim3 grid((unsigned)gx, (unsigned)ncomp);
     cudaError_t e;

@@ -9,7 +9,7 @@
 // elements n = o + 16 r of its row, radix-16 in registers, twiddle, one exchange through shared memory, radix-16
 // in registers.  The rows are staged in shared memory both ways so that every global access is a coalesced run
 // along a row (a warp per row), and the index rules of the boundary conditions touch shared memory only.  The
-// exchange buffer and the staged spectrum rows share their storage: 57 KB per CTA, three CTAs per SM; persistent
+// exchange buffer and the staged spectrum rows and the staged real rows all share one 33 KB region (they are never live together): four CTAs per SM; persistent
 // grid over the row tiles.
 #pragma once
 #include "sf_fast64.cuh"
@@ -21,8 +21,9 @@ constexpr int kXgThreads = 128;
 constexpr int kXgRows = 8;
 constexpr int kXgRP = 258;     // doubles per staged real row: 2064 B = 16 (mod 128)
 constexpr int kXgSP = 257;     // complex doubles per staged spectrum row: 4112 B = 16 (mod 128)
-constexpr size_t kXgSmem = (size_t)kXgRows * kXgRP * sizeof(double) + (size_t)kXgRows * kXgSP * sizeof(D);
-static_assert(((size_t)kXgRows * kXgRP * sizeof(double)) % 64 == 0 && (size_t)kXgRows * kXgSP >= 16 * 16 * 8, "staging layout");
+// the staged real rows, the exchange buffer and the staged spectrum rows are never live together: one region
+constexpr size_t kXgSmem = (size_t)kXgRows * kXgSP * sizeof(D);
+static_assert((size_t)kXgRows * kXgRP * sizeof(double) <= kXgSmem && (size_t)kXgRows * kXgSP >= 16 * 16 * 8, "staging layout");
 
 // extended sequence x~[m], m < 512, from the staged row (the rules of sf_xpass.cuh: x_ext)
 template <int MODE> __device__ __forceinline__ double xg_ext(const double* row, int m, int n)
@@ -37,11 +38,11 @@ template <int MODE> __device__ __forceinline__ double xg_ext(const double* row, 
     }
 }
 
-template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 3) fast_xg_kernel(const sf::XParams<double> p)
+template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 4) fast_xg_kernel(const sf::XParams<double> p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* rbuf = reinterpret_cast<double*>(smem_raw);                                         // [8][kXgRP] reals
-    D* sbuf = reinterpret_cast<D*>(smem_raw + (size_t)kXgRows * kXgRP * sizeof(double));       // [8][kXgSP] complex
+    D* sbuf = reinterpret_cast<D*>(smem_raw);                                                   // [8][kXgSP] complex, same storage
     D* xbuf = sbuf;                                                                             // exchange [16 q][16 o][8 rows]
     __shared__ __align__(16) D s_t256[256];   // [o][q] = w256^(q o)
     __shared__ __align__(16) D s_tsp[136];    // w512^k, k <= 128
@@ -106,11 +107,20 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 3) f
             __syncthreads();
             // packed extended sequence z[nn] = x~[2 nn] + i x~[2 nn + 1], nn = o + 16 r
 #pragma unroll
+            // (n = 255 or 256: for r < 8 both positions 2 nn, 2 nn + 1 <= 255 lie in the stored half of the extension, for
+            // r >= 8 in the mirrored / padded half -- the rules of xg_ext resolved at compile time)
             for (int r = 0; r < 16; ++r) {
                 const int nn = o + 16 * r;
-                if (MODE == sf::X_ZEROPAD && r >= 8) v[r] = make_double2(0.0, 0.0);
-                else v[r] = make_double2(xg_ext<MODE>(rrow, 2 * nn, n), xg_ext<MODE>(rrow, 2 * nn + 1, n));
+                if (r < 8) {
+                    if (MODE == sf::X_DST1) v[r] = make_double2(nn == 0 ? 0.0 : rrow[max(2 * nn - 1, 0)], rrow[2 * nn]);
+                    else v[r] = make_double2(rrow[2 * nn], rrow[2 * nn + 1]);
+                } else {
+                    if (MODE == sf::X_ZEROPAD) v[r] = make_double2(0.0, 0.0);
+                    else if (MODE == sf::X_DST1) v[r] = make_double2(nn == 128 ? 0.0 : -rrow[min(511 - 2 * nn, 254)], -rrow[510 - 2 * nn]);
+                    else v[r] = make_double2(rrow[511 - 2 * nn], rrow[510 - 2 * nn]);
+                }
             }
+            __syncthreads();   // the staged rows are in registers: their storage becomes the exchange buffer
             dft16<false>(v);
 #pragma unroll
             for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul(v[brev4(q)], t256[q]);
@@ -214,6 +224,7 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 3) f
             __syncthreads();
 #pragma unroll
             for (int j = 0; j < 16; ++j) v[j] = xr[j * 8];
+            __syncthreads();   // the exchange buffer has been read: its storage becomes the staged real rows
             dft16<true>(v);
             // unpack z[nn] = (x~[2 nn], x~[2 nn + 1]), nn = o + 16 k2; the stored unknowns lie in x~[0 .. 256)
 #pragma unroll
