@@ -103,6 +103,7 @@ struct sf_plan_s {
     int tstride = 1;              // record every tstride-th compute call
     bool fastper = false;         // periodic fp32 plans with 256-point y / z pencils: generation-2 strided passes
     bool fastper_x = false;       // ... and rows of 256 reals: generation-2 X passes
+    bool fastper64 = false;       // the same strided passes in double precision (sf_fastper64.cuh)
     long long tcalls = 0;         // compute calls seen since timing was enabled
     std::vector<cudaEvent_t> ev;  // 6 events per slot
     // copy pipeline (sf_set_pipeline): host copies on streams of their own, two source and two result buffers
@@ -547,7 +548,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         px.nyq = (sf2::C*)p->nyqA;
         SF_CUDA(p, sf2::launch_fast_xper(false, px, st));
     } else {
-        if (p->fastper && (outk == OUT_SOLVE || outk == OUT_GRAD)) xp.nyq_side = p->nyqA;
+        if ((p->fastper || p->fastper64) && (outk == OUT_SOLVE || outk == OUT_GRAD)) xp.nyq_side = p->nyqA;
         if (p->fast && outk == OUT_SOLVE && p->nyqA) { xp.nyq_side = p->nyqA; xp.nyq_side_yz = 1; }   // [y][z], as fast_x_kernel writes it
         SF_CUDA(p, x_forward<T>(p, xp, ncomp, st));
         xp.nyq_side = nullptr; xp.nyq_side_yz = 0;
@@ -735,6 +736,50 @@ template <typename T> sf_status run(sf_plan p, int outk)
         } else {
             SF_CUDA(p, x_backward<T>(p, xp, nf_out, st));
         }
+        p->launches++;
+        mark(5);
+        if (timed) p->tcount++;
+        p->last_kind = outk;
+        p->out_last = p->out;
+        return SF_OK;
+    }
+
+    if (p->fastper64 && (outk == OUT_SOLVE || outk == OUT_GRAD)) {
+        // kernel generation 2, periodic, double precision: S2, S3, S4 in place on W1 (tiles of 16 columns)
+        sf2::FastPer64Params fp;
+        memset(&fp, 0, sizeof(fp));
+        fp.sched = (int*)p->sched;
+        fp.in = (const double2*)p->W1; fp.out = (double2*)p->W1;
+        fp.nx = p->nspec_x;
+        fp.nct = p->nspec_x / 16;
+        fp.nyq_col = (p->nspec_x % 16) ? fp.nct * 16 : -1;
+        fp.nyq = (double2*)p->nyqA;
+        fp.in_ps = fp.out_ps = hp; fp.in_bs = fp.out_bs = hp * n1; fp.nb = n2;
+        fp.nyq_ps = 1; fp.nyq_bs = n1;
+        SF_CUDA(p, sf2::launch_fast_per64(sf2::FMODE_FWD, fp, st));
+        p->launches++;
+        mark(2);
+        fp.in_ps = fp.out_ps = hp * n1; fp.in_bs = fp.out_bs = hp; fp.nb = n1;
+        fp.nyq_ps = n1; fp.nyq_bs = 1;
+        fp.lam_x = (const double*)p->lam[0]; fp.lam_b = (const double*)p->lam[1]; fp.lam_p = (const double*)p->lam[2];
+        fp.scale = p->scale; fp.zero_mode = 1;
+        if (outk == OUT_GRAD) {
+            fp.grad = 1;
+            fp.kap_x = (const double*)p->kap[0]; fp.kap_b = (const double*)p->kap[1]; fp.kap_p = (const double*)p->kap[2];
+            fp.out_cs = p->w1_field; fp.nyq_cs = (long long)n1 * n2;
+        }
+        SF_CUDA(p, sf2::launch_fast_per64(sf2::FMODE_FUSED, fp, st));
+        fp.grad = 0;
+        p->launches++;
+        mark(3);
+        fp.in_ps = fp.out_ps = hp; fp.in_bs = fp.out_bs = hp * n1; fp.nb = n2 * nf_out;
+        fp.nyq_ps = 1; fp.nyq_bs = n1;
+        SF_CUDA(p, sf2::launch_fast_per64(sf2::FMODE_INV, fp, st));
+        p->launches++;
+        mark(4);
+        xp.spec_in = p->W1; xp.real_out = (T*)p->out;
+        xp.nyq_side = p->nyqA;
+        SF_CUDA(p, x_backward<T>(p, xp, nf_out, st));
         p->launches++;
         mark(5);
         if (timed) p->tcount++;
@@ -1164,6 +1209,15 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         p->fastper = true;
         p->fastper_x = (p->n[0] == 256) && !getenv("SF_DISABLE_FAST_X");
     }
+    // ... and the same in double precision
+    if (prec == SF_F64 && b == SF_BC_PERIODIC && ndim == 3 && ncomp == 1 && p->n[1] == 256 && p->n[2] == 256 && p->nspec_x >= 16 &&
+        (p->nspec_x % 16) <= 1 && p->n[0] <= 4096 && !getenv("SF_DISABLE_FAST")) {
+        if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fast path failed"); }
+        if ((st = dev_alloc(p, &p->sched, 2 * sizeof(int))) != SF_OK) return bail(st, "");
+        if (cudaMemsetAsync(p->sched, 0, 2 * sizeof(int), p->stream) != cudaSuccess) return bail(SF_ERR_CUDA, "memset failed");
+        if ((st = dev_alloc(p, &p->nyqA, (size_t)p->nfields * p->n[1] * p->n[2] * 16)) != SF_OK) return bail(st, "");   // Nyquist column [field][z][y]
+        p->fastper64 = true;
+    }
     // fp64 Dirichlet / Neumann plans with 255- / 256-long y and z pencils: generation-2 strided passes
     if (prec == SF_F64 && ndim == 3 && ncomp == 1 && !getenv("SF_DISABLE_FAST") &&
         ((p->r2r == R2R_DST1 && p->n[1] == 255 && p->n[2] == 255) || (p->r2r == R2R_DCT && p->n[1] == 256 && p->n[2] == 256))) {
@@ -1257,7 +1311,7 @@ sf_status sf_gradient(sf_plan plan)
         // the fused pass holds two tiles (psi and one derivative)
         const int ax = plan->ndim - 1;
         const size_t need = (plan->prec == SF_F32) ? spass_smem_bytes<float>(plan->La[ax], 2) : spass_smem_bytes<double>(plan->La[ax], 2);
-        if (need > 227 * 1024 && !plan->fastper)
+        if (need > 227 * 1024 && !plan->fastper && !plan->fastper64)
             return fail(plan, SF_ERR_UNSUPPORTED, "gradient: the fused pass does not fit in shared memory for this size / precision");
     }
     if (plan->bc == SF_BC_PERIODIC) return run_any(plan, OUT_GRAD);

@@ -8,6 +8,7 @@
 #include "sf_tcprobe.cuh"
 #include "sf_fastx64.cuh"
 #include "sf_fastr2r64.cuh"
+#include "sf_fastper64.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -288,6 +289,40 @@ cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st)
             fast_per_kernel<FMODE_FUSED, true><<<grid, kThreads, kPerSmem, st>>>(p);
         } else {
             fast_per_kernel<FMODE_FUSED><<<grid, kThreads, kPerSmem, st>>>(p);
+        }
+        break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fast_per64(int mode, const FastPer64Params& p, cudaStream_t st)
+{
+    if (p.nyq_col >= 0 && !p.nyq) return cudaErrorInvalidValue;
+    if (p.nct <= 0 || p.nb <= 0) return cudaErrorInvalidValue;
+    if (p.grad && mode != FMODE_FUSED) return cudaErrorInvalidValue;
+    if (mode == FMODE_FUSED && (!p.lam_x || !p.lam_b || !p.lam_p || (p.grad && (!p.kap_x || !p.kap_b || !p.kap_p)))) return cudaErrorInvalidValue;
+    const long long ntiles = (long long)p.nb * p.nct + (p.nyq_col >= 0 ? (p.nb + kPer64Tile - 1) / kPer64Tile : 0);
+    if (ntiles + 4ll * g_sms >= (1ll << 31)) return cudaErrorInvalidValue;
+    int grid = 2 * g_sms;
+    if (grid > ntiles) grid = (int)ntiles;
+    cudaError_t e = cudaSuccess;
+    switch (mode) {
+    case FMODE_FWD:
+        if ((e = cudaFuncSetAttribute(fast_per64_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPer64Smem)) != cudaSuccess) return e;
+        fast_per64_kernel<FMODE_FWD><<<grid, kT64, kPer64Smem, st>>>(p);
+        break;
+    case FMODE_INV:
+        if ((e = cudaFuncSetAttribute(fast_per64_kernel<FMODE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPer64Smem)) != cudaSuccess) return e;
+        fast_per64_kernel<FMODE_INV><<<grid, kT64, kPer64Smem, st>>>(p);
+        break;
+    case FMODE_FUSED:
+        if (p.grad) {
+            if ((e = cudaFuncSetAttribute(fast_per64_kernel<FMODE_FUSED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPer64Smem)) != cudaSuccess) return e;
+            fast_per64_kernel<FMODE_FUSED, true><<<grid, kT64, kPer64Smem, st>>>(p);
+        } else {
+            if ((e = cudaFuncSetAttribute(fast_per64_kernel<FMODE_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPer64Smem)) != cudaSuccess) return e;
+            fast_per64_kernel<FMODE_FUSED><<<grid, kT64, kPer64Smem, st>>>(p);
         }
         break;
     default: return cudaErrorInvalidValue;

@@ -177,6 +177,25 @@ cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st);
 cudaError_t launch_fast_per(int mode, const FastPerParams& p, cudaStream_t st);
 cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st);
 
+// strided passes of fp64 periodic plans with 256-point pencils (fast_per64_kernel, sf_fastper64.cuh): tiles of 16 columns
+struct FastPer64Params {
+    const double2* in;
+    double2* out;
+    long long in_ps, in_bs, out_ps, out_bs;   // row and batch strides, complex elements
+    int nb, nx, nct;            // batches, valid columns, full 16-column tiles per batch
+    int nyq_col;                // column handled 16 batches at a time, -1: none
+    int* sched;
+    double2* nyq;               // side array that holds column nyq_col: element (row, batch) at row * nyq_ps + batch * nyq_bs
+    long long nyq_ps, nyq_bs;
+    const double* lam_x; const double* lam_b; const double* lam_p;
+    double scale;
+    int zero_mode;
+    int grad;                   // fused mode: fields 1 .. 3 = d/dx, d/dy (batch axis), d/dz (pencil axis)
+    const double* kap_x; const double* kap_b; const double* kap_p;
+    long long out_cs, nyq_cs;   // field strides of out and of the side array
+};
+cudaError_t launch_fast_per64(int mode, const FastPer64Params& p, cudaStream_t st);
+
 // strided passes of fp64 Dirichlet (DST-I, 255 rows) / Neumann (DCT-II / III, 256 rows) plans (fast_r2r64_kernel,
 // sf_fastr2r64.cuh): the real work array is addressed as complex columns (pairs of real columns), tiles of 8
 struct FastR64Params {

@@ -463,3 +463,33 @@ def test_periodic_fast_path_white_noise(nx, op, monkeypatch):
     nrm = np.linalg.norm(ref.reshape(256, -1), axis=1)
     assert (err <= 10 * TOL["f32"] * nrm).all()
     assert rel_l2(got["generation 2"], got["generation 1"].astype(np.float64)) <= 1e-6
+
+
+@pytest.mark.parametrize("nx,op", [(32, "fd2"), (64, "ps"), (256, "fd2")])
+def test_periodic_fast_path_f64_white_noise(nx, op):
+    """the same in double precision (sf_fastper64.cuh: 16-column tiles plus the Nyquist column; the gradient parks
+    psi_hat in tensor memory): sf_solve, sf_gradient, sf_solve again on one plan, against the oracle, plane by plane"""
+    shape = (256, 256, nx)
+    f = W.Rng(7100 + nx).normal(int(np.prod(shape))).reshape(shape)
+    f -= f.mean()
+    L = (2.0, 1.0, 3.0)
+    h = (L[0] / nx, L[1] / 256, L[2] / 256)
+    oop, sop = (O.OP_PS, sf.SF_OP_PSEUDO_SPECTRAL) if op == "ps" else (O.OP_FD2, sf.SF_OP_FD2)
+    ref, grad_o = O.periodic(f, L, oop, rhs_sign=-1.0, want_grad=True)
+    with Plan(shape, h, sf.SF_BC_PERIODIC, op=sop, prec="f64", rhs_sign=-1.0) as p:
+        p.set_source(f)
+        for _ in range(3):
+            sf.sf_solve(p.plan)
+        got = p.get(sf.SF_OUT_PSI)
+        _check(f"periodic 256x256x{nx} {op} f64", got, ref, "f64")
+        sf.sf_gradient(p.plan)
+        _check("psi (gradient call)", p.get(sf.SF_OUT_PSI), ref, "f64")
+        for a in range(3):
+            _check(f"grad[{a}]", p.get(sf.SF_OUT_GRAD, a), grad_o[a], "f64")
+        sf.sf_gradient(p.plan)
+        _check("grad[2] (again)", p.get(sf.SF_OUT_GRAD, 2), grad_o[2], "f64")
+        sf.sf_solve(p.plan)
+        _check("psi (solve again)", p.get(sf.SF_OUT_PSI), ref, "f64")
+    err = np.linalg.norm((got - ref).reshape(256, -1), axis=1)
+    nrm = np.linalg.norm(ref.reshape(256, -1), axis=1)
+    assert (err <= 10 * TOL["f64"] * nrm).all()
