@@ -108,7 +108,7 @@ def step_names(wname):
         return ["S1 fast_xper_kernel<fwd>", "S2 fast_per_kernel<FWD>", "S3 fast_per_kernel<FUSED>", "S4 fast_per_kernel<INV>",
                 "S5 fast_xper_kernel<inv>"]
     if wname == "cfg2_periodic_256_f64_grad":
-        return ["S1 xfwd_kernel", "S2 fast_per64_kernel<FWD>", "S3 fast_per64_kernel<FUSED,GRAD>", "S4 fast_per64_kernel<INV>", "S5 xinv_kernel"]
+        return ["S1 fast_xp64_kernel<fwd>", "S2 fast_per64_kernel<FWD>", "S3 fast_per64_kernel<FUSED,GRAD>", "S4 fast_per64_kernel<INV>", "S5 fast_xp64_kernel<inv>"]
     if wname == "cfg5_vector_512_f32_curl":
         return ["S1 fast_x5_kernel<fwd>", "S2 fast5_kernel<FWD>", "S3 fast5_kernel<CURL>", "S4 fast5_kernel<INV>", "S5 fast_x5_kernel<inv>"]
     return ["S1 xfwd_kernel", "S2 spass_kernel<0>", "S3 spass_kernel<2>", "S4 spass_kernel<1>", "S5 xinv_kernel"]

@@ -89,6 +89,7 @@ struct sf_plan_s {
     // ... and in double precision with 256-long y and z pencils (sf_fast64.cuh), scalar
     bool fast64 = false;
     bool r2r64 = false;    // fp64 Dirichlet (DST-I, 255) / Neumann (DCT, 256) strided passes (sf_fastr2r64.cuh)
+    bool xp64 = false;     // fp64 periodic X passes for rows of 256 reals (sf_fastx64.cuh)
     bool xg64 = false;     // fp64 X passes with complex length 256: zero-padded 256, DST-I 255, DCT-II / III 256 (sf_fastx64.cuh)
 
     // per-solve state
@@ -475,6 +476,7 @@ template <typename T> cudaError_t x_forward(sf_plan p, const XParams<T>& xp, int
 {
     if constexpr (std::is_same<T, double>::value) {
         if (p->xg64 && !xp.nyq_side) return sf2::launch_fast_xg(false, xp, ncomp, st);
+        if (p->xp64 && !xp.nyq_side_yz && !xp.has_faces) return sf2::launch_fast_xp64(false, xp, ncomp, st);
     }
     return launch_xfwd<T>(p->Lx, xp, ncomp, st);
 }
@@ -482,6 +484,7 @@ template <typename T> cudaError_t x_backward(sf_plan p, const XParams<T>& xp, in
 {
     if constexpr (std::is_same<T, double>::value) {
         if (p->xg64 && !xp.nyq_side && !xp.dfield1) return sf2::launch_fast_xg(true, xp, nf, st);
+        if (p->xp64 && !xp.nyq_side_yz && !xp.dfield1) return sf2::launch_fast_xp64(true, xp, nf, st);
     }
     return launch_xinv<T>(p->Lx, xp, nf, st);
 }
@@ -1239,6 +1242,10 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         !getenv("SF_DISABLE_FAST_X")) {
         if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fast path failed"); }
         p->xg64 = true;
+    }
+    if (prec == SF_F64 && p->xmode == X_PERIODIC && p->n[0] == 256 && !getenv("SF_DISABLE_FAST") && !getenv("SF_DISABLE_FAST_X")) {
+        if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fast path failed"); }
+        p->xp64 = true;
     }
     // everything the plan built (uploads on the legacy stream, kernels and memsets on the plan's stream) is complete
     // before the first compute call can be enqueued

@@ -370,6 +370,25 @@ cudaError_t launch_fast_xg(bool inv, const sf::XParams<double>& p, int ncomp, cu
     }
 }
 
+cudaError_t launch_fast_xp64(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st)
+{
+    if (p.mode != sf::X_PERIODIC || p.n != 256 || p.nyq_side_yz || p.dfield1 || p.has_faces || p.ny <= 0 || p.nz <= 0 || ncomp <= 0 || g_sms <= 0)
+        return cudaErrorInvalidValue;
+    const long long ntiles = ((long long)p.ny * p.nz + kXp64Rows - 1) / kXp64Rows;
+    long long gx = 4ll * g_sms;
+    if (gx > ntiles) gx = ntiles;
+    const dim3 grid((unsigned)gx, (unsigned)ncomp);
+    cudaError_t e;
+    if (inv) {
+        if ((e = cudaFuncSetAttribute(fast_xp64_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXp64Smem)) != cudaSuccess) return e;
+        fast_xp64_kernel<true><<<grid, kXp64Threads, kXp64Smem, st>>>(p);
+    } else {
+        if ((e = cudaFuncSetAttribute(fast_xp64_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXp64Smem)) != cudaSuccess) return e;
+        fast_xp64_kernel<false><<<grid, kXp64Threads, kXp64Smem, st>>>(p);
+    }
+    return cudaGetLastError();
+}
+
 cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st)
 {
     if (p.nrows <= 0 || p.nrows % kX5Rows || p.spec_pitch < kX5SpPitch || p.nyq) return cudaErrorInvalidValue;

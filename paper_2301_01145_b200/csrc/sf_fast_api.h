@@ -220,6 +220,10 @@ cudaError_t launch_fast_r2r64(int kind, int mode, const FastR64Params& p, const 
 // sf_fastx64.cuh): p.mode X_ZEROPAD (n = 256), X_DST1 (n = 255) or X_DCT2 (n = 256); no side array, no differentiated field
 cudaError_t launch_fast_xg(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st);
 
+// the same for periodic fp64 rows of 256 reals (fast_xp64_kernel): p.mode X_PERIODIC, n = 256; the side array [field][row] of
+// the Nyquist coefficient is honoured when p.nyq_side is set
+cudaError_t launch_fast_xp64(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st);
+
 // tensor-core probe (sf_tcprobe.cuh): `reps` applications of one radix-16 exchange + DFT stage on `ntiles` tiles
 cudaError_t probe_dft16_stage(int variant, int reps, int ntiles, const void* in, void* out, float* ms, cudaStream_t st);
 

@@ -247,3 +247,174 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 4) f
 }
 
 } // namespace sf2
+
+namespace sf2 {
+
+// ==================================================================================== periodic rows of 256 reals, fp64
+// S1 (real-to-complex) / S5 (complex-to-real) of periodic plans (PAPER.md:87 half spectrum): the row is packed as
+// z[n] = x[2n] + i x[2n+1], n < 128; Z = DFT128(z) = radix-16 over r (n = w + 8 r) in registers, twiddle w128^(q w), one
+// exchange, two radix-8 (outputs k = w + 16 k2 and w + 8 + 16 k2); then the real-transform split to X[0..128].  A CTA of
+// 128 threads owns 16 rows (thread = (w, row)); staged real rows, exchange buffer and staged spectrum rows share one
+// 33 KB region.  X[128] goes to / comes from the side array of the strided passes when the plan has one.
+constexpr int kXp64Threads = 128;
+constexpr int kXp64Rows = 16;
+constexpr int kXp64RP = 258;     // doubles per staged real row
+constexpr int kXp64SP = 129;     // complex doubles per staged spectrum row (X[0..128])
+constexpr size_t kXp64Smem = (size_t)kXp64Rows * kXp64RP * sizeof(double);
+static_assert((size_t)kXp64Rows * kXp64SP * sizeof(D) <= kXp64Smem && (size_t)16 * 8 * 16 * sizeof(D) <= kXp64Smem, "one region");
+
+template <bool INV> __global__ void __launch_bounds__(kXp64Threads, 4) fast_xp64_kernel(const sf::XParams<double> p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* rbuf = reinterpret_cast<double*>(smem_raw);
+    D* sbuf = reinterpret_cast<D*>(smem_raw);
+    D* xbuf = sbuf;
+    __shared__ __align__(16) D s_t128[128];   // [w][q] = w128^(q w)
+    __shared__ __align__(16) D s_tsp[72];     // w256^k, k <= 64
+    __shared__ int s_ok[kXp64Rows];
+    __shared__ long long s_rin[kXp64Rows], s_sp[kXp64Rows];
+
+    const int tid = threadIdx.x;
+    const int row = tid & 15;
+    const int w = tid >> 4;
+    const int warp = tid >> 5, lane = tid & 31;
+    const int comp = blockIdx.y;
+    s_t128[tid] = c_tw1024d[(8 * (tid & 15) * (tid >> 4)) & 1023];
+    if (tid <= 64) s_tsp[tid] = c_tw1024d[4 * tid];
+    const D* t128 = s_t128 + w * 16;
+    double* rrow = rbuf + row * kXp64RP;
+    D* srow = sbuf + row * kXp64SP;
+    D* xw = xbuf + (w * 16 + row);                 // slot (q, w) at stride 128
+    const D* xra = xbuf + (w * 128 + row);         // slot (w, o') at stride 16
+    const D* xrb = xbuf + ((w + 8) * 128 + row);   // slot (w + 8, o')
+
+    const long long nrows = (long long)p.ny * p.nz;
+    const long long ntiles = (nrows + kXp64Rows - 1) / kXp64Rows;
+    D* nyq = reinterpret_cast<D*>(p.nyq_side);
+
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const long long row0 = tile * kXp64Rows;
+        __syncthreads();
+        if (tid < kXp64Rows) {
+            const long long r = row0 + tid;
+            const int iy = (int)(r % p.ny), iz = (int)(r / p.ny);
+            s_ok[tid] = r < nrows;
+            s_rin[tid] = iy * p.rin_py + iz * p.rin_pz;
+            s_sp[tid] = iy * p.sp_py + iz * p.sp_pz;
+        }
+        __syncthreads();
+        D v[16], a[8], b[8];
+        if constexpr (!INV) {
+            const double* rin = p.real_in + comp * p.rin_pc;
+            for (int r = warp; r < kXp64Rows; r += kXp64Threads / 32) {
+                double t[8];
+                const double* rp = rin + s_rin[r];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) t[j] = s_ok[r] ? __ldg(rp + lane + 32 * j) : 0.0;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) rbuf[r * kXp64RP + lane + 32 * j] = t[j];
+            }
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = make_double2(rrow[2 * (w + 8 * r)], rrow[2 * (w + 8 * r) + 1]);
+            __syncthreads();   // the staged rows are in registers: their storage becomes the exchange buffer
+            dft16<false>(v);
+#pragma unroll
+            for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul(v[brev4(q)], t128[q]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) xw[q * 128] = v[brev4(q)];
+            __syncthreads();
+#pragma unroll
+            for (int i = 0; i < 8; ++i) { a[i] = xra[i * 16]; b[i] = xrb[i * 16]; }
+            dft8<false>(a);
+            dft8<false>(b);
+            __syncthreads();   // the exchange buffer has been read: its storage becomes the spectrum rows
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) { srow[w + 16 * k2] = a[brev3(k2)]; srow[w + 8 + 16 * k2] = b[brev3(k2)]; }
+            __syncthreads();
+            // split in place: pairs (k, 128 - k), k = w + 8 m
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const int k = w + 8 * m;
+                if (m < 8 || w == 0) {
+                    const D zk = srow[k], zm = srow[(128 - k) & 127];
+                    const D e = make_double2(zk.x + zm.x, zk.y - zm.y);
+                    const D d = make_double2(zk.x - zm.x, zk.y + zm.y);
+                    const D wd = cmul(d, s_tsp[k]);
+                    srow[k] = make_double2(0.5 * (e.x + wd.y), 0.5 * (e.y - wd.x));
+                    srow[128 - k] = make_double2(0.5 * (e.x - wd.y), 0.5 * (-e.y - wd.x));
+                }
+            }
+            __syncthreads();
+            D* so = reinterpret_cast<D*>(p.spec_out) + comp * p.sp_pc;
+            for (int r = warp; r < kXp64Rows; r += kXp64Threads / 32) {
+                if (!s_ok[r]) continue;
+                const D* sr = sbuf + r * kXp64SP;
+                D* dst = so + s_sp[r];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dst[lane + 32 * j] = sr[lane + 32 * j];
+                if (lane == 0) {
+                    if (nyq) nyq[comp * nrows + row0 + r] = sr[128];
+                    else dst[128] = sr[128];
+                }
+            }
+        } else {
+            const D* si = reinterpret_cast<const D*>(p.spec_in) + comp * p.sp_pc;
+            for (int r = warp; r < kXp64Rows; r += kXp64Threads / 32) {
+                D* sr = sbuf + r * kXp64SP;
+                const D* src = si + s_sp[r];
+                D t[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) t[j] = s_ok[r] ? ldg_d(src + lane + 32 * j) : make_double2(0.0, 0.0);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) sr[lane + 32 * j] = t[j];
+                if (lane == 0) sr[128] = !s_ok[r] ? make_double2(0.0, 0.0) : (nyq ? nyq[comp * nrows + row0 + r] : src[128]);
+            }
+            __syncthreads();
+            // merge in place: Z[k] = (X[k] + conj X[128-k]) + i conj(w256^k) (X[k] - conj X[128-k])
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const int k = w + 8 * m;
+                if (m < 8 || w == 0) {
+                    const D xk = srow[k], xm = srow[128 - k];
+                    const D e = make_double2(xk.x + xm.x, xk.y - xm.y);
+                    const D d = make_double2(xk.x - xm.x, xk.y + xm.y);
+                    const D wd = cmulc(d, s_tsp[k]);
+                    srow[k] = make_double2(e.x - wd.y, e.y + wd.x);
+                    if (k > 0) srow[128 - k] = make_double2(e.x + wd.y, wd.x - e.y);
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = srow[w + 8 * j];
+            __syncthreads();
+            dft16<true>(v);
+#pragma unroll
+            for (int q = 1; q < 16; ++q) v[brev4(q)] = cmulc(v[brev4(q)], t128[q]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) xw[q * 128] = v[brev4(q)];
+            __syncthreads();
+#pragma unroll
+            for (int i = 0; i < 8; ++i) { a[i] = xra[i * 16]; b[i] = xrb[i * 16]; }
+            __syncthreads();
+            dft8<true>(a);
+            dft8<true>(b);
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) {
+                const int na = w + 16 * k2, nb = w + 8 + 16 * k2;
+                rrow[2 * na] = a[brev3(k2)].x; rrow[2 * na + 1] = a[brev3(k2)].y;
+                rrow[2 * nb] = b[brev3(k2)].x; rrow[2 * nb + 1] = b[brev3(k2)].y;
+            }
+            __syncthreads();
+            double* ro = p.real_out + comp * p.rin_pc;
+            for (int r = warp; r < kXp64Rows; r += kXp64Threads / 32) {
+                if (!s_ok[r]) continue;
+                double* dst = ro + s_rin[r];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) dst[lane + 32 * j] = rbuf[r * kXp64RP + lane + 32 * j];
+            }
+        }
+    }
+}
+
+} // namespace sf2
