@@ -268,6 +268,23 @@ def neumann_staggered(f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
     return psi
 
 
+KIND_DIRICHLET_BOUNDARY, KIND_NEUMANN_CENTRE, KIND_DIRICHLET_CENTRE, KIND_NEUMANN_BOUNDARY = 0, 1, 2, 3
+
+
+def bounded_mixed(kinds_xyz, f, h, faces=None, op=OP_FD2, rhs_sign=1.0):
+    """O-MIX.  Dirichlet / Neumann mixed per axis: kinds_xyz[a] selects the Table-1 row of axis a (KIND_* above;
+    0 and 3 live on the cell-boundary grid, 1 and 2 on the cell-centre grid).  Conventions as the uniform solvers."""
+    f = _f64(f)
+    nd, n = _dims(f.shape)
+    assert nd == 3
+    psi = np.empty_like(f)
+    arr, keep = _faces_arg(faces)
+    kk = (C.c_int * 3)(*[int(k) for k in kinds_xyz])
+    _chk(lib().orc_bounded_mixed(kk, _i64x3(n), _f64x3(h), C.c_int(op), C.c_double(rhs_sign), _ptr(f), arr, _ptr(psi)),
+         "bounded_mixed")
+    return psi
+
+
 def green_gauss2(r, eps):
     return float(lib().orc_green_gauss2(float(r), float(eps)))
 

@@ -783,6 +783,100 @@ done:
 }
 
 /* ------------------------------------------------------------------------------------------
+ * O-MIX: Dirichlet and Neumann conditions mixed per axis (PAPER.md:191-199 describes the approach --
+ * 1-D transforms chosen per direction -- and leaves it as future work).  Nothing new is computed:
+ * axis a uses the row of Table 1 that its own condition selects on the plan's grid type,
+ *   kind 0: Dirichlet, cell-boundary   DST-I  / DST-I    n interior nodes, L = (n+1) h, index k+1, norm 2 (n+1)
+ *   kind 1: Neumann,   cell-centre     DCT-II / DCT-III  n cells,          L = n h,     index k,   norm 2 n
+ *   kind 2: Dirichlet, cell-centre     DST-II / DST-III  n cells,          L = n h,     index k+1, norm 2 n
+ *   kind 3: Neumann,   cell-boundary   DCT-I  / DCT-I    n nodes,          L = (n-1) h, index k,   norm 2 (n-1)
+ * (kinds 0 and 3 share the cell-boundary grid, kinds 1 and 2 the cell-centre grid), its eigenvalue column and its
+ * fold weight (reading A18).  The zero mode exists only when every axis is Neumann.
+ * psi = B_z B_y B_x ( rhs_sign * F_x F_y F_z f' / (lam_x + lam_y + lam_z) ) / prod_a norm_a.
+ * ---------------------------------------------------------------------------------------- */
+int orc_bounded_mixed(const int kind[3], const i64 n[3], const double h[3], int op, double rhs_sign, const double *f,
+                      const double *const faces[6], double *psi)
+{
+    i64 tot = n[0] * n[1] * n[2];
+    trig_table tab[3];
+    double *lam[3] = { 0, 0, 0 };
+    real_xform fwd[3], bwd[3];
+    int err = ORC_OK, ntab = 0, all_neumann = 1;
+    double norm = 1.0;
+    for (int a = 0; a < 3; ++a)
+        if (kind[a] < 0 || kind[a] > 3) return ORC_ERR_ARG;
+    memcpy(psi, f, sizeof(double) * (size_t)tot);
+    /* fold the face values of every axis with the weight of that axis' own condition */
+    if (op == 1 && faces) {
+        i64 st[3] = { 1, n[0], n[0] * n[1] };
+        for (int axis = 0; axis < 3; ++axis) {
+            int a = (axis == 0) ? 1 : 0, b = (axis == 2) ? 1 : 2;
+            for (int side = 0; side < 2; ++side) {
+                const double *g = faces[2 * axis + side];
+                if (!g) continue;
+                i64 ic = side ? n[axis] - 1 : 0;
+                double w;
+                switch (kind[axis]) {
+                case 0: w = -1.0 / (h[axis] * h[axis]); break;
+                case 1: w = side ? -1.0 / h[axis] : +1.0 / h[axis]; break;
+                case 2: w = -2.0 / (h[axis] * h[axis]); break;
+                default: w = side ? -2.0 / h[axis] : +2.0 / h[axis]; break;
+                }
+                w /= rhs_sign;
+                for (i64 jb = 0; jb < n[b]; ++jb)
+                    for (i64 ja = 0; ja < n[a]; ++ja)
+                        psi[ic * st[axis] + ja * st[a] + jb * st[b]] += w * g[ja + n[a] * jb];
+            }
+        }
+    }
+    for (int a = 0; a < 3; ++a) {
+        i64 period, cells, shift;
+        switch (kind[a]) {
+        case 0: period = 2 * (n[a] + 1); cells = n[a] + 1; shift = 1; fwd[a] = dst1_tab; bwd[a] = dst1_tab; break;
+        case 1: period = 4 * n[a];       cells = n[a];     shift = 0; fwd[a] = dct2_tab; bwd[a] = dct3_tab; break;
+        case 2: period = 4 * n[a];       cells = n[a];     shift = 1; fwd[a] = dst2_tab; bwd[a] = dst3_tab; break;
+        default: period = 2 * (n[a] - 1); cells = n[a] - 1; shift = 0; fwd[a] = dct1_tab; bwd[a] = dct1_tab; break;
+        }
+        if (cells < 1) { err = ORC_ERR_ARG; goto done; }
+        if (kind[a] == 0 || kind[a] == 2) all_neumann = 0;
+        norm *= 2.0 * (double)cells;
+        if ((err = trig_table_init(&tab[a], (int)n[a], period)) != ORC_OK) { ntab = a + 1; goto done; }
+        ntab = a + 1;
+        lam[a] = (double *)malloc(sizeof(double) * (size_t)n[a]);
+        if (!lam[a]) { err = ORC_ERR_ALLOC; goto done; }
+        double Ldom = (double)cells * h[a];
+        for (i64 k = 0; k < n[a]; ++k) {
+            if (op == 0) {
+                double kk = PI * (double)(k + shift) / Ldom;
+                lam[a][k] = -kk * kk;
+            } else {
+                double sn, cs;
+                sincos2pi(k + shift, 4 * cells, &sn, &cs);   /* sin(pi (k + shift) / (2 cells)) */
+                lam[a][k] = -(4.0 / (h[a] * h[a])) * sn * sn;
+            }
+        }
+    }
+    for (int a = 0; a < 3; ++a)
+        if ((err = r2r_axis(psi, n, a, fwd[a], &tab[a])) != ORC_OK) goto done;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (i64 kz = 0; kz < n[2]; ++kz)
+        for (i64 ky = 0; ky < n[1]; ++ky)
+            for (i64 kx = 0; kx < n[0]; ++kx) {
+                i64 i = kx + n[0] * (ky + n[1] * kz);
+                if (all_neumann && kx == 0 && ky == 0 && kz == 0) { psi[i] = 0.0; continue; }
+                psi[i] = rhs_sign * psi[i] / (lam[0][kx] + lam[1][ky] + lam[2][kz]);
+            }
+    for (int a = 2; a >= 0; --a)
+        if ((err = r2r_axis(psi, n, a, bwd[a], &tab[a])) != ORC_OK) goto done;
+#pragma omp parallel for schedule(static)
+    for (i64 i = 0; i < tot; ++i) psi[i] /= norm;
+done:
+    for (int a = 0; a < ntab; ++a) trig_table_free(&tab[a]);
+    for (int a = 0; a < 3; ++a) free(lam[a]);
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------------
  * Spectral gradient on Dirichlet / Neumann plans (eq. (10), applied to the sine / cosine
  * series of Table 1; SURVEY f3 "sine <-> cosine on the inverse").  The solve gives the coefficients
  * c_k = rhs_sign * T_3(f') / Lambda of the series psi = (1/norm) S_3(c), S the synthesis (backward) sum of
