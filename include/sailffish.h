@@ -50,8 +50,12 @@ typedef enum {
     SF_ERR_STATE = -5        /* call out of order (solve before source, output before solve)    */
 } sf_status;
 
-/* Boundary condition per axis.  The paper's solvers use one type on all axes
- * (PAPER.md:126); mixed types return SF_ERR_UNSUPPORTED. */
+/* Boundary condition per axis.  The paper's solvers use one type on all axes and
+ * leave mixed conditions, by 1-D transforms chosen per direction, as future work.  Built here:
+ * Dirichlet and Neumann may be mixed freely per axis -- every axis takes the row of Table 1 that its
+ * own condition selects on the plan's grid type, its eigenvalue column and its boundary-value weights; the size rule
+ * of sf_plan_create applies per axis.  sf_solve only (sf_gradient returns UNSUPPORTED on such plans).  A periodic or
+ * unbounded axis next to another type returns SF_ERR_UNSUPPORTED. */
 typedef enum { SF_BC_PERIODIC = 0, SF_BC_DIRICHLET = 1, SF_BC_NEUMANN = 2, SF_BC_UNBOUNDED = 3 } sf_bc;
 
 /* Grid type (eq. 9): REGULAR = cell-boundary nodes, STAGGERED = cell centres. */
@@ -119,7 +123,7 @@ typedef struct {
  *   opt    [host] may be NULL (defaults above).
  * For unbounded plans this call evaluates G on the doubled grid, transforms it with the library's
  * own fp64 kernels and stores the real, even spectrum as a compact (n+1)^3 table.
- * Errors: INVALID_ARG, UNSUPPORTED (mixed BCs, sizes above, GREEN_SPECTRAL in 2-D, ncomp not 1 or 3,
+ * Errors: INVALID_ARG, UNSUPPORTED (a periodic / unbounded axis mixed with another type, sizes above, GREEN_SPECTRAL in 2-D, ncomp not 1 or 3,
  * PS/FD2 on unbounded or GREEN on bounded plans), ALLOC, CUDA.
  */
 sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const double h[3], const sf_bc bc[3],

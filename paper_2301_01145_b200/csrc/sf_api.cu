@@ -38,6 +38,9 @@ struct sf_plan_s {
     double h[3] = { 1, 1, 1 };
     sf_bc bc = SF_BC_PERIODIC;
     sf_grid grid = SF_GRID_CELL_CENTRE;
+    sf_bc bca[3] = { SF_BC_PERIODIC, SF_BC_PERIODIC, SF_BC_PERIODIC };   // per axis (Dirichlet / Neumann may be mixed)
+    bool mixed = false;
+    int r2ra[3] = { 0, 0, 0 };   // R2R_* of the pass along each axis
     sf_operator op = SF_OP_PSEUDO_SPECTRAL;
     sf_precision prec = SF_F32;
     int ncomp = 1;
@@ -208,7 +211,7 @@ void axis_tables(const sf_plan_s& pl, int a, int count, std::vector<long double>
     const long long n = pl.n[a];
     const long double h = pl.h[a];
     for (int k = 0; k < count; ++k) {
-        switch (pl.bc) {
+        switch (pl.bca[a]) {
         case SF_BC_PERIODIC: {
             const long double Ld = (long double)n * h;
             const long long m = (2 * k < n) ? k : k - n;
@@ -444,8 +447,8 @@ template <typename T> sf_status build_tables(sf_plan p)
         p->LT[a] = (p->r2r == R2R_NONE) ? p->La[a] : 2 * p->La[a];
         if ((st = upload_twiddles<T>(p, &p->tw[a], p->LT[a])) != SF_OK) return st;
     }
-    if (p->r2r == R2R_DCT || p->r2r == R2R_DST2)
-        for (int a = 0; a < p->ndim; ++a)
+    for (int a = 0; a < p->ndim; ++a)
+        if (p->r2ra[a] == R2R_DCT || p->r2ra[a] == R2R_DST2)
             if ((st = upload_dct_shift<T>(p, &p->ptw[a], (int)p->n[a])) != SF_OK) return st;
     std::vector<long double> z1(1, 0.0L);
     if ((st = upload_real<T>(p, &p->zero1, z1)) != SF_OK) return st;
@@ -521,11 +524,11 @@ template <typename T> sf_status run(sf_plan p, int outk)
                 if (xp.face[2 * a + s]) xp.has_faces = 1;
                 // reading A18: the face sits one spacing (cell-boundary Dirichlet, cell-centre Neumann: weight 1)
                 // or half a spacing / a mirrored ghost node (the other two Table-1 rows: weight 2) from the layer
-                const double wf = ((p->bc == SF_BC_DIRICHLET) == (p->grid == SF_GRID_CELL_BOUNDARY)) ? 1.0 : 2.0;
+                const double wf = ((p->bca[a] == SF_BC_DIRICHLET) == (p->grid == SF_GRID_CELL_BOUNDARY)) ? 1.0 : 2.0;
                 // the discrete equation is lap_h psi = rhs_sign f with the face value in the ghost layer (eq. (2)
                 // PAPER.md:22, reading A8): interior stencil = rhs_sign f + w g.  The multiplier carries rhs_sign for
                 // the whole folded source, so the fold adds (w / rhs_sign) g -- the face value keeps its sign.
-                if (p->bc == SF_BC_DIRICHLET) xp.wface[2 * a + s] = (T)(-wf / (p->h[a] * p->h[a]) / p->rhs_sign);
+                if (p->bca[a] == SF_BC_DIRICHLET) xp.wface[2 * a + s] = (T)(-wf / (p->h[a] * p->h[a]) / p->rhs_sign);
                 else xp.wface[2 * a + s] = (T)((s ? -wf : wf) / p->h[a] / p->rhs_sign);
             }
     }
@@ -564,7 +567,11 @@ template <typename T> sf_status run(sf_plan p, int outk)
     sp.nx = p->nspec_x; sp.r2r = p->r2r;
     sp.mul = (p->bc == SF_BC_UNBOUNDED) ? MUL_GREEN : MUL_SYMBOL;
     sp.scale = (T)p->scale;
-    sp.zero_mode = (p->bc == SF_BC_PERIODIC || p->bc == SF_BC_NEUMANN) ? 1 : 0;
+    {   // the all-zero index is singular only when no axis is Dirichlet
+        bool all_neumann = (p->bc == SF_BC_NEUMANN);
+        for (int a = 0; a < nd; ++a) all_neumann = all_neumann && p->bca[a] == SF_BC_NEUMANN;
+        sp.zero_mode = (p->bc == SF_BC_PERIODIC || all_neumann) ? 1 : 0;
+    }
     sp.green = (const T*)p->green;
 
     if (p->fast && outk == OUT_SOLVE) {
@@ -853,6 +860,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         sp.out_ps = hp; sp.out_bs = hp * P1; sp.out_cs = p->w2_field;
         sp.n_in = n1; sp.n_out = (p->r2r == R2R_NONE) ? p->La[1] : n1;
         sp.LT = p->LT[1]; sp.tw = (const C*)p->tw[1]; sp.ptw = (const C*)p->ptw[1];
+        sp.r2r = p->r2ra[1];
         SF_CUDA(p, launch_spass<T>(p->La[1], 0, sp, n2, ncomp, 1, st));
         p->launches++;
     }
@@ -886,6 +894,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         const int nb = (nd == 3) ? P1 : 1;
         const int nbuf = (outk == OUT_CURL || outk == OUT_DIV) ? 3 : (outk == OUT_GRAD ? 2 : 1);
         const int gz = (outk == OUT_SOLVE || outk == OUT_LAP) ? ncomp : 1;
+        sp.r2r = p->r2ra[ax];
         SF_CUDA(p, launch_spass<T>(p->La[ax], 2, sp, nb, gz, nbuf, st));
         p->launches++;
     }
@@ -899,6 +908,7 @@ template <typename T> sf_status run(sf_plan p, int outk)
         sp.LT = p->LT[1]; sp.tw = (const C*)p->tw[1]; sp.ptw = (const C*)p->ptw[1];
         sp.kap_ext = (const T*)p->kap_ext[1];
         sp.dfield1 = (p->r2r != R2R_NONE && outk == OUT_GRAD) ? 3 : 0;   // field 2 = d psi / dy
+        sp.r2r = p->r2ra[1];
         SF_CUDA(p, launch_spass<T>(p->La[1], 1, sp, n2, nf_out, 1, st));
         p->launches++;
     }
@@ -988,7 +998,12 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         if (bc[a] < SF_BC_PERIODIC || bc[a] > SF_BC_UNBOUNDED) return fail(nullptr, SF_ERR_INVALID_ARG, "unknown boundary condition");
         if (n[a] <= 0) return fail(nullptr, SF_ERR_INVALID_ARG, "sizes must be positive");
         if (!(h[a] > 0.0) || !std::isfinite(h[a])) return fail(nullptr, SF_ERR_INVALID_ARG, "spacings must be positive and finite");
-        if (bc[a] != bc[0]) return fail(nullptr, SF_ERR_UNSUPPORTED, "mixed boundary conditions per axis are not part of the method (PAPER.md:126)");
+        if (bc[a] != bc[0]) {
+            // Dirichlet and Neumann may be mixed per axis (each axis takes its own row of Table 1); periodic and
+            // unbounded axes cannot be combined with others (that is the paper's semi-unbounded future work)
+            const bool dn = (bc[a] == SF_BC_DIRICHLET || bc[a] == SF_BC_NEUMANN) && (bc[0] == SF_BC_DIRICHLET || bc[0] == SF_BC_NEUMANN);
+            if (!dn) return fail(nullptr, SF_ERR_UNSUPPORTED, "periodic / unbounded axes cannot be mixed with other boundary conditions (PAPER.md:126, :191-199)");
+        }
     }
     int ncomp = (opt && opt->ncomp) ? opt->ncomp : 1;
     if (ncomp != 1 && ncomp != 3) return fail(nullptr, SF_ERR_UNSUPPORTED, "ncomp must be 1 or 3");
@@ -1006,6 +1021,10 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
     p->ndim = ndim;
     for (int a = 0; a < 3; ++a) { p->n[a] = (a < ndim) ? n[a] : 1; p->h[a] = (a < ndim) ? h[a] : 1.0; }
     p->bc = b; p->grid = grid; p->op = op; p->prec = prec; p->ncomp = ncomp;
+    for (int a = 0; a < 3; ++a) {
+        p->bca[a] = (a < ndim) ? bc[a] : b;
+        if (p->bca[a] != b) p->mixed = true;
+    }
     p->stream = opt ? (cudaStream_t)opt->stream : nullptr;
     p->rhs_sign = (opt && opt->rhs_sign != 0.0) ? opt->rhs_sign : 1.0;
     p->eps_over_h = (opt && opt->eps_over_h != 0.0) ? opt->eps_over_h : 2.0;
@@ -1022,7 +1041,7 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
     for (int a = 0; a < ndim; ++a) {
         const long long na = p->n[a];
         long long len; // complex FFT length of the pass along this axis
-        switch (b) {
+        switch (p->bca[a]) {
         case SF_BC_PERIODIC:
             if (!is_pow2(na)) return bail(SF_ERR_UNSUPPORTED, "periodic sizes must be powers of two");
             len = (a == 0) ? na / 2 : na; p->P[a] = (int)na; norm *= (double)na; break;
@@ -1065,6 +1084,11 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         if (grid == SF_GRID_CELL_CENTRE) { p->xmode = X_DCT2; p->r2r = R2R_DCT; }
         else { p->xmode = X_DCT1; p->r2r = R2R_DCT1; }
         break;
+    }
+    for (int a = 0; a < 3; ++a) {
+        if (p->bca[a] == SF_BC_DIRICHLET) p->r2ra[a] = (grid == SF_GRID_CELL_BOUNDARY) ? R2R_DST1 : R2R_DST2;
+        else if (p->bca[a] == SF_BC_NEUMANN) p->r2ra[a] = (grid == SF_GRID_CELL_CENTRE) ? R2R_DCT : R2R_DCT1;
+        else p->r2ra[a] = R2R_NONE;
     }
     p->nspec_x = (p->r2r == R2R_NONE) ? p->Lx + 1 : (int)p->n[0];
     p->pitch = round_up(p->nspec_x, 16);
@@ -1222,7 +1246,7 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         p->fastper64 = true;
     }
     // fp64 Dirichlet / Neumann plans with 255- / 256-long y and z pencils: generation-2 strided passes
-    if (prec == SF_F64 && ndim == 3 && ncomp == 1 && !getenv("SF_DISABLE_FAST") &&
+    if (prec == SF_F64 && ndim == 3 && ncomp == 1 && !p->mixed && !getenv("SF_DISABLE_FAST") &&
         ((p->r2r == R2R_DST1 && p->n[1] == 255 && p->n[2] == 255) || (p->r2r == R2R_DCT && p->n[1] == 256 && p->n[2] == 256))) {
         if (sf2::fast_init() != cudaSuccess) { cudaGetLastError(); return bail(SF_ERR_CUDA, "set-up of the fast path failed"); }
         // the real work array as 8-byte words: (column, y, z); a tile is 16 words x all rows of a pencil
@@ -1290,7 +1314,7 @@ sf_status sf_set_bc_values(sf_plan plan, int axis, int side, const void* face, s
 {
     if (!plan) return SF_ERR_INVALID_ARG;
     if (axis < 0 || axis >= plan->ndim || side < 0 || side > 1) return fail(plan, SF_ERR_INVALID_ARG, "axis / side out of range");
-    if (plan->bc != SF_BC_DIRICHLET && plan->bc != SF_BC_NEUMANN)
+    if (plan->bca[axis] != SF_BC_DIRICHLET && plan->bca[axis] != SF_BC_NEUMANN)
         return fail(plan, SF_ERR_UNSUPPORTED, "boundary values apply to Dirichlet / Neumann plans only (PAPER.md:302)");
     if (plan->op != SF_OP_FD2) return fail(plan, SF_ERR_UNSUPPORTED, "boundary values need the FD2 operator (PAPER.md:173)");
     const int i = 2 * axis + side;
@@ -1314,6 +1338,7 @@ sf_status sf_gradient(sf_plan plan)
 {
     if (!plan) return SF_ERR_INVALID_ARG;
     if (plan->ncomp != 1) return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient is built for scalar plans");
+    if (plan->mixed) return fail(plan, SF_ERR_UNSUPPORTED, "sf_gradient is not built for plans with mixed boundary conditions");
     {
         // the fused pass holds two tiles (psi and one derivative)
         const int ax = plan->ndim - 1;
