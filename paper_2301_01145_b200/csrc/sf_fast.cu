@@ -349,11 +349,13 @@ template <int MODE> cudaError_t launch_xg_mode(bool inv, const sf::XParams<doubl
     const dim3 grid((unsigned)gx, (unsigned)ncomp);
     cudaError_t e;
     if (inv) {
-        if ((e = cudaFuncSetAttribute(fast_xg_kernel<MODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXgSmem)) != cudaSuccess) return e;
-        fast_xg_kernel<MODE, true><<<grid, kXgThreads, kXgSmem, st>>>(p);
+        constexpr size_t sm = xg_smem<MODE, true>();
+        if ((e = cudaFuncSetAttribute(fast_xg_kernel<MODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)) != cudaSuccess) return e;
+        fast_xg_kernel<MODE, true><<<grid, kXgThreads, sm, st>>>(p);
     } else {
-        if ((e = cudaFuncSetAttribute(fast_xg_kernel<MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXgSmem)) != cudaSuccess) return e;
-        fast_xg_kernel<MODE, false><<<grid, kXgThreads, kXgSmem, st>>>(p);
+        constexpr size_t sm = xg_smem<MODE, false>();
+        if ((e = cudaFuncSetAttribute(fast_xg_kernel<MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)) != cudaSuccess) return e;
+        fast_xg_kernel<MODE, false><<<grid, kXgThreads, sm, st>>>(p);
     }
     return cudaGetLastError();
 }

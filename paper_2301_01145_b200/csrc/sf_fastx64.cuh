@@ -13,6 +13,7 @@
 // grid over the row tiles.
 #pragma once
 #include "sf_fast64.cuh"
+#include "sf_fastper.cuh"
 #include "sf_xpass.cuh"
 
 namespace sf2 {
@@ -38,16 +39,23 @@ template <int MODE> __device__ __forceinline__ double xg_ext(const double* row, 
     }
 }
 
+// raw rows of the NEXT tile are fetched by asynchronous 8-byte copies (LDGSTS) into a buffer of their own while the
+// current tile is transformed (all cases but the backward zero-padded pass, whose input rows are 4 KB each)
+template <int MODE, bool INV> constexpr bool xg_prefetch() { return !(INV && MODE == sf::X_ZEROPAD); }
+template <int MODE, bool INV> constexpr size_t xg_smem() { return kXgSmem + (xg_prefetch<MODE, INV>() ? (size_t)kXgRows * kXgRP * sizeof(double) : 0); }
+
 template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 4) fast_xg_kernel(const sf::XParams<double> p)
 {
+    constexpr bool PF = xg_prefetch<MODE, INV>();
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* rbuf = reinterpret_cast<double*>(smem_raw);                                         // [8][kXgRP] reals
     D* sbuf = reinterpret_cast<D*>(smem_raw);                                                   // [8][kXgSP] complex, same storage
     D* xbuf = sbuf;                                                                             // exchange [16 q][16 o][8 rows]
+    double* pbuf = reinterpret_cast<double*>(smem_raw + kXgSmem);                               // [8][kXgRP] raw rows of the next tile
     __shared__ __align__(16) D s_t256[256];   // [o][q] = w256^(q o)
     __shared__ __align__(16) D s_tsp[136];    // w512^k, k <= 128
-    __shared__ int s_iy[kXgRows], s_iz[kXgRows];
-    __shared__ long long s_rin[kXgRows], s_sp[kXgRows];
+    __shared__ int s_iy[2][kXgRows], s_iz[2][kXgRows];
+    __shared__ long long s_rin[2][kXgRows], s_sp[2][kXgRows];
 
     const int tid = threadIdx.x;
     const int row = tid & 7;
@@ -59,68 +67,85 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 4) f
     for (int i = tid; i <= 128; i += kXgThreads) s_tsp[i] = c_tw1024d[2 * i];
     const D* t256 = s_t256 + o * 16;
     double* rrow = rbuf + row * kXgRP;
+    const double* prow = pbuf + row * kXgRP;
     D* srow = sbuf + row * kXgSP;
     D* xw = xbuf + (o * 8 + row);            // slot (q, o) at stride 128
     const D* xr = xbuf + (o * 128 + row);    // slot (o, o') at stride 8
 
     const long long nrows = (long long)p.ny * p.nz;
     const long long ntiles = (nrows + kXgRows - 1) / kXgRows;
-    const double* rin = INV ? nullptr : p.real_in + comp * p.rin_pc;
+    // the rows this pass reads: the source (S1) or the real spectrum rows (S5, real-to-real modes)
+    const double* rsrc = INV ? reinterpret_cast<const double*>(p.spec_in) + comp * p.sp_pc : p.real_in + comp * p.rin_pc;
 
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const long long row0 = tile * kXgRows;
-        __syncthreads();   // the previous tile's stores have read the staged rows; (first tile: the tables are in place)
-        if (tid < kXgRows) {
-            const long long r = row0 + tid;
-            const int iy = (int)(r % p.ny), iz = (int)(r / p.ny);
-            s_iy[tid] = (r < nrows) ? iy : -1;
-            s_iz[tid] = iz;
-            s_rin[tid] = iy * p.rin_py + iz * p.rin_pz;
-            s_sp[tid] = iy * p.sp_py + iz * p.sp_pz;
+    auto geometry = [&](long long tile, int g) {      // threads 0 .. 7
+        const long long r = tile * kXgRows + tid;
+        const int iy = (int)(r % p.ny), iz = (int)(r / p.ny);
+        s_iy[g][tid] = (tile < ntiles && r < nrows) ? iy : -1;
+        s_iz[g][tid] = iz;
+        s_rin[g][tid] = iy * p.rin_py + iz * p.rin_pz;
+        s_sp[g][tid] = iy * p.sp_py + iz * p.sp_pz;
+    };
+    auto prefetch = [&](int g) {                      // a warp per row, lanes along the row
+        for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
+            double* dst = pbuf + r * kXgRP;
+            if (s_iy[g][r] >= 0) {
+                const double* src = rsrc + (INV ? s_sp[g][r] : s_rin[g][r]);
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    if (lane + 32 * j < n) cp_async8(dst + lane + 32 * j, src + lane + 32 * j);
+            } else {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) dst[lane + 32 * j] = 0.0;
+            }
         }
-        __syncthreads();
+        cp_async_commit();
+    };
+
+    int g = 0;
+    if (tid < kXgRows) geometry(blockIdx.x, 0);
+    __syncthreads();
+    if (PF) prefetch(0);
+
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, g ^= 1) {
+        if (PF) cp_async_wait_all();
+        __syncthreads();   // this tile's raw rows have landed; the previous tile's stores have read the staged rows
         D v[16];
         if constexpr (!INV) {
             // ---------------------------------------------------------------- S1
-            // stage the (folded) source rows: a warp per row, lanes along the row
-            for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
-                const int iy = s_iy[r];
-                double* dst = rbuf + r * kXgRP;
-                if (iy >= 0) {
-                    // all loads of the row first (n <= 256: eight per lane), then the boundary terms and the stores
-                    const double* rp = rin + s_rin[r];
-                    double t[8];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) t[j] = (lane + 32 * j < n) ? __ldg(rp + lane + 32 * j) : 0.0;
-                    if (p.has_faces) {
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            if (lane + 32 * j < n) t[j] += sf::x_face_term(p, lane + 32 * j, iy, s_iz[r]);
+            if (p.has_faces) {
+                // boundary values folded into the staged rows: a warp per row
+                for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
+                    const int iy = s_iy[g][r];
+                    if (iy < 0) continue;
+                    const int iz = s_iz[g][r];
+                    double* dst = pbuf + r * kXgRP;
+                    if (iy == 0 || iy == p.ny - 1 || iz == 0 || iz == p.nz - 1) {
+                        for (int ix = lane; ix < n; ix += 32) dst[ix] += sf::x_face_term(p, ix, iy, iz);
+                    } else if (lane < 2) {
+                        const int ix = lane ? n - 1 : 0;
+                        dst[ix] += sf::x_face_term(p, ix, iy, iz);
                     }
-#pragma unroll
-                    for (int j = 0; j < 8; ++j)
-                        if (lane + 32 * j < n) dst[lane + 32 * j] = t[j];
-                } else {
-                    for (int ix = lane; ix < n; ix += 32) dst[ix] = 0.0;
                 }
+                __syncthreads();
             }
-            __syncthreads();
             // packed extended sequence z[nn] = x~[2 nn] + i x~[2 nn + 1], nn = o + 16 r
-#pragma unroll
             // (n = 255 or 256: for r < 8 both positions 2 nn, 2 nn + 1 <= 255 lie in the stored half of the extension, for
             // r >= 8 in the mirrored / padded half -- the rules of xg_ext resolved at compile time)
+#pragma unroll
             for (int r = 0; r < 16; ++r) {
                 const int nn = o + 16 * r;
                 if (r < 8) {
-                    if (MODE == sf::X_DST1) v[r] = make_double2(nn == 0 ? 0.0 : rrow[max(2 * nn - 1, 0)], rrow[2 * nn]);
-                    else v[r] = make_double2(rrow[2 * nn], rrow[2 * nn + 1]);
+                    if (MODE == sf::X_DST1) v[r] = make_double2(nn == 0 ? 0.0 : prow[max(2 * nn - 1, 0)], prow[2 * nn]);
+                    else v[r] = make_double2(prow[2 * nn], prow[2 * nn + 1]);
                 } else {
                     if (MODE == sf::X_ZEROPAD) v[r] = make_double2(0.0, 0.0);
-                    else if (MODE == sf::X_DST1) v[r] = make_double2(nn == 128 ? 0.0 : -rrow[min(511 - 2 * nn, 254)], -rrow[510 - 2 * nn]);
-                    else v[r] = make_double2(rrow[511 - 2 * nn], rrow[510 - 2 * nn]);
+                    else if (MODE == sf::X_DST1) v[r] = make_double2(nn == 128 ? 0.0 : -prow[min(511 - 2 * nn, 254)], -prow[510 - 2 * nn]);
+                    else v[r] = make_double2(prow[511 - 2 * nn], prow[510 - 2 * nn]);
                 }
             }
-            __syncthreads();   // the staged rows are in registers: their storage becomes the exchange buffer
+            if (tid < kXgRows) geometry(tile + gridDim.x, g ^ 1);
+            __syncthreads();   // the raw rows are in registers: fetch the next tile's while this one is transformed
+            prefetch(g ^ 1);
             dft16<false>(v);
 #pragma unroll
             for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul(v[brev4(q)], t256[q]);
@@ -150,13 +175,13 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 4) f
             __syncthreads();
             // extraction rule and store, a warp per row
             for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
-                if (s_iy[r] < 0) continue;
+                if (s_iy[g][r] < 0) continue;
                 const D* sr = sbuf + r * kXgSP;
                 if constexpr (MODE == sf::X_ZEROPAD) {
-                    D* so = reinterpret_cast<D*>(p.spec_out) + comp * p.sp_pc + s_sp[r];
+                    D* so = reinterpret_cast<D*>(p.spec_out) + comp * p.sp_pc + s_sp[g][r];
                     for (int k = lane; k <= 256; k += 32) so[k] = sr[k];
                 } else {
-                    double* ro = p.real_out + comp * p.sp_pc + s_sp[r];
+                    double* ro = p.real_out + comp * p.sp_pc + s_sp[g][r];
                     for (int k = lane; k < n; k += 32) {
                         if constexpr (MODE == sf::X_DST1) {
                             ro[k] = -sr[k + 1].y;                        // DST-I: Y_k = -Im X~[k+1]
@@ -172,9 +197,9 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 4) f
             // half spectrum X~[0..256] of the extended sequence into the staged rows, a warp per row
             for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
                 D* sr = sbuf + r * kXgSP;
-                const bool valid = s_iy[r] >= 0;
+                const bool valid = s_iy[g][r] >= 0;
                 if constexpr (MODE == sf::X_ZEROPAD) {
-                    const D* si = reinterpret_cast<const D*>(p.spec_in) + comp * p.sp_pc + s_sp[r];
+                    const D* si = reinterpret_cast<const D*>(p.spec_in) + comp * p.sp_pc + s_sp[g][r];
                     D t[9];
 #pragma unroll
                     for (int j = 0; j < 9; ++j) t[j] = (valid && lane + 32 * j <= 256) ? ldg_d(si + lane + 32 * j) : make_double2(0.0, 0.0);
@@ -182,7 +207,7 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 4) f
                     for (int j = 0; j < 9; ++j)
                         if (lane + 32 * j <= 256) sr[lane + 32 * j] = t[j];
                 } else {
-                    const double* ri = reinterpret_cast<const double*>(p.spec_in) + comp * p.sp_pc + s_sp[r];
+                    const double* ri = pbuf + r * kXgRP;     // the real spectrum row, prefetched
                     for (int k = lane; k <= 256; k += 32) {
                         D x = make_double2(0.0, 0.0);
                         if (valid) {
@@ -198,7 +223,9 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 4) f
                     }
                 }
             }
+            if (tid < kXgRows) geometry(tile + gridDim.x, g ^ 1);
             __syncthreads();
+            if (PF) prefetch(g ^ 1);   // the raw rows have been consumed: fetch the next tile's
             // merge in place: Z[k] = (X[k] + conj X[256-k]) + i conj(w512^k) (X[k] - conj X[256-k]), pairs (k, 256 - k)
 #pragma unroll
             for (int m = 0; m < 9; ++m) {
@@ -237,9 +264,9 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXgThreads, 4) f
             // extraction rule and store, a warp per row: x_j = x~[j] (zero-padded, DCT) or x~[j + 1] (DST-I)
             double* ro = p.real_out + comp * p.rin_pc;
             for (int r = warp; r < kXgRows; r += kXgThreads / 32) {
-                if (s_iy[r] < 0) continue;
+                if (s_iy[g][r] < 0) continue;
                 const double* src = rbuf + r * kXgRP + (MODE == sf::X_DST1 ? 1 : 0);
-                double* dst = ro + s_rin[r];
+                double* dst = ro + s_rin[g][r];
                 for (int j = lane; j < n; j += 32) dst[j] = src[j];
             }
         }
