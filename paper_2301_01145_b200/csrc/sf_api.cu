@@ -723,14 +723,19 @@ template <typename T> sf_status run(sf_plan p, int outk)
         fp.reverse_batches = 0;
         p->launches++;
         mark(2);
-        // S3: W2 in place along z
+        // S3: W2 in place along z, tiles of 8 columns
         fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W2;
         fp.in_ps = fp.out_ps = hp * P1; fp.in_bs = fp.out_bs = hp; fp.in_cs = fp.out_cs = p->w2_field; fp.nb = P1;
+        const int nct16 = fp.nct, shift16 = fp.nct_shift, nyq16 = fp.nyq_col;
+        fp.nct = p->nspec_x / 8;
+        for (fp.nct_shift = 0; (1 << fp.nct_shift) < fp.nct; ++fp.nct_shift) {}
+        fp.nyq_col = (p->nspec_x % 8) ? fp.nct * 8 : -1;
         fp.pair_batches = 1;
         fp.green_tiles = (const float*)p->green_tiles; fp.Pb = P1;
         fp.kap_x = (const float*)p->kap[0]; fp.kap_b = (const float*)p->kap[1]; fp.kap_p = (const float*)p->kap[2];
         SF_CUDA(p, sf2::launch_fast5(outk == OUT_CURL ? sf2::F5_CURL : sf2::F5_FUSED, fp, p->map_s3, st));
         fp.pair_batches = 0;
+        fp.nct = nct16; fp.nct_shift = shift16; fp.nyq_col = nyq16;
         p->launches++;
         mark(3);
         // S4: W2 [c][z][ky][hp] -> W1 [c][z][y][hp]
@@ -1206,19 +1211,19 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
             e1 = sf2::fast_make_map(&p->map_s2, p->W1, d, sb, bx);
         }
         {
-            // S3: W2 as (column, ky, z, component)
+            // S3: W2 as (column, ky, z, component); the multiplying passes work on tiles of 8 columns
             const unsigned long long d[4] = { hpc, PP, N2, (unsigned long long)ncomp }, sb[3] = { hpB, hpB * PP, hpB * PP * N2 };
-            const unsigned bx[4] = { 16, 1, 256, 1 };
+            const unsigned bx[4] = { 8, 1, 256, 1 };
             e2 = sf2::fast_make_map(&p->map_s3, p->W2, d, sb, bx);
         }
         p->map_s4 = p->map_s3;   // S4 loads straight into registers: no map of its own
         if (e1 != cudaSuccess || e2 != cudaSuccess) return bail(SF_ERR_CUDA, "tensor map encoding failed");
         {
-            const int nct = p->nspec_x / sf2::kTile, nyq = (p->nspec_x % sf2::kTile) ? nct * sf2::kTile : -1;
-            const size_t ne = sf2::fast_green_tiles_elems_rows(1024, nct, nyq, sf2::kGreenRows5);
+            const int nct = p->nspec_x / 8, nyq = (p->nspec_x % 8) ? nct * 8 : -1;
+            const size_t ne = sf2::fast_green_tiles_elems_rows_w(1024, nct, nyq, sf2::kGreenRows5, 8);
             if ((st = dev_alloc(p, &p->green_tiles, ne * sizeof(float))) != SF_OK) return bail(st, "");
-            if (sf2::fast_green_tiles_rows((float*)p->green_tiles, (const float*)p->green, p->pitch, p->pitch * (p->n[1] + 1), 1024, nct, nyq,
-                                           sf2::kGreenRows5, p->stream) != cudaSuccess)
+            if (sf2::fast_green_tiles_rows_w((float*)p->green_tiles, (const float*)p->green, p->pitch, p->pitch * (p->n[1] + 1), 1024, nct, nyq,
+                                             sf2::kGreenRows5, 8, p->stream) != cudaSuccess)
                 return bail(SF_ERR_CUDA, "building the tile-major Green's table failed");
         }
         if ((st = dev_alloc(p, &p->sched, 2 * sizeof(int))) != SF_OK) return bail(st, "");

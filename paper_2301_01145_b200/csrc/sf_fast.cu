@@ -82,10 +82,10 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FUSED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5NoSlot)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_CURL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FWD, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_INV, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5NoSlot)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FUSED, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_CURL, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x5_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x5_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_fused2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem2)) != cudaSuccess) return e;
@@ -129,7 +129,7 @@ cudaError_t fast_make_map(TileMap* out, const void* base, const unsigned long lo
 
 namespace {
 __global__ void green_tiles_kernel(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
-                                   int rows, long long total)
+                                   int rows, int kTile, long long total)
 {
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
         const int pen = (int)(i % kTile);
@@ -153,8 +153,13 @@ __global__ void green_tiles_kernel(float* tiles, const float* green, long long g
 cudaError_t fast_green_tiles_rows(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
                                   int rows, cudaStream_t st)
 {
-    const long long total = (long long)fast_green_tiles_elems_rows(Pb, nct, nyq_col, rows);
-    green_tiles_kernel<<<148 * 8, 256, 0, st>>>(tiles, green, g_pb, g_pp, Pb, nct, nyq_col, rows, total);
+    return fast_green_tiles_rows_w(tiles, green, g_pb, g_pp, Pb, nct, nyq_col, rows, kTile, st);
+}
+cudaError_t fast_green_tiles_rows_w(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
+                                    int rows, int width, cudaStream_t st)
+{
+    const long long total = (long long)fast_green_tiles_elems_rows_w(Pb, nct, nyq_col, rows, width);
+    green_tiles_kernel<<<148 * 8, 256, 0, st>>>(tiles, green, g_pb, g_pp, Pb, nct, nyq_col, rows, width, total);
     return cudaGetLastError();
 }
 cudaError_t fast_green_tiles(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
@@ -196,16 +201,20 @@ cudaError_t launch_fast5(int mode, const Fast5Params& p, const TileMap& in_map, 
         return cudaErrorInvalidValue;
     if (mode == F5_CURL && (p.ncomp != 3 || !p.kap_x || !p.kap_b || !p.kap_p || 3 * p.out_cs >= (1ll << 31))) return cudaErrorInvalidValue;
     if ((mode == F5_CURL || mode == F5_FUSED) && !p.green_tiles) return cudaErrorInvalidValue;
-    const long long ntiles = (long long)fast_ntiles(p.nb, p.nct, p.nyq_col) * (mode == F5_FUSED ? p.ncomp : 1);
+    // FWD / INV: 16-pencil tiles, one CTA per SM; FUSED / CURL: 8-pencil tiles, two CTAs per SM (p.nct counts those)
+    const bool half = (mode == F5_FUSED || mode == F5_CURL);
+    const int pen = half ? 8 : 16;
+    const long long ntiles = ((long long)p.nb * p.nct + (p.nyq_col >= 0 ? (p.nb + pen - 1) / pen : 0)) * (mode == F5_FUSED ? p.ncomp : 1);
     if (ntiles + 4ll * g_sms >= (1ll << 31)) return cudaErrorInvalidValue;
-    int grid = g_sms;
+    int grid = half ? 2 * g_sms : g_sms;
     if (grid > ntiles) grid = (int)ntiles;
     if (grid <= 0) return cudaErrorInvalidValue;
     switch (mode) {
-    case F5_FWD: fast5_kernel<F5_FWD><<<grid, kT5, kSmem5, st>>>(p, tm); break;
-    case F5_INV: fast5_kernel<F5_INV><<<grid, kT5, kSmem5NoSlot, st>>>(p, tm); break;
-    case F5_FUSED: fast5_kernel<F5_FUSED><<<grid, kT5, kSmem5, st>>>(p, tm); break;
-    case F5_CURL: fast5_kernel<F5_CURL><<<grid, kT5, kSmem5, st>>>(p, tm); break;
+    case F5_FWD: fast5_kernel<F5_FWD, 16><<<grid, kT5, kSmem5, st>>>(p, tm); break;
+    case F5_INV: fast5_kernel<F5_INV, 16><<<grid, kT5, kSmem5NoSlot, st>>>(p, tm); break;
+    // the multiplying passes work on 8-pencil tiles: two 512-thread CTAs per SM
+    case F5_FUSED: fast5_kernel<F5_FUSED, 8><<<grid, kT5 / 2, kSmem5 / 2, st>>>(p, tm); break;
+    case F5_CURL: fast5_kernel<F5_CURL, 8><<<grid, kT5 / 2, kSmem5 / 2, st>>>(p, tm); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

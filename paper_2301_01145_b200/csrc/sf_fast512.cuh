@@ -63,21 +63,21 @@ template <int I32, bool INV> __device__ __forceinline__ C mul_w32(C d)
 }
 
 // first half: radix-16 over r, twiddle w512^(q w) (row w of a shared-memory table), write slots (q, w)
-template <bool INV, typename TW> __device__ __forceinline__ void fft512_a(C (&v)[16], TW&& tw, C* xw)
+template <bool INV, int LW = 32, typename TW> __device__ __forceinline__ void fft512_a(C (&v)[16], TW&& tw, C* xw)
 {
     dft16<INV>(v);
 #pragma unroll
     for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], tw(q));
 #pragma unroll
-    for (int q = 0; q < 16; ++q) xw[q * 1024] = v[brev4(q)];
+    for (int q = 0; q < 16; ++q) xw[q * (32 * LW)] = v[brev4(q)];
 }
 // second half (after a barrier): slots (q0, o), o < 32, radix-2 keeping parity p, radix-16.
 // X[w + 32 j] at v[brev4(j)] out.
-template <bool INV, int P> __device__ __forceinline__ void fft512_b_p(C (&v)[16], const C* xr)
+template <bool INV, int P, int LW> __device__ __forceinline__ void fft512_b_p(C (&v)[16], const C* xr)
 {
     auto step = [&](auto tag) {
         constexpr int o2 = decltype(tag)::value;
-        const C a = xr[o2 * 32], b = xr[(o2 + 16) * 32];
+        const C a = xr[o2 * LW], b = xr[(o2 + 16) * LW];
         if constexpr (P == 0) v[o2] = cadd(a, b);
         else v[o2] = mul_w32<o2, INV>(csub(a, b));
     };
@@ -91,22 +91,22 @@ template <bool INV, int P> __device__ __forceinline__ void fft512_b_p(C (&v)[16]
     step(std::integral_constant<int, 14>()); step(std::integral_constant<int, 15>());
     dft16<INV>(v);
 }
-template <bool INV> __device__ __forceinline__ void fft512_b(C (&v)[16], const C* xr, int p)
+template <bool INV, int LW = 32> __device__ __forceinline__ void fft512_b(C (&v)[16], const C* xr, int p)
 {
-    if (p) fft512_b_p<INV, 1>(v, xr);     // p is warp-uniform: no divergence
-    else fft512_b_p<INV, 0>(v, xr);
+    if (p) fft512_b_p<INV, 1, LW>(v, xr);     // p is warp-uniform: no divergence
+    else fft512_b_p<INV, 0, LW>(v, xr);
 }
 
 // ------------------------------------------------------------------------------------ tensor memory as a parking lot
 // 32x32b shape: lane i of the warp reads / writes TMEM lane (32 (warp mod 4) + i), consecutive 32-bit columns
-__device__ __forceinline__ void tmem_alloc512(uint32_t* smem_dst)
+__device__ __forceinline__ void tmem_alloc_cols(uint32_t* smem_dst, uint32_t cols)   // cols: a power of two >= 32
 {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_dst)), "r"(512u) : "memory");
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_dst)), "r"(cols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
 }
-__device__ __forceinline__ void tmem_free512(uint32_t base)
+__device__ __forceinline__ void tmem_free_cols(uint32_t base, uint32_t cols)
 {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "r"(512u) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "r"(cols) : "memory");
 }
 __device__ __forceinline__ void tmem_st16(uint32_t addr, const C (&v)[8])
 {
@@ -170,10 +170,10 @@ __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.
 
 // ------------------------------------------------------------------------------------ tiles
 // chunk of the tile-major Green's table that belongs to a tile (as green_tile_index of sf_fast.cuh)
-__device__ __forceinline__ int green_tile_index5(const Fast5Params& p, bool full, int b, int col)
+template <int PEN> __device__ __forceinline__ int green_tile_index5(const Fast5Params& p, bool full, int b, int col)
 {
-    if (full) return (min(b, p.Pb - b) << p.nct_shift) + (col >> 4);
-    return ((p.Pb / 2 + 1) << p.nct_shift) + (b >> 4);
+    if (full) return (min(b, p.Pb - b) << p.nct_shift) + (col / PEN);
+    return ((p.Pb / 2 + 1) << p.nct_shift) + (b / PEN);
 }
 
 // MODE F5_FWD   : in rows n < 512 -> out rows k < 1024                       (S2; components are more batches)
@@ -184,14 +184,19 @@ __device__ __forceinline__ int green_tile_index5(const Fast5Params& p, bool full
 //   FWD            dims (column, row, batch, 1)          box {16, 256, 1, 1}   coordinates {col, 0 | 256, b, 0}
 //   FUSED / CURL   dims (column, batch, row, component)  box {16, 1, 256, 1}   coordinates {col, b, 0 | 256, c}
 // The Nyquist column (column nyq_col of every batch) is handled 16 batches at a time with gathered 8-byte accesses.
-template <int MODE>
-__global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, const __grid_constant__ CUtensorMap tm)
+// PEN = pencils per tile: 16 (one CTA of 1024 threads per SM; FWD / INV) or 8 (two CTAs of 512 threads per SM: two
+// independent barrier domains, one transforms while the other waits at a barrier; FUSED / CURL, where a tile is a
+// chain of two to six transforms).  A residue w owns LW = 2 PEN consecutive threads.
+template <int MODE, int PEN>
+__global__ void __launch_bounds__(64 * PEN, 16 / PEN) fast5_kernel(const Fast5Params p, const __grid_constant__ CUtensorMap tm)
 {
+    constexpr int LW = 2 * PEN;            // threads per residue: PEN pencils x 2 halves
+    constexpr int NT = 64 * PEN;           // threads per CTA
     constexpr bool kTma = (MODE != F5_INV);
     constexpr bool kMul = (MODE == F5_FUSED || MODE == F5_CURL);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     C* xbuf = reinterpret_cast<C*>(smem_raw);
-    C* slot = xbuf + kXchg5Elems;
+    C* slot = xbuf + 16 * 32 * LW;
     __shared__ __align__(8) uint64_t bar;
     // Twiddle factors: w512^(q w) between the two halves of a transform and w1024^(w + 32 r) of the odd half
     // (h = 1; the even half multiplies by one).  Both are warp-uniform and live in shared-memory tables (base
@@ -202,27 +207,32 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
     // CURL: per-thread values of the current tile that are needed between the transforms only (kappa_x, kappa_y,
     // output offset): parked here, because the 64 registers of a 1024-thread CTA cannot hold them across the
     // transforms and a spill to local memory misses the (28 KB) L1
-    __shared__ float s_qx[MODE == F5_CURL ? kT5 : 1], s_qy[MODE == F5_CURL ? kT5 : 1];
-    __shared__ unsigned s_oo[MODE == F5_CURL ? kT5 : 1];
+    constexpr bool kPark = (MODE == F5_CURL && PEN == 16);   // (PEN = 8: the shared memory of two CTAs has no room for it)
+    __shared__ float s_qx[kPark ? NT : 1], s_qy[kPark ? NT : 1];
+    __shared__ unsigned s_oo[kPark ? NT : 1];
     __shared__ __align__(16) C s_tw512[kTwc ? 1 : 32 * 16];        // [w][q] = w512^(q w)
-    __shared__ __align__(16) C s_tw1024[kTwc ? 1 : 2 * 32 * 16];   // [h][w][r] = h ? w1024^(w + 32 r) : 1
+    // (PEN = 8: only the h = 1 half of the second table is kept, the even half selects one: shared memory for two CTAs)
+    constexpr bool kHalfTab = (PEN == 8);
+    __shared__ __align__(16) C s_tw1024[kTwc ? 1 : (kHalfTab ? 1 : 2) * 32 * 16];   // [h][w][r] = h ? w1024^(w + 32 r) : 1
     __shared__ int s_tile[2];
     __shared__ uint32_t s_tmem;
 
     const int tid = threadIdx.x;
-    const int lane = tid & 31;
-    const int pen = lane & 15;
-    const int h = lane >> 4;
-    const int w = (int)__reduce_max_sync(0xffffffffu, (unsigned)(tid >> 5));
-    const int q0 = w & 15, par = w >> 4;
-    C* xw = xbuf + (w * 32 + lane);                 // slot (q, w) at ((q * 32 + w) * 32 + lane)
-    const C* xr = xbuf + (q0 * 1024 + lane);        // slot (q0, o) at stride 32
+    const int lane = tid % LW;
+    const int pen = lane % PEN;
+    const int h = lane / PEN;
+    // PEN = 16: the residue is the warp index (warp-uniform: REDUX puts it in a uniform register)
+    const int w = (PEN == 16) ? (int)__reduce_max_sync(0xffffffffu, (unsigned)(tid >> 5)) : tid / LW;
+    const int q0 = w & 15, par = w >> 4;            // (PEN = 8: the two residues of a warp share their parity)
+    C* xw = xbuf + (w * LW + lane);                 // slot (q, w) at ((q * 32 + w) * LW + lane)
+    const C* xr = xbuf + (q0 * 32 * LW + lane);     // slot (q0, o) at stride LW
     const C* t512 = s_tw512 + w * 16;
-    const C* t1024 = s_tw1024 + (h * 32 + w) * 16;
+    const C* t1024 = s_tw1024 + ((kHalfTab ? 0 : h * 32) + w) * 16;
     const float hf = (float)h;
     auto tw512 = [&](int q) -> C { return kTwc ? c_tw1024[(2 * q * w) & 1023] : t512[q]; };
     // 1 + h (w1024^(w + 32 r) - 1): one packed multiply-add on the table of (Re w - 1, Im w)
     auto tw1024 = [&](int r) -> C {
+        if (!kTwc && kHalfTab) { const C t = t1024[r]; return h ? t : make_float2(1.f, 0.f); }
         if (!kTwc) return t1024[r];
         const C m = c_tw1024m1[w + 32 * r];
         return __ffma2_rn(make_float2(hf, hf), m, make_float2(1.f, 0.f));
@@ -230,7 +240,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
 
     const int ncomp_tiles = (MODE == F5_FUSED) ? p.ncomp : 1;     // FUSED: components are independent tile sets
     const int nfull = p.nb << p.nct_shift;
-    const int nnyq = (p.nyq_col >= 0) ? (p.nb + kTile - 1) / kTile : 0;
+    const int nnyq = (p.nyq_col >= 0) ? (p.nb + PEN - 1) / PEN : 0;
     const int ntile1 = nfull + nnyq;
     const int ntiles = ntile1 * ncomp_tiles;
     const int ips = (int)p.in_ps, ops = (int)p.out_ps, ibs = (int)p.in_bs, obs = (int)p.out_bs;
@@ -243,7 +253,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
         if (MODE == F5_FUSED) { g.comp = t / ntile1; t -= g.comp * ntile1; }
         if (t < nnyq) {               // Nyquist-column tiles first: they are the slow ones
             g.full = false;
-            g.b = t * kTile;
+            g.b = t * PEN;
             g.col = p.nyq_col;
         } else {
             const int tf = t - nnyq;
@@ -255,7 +265,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
             }
             g.full = true;
             g.b = bi;
-            g.col = (tf & (p.nct - 1)) * kTile;
+            g.col = (tf & (p.nct - 1)) * PEN;
         }
         return g;
     };
@@ -264,14 +274,14 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
         if (!kTma || tid != 0 || t >= ntiles) return;
         const Geom g = geom(t);
         if (!g.full) return;
-        mbar_expect_tx(&bar, kSlot5Elems * (uint32_t)sizeof(C));
+        mbar_expect_tx(&bar, (uint32_t)(kL5 * PEN * sizeof(C)));
         if (MODE == F5_FWD) {
             tma_load_4d(slot, &tm, g.col, 0, g.b, 0, &bar);
-            tma_load_4d(slot + 256 * kTile, &tm, g.col, 256, g.b, 0, &bar);
+            tma_load_4d(slot + 256 * PEN, &tm, g.col, 256, g.b, 0, &bar);
         } else {
             const int cc = (MODE == F5_CURL) ? c : g.comp;
             tma_load_4d(slot, &tm, g.col, g.b, 0, cc, &bar);
-            tma_load_4d(slot + 256 * kTile, &tm, g.col, g.b, 256, cc, &bar);
+            tma_load_4d(slot + 256 * PEN, &tm, g.col, g.b, 256, cc, &bar);
         }
     };
     // v[r] = x[w + 32 r] of this thread's pencil (FWD / FUSED / CURL)
@@ -283,7 +293,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
                 parity ^= 1;
             }
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = slot[(w + 32 * r) * kTile + pen];
+            for (int r = 0; r < 16; ++r) v[r] = slot[(w + 32 * r) * PEN + pen];
         } else {
             const C* inp = p.in + ((size_t)c * p.in_cs + (size_t)min(g.b + pen, p.nb - 1) * ibs + g.col + (size_t)w * ips);
 #pragma unroll
@@ -299,9 +309,9 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
         for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], tw1024(r));
         __syncthreads();
         after_barrier();
-        fft512_a<false>(v, tw512, xw);
+        fft512_a<false, LW>(v, tw512, xw);
         __syncthreads();
-        fft512_b<false>(v, xr, par);
+        fft512_b<false, LW>(v, xr, par);
     };
     // backward transform (u natural order in: u[j] = U_h[w + 32 j]) and recombination of the halves:
     // x_j = e_j + conj(w1024^j) o_j, j = w + 32 r.  Thread h = 0 ends with rows w + 32 r (r < 8) in out[r],
@@ -309,17 +319,17 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
     auto backward = [&](C (&u)[16], C (&out)[8], auto&& after_barrier) {
         __syncthreads();
         after_barrier();
-        fft512_a<true>(u, tw512, xw);
+        fft512_a<true, LW>(u, tw512, xw);
         __syncthreads();
-        fft512_b<true>(u, xr, par);
+        fft512_b<true, LW>(u, xr, par);
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             const C tl = cmulc(u[brev4(r)], tw1024(r)), th = cmulc(u[brev4(r + 8)], tw1024(r + 8));
             const C send = h ? tl : th;
             const C keep = h ? th : tl;
             C recv;
-            recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
-            recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+            recv.x = __shfl_xor_sync(0xffffffffu, send.x, PEN);
+            recv.y = __shfl_xor_sync(0xffffffffu, send.y, PEN);
             out[r] = cadd(keep, recv);
         }
     };
@@ -327,10 +337,10 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
     // u[j] = G X_h[w + 32 j]: Green's factors of this thread's 16 spectral rows kp = 2 (w + 32 j) + h, folded to
     // min(kp, 1024 - kp), fetched when they are used (the registers cannot hold them across the transform)
     auto mul_green = [&](const Geom& g, const C (&v)[16], C (&u)[16]) {
-        const float* glo = p.green_tiles + ((size_t)green_tile_index5(p, g.full, g.b, g.col) * (kGreenRows5 * kTile) + pen + (2 * w + h) * kTile);
-        const float* ghi = glo + (2 * kL5 - 4 * w - 2 * h) * kTile;   // 1024 - kp     (j >= 8)
+        const float* glo = p.green_tiles + ((size_t)green_tile_index5<PEN>(p, g.full, g.b, g.col) * (kGreenRows5 * PEN) + pen + (2 * w + h) * PEN);
+        const float* ghi = glo + (2 * kL5 - 4 * w - 2 * h) * PEN;   // 1024 - kp     (j >= 8)
 #pragma unroll
-        for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], __ldg(j < 8 ? glo + j * 64 * kTile : ghi - j * 64 * kTile));
+        for (int j = 0; j < 16; ++j) u[j] = cscale(v[brev4(j)], __ldg(j < 8 ? glo + j * 64 * PEN : ghi - j * 64 * PEN));
     };
 
     // ---------------------------------------------------------------- prologue
@@ -343,23 +353,26 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
         s_tile[1] = (int)(blockIdx.x + gridDim.x);
         issue(s_tile[0], MODE == F5_CURL ? 2 : 0);
     }
-    if (MODE == F5_CURL) s_kapp[tid] = __ldg(p.kap_p + tid);
+    if (MODE == F5_CURL)
+        for (int i = tid; i < 1024; i += NT) s_kapp[i] = __ldg(p.kap_p + i);
     if (!kTwc) {
         if (tid < 512) s_tw512[tid] = c_tw1024[(2 * (tid & 15) * (tid >> 4)) & 1023];
-        const int r = tid & 15, ww = (tid >> 4) & 31, hh = tid >> 9;
-        s_tw1024[tid] = hh ? c_tw1024[ww + 32 * r] : make_float2(1.f, 0.f);
+        for (int i = tid; i < (kHalfTab ? 1 : 2) * 512; i += NT) {
+            const int r = i & 15, ww = (i >> 4) & 31, hh = kHalfTab ? 1 : (i >> 9);
+            s_tw1024[i] = hh ? c_tw1024[ww + 32 * r] : make_float2(1.f, 0.f);
+        }
     }
     uint32_t tbase = 0;
     if (MODE == F5_CURL) {
-        if (tid < 32) tmem_alloc512(&s_tmem);
+        if (tid < 32) tmem_alloc_cols(&s_tmem, (uint32_t)(NT / 2));   // 64 columns per warp, four warps (lane quadrants) side by side
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     }
     __syncthreads();
     if (MODE == F5_CURL) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        tbase = s_tmem + ((uint32_t)(w & 3) << 21);    // lane field (bits 16..31) = 32 (w mod 4)
+        tbase = s_tmem + ((uint32_t)((tid >> 5) & 3) << 21);    // lane field (bits 16..31) = 32 (warp mod 4)
     }
-    const uint32_t t_A = tbase + (uint32_t)(w >> 2) * 64;   // this warp's 2 x 32 columns: 16 complex numbers per thread each
+    const uint32_t t_A = tbase + (uint32_t)(tid >> 7) * 64;   // this warp's 2 x 32 columns: 16 complex numbers per thread each
     const uint32_t t_B = t_A + 32;
     (void)t_A; (void)t_B;
 
@@ -419,14 +432,15 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
             gg.full = FULL;
             const int kx = FULL ? g.col + pen : g.col;
             const int kb = FULL ? g.b : min(g.b + pen, p.nb - 1);
-            s_qx[tid] = __ldg(p.kap_x + kx);
-            s_qy[tid] = __ldg(p.kap_b + kb);
+            const float qx_r = __ldg(p.kap_x + kx), qy_r = __ldg(p.kap_b + kb);
+            if (kPark) { s_qx[tid] = qx_r; s_qy[tid] = qy_r; }
             // element offsets of the outputs fit 32 bits (checked by the launcher)
-            s_oo[tid] = (unsigned)((FULL ? g.b : g.b + pen) * obs + g.col + (FULL ? pen : 0) + (w + 256 * h) * ops);
+            const unsigned oo_r = (unsigned)((FULL ? g.b : g.b + pen) * obs + g.col + (FULL ? pen : 0) + (w + 256 * h) * ops);
+            if (kPark) s_oo[tid] = oo_r;
             const float* kz = s_kapp + (2 * w + h);    // kappa_z of spectral row 2 (w + 32 j) + h at kz[64 j]
             auto store = [&](int c, const C (&o8)[8]) {
                 if (!FULL && !pvalid) return;
-                C* q = p.out + (s_oo[tid] + (unsigned)c * (unsigned)p.out_cs);
+                C* q = p.out + ((kPark ? s_oo[tid] : oo_r) + (unsigned)c * (unsigned)p.out_cs);
 #pragma unroll
                 for (int r = 0; r < 8; ++r) q[(size_t)r * 32 * ops] = cmuli(o8[r]);   // the factor i of i kappa x psi_hat
             };
@@ -445,7 +459,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
                 mul_green(gg, v, u);
                 tmem_st32(t_B, u);
                 tmem_wait_st();
-                const float qy = s_qy[tid];
+                const float qy = kPark ? s_qy[tid] : qy_r;
 #pragma unroll
                 for (int c4 = 0; c4 < 4; ++c4) {
                     C pa[4];
@@ -466,7 +480,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
                 } else {
                     load_x(gg, 0, u);
 #pragma unroll
-                    for (int r = 0; r < 16; ++r) slot[(w + 32 * r) * kTile + pen] = u[r];
+                    for (int r = 0; r < 16; ++r) slot[(w + 32 * r) * PEN + pen] = u[r];
                 }
                 store(0, o8);
             }
@@ -476,7 +490,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
                 load_x(gg, 0, v, true);
                 forward(v, [&]() { if (tid == 0) issue(s_tile[(it + 1) & 1], 2); });
                 mul_green(gg, v, u);
-                const float qx = s_qx[tid], qy = s_qy[tid];
+                const float qx = kPark ? s_qx[tid] : qx_r, qy = kPark ? s_qy[tid] : qy_r;
 #pragma unroll
                 for (int c2 = 0; c2 < 8; ++c2) {
                     C pa[2], pb[2];
@@ -507,7 +521,7 @@ __global__ void __launch_bounds__(kT5, 1) fast5_kernel(const Fast5Params p, cons
     if (MODE == F5_CURL) {
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
-        if (tid < 32) tmem_free512(s_tmem);
+        if (tid < 32) tmem_free_cols(s_tmem, (uint32_t)(NT / 2));
     }
     // the last CTA to finish re-arms the counter for the next launch
     if (tid == 0) {

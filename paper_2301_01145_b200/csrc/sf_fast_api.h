@@ -145,6 +145,13 @@ inline size_t fast_green_tiles_elems_rows(int Pb, int nct, int nyq_col, int rows
 }
 cudaError_t fast_green_tiles_rows(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
                                   int rows, cudaStream_t st);
+// the same for tiles of `width` pencils (nct = tiles of that width per batch; Nyquist tiles of `width` batches)
+inline size_t fast_green_tiles_elems_rows_w(int Pb, int nct, int nyq_col, int rows, int width)
+{
+    return ((size_t)(Pb / 2 + 1) * nct + (nyq_col >= 0 ? (size_t)(Pb + width - 1) / width : 0)) * rows * width;
+}
+cudaError_t fast_green_tiles_rows_w(float* tiles, const float* green, long long g_pb, long long g_pp, int Pb, int nct, int nyq_col,
+                                    int rows, int width, cudaStream_t st);
 // launch one 512 -> 1024 padded pass (mode = F5_*) as a persistent grid of one 1024-thread CTA per SM; `in_map`
 // describes p.in as documented at fast5_kernel
 cudaError_t launch_fast5(int mode, const Fast5Params& p, const TileMap& in_map, cudaStream_t st);
