@@ -53,6 +53,10 @@ def lib() -> C.CDLL:
         L.orc_exp1.argtypes = [C.c_double]
         L.orc_green2d_gauss.restype = C.c_double
         L.orc_green2d_gauss.argtypes = [C.c_int, C.c_double, C.c_double]
+        L.orc_bessel_cin.restype = C.c_double
+        L.orc_bessel_cin.argtypes = [C.c_double]
+        L.orc_green2d_spectral.restype = C.c_double
+        L.orc_green2d_spectral.argtypes = [C.c_double, C.c_double]
         L.orc_unbounded_spec_size.restype = C.c_longlong
         _lib = L
     return _lib
@@ -383,6 +387,16 @@ def _i64x2(n):
 
 def _f64x2(h):
     return (C.c_double * 2)(float(h[0]), float(h[1]))
+
+
+def bessel_cin(x):
+    """C(x) = int_0^x (1 - J0(t)) / t dt"""
+    return float(lib().orc_bessel_cin(float(x)))
+
+
+def green2d_spectral(r, h):
+    """the 2-D spectrally compact kernel (C(pi r / h) - ln(pi / 2h) - gamma) / (2 pi) at distance r (reading A30)"""
+    return float(lib().orc_green2d_spectral(float(r), float(h)))
 
 
 def unbounded2d_green(n_xy, h, eps, order=2):

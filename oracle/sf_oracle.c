@@ -1601,26 +1601,83 @@ static int unb2_backward_extract(const i64 n[2], cplx *spec, double *out)
     return ORC_OK;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * The spectrally compact kernel in 2-D ("1D, 2D and 3D"; reading A30 = A26 in the plane): the singular
+ * spectrum -1/k^2 kept inside the disc |k| <= k_c = pi/h and dropped outside.  Its radial inverse transform diverges
+ * logarithmically at k -> 0 (a 2-D potential is defined up to a constant); with the constant fixed so that
+ * G -> ln(r) / (2 pi) far away, as for the Gaussian kernels of reading A28,
+ *     G(r) = ( C(k_c r) - ln(k_c / 2) - gamma ) / (2 pi),   C(x) = int_0^x (1 - J0(t)) / t dt,
+ *     G(0) = -( ln(k_c / 2) + gamma ) / (2 pi).
+ * C(x) is computed from its definition: the power series sum_{m>=1} (-1)^(m+1) (x/2)^(2m) / (2m (m!)^2) in extended
+ * precision up to x = 12, beyond that C(12) + ln(x / 12) - int_12^x J0(t) / t dt with composite 16-point Gauss-Legendre
+ * panels of length <= 2 on the library's j0().
+ * ---------------------------------------------------------------------------------------- */
+extern double j0(double);   /* POSIX Bessel function of the C library (not declared under strict ISO C) */
+static double cin_series(double x)
+{
+    long double q = 0.25L * (long double)x * (long double)x, term = 1.0L, sum = 0.0L;
+    for (int m = 1; m < 200; ++m) {
+        term *= -q / ((long double)m * (long double)m);          /* (-1)^m (x/2)^(2m) / (m!)^2 */
+        long double add = -term / (2.0L * (long double)m);
+        sum += add;
+        if (fabsl(add) < 1e-22L * fabsl(sum) && m > (int)x) break;
+    }
+    return (double)sum;
+}
+double orc_bessel_cin(double x)
+{
+    static const double gx[8] = { 0.0950125098376374401853193, 0.2816035507792589132304605, 0.4580167776572273863424194,
+                                  0.6178762444026437484466718, 0.7554044083550030338951012, 0.8656312023878317438804679,
+                                  0.9445750230732325760779884, 0.9894009349916499325961542 };
+    static const double gw[8] = { 0.1894506104550684962853967, 0.1826034150449235888667637, 0.1691565193950025381893121,
+                                  0.1495959888165767320815017, 0.1246289712555338720524763, 0.0951585116824927848099251,
+                                  0.0622535239386478928628438, 0.0271524594117540948517806 };
+    if (x < 0.0) x = -x;
+    if (x <= 12.0) return cin_series(x);
+    double acc = 0.0;
+    int panels = (int)ceil((x - 12.0) / 2.0);
+    double len = (x - 12.0) / (double)panels;
+    for (int p = 0; p < panels; ++p) {
+        double a = 12.0 + len * (double)p, mid = a + 0.5 * len, half = 0.5 * len, s = 0.0;
+        for (int i = 0; i < 8; ++i) {
+            double t1 = mid + half * gx[i], t2 = mid - half * gx[i];
+            s += gw[i] * (j0(t1) / t1 + j0(t2) / t2);
+        }
+        acc += s * half;
+    }
+    return cin_series(12.0) + log(x / 12.0) - acc;
+}
+double orc_green2d_spectral(double r, double h)
+{
+    const double kc = PI / h, euler = 0.57721566490153286061;
+    if (r == 0.0) return -(log(0.5 * kc) + euler) / (2.0 * PI);
+    return (orc_bessel_cin(kc * r) - log(0.5 * kc) - euler) / (2.0 * PI);
+}
+
+/* order 2 .. 10: Gaussian-regularised kernels (reading A28); order 0: the spectrally compact kernel above with
+ * h = max spacing (eps ignored, as for the 3-D kernel) */
 int orc_unbounded2d_green(const i64 n[2], const double h[2], double eps, int order, cplx *ghat)
 {
-    if (order < 2 || order > 10 || (order & 1)) return ORC_ERR_ARG;
+    if (order != 0 && (order < 2 || order > 10 || (order & 1))) return ORC_ERR_ARG;
     for (int a = 0; a < 2; ++a) if (!is_pow2(n[a])) return ORC_ERR_ARG;
     i64 P0 = 2 * n[0], P1 = 2 * n[1];
     double *g = (double *)malloc(sizeof(double) * (size_t)(P0 * P1));
     if (!g) return ORC_ERR_ALLOC;
     double area = h[0] * h[1];
+    double hmax = h[0] > h[1] ? h[0] : h[1];
+#pragma omp parallel for schedule(dynamic, 1)
     for (i64 iy = 0; iy < P1; ++iy)
         for (i64 ix = 0; ix < P0; ++ix) {
             double dx = (double)(ix < P0 - ix ? ix : P0 - ix) * h[0];
             double dy = (double)(iy < P1 - iy ? iy : P1 - iy) * h[1];
-            g[ix + P0 * iy] = area * orc_green2d_gauss(order, sqrt(dx * dx + dy * dy), eps);
+            double r = sqrt(dx * dx + dy * dy);
+            g[ix + P0 * iy] = area * (order == 0 ? orc_green2d_spectral(r, hmax) : orc_green2d_gauss(order, r, eps));
         }
     int err = unb2_forward(n, g, 0, ghat);
     free(g);
     return err;
 }
 
-/* psi and, if grad != NULL, d psi / dx, d psi / dy (eq. (10), wavenumbers of the doubled grid, Nyquist -> 0) */
 int orc_unbounded2d_solve(const i64 n[2], const double h[2], const cplx *ghat, double rhs_sign, const double *f,
                           double *psi, double *grad)
 {

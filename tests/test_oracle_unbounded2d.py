@@ -89,3 +89,59 @@ def test_gaussian_charges_closed_form(order):
         scale = max(np.abs(gx_a).max(), np.abs(gy_a).max())
         assert np.abs(grad[0] - gx_a).max() < 1e-7 * scale
         assert np.abs(grad[1] - gy_a).max() < 1e-7 * scale
+
+
+# ------------------------------------------------------------------------- the spectrally compact kernel in 2-D (A30)
+def test_bessel_cin_against_its_definition_and_a_bessel_series():
+    """C(x) = int_0^x (1 - J0(t)) / t dt: adaptive quadrature of the definition, its derivative, the identity
+    C(x) = sum_{i>=1} (2 H_i - 1/i) J_{2i}(x) with scipy's Bessel functions, and the large-argument form ln(x/2) + gamma"""
+    from scipy import integrate, special
+
+    for x in (0.0, 1e-3, 0.7, 3.0, 11.9, 12.0, 12.1, 25.0, 80.0, 303.5):
+        ref = integrate.quad(lambda t: (1.0 - special.j0(t)) / t if t > 0 else 0.0, 0.0, x, limit=2000, epsabs=1e-13, epsrel=1e-13)[0] if x > 0 else 0.0
+        assert abs(O.bessel_cin(x) - ref) <= 2e-12 * max(1.0, abs(ref)), x
+        if x > 0:
+            i = np.arange(1, int(x) + 60)
+            hs = np.cumsum(1.0 / i)
+            ser = float(np.sum((2.0 * hs - 1.0 / i) * special.jv(2 * i, x)))
+            assert abs(O.bessel_cin(x) - ser) <= 1e-12 * max(1.0, abs(ser)), x
+    for x in (2.0, 9.0, 40.0):       # d C / d x = (1 - J0(x)) / x
+        d = 1e-5
+        num = (O.bessel_cin(x + d) - O.bessel_cin(x - d)) / (2 * d)
+        assert abs(num - (1.0 - special.j0(x)) / x) <= 1e-8
+    x = 5000.0
+    assert abs(O.bessel_cin(x) - (np.log(x / 2) + np.euler_gamma)) <= 2.0 / x ** 1.5
+
+
+def test_spectral_kernel_2d_origin_far_field_and_quadrature_of_its_definition():
+    h = 0.05
+    kc = np.pi / h
+    assert abs(O.green2d_spectral(0.0, h) + (np.log(kc / 2) + np.euler_gamma) / (2 * np.pi)) <= 1e-15
+    r = 40.0 * h      # far field: ln r / (2 pi) up to the decaying oscillation ~ (k_c r)^(-3/2)
+    assert abs(O.green2d_spectral(r, h) - np.log(r) / (2 * np.pi)) <= 1.0 / (2 * np.pi) / (kc * r) ** 1.5
+    # the definition: -1/k^2 inside the disc, i.e. G(r) - G(0) = (1 / 2 pi) int_0^kc (1 - J0(k r)) / k dk
+    from scipy import integrate, special
+    for r in (0.3 * h, 2.0 * h, 7.5 * h):
+        q = integrate.quad(lambda k: (1.0 - special.j0(k * r)) / k, 0.0, kc, limit=500, epsabs=1e-13, epsrel=1e-13)[0]
+        assert abs((O.green2d_spectral(r, h) - O.green2d_spectral(0.0, h)) - q / (2 * np.pi)) <= 1e-12
+
+
+def test_spectral_kernel_2d_solves_a_resolved_gaussian_charge_to_rounding():
+    """a Gaussian charge whose spectrum has died out at k_c is solved exactly by the truncated kernel:
+    psi = q (ln r + E1(r^2 / 2 s^2) / 2) / (2 pi) (the closed form of reading A28 with eps -> 0)"""
+    from scipy import special
+    n, L = 64, 1.0
+    h = (L / n, L / n)
+    s = 3.0 * h[0]      # spectrum e^{-(k s)^2 / 2} = 5e-20 at k_c; 9 widths from the nearest edge of the box
+    x = (np.arange(n) + 0.5) * h[0]
+    X, Y = np.meshgrid(x, x, indexing="xy")
+    cx, cy = 0.47, 0.55
+    r2 = (X - cx) ** 2 + (Y - cy) ** 2
+    f = np.exp(-r2 / (2 * s * s)) / (2 * np.pi * s * s)
+    gh = O.unbounded2d_green((n, n), h, 0.0, order=0)
+    psi = O.unbounded2d_solve(f, h, gh)
+    r = np.sqrt(r2)
+    exact = (np.log(r) + 0.5 * special.exp1(r2 / (2 * s * s))) / (2 * np.pi)
+    err = np.abs(psi - exact).max()
+    print("2-D spectral kernel, resolved Gaussian charge: max error", err)
+    assert err <= 5e-13
