@@ -72,7 +72,8 @@ typedef enum {
     SF_OP_GREEN_GAUSS8 = 5,    /* polynomials L_m^(1/2):  G_P = G_2 - sum_{n=1}^{P/2-1} eps^2/(2n) L_{n-1}(x) g */
     SF_OP_GREEN_GAUSS10 = 6,   /* (spectrum -exp(-s^2/2) sum_{n<P/2} (s^2/2)^n/n! / k^2, s = eps k)           */
     SF_OP_GREEN_SPECTRAL = 7   /* spectrally compact kernel: -1/k^2 inside |k| <= pi/h,        */
-                               /* G(r) = -Si(pi r/h) / (2 pi^2 r), h = max spacing; eps_over_h is ignored     */
+                               /* 3-D: G(r) = -Si(pi r/h) / (2 pi^2 r); 2-D: (C(pi r/h) - ln(pi/2h) - gamma) / (2 pi),  */
+                               /* C(x) = int_0^x (1 - J0(t)) / t dt; h = max spacing; eps_over_h is ignored   */
 } sf_operator;
 
 typedef enum { SF_F32 = 0, SF_F64 = 1 } sf_precision;
@@ -118,12 +119,12 @@ typedef struct {
  *          DCT-III; periodic and unbounded accept both (identical numerics).
  *   op     PS / FD2 for periodic, Dirichlet, Neumann; GREEN_GAUSS2 .. GREEN_GAUSS10 for unbounded plans
  *          (3-D: -erf(r / sqrt2 eps) / (4 pi r) and its higher orders; 2-D: (ln r + E1(r^2 / 2 eps^2) / 2) / (2 pi)
- *          and its higher orders), GREEN_SPECTRAL for 3-D unbounded plans.
+ *          and its higher orders), GREEN_SPECTRAL for 3-D and 2-D unbounded plans.
  *   prec   arithmetic and storage type of every array passed later.
  *   opt    [host] may be NULL (defaults above).
  * For unbounded plans this call evaluates G on the doubled grid, transforms it with the library's
  * own fp64 kernels and stores the real, even spectrum as a compact (n+1)^3 table.
- * Errors: INVALID_ARG, UNSUPPORTED (a periodic / unbounded axis mixed with another type, sizes above, GREEN_SPECTRAL in 2-D, ncomp not 1 or 3,
+ * Errors: INVALID_ARG, UNSUPPORTED (a periodic / unbounded axis mixed with another type, sizes above, ncomp not 1 or 3,
  * PS/FD2 on unbounded or GREEN on bounded plans), ALLOC, CUDA.
  */
 sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const double h[3], const sf_bc bc[3],

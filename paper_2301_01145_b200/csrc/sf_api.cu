@@ -322,8 +322,42 @@ __device__ double laguerre_tail(int order, double alpha, double x)
     }
     return acc;
 }
+// C(x) = int_0^x (1 - J0(t)) / t dt for the 2-D spectrally compact kernel, as a Neumann series: with 1 = J0 + 2 sum J_2k,
+// J_2k / t = (J_{2k-1} + J_{2k+1}) / 4k and int_0^x J_m = 2 sum_{j>=0} J_{m+1+2j}(x) the integral collapses to
+//     C(x) = sum_{i>=1} (2 H_i - 1/i) J_{2i}(x),   H_i the harmonic numbers,
+// the Bessel functions by Miller's downward recurrence J_{n-1} = (2n / x) J_n - J_{n+1}, normalised with J0 + 2 sum J_2k = 1
+__device__ double bessel_cin(double x)
+{
+    if (x < 1e-4) return 0.125 * x * x;                       // (x/2)^2 / 2, next term x^4 / 256
+    // start at J_{2M} far above the turning point n ~ x: beyond it J_n(x) falls off like exp(-(2/3) sqrt(2/x) (n - x)^(3/2)),
+    // so n - x ~ 14 x^(1/3) + 30 puts the start below 1e-20 of the values that matter
+    const int M = ((int)(x + 30.0 + 14.0 * cbrt(x))) / 2 + 1;
+    double hi = 0.0;
+    for (int i = 1; i <= M; ++i) hi += 1.0 / (double)i;       // H_M
+    double jp = 0.0, jn = 1e-30;                              // J_{n+1}, J_n (unnormalised), n = 2 M
+    double norm = 0.0, acc = 0.0;
+    const double ix = 1.0 / x;
+    for (int i = M; i >= 1; --i) {
+        // n = 2 i
+        norm += 2.0 * jn;
+        acc += (2.0 * hi - 1.0 / (double)i) * jn;
+        hi -= 1.0 / (double)i;                                // H_{i-1}
+        const double jo = (4.0 * i) * ix * jn - jp;           // J_{2i-1}
+        const double je = (4.0 * i - 2.0) * ix * jo - jn;     // J_{2i-2}
+        jp = jo; jn = je;
+        if (fabs(jn) > 1e120 || fabs(jp) > 1e120) { jn *= 1e-120; jp *= 1e-120; norm *= 1e-120; acc *= 1e-120; }
+    }
+    norm += jn;                                               // J_0
+    return acc / norm;
+}
 __device__ double green2d_value(double r, double eps, int order)
 {
+    if (order == 0) {
+        // spectrally compact kernel (reading A30), the grid spacing passed in `eps`: k_c = pi / h
+        const double kc = 3.14159265358979323846 / eps;
+        const double c0 = log(0.5 * kc) + 0.57721566490153286061;
+        return ((r == 0.0 ? 0.0 : bessel_cin(kc * r)) - c0) / 6.2831853071795864769;
+    }
     const double x = r * r / (2.0 * eps * eps);
     double v = (r == 0.0) ? (log(2.0 * eps * eps) - 0.57721566490153286061) / 12.566370614359172954
                           : (log(r) + 0.5 * exp_integral1(x)) / 6.2831853071795864769;
@@ -1016,7 +1050,6 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
     const sf_bc b = bc[0];
     if (b == SF_BC_UNBOUNDED) {
         if (!green_op) return fail(nullptr, SF_ERR_UNSUPPORTED, "unbounded plans use a Green's function operator");
-        if (ndim != 3 && op == SF_OP_GREEN_SPECTRAL) return fail(nullptr, SF_ERR_UNSUPPORTED, "the spectrally compact kernel is built for 3-D");
     } else if (green_op) {
         return fail(nullptr, SF_ERR_UNSUPPORTED, "Green's function operators need unbounded boundary conditions");
     }
