@@ -220,6 +220,9 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t by
 {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
 }
+// pull one 128-byte line towards the L2 (no register, no dependency); used where a pass loads its tiles straight into
+// registers and a tile is large (sf_fast512.cuh S4: 1024 rows; measured: -4 %; no gain for the 256- / 512-row tiles)
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 // all bulk stores of this thread have finished READING shared memory
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }

@@ -401,6 +401,13 @@ __global__ void __launch_bounds__(64 * PEN, 16 / PEN) fast5_kernel(const Fast5Pa
             }
         } else if constexpr (MODE == F5_INV) {
             // rows 2 k + h, k = w + 32 j
+            {   // the next tile's 1024 rows (one 128-byte line each) are asked into the L2 now
+                const int tn = s_tile[(it + 1) & 1];
+                if (tn < ntiles) {
+                    const Geom gn = geom(tn);
+                    if (gn.full) prefetch_l2(p.in + ((size_t)gn.b * ibs + gn.col + (size_t)tid * ips));
+                }
+            }
             const C* inp = p.in + ((size_t)(g.full ? g.b : min(g.b + pen, p.nb - 1)) * ibs + g.col + (g.full ? pen : 0) + (size_t)(2 * w + h) * ips);
 #pragma unroll
             for (int j = 0; j < 16; ++j) v[j] = __ldg(inp + (size_t)j * 64 * ips);
