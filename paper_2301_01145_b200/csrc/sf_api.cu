@@ -753,6 +753,11 @@ template <typename T> sf_status run(sf_plan p, int outk)
         fp.in = (const sf2::C*)p->W1; fp.out = (sf2::C*)p->W2;
         fp.in_ps = hp; fp.in_bs = hp * n1; fp.out_ps = hp; fp.out_bs = hp * P1; fp.nb = n2 * ncomp;
         fp.reverse_batches = 1;   // S1 wrote the last planes last: start there while they are in L2
+        // (S2, S3 on tiles of 8 columns -- two CTAs per SM; S4 on tiles of 16)
+        const int nct16 = fp.nct, shift16 = fp.nct_shift, nyq16 = fp.nyq_col;
+        fp.nct = p->nspec_x / 8;
+        for (fp.nct_shift = 0; (1 << fp.nct_shift) < fp.nct; ++fp.nct_shift) {}
+        fp.nyq_col = (p->nspec_x % 8) ? fp.nct * 8 : -1;
         SF_CUDA(p, sf2::launch_fast5(sf2::F5_FWD, fp, p->map_s2, st));
         fp.reverse_batches = 0;
         p->launches++;
@@ -760,10 +765,6 @@ template <typename T> sf_status run(sf_plan p, int outk)
         // S3: W2 in place along z, tiles of 8 columns
         fp.in = (const sf2::C*)p->W2; fp.out = (sf2::C*)p->W2;
         fp.in_ps = fp.out_ps = hp * P1; fp.in_bs = fp.out_bs = hp; fp.in_cs = fp.out_cs = p->w2_field; fp.nb = P1;
-        const int nct16 = fp.nct, shift16 = fp.nct_shift, nyq16 = fp.nyq_col;
-        fp.nct = p->nspec_x / 8;
-        for (fp.nct_shift = 0; (1 << fp.nct_shift) < fp.nct; ++fp.nct_shift) {}
-        fp.nyq_col = (p->nspec_x % 8) ? fp.nct * 8 : -1;
         fp.pair_batches = 1;
         fp.green_tiles = (const float*)p->green_tiles; fp.Pb = P1;
         fp.kap_x = (const float*)p->kap[0]; fp.kap_b = (const float*)p->kap[1]; fp.kap_p = (const float*)p->kap[2];
@@ -1240,7 +1241,7 @@ sf_status sf_plan_create(sf_plan* out, int ndim, const long long n[3], const dou
         {
             // S2: W1 as (column, y, batch = component * n2 + z)
             const unsigned long long d[4] = { hpc, N1, N2 * (unsigned long long)ncomp, 1 }, sb[3] = { hpB, hpB * N1, hpB * N1 * N2 * ncomp };
-            const unsigned bx[4] = { 16, 256, 1, 1 };
+            const unsigned bx[4] = { 8, 256, 1, 1 };
             e1 = sf2::fast_make_map(&p->map_s2, p->W1, d, sb, bx);
         }
         {

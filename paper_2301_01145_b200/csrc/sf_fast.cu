@@ -82,7 +82,7 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FUSED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FWD, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FWD, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_INV, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5NoSlot)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FUSED, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_CURL, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
@@ -201,8 +201,8 @@ cudaError_t launch_fast5(int mode, const Fast5Params& p, const TileMap& in_map, 
         return cudaErrorInvalidValue;
     if (mode == F5_CURL && (p.ncomp != 3 || !p.kap_x || !p.kap_b || !p.kap_p || 3 * p.out_cs >= (1ll << 31))) return cudaErrorInvalidValue;
     if ((mode == F5_CURL || mode == F5_FUSED) && !p.green_tiles) return cudaErrorInvalidValue;
-    // FWD / INV: 16-pencil tiles, one CTA per SM; FUSED / CURL: 8-pencil tiles, two CTAs per SM (p.nct counts those)
-    const bool half = (mode == F5_FUSED || mode == F5_CURL);
+    // INV: 16-pencil tiles, one CTA per SM; FWD / FUSED / CURL: 8-pencil tiles, two CTAs per SM (p.nct counts those)
+    const bool half = (mode != F5_INV);
     const int pen = half ? 8 : 16;
     const long long ntiles = ((long long)p.nb * p.nct + (p.nyq_col >= 0 ? (p.nb + pen - 1) / pen : 0)) * (mode == F5_FUSED ? p.ncomp : 1);
     if (ntiles + 4ll * g_sms >= (1ll << 31)) return cudaErrorInvalidValue;
@@ -210,8 +210,8 @@ cudaError_t launch_fast5(int mode, const Fast5Params& p, const TileMap& in_map, 
     if (grid > ntiles) grid = (int)ntiles;
     if (grid <= 0) return cudaErrorInvalidValue;
     switch (mode) {
-    case F5_FWD: fast5_kernel<F5_FWD, 16><<<grid, kT5, kSmem5, st>>>(p, tm); break;
-    case F5_INV: fast5_kernel<F5_INV, 16><<<grid, kT5, kSmem5NoSlot, st>>>(p, tm); break;
+    case F5_FWD: fast5_kernel<F5_FWD, 8><<<grid, kT5 / 2, kSmem5 / 2, st>>>(p, tm); break;   // (measured: 2.08 -> 1.98 ms on cfg 5)
+    case F5_INV: fast5_kernel<F5_INV, 16><<<grid, kT5, kSmem5NoSlot, st>>>(p, tm); break;      // (8-pencil tiles: 2.13 -> 2.21 ms)
     // the multiplying passes work on 8-pencil tiles: two 512-thread CTAs per SM
     case F5_FUSED: fast5_kernel<F5_FUSED, 8><<<grid, kT5 / 2, kSmem5 / 2, st>>>(p, tm); break;
     case F5_CURL: fast5_kernel<F5_CURL, 8><<<grid, kT5 / 2, kSmem5 / 2, st>>>(p, tm); break;
