@@ -326,7 +326,10 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
         "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": DEFAULT_WORKLOAD, "grid": "256^3 cell-centre padded to 512^3", "sample": sample},
+        # the same keys as the line of our own arm (the workload is the same; the sample of it that is timed is stated)
+        "config": {"workload": DEFAULT_WORKLOAD, "grid": "256^3 padded to 512^3", "call": "sf_solve", "ncomp": 1,
+                   "parallelism": "replicas x1", "l2": "host run: not applicable",
+                   "timed_region": "the oracle's solve on the host cores, Green's spectrum precomputed outside (PAPER.md:53, :344); " + sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,

@@ -6,14 +6,16 @@
 //
 // Same ideas as sf_fast.cuh, one size up.  The 1024-point transform of (x, 0) is two 512-point transforms
 // (h = 0: x -> even outputs; h = 1: x w1024^n -> odd outputs) that run side by side in the two half-warps.
-// A CTA of 1024 threads owns a tile of 16 neighbouring pencils (one 128-byte run per row): warp index
-// w in 0..31 (warp-uniform), lane = pencil + 16 h.  Thread (w, pencil, h) holds the 16 elements
-// n = w + 32 r of its sequence.  A 512-point transform is
+// A residue w in 0..31 of the 512-point transform owns 2 PEN consecutive threads = PEN neighbouring pencils x the two
+// halves h; thread (w, pencil, h) holds the 16 elements n = w + 32 r of its sequence.  A 512-point transform is
 //     radix-16 over r (registers) -> twiddle w512^(q w) -> ONE shared-memory exchange ->
 //     radix-32 over the 32 values o of slot row q0 = w mod 16, done as a radix-2 step that keeps the
 //     output parity p = w div 16 (16 sums or twiddled differences) and a radix-16 over the rest (registers)
 // and leaves X[w + 32 j] in thread w: input and output distributions agree, so forward, multiply and
-// backward chain without reordering.  One CTA per SM (128 KB exchange buffer + 64 KB TMA slot).
+// backward chain without reordering.  PEN = 16 (S4): one CTA of 1024 threads per SM, warp = residue (warp-uniform
+// twiddles), 128 KB exchange buffer, the tile loaded straight into registers.  PEN = 8 (S2, S3): two CTAs of 512
+// threads per SM (64 KB exchange buffer + 32 KB TMA slot each) -- two barrier domains, one transforms while the
+// other waits; measured on cfg 5: S2 2.08 -> 1.98 ms, S3 (a chain of six transforms per tile) 7.14 -> 6.39 ms.
 //
 // Vector plans: sf_curl needs psi_hat of all three components at every spectral point, 393 KB per tile --
 // more than the registers or the shared memory of an SM hold next to the exchange buffer.  The two spectra
