@@ -977,7 +977,8 @@ int orc_bounded_gradient(int kind, const i64 n[3], const double h[3], int op, do
                 double kk = PI * idx / (cells * h[a]);
                 lam[a][k] = -kk * kk;
             } else {
-                double sn = sin(PI * idx / (2.0 * cells));
+                double sn, cs;
+                sincos2pi((i64)idx, 4 * (i64)cells, &sn, &cs);   /* sin(pi idx / (2 cells)), integer-reduced like every other eigenvalue */
                 lam[a][k] = -(4.0 / (h[a] * h[a])) * sn * sn;
             }
         }
