@@ -9,6 +9,7 @@
 #include "sf_fastx64.cuh"
 #include "sf_fastr2r64.cuh"
 #include "sf_fastper64.cuh"
+#include "sf_fastxw.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -69,6 +70,17 @@ cudaError_t fast_init()
             }
         if ((e = cudaMemcpyToSymbol(g_tab_pad, tp.data(), sizeof(float2) * 768)) != cudaSuccess) return e;
         if ((e = cudaMemcpyToSymbol(g_tab_x, tx.data(), sizeof(float2) * 544)) != cudaSuccess) return e;
+        // the same factors for the warp-autonomous X passes (sf_fastxw.cuh), residue w fastest
+        std::vector<float2> txw(kXwTab, make_float2(0.f, 0.f));
+        for (int a = 0; a < 16; ++a)
+            for (int w = 0; w < 8; ++w) {
+                txw[a * 8 + w] = tw[8 * a * w];
+                txw[128 + a * 16 + w] = make_float2(1.f, 0.f);
+                txw[128 + a * 16 + 8 + w] = tw[4 * (w + 8 * a)];
+            }
+        for (int m = 0; m < 9; ++m)
+            for (int i = 0; i < 16; ++i) txw[384 + m * 16 + i] = tw[2 * (i + 16 * m)];
+        if ((e = cudaMemcpyToSymbol(g_tab_xw, txw.data(), sizeof(float2) * kXwTab)) != cudaSuccess) return e;
     }
     if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_FWD>::kSmem)) != cudaSuccess) return e;
@@ -82,6 +94,8 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_per_kernel<FMODE_FUSED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPerSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_xw_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXwSmemFwd)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_xw_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXwSmemInv)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FWD, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_INV, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5NoSlot)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FUSED, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
@@ -414,6 +428,15 @@ cudaError_t launch_fast_x(bool inv, const FastXParams& p, cudaStream_t st)
 {
     if (p.nrows <= 0 || p.nrows % kXRows) return cudaErrorInvalidValue;
     int grid = 2 * g_sms;
+    // one pipeline per warp (sf_fastxw.cuh); SF_X_CTA=1 selects the kernel with one pipeline per CTA
+    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    if (!cta_kernel) {
+        const int need = (p.nrows / 2 + kXwWarps - 1) / kXwWarps;
+        if (grid > need) grid = need;
+        if (inv) fast_xw_kernel<true><<<grid, kXwThreads, kXwSmemInv, st>>>(p);
+        else fast_xw_kernel<false><<<grid, kXwThreads, kXwSmemFwd, st>>>(p);
+        return cudaGetLastError();
+    }
     if (grid > p.nrows / kXRows) grid = p.nrows / kXRows;
     if (inv) fast_x_kernel<true><<<grid, kXThreads, kXSmem, st>>>(p);
     else fast_x_kernel<false><<<grid, kXThreads, kXSmem, st>>>(p);
