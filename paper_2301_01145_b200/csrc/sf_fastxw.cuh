@@ -10,10 +10,15 @@
 // only synchronisation left is __syncwarp.  Sixteen such pipelines run per SM, each at its own phase.
 //   forward: the padded real row is packed as z[n] = x[2n] + i x[2n+1], n < 256, non-zero for n < 128.
 //   Z = DFT256(z) = two 128-point transforms, of z (even outputs, h = 0) and of z w256^n (odd outputs, h = 1);
-//   then the real-transform split X[k] = ((Z[k] + conj Z[256-k]) - i w512^k (Z[k] - conj Z[256-k])) / 2 in the
-//   staged row, which leaves by one bulk store.  backward: the mirror.
+//   then the real-transform split X[k] = ((Z[k] + conj Z[256-k]) - i w512^k (Z[k] - conj Z[256-k])) / 2.
+//   backward: the mirror.
 //   128-point transform: radix-16 over r (n = w + 8 r), twiddle w128^(q w), one exchange between the eight
 //   threads of the group, two radix-8 over o' for q = w and q = w + 8.
+// Both passes are bound by shared-memory bandwidth, not by HBM (ncu: l1tex 78 % with staged output rows), so the
+// shared memory is used for the input rows and the one exchange only: the thread with lane index idx = 2 w + h ends
+// up with Z[idx + 16 j], j < 16, the partner 256 - k of its k sits in the thread 16 - idx as j' = 15 - j, so the
+// split (and the merge of S5) pair up through 16 shuffles, and the results leave by plain 8-byte stores: the 16
+// lanes of a row write 128 consecutive bytes.
 // Shared-memory words are 8 bytes (one complex); every access of a half-warp (one row, 8 residues x 2 halves) is
 // either 16 consecutive words or 8 words with stride 9 plus the same 8 shifted by 8 (mod 16): no bank conflicts.
 #pragma once
@@ -30,9 +35,9 @@ constexpr int kXwTab = 528;                   // tw128[q][w] | twin[j][h][w] | t
 constexpr size_t kXwRealBytes = 2 * (size_t)kXwInPitch * sizeof(float);   // a pair of real rows
 constexpr size_t kXwSpecBytes = 2 * (size_t)kXSpPitch * sizeof(C);        // a pair of spectrum rows
 constexpr size_t kXwXchBytes = 4 * (size_t)kXwGP * sizeof(C);
-// forward: two input pairs (prefetch distance two), exchange, one output pair;  backward: one of each
-constexpr size_t kXwWarpBytesFwd = 2 * kXwRealBytes + kXwXchBytes + kXwSpecBytes;
-constexpr size_t kXwWarpBytesInv = kXwSpecBytes + kXwXchBytes + kXwRealBytes;
+// forward: two input pairs (prefetch distance two) and the exchange;  backward: one input pair and the exchange
+constexpr size_t kXwWarpBytesFwd = 2 * kXwRealBytes + kXwXchBytes;
+constexpr size_t kXwWarpBytesInv = kXwSpecBytes + kXwXchBytes;
 constexpr size_t kXwSmemFwd = kXwWarps * kXwWarpBytesFwd;
 constexpr size_t kXwSmemInv = kXwWarps * kXwWarpBytesInv;
 
@@ -56,6 +61,7 @@ template <bool INV> __device__ __forceinline__ void fftw128_b(C (&a)[8], C (&b)[
     dft8<INV>(b);
 }
 
+
 template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_kernel(const FastXParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -69,6 +75,8 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
     const int h = (lane >> 3) & 1;
     const int rr = lane >> 4;
     const int idx = 2 * w + h;
+    // the thread that holds the residue 16 - idx (mod 16) of the same row: idx = 0 and idx = 8 are their own partners
+    const int plane = ((8 - w - h) & 7) + 8 * h + 16 * rr;
 
     for (int i = tid; i < kXwTab / 2; i += kXwThreads) reinterpret_cast<float4*>(s_tab)[i] = reinterpret_cast<const float4*>(g_tab_xw)[i];
     if (lane == 0) {
@@ -78,18 +86,19 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
     }
     const C* t128 = s_tab + w;                    // [q * 8]
     const C* tin = s_tab + 128 + h * 8 + w;       // [j * 16]: w256^(w + 8 j) for h = 1, 1 for h = 0
-    const C* tsp = s_tab + 384 + idx;             // [m * 16]: w512^(idx + 16 m)
+    __syncthreads();
+    C tsp[8];                                     // w512^(idx + 16 m): the same in every iteration
+#pragma unroll
+    for (int m = 0; m < 8; ++m) tsp[m] = s_tab[384 + idx + 16 * m];
 
     unsigned char* wbase = smem_raw + (size_t)wid * (INV ? kXwWarpBytesInv : kXwWarpBytesFwd);
-    // forward: rin[2][2][kXwInPitch] | xch | sp[2][kXSpPitch];   backward: sp | xch | rout[2][kXwInPitch]
-    float* rbuf = reinterpret_cast<float*>(INV ? wbase + kXwSpecBytes + kXwXchBytes : wbase);
+    // forward: rin[2][2][kXwInPitch] | xch;   backward: sp[2][kXSpPitch] | xch
+    float* rbuf = reinterpret_cast<float*>(wbase);
+    C* sp = reinterpret_cast<C*>(wbase);
     C* xch = reinterpret_cast<C*>(wbase + (INV ? kXwSpecBytes : 2 * kXwRealBytes));
-    C* sp = reinterpret_cast<C*>(INV ? wbase : wbase + 2 * kXwRealBytes + kXwXchBytes);
     C* xw = xch + (rr * 2 + h) * kXwGP + w;              // slot (q, w) at q * kXwQP
     const C* xr = xch + (rr * 2 + h) * kXwGP + w * kXwQP; // slots (w, o') and (w + 8, o')
-    C* srow = sp + rr * kXSpPitch;
-    if (!INV && idx == 0) srow[kXN + 1] = make_float2(0.f, 0.f);   // pad column 257 leaves as zero
-    __syncthreads();
+    const C* srow = sp + rr * kXSpPitch;
 
     const long long npairs = p.nrows / 2;
     const long long gw = (long long)blockIdx.x * kXwWarps + wid;
@@ -125,7 +134,7 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
     issue(0);
     if (!INV) issue(1);
     for (int i = 0; i < nit; ++i) {
-        const long long row0 = first_row(i);
+        const long long row = first_row(i) + rr;
         C v[16];
         if constexpr (!INV) {
             // ---------------------------------------------------------------- S1
@@ -138,92 +147,74 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
             issue(i + 2);                         // this input buffer is in registers in every lane
             C a[8], b[8];
             fftw128_b<false>(a, b, xr);
-            if (lane == 0) bulk_wait_read();      // the previous pair's stores have left the staged rows
-            __syncwarp();
-            // Z[2 k' + h], k' = w + 16 k2 (a) and w + 8 + 16 k2 (b), natural order into the staged row
+            // this thread now holds Z[idx + 16 j]: j = 2 k2 in a[brev3(k2)], j = 2 k2 + 1 in b[brev3(k2)].
+            // The real-transform split pairs k = idx + 16 m, m < 8, with 256 - k = (16 - idx) + 16 (15 - m): the
+            // upper half j >= 8 of the partner thread, which arrives by shuffle (idx = 0: 256 - 16 m is its own)
+            C* orow = p.spec + row * p.spec_pitch;
 #pragma unroll
-            for (int k2 = 0; k2 < 8; ++k2) {
-                srow[2 * (w + 16 * k2) + h] = a[brev3(k2)];
-                srow[2 * (w + 8 + 16 * k2) + h] = b[brev3(k2)];
-            }
-            __syncwarp();
-            // split in place: the 16 threads of a row own the pairs (k, 256 - k), k = idx + 16 m
-            C xn = make_float2(0.f, 0.f);
-            {
-                C zk[9], zm[9];
-#pragma unroll
-                for (int m = 0; m < 9; ++m) {
-                    const int k = idx + 16 * m;
-                    if (m < 8 || idx == 0) { zk[m] = srow[k]; zm[m] = srow[(kXN - k) & (kXN - 1)]; }
-                }
-#pragma unroll
-                for (int m = 0; m < 9; ++m) {
-                    const int k = idx + 16 * m;
-                    if (m < 8 || idx == 0) {
-                        const C e = cadd(zk[m], make_float2(zm[m].x, -zm[m].y));
-                        const C d = csub(zk[m], make_float2(zm[m].x, -zm[m].y));
-                        const C wd = cmul(d, tsp[16 * m]);   // w512^k d
-                        // X[k] = (e - i wd) / 2,  X[256 - k] = (conj e - i conj wd) / 2
-                        const C xhi = cscale(make_float2(e.x - wd.y, -e.y - wd.x), 0.5f);
-                        srow[k] = cscale(cadd(e, make_float2(wd.y, -wd.x)), 0.5f);
-                        srow[kXN - k] = xhi;
-                        if (m == 0) xn = xhi;
-                    }
+            for (int m = 0; m < 8; ++m) {
+                const int js = 15 - m, jo = (16 - m) & 15;
+                const C snd = (js & 1) ? b[brev3(js >> 1)] : a[brev3(js >> 1)];
+                const C own = (jo & 1) ? b[brev3(jo >> 1)] : a[brev3(jo >> 1)];
+                C zm;
+                zm.x = __shfl_sync(0xffffffffu, snd.x, plane);
+                zm.y = __shfl_sync(0xffffffffu, snd.y, plane);
+                if (idx == 0) zm = own;
+                const C zk = (m & 1) ? b[brev3(m >> 1)] : a[brev3(m >> 1)];
+                const C e = cadd(zk, make_float2(zm.x, -zm.y));
+                const C d = csub(zk, make_float2(zm.x, -zm.y));
+                const C wd = cmul(d, tsp[m]);   // w512^k d
+                // X[k] = (e - i wd) / 2,  X[256 - k] = (conj e - i conj wd) / 2
+                const int k = idx + 16 * m;
+                const C xhi = cscale(make_float2(e.x - wd.y, -e.y - wd.x), 0.5f);
+                orow[k] = cscale(cadd(e, make_float2(wd.y, -wd.x)), 0.5f);
+                orow[kXN - k] = xhi;
+                if (m == 0 && idx == 0) {
+                    // the Nyquist coefficient X[256] of row (z, y) also goes to the side array [y][z] that the
+                    // strided passes read it from in 128-byte runs; pad column 257 leaves as zero
+                    orow[kXN + 1] = make_float2(0.f, 0.f);
+                    if (p.nyq) p.nyq[((int)row % p.n1) * p.n2 + (int)row / p.n1] = xhi;
                 }
             }
-            fence_async_smem();
-            __syncwarp();
-            if (lane == 0) {
-                bulk_s2g(p.spec + row0 * p.spec_pitch, sp, kXSpPitch * (uint32_t)sizeof(C));
-                bulk_s2g(p.spec + (row0 + 1) * p.spec_pitch, sp + kXSpPitch, kXSpPitch * (uint32_t)sizeof(C));
-                bulk_commit();
-            }
-            // the Nyquist coefficient X[256] of row (z, y) also goes to the side array [y][z] that the strided
-            // passes read it from in 128-byte runs
-            if (p.nyq && idx == 0) {
-                const int row = (int)row0 + rr;
-                p.nyq[(row % p.n1) * p.n2 + row / p.n1] = xn;
-            }
+            if (idx == 0) orow[kXN / 2] = make_float2(a[brev3(4)].x, -a[brev3(4)].y);   // k = 128 pairs with itself: conj Z[128]
         } else {
             // ---------------------------------------------------------------- S5
             const C xnyq = xnyq_next;
             mbar_wait(&bars[wid][0], i & 1);
-            // merge in place: Z[k] = e + i conj(w512^k) d, Z[256 - k] = conj e + i conj(conj(w512^k) d)
-            {
-                C xk[9], xm[9];
+            // merge: Z[k] = e + i conj(w512^k) d, Z[256 - k] = conj e + i conj(conj(w512^k) d) for the pairs
+            // k = idx + 16 m, m < 8.  Z[k] is this thread's v[m]; Z[256 - k] is v[15 - m] of the partner thread
+            C zhi[8];
 #pragma unroll
-                for (int m = 0; m < 9; ++m) {
-                    const int k = idx + 16 * m;
-                    if (m < 8 || idx == 0) { xk[m] = srow[k]; xm[m] = srow[kXN - k]; }
-                    if (m == 0 && idx == 0 && p.nyq) xm[0] = xnyq;
-                }
-#pragma unroll
-                for (int m = 0; m < 9; ++m) {
-                    const int k = idx + 16 * m;
-                    if (m < 8 || idx == 0) {
-                        const C e = cadd(xk[m], make_float2(xm[m].x, -xm[m].y));
-                        const C d = csub(xk[m], make_float2(xm[m].x, -xm[m].y));
-                        const C wd = cmulc(d, tsp[16 * m]);   // conj(w512^k) d
-                        srow[k] = cadd(e, make_float2(-wd.y, wd.x));
-                        if (k > 0) srow[kXN - k] = make_float2(e.x + wd.y, wd.x - e.y);
-                    }
-                }
+            for (int m = 0; m < 8; ++m) {
+                const int k = idx + 16 * m;
+                const C xk = srow[k];
+                C xm = srow[kXN - k];
+                if (m == 0 && idx == 0 && p.nyq) xm = xnyq;
+                const C e = cadd(xk, make_float2(xm.x, -xm.y));
+                const C d = csub(xk, make_float2(xm.x, -xm.y));
+                const C wd = cmulc(d, tsp[m]);   // conj(w512^k) d
+                v[m] = cadd(e, make_float2(-wd.y, wd.x));
+                zhi[m] = make_float2(e.x + wd.y, wd.x - e.y);
             }
-            __syncwarp();
+            const C x128 = srow[kXN / 2];
 #pragma unroll
-            for (int j = 0; j < 16; ++j) v[j] = srow[2 * (w + 8 * j) + h];   // Z[2 k' + h], k' = w + 8 j
-            fftw128_a<true>(v, t128, xw);
-            fence_async_smem();                   // the merged values in the staged rows are overwritten by the next bulk load
+            for (int j = 8; j < 16; ++j) {
+                C r;
+                r.x = __shfl_sync(0xffffffffu, zhi[15 - j].x, plane);
+                r.y = __shfl_sync(0xffffffffu, zhi[15 - j].y, plane);
+                // idx = 0: 256 - 16 m = 16 (16 - m) is its own; Z[128] = 2 conj X[128]
+                if (idx == 0) r = (j == 8) ? make_float2(2.f * x128.x, -2.f * x128.y) : zhi[(16 - j) & 7];
+                v[j] = r;
+            }
+            fftw128_a<true>(v, t128, xw);   // v[j] = Z[2 k' + h], k' = w + 8 j
             __syncwarp();
             issue(i + 1);                         // the staged rows are in registers in every lane
             xnyq_next = load_nyq(i + 1);
             C a[8], b[8];
             fftw128_b<true>(a, b, xr);
-            if (lane == 0) bulk_wait_read();      // the previous pair's stores have left the real rows
-            __syncwarp();
             // z[n] = z0[n] + conj(w256^n) z1[n], n = w + 16 k2 (a) / w + 8 + 16 k2 (b): h = 0 holds z0, h = 1 holds
             // z1; h = 0 finishes the a set, h = 1 the b set
-            float* rrow = rbuf + rr * kXwInPitch;
+            C* orow = reinterpret_cast<C*>(p.real_out + row * kXN);
 #pragma unroll
             for (int k2 = 0; k2 < 8; ++k2) {
                 // (the table row of h = 0 is all ones)
@@ -233,20 +224,10 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
                 C recv;
                 recv.x = __shfl_xor_sync(0xffffffffu, send.x, 8);
                 recv.y = __shfl_xor_sync(0xffffffffu, send.y, 8);
-                const C z = cadd(keep, recv);
-                const int n = w + 8 * h + 16 * k2;
-                *reinterpret_cast<C*>(rrow + 2 * n) = z;   // (x[2n], x[2n+1])
-            }
-            fence_async_smem();
-            __syncwarp();
-            if (lane == 0) {
-                bulk_s2g(p.real_out + row0 * kXN, rbuf, kXN * (uint32_t)sizeof(float));
-                bulk_s2g(p.real_out + (row0 + 1) * kXN, rbuf + kXwInPitch, kXN * (uint32_t)sizeof(float));
-                bulk_commit();
+                orow[w + 8 * h + 16 * k2] = cadd(keep, recv);   // (x[2n], x[2n+1])
             }
         }
     }
-    if (lane == 0) bulk_wait_read();
 }
 
 } // namespace sf2
