@@ -72,14 +72,14 @@ cudaError_t fast_init()
         if ((e = cudaMemcpyToSymbol(g_tab_x, tx.data(), sizeof(float2) * 544)) != cudaSuccess) return e;
         // the same factors for the warp-autonomous X passes (sf_fastxw.cuh), residue w fastest
         std::vector<float2> txw(kXwTab, make_float2(0.f, 0.f));
-        for (int a = 0; a < 16; ++a)
-            for (int w = 0; w < 8; ++w) {
-                txw[a * 8 + w] = tw[8 * a * w];
-                txw[128 + a * 16 + w] = make_float2(1.f, 0.f);
-                txw[128 + a * 16 + 8 + w] = tw[4 * (w + 8 * a)];
-            }
-        for (int m = 0; m < 9; ++m)
-            for (int i = 0; i < 16; ++i) txw[384 + m * 16 + i] = tw[2 * (i + 16 * m)];
+        for (int q = 0; q < 16; ++q)
+            for (int h = 0; h < 2; ++h)
+                for (int w = 0; w < 8; ++w) {
+                    txw[q * 16 + h * 8 + w] = tw[(4 * (2 * q + h) * w) & 1023];
+                    txw[256 + q * 16 + h * 8 + w] = tw[(4 * q * (2 * w + h)) & 1023];
+                }
+        for (int m = 0; m < 8; ++m)
+            for (int i = 0; i < 16; ++i) txw[512 + m * 16 + i] = tw[2 * (i + 16 * m)];
         if ((e = cudaMemcpyToSymbol(g_tab_xw, txw.data(), sizeof(float2) * kXwTab)) != cudaSuccess) return e;
     }
     if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;

@@ -23,6 +23,7 @@
 // either 16 consecutive words or 8 words with stride 9 plus the same 8 shifted by 8 (mod 16): no bank conflicts.
 #pragma once
 #include "sf_fast.cuh"
+#include "sf_fast512.cuh"   // mul_w32
 
 namespace sf2 {
 
@@ -31,7 +32,8 @@ constexpr int kXwThreads = 32 * kXwWarps;
 constexpr int kXwInPitch = kXN + 16;          // floats per staged real row: 1088 B = 64 (mod 128)
 constexpr int kXwQP = 9;                      // exchange: words per q
 constexpr int kXwGP = 152;                    // exchange: words per (row, half) group, 8 (mod 16)
-constexpr int kXwTab = 528;                   // tw128[q][w] | twin[j][h][w] | twsp[m][2 w + h]
+constexpr int kXwTab = 640;                   // forward tw[q][h][w] | backward tw[q][h][w] | twsp[m][2 w + h]
+constexpr int kXwTabCta = 384;                // what one kernel keeps in shared memory: its tw and twsp
 constexpr size_t kXwRealBytes = 2 * (size_t)kXwInPitch * sizeof(float);   // a pair of real rows
 constexpr size_t kXwSpecBytes = 2 * (size_t)kXSpPitch * sizeof(C);        // a pair of spectrum rows
 constexpr size_t kXwXchBytes = 4 * (size_t)kXwGP * sizeof(C);
@@ -43,12 +45,14 @@ constexpr size_t kXwSmemInv = kXwWarps * kXwWarpBytesInv;
 
 __device__ float2 g_tab_xw[kXwTab];
 
-// v[r] = a[w + 8 r] in; writes the twiddled radix-16 outputs into the group's exchange slots (q, w)
+// v[r] = a[w + 8 r] in; writes the twiddled radix-16 outputs into the group's exchange slots (q, w).  The table row
+// holds w128^(q w) times the factor of the odd half that does not depend on r (forward: w256^w of the input factor
+// w256^(w + 8 r); backward: w256^q of the output factor w256^(q + 16 k2)); the rest of those factors are immediates
 template <bool INV> __device__ __forceinline__ void fftw128_a(C (&v)[16], const C* t128, C* xw)
 {
     dft16<INV>(v);
 #pragma unroll
-    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], t128[q * 8]);   // w128^(q w)
+    for (int q = 0; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], t128[q * 16]);
 #pragma unroll
     for (int q = 0; q < 16; ++q) xw[q * kXwQP] = v[brev4(q)];
 }
@@ -66,7 +70,7 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bars[kXwWarps][2];
-    __shared__ __align__(16) C s_tab[kXwTab];
+    __shared__ __align__(16) C s_tab[kXwTabCta];
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
@@ -78,18 +82,19 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
     // the thread that holds the residue 16 - idx (mod 16) of the same row: idx = 0 and idx = 8 are their own partners
     const int plane = ((8 - w - h) & 7) + 8 * h + 16 * rr;
 
-    for (int i = tid; i < kXwTab / 2; i += kXwThreads) reinterpret_cast<float4*>(s_tab)[i] = reinterpret_cast<const float4*>(g_tab_xw)[i];
+    for (int i = tid; i < kXwTabCta / 2; i += kXwThreads)
+        reinterpret_cast<float4*>(s_tab)[i] = reinterpret_cast<const float4*>(g_tab_xw)[i + (i < 128 ? (INV ? 128 : 0) : 128)];
     if (lane == 0) {
         mbar_init(&bars[wid][0], 1);
         mbar_init(&bars[wid][1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    const C* t128 = s_tab + w;                    // [q * 8]
-    const C* tin = s_tab + 128 + h * 8 + w;       // [j * 16]: w256^(w + 8 j) for h = 1, 1 for h = 0
+    // [q * 16]: forward w256^((2 q + h) w), backward w256^(q (2 w + h))
+    const C* t128 = s_tab + h * 8 + w;
     __syncthreads();
     C tsp[8];                                     // w512^(idx + 16 m): the same in every iteration
 #pragma unroll
-    for (int m = 0; m < 8; ++m) tsp[m] = s_tab[384 + idx + 16 * m];
+    for (int m = 0; m < 8; ++m) tsp[m] = s_tab[256 + idx + 16 * m];
 
     unsigned char* wbase = smem_raw + (size_t)wid * (INV ? kXwWarpBytesInv : kXwWarpBytesFwd);
     // forward: rin[2][2][kXwInPitch] | xch;   backward: sp[2][kXSpPitch] | xch
@@ -141,7 +146,15 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
             mbar_wait(&bars[wid][i & 1], (i >> 1) & 1);
             const C* zin = reinterpret_cast<const C*>(rbuf + ((i & 1) * 2 + rr) * kXwInPitch) + w;
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(zin[8 * r], tin[16 * r]);   // h = 1: z w256^n
+            for (int r = 0; r < 16; ++r) v[r] = zin[8 * r];
+            // h = 1: z w256^n, n = w + 8 r: the factor w32^r here, w256^w with the twiddles after the radix-16
+            if (h) {
+                v[1] = mul_w32<1, false>(v[1]);   v[2] = mul_w32<2, false>(v[2]);   v[3] = mul_w32<3, false>(v[3]);
+                v[4] = mul_w32<4, false>(v[4]);   v[5] = mul_w32<5, false>(v[5]);   v[6] = mul_w32<6, false>(v[6]);
+                v[7] = mul_w32<7, false>(v[7]);   v[8] = mul_w32<8, false>(v[8]);   v[9] = mul_w32<9, false>(v[9]);
+                v[10] = mul_w32<10, false>(v[10]); v[11] = mul_w32<11, false>(v[11]); v[12] = mul_w32<12, false>(v[12]);
+                v[13] = mul_w32<13, false>(v[13]); v[14] = mul_w32<14, false>(v[14]); v[15] = mul_w32<15, false>(v[15]);
+            }
             fftw128_a<false>(v, t128, xw);
             __syncwarp();
             issue(i + 2);                         // this input buffer is in registers in every lane
@@ -212,13 +225,22 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
             xnyq_next = load_nyq(i + 1);
             C a[8], b[8];
             fftw128_b<true>(a, b, xr);
-            // z[n] = z0[n] + conj(w256^n) z1[n], n = w + 16 k2 (a) / w + 8 + 16 k2 (b): h = 0 holds z0, h = 1 holds
-            // z1; h = 0 finishes the a set, h = 1 the b set
+            // z[n] = z0[n] + conj(w256^n) z1[n], n = q + 16 k2, q = w (a) / w + 8 (b): h = 0 holds z0, h = 1 holds
+            // z1 conj(w256^q) (the factor came with the twiddles), conj(w16^k2) is applied here; h = 0 finishes the
+            // a set, h = 1 the b set
+            if (h) {
+                a[brev3(1)] = mul_w16<1, true>(a[brev3(1)]); b[brev3(1)] = mul_w16<1, true>(b[brev3(1)]);
+                a[brev3(2)] = mul_w16<2, true>(a[brev3(2)]); b[brev3(2)] = mul_w16<2, true>(b[brev3(2)]);
+                a[brev3(3)] = mul_w16<3, true>(a[brev3(3)]); b[brev3(3)] = mul_w16<3, true>(b[brev3(3)]);
+                a[brev3(4)] = mul_w16<4, true>(a[brev3(4)]); b[brev3(4)] = mul_w16<4, true>(b[brev3(4)]);
+                a[brev3(5)] = mul_w16<5, true>(a[brev3(5)]); b[brev3(5)] = mul_w16<5, true>(b[brev3(5)]);
+                a[brev3(6)] = mul_w16<6, true>(a[brev3(6)]); b[brev3(6)] = mul_w16<6, true>(b[brev3(6)]);
+                a[brev3(7)] = mul_w16<7, true>(a[brev3(7)]); b[brev3(7)] = mul_w16<7, true>(b[brev3(7)]);
+            }
             C* orow = reinterpret_cast<C*>(p.real_out + row * kXN);
 #pragma unroll
             for (int k2 = 0; k2 < 8; ++k2) {
-                // (the table row of h = 0 is all ones)
-                const C ta = cmulc(a[brev3(k2)], tin[32 * k2]), tb = cmulc(b[brev3(k2)], tin[32 * k2 + 16]);
+                const C ta = a[brev3(k2)], tb = b[brev3(k2)];
                 const C send = h ? ta : tb;
                 const C keep = h ? tb : ta;
                 C recv;
