@@ -10,6 +10,7 @@
 #include "sf_fastr2r64.cuh"
 #include "sf_fastper64.cuh"
 #include "sf_fastxw.cuh"
+#include "sf_fastxw64.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -364,8 +365,22 @@ cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st)
 }
 
 namespace {
+template <int MODE, bool INV> cudaError_t launch_xgw(const sf::XParams<double>& p, int ncomp, cudaStream_t st)
+{
+    constexpr size_t sm = xw64_smem<MODE, INV>();
+    const long long npairs = ((long long)p.ny * p.nz + 1) / 2;
+    long long gx = 2ll * g_sms;
+    if (gx > (npairs + kXw64Warps - 1) / kXw64Warps) gx = (npairs + kXw64Warps - 1) / kXw64Warps;
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(fast_xgw_kernel<MODE, INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)) != cudaSuccess) return e;
+    fast_xgw_kernel<MODE, INV><<<dim3((unsigned)gx, (unsigned)ncomp), kXw64Threads, sm, st>>>(p);
+    return cudaGetLastError();
+}
 template <int MODE> cudaError_t launch_xg_mode(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st)
 {
+    // one pipeline per warp (sf_fastxw64.cuh); SF_X_CTA=1 selects the kernel with one pipeline per CTA
+    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    if (!cta_kernel) return inv ? launch_xgw<MODE, true>(p, ncomp, st) : launch_xgw<MODE, false>(p, ncomp, st);
     const long long ntiles = ((long long)p.ny * p.nz + kXgRows - 1) / kXgRows;
     long long gx = 4ll * g_sms;
     if (gx > ntiles) gx = ntiles;
