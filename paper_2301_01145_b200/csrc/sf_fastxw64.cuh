@@ -21,13 +21,14 @@ constexpr int kXw64Threads = 32 * kXw64Warps;
 constexpr int kXw64QP = 17;                                    // exchange: 16-byte words per q (odd: conflict-free reads)
 constexpr int kXw64GP = 16 * kXw64QP;                          // exchange: words per row
 constexpr size_t kXw64XchBytes = 2 * (size_t)kXw64GP * sizeof(D);
+constexpr int kXw64RP = 258;   // doubles per staged real row
 template <int MODE, bool INV> constexpr bool xw64_cplx_in() { return INV && MODE == sf::X_ZEROPAD; }
 // raw rows: real rows are double-buffered (prefetch distance two), the 4 KB complex rows of the backward zero-padded
 // pass single-buffered, so that twelve warps fit an SM in every mode
 template <int MODE, bool INV> constexpr int xw64_nbuf() { return xw64_cplx_in<MODE, INV>() ? 1 : 2; }
 template <int MODE, bool INV> constexpr size_t xw64_raw_bytes()
 {
-    return 2 * (xw64_cplx_in<MODE, INV>() ? (size_t)kXgSP * sizeof(D) : (size_t)kXgRP * sizeof(double));
+    return 2 * (xw64_cplx_in<MODE, INV>() ? (size_t)kXgSP * sizeof(D) : (size_t)kXw64RP * sizeof(double));
 }
 template <int MODE, bool INV> constexpr size_t xw64_warp_bytes() { return xw64_nbuf<MODE, INV>() * xw64_raw_bytes<MODE, INV>() + kXw64XchBytes; }
 template <int MODE, bool INV> constexpr size_t xw64_smem() { return kXw64Warps * xw64_warp_bytes<MODE, INV>(); }
@@ -82,46 +83,49 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
     // the rows this pass reads: the source (S1), the real spectrum rows (S5, real-to-real) or the half spectra (S5, padded)
     const double* rsrc = INV ? reinterpret_cast<const double*>(p.spec_in) + comp * p.sp_pc : p.real_in + comp * p.rin_pc;
 
+    // a lane's row of iteration i; past the end (odd row count) the last row is done twice, by both half-warps, with
+    // identical stores: no validity tests anywhere
     struct Geom {
-        bool valid;
         int iy, iz;
-        long long rin, sp;
     };
+    const unsigned last_row = (unsigned)(nrows - 1);
     auto geometry = [&](int i) {
-        Geom g;
         const long long r = 2 * (gw + (long long)i * nw) + rr;
-        g.valid = i < nit && r < nrows;
-        g.iy = (int)(r % p.ny);
-        g.iz = (int)(r / p.ny);
-        g.rin = g.iy * p.rin_py + g.iz * p.rin_pz;
-        g.sp = g.iy * p.sp_py + g.iz * p.sp_pz;
+        const unsigned rc = r < (long long)last_row ? (unsigned)r : last_row;
+        Geom g;
+        g.iz = (int)(rc / (unsigned)p.ny);
+        g.iy = (int)(rc - (unsigned)g.iz * (unsigned)p.ny);
         return g;
     };
+    auto rin_of = [&](const Geom& g) { return g.iy * p.rin_py + g.iz * p.rin_pz; };
+    auto sp_of = [&](const Geom& g) { return g.iy * p.sp_py + g.iz * p.sp_pz; };
     // the half-warp of a row copies it into buffer i % NBUF, lanes along the row
-    auto prefetch = [&](int i) {
+    auto prefetch = [&](int i, const Geom& g) {
         if (i < nit) {
-            const Geom g = geometry(i);
             unsigned char* buf = wbase + (i % NBUF) * RAW;
             if constexpr (CIN) {
                 D* dst = reinterpret_cast<D*>(buf) + rr * kXgSP;
-                const D* src = reinterpret_cast<const D*>(p.spec_in) + comp * p.sp_pc + g.sp;
+                const D* src = reinterpret_cast<const D*>(p.spec_in) + comp * p.sp_pc + sp_of(g);
 #pragma unroll
-                for (int t = 0; t < 17; ++t) {
-                    const int k = o + 16 * t;
-                    if (k <= 256) {
-                        if (g.valid) cp_async16(dst + k, src + k);
-                        else dst[k] = make_double2(0.0, 0.0);
-                    }
-                }
+                for (int t = 0; t < 16; ++t) cp_async16(dst + o + 16 * t, src + o + 16 * t);
+                if (o == 0) cp_async16(dst + 256, src + 256);
             } else {
-                double* dst = reinterpret_cast<double*>(buf) + rr * kXgRP;
-                const double* src = rsrc + (INV ? g.sp : g.rin);
+                // 16-byte copies when both rows of the pair start at 0 (mod 16) bytes (the last chunk of an odd row
+                // shrinks to the one element inside), 8-byte copies otherwise (dense rows of 255)
+                double* dst = reinterpret_cast<double*>(buf) + rr * kXw64RP;
+                const double* src = rsrc + (INV ? sp_of(g) : rin_of(g));
+                if (__all_sync(0xffffffffu, (reinterpret_cast<unsigned long long>(src) & 15ull) == 0ull)) {
 #pragma unroll
-                for (int t = 0; t < 16; ++t) {
-                    const int j = o + 16 * t;
-                    if (j < n) {
-                        if (g.valid) cp_async8(dst + j, src + j);
-                        else dst[j] = 0.0;
+                    for (int t = 0; t < 8; ++t) {
+                        const int j = 2 * (o + 16 * t);
+                        if (t < 7 || j + 2 <= n) cp_async16(dst + j, src + j);
+                        else if (j < n) cp_async8(dst + j, src + j);
+                    }
+                } else {
+#pragma unroll
+                    for (int t = 0; t < 16; ++t) {
+                        const int j = o + 16 * t;
+                        if (t < 15 || j < n) cp_async8(dst + j, src + j);
                     }
                 }
             }
@@ -129,26 +133,38 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
         cp_async_commit();
     };
 
-    prefetch(0);
-    if (NBUF == 2) prefetch(1);
+    // S1 with boundary values: a row off the y / z faces takes a term at its two ends only, which the lanes o < 2
+    // fetch one iteration ahead (rows on a face are rare and fold the whole row when they come up)
+    auto on_face = [&](const Geom& g) { return g.iy == 0 || g.iy == p.ny - 1 || g.iz == 0 || g.iz == p.nz - 1; };
+    auto end_term = [&](const Geom& g) -> double {
+        if (INV || !p.has_faces || o >= 2 || on_face(g)) return 0.0;
+        return sf::x_face_term(p, o ? n - 1 : 0, g.iy, g.iz);
+    };
+
+    Geom g0 = geometry(0), g1 = geometry(1);
+    prefetch(0, g0);
+    if (NBUF == 2) prefetch(1, g1);
+    double fterm_next = end_term(g0);
     for (int i = 0; i < nit; ++i) {
-        const Geom g = geometry(i);
+        const Geom g = g0;
+        const Geom gpf = NBUF == 2 ? geometry(i + 2) : g1;   // the rows of the next prefetch
+        g0 = g1;
+        g1 = NBUF == 2 ? gpf : geometry(i + 2);
+        const double fterm = fterm_next;
+        fterm_next = end_term(g0);
         cp_async_wait<NBUF - 1>();
         __syncwarp();
         unsigned char* buf = wbase + (i % NBUF) * RAW;
         D v[16];
         if constexpr (!INV) {
             // ---------------------------------------------------------------- S1
-            double* prow = reinterpret_cast<double*>(buf) + rr * kXgRP;
+            double* prow = reinterpret_cast<double*>(buf) + rr * kXw64RP;
             if (p.has_faces) {
                 // boundary values folded into the staged row
-                if (g.valid) {
-                    if (g.iy == 0 || g.iy == p.ny - 1 || g.iz == 0 || g.iz == p.nz - 1) {
-                        for (int ix = o; ix < n; ix += 16) prow[ix] += sf::x_face_term(p, ix, g.iy, g.iz);
-                    } else if (o < 2) {
-                        const int ix = o ? n - 1 : 0;
-                        prow[ix] += sf::x_face_term(p, ix, g.iy, g.iz);
-                    }
+                if (on_face(g)) {
+                    for (int ix = o; ix < n; ix += 16) prow[ix] += sf::x_face_term(p, ix, g.iy, g.iz);
+                } else if (o < 2) {
+                    prow[o ? n - 1 : 0] += fterm;
                 }
                 __syncwarp();
             }
@@ -171,7 +187,7 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
                 }
             }
             __syncwarp();   // the raw rows are in registers: fetch the rows of two iterations ahead
-            prefetch(i + NBUF);
+            prefetch(i + NBUF, gpf);
             dft16<false>(v);
 #pragma unroll
             for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul(v[brev4(q)], t256[q * 16]);
@@ -183,8 +199,8 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
             dft16<false>(v);
             // Z[o + 16 k2] at v[brev4(k2)].  Split X[k] = ((Z[k] + conj Z[256-k]) - i w512^k (Z[k] - conj Z[256-k])) / 2
             // for the pairs k = o + 16 m, m < 8, and 256 - k = (16 - o) + 16 (15 - m) of the partner thread
-            D* so = reinterpret_cast<D*>(p.spec_out) + comp * p.sp_pc + g.sp;
-            double* ro = p.real_out + comp * p.sp_pc + g.sp;
+            D* so = reinterpret_cast<D*>(p.spec_out) + comp * p.sp_pc + sp_of(g);
+            double* ro = p.real_out + comp * p.sp_pc + sp_of(g);
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
                 const D zk = v[brev4(m)];
@@ -194,7 +210,7 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
                 const D d = make_double2(zk.x - zm.x, zk.y + zm.y);
                 const D wd = cmul(d, tsp[m * 16]);
                 const int k = o + 16 * m;
-                if (g.valid) {
+                {
                     if constexpr (MODE == sf::X_ZEROPAD) {
                         so[k] = make_double2(0.5 * (e.x + wd.y), 0.5 * (e.y - wd.x));
                         so[256 - k] = make_double2(0.5 * (e.x - wd.y), 0.5 * (-e.y - wd.x));
@@ -212,7 +228,7 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
                     }
                 }
             }
-            if (o == 0 && g.valid) {
+            if (o == 0) {
                 // k = 128 pairs with itself: X~[128] = conj Z[128]
                 const D z = v[brev4(8)];
                 if constexpr (MODE == sf::X_ZEROPAD) so[128] = make_double2(z.x, -z.y);
@@ -225,7 +241,7 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
             // Z[k] = (X[k] + conj X[256-k]) + i conj(w512^k) (X[k] - conj X[256-k]); Z[k] is this thread's v[m],
             // Z[256 - k] the partner's v[15 - m]
             const D* sr = reinterpret_cast<const D*>(buf) + rr * kXgSP;
-            const double* ri = reinterpret_cast<const double*>(buf) + rr * kXgRP;
+            const double* ri = reinterpret_cast<const double*>(buf) + rr * kXw64RP;
             D zhi[8];
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
@@ -263,7 +279,7 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
                 v[j] = r;
             }
             __syncwarp();   // the raw rows have been consumed
-            prefetch(i + NBUF);
+            prefetch(i + NBUF, gpf);
             dft16<true>(v);   // v[j] = Z[o + 16 j]
 #pragma unroll
             for (int q = 1; q < 16; ++q) v[brev4(q)] = cmulc(v[brev4(q)], t256[q * 16]);
@@ -275,8 +291,8 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
             dft16<true>(v);
             // z[nn] = (x~[2 nn], x~[2 nn + 1]), nn = o + 16 k2; the stored unknowns lie in x~[0 .. 256): x_j = x~[j]
             // (zero-padded, DCT) or x~[j + 1] (DST-I)
-            if (g.valid) {
-                double* dst = p.real_out + comp * p.rin_pc + g.rin;
+            {
+                double* dst = p.real_out + comp * p.rin_pc + rin_of(g);
                 const bool al16 = ((reinterpret_cast<unsigned long long>(dst) & 15ull) == 0ull);
 #pragma unroll
                 for (int k2 = 0; k2 < 8; ++k2) {
