@@ -97,6 +97,8 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_x_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_xw_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXwSmemFwd)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_xw_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXwSmemInv)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_xpw_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXpwSmemFwd)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_xpw_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXpwSmemInv)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FWD, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_INV, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem5NoSlot)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FUSED, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
@@ -358,6 +360,17 @@ cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st)
 {
     if (p.nrows <= 0 || p.nrows % kXpRows || !p.nyq) return cudaErrorInvalidValue;
     int grid = 2 * g_sms;
+    // one pipeline per warp (sf_fastxw.cuh; its bulk copies want 16-byte aligned spectrum rows); SF_X_CTA=1 selects
+    // the kernel with one pipeline per CTA
+    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    if (!cta_kernel && p.spec_pitch % 2 == 0 && (reinterpret_cast<unsigned long long>(p.spec) & 15ull) == 0ull &&
+        (reinterpret_cast<unsigned long long>(inv ? (const void*)p.real_out : (const void*)p.real_in) & 15ull) == 0ull) {
+        const int need = (p.nrows / 4 + kXwWarps - 1) / kXwWarps;
+        if (grid > need) grid = need;
+        if (inv) fast_xpw_kernel<true><<<grid, kXwThreads, kXpwSmemInv, st>>>(p);
+        else fast_xpw_kernel<false><<<grid, kXwThreads, kXpwSmemFwd, st>>>(p);
+        return cudaGetLastError();
+    }
     if (grid > p.nrows / kXpRows) grid = p.nrows / kXpRows;
     if (inv) fast_xper_kernel<true><<<grid, kXpThreads, kXpSmem, st>>>(p);
     else fast_xper_kernel<false><<<grid, kXpThreads, kXpSmem, st>>>(p);

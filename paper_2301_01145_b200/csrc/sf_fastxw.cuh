@@ -252,4 +252,167 @@ template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xw_ker
     }
 }
 
+
+// ==================================================================================== periodic rows of 256 reals
+// S1 (real-to-complex) / S5 (complex-to-real) of periodic plans (PAPER.md:87 half spectrum), same scheme: the row is
+// packed as z[n] = x[2n] + i x[2n+1], n < 128, Z = DFT128(z) by eight threads (lane = w + 8 rq, four rows per warp),
+//     X[k] = ((Z[k] + conj Z[128-k]) - i w256^k (Z[k] - conj Z[128-k])) / 2,   k = 0..128.
+// Thread w ends with Z[w + 8 j], j < 16; the partner 128 - k of k = w + 8 m, m < 8, is j' = 15 - m of thread 8 - w.
+// X[0..127] go to the spectrum array, X[128] to the side array [row].
+constexpr size_t kXpwRowBytes = (size_t)kXwInPitch * sizeof(float);   // 1088 B = 64 (mod 128): 256 reals or 128 complex
+constexpr size_t kXpwWarpBytesFwd = 2 * 4 * kXpwRowBytes + kXwXchBytes;
+constexpr size_t kXpwWarpBytesInv = 4 * kXpwRowBytes + kXwXchBytes;
+constexpr size_t kXpwSmemFwd = kXwWarps * kXpwWarpBytesFwd;
+constexpr size_t kXpwSmemInv = kXwWarps * kXpwWarpBytesInv;
+
+template <bool INV> __device__ __forceinline__ void fftp128_a(C (&v)[16], const C* t128, C* xw)
+{
+    dft16<INV>(v);
+#pragma unroll
+    for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul_sel<INV>(v[brev4(q)], t128[q * 8]);   // w128^(q w)
+#pragma unroll
+    for (int q = 0; q < 16; ++q) xw[q * kXwQP] = v[brev4(q)];
+}
+
+template <bool INV> __global__ void __launch_bounds__(kXwThreads, 2) fast_xpw_kernel(const FastXPerParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bars[kXwWarps][2];
+    __shared__ __align__(16) C s_t128[128];   // [q][w] = w128^(q w)
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int wid = tid >> 5;
+    const int w = lane & 7;
+    const int rq = lane >> 3;
+    const int plane = ((8 - w) & 7) + 8 * rq;   // holds the residue 8 - w of the same row; 0 and 4 pair with themselves
+
+    if (tid < 128) s_t128[tid] = c_tw1024[(8 * (tid >> 3) * (tid & 7)) & 1023];
+    if (lane == 0) {
+        mbar_init(&bars[wid][0], 1);
+        mbar_init(&bars[wid][1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    const C* t128 = s_t128 + w;   // [q * 8]
+    C tsp[8];                     // w256^(w + 8 m): the same in every iteration
+#pragma unroll
+    for (int m = 0; m < 8; ++m) tsp[m] = c_tw1024[4 * (w + 8 * m)];
+    __syncthreads();
+
+    unsigned char* wbase = smem_raw + (size_t)wid * (INV ? kXpwWarpBytesInv : kXpwWarpBytesFwd);
+    C* xch = reinterpret_cast<C*>(wbase + (INV ? 4 : 8) * kXpwRowBytes);
+    C* xw = xch + rq * kXwGP + w;               // slot (q, w) at q * kXwQP
+    const C* xr = xch + rq * kXwGP + w * kXwQP; // slots (w, o') and (w + 8, o')
+
+    const long long nquads = p.nrows / 4;
+    const long long gw = (long long)blockIdx.x * kXwWarps + wid;
+    const long long nw = (long long)gridDim.x * kXwWarps;
+    const int nit = gw < nquads ? (int)((nquads - gw + nw - 1) / nw) : 0;
+    auto first_row = [&](int i) -> long long { return 4 * (gw + (long long)i * nw); };
+    // lane 0 starts the four row copies of iteration i (forward: into input buffer i & 1)
+    auto issue = [&](int i) {
+        if (lane != 0 || i >= nit) return;
+        const long long row = first_row(i);
+        uint64_t* bar = &bars[wid][INV ? 0 : (i & 1)];
+        unsigned char* dst = wbase + (INV ? 0 : (i & 1)) * 4 * kXpwRowBytes;
+        mbar_expect_tx(bar, 4 * 1024u);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            if (INV) bulk_g2s(dst + r * kXpwRowBytes, p.spec + (row + r) * p.spec_pitch, 1024u, bar);
+            else bulk_g2s(dst + r * kXpwRowBytes, p.real_in + (row + r) * kXN, 1024u, bar);
+        }
+    };
+    // S5: X[128] of this thread's row of iteration i from the side array, for the owner of the pair (0, 128)
+    auto load_nyq = [&](int i) -> C {
+        if (!INV || w != 0 || i >= nit) return make_float2(0.f, 0.f);
+        return __ldg(p.nyq + first_row(i) + rq);
+    };
+
+    C xnyq_next = load_nyq(0);
+    issue(0);
+    if (!INV) issue(1);
+    for (int i = 0; i < nit; ++i) {
+        const long long row = first_row(i) + rq;
+        C v[16];
+        if constexpr (!INV) {
+            // ---------------------------------------------------------------- S1
+            mbar_wait(&bars[wid][i & 1], (i >> 1) & 1);
+            const C* zin = reinterpret_cast<const C*>(wbase + ((i & 1) * 4 + rq) * kXpwRowBytes) + w;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = zin[8 * r];
+            fftp128_a<false>(v, t128, xw);
+            __syncwarp();
+            issue(i + 2);                         // this input buffer is in registers in every lane
+            C a[8], b[8];
+            fftw128_b<false>(a, b, xr);
+            // Z[w + 8 j]: j = 2 k2 in a[brev3(k2)], j = 2 k2 + 1 in b[brev3(k2)]
+            C* orow = p.spec + row * p.spec_pitch;
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const int js = 15 - m, jo = (16 - m) & 15;
+                const C snd = (js & 1) ? b[brev3(js >> 1)] : a[brev3(js >> 1)];
+                const C own = (jo & 1) ? b[brev3(jo >> 1)] : a[brev3(jo >> 1)];
+                C zm;
+                zm.x = __shfl_sync(0xffffffffu, snd.x, plane);
+                zm.y = __shfl_sync(0xffffffffu, snd.y, plane);
+                if (w == 0) zm = own;
+                const C zk = (m & 1) ? b[brev3(m >> 1)] : a[brev3(m >> 1)];
+                const C e = cadd(zk, make_float2(zm.x, -zm.y));
+                const C d = csub(zk, make_float2(zm.x, -zm.y));
+                const C wd = cmul(d, tsp[m]);   // w256^k d
+                const int k = w + 8 * m;
+                const C xhi = cscale(make_float2(e.x - wd.y, -e.y - wd.x), 0.5f);
+                orow[k] = cscale(cadd(e, make_float2(wd.y, -wd.x)), 0.5f);
+                if (m == 0) {
+                    if (w == 0) p.nyq[row] = xhi;
+                    else orow[128 - k] = xhi;
+                } else {
+                    orow[128 - k] = xhi;
+                }
+            }
+            if (w == 0) orow[64] = make_float2(a[brev3(4)].x, -a[brev3(4)].y);   // k = 64 pairs with itself: conj Z[64]
+        } else {
+            // ---------------------------------------------------------------- S5
+            const C xnyq = xnyq_next;
+            mbar_wait(&bars[wid][0], i & 1);
+            const C* srow = reinterpret_cast<const C*>(wbase + rq * kXpwRowBytes);
+            C zhi[8];
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const int k = w + 8 * m;
+                const C xk = srow[k];
+                C xm = srow[(128 - k) & 127];
+                if (m == 0 && w == 0) xm = xnyq;
+                const C e = cadd(xk, make_float2(xm.x, -xm.y));
+                const C d = csub(xk, make_float2(xm.x, -xm.y));
+                const C wd = cmulc(d, tsp[m]);   // conj(w256^k) d
+                v[m] = cadd(e, make_float2(-wd.y, wd.x));
+                zhi[m] = make_float2(e.x + wd.y, wd.x - e.y);
+            }
+            const C x64 = srow[64];
+#pragma unroll
+            for (int j = 8; j < 16; ++j) {
+                C r;
+                r.x = __shfl_sync(0xffffffffu, zhi[15 - j].x, plane);
+                r.y = __shfl_sync(0xffffffffu, zhi[15 - j].y, plane);
+                // w = 0: 128 - 8 m = 8 (16 - m) is its own; Z[64] = 2 conj X[64]
+                if (w == 0) r = (j == 8) ? make_float2(2.f * x64.x, -2.f * x64.y) : zhi[(16 - j) & 7];
+                v[j] = r;
+            }
+            fftp128_a<true>(v, t128, xw);   // v[j] = Z[w + 8 j]
+            __syncwarp();
+            issue(i + 1);                         // the staged rows are in registers in every lane
+            xnyq_next = load_nyq(i + 1);
+            C a[8], b[8];
+            fftw128_b<true>(a, b, xr);
+            C* orow = reinterpret_cast<C*>(p.real_out + row * kXN);
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) {
+                orow[w + 16 * k2] = a[brev3(k2)];        // (x[2n], x[2n+1]), n = w + 16 k2
+                orow[w + 8 + 16 * k2] = b[brev3(k2)];
+            }
+        }
+    }
+}
+
 } // namespace sf2
