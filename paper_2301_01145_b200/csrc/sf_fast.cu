@@ -427,6 +427,23 @@ cudaError_t launch_fast_xp64(bool inv, const sf::XParams<double>& p, int ncomp, 
 {
     if (p.mode != sf::X_PERIODIC || p.n != 256 || p.nyq_side_yz || p.dfield1 || p.has_faces || p.ny <= 0 || p.nz <= 0 || ncomp <= 0 || g_sms <= 0)
         return cudaErrorInvalidValue;
+    // one pipeline per warp (sf_fastxw64.cuh); SF_X_CTA=1 selects the kernel with one pipeline per CTA
+    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    if (!cta_kernel) {
+        const long long nquads = ((long long)p.ny * p.nz + 3) / 4;
+        long long gw = 2ll * g_sms;
+        if (gw > (nquads + kXw64Warps - 1) / kXw64Warps) gw = (nquads + kXw64Warps - 1) / kXw64Warps;
+        const dim3 gridw((unsigned)gw, (unsigned)ncomp);
+        cudaError_t ew;
+        if (inv) {
+            if ((ew = cudaFuncSetAttribute(fast_xpw64_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXpw64Smem)) != cudaSuccess) return ew;
+            fast_xpw64_kernel<true><<<gridw, kXw64Threads, kXpw64Smem, st>>>(p);
+        } else {
+            if ((ew = cudaFuncSetAttribute(fast_xpw64_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXpw64Smem)) != cudaSuccess) return ew;
+            fast_xpw64_kernel<false><<<gridw, kXw64Threads, kXpw64Smem, st>>>(p);
+        }
+        return cudaGetLastError();
+    }
     const long long ntiles = ((long long)p.ny * p.nz + kXp64Rows - 1) / kXp64Rows;
     long long gx = 4ll * g_sms;
     if (gx > ntiles) gx = ntiles;

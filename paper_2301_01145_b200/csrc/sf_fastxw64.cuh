@@ -314,4 +314,190 @@ template <int MODE, bool INV> __global__ void __launch_bounds__(kXw64Threads, 2)
     cp_async_wait<0>();
 }
 
+
+// ==================================================================================== periodic rows of 256 reals, fp64
+// S1 (real-to-complex) / S5 (complex-to-real) of periodic plans (PAPER.md:87 half spectrum), same scheme: the row is
+// packed as z[n] = x[2n] + i x[2n+1], n < 128, Z = DFT128(z) by eight threads (lane = w + 8 rq, four rows per warp),
+//     X[k] = ((Z[k] + conj Z[128-k]) - i w256^k (Z[k] - conj Z[128-k])) / 2,   k = 0..128.
+// Thread w ends with Z[w + 8 j], j < 16; the partner 128 - k of k = w + 8 m, m < 8, is j' = 15 - m of thread 8 - w.
+// X[128] goes to / comes from the side array of the strided passes when the plan has one.
+constexpr int kXpw64QP = 9;                                          // exchange: 16-byte words per q
+constexpr int kXpw64GP = 16 * kXpw64QP;                              // exchange: words per row
+constexpr size_t kXpw64RawBytes = 4 * 256 * sizeof(double);          // four rows of 256 reals or 128 complex
+constexpr size_t kXpw64WarpBytes = kXpw64RawBytes + 4 * (size_t)kXpw64GP * sizeof(D);
+constexpr size_t kXpw64Smem = kXw64Warps * kXpw64WarpBytes;
+
+template <bool INV> __global__ void __launch_bounds__(kXw64Threads, 2) fast_xpw64_kernel(const sf::XParams<double> p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(16) D s_t128[128];   // [q][w] = w128^(q w)
+    __shared__ __align__(16) D s_tsp[64];     // [m][w] = w256^(w + 8 m)
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int wid = tid >> 5;
+    const int w = lane & 7;
+    const int rq = lane >> 3;
+    const int plane = ((8 - w) & 7) + 8 * rq;   // holds the residue 8 - w of the same row; 0 and 4 pair with themselves
+    const int comp = blockIdx.y;
+    if (tid < 128) s_t128[tid] = c_tw1024d[(8 * (tid >> 3) * (tid & 7)) & 1023];
+    if (tid < 64) s_tsp[tid] = c_tw1024d[4 * tid];
+    __syncthreads();
+    const D* t128 = s_t128 + w;   // [q * 8]
+    const D* tsp = s_tsp + w;     // [m * 8]
+
+    unsigned char* wbase = smem_raw + (size_t)wid * kXpw64WarpBytes;
+    D* xch = reinterpret_cast<D*>(wbase + kXpw64RawBytes);
+    D* xw = xch + rq * kXpw64GP + w;                     // slot (q, w) at q * kXpw64QP
+    const D* xr = xch + rq * kXpw64GP + w * kXpw64QP;    // slots (w, o') and (w + 8, o')
+    const D* srow = reinterpret_cast<const D*>(wbase) + rq * 128;
+
+    const long long nrows = (long long)p.ny * p.nz;
+    const long long nquads = (nrows + 3) / 4;
+    const long long gw = (long long)blockIdx.x * kXw64Warps + wid;
+    const long long nw = (long long)gridDim.x * kXw64Warps;
+    const int nit = gw < nquads ? (int)((nquads - gw + nw - 1) / nw) : 0;
+    D* nyq = reinterpret_cast<D*>(p.nyq_side);
+
+    // a lane's row of iteration i; past the end the last row is done again, with identical stores
+    struct Geom {
+        int iy, iz;
+        long long r;
+    };
+    const unsigned last_row = (unsigned)(nrows - 1);
+    auto geometry = [&](int i) {
+        const long long r = 4 * (gw + (long long)i * nw) + rq;
+        const unsigned rc = r < (long long)last_row ? (unsigned)r : last_row;
+        Geom g;
+        g.r = rc;
+        g.iz = (int)(rc / (unsigned)p.ny);
+        g.iy = (int)(rc - (unsigned)g.iz * (unsigned)p.ny);
+        return g;
+    };
+    auto rin_of = [&](const Geom& g) { return g.iy * p.rin_py + g.iz * p.rin_pz; };
+    auto sp_of = [&](const Geom& g) { return g.iy * p.sp_py + g.iz * p.sp_pz; };
+    // the eight lanes of a row copy it (256 reals or X[0..127]) into the staging buffer
+    auto prefetch = [&](int i, const Geom& g) {
+        if (i < nit) {
+            double* dst = reinterpret_cast<double*>(wbase) + rq * 256;
+            const double* src = INV ? reinterpret_cast<const double*>(reinterpret_cast<const D*>(p.spec_in) + comp * p.sp_pc + sp_of(g))
+                                    : p.real_in + comp * p.rin_pc + rin_of(g);
+            if (INV || __all_sync(0xffffffffu, (reinterpret_cast<unsigned long long>(src) & 15ull) == 0ull)) {
+#pragma unroll
+                for (int t = 0; t < 16; ++t) cp_async16(dst + 2 * (w + 8 * t), src + 2 * (w + 8 * t));
+            } else {
+#pragma unroll
+                for (int t = 0; t < 32; ++t) cp_async8(dst + w + 8 * t, src + w + 8 * t);
+            }
+        }
+        cp_async_commit();
+    };
+    // S5: X[128] of this thread's row, for the owner of the pair (0, 128)
+    auto load_nyq = [&](int i, const Geom& g) -> D {
+        if (!INV || w != 0 || i >= nit) return make_double2(0.0, 0.0);
+        return nyq ? ldg_d(nyq + comp * nrows + g.r) : ldg_d(reinterpret_cast<const D*>(p.spec_in) + comp * p.sp_pc + sp_of(g) + 128);
+    };
+
+    Geom g0 = geometry(0);
+    prefetch(0, g0);
+    D xnyq_next = load_nyq(0, g0);
+    for (int i = 0; i < nit; ++i) {
+        const Geom g = g0;
+        g0 = geometry(i + 1);
+        cp_async_wait<0>();
+        __syncwarp();
+        D v[16], a[8], b[8];
+        if constexpr (!INV) {
+            // ---------------------------------------------------------------- S1
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = srow[w + 8 * r];
+            __syncwarp();   // the raw rows are in registers: fetch the next ones
+            prefetch(i + 1, g0);
+            dft16<false>(v);
+#pragma unroll
+            for (int q = 1; q < 16; ++q) v[brev4(q)] = cmul(v[brev4(q)], t128[q * 8]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) xw[q * kXpw64QP] = v[brev4(q)];
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { a[j] = xr[j]; b[j] = xr[8 * kXpw64QP + j]; }
+            dft8<false>(a);
+            dft8<false>(b);
+            // Z[w + 8 j]: j = 2 k2 in a[brev3(k2)], j = 2 k2 + 1 in b[brev3(k2)]
+            D* so = reinterpret_cast<D*>(p.spec_out) + comp * p.sp_pc + sp_of(g);
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const int js = 15 - m, jo = (16 - m) & 15;
+                D zm = shfl_d((js & 1) ? b[brev3(js >> 1)] : a[brev3(js >> 1)], plane);
+                if (w == 0) zm = (jo & 1) ? b[brev3(jo >> 1)] : a[brev3(jo >> 1)];
+                const D zk = (m & 1) ? b[brev3(m >> 1)] : a[brev3(m >> 1)];
+                const D e = make_double2(zk.x + zm.x, zk.y - zm.y);
+                const D d = make_double2(zk.x - zm.x, zk.y + zm.y);
+                const D wd = cmul(d, tsp[m * 8]);
+                const int k = w + 8 * m;
+                const D xhi = make_double2(0.5 * (e.x - wd.y), 0.5 * (-e.y - wd.x));
+                so[k] = make_double2(0.5 * (e.x + wd.y), 0.5 * (e.y - wd.x));
+                if (m == 0 && w == 0) {
+                    if (nyq) nyq[comp * nrows + g.r] = xhi;
+                    else so[128] = xhi;
+                } else {
+                    so[128 - k] = xhi;
+                }
+            }
+            if (w == 0) so[64] = make_double2(a[brev3(4)].x, -a[brev3(4)].y);   // k = 64 pairs with itself: conj Z[64]
+        } else {
+            // ---------------------------------------------------------------- S5
+            const D xnyq = xnyq_next;
+            D zhi[8];
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const int k = w + 8 * m;
+                const D xk = srow[k];
+                D xm = srow[(128 - k) & 127];
+                if (m == 0 && w == 0) xm = xnyq;
+                const D e = make_double2(xk.x + xm.x, xk.y - xm.y);
+                const D d = make_double2(xk.x - xm.x, xk.y + xm.y);
+                const D wd = cmulc(d, tsp[m * 8]);
+                v[m] = make_double2(e.x - wd.y, e.y + wd.x);
+                zhi[m] = make_double2(e.x + wd.y, wd.x - e.y);
+            }
+            const D x64 = srow[64];
+#pragma unroll
+            for (int j = 8; j < 16; ++j) {
+                D r = shfl_d(zhi[15 - j], plane);
+                // w = 0: 128 - 8 m = 8 (16 - m) is its own; Z[64] = 2 conj X[64]
+                if (w == 0) r = (j == 8) ? make_double2(2.0 * x64.x, -2.0 * x64.y) : zhi[(16 - j) & 7];
+                v[j] = r;
+            }
+            __syncwarp();   // the raw rows have been consumed
+            prefetch(i + 1, g0);
+            xnyq_next = load_nyq(i + 1, g0);
+            dft16<true>(v);   // v[j] = Z[w + 8 j]
+#pragma unroll
+            for (int q = 1; q < 16; ++q) v[brev4(q)] = cmulc(v[brev4(q)], t128[q * 8]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) xw[q * kXpw64QP] = v[brev4(q)];
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { a[j] = xr[j]; b[j] = xr[8 * kXpw64QP + j]; }
+            dft8<true>(a);
+            dft8<true>(b);
+            double* dst = p.real_out + comp * p.rin_pc + rin_of(g);
+            const bool al16 = ((reinterpret_cast<unsigned long long>(dst) & 15ull) == 0ull);
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) {
+                const int na = w + 16 * k2, nb = na + 8;   // (x[2n], x[2n+1])
+                if (al16) {
+                    *reinterpret_cast<D*>(dst + 2 * na) = a[brev3(k2)];
+                    *reinterpret_cast<D*>(dst + 2 * nb) = b[brev3(k2)];
+                } else {
+                    dst[2 * na] = a[brev3(k2)].x; dst[2 * na + 1] = a[brev3(k2)].y;
+                    dst[2 * nb] = b[brev3(k2)].x; dst[2 * nb + 1] = b[brev3(k2)].y;
+                }
+            }
+        }
+    }
+    cp_async_wait<0>();
+}
+
 } // namespace sf2
