@@ -276,6 +276,33 @@ sf_status sf_set_step_timing_stride(sf_plan plan, int stride);
  * sf_plan_create on this thread).  Never NULL; owned by the library. */
 const char* sf_last_error(sf_plan plan);
 
+/*
+ * sf_periodic2d_solve_static -- the periodic 2-D solve WITHOUT any allocation, for callers that may not call
+ * cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it): no plan, one kernel launch,
+ * no cudaMalloc / cudaFree / allocating library call on any path through it.  Computes what sf_solve computes on a
+ * 2-D periodic fp64 plan with default options: psi with lap(psi) = f, zero-mean (PAPER.md:103-109 four-step solve;
+ * eq. (8) :79-81; Table 1 periodic row :166-167; zero mode :69).
+ *   n        [host] grid points per axis, powers of two, 4 <= n[a] <= SF_STATIC_MAX_N.
+ *   h        [host] grid spacing per axis (domain length n[a] * h[a]).
+ *   op       SF_OP_PSEUDO_SPECTRAL or SF_OP_FD2.
+ *   src_dev  [device, borrowed until the launch completes] f, n[0] * n[1] doubles, x fastest.
+ *   psi_dev  [device, caller-owned] psi, same layout; may be the same buffer as src_dev.
+ *   stream   cudaStream_t (NULL = legacy default stream); the call is asynchronous on it.
+ * The work array between the transform steps is a file-scope device array of SF_STATIC_MAX_N * (SF_STATIC_MAX_N/2 + 1)
+ * complex doubles = 528 384 bytes, which every GPU that loads the library holds until the process exits.  ALL calls
+ * on a device share it: calls that can overlap on the GPU (different streams, different host threads) race on it
+ * and must be ordered by the caller; calls on one stream are safe back to back.  Nothing in it needs clearing and
+ * nothing is carried between calls (the kernel writes every word before it reads it).  The first call on a device
+ * looks up the array's device address and sets the kernel's shared-memory limit; make that call outside a stream
+ * capture.  One CTA does the whole solve: meant for small grids, use a plan for throughput.
+ * Errors: INVALID_ARG (null pointer, size not a power of two, or beyond SF_STATIC_MAX_N -- the message names the
+ * limit), UNSUPPORTED (operator), CUDA.  Message: sf_static_last_error() (per host thread; never NULL).
+ */
+#define SF_STATIC_MAX_N 256
+sf_status sf_periodic2d_solve_static(const long long n[2], const double h[2], sf_operator op, const void* src_dev, void* psi_dev,
+                                     void* stream);
+const char* sf_static_last_error(void);
+
 /* Free everything the plan owns.  Never frees caller memory.  NULL is accepted. */
 sf_status sf_plan_destroy(sf_plan plan);
 

@@ -32,6 +32,7 @@ EXPORTS = (
     "sf_divergence", "sf_laplacian", "sf_get_output", "sf_output_device_ptr", "sf_synchronize",
     "sf_set_pipeline", "sf_get_output_async", "sf_pipeline_join", "sf_probe_dft16_stage", "sf_last_launch_count", "sf_device_bytes",
     "sf_enable_step_timing", "sf_step_times_ms", "sf_set_step_timing_stride", "sf_last_error", "sf_plan_destroy", "sf_version",
+    "sf_periodic2d_solve_static", "sf_static_last_error",
 )
 
 
@@ -83,6 +84,8 @@ def lib() -> C.CDLL:
         L.sf_last_error.restype = C.c_char_p
         L.sf_plan_destroy.argtypes = [vp]
         L.sf_version.restype = C.c_char_p
+        L.sf_periodic2d_solve_static.argtypes = [C.POINTER(ll), C.POINTER(C.c_double), i, vp, vp, vp]
+        L.sf_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -197,6 +200,22 @@ def sf_probe_dft16_stage(variant, reps, ntiles, src, dst) -> float:
     ms = C.c_float(0.0)
     _check(None, lib().sf_probe_dft16_stage(int(variant), int(reps), int(ntiles), a, b, C.byref(ms)))
     return float(ms.value)
+
+
+SF_STATIC_MAX_N = 256
+
+
+def sf_periodic2d_solve_static(n, h, op, src, psi, stream=None):
+    """(see include/sailffish.h) periodic 2-D fp64 solve on device buffers without any allocation"""
+    a, wa = _addr(src)
+    b, wb = _addr(psi)
+    if wa != SF_MEM_DEVICE or wb != SF_MEM_DEVICE:
+        raise ValueError("sf_periodic2d_solve_static works on device buffers")
+    nn = (C.c_longlong * 2)(int(n[0]), int(n[1]))
+    hh = (C.c_double * 2)(float(h[0]), float(h[1]))
+    st = lib().sf_periodic2d_solve_static(nn, hh, int(op), a, b, C.c_void_p(stream or 0))
+    if st != SF_OK:
+        raise SailffishError(st, lib().sf_static_last_error().decode())
 
 
 def sf_pipeline_join(plan):

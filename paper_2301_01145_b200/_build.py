@@ -22,7 +22,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-std=c++17", "-O3", "-lineinfo", "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"] + ARCH + os.environ.get("SF_NVCC_EXTRA", "").split()
 
-UNITS = [("sf_api", "sf_api.cu", []), ("sf_fast", "sf_fast.cu", [])]
+UNITS = [("sf_api", "sf_api.cu", []), ("sf_fast", "sf_fast.cu", []), ("sf_static", "sf_static.cu", [])]
 for kind in range(4):
     for tname, t in (("f32", "float"), ("f64", "double")):
         UNITS.append((f"sf_inst_k{kind}_{tname}", "sf_inst.cu", [f"-DSF_INST_KIND={kind}", f"-DSF_INST_T={t}"]))
