@@ -11,6 +11,7 @@
 #include "sf_fastper64.cuh"
 #include "sf_fastxw.cuh"
 #include "sf_fastxw64.cuh"
+#include "sf_fastx5w.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -82,6 +83,17 @@ cudaError_t fast_init()
         for (int m = 0; m < 8; ++m)
             for (int i = 0; i < 16; ++i) txw[512 + m * 16 + i] = tw[2 * (i + 16 * m)];
         if ((e = cudaMemcpyToSymbol(g_tab_xw, txw.data(), sizeof(float2) * kXwTab)) != cudaSuccess) return e;
+        // and for the rows of 512 (sf_fastx5w.cuh)
+        std::vector<float2> tx5(kX5wTab);
+        for (int q = 0; q < 16; ++q)
+            for (int h = 0; h < 2; ++h)
+                for (int o = 0; o < 16; ++o) {
+                    tx5[q * 32 + h * 16 + o] = tw[(2 * (2 * q + h) * o) & 1023];
+                    tx5[512 + q * 32 + h * 16 + o] = tw[(2 * q * (2 * o + h)) & 1023];
+                }
+        for (int m = 0; m < 8; ++m)
+            for (int i = 0; i < 32; ++i) tx5[1024 + m * 32 + i] = tw[i + 32 * m];
+        if ((e = cudaMemcpyToSymbol(g_tab_x5w, tx5.data(), sizeof(float2) * kX5wTab)) != cudaSuccess) return e;
     }
     if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_pad_kernel<FMODE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FastCfg<FMODE_FWD>::kSmem)) != cudaSuccess) return e;
@@ -97,6 +109,8 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_x_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_xw_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXwSmemFwd)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_xw_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXwSmemInv)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_x5w_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5wSmemFwd)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_x5w_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5wSmemInv)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_xpw_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXpwSmemFwd)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_xpw_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXpwSmemInv)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast5_kernel<F5_FWD, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmem5 / 2))) != cudaSuccess) return e;
@@ -463,6 +477,16 @@ cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st)
 {
     if (p.nrows <= 0 || p.nrows % kX5Rows || p.spec_pitch < kX5SpPitch || p.nyq) return cudaErrorInvalidValue;
     int grid = 2 * g_sms;
+    // one pipeline per warp (sf_fastx5w.cuh; its bulk copies want 16-byte aligned spectrum rows); SF_X_CTA=1 selects
+    // the kernel with one pipeline per CTA
+    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    if (!cta_kernel && p.spec_pitch % 2 == 0 && (reinterpret_cast<unsigned long long>(p.spec) & 15ull) == 0ull) {
+        const int need = (p.nrows + kX5wWarps - 1) / kX5wWarps;
+        if (grid > need) grid = need;
+        if (inv) fast_x5w_kernel<true><<<grid, kX5wThreads, kX5wSmemInv, st>>>(p);
+        else fast_x5w_kernel<false><<<grid, kX5wThreads, kX5wSmemFwd, st>>>(p);
+        return cudaGetLastError();
+    }
     if (grid > p.nrows / kX5Rows) grid = p.nrows / kX5Rows;
     if (inv) fast_x5_kernel<true><<<grid, kX5Threads, kX5Smem, st>>>(p);
     else fast_x5_kernel<false><<<grid, kX5Threads, kX5Smem, st>>>(p);
