@@ -91,8 +91,8 @@ def model_bytes(w):
 
 
 STEP_EVENT_STRIDE = 8   # per-step CUDA events are recorded on every 8th solve of the timed region
-STEP_NAMES = ["S1 fast_x_kernel<fwd>", "S2 fast_pad_kernel<FWD>", "S3 fast_fused2_kernel", "S4 fast_pad_kernel<INV>",
-              "S5 fast_x_kernel<inv>"]
+STEP_NAMES = ["S1 fast_xw_kernel<fwd>", "S2 fast_pad_kernel<FWD>", "S3 fast_fused2h_kernel", "S4 fast_pad_kernel<INV>",
+              "S5 fast_xw_kernel<inv>"]
 
 
 def step_names(wname):
@@ -100,17 +100,17 @@ def step_names(wname):
     if wname == "cfg4_unbounded_256_f32":
         return STEP_NAMES
     if wname == "cfg4_unbounded_256_f64":
-        return ["S1 fast_xg_kernel<fwd>", "S2 fast64_kernel<FWD>", "S3 fast64_kernel<FUSED>", "S4 fast64_kernel<INV>", "S5 fast_xg_kernel<inv>"]
+        return ["S1 fast_xgw_kernel<fwd>", "S2 fast64_kernel<FWD>", "S3 fast64_kernel<FUSED>", "S4 fast64_kernel<INV>", "S5 fast_xgw_kernel<inv>"]
     if wname in ("cfg3_dirichlet_255_f64", "cfg3_neumann_256_f64"):
-        return ["S1 fast_xg_kernel<fwd>", "S2 fast_r2r64_kernel<FWD>", "S3 fast_r2r64_kernel<FUSED>",
-                "S4 fast_r2r64_kernel<" + ("FWD" if "dirichlet" in wname else "INV") + ">", "S5 fast_xg_kernel<inv>"]
+        return ["S1 fast_xgw_kernel<fwd>", "S2 fast_r2r64_kernel<FWD>", "S3 fast_r2r64_kernel<FUSED>",
+                "S4 fast_r2r64_kernel<" + ("FWD" if "dirichlet" in wname else "INV") + ">", "S5 fast_xgw_kernel<inv>"]
     if wname in ("cfg2_periodic_256_f32", "cfg2_periodic_256_f32_grad"):
-        return ["S1 fast_xper_kernel<fwd>", "S2 fast_per_kernel<FWD>", "S3 fast_per_kernel<FUSED>", "S4 fast_per_kernel<INV>",
-                "S5 fast_xper_kernel<inv>"]
+        return ["S1 fast_xpw_kernel<fwd>", "S2 fast_per_kernel<FWD>", "S3 fast_per_kernel<FUSED>", "S4 fast_per_kernel<INV>",
+                "S5 fast_xpw_kernel<inv>"]
     if wname == "cfg2_periodic_256_f64_grad":
-        return ["S1 fast_xp64_kernel<fwd>", "S2 fast_per64_kernel<FWD>", "S3 fast_per64_kernel<FUSED,GRAD>", "S4 fast_per64_kernel<INV>", "S5 fast_xp64_kernel<inv>"]
+        return ["S1 fast_xpw64_kernel<fwd>", "S2 fast_per64_kernel<FWD>", "S3 fast_per64_kernel<FUSED,GRAD>", "S4 fast_per64_kernel<INV>", "S5 fast_xpw64_kernel<inv>"]
     if wname == "cfg5_vector_512_f32_curl":
-        return ["S1 fast_x5_kernel<fwd>", "S2 fast5_kernel<FWD>", "S3 fast5_kernel<CURL>", "S4 fast5_kernel<INV>", "S5 fast_x5_kernel<inv>"]
+        return ["S1 fast_x5w_kernel<fwd>", "S2 fast5_kernel<FWD>", "S3 fast5_kernel<CURL>", "S4 fast5_kernel<INV>", "S5 fast_x5w_kernel<inv>"]
     return ["S1 xfwd_kernel", "S2 spass_kernel<0>", "S3 spass_kernel<2>", "S4 spass_kernel<1>", "S5 xinv_kernel"]
 
 

@@ -120,6 +120,7 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_x5_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_x5_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_fused2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem2)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_fused2h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem2)) != cudaSuccess) return e;
     {
         std::vector<double2> td(1024);
         for (int j = 0; j < 1024; ++j) {
@@ -214,9 +215,11 @@ cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map
     case FMODE_FWD: fast_pad_kernel<FMODE_FWD><<<grid, kThreads, FastCfg<FMODE_FWD>::kSmem, st>>>(p, tm); break;
     case FMODE_INV: fast_pad_kernel<FMODE_INV><<<grid, kThreads, FastCfg<FMODE_INV>::kSmem, st>>>(p, tm); break;
     case FMODE_FUSED:
-        // two pencils per thread (sf_fast2p.cuh) unless switched off; it needs an even number of batches
-        if ((p.nb & 1) == 0 && !getenv("SF_FUSED_1P")) fast_fused2_kernel<<<grid, kT2, kSmem2, st>>>(p, tm);
-        else fast_pad_kernel<FMODE_FUSED><<<grid, kThreads, FastCfg<FMODE_FUSED>::kSmem, st>>>(p, tm);
+        // both halves of a pencil's padded transform per thread (sf_fast2p.cuh); SF_FUSED_2P=1: one half of two pencils
+        // per thread (needs an even number of batches); SF_FUSED_1P=1: one half of one pencil per thread (sf_fast.cuh)
+        if (getenv("SF_FUSED_1P")) fast_pad_kernel<FMODE_FUSED><<<grid, kThreads, FastCfg<FMODE_FUSED>::kSmem, st>>>(p, tm);
+        else if (getenv("SF_FUSED_2P") && (p.nb & 1) == 0) fast_fused2_kernel<<<grid, kT2, kSmem2, st>>>(p, tm);
+        else fast_fused2h_kernel<<<grid, kT2, kSmem2, st>>>(p, tm);
         break;
     default: return cudaErrorInvalidValue;
     }
@@ -376,7 +379,7 @@ cudaError_t launch_fast_xper(bool inv, const FastXPerParams& p, cudaStream_t st)
     int grid = 2 * g_sms;
     // one pipeline per warp (sf_fastxw.cuh; its bulk copies want 16-byte aligned spectrum rows); SF_X_CTA=1 selects
     // the kernel with one pipeline per CTA
-    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
     if (!cta_kernel && p.spec_pitch % 2 == 0 && (reinterpret_cast<unsigned long long>(p.spec) & 15ull) == 0ull &&
         (reinterpret_cast<unsigned long long>(inv ? (const void*)p.real_out : (const void*)p.real_in) & 15ull) == 0ull) {
         const int need = (p.nrows / 4 + kXwWarps - 1) / kXwWarps;
@@ -406,7 +409,7 @@ template <int MODE, bool INV> cudaError_t launch_xgw(const sf::XParams<double>& 
 template <int MODE> cudaError_t launch_xg_mode(bool inv, const sf::XParams<double>& p, int ncomp, cudaStream_t st)
 {
     // one pipeline per warp (sf_fastxw64.cuh); SF_X_CTA=1 selects the kernel with one pipeline per CTA
-    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
     if (!cta_kernel) return inv ? launch_xgw<MODE, true>(p, ncomp, st) : launch_xgw<MODE, false>(p, ncomp, st);
     const long long ntiles = ((long long)p.ny * p.nz + kXgRows - 1) / kXgRows;
     long long gx = 4ll * g_sms;
@@ -442,7 +445,7 @@ cudaError_t launch_fast_xp64(bool inv, const sf::XParams<double>& p, int ncomp, 
     if (p.mode != sf::X_PERIODIC || p.n != 256 || p.nyq_side_yz || p.dfield1 || p.has_faces || p.ny <= 0 || p.nz <= 0 || ncomp <= 0 || g_sms <= 0)
         return cudaErrorInvalidValue;
     // one pipeline per warp (sf_fastxw64.cuh); SF_X_CTA=1 selects the kernel with one pipeline per CTA
-    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
     if (!cta_kernel) {
         const long long nquads = ((long long)p.ny * p.nz + 3) / 4;
         long long gw = 2ll * g_sms;
@@ -479,7 +482,7 @@ cudaError_t launch_fast_x5(bool inv, const FastXParams& p, cudaStream_t st)
     int grid = 2 * g_sms;
     // one pipeline per warp (sf_fastx5w.cuh; its bulk copies want 16-byte aligned spectrum rows); SF_X_CTA=1 selects
     // the kernel with one pipeline per CTA
-    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
     if (!cta_kernel && p.spec_pitch % 2 == 0 && (reinterpret_cast<unsigned long long>(p.spec) & 15ull) == 0ull) {
         const int need = (p.nrows + kX5wWarps - 1) / kX5wWarps;
         if (grid > need) grid = need;
@@ -498,7 +501,7 @@ cudaError_t launch_fast_x(bool inv, const FastXParams& p, cudaStream_t st)
     if (p.nrows <= 0 || p.nrows % kXRows) return cudaErrorInvalidValue;
     int grid = 2 * g_sms;
     // one pipeline per warp (sf_fastxw.cuh); SF_X_CTA=1 selects the kernel with one pipeline per CTA
-    static const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
+    const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
     if (!cta_kernel) {
         const int need = (p.nrows / 2 + kXwWarps - 1) / kXwWarps;
         if (grid > need) grid = need;

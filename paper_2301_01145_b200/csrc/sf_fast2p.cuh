@@ -200,4 +200,131 @@ __global__ void __launch_bounds__(kT2, 2) fast_fused2_kernel(const FastParams p,
     }
 }
 
+
+// ------------------------------------------------------------------------------------ both halves per thread
+// The same pass with the two register sets of a thread holding the EVEN and the ODD half of ONE pencil's padded
+// transform instead of one half of two pencils: half-warp = residue o, its 16 lanes = the 16 pencils of the tile.
+// The even half then needs no input factor and no output factor (in the kernel above every lane multiplies, the
+// lanes of the even half by one), the combine x_j = e_j + conj(w512^j) o_j is local (no shuffles, no selects), and a
+// tile needs no pairing of pencils (odd batch counts run here too).  Exchange, slot, tile queue as above.
+__global__ void __launch_bounds__(kT2, 2) fast_fused2h_kernel(const FastParams p, const __grid_constant__ CUtensorMap tm)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float4* x4 = reinterpret_cast<float4*>(smem_raw);
+    C* slot = reinterpret_cast<C*>(smem_raw + (size_t)kXchg2Elems * sizeof(float4));
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ __align__(16) C s_tab[512];   // [0, 256) tw256[o][q]; [256, 512) tw512[o][r] = w512^(o + 16 r)
+    __shared__ int s_tile[2];
+
+    const int tid = threadIdx.x;
+    const int pen = tid & 15;
+    const int o = tid >> 4;
+    const int ea = o * 16 + pen;
+    const int eb = o * 256 + pen;
+    const C* t256 = s_tab + o * 16;
+    const C* t512 = s_tab + 256 + o * 16;
+
+    const int ntiles = fast_ntiles(p.nb, p.nct, p.nyq_col);
+    const int ips = (int)p.in_ps, ops = (int)p.out_ps, ibs = (int)p.in_bs, obs = (int)p.out_bs;
+    uint32_t parity = 0;
+
+    auto issue = [&](int t) {
+        if (tid != 0 || t >= ntiles) return;
+        const TileGeom g = tile_geom(p, t);
+        if (!g.full) return;
+        mbar_expect_tx(&bar, kL * kTile * (uint32_t)sizeof(C));
+        tma_load_4d(slot, &tm, g.col, g.b, 0, 0, &bar);
+    };
+    auto advance = [&](int it) {
+        if (tid != 0) return;
+        issue(s_tile[(it + 1) & 1]);
+        s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;
+    };
+
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        s_tile[0] = (int)blockIdx.x;
+        s_tile[1] = (int)(blockIdx.x + gridDim.x);
+        issue(s_tile[0]);
+    }
+    // g_tab_pad: [0, 256) tw256, [256, 512) ones (row h = 0), [512, 768) tw512 (row h = 1)
+    if (tid < 128) reinterpret_cast<float4*>(s_tab)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid];
+    else reinterpret_cast<float4*>(s_tab)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid + 128];
+    __syncthreads();
+
+    for (int it = 0;; ++it) {
+        const int t = s_tile[it & 1];
+        if (t >= ntiles) break;
+        const TileGeom g = tile_geom(p, t);
+        // a Nyquist-column tile is 16 batches of one column; in the side array [row][batch] they are neighbours too
+        const bool side = !g.full && p.nyq_in != nullptr;
+        const bool pvalid = g.full || (g.b + pen < p.nb);
+        C v0[16], v1[16];
+        if (g.full) {
+            mbar_wait(&bar, parity);
+            parity ^= 1;
+            const C* s = slot + (o * kTile + pen);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v0[r] = s[r * 16 * kTile];
+        } else if (side) {
+            const C* inp = p.nyq_in + ((size_t)o * p.nb + min(g.b + pen, p.nb - 1));
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v0[r] = __ldg(inp + (size_t)r * 16 * p.nb);
+        } else {
+            const C* inp = p.in + (min(g.b + pen, p.nb - 1) * ibs + g.col + o * ips);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v0[r] = __ldg(inp + r * 16 * ips);
+        }
+        // even outputs: x;  odd outputs: x w512^n, n = o + 16 r
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v1[r] = cmul(v0[r], t512[r]);
+        fft256_a2<false, false>(v0, v1, t256, x4, ea, eb);
+        __syncthreads();
+        advance(it);
+        // Green's factors of the spectral rows kp = 2 (o + 16 k2) + h, folded to min(kp, 512 - kp)
+        float g0[16], g1[16];
+        {
+            const float* gt = p.green_tiles + ((size_t)green_tile_index(p, g) * (kGreenRows * kTile) + pen);
+            const float* glo = gt + (2 * o) * kTile;
+            const float* ghi = gt + (2 * kL - 2 * o) * kTile;
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) {
+                g0[k2] = __ldg(k2 < 8 ? glo + k2 * 32 * kTile : ghi - k2 * 32 * kTile);
+                g1[k2] = __ldg(k2 < 8 ? glo + (k2 * 32 + 1) * kTile : ghi - (k2 * 32 + 1) * kTile);
+            }
+        }
+        fft256_b2<false, false>(v0, v1, x4, ea, eb);
+        {
+            C u0[16], u1[16];
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) { u0[k2] = cscale(v0[brev4(k2)], g0[k2]); u1[k2] = cscale(v1[brev4(k2)], g1[k2]); }
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) { v0[k2] = u0[k2]; v1[k2] = u1[k2]; }
+        }
+        fft256_a2<true, true>(v0, v1, t256, x4, ea, eb);
+        __syncthreads();
+        fft256_b2<true, true>(v0, v1, x4, ea, eb);
+        // x_j = e_j + conj(w512^j) o_j, j = o + 16 r < 256
+        C* outp;
+        int ost;
+        if (g.full) { outp = p.out + (g.b * obs + g.col + pen); ost = ops; }
+        else if (side) { outp = p.nyq_out + (g.b + pen); ost = p.nb; }
+        else { outp = p.out + ((g.b + pen) * obs + g.col); ost = ops; }
+        outp += (size_t)o * ost;
+        if (pvalid) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) outp[(size_t)r * 16 * ost] = cadd(v0[brev4(r)], cmulc(v1[brev4(r)], t512[r]));
+        }
+    }
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(p.sched + 1, 1) == (int)gridDim.x - 1) {
+            p.sched[0] = 0;
+            p.sched[1] = 0;
+            __threadfence();
+        }
+    }
+}
+
 } // namespace sf2

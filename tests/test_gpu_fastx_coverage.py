@@ -89,3 +89,55 @@ def test_scalar_plan_on_512_pencils():
         for _ in range(2):
             sf.sf_solve(p.plan)
         _report("scalar 512x512x16 f32", p.get(sf.SF_OUT_PSI), ref, "f32")
+
+
+@pytest.mark.parametrize("env", ["SF_X_CTA", "SF_FUSED_2P", "SF_FUSED_1P"])
+def test_launch_time_kernel_switches_agree(env, monkeypatch):
+    """the kernels that the default launch no longer picks (X passes with one pipeline per CTA; the fused z pass with one
+    half of two pencils / of one pencil per thread) stay correct: same plan, same source, switch read at launch time"""
+    shape = (256, 256, 32)
+    f = rounded(_rand(shape, 77), "f32")
+    h = (0.010, 0.012, 0.011)
+    gh = O.unbounded_green((32, 256, 256), h, 2.0 * max(h))
+    ref = O.unbounded_solve(f.astype(np.float64), h, gh)
+    with Plan(shape, h, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec="f32") as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        a = p.get(sf.SF_OUT_PSI)
+        monkeypatch.setenv(env, "1")
+        sf.sf_solve(p.plan)
+        b = p.get(sf.SF_OUT_PSI)
+        monkeypatch.delenv(env)
+    _report("default kernels", a, ref, "f32")
+    _report(f"{env}=1", b, ref, "f32")
+    assert rel_l2(a, b.astype(np.float64)) <= 1e-6
+
+
+@pytest.mark.parametrize("case", ["periodic_f32", "periodic_f64", "dirichlet_f64", "vector_f32"])
+def test_cta_x_kernels_agree(case, monkeypatch):
+    """SF_X_CTA=1 on the other plans with warp-autonomous X passes"""
+    if case.startswith("periodic"):
+        prec = case[-3:]
+        shape = (256, 256, 256) if prec == "f32" else (256, 256, 256)
+        f = rounded(_rand(shape, 5), prec)
+        f -= f.mean(dtype=np.float64).astype(f.dtype)
+        mk = lambda: Plan(shape, (1.0 / 256,) * 3, sf.SF_BC_PERIODIC, prec=prec)
+    elif case == "dirichlet_f64":
+        prec, shape = "f64", (255, 255, 255)
+        f = rounded(_rand(shape, 6), prec)
+        mk = lambda: Plan(shape, (1.0 / 256,) * 3, sf.SF_BC_DIRICHLET, grid=sf.SF_GRID_CELL_BOUNDARY, op=sf.SF_OP_FD2, prec=prec)
+    else:
+        prec, shape = "f32", (512, 16, 512)
+        f = rounded(_rand(shape, 7), prec)
+        mk = lambda: Plan(shape, (0.01,) * 3, sf.SF_BC_UNBOUNDED, op=sf.SF_OP_GREEN_GAUSS2, prec=prec)
+    with mk() as p:
+        p.set_source(f)
+        sf.sf_solve(p.plan)
+        a = p.get(sf.SF_OUT_PSI).astype(np.float64)
+        monkeypatch.setenv("SF_X_CTA", "1")
+        sf.sf_solve(p.plan)
+        b = p.get(sf.SF_OUT_PSI).astype(np.float64)
+        monkeypatch.delenv("SF_X_CTA")
+    e = rel_l2(a, b)
+    print(f"{case}: warp vs CTA X kernels rel-L2 {e:.3e}")
+    assert np.isfinite(e) and e <= (1e-6 if prec == "f32" else 1e-13)
