@@ -91,7 +91,7 @@ def model_bytes(w):
 
 
 STEP_EVENT_STRIDE = 8   # per-step CUDA events are recorded on every 8th solve of the timed region
-STEP_NAMES = ["S1 fast_xw_kernel<fwd>", "S2 fast_pad_kernel<FWD>", "S3 fast_fused2h_kernel", "S4 fast_pad_kernel<INV>",
+STEP_NAMES = ["S1 fast_xw_kernel<fwd>", "S2 fast_fwd2h_kernel", "S3 fast_fused2h_kernel", "S4 fast_inv2h_kernel",
               "S5 fast_xw_kernel<inv>"]
 
 

@@ -121,6 +121,8 @@ cudaError_t fast_init()
     if ((e = cudaFuncSetAttribute(fast_x5_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kX5Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_fused2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem2)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(fast_fused2h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem2)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_inv2h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemInv2)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(fast_fwd2h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem2)) != cudaSuccess) return e;
     {
         std::vector<double2> td(1024);
         for (int j = 0; j < 1024; ++j) {
@@ -212,8 +214,15 @@ cudaError_t launch_fast_pad(int mode, const FastParams& p, const TileMap& in_map
     if (grid > ntiles) grid = ntiles;
     if (grid <= 0) return cudaErrorInvalidValue;
     switch (mode) {
-    case FMODE_FWD: fast_pad_kernel<FMODE_FWD><<<grid, kThreads, FastCfg<FMODE_FWD>::kSmem, st>>>(p, tm); break;
-    case FMODE_INV: fast_pad_kernel<FMODE_INV><<<grid, kThreads, FastCfg<FMODE_INV>::kSmem, st>>>(p, tm); break;
+    case FMODE_FWD:
+        // both halves of a pencil's padded transform per thread (sf_fast2p.cuh); SF_PAD_1H=1: one half per thread (sf_fast.cuh)
+        if (!getenv("SF_PAD_1H")) fast_fwd2h_kernel<<<grid, kT2, kSmem2, st>>>(p, tm);
+        else fast_pad_kernel<FMODE_FWD><<<grid, kThreads, FastCfg<FMODE_FWD>::kSmem, st>>>(p, tm);
+        break;
+    case FMODE_INV:
+        if (!getenv("SF_PAD_1H")) fast_inv2h_kernel<<<grid, kT2, kSmemInv2, st>>>(p);
+        else fast_pad_kernel<FMODE_INV><<<grid, kThreads, FastCfg<FMODE_INV>::kSmem, st>>>(p, tm);
+        break;
     case FMODE_FUSED:
         // both halves of a pencil's padded transform per thread (sf_fast2p.cuh); SF_FUSED_2P=1: one half of two pencils
         // per thread (needs an even number of batches); SF_FUSED_1P=1: one half of one pencil per thread (sf_fast.cuh)

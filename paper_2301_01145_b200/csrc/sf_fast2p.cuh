@@ -327,4 +327,222 @@ __global__ void __launch_bounds__(kT2, 2) fast_fused2h_kernel(const FastParams p
     }
 }
 
+
+// ------------------------------------------------------------------------------------ S4 with both halves per thread
+// FMODE_INV of fast_pad_kernel (rows k < 512 -> rows j < 256) in the same mapping: a thread reads the even row 2 m
+// and the odd row 2 m + 1, m = o + 16 k2, of its pencil (32 loads in flight), runs the two inverse 256-point
+// transforms through one float4 exchange and combines them locally.  No slot (the rows go straight into registers);
+// consecutive tiles alternate the orientation of the exchange buffer: one barrier per tile.
+constexpr size_t kSmemInv2 = (size_t)kXchg2Elems * sizeof(float4);
+
+__global__ void __launch_bounds__(kT2, 2) fast_inv2h_kernel(const FastParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float4* x4 = reinterpret_cast<float4*>(smem_raw);
+    C* xbuf = reinterpret_cast<C*>(smem_raw);   // staging of a Nyquist tile image: 512 rows x 16 pencils = the same 64 KB
+    __shared__ __align__(16) C s_tab[512];      // [0, 256) tw256[o][q]; [256, 512) tw512[o][r] = w512^(o + 16 r)
+    __shared__ int s_tile[2];
+
+    const int tid = threadIdx.x;
+    const int pen = tid & 15;
+    const int o = tid >> 4;
+    const int ea = o * 16 + pen;
+    const int eb = o * 256 + pen;
+    const C* t256 = s_tab + o * 16;
+    const C* t512 = s_tab + 256 + o * 16;
+
+    const int ntiles = fast_ntiles(p.nb, p.nct, p.nyq_col);
+    const int ips = (int)p.in_ps, ops = (int)p.out_ps, ibs = (int)p.in_bs, obs = (int)p.out_bs;
+    auto stage = [&](int row, int pencil) -> C& { return xbuf[row * kTile + ((pencil + row) & 15)]; };
+
+    if (tid == 0) {
+        s_tile[0] = (int)blockIdx.x;
+        s_tile[1] = (int)(blockIdx.x + gridDim.x);
+    }
+    if (tid < 128) reinterpret_cast<float4*>(s_tab)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid];
+    else reinterpret_cast<float4*>(s_tab)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid + 128];
+    __syncthreads();
+
+    auto tile = [&](int t, int it, auto orient_tag) {
+        constexpr bool OB = decltype(orient_tag)::value;
+        const TileGeom g = tile_geom(p, t);
+        const bool side = !g.full && p.nyq_in != nullptr;
+        const bool pvalid = g.full || (g.b + pen < p.nb);
+        C v0[16], v1[16];
+        if (side) {
+            // the producer (S3) left this column as [pencil of S4 = z][ky]: read 512 contiguous ky per z and transpose
+            // through the exchange buffer (which the previous tile's second half may still be reading)
+            if (it > 0) __syncthreads();
+            for (int idx = tid; idx < 2 * kL * kTile; idx += kT2) {
+                const int pp = idx >> 9, ky = idx & (2 * kL - 1);
+                stage(ky, pp) = (g.b + pp < p.nb) ? __ldg(p.nyq_in + (g.b + pp) * (2 * kL) + ky) : make_float2(0.f, 0.f);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) { v0[k2] = stage(2 * (o + 16 * k2), pen); v1[k2] = stage(2 * (o + 16 * k2) + 1, pen); }
+            __syncthreads();   // before the exchange overwrites the staging
+        } else {
+            const C* inp = p.in + ((g.full ? (g.b * ibs + g.col + pen) : (min(g.b + pen, p.nb - 1) * ibs + g.col)) + 2 * o * ips);
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) { v0[k2] = __ldg(inp + k2 * 32 * ips); v1[k2] = __ldg(inp + ips + k2 * 32 * ips); }
+        }
+        fft256_a2<true, OB>(v0, v1, t256, x4, ea, eb);
+        __syncthreads();
+        if (tid == 0) s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;
+        fft256_b2<true, OB>(v0, v1, x4, ea, eb);
+        // x_j = e_j + conj(w512^j) o_j, j = o + 16 r < 256
+        C* outp;
+        int ost;
+        if (g.full) { outp = p.out + (g.b * obs + g.col + pen); ost = ops; }
+        else if (side) { outp = p.nyq_out + (g.b + pen); ost = p.nb; }
+        else { outp = p.out + ((g.b + pen) * obs + g.col); ost = ops; }
+        outp += (size_t)o * ost;
+        if (pvalid) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) outp[(size_t)r * 16 * ost] = cadd(v0[brev4(r)], cmulc(v1[brev4(r)], t512[r]));
+        }
+    };
+
+    for (int it = 0;; it += 2) {
+        int t = s_tile[0];
+        if (t >= ntiles) break;
+        tile(t, it, std::false_type());
+        t = s_tile[1];
+        if (t >= ntiles) break;
+        tile(t, it + 1, std::true_type());
+    }
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(p.sched + 1, 1) == (int)gridDim.x - 1) {
+            p.sched[0] = 0;
+            p.sched[1] = 0;
+            __threadfence();
+        }
+    }
+}
+
+
+// ------------------------------------------------------------------------------------ S2 with both halves per thread
+// FMODE_FWD of fast_pad_kernel (rows n < 256 -> rows k < 512) in the same mapping: the staged tile is read once per
+// element (not once per half), the odd half's input factor is the only one applied, and a thread stores the even row
+// 2 m and the odd row 2 m + 1, m = o + 16 k2, of its pencil.  TMA-fed slot and tile queue as in fast_fused2h_kernel;
+// consecutive tiles alternate the orientation of the exchange buffer.  `tm`: dims (column, row, batch, 1).
+__global__ void __launch_bounds__(kT2, 2) fast_fwd2h_kernel(const FastParams p, const __grid_constant__ CUtensorMap tm)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float4* x4 = reinterpret_cast<float4*>(smem_raw);
+    C* xbuf = reinterpret_cast<C*>(smem_raw);   // staging of a Nyquist tile image (512 rows x 16 pencils)
+    C* slot = reinterpret_cast<C*>(smem_raw + (size_t)kXchg2Elems * sizeof(float4));
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ __align__(16) C s_tab[512];
+    __shared__ int s_tile[2];
+
+    const int tid = threadIdx.x;
+    const int pen = tid & 15;
+    const int o = tid >> 4;
+    const int ea = o * 16 + pen;
+    const int eb = o * 256 + pen;
+    const C* t256 = s_tab + o * 16;
+    const C* t512 = s_tab + 256 + o * 16;
+
+    const int ntiles = fast_ntiles(p.nb, p.nct, p.nyq_col);
+    const int ips = (int)p.in_ps, ops = (int)p.out_ps, ibs = (int)p.in_bs, obs = (int)p.out_bs;
+    uint32_t parity = 0;
+    auto stage = [&](int row, int pencil) -> C& { return xbuf[row * kTile + ((pencil + row) & 15)]; };
+    auto issue = [&](int t) {
+        if (tid != 0 || t >= ntiles) return;
+        const TileGeom g = tile_geom(p, t);
+        if (!g.full) return;
+        mbar_expect_tx(&bar, kL * kTile * (uint32_t)sizeof(C));
+        tma_load_4d(slot, &tm, g.col, 0, g.b, 0, &bar);
+    };
+    auto advance = [&](int it) {
+        if (tid != 0) return;
+        issue(s_tile[(it + 1) & 1]);
+        s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;
+    };
+
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        s_tile[0] = (int)blockIdx.x;
+        s_tile[1] = (int)(blockIdx.x + gridDim.x);
+        issue(s_tile[0]);
+    }
+    if (tid < 128) reinterpret_cast<float4*>(s_tab)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid];
+    else reinterpret_cast<float4*>(s_tab)[tid] = reinterpret_cast<const float4*>(g_tab_pad)[tid + 128];
+    __syncthreads();
+
+    auto tile = [&](int t, int it, auto orient_tag) {
+        constexpr bool OB = decltype(orient_tag)::value;
+        const TileGeom g = tile_geom(p, t);
+        const bool side = !g.full && p.nyq_in != nullptr;
+        const bool pvalid = g.full || (g.b + pen < p.nb);
+        C v0[16], v1[16];
+        if (g.full) {
+            mbar_wait(&bar, parity);
+            parity ^= 1;
+            const C* s = slot + (o * kTile + pen);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v0[r] = s[r * 16 * kTile];
+        } else if (side) {
+            // Nyquist column from its side array [row][batch]: the 16 batches are contiguous
+            const C* inp = p.nyq_in + ((size_t)o * p.nb + min(g.b + pen, p.nb - 1));
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v0[r] = __ldg(inp + (size_t)r * 16 * p.nb);
+        } else {
+            const C* inp = p.in + (min(g.b + pen, p.nb - 1) * ibs + g.col + o * ips);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v0[r] = __ldg(inp + r * 16 * ips);
+        }
+        // even outputs: x;  odd outputs: x w512^n, n = o + 16 r
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v1[r] = cmul(v0[r], t512[r]);
+        fft256_a2<false, OB>(v0, v1, t256, x4, ea, eb);
+        __syncthreads();
+        advance(it);
+        fft256_b2<false, OB>(v0, v1, x4, ea, eb);
+        if (side) {
+            // the consumer (S3) wants this column as [pencil of S2 = z][ky]: transpose through the exchange buffer and
+            // write 512 contiguous ky per z
+            __syncthreads();   // every thread is done reading the exchange buffer
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) {
+                stage(2 * (o + 16 * k2), pen) = v0[brev4(k2)];
+                stage(2 * (o + 16 * k2) + 1, pen) = v1[brev4(k2)];
+            }
+            __syncthreads();
+            for (int idx = tid; idx < 2 * kL * kTile; idx += kT2) {
+                const int pp = idx >> 9, ky = idx & (2 * kL - 1);
+                if (g.b + pp < p.nb) p.nyq_out[(g.b + pp) * (2 * kL) + ky] = stage(ky, pp);
+            }
+            __syncthreads();   // before the next tile's exchange
+        } else if (pvalid) {
+            C* q = p.out + ((g.full ? (g.b * obs + g.col + pen) : ((g.b + pen) * obs + g.col)) + 2 * o * ops);   // row 2 (o + 16 k2) + h
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) {
+                q[k2 * 32 * ops] = v0[brev4(k2)];
+                q[k2 * 32 * ops + ops] = v1[brev4(k2)];
+            }
+        }
+    };
+
+    for (int it = 0;; it += 2) {
+        int t = s_tile[0];
+        if (t >= ntiles) break;
+        tile(t, it, std::false_type());
+        t = s_tile[1];
+        if (t >= ntiles) break;
+        tile(t, it + 1, std::true_type());
+    }
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(p.sched + 1, 1) == (int)gridDim.x - 1) {
+            p.sched[0] = 0;
+            p.sched[1] = 0;
+            __threadfence();
+        }
+    }
+}
+
 } // namespace sf2

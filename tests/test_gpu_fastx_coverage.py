@@ -91,10 +91,11 @@ def test_scalar_plan_on_512_pencils():
         _report("scalar 512x512x16 f32", p.get(sf.SF_OUT_PSI), ref, "f32")
 
 
-@pytest.mark.parametrize("env", ["SF_X_CTA", "SF_FUSED_2P", "SF_FUSED_1P"])
+@pytest.mark.parametrize("env", ["SF_X_CTA", "SF_FUSED_2P", "SF_FUSED_1P", "SF_PAD_1H"])
 def test_launch_time_kernel_switches_agree(env, monkeypatch):
     """the kernels that the default launch no longer picks (X passes with one pipeline per CTA; the fused z pass with one
-    half of two pencils / of one pencil per thread) stay correct: same plan, same source, switch read at launch time"""
+    half of two pencils / of one pencil per thread; the y passes with one half per thread) stay correct: same plan, same
+    source, switch read at launch time"""
     shape = (256, 256, 32)
     f = rounded(_rand(shape, 77), "f32")
     h = (0.010, 0.012, 0.011)
