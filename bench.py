@@ -154,7 +154,7 @@ def ncu_counts(wname, step_index):
 
 
 def issue_view(wname, dom, kernel_ms, clocks, names):
-    """The dominant kernel of the default workload is bound by instruction issue, not by HBM (profiles/r02_a.md):
+    """The dominant kernel of the default workload is bound by instruction issue, not by HBM (profiles/r02_b.md):
     besides the HBM roofline the line carries its issue-slot utilisation = (warp instructions + packed fp32x2
     instructions: a packed instruction occupies its scheduler for two cycles) / (148 SMs x 4 schedulers x the SM clock
     sampled during the timed region) / measured kernel time.  None without a capture of the current sources."""
