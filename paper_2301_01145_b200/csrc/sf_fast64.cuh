@@ -49,6 +49,18 @@ template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256d_b(D (
     dft16<INV>(v);
 }
 
+// 1 / d for the spectral multipliers: hardware seed (rcp.approx.ftz.f64, ~20 bits) and two Newton steps, 1 - 2 ulp; about half
+// the instructions of the correctly rounded __drcp_rn (no special-case branch: d is a finite, normal sum of eigenvalues,
+// or zero at the zero mode, whose multiplier is replaced afterwards)
+__device__ __forceinline__ double fast_rcp(double d)
+{
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
+    double e = fma(-d, x, 1.0);
+    x = fma(x, e, x);
+    e = fma(-d, x, 1.0);
+    return fma(x, e, x);
+}
 __device__ __forceinline__ D ldg_d(const D* p)
 {
     const double2 t = __ldg(reinterpret_cast<const double2*>(p));

@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(kT64, 2) fast_per64_kernel(const FastPer64Para
             D w[16];
 #pragma unroll
             for (int k2 = 0; k2 < 16; ++k2) {
-                double m = p.scale * __drcp_rn(lxb + s_lamp[o + 16 * k2]);
+                double m = p.scale * fast_rcp(lxb + s_lamp[o + 16 * k2]);
                 if (k2 == 0 && zero0) m = 0.0;
                 w[k2] = cscale(v[brev4(k2)], m);
             }

@@ -14,7 +14,7 @@
 // The fused pass needs no sine / cosine bookkeeping at all: the backward transform is the inverse FFT of the same
 // symmetric spectrum, so it is   extension -> FFT512 -> F[k] *= scale / (lambda_x + lambda_y + lambda_z[fold(k)])
 // -> inverse FFT512 truncated to the stored rows   with fold(k) = min(k, 512 - k): the structure of the padded
-// fused kernel with the multiplier computed on the fly (one IEEE reciprocal per real column and spectral row).  The two
+// fused kernel with the multiplier computed on the fly (one reciprocal per real column and spectral row: fast_rcp of sf_fast64.cuh).  The two
 // real columns have different multipliers and are separated in Y, not in F, so F is rotated to Y around the multiply
 // (a swap of the two factors for DST-I, two complex multiplications by w1024^k for DCT).
 // Tiles of 8 complex = 16 real columns (128-byte rows) arrive by TMA; 256 threads, two CTAs per SM.
@@ -179,8 +179,8 @@ __global__ void __launch_bounds__(kT64, 2) fast_r2r64_kernel(const FastR64Params
                 double ma = 0.0, mb = 0.0;
                 if (li >= 0 && li < n) {
                     const double lp = s_lamp[li];
-                    ma = p.scale * __drcp_rn(lxa + lp);
-                    mb = p.scale * __drcp_rn(lxb + lp);
+                    ma = p.scale * fast_rcp(lxa + lp);
+                    mb = p.scale * fast_rcp(lxb + lp);
                     if (p.zero_mode && li == 0 && b == 0) {                   // the all-zero index
                         if (cx == 0) ma = 0.0;
                         if (cx + 1 == 0) mb = 0.0;
