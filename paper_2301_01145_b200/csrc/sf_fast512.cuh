@@ -212,10 +212,12 @@ __global__ void __launch_bounds__(64 * PEN, 16 / PEN) fast5_kernel(const Fast5Pa
     constexpr bool kPark = (MODE == F5_CURL && PEN == 16);   // (PEN = 8: the shared memory of two CTAs has no room for it)
     __shared__ float s_qx[kPark ? NT : 1], s_qy[kPark ? NT : 1];
     __shared__ unsigned s_oo[kPark ? NT : 1];
-    __shared__ __align__(16) C s_tw512[kTwc ? 1 : 32 * 16];        // [w][q] = w512^(q w)
+    // (rows of 17 entries: with PEN = 8 a warp holds two residues w, whose rows must not start on the same bank)
+    constexpr int kTwRow = 17;
+    __shared__ __align__(16) C s_tw512[kTwc ? 1 : 32 * kTwRow];    // [w][q] = w512^(q w)
     // (PEN = 8: only the h = 1 half of the second table is kept, the even half selects one: shared memory for two CTAs)
     constexpr bool kHalfTab = (PEN == 8);
-    __shared__ __align__(16) C s_tw1024[kTwc ? 1 : (kHalfTab ? 1 : 2) * 32 * 16];   // [h][w][r] = h ? w1024^(w + 32 r) : 1
+    __shared__ __align__(16) C s_tw1024[kTwc ? 1 : (kHalfTab ? 1 : 2) * 32 * kTwRow];   // [h][w][r] = h ? w1024^(w + 32 r) : 1
     __shared__ int s_tile[2];
     __shared__ uint32_t s_tmem;
 
@@ -228,8 +230,8 @@ __global__ void __launch_bounds__(64 * PEN, 16 / PEN) fast5_kernel(const Fast5Pa
     const int q0 = w & 15, par = w >> 4;            // (PEN = 8: the two residues of a warp share their parity)
     C* xw = xbuf + (w * LW + lane);                 // slot (q, w) at ((q * 32 + w) * LW + lane)
     const C* xr = xbuf + (q0 * 32 * LW + lane);     // slot (q0, o) at stride LW
-    const C* t512 = s_tw512 + w * 16;
-    const C* t1024 = s_tw1024 + ((kHalfTab ? 0 : h * 32) + w) * 16;
+    const C* t512 = s_tw512 + w * kTwRow;
+    const C* t1024 = s_tw1024 + ((kHalfTab ? 0 : h * 32) + w) * kTwRow;
     const float hf = (float)h;
     auto tw512 = [&](int q) -> C { return kTwc ? c_tw1024[(2 * q * w) & 1023] : t512[q]; };
     // 1 + h (w1024^(w + 32 r) - 1): one packed multiply-add on the table of (Re w - 1, Im w)
@@ -358,10 +360,10 @@ __global__ void __launch_bounds__(64 * PEN, 16 / PEN) fast5_kernel(const Fast5Pa
     if (MODE == F5_CURL)
         for (int i = tid; i < 1024; i += NT) s_kapp[i] = __ldg(p.kap_p + i);
     if (!kTwc) {
-        if (tid < 512) s_tw512[tid] = c_tw1024[(2 * (tid & 15) * (tid >> 4)) & 1023];
+        if (tid < 512) s_tw512[(tid >> 4) * kTwRow + (tid & 15)] = c_tw1024[(2 * (tid & 15) * (tid >> 4)) & 1023];
         for (int i = tid; i < (kHalfTab ? 1 : 2) * 512; i += NT) {
             const int r = i & 15, ww = (i >> 4) & 31, hh = kHalfTab ? 1 : (i >> 9);
-            s_tw1024[i] = hh ? c_tw1024[ww + 32 * r] : make_float2(1.f, 0.f);
+            s_tw1024[(i >> 4) * kTwRow + r] = hh ? c_tw1024[ww + 32 * r] : make_float2(1.f, 0.f);
         }
     }
     uint32_t tbase = 0;
