@@ -512,10 +512,11 @@ cudaError_t launch_fast_x(bool inv, const FastXParams& p, cudaStream_t st)
     // one pipeline per warp (sf_fastxw.cuh); SF_X_CTA=1 selects the kernel with one pipeline per CTA
     const bool cta_kernel = (getenv("SF_X_CTA") != nullptr);
     if (!cta_kernel) {
-        const int need = (p.nrows / 2 + kXwWarps - 1) / kXwWarps;
+        const int nwarps = xw_warps(inv);
+        const int need = (p.nrows / 2 + nwarps - 1) / nwarps;
         if (grid > need) grid = need;
-        if (inv) fast_xw_kernel<true><<<grid, kXwThreads, kXwSmemInv, st>>>(p);
-        else fast_xw_kernel<false><<<grid, kXwThreads, kXwSmemFwd, st>>>(p);
+        if (inv) fast_xw_kernel<true><<<grid, 32 * nwarps, kXwSmemInv, st>>>(p);
+        else fast_xw_kernel<false><<<grid, 32 * nwarps, kXwSmemFwd, st>>>(p);
         return cudaGetLastError();
     }
     if (grid > p.nrows / kXRows) grid = p.nrows / kXRows;
