@@ -11,6 +11,7 @@
 // backward exp(+2 pi i nk/N), both unnormalised here; the 1/N is folded into the spectral
 // multiplier by the host.
 #pragma once
+#include "sf_trig.cuh"
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -54,16 +55,8 @@ template <typename C> __device__ __forceinline__ C cmuli(C a) { C r; r.x = -a.y;
 template <typename C> __device__ __forceinline__ C cmulmi(C a) { C r; r.x = a.y; r.y = -a.x; return r; }
 
 // ------------------------------------------------------------------------------------ radix DFTs
-// cos / sin of 2 pi i / 16
-__host__ __device__ constexpr double cos16(int i)
-{
-    constexpr double c[16] = { 1.0, 0.92387953251128675613, 0.70710678118654752440, 0.38268343236508977173,
-                               0.0, -0.38268343236508977173, -0.70710678118654752440, -0.92387953251128675613,
-                               -1.0, -0.92387953251128675613, -0.70710678118654752440, -0.38268343236508977173,
-                               0.0, 0.38268343236508977173, 0.70710678118654752440, 0.92387953251128675613 };
-    return c[i & 15];
-}
-__host__ __device__ constexpr double sin16(int i) { return cos16(i - 4); }
+using sftrig::cos16;   // cos / sin of 2 pi i / 16 (sf_trig.cuh)
+using sftrig::sin16;
 
 // multiply d by exp(-/+ 2 pi i * I16 / 16) (forward: minus) with the trivial cases special-cased
 template <int I16, bool INV, typename C> __device__ __forceinline__ C mul_w16(C d)

@@ -34,6 +34,7 @@
 // Persistent CTAs, two per SM (64 registers per thread): the two CTAs are independent barrier
 // domains, so one does arithmetic while the other exchanges, loads or stores.
 #pragma once
+#include "sf_trig.cuh"
 #include "sf_fast_api.h"
 #include <cuda.h>
 #include <stdint.h>
@@ -81,15 +82,8 @@ __device__ __forceinline__ C cmuli(C a) { return make_float2(-a.y, a.x); }
 __device__ __forceinline__ C cmulmi(C a) { return make_float2(a.y, -a.x); }
 
 // ------------------------------------------------------------------------------------ radix-16
-__host__ __device__ constexpr double cos16(int i)
-{
-    constexpr double c[16] = { 1.0, 0.92387953251128675613, 0.70710678118654752440, 0.38268343236508977173,
-                               0.0, -0.38268343236508977173, -0.70710678118654752440, -0.92387953251128675613,
-                               -1.0, -0.92387953251128675613, -0.70710678118654752440, -0.38268343236508977173,
-                               0.0, 0.38268343236508977173, 0.70710678118654752440, 0.92387953251128675613 };
-    return c[i & 15];
-}
-__host__ __device__ constexpr double sin16(int i) { return cos16(i - 4); }
+using sftrig::cos16;   // cos / sin of 2 pi i / 16 (sf_trig.cuh)
+using sftrig::sin16;
 
 // the same complex helpers for double precision (sf_fast64.cuh): plain DADD / DMUL / DFMA
 typedef double2 D;

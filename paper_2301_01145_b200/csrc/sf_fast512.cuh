@@ -28,6 +28,7 @@
 // (the common factor i is applied at the store).  Three forward and three backward transforms per tile, every
 // component read once and every velocity component written once.
 #pragma once
+#include "sf_trig.cuh"
 #include "sf_fast.cuh"
 
 namespace sf2 {
@@ -40,16 +41,8 @@ constexpr int kSlot5Elems = kL5 * kTile;                  // 64 KB
 constexpr size_t kSmem5 = ((size_t)kXchg5Elems + kSlot5Elems) * sizeof(C);
 constexpr size_t kSmem5NoSlot = (size_t)kXchg5Elems * sizeof(C);
 
-__host__ __device__ constexpr double cos32(int i)
-{
-    constexpr double c[9] = { 1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
-                              0.70710678118654752440, 0.55557023301960222474, 0.38268343236508977173,
-                              0.19509032201612826785, 0.0 };
-    i &= 31;
-    if (i > 16) i = 32 - i;
-    return i <= 8 ? c[i] : -c[16 - i];
-}
-__host__ __device__ constexpr double sin32(int i) { return cos32(i - 8); }
+using sftrig::cos32;   // cos / sin of 2 pi i / 32 (sf_trig.cuh)
+using sftrig::sin32;
 // d * exp(-/+ 2 pi i I32 / 32)   (forward: minus)
 template <int I32, bool INV> __device__ __forceinline__ C mul_w32(C d)
 {
