@@ -51,6 +51,34 @@ template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256_b2(C (
     dft16<INV>(vb);
 }
 
+// the same two halves with the exchange buffer as two planes of 8-byte slots (one per register set) instead of 16-byte
+// slots: two 8-byte stores / loads per slot pair, but no moves that pack two register pairs into an aligned quad
+constexpr int kPlane2 = 16 * 16 * 16;   // C elements per plane
+template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256_a2p(C (&va)[16], C (&vb)[16], const C* tw256, C* xp, int ea, int eb)
+{
+    dft16<INV>(va);
+    dft16<INV>(vb);
+#pragma unroll
+    for (int q = 1; q < 16; ++q) {
+        const C w = tw256[q];
+        va[brev4(q)] = cmul_sel<INV>(va[brev4(q)], w);
+        vb[brev4(q)] = cmul_sel<INV>(vb[brev4(q)], w);
+    }
+    C* w0 = xp + (ORIENT_B ? eb : ea);
+    constexpr int ws = (ORIENT_B ? 16 : 256);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) { w0[q * ws] = va[brev4(q)]; w0[kPlane2 + q * ws] = vb[brev4(q)]; }
+}
+template <bool INV, bool ORIENT_B> __device__ __forceinline__ void fft256_b2p(C (&va)[16], C (&vb)[16], const C* xp, int ea, int eb)
+{
+    const C* r0 = xp + (ORIENT_B ? ea : eb);
+    constexpr int rs = (ORIENT_B ? 256 : 16);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { va[i] = r0[i * rs]; vb[i] = r0[kPlane2 + i * rs]; }
+    dft16<INV>(va);
+    dft16<INV>(vb);
+}
+
 __global__ void __launch_bounds__(kT2, 2) fast_fused2_kernel(const FastParams p, const __grid_constant__ CUtensorMap tm)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -210,7 +238,7 @@ __global__ void __launch_bounds__(kT2, 2) fast_fused2_kernel(const FastParams p,
 __global__ void __launch_bounds__(kT2, 2) fast_fused2h_kernel(const FastParams p, const __grid_constant__ CUtensorMap tm)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float4* x4 = reinterpret_cast<float4*>(smem_raw);
+    C* xp = reinterpret_cast<C*>(smem_raw);
     C* slot = reinterpret_cast<C*>(smem_raw + (size_t)kXchg2Elems * sizeof(float4));
     __shared__ __align__(8) uint64_t bar;
     __shared__ __align__(16) C s_tab[512];   // [0, 256) tw256[o][q]; [256, 512) tw512[o][r] = w512^(o + 16 r)
@@ -279,7 +307,7 @@ __global__ void __launch_bounds__(kT2, 2) fast_fused2h_kernel(const FastParams p
         // even outputs: x;  odd outputs: x w512^n, n = o + 16 r
 #pragma unroll
         for (int r = 0; r < 16; ++r) v1[r] = cmul(v0[r], t512[r]);
-        fft256_a2<false, false>(v0, v1, t256, x4, ea, eb);
+        fft256_a2p<false, false>(v0, v1, t256, xp, ea, eb);
         __syncthreads();
         advance(it);
         // Green's factors of the spectral rows kp = 2 (o + 16 k2) + h, folded to min(kp, 512 - kp)
@@ -294,7 +322,7 @@ __global__ void __launch_bounds__(kT2, 2) fast_fused2h_kernel(const FastParams p
                 g1[k2] = __ldg(k2 < 8 ? glo + (k2 * 32 + 1) * kTile : ghi - (k2 * 32 + 1) * kTile);
             }
         }
-        fft256_b2<false, false>(v0, v1, x4, ea, eb);
+        fft256_b2p<false, false>(v0, v1, xp, ea, eb);
         {
             C u0[16], u1[16];
 #pragma unroll
@@ -302,9 +330,9 @@ __global__ void __launch_bounds__(kT2, 2) fast_fused2h_kernel(const FastParams p
 #pragma unroll
             for (int k2 = 0; k2 < 16; ++k2) { v0[k2] = u0[k2]; v1[k2] = u1[k2]; }
         }
-        fft256_a2<true, true>(v0, v1, t256, x4, ea, eb);
+        fft256_a2p<true, true>(v0, v1, t256, xp, ea, eb);
         __syncthreads();
-        fft256_b2<true, true>(v0, v1, x4, ea, eb);
+        fft256_b2p<true, true>(v0, v1, xp, ea, eb);
         // x_j = e_j + conj(w512^j) o_j, j = o + 16 r < 256
         C* outp;
         int ost;
@@ -338,7 +366,6 @@ constexpr size_t kSmemInv2 = (size_t)kXchg2Elems * sizeof(float4);
 __global__ void __launch_bounds__(kT2, 2) fast_inv2h_kernel(const FastParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float4* x4 = reinterpret_cast<float4*>(smem_raw);
     C* xbuf = reinterpret_cast<C*>(smem_raw);   // staging of a Nyquist tile image: 512 rows x 16 pencils = the same 64 KB
     __shared__ __align__(16) C s_tab[512];      // [0, 256) tw256[o][q]; [256, 512) tw512[o][r] = w512^(o + 16 r)
     __shared__ int s_tile[2];
@@ -386,10 +413,10 @@ __global__ void __launch_bounds__(kT2, 2) fast_inv2h_kernel(const FastParams p)
 #pragma unroll
             for (int k2 = 0; k2 < 16; ++k2) { v0[k2] = __ldg(inp + k2 * 32 * ips); v1[k2] = __ldg(inp + ips + k2 * 32 * ips); }
         }
-        fft256_a2<true, OB>(v0, v1, t256, x4, ea, eb);
+        fft256_a2p<true, OB>(v0, v1, t256, xbuf, ea, eb);
         __syncthreads();
         if (tid == 0) s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;
-        fft256_b2<true, OB>(v0, v1, x4, ea, eb);
+        fft256_b2p<true, OB>(v0, v1, xbuf, ea, eb);
         // x_j = e_j + conj(w512^j) o_j, j = o + 16 r < 256
         C* outp;
         int ost;
@@ -430,7 +457,6 @@ __global__ void __launch_bounds__(kT2, 2) fast_inv2h_kernel(const FastParams p)
 __global__ void __launch_bounds__(kT2, 2) fast_fwd2h_kernel(const FastParams p, const __grid_constant__ CUtensorMap tm)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float4* x4 = reinterpret_cast<float4*>(smem_raw);
     C* xbuf = reinterpret_cast<C*>(smem_raw);   // staging of a Nyquist tile image (512 rows x 16 pencils)
     C* slot = reinterpret_cast<C*>(smem_raw + (size_t)kXchg2Elems * sizeof(float4));
     __shared__ __align__(8) uint64_t bar;
@@ -498,10 +524,10 @@ __global__ void __launch_bounds__(kT2, 2) fast_fwd2h_kernel(const FastParams p, 
         // even outputs: x;  odd outputs: x w512^n, n = o + 16 r
 #pragma unroll
         for (int r = 0; r < 16; ++r) v1[r] = cmul(v0[r], t512[r]);
-        fft256_a2<false, OB>(v0, v1, t256, x4, ea, eb);
+        fft256_a2p<false, OB>(v0, v1, t256, xbuf, ea, eb);
         __syncthreads();
         advance(it);
-        fft256_b2<false, OB>(v0, v1, x4, ea, eb);
+        fft256_b2p<false, OB>(v0, v1, xbuf, ea, eb);
         if (side) {
             // the consumer (S3) wants this column as [pencil of S2 = z][ky]: transpose through the exchange buffer and
             // write 512 contiguous ky per z
