@@ -415,6 +415,18 @@ __global__ void __launch_bounds__(kT2, 2) fast_inv2h_kernel(const FastParams p)
         }
         fft256_a2p<true, OB>(v0, v1, t256, xbuf, ea, eb);
         __syncthreads();
+        {
+            // ask the next tile's 512 rows of 128 bytes into the L2 while this one is transformed
+            const int tn = s_tile[(it + 1) & 1];
+            if (tn < ntiles) {
+                const TileGeom gn = tile_geom(p, tn);
+                if (gn.full) {
+                    const C* nx = p.in + (gn.b * ibs + gn.col);
+                    prefetch_l2(nx + (size_t)tid * ips);
+                    prefetch_l2(nx + (size_t)(tid + kT2) * ips);
+                }
+            }
+        }
         if (tid == 0) s_tile[it & 1] = atomicAdd(p.sched, 1) + 2 * (int)gridDim.x;
         fft256_b2p<true, OB>(v0, v1, xbuf, ea, eb);
         // x_j = e_j + conj(w512^j) o_j, j = o + 16 r < 256
